@@ -1,0 +1,605 @@
+/* vlbm_oracle.c — CPU ORACLE (test infrastructure only; see vlbm_oracle.h).
+ *
+ * Plain, slow, per-cell restatement of the vectorial LBM step of arxiv/paper_2606_00641:
+ *   Eq.2  PAPER.md:78   f_{k,i}(x + c_i, t+1) = f_{k,i} + Omega^C + Omega^S
+ *   Eq.3  PAPER.md:84   f^eq_{k,i} = w_i (Q_k + c_i . Phi_k / c_s^2)
+ *   Eq.4  PAPER.md:90   Q_k = sum_i f_{k,i},  Phi_k = sum_i f_{k,i} c_i
+ *   Eq.5  PAPER.md:98   D = (tau - 1/2) c_s^2
+ *   Eq.8  PAPER.md:128  p = (gamma-1)(E - rho|u|^2/2 - |B|^2/2)
+ *   Eq.11 PAPER.md:142  ideal-MHD Q and Phi
+ *   Eq.12 PAPER.md:148  Powell source S = -(div B)(0, B, u.B, u)
+ *   Eq.13-14 PAPER.md:160-162  homogenised solid: u^ = d u + (1-d) u^B, B^ likewise
+ *   PAPER.md:154        static boundaries: Dirichlet (value defined) / Neumann (value from the
+ *                       next cell along the discrete normal, new equilibrium assigned)
+ * Stored state = post-collision populations g; one step = pull, moments, source, blend, flux,
+ * BGK collide + direct injection, store.  fp64 throughout.
+ * Compile: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC.
+ */
+#include "vlbm_oracle.h"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define MAXK 8
+#define MAXQ 19
+
+/* ---- lattice tables (A2): rest; +x,-x,+y,-y,+z,-z; diagonals (+,+),(-,-),(+,-),(-,+) per plane
+ * xy, xz, yz.  Weights are the Gauss-Hermite ones of the textbook lattices, c_s^2 = 1/3.
+ * D2Q5 / D3Q7 (the paper's own lattices): rest weight 1/3 resp. 1/4, which is
+ * what sum_i w_i c_ia c_ib = c_s^2 delta_ab with c_s^2 = 1/3 resp. 1/4 forces. ---- */
+typedef struct { int D, Q; int c[MAXQ][3]; double w[MAXQ]; double cs2; } lattice_t;
+
+static int lattice_make(int id, lattice_t *L)
+{
+  static const int c19[19][3] = {
+    {0,0,0},
+    {1,0,0},{-1,0,0},{0,1,0},{0,-1,0},{0,0,1},{0,0,-1},
+    {1,1,0},{-1,-1,0},{1,-1,0},{-1,1,0},
+    {1,0,1},{-1,0,-1},{1,0,-1},{-1,0,1},
+    {0,1,1},{0,-1,-1},{0,1,-1},{0,-1,1} };
+  static const int c9[9][3] = {
+    {0,0,0},{1,0,0},{-1,0,0},{0,1,0},{0,-1,0},{1,1,0},{-1,-1,0},{1,-1,0},{-1,1,0} };
+  memset(L, 0, sizeof *L);
+  int i;
+  switch (id) {
+  case ORC_D1Q3:
+    L->D = 1; L->Q = 3; L->cs2 = 1.0 / 3.0;
+    L->c[1][0] = 1; L->c[2][0] = -1;
+    L->w[0] = 2.0 / 3.0; L->w[1] = L->w[2] = 1.0 / 6.0;
+    return 0;
+  case ORC_D2Q9:
+    L->D = 2; L->Q = 9; L->cs2 = 1.0 / 3.0;
+    memcpy(L->c, c9, sizeof c9);
+    L->w[0] = 4.0 / 9.0;
+    for (i = 1; i < 5; i++) L->w[i] = 1.0 / 9.0;
+    for (i = 5; i < 9; i++) L->w[i] = 1.0 / 36.0;
+    return 0;
+  case ORC_D3Q19:
+    L->D = 3; L->Q = 19; L->cs2 = 1.0 / 3.0;
+    memcpy(L->c, c19, sizeof c19);
+    L->w[0] = 1.0 / 3.0;
+    for (i = 1; i < 7; i++) L->w[i] = 1.0 / 18.0;
+    for (i = 7; i < 19; i++) L->w[i] = 1.0 / 36.0;
+    return 0;
+  case ORC_D2Q5:
+    L->D = 2; L->Q = 5; L->cs2 = 1.0 / 3.0;
+    memcpy(L->c, c9, 5 * sizeof c9[0]);
+    L->w[0] = 1.0 / 3.0;
+    for (i = 1; i < 5; i++) L->w[i] = 1.0 / 6.0;
+    return 0;
+  case ORC_D3Q7:
+    L->D = 3; L->Q = 7; L->cs2 = 1.0 / 4.0;
+    memcpy(L->c, c19, 7 * sizeof c19[0]);
+    L->w[0] = 1.0 / 4.0;
+    for (i = 1; i < 7; i++) L->w[i] = 1.0 / 8.0;
+    return 0;
+  }
+  return -1;
+}
+
+int oracle_lattice(int lattice, int *D, int *Q, int *c, double *w, double *cs2)
+{
+  lattice_t L;
+  if (lattice_make(lattice, &L)) return -1;
+  *D = L.D; *Q = L.Q; *cs2 = L.cs2;
+  for (int i = 0; i < L.Q; i++) { w[i] = L.w[i]; for (int a = 0; a < 3; a++) c[3 * i + a] = L.c[i][a]; }
+  return 0;
+}
+
+static int num_vars(int scheme, int D) { return scheme == ORC_IDEAL ? 8 : 1 + 2 * D; }
+
+int oracle_num_vars(const oracle_params *p)
+{
+  lattice_t L;
+  if (lattice_make(p->lattice, &L)) return -1;
+  return num_vars(p->scheme, L.D);
+}
+int oracle_num_dirs(const oracle_params *p)
+{
+  lattice_t L;
+  if (lattice_make(p->lattice, &L)) return -1;
+  return L.Q;
+}
+
+static int g_threads = 0;
+void oracle_set_threads(int n) { g_threads = n; }
+int oracle_get_threads(void)
+{
+#ifdef _OPENMP
+  return g_threads > 0 ? g_threads : omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+/* ---- fluxes Phi_k,alpha(Q), alpha over the D lattice axes ---- */
+/* IDEAL: Eq.11 PAPER.md:142 with the EOS Eq.8; magnetic pressure |B|^2/2.
+ * INCRES (A3): P carries kinematic pressure, dP/dt + c0^2 div u = 0; momentum flux u u + (P + B^2/2) I - B B;
+ * induction flux u B - B u. */
+static void flux_eval(int scheme, int D, double gamma, double c0sq, const double *Q, double Phi[MAXK][3])
+{
+  int a, b;
+  if (scheme == ORC_IDEAL) {
+    double rho = Q[0], E = Q[4];
+    const double *m = Q + 1, *B = Q + 5;
+    double u[3];
+    for (b = 0; b < 3; b++) u[b] = m[b] / rho;
+    double B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
+    double mu = m[0] * u[0] + m[1] * u[1] + m[2] * u[2];
+    double p = (gamma - 1.0) * (E - 0.5 * mu - 0.5 * B2);
+    double pt = p + 0.5 * B2;
+    double uB = u[0] * B[0] + u[1] * B[1] + u[2] * B[2];
+    for (a = 0; a < D; a++) {
+      Phi[0][a] = m[a];
+      for (b = 0; b < 3; b++) Phi[1 + b][a] = m[b] * u[a] + (a == b ? pt : 0.0) - B[b] * B[a];
+      Phi[4][a] = (E + pt) * u[a] - B[a] * uB;
+      for (b = 0; b < 3; b++) Phi[5 + b][a] = u[a] * B[b] - B[a] * u[b];
+    }
+  } else {
+    double P = Q[0];
+    const double *u = Q + 1, *B = Q + 1 + D;
+    double B2 = 0.0;
+    for (b = 0; b < D; b++) B2 += B[b] * B[b];
+    double pt = P + 0.5 * B2;
+    for (a = 0; a < D; a++) {
+      Phi[0][a] = c0sq * u[a];
+      for (b = 0; b < D; b++) Phi[1 + b][a] = u[b] * u[a] + (a == b ? pt : 0.0) - B[b] * B[a];
+      for (b = 0; b < D; b++) Phi[1 + D + b][a] = u[a] * B[b] - B[a] * u[b];
+    }
+  }
+}
+
+/* Eq.3 */
+static double feq_eval(const lattice_t *L, int i, double Qk, const double *Phik)
+{
+  double cPhi = 0.0;
+  for (int a = 0; a < L->D; a++) cPhi += (double)L->c[i][a] * Phik[a];
+  return L->w[i] * (Qk + cPhi / L->cs2);
+}
+
+int oracle_flux(const oracle_params *p, const double *Qv, double *Phi)
+{
+  lattice_t L;
+  if (lattice_make(p->lattice, &L)) return -1;
+  int K = num_vars(p->scheme, L.D);
+  double F[MAXK][3];
+  memset(F, 0, sizeof F);
+  flux_eval(p->scheme, L.D, p->gamma, p->c0sq, Qv, F);
+  for (int k = 0; k < K; k++) for (int a = 0; a < 3; a++) Phi[3 * k + a] = a < L.D ? F[k][a] : 0.0;
+  return 0;
+}
+
+int oracle_equilibrium(const oracle_params *p, const double *Qv, double *feq)
+{
+  lattice_t L;
+  if (lattice_make(p->lattice, &L)) return -1;
+  int K = num_vars(p->scheme, L.D);
+  double F[MAXK][3];
+  memset(F, 0, sizeof F);
+  flux_eval(p->scheme, L.D, p->gamma, p->c0sq, Qv, F);
+  for (int k = 0; k < K; k++)
+    for (int i = 0; i < L.Q; i++) feq[k * L.Q + i] = feq_eval(&L, i, Qv[k], F[k]);
+  return 0;
+}
+
+/* ---- state ---- */
+struct oracle {
+  oracle_params p;
+  lattice_t L;
+  int K;
+  long N;
+  double omega[MAXK];  /* 1/tau_k */
+  double tauB;         /* tau of the magnetic sets (all equal, A7) */
+  int iB;              /* index of B_x in Q */
+  int iU;              /* index of the first momentum / velocity component */
+  double *g[2];        /* A/B population arrays [K][Q][N] */
+  int cur;
+  unsigned char *mask; /* [N] */
+  double *Bsolid;      /* [3][N] or NULL */
+  double usolid[3];
+  int has_sphere;
+  double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs;
+  long sph_t0;         /* step count at which the centre was sph_c0 */
+  long t;              /* steps done so far */
+  double srclog[MAXK];
+};
+
+static long cell_index(const oracle_t *o, int x, int y, int z)
+{
+  return ((long)z * o->p.ny + y) * o->p.nx + x;
+}
+static double *pop(const oracle_t *o, double *g, int k, int i) { return g + ((long)k * o->L.Q + i) * o->N; }
+
+int oracle_create(const oracle_params *p, const unsigned char *cell_mask, oracle_t **out)
+{
+  lattice_t L;
+  *out = NULL;
+  if (lattice_make(p->lattice, &L)) return -1;
+  if (p->scheme != ORC_IDEAL && p->scheme != ORC_INCRES) return -1;
+  if (p->nx < 1 || p->ny < 1 || p->nz < 1) return -1;
+  if (L.D < 2 && p->ny != 1) return -1;
+  if (L.D < 3 && p->nz != 1) return -1;
+  const int n[3] = { p->nx, p->ny, p->nz };
+  for (int a = 0; a < L.D; a++) {
+    int lo = p->bc[2 * a], hi = p->bc[2 * a + 1];
+    if (lo < 0 || lo > 2 || hi < 0 || hi > 2) return -1;
+    if ((lo == ORC_BC_PERIODIC) != (hi == ORC_BC_PERIODIC)) return -1;
+    if (lo != ORC_BC_PERIODIC && n[a] < 3) return -1;                     /* A9 needs an inward neighbour */
+  }
+  oracle_t *o = (oracle_t *)calloc(1, sizeof *o);
+  if (!o) return -2;
+  o->p = *p; o->L = L;
+  o->K = num_vars(p->scheme, L.D);
+  o->N = (long)p->nx * p->ny * p->nz;
+  o->iU = 1;
+  o->iB = p->scheme == ORC_IDEAL ? 5 : 1 + L.D;
+  int nvec = p->scheme == ORC_IDEAL ? 3 : L.D;
+  double tau[MAXK] = { 0 };
+  for (int k = 0; k < o->K; k++) tau[k] = p->tau[k];
+  /* Eq.5: tau = 1/2 + D / c_s^2 for the sets that carry a physical diffusivity (A3) */
+  if (p->nu > 0.0) {
+    for (int b = 0; b < nvec; b++) tau[o->iU + b] = 0.5 + p->nu / L.cs2;
+    if (p->scheme == ORC_INCRES) tau[0] = 0.5 + p->nu / L.cs2;
+  }
+  if (p->eta > 0.0) for (int b = 0; b < nvec; b++) tau[o->iB + b] = 0.5 + p->eta / L.cs2;
+  for (int k = 0; k < o->K; k++) {
+    if (!(tau[k] > 0.5)) { free(o); return -1; }
+    o->omega[k] = 1.0 / tau[k];
+  }
+  o->tauB = tau[o->iB];
+  for (int b = 1; b < nvec; b++) if (tau[o->iB + b] != o->tauB) { free(o); return -1; }   /* A7 */
+  if (p->scheme == ORC_IDEAL && !(p->gamma > 1.0)) { free(o); return -1; }
+  size_t bytes = (size_t)o->K * L.Q * o->N * sizeof(double);
+  o->g[0] = (double *)calloc(1, bytes);
+  o->g[1] = (double *)calloc(1, bytes);
+  o->mask = (unsigned char *)calloc(1, (size_t)o->N);
+  if (!o->g[0] || !o->g[1] || !o->mask) { oracle_destroy(o); return -2; }
+  if (cell_mask) memcpy(o->mask, cell_mask, (size_t)o->N);
+  *out = o;
+  return 0;
+}
+
+void oracle_destroy(oracle_t *o)
+{
+  if (!o) return;
+  free(o->g[0]); free(o->g[1]); free(o->mask); free(o->Bsolid); free(o);
+}
+
+int oracle_set_obstacle(oracle_t *o, const unsigned char *mask, const double u_solid[3], const double *B_solid)
+{
+  if (!o || !mask) return -1;
+  memcpy(o->mask, mask, (size_t)o->N);
+  for (int a = 0; a < 3; a++) o->usolid[a] = u_solid ? u_solid[a] : 0.0;
+  free(o->Bsolid); o->Bsolid = NULL;
+  if (B_solid) {
+    o->Bsolid = (double *)malloc(3 * (size_t)o->N * sizeof(double));
+    if (!o->Bsolid) return -2;
+    memcpy(o->Bsolid, B_solid, 3 * (size_t)o->N * sizeof(double));
+  }
+  return 0;
+}
+
+int oracle_set_sphere(oracle_t *o, const double centre[3], double radius, const double u_solid[3],
+                      const double dipole_dir[3], double B_surface)
+{
+  if (!o || !(radius > 0.0)) return -1;
+  o->has_sphere = 1;
+  for (int a = 0; a < 3; a++) {
+    o->sph_c0[a] = centre[a];   /* A12: centre before the next step; before step t it is c0 + (t - t0) u^B */
+    o->sph_u[a] = u_solid[a]; o->sph_m[a] = dipole_dir[a];
+  }
+  o->sph_R = radius; o->sph_Bs = B_surface; o->sph_t0 = o->t;
+  return 0;
+}
+
+/* Eq.3: g = f^eq(Q) from the given macroscopic fields */
+int oracle_init(oracle_t *o, const double *fields)
+{
+  if (!o || !fields) return -1;
+  const int K = o->K, Qn = o->L.Q;
+  for (long n = 0; n < o->N; n++) {
+    double Qv[MAXK], Phi[MAXK][3];
+    for (int k = 0; k < K; k++) Qv[k] = fields[(long)k * o->N + n];
+    memset(Phi, 0, sizeof Phi);
+    flux_eval(o->p.scheme, o->L.D, o->p.gamma, o->p.c0sq, Qv, Phi);
+    for (int k = 0; k < K; k++)
+      for (int i = 0; i < Qn; i++) {
+        double v = feq_eval(&o->L, i, Qv[k], Phi[k]);
+        pop(o, o->g[0], k, i)[n] = v;
+        pop(o, o->g[1], k, i)[n] = v;
+      }
+  }
+  o->cur = 0; o->t = 0; o->sph_t0 = 0;
+  memset(o->srclog, 0, sizeof o->srclog);
+  return 0;
+}
+
+int oracle_get_populations(oracle_t *o, double *g_out)
+{
+  memcpy(g_out, o->g[o->cur], (size_t)o->K * o->L.Q * o->N * sizeof(double));
+  return 0;
+}
+int oracle_set_populations(oracle_t *o, const double *g_in)
+{
+  memcpy(o->g[o->cur], g_in, (size_t)o->K * o->L.Q * o->N * sizeof(double));
+  return 0;
+}
+int oracle_source_log(oracle_t *o, double *acc)
+{
+  for (int k = 0; k < o->K; k++) acc[k] = o->srclog[k];
+  return 0;
+}
+
+/* ---- solid state at a cell (A8, A11, A12) ----
+ * returns porosity d in {0,1}; fills uB[3], BB[3] when d < 1.
+ * Sphere: SOLID iff |x - c(t)|^2 <= R^2 with x the integer cell coordinates and
+ * c(t) = c0 + (t - t0) u^B; dipole B^B(r) = 1/2 B_s (R / max(|r|, R/2))^3 [3 (m.r^) r^ - m],
+ * r^ = r/|r| (0 at r = 0). */
+static double solid_state(const oracle_t *o, int x, int y, int z, long n, double uB[3], double BB[3])
+{
+  if (o->has_sphere) {
+    double dt = (double)(o->t - o->sph_t0);
+    double r[3], xi[3] = { (double)x, (double)y, (double)z };
+    double r2 = 0.0;
+    for (int a = 0; a < 3; a++) {
+      double c = o->sph_c0[a] + dt * o->sph_u[a];
+      r[a] = a < o->L.D ? xi[a] - c : 0.0;
+      r2 = r2 + r[a] * r[a];
+    }
+    if (r2 <= o->sph_R * o->sph_R) {
+      double rn = sqrt(r2);
+      double rc = rn > 0.5 * o->sph_R ? rn : 0.5 * o->sph_R;
+      double q = o->sph_R / rc;
+      double amp = 0.5 * o->sph_Bs * (q * q * q);
+      double rh[3], mr = 0.0;
+      for (int a = 0; a < 3; a++) { rh[a] = rn > 0.0 ? r[a] / rn : 0.0; mr += o->sph_m[a] * rh[a]; }
+      for (int a = 0; a < 3; a++) { BB[a] = amp * (3.0 * mr * rh[a] - o->sph_m[a]); uB[a] = o->sph_u[a]; }
+      return 0.0;
+    }
+  }
+  if (o->mask[n] == ORC_CELL_SOLID) {
+    for (int a = 0; a < 3; a++) { uB[a] = o->usolid[a]; BB[a] = o->Bsolid ? o->Bsolid[(long)a * o->N + n] : 0.0; }
+    return 0.0;
+  }
+  return 1.0;
+}
+
+/* ---- one cell of one step ---- */
+static void cell_update(const oracle_t *o, const double *src, double *dst, int x, int y, int z, double *srcacc)
+{
+  const lattice_t *L = &o->L;
+  const int K = o->K, Qn = L->Q, D = L->D;
+  const int nn[3] = { o->p.nx, o->p.ny, o->p.nz };
+  const int xi[3] = { x, y, z };
+  const long n = cell_index(o, x, y, z);
+  const long N = o->N;
+  int k, i, a, b;
+
+  /* frozen: mask FROZEN or on an INFLOW face (A10): g' = g */
+  int frozen = o->mask[n] == ORC_CELL_FROZEN;
+  for (a = 0; a < D; a++) {
+    if (xi[a] == 0 && o->p.bc[2 * a] == ORC_BC_INFLOW) frozen = 1;
+    if (xi[a] == nn[a] - 1 && o->p.bc[2 * a + 1] == ORC_BC_INFLOW) frozen = 1;
+  }
+  if (frozen) {
+    for (k = 0; k < K; k++) for (i = 0; i < Qn; i++) dst[((long)k * Qn + i) * N + n] = src[((long)k * Qn + i) * N + n];
+    return;
+  }
+
+  /* 1. pull  f[k][i] = g[k][i](x - c_i); periodic wrap; A9 substitution when the source is outside */
+  double f[MAXK][MAXQ];
+  int have_nb = 0;
+  double Qnb[MAXK], Phinb[MAXK][3];
+  for (i = 0; i < Qn; i++) {
+    int s[3] = { x, y, z }, outside = 0;
+    for (a = 0; a < D; a++) {
+      s[a] = xi[a] - L->c[i][a];
+      if (s[a] < 0) { if (o->p.bc[2 * a] == ORC_BC_PERIODIC) s[a] += nn[a]; else outside = 1; }
+      else if (s[a] >= nn[a]) { if (o->p.bc[2 * a + 1] == ORC_BC_PERIODIC) s[a] -= nn[a]; else outside = 1; }
+    }
+    if (!outside) {
+      long ns = cell_index(o, s[0], s[1], s[2]);
+      for (k = 0; k < K; k++) f[k][i] = src[((long)k * Qn + i) * N + ns];
+    } else {
+      if (!have_nb) {
+        /* A9 / PAPER.md:154: take the state of the next cell along the inward discrete normal */
+        int q[3] = { x, y, z };
+        for (a = 0; a < D; a++) {
+          if (xi[a] == 0 && o->p.bc[2 * a] != ORC_BC_PERIODIC) q[a] = xi[a] + 1;
+          if (xi[a] == nn[a] - 1 && o->p.bc[2 * a + 1] != ORC_BC_PERIODIC) q[a] = xi[a] - 1;
+        }
+        long nb = cell_index(o, q[0], q[1], q[2]);
+        for (k = 0; k < K; k++) {
+          double sum = 0.0;
+          for (int j = 0; j < Qn; j++) sum += src[((long)k * Qn + j) * N + nb];
+          Qnb[k] = sum;
+        }
+        memset(Phinb, 0, sizeof Phinb);
+        flux_eval(o->p.scheme, D, o->p.gamma, o->p.c0sq, Qnb, Phinb);
+        have_nb = 1;
+      }
+      for (k = 0; k < K; k++) f[k][i] = feq_eval(L, i, Qnb[k], Phinb[k]);
+    }
+  }
+
+  /* 2. zeroth moments (Eq.4), sums in index order */
+  double Qv[MAXK];
+  for (k = 0; k < K; k++) { double sum = 0.0; for (i = 0; i < Qn; i++) sum += f[k][i]; Qv[k] = sum; }
+
+  /* 3. local div B estimate (A6): delta = - tr Pi_B / (tau_B c_s^2) */
+  double tr = 0.0;
+  for (b = 0; b < D; b++) for (i = 0; i < Qn; i++) tr += (double)L->c[i][b] * f[o->iB + b][i];
+  double delta = -tr / (o->tauB * L->cs2);
+
+  /* 4. Powell source (Eq.12), direct injection (A5) */
+  double S[MAXK];
+  for (k = 0; k < K; k++) S[k] = 0.0;
+  double kd = o->p.powell * delta;
+  if (o->p.scheme == ORC_IDEAL) {
+    double u[3], uBdot = 0.0;
+    for (b = 0; b < 3; b++) { u[b] = Qv[1 + b] / Qv[0]; uBdot += u[b] * Qv[5 + b]; }
+    for (b = 0; b < 3; b++) { S[1 + b] = -kd * Qv[5 + b]; S[5 + b] = -kd * u[b]; }
+    S[4] = -kd * uBdot;
+  } else {
+    for (b = 0; b < D; b++) { S[1 + b] = -kd * Qv[1 + D + b]; S[1 + D + b] = -kd * Qv[1 + b]; }
+  }
+
+  /* 5. homogenised solid (Eq.13-14, A8): Q^ and the shift dQh = Q^ - Q; source scaled by d */
+  double Qh[MAXK], dQh[MAXK];
+  for (k = 0; k < K; k++) { Qh[k] = Qv[k]; dQh[k] = 0.0; }
+  double uSol[3], BSol[3];
+  double d = solid_state(o, x, y, z, n, uSol, BSol);
+  if (d < 1.0) {
+    if (o->p.scheme == ORC_IDEAL) {
+      double rho = Qv[0], u[3], uh[3], Bh[3], mu = 0.0, B2 = 0.0, uh2 = 0.0, Bh2 = 0.0;
+      for (b = 0; b < 3; b++) {
+        u[b] = Qv[1 + b] / rho;
+        mu += Qv[1 + b] * u[b];
+        B2 += Qv[5 + b] * Qv[5 + b];
+      }
+      double p = (o->p.gamma - 1.0) * (Qv[4] - 0.5 * mu - 0.5 * B2);
+      for (b = 0; b < 3; b++) {
+        uh[b] = d * u[b] + (1.0 - d) * uSol[b];
+        Bh[b] = d * Qv[5 + b] + (1.0 - d) * BSol[b];
+        uh2 += uh[b] * uh[b];
+        Bh2 += Bh[b] * Bh[b];
+      }
+      for (b = 0; b < 3; b++) { Qh[1 + b] = rho * uh[b]; Qh[5 + b] = Bh[b]; }
+      Qh[4] = p / (o->p.gamma - 1.0) + 0.5 * rho * uh2 + 0.5 * Bh2;
+    } else {
+      for (b = 0; b < D; b++) {
+        Qh[1 + b] = d * Qv[1 + b] + (1.0 - d) * uSol[b];
+        Qh[1 + D + b] = d * Qv[1 + D + b] + (1.0 - d) * BSol[b];
+      }
+    }
+    for (k = 0; k < K; k++) { dQh[k] = Qh[k] - Qv[k]; S[k] *= d; }
+  }
+  if (srcacc) for (k = 0; k < K; k++) srcacc[k] += S[k];
+
+  /* 6. flux of the (blended) state (Eq.11) */
+  double Phi[MAXK][3];
+  memset(Phi, 0, sizeof Phi);
+  flux_eval(o->p.scheme, D, o->p.gamma, o->p.c0sq, Qh, Phi);
+
+  /* 7./8. BGK + direct injection (Eq.2-3), store */
+  for (k = 0; k < K; k++)
+    for (i = 0; i < Qn; i++) {
+      double feq = feq_eval(L, i, Qv[k], Phi[k]);
+      dst[((long)k * Qn + i) * N + n] = f[k][i] + o->omega[k] * (feq - f[k][i]) + L->w[i] * (dQh[k] + S[k]);
+    }
+}
+
+int oracle_step(oracle_t *o, int n_steps)
+{
+  if (!o || n_steps < 0) return -1;
+  const int nx = o->p.nx, ny = o->p.ny, nz = o->p.nz;
+  const long rows = (long)ny * nz;
+  double *rowacc = (double *)calloc((size_t)rows * MAXK, sizeof(double));
+  if (!rowacc) return -2;
+  for (int s = 0; s < n_steps; s++) {
+    const double *src = o->g[o->cur];
+    double *dst = o->g[1 - o->cur];
+    memset(rowacc, 0, (size_t)rows * MAXK * sizeof(double));
+    if (rows >= 4) {
+#pragma omp parallel for schedule(static) num_threads(oracle_get_threads())
+      for (long r = 0; r < rows; r++) {
+        int z = (int)(r / ny), y = (int)(r % ny);
+        for (int x = 0; x < nx; x++) cell_update(o, src, dst, x, y, z, rowacc + r * MAXK);
+      }
+    } else {
+      /* 1D / thin domains: parallelise over x, source log kept serial-free by per-cell slots */
+      double *cellacc = (double *)calloc((size_t)o->N * MAXK, sizeof(double));
+      if (!cellacc) { free(rowacc); return -2; }
+#pragma omp parallel for schedule(static) num_threads(oracle_get_threads())
+      for (long n = 0; n < o->N; n++) {
+        int x = (int)(n % nx), y = (int)((n / nx) % ny), z = (int)(n / ((long)nx * ny));
+        cell_update(o, src, dst, x, y, z, cellacc + n * MAXK);
+      }
+      for (long n = 0; n < o->N; n++) for (int k = 0; k < o->K; k++) rowacc[k] += cellacc[n * MAXK + k];
+      free(cellacc);
+    }
+    for (long r = 0; r < rows; r++) for (int k = 0; k < o->K; k++) o->srclog[k] += rowacc[r * MAXK + k];
+    o->cur = 1 - o->cur;
+    o->t += 1;
+  }
+  free(rowacc);
+  return 0;
+}
+
+/* ---- moments and diagnostics of the stored populations (Eq.4) ----
+ * diag = [ sum_x Q_k (K) | sum_x |Q_k| (K) | max_x |Q_k| (K) | max|div_h B|, min rho, min p, flag ]
+ * div_h B(x) = sum_i w_i c_i . B(x + c_i) / c_s^2 (P4), neighbour index wrapped on periodic axes and
+ * clamped on the others.  flag: +1 if any non-finite value, +2 if any rho <= 0.
+ * INCRES: "min rho" slot = 1 (constant density), "min p" slot = min P. */
+int oracle_moments(oracle_t *o, double *fields_out, double *diag_out)
+{
+  if (!o) return -1;
+  const lattice_t *L = &o->L;
+  const int K = o->K, Qn = L->Q, D = L->D;
+  const long N = o->N;
+  const double *g = o->g[o->cur];
+  double *F = fields_out;
+  double *tmp = NULL;
+  if (!F) { tmp = (double *)malloc((size_t)K * N * sizeof(double)); if (!tmp) return -2; F = tmp; }
+  for (int k = 0; k < K; k++)
+    for (long n = 0; n < N; n++) {
+      double sum = 0.0;
+      for (int i = 0; i < Qn; i++) sum += g[((long)k * Qn + i) * N + n];
+      F[(long)k * N + n] = sum;
+    }
+  if (diag_out) {
+    const int nn[3] = { o->p.nx, o->p.ny, o->p.nz };
+    int flag_nan = 0, flag_rho = 0;
+    for (int k = 0; k < K; k++) {
+      double s = 0.0, sa = 0.0, mx = 0.0;
+      for (long n = 0; n < N; n++) {
+        double v = F[(long)k * N + n];
+        if (!isfinite(v)) flag_nan = 1;
+        s += v; sa += fabs(v);
+        if (fabs(v) > mx) mx = fabs(v);
+      }
+      diag_out[k] = s; diag_out[K + k] = sa; diag_out[2 * K + k] = mx;
+    }
+    double maxdiv = 0.0, minrho = INFINITY, minp = INFINITY;
+    for (int z = 0; z < nn[2]; z++) for (int y = 0; y < nn[1]; y++) for (int x = 0; x < nn[0]; x++) {
+      const int xi[3] = { x, y, z };
+      long n = cell_index(o, x, y, z);
+      double div = 0.0;
+      for (int i = 0; i < Qn; i++) {
+        int q[3] = { x, y, z };
+        for (int a = 0; a < D; a++) {
+          q[a] = xi[a] + L->c[i][a];
+          if (q[a] < 0) q[a] = o->p.bc[2 * a] == ORC_BC_PERIODIC ? q[a] + nn[a] : 0;
+          else if (q[a] >= nn[a]) q[a] = o->p.bc[2 * a + 1] == ORC_BC_PERIODIC ? q[a] - nn[a] : nn[a] - 1;
+        }
+        long nq = cell_index(o, q[0], q[1], q[2]);
+        double cB = 0.0;
+        for (int a = 0; a < D; a++) cB += (double)L->c[i][a] * F[(long)(o->iB + a) * N + nq];
+        div += L->w[i] * cB;
+      }
+      div /= L->cs2;
+      if (fabs(div) > maxdiv) maxdiv = fabs(div);
+      if (o->p.scheme == ORC_IDEAL) {
+        double rho = F[n], mu = 0.0, B2 = 0.0;
+        for (int b = 0; b < 3; b++) {
+          double m = F[(long)(1 + b) * N + n], B = F[(long)(5 + b) * N + n];
+          mu += m * (m / rho); B2 += B * B;
+        }
+        double p = (o->p.gamma - 1.0) * (F[4 * N + n] - 0.5 * mu - 0.5 * B2);
+        if (rho < minrho) minrho = rho;
+        if (p < minp) minp = p;
+        if (!(rho > 0.0)) flag_rho = 1;
+      } else {
+        if (F[n] < minp) minp = F[n];
+        minrho = 1.0;
+      }
+    }
+    diag_out[3 * K] = maxdiv; diag_out[3 * K + 1] = minrho; diag_out[3 * K + 2] = minp;
+    diag_out[3 * K + 3] = (double)(flag_nan + 2 * flag_rho);
+  }
+  free(tmp);
+  return 0;
+}

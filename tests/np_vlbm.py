@@ -1,0 +1,254 @@
+"""A second, independent writing of the VLBM step (Eq.2-4, 8, 11-14):
+array-at-a-time numpy with np.roll streaming, no per-cell loop.  It exists only to pin the C oracle
+(pin P6) — two writings of the same equations by different routes must agree to round-off.
+Everything here is typed from the paper's formulas in tensor form (outer products, traces), not
+from oracle/vlbm_oracle.c.
+"""
+import numpy as np
+
+PERIODIC, ZEROGRAD, INFLOW = 0, 1, 2
+FLUID, FROZEN, SOLID = 0, 1, 2
+
+
+def lattice_np(name):
+    """velocities [Q, 3] and weights [Q] built from shells, then ordered as reading A2."""
+    if name == "D1Q3":
+        c = [(0, 0, 0), (1, 0, 0), (-1, 0, 0)]
+        w = [2 / 3, 1 / 6, 1 / 6]
+        D = 1
+    elif name == "D2Q9":
+        c = [(0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0),
+             (1, 1, 0), (-1, -1, 0), (1, -1, 0), (-1, 1, 0)]
+        w = [4 / 9] + [1 / 9] * 4 + [1 / 36] * 4
+        D = 2
+    elif name == "D3Q19":
+        c = [(0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)]
+        for (a, b) in ((0, 1), (0, 2), (1, 2)):
+            for (sa, sb) in ((1, 1), (-1, -1), (1, -1), (-1, 1)):
+                v = [0, 0, 0]
+                v[a], v[b] = sa, sb
+                c.append(tuple(v))
+        w = [1 / 3] + [1 / 18] * 6 + [1 / 36] * 12
+        D = 3
+    elif name == "D2Q5":
+        c = [(0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0)]
+        w = [1 / 3] + [1 / 6] * 4
+        D = 2
+    elif name == "D3Q7":
+        c = [(0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)]
+        w = [1 / 4] + [1 / 8] * 6
+        D = 3
+    else:
+        raise ValueError(name)
+    c = np.array(c, dtype=int)
+    w = np.array(w, dtype=float)
+    cs2 = float((w * c[:, 0] ** 2).sum())
+    return D, c, w, cs2
+
+
+def flux_ideal(Q, gamma, D):
+    """Eq.11 in tensor form. Q: [8, ...] -> Phi [8, 3, ...] (axes >= D are zero)."""
+    rho, m, E, B = Q[0], Q[1:4], Q[4], Q[5:8]
+    u = m / rho
+    B2 = (B * B).sum(0)
+    p = (gamma - 1.0) * (E - 0.5 * (m * u).sum(0) - 0.5 * B2)     # Eq.8
+    pt = p + 0.5 * B2
+    uB = (u * B).sum(0)
+    Phi = np.zeros((8, 3) + Q.shape[1:])
+    eye = np.eye(3).reshape((3, 3) + (1,) * (Q.ndim - 1))
+    Phi[0] = m
+    Phi[1:4] = m[:, None] * u[None, :] + pt[None, None] * eye - B[:, None] * B[None, :]   # [beta, alpha]
+    Phi[4] = (E + pt)[None] * u - B * uB[None]
+    Phi[5:8] = u[None, :] * B[:, None] - B[None, :] * u[:, None]                           # [beta, alpha]
+    Phi[:, D:] = 0.0
+    return Phi
+
+
+def flux_incres(Q, c0sq, D):
+    """A3. Q: [1+2D, ...] = (P, u, B)."""
+    P, u, B = Q[0], Q[1:1 + D], Q[1 + D:1 + 2 * D]
+    B2 = (B * B).sum(0)
+    Phi = np.zeros((1 + 2 * D, 3) + Q.shape[1:])
+    eye = np.eye(D).reshape((D, D) + (1,) * (Q.ndim - 1))
+    Phi[0, :D] = c0sq * u
+    Phi[1:1 + D, :D] = u[:, None] * u[None, :] + (P + 0.5 * B2)[None, None] * eye - B[:, None] * B[None, :]
+    Phi[1 + D:, :D] = u[None, :] * B[:, None] - B[None, :] * u[:, None]
+    return Phi
+
+
+class NpVLBM:
+    """fields / populations are indexed [k, (i,) z, y, x]."""
+
+    def __init__(self, scheme, lat, shape_zyx, tau, gamma=5 / 3, c0sq=1 / 12, powell=1.0,
+                 bc=(0,) * 6, mask=None):
+        self.scheme = scheme
+        self.D, self.c, self.w, self.cs2 = lattice_np(lat)
+        self.Qn = len(self.w)
+        self.shape = tuple(shape_zyx)
+        self.K = 8 if scheme == "IDEAL" else 1 + 2 * self.D
+        self.tau = np.broadcast_to(np.asarray(tau, dtype=float), (self.K,)).copy()
+        self.gamma, self.c0sq, self.kappa = gamma, c0sq, powell
+        self.bc = tuple(bc)
+        self.iB = 5 if scheme == "IDEAL" else 1 + self.D
+        self.mask = np.zeros(self.shape, dtype=np.uint8) if mask is None else np.asarray(mask, dtype=np.uint8).reshape(self.shape)
+        self.u_solid = np.zeros(3)
+        self.B_solid = None
+        self.sphere = None
+        self.t = 0
+        self.src_acc = np.zeros(self.K)
+        zz, yy, xx = np.meshgrid(*[np.arange(n) for n in self.shape], indexing="ij")
+        self.coord = (xx, yy, zz)
+        self.n_axis = (self.shape[2], self.shape[1], self.shape[0])
+
+    def flux(self, Q):
+        return flux_ideal(Q, self.gamma, self.D) if self.scheme == "IDEAL" else flux_incres(Q, self.c0sq, self.D)
+
+    def feq(self, Q, Phi):
+        # Eq.3: w_i (Q_k + c_i.Phi_k / cs2) -> [K, Qn, ...]
+        cPhi = np.tensordot(self.c.astype(float), Phi, axes=([1], [1]))     # [Qn, K, ...]
+        cPhi = np.moveaxis(cPhi, 0, 1)
+        wv = self.w.reshape((1, self.Qn) + (1,) * (Q.ndim - 1))
+        return wv * (Q[:, None] + cPhi / self.cs2)
+
+    def init(self, fields):
+        Q = np.asarray(fields, dtype=float).reshape((self.K,) + self.shape)
+        self.g = self.feq(Q, self.flux(Q))
+        self.t = 0
+
+    def moments(self):
+        return self.g.sum(1)
+
+    # -- helpers for boundaries
+    def _frozen(self):
+        fr = self.mask == FROZEN
+        for a in range(self.D):
+            if self.bc[2 * a] == INFLOW:
+                fr = fr | (self.coord[a] == 0)
+            if self.bc[2 * a + 1] == INFLOW:
+                fr = fr | (self.coord[a] == self.n_axis[a] - 1)
+        return fr
+
+    def _shift(self, arr, cvec):
+        """arr(x - c): np.roll by +c along each axis (array axes are ..., z, y, x)."""
+        out = arr
+        for a in range(self.D):
+            if cvec[a]:
+                out = np.roll(out, int(cvec[a]), axis=arr.ndim - 1 - a)
+        return out
+
+    def _solid(self):
+        """porosity d [z,y,x], uB [3,...], BB [3,...]"""
+        d = np.ones(self.shape)
+        uB = np.zeros((3,) + self.shape)
+        BB = np.zeros((3,) + self.shape)
+        sol = self.mask == SOLID
+        if sol.any():
+            d[sol] = 0.0
+            for a in range(3):
+                uB[a][sol] = self.u_solid[a]
+                if self.B_solid is not None:
+                    BB[a][sol] = self.B_solid[a][sol]
+        if self.sphere is not None:
+            c0, R, us, mh, Bs, t0 = self.sphere
+            cen = c0 + (self.t - t0) * us
+            r = np.zeros((3,) + self.shape)
+            for a in range(self.D):
+                r[a] = self.coord[a] - cen[a]
+            r2 = (r * r).sum(0)
+            ins = r2 <= R * R
+            rn = np.sqrt(r2)
+            rc = np.maximum(rn, 0.5 * R)
+            with np.errstate(invalid="ignore", divide="ignore"):
+                rh = np.where(rn > 0, r / np.where(rn > 0, rn, 1.0), 0.0)
+            mr = (mh.reshape(3, 1, 1, 1) * rh).sum(0)
+            dip = 0.5 * Bs * (R / rc) ** 3 * (3.0 * mr * rh - mh.reshape(3, 1, 1, 1))
+            d[ins] = 0.0
+            for a in range(3):
+                uB[a][ins] = us[a]
+                BB[a][ins] = dip[a][ins]
+        return d, uB, BB
+
+    def step(self, n=1):
+        for _ in range(n):
+            self._one()
+
+    def _one(self):
+        g = self.g
+        K, Qn, D = self.K, self.Qn, self.D
+        # 1. pull with periodic roll
+        f = np.empty_like(g)
+        for i in range(Qn):
+            f[:, i] = self._shift(g[:, i], self.c[i])
+        # A9: outside sources -> equilibrium of the inward neighbour's state
+        nonper = [a for a in range(D) if self.bc[2 * a] != PERIODIC]
+        if nonper:
+            Qst = g.sum(1)
+            idx = [self.coord[2], self.coord[1], self.coord[0]]      # z, y, x index arrays
+            for a in nonper:
+                na = self.n_axis[a]
+                ia = idx[2 - a].copy()
+                ia[self.coord[a] == 0] = 1
+                ia[self.coord[a] == na - 1] = na - 2
+                idx[2 - a] = ia
+            Qnb = Qst[:, idx[0], idx[1], idx[2]]
+            fnb = self.feq(Qnb, self.flux(Qnb))
+            for i in range(Qn):
+                out = np.zeros(self.shape, dtype=bool)
+                for a in nonper:
+                    s = self.coord[a] - self.c[i][a]
+                    out |= (s < 0) | (s >= self.n_axis[a])
+                f[:, i] = np.where(out[None], fnb[:, i], f[:, i])
+        # 2. moments
+        Q = f.sum(1)
+        # 3. delta = -tr(Pi_B) / (tau_B cs2)
+        tr = np.zeros(self.shape)
+        for b in range(D):
+            tr += np.tensordot(self.c[:, b].astype(float), f[self.iB + b], axes=([0], [0]))
+        delta = -tr / (self.tau[self.iB] * self.cs2)
+        # 4. Powell source
+        S = np.zeros_like(Q)
+        if self.scheme == "IDEAL":
+            u = Q[1:4] / Q[0]
+            B = Q[5:8]
+            S[1:4] = -self.kappa * delta * B
+            S[4] = -self.kappa * delta * (u * B).sum(0)
+            S[5:8] = -self.kappa * delta * u
+        else:
+            u, B = Q[1:1 + D], Q[1 + D:]
+            S[1:1 + D] = -self.kappa * delta * B
+            S[1 + D:] = -self.kappa * delta * u
+        # 5. homogenised solid
+        d, uB, BB = self._solid()
+        Qh = Q.copy()
+        if self.scheme == "IDEAL":
+            rho = Q[0]
+            u = Q[1:4] / rho
+            B = Q[5:8]
+            p = (self.gamma - 1.0) * (Q[4] - 0.5 * (Q[1:4] * u).sum(0) - 0.5 * (B * B).sum(0))
+            uh = d * u + (1.0 - d) * uB
+            Bh = d * B + (1.0 - d) * BB
+            Eh = p / (self.gamma - 1.0) + 0.5 * rho * (uh * uh).sum(0) + 0.5 * (Bh * Bh).sum(0)
+            sol = d < 1.0
+            for b in range(3):
+                Qh[1 + b] = np.where(sol, rho * uh[b], Q[1 + b])
+                Qh[5 + b] = np.where(sol, Bh[b], Q[5 + b])
+            Qh[4] = np.where(sol, Eh, Q[4])
+        else:
+            sol = d < 1.0
+            for b in range(D):
+                Qh[1 + b] = np.where(sol, d * Q[1 + b] + (1 - d) * uB[b], Q[1 + b])
+                Qh[1 + D + b] = np.where(sol, d * Q[1 + D + b] + (1 - d) * BB[b], Q[1 + D + b])
+        dQh = Qh - Q
+        S = S * d
+        # 6./7. flux, BGK, injection
+        feq = self.feq(Q, self.flux(Qh))
+        om = (1.0 / self.tau).reshape((K, 1) + (1,) * len(self.shape))
+        wv = self.w.reshape((1, Qn) + (1,) * len(self.shape))
+        gnew = f + om * (feq - f) + wv * (dQh + S)[:, None]
+        fr = self._frozen()
+        if fr.any():
+            gnew = np.where(fr[None, None], g, gnew)
+            S = np.where(fr[None], 0.0, S)
+        self.src_acc += S.reshape(K, -1).sum(1)
+        self.g = gnew
+        self.t += 1
