@@ -1,0 +1,133 @@
+/* lbmhd.h — C ABI of the B200-native vectorial lattice Boltzmann step for MHD.
+ *
+ * Implements the data-parallel hot path of arxiv/paper_2606_00641: every transported
+ * variable k carries its own population set f_{k,i}; one step is
+ *     f_{k,i}(x + c_i, t+1) = f_{k,i} + Omega^C + Omega^S                      (Eq.2)
+ * with the linear equilibrium f^eq_{k,i} = w_i (Q_k + c_i.Phi_k / c_s^2)       (Eq.3),
+ * moments Q_k = sum_i f_{k,i}                                                  (Eq.4),
+ * BGK collision and direct-injection source, the ideal-MHD flux and EOS
+ * (Eq.11, Eq.8), the Powell source (Eq.12), equilibrium-based
+ * static boundaries and homogenised moving solids (Eq.13-14).
+ * Where the paper is silent the readings A1-A15 of DESIGN.md §3 apply.
+ *
+ * Conventions
+ *  - Everything is in lattice units (dx = dt = 1, c_i in {-1,0,1}^D); the caller scales (A1).
+ *  - Macroscopic fields are fp64 SoA [K][nz][ny][nx], x fastest, at this boundary in both precisions.
+ *    IDEAL: K = 8 in every dimension, order rho, m_x, m_y, m_z, E, B_x, B_y, B_z.
+ *    INCRES: K = 1 + 2D, order P, u_1..u_D, B_1..B_D (P = kinematic pressure carrier, A3).
+ *  - Direction order: rest; +x,-x,+y,-y,+z,-z; diagonals (+,+),(-,-),(+,-),(-,+) per plane xy, xz, yz.
+ *  - Every pointer argument says whether it is a HOST or a DEVICE pointer.  The caller owns every
+ *    buffer it passes, including `workspace` (device memory, e.g. a torch tensor): the library never
+ *    allocates or frees device memory and keeps no host pointer after a call returns.
+ *  - All work is enqueued on `stream`; calls that return data to HOST memory synchronise that stream.
+ *  - No call throws or aborts.  Return value 0 = success, < 0 = error code below; the text of the last
+ *    error (per thread) is available from lbmhd_last_error().
+ *  - There is no CPU fallback: without a CUDA device every call that needs one returns LBMHD_ECUDA.
+ */
+#ifndef LBMHD_H
+#define LBMHD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lbmhd lbmhd_t;
+
+enum { LBMHD_D1Q3 = 1, LBMHD_D2Q9 = 2, LBMHD_D3Q19 = 3 };
+enum { LBMHD_IDEAL = 0, LBMHD_INCRES = 1 };
+enum { LBMHD_BC_PERIODIC = 0, LBMHD_BC_ZEROGRAD = 1, LBMHD_BC_INFLOW = 2 };
+enum { LBMHD_CELL_FLUID = 0, LBMHD_CELL_FROZEN = 1, LBMHD_CELL_SOLID = 2 };
+enum { LBMHD_STREAM_AB = 0, LBMHD_STREAM_INPLACE = 1 };
+enum {
+  LBMHD_OK = 0,
+  LBMHD_EINVAL = -1,   /* bad lattice / dims / tau <= 1/2 / NULL / inconsistent boundary kinds */
+  LBMHD_ENOMEM = -2,   /* workspace too small or misaligned */
+  LBMHD_ECUDA = -3,    /* CUDA error (sticky), text in lbmhd_last_error() */
+  LBMHD_ENUMERIC = -4  /* lbmhd_moments saw NaN/Inf or rho <= 0 (p < 0 alone is not an error) */
+};
+
+typedef struct {
+  int    scheme;        /* LBMHD_IDEAL | LBMHD_INCRES */
+  int    lattice;       /* LBMHD_D1Q3 | LBMHD_D2Q9 | LBMHD_D3Q19 */
+  int    precision;     /* 64 (fp64 populations and arithmetic) or 32 (fp32 populations and arithmetic) */
+  int    nx, ny, nz;    /* unused dims = 1 */
+  double gamma;         /* IDEAL: adiabatic index, Eq.8 */
+  double c0sq;          /* INCRES: artificial sound speed squared (A3) */
+  double nu, eta;       /* if > 0: tau of the velocity (and P) / magnetic sets := 1/2 + D/c_s^2, Eq.5 */
+  double tau[8];        /* per variable, > 1/2, order of `scheme`; all magnetic sets must share one value (A7) */
+  double powell;        /* kappa: 0 = off, 1 = Eq.12 */
+  int    bc[6];         /* xmin, xmax, ymin, ymax, zmin, zmax; periodic must be paired per axis */
+  int    streaming;     /* LBMHD_STREAM_AB (two population copies) | LBMHD_STREAM_INPLACE (one copy) */
+  int    device;        /* CUDA device ordinal */
+  void  *stream;        /* cudaStream_t to enqueue on (0 = default stream) */
+  void  *workspace;     /* DEVICE pointer, 256-byte aligned, >= lbmhd_workspace_bytes() bytes */
+  size_t workspace_bytes;
+} lbmhd_params;
+
+/* K (number of population sets) and Q (directions) for the scheme/lattice in *p; < 0 on bad input. */
+int lbmhd_num_vars(const lbmhd_params *p);
+int lbmhd_num_dirs(const lbmhd_params *p);
+
+/* Device bytes the handle needs: populations (1 or 2 copies of K*Q planes), cell mask, solid field,
+ * moments scratch, reduction scratch.  0 on bad input.  Needs no device. */
+size_t lbmhd_workspace_bytes(const lbmhd_params *p);
+
+/* Validates *p, lays the workspace out, uploads `cell_mask` (HOST uint8 [N], values LBMHD_CELL_*, or
+ * NULL = all FLUID).  Cells on a face whose kind is LBMHD_BC_INFLOW are FROZEN whatever the mask says (A10). */
+int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t **out);
+
+/* Frees the handle only (never the workspace). */
+void lbmhd_destroy(lbmhd_t *h);
+
+/* g_{k,i} = f^eq_{k,i}(Q) (Eq.3) from `fields` = fp64 [K][N]; HOST pointer if on_device == 0 (copied
+ * synchronously through the moments scratch), DEVICE pointer otherwise.  Resets the step counter. */
+int lbmhd_init(lbmhd_t *h, const double *fields, int on_device);
+
+/* n_steps >= 0 applications of the fused update (pull-stream, moments, div-B estimate, Powell source,
+ * solid blend, flux, BGK + injection, store: DESIGN.md §2), asynchronous on the stream.  A sphere set
+ * by lbmhd_set_sphere advances its centre by u_solid per step. */
+int lbmhd_step(lbmhd_t *h, int n_steps);
+
+/* Q_k(x) = sum_i g_{k,i}(x) of the stored populations into fields_out (fp64 [K][N], NULL to skip) and the
+ * diagnostics into diag_out (3K+4 doubles, NULL to skip):
+ *   [0,K) sum_x Q_k | [K,2K) sum_x |Q_k| | [2K,3K) max_x |Q_k| | max_x |div_h B|, min rho, min p, flag
+ * div_h B = sum_i w_i c_i.B(x + c_i)/c_s^2 (neighbour wrapped on periodic axes, clamped otherwise);
+ * flag = 1*(non-finite seen) + 2*(rho <= 0 seen).  INCRES: "min rho" = 1, "min p" = min P.
+ * Both pointers are HOST (on_device == 0: the call synchronises) or both DEVICE.
+ * Returns LBMHD_ENUMERIC if flag != 0 and the outputs are HOST pointers (outputs are still written). */
+int lbmhd_moments(lbmhd_t *h, double *fields_out, double *diag_out, int on_device);
+
+/* Masked solid (A8, A11): cells with mask == LBMHD_CELL_SOLID take u^B = u_solid (HOST double[3]) and
+ * B^B from B_solid (fp64 [3][N], NULL = 0); FROZEN cells keep their populations.  mask / B_solid are HOST
+ * or DEVICE pointers according to on_device.  Replaces the mask given at create. */
+int lbmhd_set_obstacle(lbmhd_t *h, const unsigned char *mask, const double u_solid[3],
+                       const double *B_solid, int on_device);
+
+/* Analytic moving sphere with a capped dipole (A12); all arguments HOST.  `centre` is the centre before
+ * the next step; before step t it is centre + (t - t_now) u_solid.  A cell is solid iff
+ * |x - c|^2 <= radius^2 with x the integer cell coordinates.  radius <= 0 removes the sphere. */
+int lbmhd_set_sphere(lbmhd_t *h, const double centre[3], double radius, const double u_solid[3],
+                     const double dipole_dir[3], double B_surface);
+
+/* Raw population access (checkpoint / tests): fp64 [K][Q][N] at this boundary in both precisions, in
+ * canonical (k, i, cell) order whatever the streaming layout.  HOST or DEVICE pointer per on_device. */
+int lbmhd_get_populations(lbmhd_t *h, double *g_out, int on_device);
+int lbmhd_set_populations(lbmhd_t *h, const double *g_in, int on_device);
+
+/* Counters: time steps done since init; kernels launched by this handle since create. */
+long long lbmhd_steps_done(const lbmhd_t *h);
+long long lbmhd_launch_count(const lbmhd_t *h);
+
+/* Measured-bandwidth probe (BabelStream-style copy b[i] = a[i] over n fp64 elements, the paper's roofline
+ * denominator is such a measurement).  a, b DEVICE pointers; enqueues `reps` launches. */
+int lbmhd_copy_probe(const double *a, double *b, size_t n, int reps, void *stream);
+
+/* Text of the last error on this thread ("" if none). */
+const char *lbmhd_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBMHD_H */

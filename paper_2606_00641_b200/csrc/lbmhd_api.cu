@@ -1,0 +1,441 @@
+// lbmhd_api.cu — host side of the C ABI declared in include/lbmhd.h: validation, workspace layout,
+// kernel dispatch on (lattice, scheme, precision), step loop.  No torch types, no device allocation:
+// the caller owns the workspace.  There is no CPU fallback anywhere in this file.
+#include "../../include/lbmhd.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <string>
+
+#include "lbmhd_kernels.cuh"
+
+using namespace lbk;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char *fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return code;
+}
+
+#define CUDA_TRY(expr)                                                                              \
+  do {                                                                                              \
+    cudaError_t e_ = (expr);                                                                        \
+    if (e_ != cudaSuccess) return fail(LBMHD_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_));      \
+  } while (0)
+
+struct Geometry {
+  int D, Q, K, NV, iU, iB;
+};
+
+bool geometry(int scheme, int lattice, Geometry *g) {
+  if (scheme != LBMHD_IDEAL && scheme != LBMHD_INCRES) return false;
+  switch (lattice) {
+    case LBMHD_D1Q3: g->D = 1; g->Q = 3; break;
+    case LBMHD_D2Q9: g->D = 2; g->Q = 9; break;
+    case LBMHD_D3Q19: g->D = 3; g->Q = 19; break;
+    default: return false;
+  }
+  g->K = scheme == LBMHD_IDEAL ? 8 : 1 + 2 * g->D;
+  g->NV = scheme == LBMHD_IDEAL ? 3 : g->D;
+  g->iU = 1;
+  g->iB = scheme == LBMHD_IDEAL ? 5 : 1 + g->D;
+  return true;
+}
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+constexpr int kMaxDiagBlocks = 1184;   // 8 x 148 SMs
+
+struct Layout {
+  size_t pstride;        // elements per population plane (N rounded up to 32)
+  size_t pop_bytes;      // one population copy
+  size_t off_pop[2], off_fields, off_mask, off_bsolid, off_partial, off_diag, total;
+};
+
+bool layout(const lbmhd_params *p, const Geometry &g, Layout *L) {
+  if (p->nx < 1 || p->ny < 1 || p->nz < 1) return false;
+  if (p->precision != 64 && p->precision != 32) return false;
+  const size_t N = (size_t)p->nx * p->ny * p->nz;
+  const size_t es = p->precision == 64 ? 8 : 4;
+  L->pstride = align_up(N, 32);
+  L->pop_bytes = align_up((size_t)g.K * g.Q * L->pstride * es, 256);
+  size_t off = 0;
+  L->off_pop[0] = off; off += L->pop_bytes;
+  L->off_pop[1] = off; off += p->streaming == LBMHD_STREAM_AB ? L->pop_bytes : 0;
+  L->off_fields = off; off += align_up((size_t)g.K * N * 8, 256);
+  L->off_mask = off; off += align_up(N, 256);
+  L->off_bsolid = off; off += align_up(3 * N * 8, 256);
+  L->off_partial = off; off += align_up((size_t)kMaxDiagBlocks * (3 * g.K + 4) * 8, 256);
+  L->off_diag = off; off += 256;
+  L->total = off;
+  return true;
+}
+
+}  // namespace
+
+struct lbmhd {
+  lbmhd_params p;
+  Geometry g;
+  Layout L;
+  size_t N;
+  double tau[8];
+  cudaStream_t stream;
+  char *ws;
+  int cur;               // which population copy holds the current state
+  long long t;           // steps done since init
+  long long launches;
+  bool have_mask, have_bsolid;
+  double usolid[3];
+  bool has_sphere;
+  double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs;
+  long long sph_t0;
+  int tx;                // x-tile of the step kernel
+};
+
+extern "C" {
+
+const char *lbmhd_last_error(void) { return g_err.c_str(); }
+
+int lbmhd_num_vars(const lbmhd_params *p) {
+  Geometry g;
+  if (!p || !geometry(p->scheme, p->lattice, &g)) return LBMHD_EINVAL;
+  return g.K;
+}
+int lbmhd_num_dirs(const lbmhd_params *p) {
+  Geometry g;
+  if (!p || !geometry(p->scheme, p->lattice, &g)) return LBMHD_EINVAL;
+  return g.Q;
+}
+
+size_t lbmhd_workspace_bytes(const lbmhd_params *p) {
+  Geometry g;
+  Layout L;
+  if (!p || !geometry(p->scheme, p->lattice, &g) || !layout(p, g, &L)) return 0;
+  return L.total;
+}
+
+void lbmhd_destroy(lbmhd_t *h) { delete h; }
+
+long long lbmhd_steps_done(const lbmhd_t *h) { return h ? h->t : -1; }
+long long lbmhd_launch_count(const lbmhd_t *h) { return h ? h->launches : -1; }
+
+int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t **out) {
+  if (!out) return fail(LBMHD_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!p) return fail(LBMHD_EINVAL, "params is NULL");
+  Geometry g;
+  if (!geometry(p->scheme, p->lattice, &g)) return fail(LBMHD_EINVAL, "unknown scheme %d or lattice %d", p->scheme, p->lattice);
+  Layout L;
+  if (!layout(p, g, &L)) return fail(LBMHD_EINVAL, "bad dims %d x %d x %d or precision %d", p->nx, p->ny, p->nz, p->precision);
+  if (p->streaming != LBMHD_STREAM_AB)
+    return fail(LBMHD_EINVAL, "streaming mode %d is not built yet (only LBMHD_STREAM_AB)", p->streaming);
+  if (g.D < 2 && p->ny != 1) return fail(LBMHD_EINVAL, "ny must be 1 on a 1D lattice");
+  if (g.D < 3 && p->nz != 1) return fail(LBMHD_EINVAL, "nz must be 1 on a 1D/2D lattice");
+  if ((size_t)p->ny > 65535 || (size_t)p->nz > 65535) return fail(LBMHD_EINVAL, "ny, nz must be <= 65535");
+  const int nn[3] = {p->nx, p->ny, p->nz};
+  for (int a = 0; a < g.D; a++) {
+    const int lo = p->bc[2 * a], hi = p->bc[2 * a + 1];
+    if (lo < 0 || lo > 2 || hi < 0 || hi > 2) return fail(LBMHD_EINVAL, "bad boundary kind on axis %d", a);
+    if ((lo == LBMHD_BC_PERIODIC) != (hi == LBMHD_BC_PERIODIC)) return fail(LBMHD_EINVAL, "periodic must be paired on axis %d", a);
+    if (lo != LBMHD_BC_PERIODIC && nn[a] < 3) return fail(LBMHD_EINVAL, "non-periodic axis %d needs >= 3 cells", a);
+  }
+  lbmhd_t *h = new lbmhd_t();
+  h->p = *p; h->g = g; h->L = L;
+  h->N = (size_t)p->nx * p->ny * p->nz;
+  for (int k = 0; k < g.K; k++) h->tau[k] = p->tau[k];
+  const double cs2 = 1.0 / 3.0;
+  if (p->nu > 0.0) {    // Eq.5
+    for (int b = 0; b < g.NV; b++) h->tau[g.iU + b] = 0.5 + p->nu / cs2;
+    if (p->scheme == LBMHD_INCRES) h->tau[0] = 0.5 + p->nu / cs2;
+  }
+  if (p->eta > 0.0)
+    for (int b = 0; b < g.NV; b++) h->tau[g.iB + b] = 0.5 + p->eta / cs2;
+  for (int k = 0; k < g.K; k++)
+    if (!(h->tau[k] > 0.5)) { delete h; return fail(LBMHD_EINVAL, "tau[%d] = %g must be > 1/2", k, p->tau[k]); }
+  for (int b = 1; b < g.NV; b++)
+    if (h->tau[g.iB + b] != h->tau[g.iB]) { delete h; return fail(LBMHD_EINVAL, "all magnetic sets must share one tau (A7)"); }
+  if (p->scheme == LBMHD_IDEAL && !(p->gamma > 1.0)) { delete h; return fail(LBMHD_EINVAL, "gamma must be > 1"); }
+  if (!p->workspace) { delete h; return fail(LBMHD_EINVAL, "workspace is NULL"); }
+  if (((uintptr_t)p->workspace & 255) != 0) { delete h; return fail(LBMHD_ENOMEM, "workspace must be 256-byte aligned"); }
+  if (p->workspace_bytes < L.total) {
+    delete h;
+    return fail(LBMHD_ENOMEM, "workspace has %zu bytes, need %zu", p->workspace_bytes, L.total);
+  }
+  h->ws = (char *)p->workspace;
+  h->stream = (cudaStream_t)p->stream;
+  h->tx = 64;
+  if (const char *e = getenv("LBMHD_TX")) {
+    const int v = atoi(e);
+    if (v == 32 || v == 64 || v == 128) h->tx = v;
+  }
+  cudaError_t e = cudaSetDevice(p->device);
+  if (e != cudaSuccess) { delete h; return fail(LBMHD_ECUDA, "cudaSetDevice(%d): %s", p->device, cudaGetErrorString(e)); }
+  h->have_mask = cell_mask != nullptr;
+  if (cell_mask) {
+    e = cudaMemcpyAsync(h->ws + L.off_mask, cell_mask, h->N, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) { delete h; return fail(LBMHD_ECUDA, "mask upload: %s", cudaGetErrorString(e)); }
+  }
+  *out = h;
+  return LBMHD_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------------
+// kernel dispatch
+// ------------------------------------------------------------------------------------------------------
+namespace {
+
+template <int LAT, int SCHEME, typename real> struct Ops {
+  using L = Lattice<LAT>;
+  static constexpr int D = L::D, Q = L::Q, K = Vars<SCHEME, L::D>::K;
+  static constexpr int TXAUX = 64;   // x-tile of init / moments
+
+  static real *pops(lbmhd_t *h, int which) { return (real *)(h->ws + h->L.off_pop[which]); }
+
+  static dim3 grid(const lbmhd_t *h, int tx) { return dim3((h->p.nx + tx - 1) / tx, h->p.ny, h->p.nz); }
+
+  template <int TX> static cudaError_t launch_step(lbmhd_t *h, const StepArgs<real> &a) {
+    step_kernel<LAT, SCHEME, real, TX><<<grid(h, TX), dim3(TX, K), 0, h->stream>>>(a);
+    return cudaGetLastError();
+  }
+
+  static int step(lbmhd_t *h, int n_steps) {
+    StepArgs<real> a;
+    memset(&a, 0, sizeof a);
+    a.pstride = h->L.pstride;
+    a.nx = h->p.nx; a.ny = h->p.ny; a.nz = h->p.nz;
+    for (int j = 0; j < 6; j++) a.bc[j] = h->p.bc[j];
+    for (int k = 0; k < K; k++) a.omega[k] = (real)(1.0 / h->tau[k]);
+    a.inv_tauB_cs2 = (real)(1.0 / (h->tau[h->g.iB] * (1.0 / 3.0)));
+    a.kappa = (real)h->p.powell; a.gamma = (real)h->p.gamma; a.c0sq = (real)h->p.c0sq;
+    a.mask = h->have_mask ? (const unsigned char *)(h->ws + h->L.off_mask) : nullptr;
+    a.Bsolid = h->have_bsolid ? (const double *)(h->ws + h->L.off_bsolid) : nullptr;
+    for (int c = 0; c < 3; c++) a.usolid[c] = h->usolid[c];
+    a.has_sphere = h->has_sphere ? 1 : 0;
+    if (h->has_sphere) {
+      a.sph_R = h->sph_R;
+      a.sph_R2 = h->sph_R * h->sph_R;
+      a.sph_Bs = h->sph_Bs;
+      for (int c = 0; c < 3; c++) { a.sph_m[c] = h->sph_m[c]; a.sph_u[c] = h->sph_u[c]; }
+    }
+    for (int s = 0; s < n_steps; s++) {
+      a.src = pops(h, h->cur);
+      a.dst = pops(h, 1 - h->cur);
+      if (h->has_sphere) {
+        // A12: centre before step t is c0 + (t - t0) u^B; product and sum rounded separately, like the oracle
+        const volatile double dt = (double)(h->t - h->sph_t0);
+        for (int c = 0; c < 3; c++) {
+          const volatile double prod = dt * h->sph_u[c];
+          a.sph_c[c] = h->sph_c0[c] + prod;
+        }
+      }
+      cudaError_t e;
+      switch (h->tx) {
+        case 32: e = launch_step<32>(h, a); break;
+        case 128: e = launch_step<128>(h, a); break;
+        default: e = launch_step<64>(h, a); break;
+      }
+      if (e != cudaSuccess) return fail(LBMHD_ECUDA, "step kernel launch: %s", cudaGetErrorString(e));
+      h->cur = 1 - h->cur;
+      h->t += 1;
+      h->launches += 1;
+    }
+    return LBMHD_OK;
+  }
+
+  static int init(lbmhd_t *h, const double *fields_dev) {
+    init_kernel<LAT, SCHEME, real, TXAUX><<<grid(h, TXAUX), dim3(TXAUX, K), 0, h->stream>>>(
+        fields_dev, pops(h, 0), h->L.pstride, h->p.nx, h->p.ny, h->p.nz, (real)h->p.gamma, (real)h->p.c0sq);
+    CUDA_TRY(cudaGetLastError());
+    h->launches += 1;
+    return LBMHD_OK;
+  }
+
+  static int moments(lbmhd_t *h, double *fields_dev) {
+    moments_kernel<LAT, SCHEME, real, TXAUX><<<grid(h, TXAUX), dim3(TXAUX, K), 0, h->stream>>>(
+        pops(h, h->cur), h->L.pstride, fields_dev, h->p.nx, h->p.ny, h->p.nz);
+    CUDA_TRY(cudaGetLastError());
+    h->launches += 1;
+    return LBMHD_OK;
+  }
+
+  static int diag(lbmhd_t *h, const double *fields_dev, double *diag_dev) {
+    size_t want = (h->N + kDiagThreads - 1) / kDiagThreads;
+    const int nb = (int)(want < (size_t)kMaxDiagBlocks ? want : (size_t)kMaxDiagBlocks);
+    double *partial = (double *)(h->ws + h->L.off_partial);
+    diag_partial_kernel<LAT, SCHEME><<<nb, kDiagThreads, 0, h->stream>>>(fields_dev, partial, h->p.nx, h->p.ny, h->p.nz,
+                                                                          h->p.bc[0], h->p.bc[2], h->p.bc[4], h->p.gamma);
+    CUDA_TRY(cudaGetLastError());
+    diag_final_kernel<<<1, kDiagThreads, 0, h->stream>>>(partial, nb, K, diag_dev);
+    CUDA_TRY(cudaGetLastError());
+    h->launches += 2;
+    return LBMHD_OK;
+  }
+
+  static int pops_export(lbmhd_t *h, double *out_dev) {
+    pops_export_kernel<real><<<1184, 256, 0, h->stream>>>(pops(h, h->cur), h->L.pstride, out_dev, h->N, K * Q);
+    CUDA_TRY(cudaGetLastError());
+    h->launches += 1;
+    return LBMHD_OK;
+  }
+  static int pops_import(lbmhd_t *h, const double *in_dev) {
+    pops_import_kernel<real><<<1184, 256, 0, h->stream>>>(in_dev, pops(h, h->cur), h->L.pstride, h->N, K * Q);
+    CUDA_TRY(cudaGetLastError());
+    h->launches += 1;
+    return LBMHD_OK;
+  }
+};
+
+struct OpTable {
+  int (*step)(lbmhd_t *, int);
+  int (*init)(lbmhd_t *, const double *);
+  int (*moments)(lbmhd_t *, double *);
+  int (*diag)(lbmhd_t *, const double *, double *);
+  int (*pops_export)(lbmhd_t *, double *);
+  int (*pops_import)(lbmhd_t *, const double *);
+};
+
+template <int LAT, int SCHEME, typename real> OpTable make_table() {
+  using O = Ops<LAT, SCHEME, real>;
+  return OpTable{O::step, O::init, O::moments, O::diag, O::pops_export, O::pops_import};
+}
+
+template <int LAT> OpTable pick2(int scheme, int precision) {
+  if (scheme == LBMHD_IDEAL) return precision == 64 ? make_table<LAT, kIdeal, double>() : make_table<LAT, kIdeal, float>();
+  return precision == 64 ? make_table<LAT, kIncres, double>() : make_table<LAT, kIncres, float>();
+}
+
+OpTable pick(const lbmhd_t *h) {
+  switch (h->p.lattice) {
+    case LBMHD_D1Q3: return pick2<1>(h->p.scheme, h->p.precision);
+    case LBMHD_D2Q9: return pick2<2>(h->p.scheme, h->p.precision);
+    default: return pick2<3>(h->p.scheme, h->p.precision);
+  }
+}
+
+int use_device(const lbmhd_t *h) {
+  CUDA_TRY(cudaSetDevice(h->p.device));
+  return LBMHD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lbmhd_init(lbmhd_t *h, const double *fields, int on_device) {
+  if (!h || !fields) return fail(LBMHD_EINVAL, "NULL argument");
+  if (int rc = use_device(h)) return rc;
+  const double *src = fields;
+  if (!on_device) {
+    double *scratch = (double *)(h->ws + h->L.off_fields);
+    CUDA_TRY(cudaMemcpyAsync(scratch, fields, (size_t)h->g.K * h->N * 8, cudaMemcpyHostToDevice, h->stream));
+    src = scratch;
+  }
+  h->cur = 0; h->t = 0; h->sph_t0 = 0;
+  const int rc = pick(h).init(h, src);
+  if (rc) return rc;
+  if (!on_device) CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LBMHD_OK;
+}
+
+int lbmhd_step(lbmhd_t *h, int n_steps) {
+  if (!h || n_steps < 0) return fail(LBMHD_EINVAL, "bad handle or n_steps");
+  if (int rc = use_device(h)) return rc;
+  return pick(h).step(h, n_steps);
+}
+
+int lbmhd_moments(lbmhd_t *h, double *fields_out, double *diag_out, int on_device) {
+  if (!h) return fail(LBMHD_EINVAL, "NULL handle");
+  if (int rc = use_device(h)) return rc;
+  const OpTable op = pick(h);
+  const size_t fbytes = (size_t)h->g.K * h->N * 8;
+  const int nd = 3 * h->g.K + 4;
+  double *fdev = (on_device && fields_out) ? fields_out : (double *)(h->ws + h->L.off_fields);
+  if (int rc = op.moments(h, fdev)) return rc;
+  double *ddev = (double *)(h->ws + h->L.off_diag);
+  if (diag_out) {
+    if (on_device) ddev = diag_out;
+    if (int rc = op.diag(h, fdev, ddev)) return rc;
+  }
+  if (on_device) return LBMHD_OK;
+  if (fields_out) CUDA_TRY(cudaMemcpyAsync(fields_out, fdev, fbytes, cudaMemcpyDeviceToHost, h->stream));
+  if (diag_out) CUDA_TRY(cudaMemcpyAsync(diag_out, ddev, nd * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  if (diag_out && diag_out[nd - 1] != 0.0)
+    return fail(LBMHD_ENUMERIC, "non-finite value or rho <= 0 seen (flag %g)", diag_out[nd - 1]);
+  return LBMHD_OK;
+}
+
+int lbmhd_set_obstacle(lbmhd_t *h, const unsigned char *mask, const double u_solid[3], const double *B_solid, int on_device) {
+  if (!h || !mask) return fail(LBMHD_EINVAL, "NULL argument");
+  if (int rc = use_device(h)) return rc;
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  CUDA_TRY(cudaMemcpyAsync(h->ws + h->L.off_mask, mask, h->N, kind, h->stream));
+  h->have_mask = true;
+  h->have_bsolid = B_solid != nullptr;
+  if (B_solid) CUDA_TRY(cudaMemcpyAsync(h->ws + h->L.off_bsolid, B_solid, 3 * h->N * 8, kind, h->stream));
+  for (int c = 0; c < 3; c++) h->usolid[c] = u_solid ? u_solid[c] : 0.0;
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LBMHD_OK;
+}
+
+int lbmhd_set_sphere(lbmhd_t *h, const double centre[3], double radius, const double u_solid[3],
+                     const double dipole_dir[3], double B_surface) {
+  if (!h) return fail(LBMHD_EINVAL, "NULL handle");
+  if (!(radius > 0.0)) { h->has_sphere = false; return LBMHD_OK; }
+  if (!centre || !u_solid || !dipole_dir) return fail(LBMHD_EINVAL, "NULL argument");
+  h->has_sphere = true;
+  for (int c = 0; c < 3; c++) { h->sph_c0[c] = centre[c]; h->sph_u[c] = u_solid[c]; h->sph_m[c] = dipole_dir[c]; }
+  h->sph_R = radius; h->sph_Bs = B_surface; h->sph_t0 = h->t;
+  return LBMHD_OK;
+}
+
+static int pops_io(lbmhd_t *h, double *out, const double *in, int on_device) {
+  if (!h || (!out && !in)) return fail(LBMHD_EINVAL, "NULL argument");
+  if (int rc = use_device(h)) return rc;
+  const OpTable op = pick(h);
+  const size_t bytes = (size_t)h->g.K * h->g.Q * h->N * 8;
+  if (on_device) return out ? op.pops_export(h, out) : op.pops_import(h, in);
+  // host path: stage through the not-current population copy when it is large enough (fp64 A/B), plane by plane otherwise
+  if (h->p.precision != 64) return fail(LBMHD_EINVAL, "host population I/O needs precision 64 (use device pointers for fp32)");
+  double *stage = (double *)(h->ws + h->L.off_pop[1 - h->cur]);
+  if (bytes > h->L.pop_bytes) return fail(LBMHD_ENOMEM, "staging buffer too small");
+  if (out) {
+    if (int rc = op.pops_export(h, stage)) return rc;
+    CUDA_TRY(cudaMemcpyAsync(out, stage, bytes, cudaMemcpyDeviceToHost, h->stream));
+  } else {
+    CUDA_TRY(cudaMemcpyAsync(stage, in, bytes, cudaMemcpyHostToDevice, h->stream));
+    if (int rc = op.pops_import(h, stage)) return rc;
+  }
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LBMHD_OK;
+}
+
+int lbmhd_get_populations(lbmhd_t *h, double *g_out, int on_device) { return pops_io(h, g_out, nullptr, on_device); }
+int lbmhd_set_populations(lbmhd_t *h, const double *g_in, int on_device) { return pops_io(h, nullptr, g_in, on_device); }
+
+int lbmhd_copy_probe(const double *a, double *b, size_t n, int reps, void *stream) {
+  if (!a || !b || reps < 0) return fail(LBMHD_EINVAL, "bad argument");
+  for (int r = 0; r < reps; r++) {
+    copy_probe_kernel<<<148 * 8, 256, 0, (cudaStream_t)stream>>>((const double2 *)a, (double2 *)b, n / 2);
+    CUDA_TRY(cudaGetLastError());
+  }
+  return LBMHD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,559 @@
+// lbmhd_kernels.cuh — CUDA kernels of the fused VLBM step for sm_100a.
+//
+// Mapping: ONE THREAD PER (CELL, VARIABLE).  A block owns TX consecutive x-cells of one (y, z) row and
+// all K population sets: blockDim = (TX, K), so every warp is 32 consecutive x of ONE variable k and
+// each of its Q loads / Q stores is one fully coalesced 32*sizeof(real) row segment of plane (k, i).
+// A thread keeps only its own Q populations in registers (19 fp64 for D3Q19) — the 8 x 19 = 152 fp64
+// of a D3Q19 cell do not fit one thread's 255 registers.  The only coupling between the K sets of a
+// cell is the K zeroth moments plus tr Pi_B; they go through (K+1)*TX reals of shared memory and one
+// __syncthreads().  The per-variable branches below are warp-uniform (k = threadIdx.y).
+//
+// DRAM traffic per cell update = K*Q loads + K*Q stores, each population read exactly once (pull
+// scheme: population (k,i) at x - c_i is read only by cell x).  Shifts in x misalign a warp's 256-byte
+// segment by one element; the straddled 32-byte sector is re-read from L2/L1, not from DRAM.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "lbmhd_lattice.cuh"
+
+namespace lbk {
+
+enum { BC_PERIODIC = 0, BC_ZEROGRAD = 1, BC_INFLOW = 2 };
+enum { CELL_FLUID = 0, CELL_FROZEN = 1, CELL_SOLID = 2 };
+
+template <typename real> struct StepArgs {
+  const real *src;              // populations read (plane (k,i) at (k*Q+i)*pstride)
+  real *dst;                    // populations written
+  size_t pstride;               // elements between planes
+  int nx, ny, nz;
+  int bc[6];
+  real omega[8];                // 1 / tau_k
+  real inv_tauB_cs2;            // 1 / (tau_B c_s^2)
+  real kappa, gamma, c0sq;
+  const unsigned char *mask;    // [N] or nullptr
+  const double *Bsolid;         // [3][N] or nullptr
+  double usolid[3];
+  int has_sphere;
+  double sph_c[3], sph_R, sph_R2, sph_m[3], sph_Bs, sph_u[3];
+};
+
+// ---- homogenised solid state at a cell (Eq.13-14; A8, A11, A12) ----------
+// Returns true when the cell is solid (porosity d = 0) and fills uS, BS.  The sphere decision
+// |x - c|^2 <= R^2 is taken in fp64 with separately rounded products and sums, the order the oracle uses,
+// so both sides agree on the integer outcome.
+template <typename real, int D>
+__device__ __forceinline__ bool solid_state(const StepArgs<real> &a, int x, int y, int z, size_t n, double uS[3],
+                                            double BS[3]) {
+  if (a.has_sphere) {
+    double r[3];
+    r[0] = __dsub_rn((double)x, a.sph_c[0]);
+    r[1] = D > 1 ? __dsub_rn((double)y, a.sph_c[1]) : 0.0;
+    r[2] = D > 2 ? __dsub_rn((double)z, a.sph_c[2]) : 0.0;
+    double r2 = __dmul_rn(r[0], r[0]);
+    r2 = __dadd_rn(r2, __dmul_rn(r[1], r[1]));
+    r2 = __dadd_rn(r2, __dmul_rn(r[2], r[2]));
+    if (r2 <= a.sph_R2) {
+      const double rn = sqrt(r2);
+      const double rc = rn > 0.5 * a.sph_R ? rn : 0.5 * a.sph_R;
+      const double q = a.sph_R / rc;
+      const double amp = 0.5 * a.sph_Bs * (q * q * q);
+      double rh[3], mr = 0.0;
+#pragma unroll
+      for (int c = 0; c < 3; c++) {
+        rh[c] = rn > 0.0 ? r[c] / rn : 0.0;
+        mr += a.sph_m[c] * rh[c];
+      }
+#pragma unroll
+      for (int c = 0; c < 3; c++) {
+        BS[c] = amp * (3.0 * mr * rh[c] - a.sph_m[c]);
+        uS[c] = a.sph_u[c];
+      }
+      return true;
+    }
+  }
+  if (a.mask != nullptr && a.mask[n] == CELL_SOLID) {
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+      uS[c] = a.usolid[c];
+      BS[c] = a.Bsolid != nullptr ? a.Bsolid[(size_t)c * ((size_t)a.nx * a.ny * a.nz) + n] : 0.0;
+    }
+    return true;
+  }
+  return false;
+}
+
+// ---- flux row of variable k: Phi_k,alpha(Qh), alpha < D (Eq.11, Eq.8; A3) -------
+// Qh is the (possibly solid-blended) state; `p` the gas pressure of the unblended state (A8 keeps p).
+// k is warp-uniform, so the switch does not diverge.
+template <int SCHEME, int D, typename real>
+__device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real c0sq, real Phi[3]) {
+  Phi[0] = Phi[1] = Phi[2] = real(0);
+  if (SCHEME == kIdeal) {
+    const real rho = Qh[0], E = Qh[4];
+    const real *m = Qh + 1, *B = Qh + 5;
+    if (k == 0) {
+#pragma unroll
+      for (int a = 0; a < D; a++) Phi[a] = m[a];
+      return;
+    }
+    const real ir = real(1) / rho;
+    const real u[3] = {m[0] * ir, m[1] * ir, m[2] * ir};
+    if (k >= 5) {   // induction: u_a B_b - B_a u_b
+      const int b = k - 5;
+      const real Bb = b == 0 ? B[0] : (b == 1 ? B[1] : B[2]);
+      const real ub = b == 0 ? u[0] : (b == 1 ? u[1] : u[2]);
+#pragma unroll
+      for (int a = 0; a < D; a++) Phi[a] = u[a] * Bb - B[a] * ub;
+      return;
+    }
+    const real B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
+    const real mu = m[0] * u[0] + m[1] * u[1] + m[2] * u[2];
+    const real p = (gamma - real(1)) * (E - real(0.5) * mu - real(0.5) * B2);
+    const real pt = p + real(0.5) * B2;
+    if (k == 4) {
+      const real uB = u[0] * B[0] + u[1] * B[1] + u[2] * B[2];
+#pragma unroll
+      for (int a = 0; a < D; a++) Phi[a] = (E + pt) * u[a] - B[a] * uB;
+      return;
+    }
+    const int b = k - 1;   // momentum: m_b u_a + pt delta_ab - B_b B_a
+    const real mb = b == 0 ? m[0] : (b == 1 ? m[1] : m[2]);
+    const real Bb = b == 0 ? B[0] : (b == 1 ? B[1] : B[2]);
+#pragma unroll
+    for (int a = 0; a < D; a++) Phi[a] = mb * u[a] + (a == b ? pt : real(0)) - Bb * B[a];
+  } else {
+    const real P = Qh[0];
+    const real *u = Qh + 1, *B = Qh + 1 + D;
+    if (k == 0) {
+#pragma unroll
+      for (int a = 0; a < D; a++) Phi[a] = c0sq * u[a];
+      return;
+    }
+    if (k >= 1 + D) {
+      const int b = k - 1 - D;
+      real Bb = B[0], ub = u[0];
+#pragma unroll
+      for (int c = 1; c < D; c++)
+        if (b == c) { Bb = B[c]; ub = u[c]; }
+#pragma unroll
+      for (int a = 0; a < D; a++) Phi[a] = u[a] * Bb - B[a] * ub;
+      return;
+    }
+    real B2 = real(0);
+#pragma unroll
+    for (int c = 0; c < D; c++) B2 += B[c] * B[c];
+    const real pt = P + real(0.5) * B2;
+    const int b = k - 1;
+    real Bb = B[0], ub = u[0];
+#pragma unroll
+    for (int c = 1; c < D; c++)
+      if (b == c) { Bb = B[c]; ub = u[c]; }
+#pragma unroll
+    for (int a = 0; a < D; a++) Phi[a] = ub * u[a] + (a == b ? pt : real(0)) - Bb * B[a];
+  }
+}
+
+// register-array element by a runtime (warp-uniform) index without spilling the array to local memory
+template <int K, typename real> __device__ __forceinline__ real pick(const real *v, int k) {
+  real r = v[0];
+#pragma unroll
+  for (int l = 1; l < K; l++)
+    if (k == l) r = v[l];
+  return r;
+}
+
+// ---- Powell source row S_k / (-kappa delta) (Eq.12): (0, B, u.B, u) resp. (0, B, u) ----------
+template <int SCHEME, int D, typename real>
+__device__ __forceinline__ real powell_row(int k, const real *Qv) {
+  if (k == 0) return real(0);
+  if (SCHEME == kIdeal) {
+    if (k <= 3) return k == 1 ? Qv[5] : (k == 2 ? Qv[6] : Qv[7]);
+    const real ir = real(1) / Qv[0];
+    if (k == 4) return (Qv[1] * Qv[5] + Qv[2] * Qv[6] + Qv[3] * Qv[7]) * ir;
+    return (k == 5 ? Qv[1] : (k == 6 ? Qv[2] : Qv[3])) * ir;
+  } else {
+    real r = real(0);
+#pragma unroll
+    for (int c = 0; c < D; c++) {
+      if (k == 1 + c) r = Qv[1 + D + c];
+      if (k == 1 + D + c) r = Qv[1 + c];
+    }
+    return r;
+  }
+}
+
+// ---- blended state Q^ of a solid cell with porosity d = 0 (A8): rho and p kept, u = u^B, B = B^B -----------
+template <int SCHEME, int D, typename real>
+__device__ __forceinline__ void solid_blend(const real *Qv, real gamma, const double uS[3], const double BS[3], real *Qh) {
+  if (SCHEME == kIdeal) {
+    const real rho = Qv[0];
+    const real ir = real(1) / rho;
+    const real mu = (Qv[1] * Qv[1] + Qv[2] * Qv[2] + Qv[3] * Qv[3]) * ir;
+    const real B2 = Qv[5] * Qv[5] + Qv[6] * Qv[6] + Qv[7] * Qv[7];
+    const real p = (gamma - real(1)) * (Qv[4] - real(0.5) * mu - real(0.5) * B2);
+    real uh2 = real(0), Bh2 = real(0);
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+      const real uh = (real)uS[c], Bh = (real)BS[c];
+      Qh[1 + c] = rho * uh;
+      Qh[5 + c] = Bh;
+      uh2 += uh * uh;
+      Bh2 += Bh * Bh;
+    }
+    Qh[0] = rho;
+    Qh[4] = p / (gamma - real(1)) + real(0.5) * rho * uh2 + real(0.5) * Bh2;
+  } else {
+    Qh[0] = Qv[0];
+#pragma unroll
+    for (int c = 0; c < D; c++) {
+      Qh[1 + c] = (real)uS[c];
+      Qh[1 + D + c] = (real)BS[c];
+    }
+  }
+}
+
+// =====================================================================================================
+// Fused step kernel, A/B buffers: pull-stream + moments + div-B estimate + Powell source + solid blend +
+// flux + BGK + direct injection + store (DESIGN.md §2 steps S1-S8; Eq.2-4, 8, 11-14).
+// =====================================================================================================
+template <int LAT, int SCHEME, typename real, int TX>
+__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K)
+step_kernel(const StepArgs<real> a) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, Q = L::Q;
+  using V = Vars<SCHEME, D>;
+  constexpr int K = V::K, iB = V::iB;
+  __shared__ real sQ[K][TX];
+  __shared__ real sTr[D][TX];
+
+  const int tx = threadIdx.x, k = threadIdx.y;
+  const int x = blockIdx.x * TX + tx, y = blockIdx.y, z = blockIdx.z;
+  const int nx = a.nx, ny = a.ny, nz = a.nz;
+  const bool active = x < nx;
+  const size_t n = ((size_t)z * ny + y) * nx + (active ? x : 0);
+  const size_t ps = a.pstride;
+  const real *__restrict__ srck = a.src + (size_t)k * Q * ps;
+  real *__restrict__ dstk = a.dst + (size_t)k * Q * ps;
+
+  const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
+  const bool x_lo = x == 0, x_hi = x == nx - 1;
+  const bool y_lo = D > 1 && y == 0, y_hi = D > 1 && y == ny - 1;
+  const bool z_lo = D > 2 && z == 0, z_hi = D > 2 && z == nz - 1;
+
+  // frozen cells keep their populations: mask FROZEN or on an INFLOW face (A10)
+  bool frozen = false;
+  if (active) {
+    frozen = (a.mask != nullptr && a.mask[n] == CELL_FROZEN) || (x_lo && a.bc[0] == BC_INFLOW) ||
+             (x_hi && a.bc[1] == BC_INFLOW) || (y_lo && a.bc[2] == BC_INFLOW) || (y_hi && a.bc[3] == BC_INFLOW) ||
+             (z_lo && a.bc[4] == BC_INFLOW) || (z_hi && a.bc[5] == BC_INFLOW);
+    if (frozen) {
+#pragma unroll
+      for (int i = 0; i < Q; i++) dstk[(size_t)i * ps + n] = srck[(size_t)i * ps + n];
+    }
+  }
+  const bool work = active && !frozen;
+
+  // S1 pull: f_i(x) = g_i(x - c_i), periodic wrap; sources outside a non-periodic face are filled below
+  const int xm = x_lo ? nx - 1 : x - 1, xp = x_hi ? 0 : x + 1;
+  const int ym = y_lo ? ny - 1 : y - 1, yp = y_hi ? 0 : y + 1;
+  const int zm = z_lo ? nz - 1 : z - 1, zp = z_hi ? 0 : z + 1;
+  const bool out_xm = npx && x_lo, out_xp = npx && x_hi;
+  const bool out_ym = npy && y_lo, out_yp = npy && y_hi;
+  const bool out_zm = npz && z_lo, out_zp = npz && z_hi;
+
+  real f[Q];
+#pragma unroll
+  for (int i = 0; i < Q; i++) {
+    const int cx = L::cx(i), cy = L::cy(i), cz = L::cz(i);
+    const int sx = cx == 1 ? xm : (cx == -1 ? xp : x);
+    const int sy = cy == 1 ? ym : (cy == -1 ? yp : y);
+    const int sz = cz == 1 ? zm : (cz == -1 ? zp : z);
+    const bool outside = (cx == 1 && out_xm) || (cx == -1 && out_xp) || (cy == 1 && out_ym) || (cy == -1 && out_yp) ||
+                         (cz == 1 && out_zm) || (cz == -1 && out_zp);
+    f[i] = (work && !outside) ? srck[(size_t)i * ps + ((size_t)sz * ny + sy) * nx + sx] : real(0);
+  }
+
+  // A9 / PAPER.md:154: directions whose source is outside take the equilibrium of the inward neighbour's state
+  const bool block_bnd = out_ym || out_yp || out_zm || out_zp || (npx && (blockIdx.x == 0 || blockIdx.x == gridDim.x - 1));
+  if (block_bnd) {
+    const bool cell_bnd = work && (out_xm || out_xp || out_ym || out_yp || out_zm || out_zp);
+    if (cell_bnd) {
+      const int qx = out_xm ? x + 1 : (out_xp ? x - 1 : x);
+      const int qy = out_ym ? y + 1 : (out_yp ? y - 1 : y);
+      const int qz = out_zm ? z + 1 : (out_zp ? z - 1 : z);
+      const size_t nb = ((size_t)qz * ny + qy) * nx + qx;
+      real s = real(0);
+#pragma unroll
+      for (int j = 0; j < Q; j++) s += srck[(size_t)j * ps + nb];
+      sQ[k][tx] = s;
+    }
+    __syncthreads();
+    if (cell_bnd) {
+      real Qnb[K], Phi[3];
+#pragma unroll
+      for (int l = 0; l < K; l++) Qnb[l] = sQ[l][tx];
+      flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, Phi);
+      const real Qnbk = pick<K, real>(Qnb, k);
+#pragma unroll
+      for (int i = 0; i < Q; i++) {
+        const int cx = L::cx(i), cy = L::cy(i), cz = L::cz(i);
+        const bool outside = (cx == 1 && out_xm) || (cx == -1 && out_xp) || (cy == 1 && out_ym) ||
+                             (cy == -1 && out_yp) || (cz == 1 && out_zm) || (cz == -1 && out_zp);
+        const real cPhi = real(cx) * Phi[0] + real(cy) * Phi[1] + real(cz) * Phi[2];
+        if (outside) f[i] = real(L::w(i)) * (Qnbk + real(3) * cPhi);
+      }
+    }
+    __syncthreads();
+  }
+
+  // S2 zeroth moment of this set (index order) and S3 this set's share of tr Pi_B
+  real Qk = real(0);
+#pragma unroll
+  for (int i = 0; i < Q; i++) Qk += f[i];
+  sQ[k][tx] = Qk;
+  if (k >= iB && k < iB + D) {
+    const int b = k - iB;
+    real t = real(0);
+#pragma unroll
+    for (int i = 0; i < Q; i++) {
+      const int cb = b == 0 ? L::cx(i) : (b == 1 ? L::cy(i) : L::cz(i));   // b is warp-uniform
+      t += real(cb) * f[i];
+    }
+    sTr[b][tx] = t;
+  }
+  __syncthreads();
+  if (!work) return;
+
+  real Qv[K];
+#pragma unroll
+  for (int l = 0; l < K; l++) Qv[l] = sQ[l][tx];
+  real tr = real(0);
+#pragma unroll
+  for (int b = 0; b < D; b++) tr += sTr[b][tx];
+  const real delta = -tr * a.inv_tauB_cs2;                      // A6
+
+  // S4 Powell source, S5 solid blend
+  real S = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
+  real Qh[K];
+#pragma unroll
+  for (int l = 0; l < K; l++) Qh[l] = Qv[l];
+  real dQh = real(0);
+  double uS[3], BS[3];
+  if (solid_state<real, D>(a, x, y, z, n, uS, BS)) {
+    solid_blend<SCHEME, D, real>(Qv, a.gamma, uS, BS, Qh);
+    dQh = pick<K, real>(Qh, k) - Qk;
+    S = real(0);
+  }
+
+  // S6 flux row of this variable, S7 BGK + direct injection, S8 store
+  real Phi[3];
+  flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, Phi);
+  const real om = a.omega[k];
+  const real inj = dQh + S;
+#pragma unroll
+  for (int i = 0; i < Q; i++) {
+    const real cPhi = real(L::cx(i)) * Phi[0] + real(L::cy(i)) * Phi[1] + real(L::cz(i)) * Phi[2];
+    const real feq = real(L::w(i)) * (Qk + real(3) * cPhi);
+    dstk[(size_t)i * ps + n] = f[i] + om * (feq - f[i]) + real(L::w(i)) * inj;
+  }
+}
+
+// ---- S10 init: g_{k,i} = w_i (Q_k + c_i.Phi_k(Q)/c_s^2) (Eq.3) from fp64 fields [K][N] ---------
+template <int LAT, int SCHEME, typename real, int TX>
+__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K)
+init_kernel(const double *__restrict__ fields, real *__restrict__ g, size_t pstride, int nx, int ny, int nz, real gamma,
+            real c0sq) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, Q = L::Q, K = Vars<SCHEME, D>::K;
+  const int k = threadIdx.y;
+  const int x = blockIdx.x * TX + threadIdx.x;
+  if (x >= nx) return;
+  const size_t N = (size_t)nx * ny * nz;
+  const size_t n = ((size_t)blockIdx.z * ny + blockIdx.y) * nx + x;
+  real Qv[K], Phi[3];
+#pragma unroll
+  for (int l = 0; l < K; l++) Qv[l] = (real)fields[(size_t)l * N + n];
+  flux_row<SCHEME, D, real>(k, Qv, gamma, c0sq, Phi);
+  const real Qk = pick<K, real>(Qv, k);
+  real *gk = g + (size_t)k * Q * pstride;
+#pragma unroll
+  for (int i = 0; i < Q; i++) {
+    const real cPhi = real(L::cx(i)) * Phi[0] + real(L::cy(i)) * Phi[1] + real(L::cz(i)) * Phi[2];
+    gk[(size_t)i * pstride + n] = real(L::w(i)) * (Qk + real(3) * cPhi);
+  }
+}
+
+// ---- S9a moments: Q_k(x) = sum_i g_{k,i}(x) (Eq.4), fp64 out [K][N] --------------------------
+template <int LAT, int SCHEME, typename real, int TX>
+__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K)
+moments_kernel(const real *__restrict__ g, size_t pstride, double *__restrict__ out, int nx, int ny, int nz) {
+  using L = Lattice<LAT>;
+  constexpr int Q = L::Q;
+  const int k = threadIdx.y;
+  const int x = blockIdx.x * TX + threadIdx.x;
+  if (x >= nx) return;
+  const size_t N = (size_t)nx * ny * nz;
+  const size_t n = ((size_t)blockIdx.z * ny + blockIdx.y) * nx + x;
+  const real *gk = g + (size_t)k * Q * pstride;
+  real s = real(0);
+#pragma unroll
+  for (int i = 0; i < Q; i++) s += gk[(size_t)i * pstride + n];
+  out[(size_t)k * N + n] = (double)s;
+}
+
+// ---- S9b diagnostics: two-stage deterministic reduction with warp shuffles --------------------------------
+// slots: [0,K) sum | [K,2K) sum|.| | [2K,3K) max|.| | 3K max|div_h B| | 3K+1 min rho | 3K+2 min p | 3K+3 flag
+constexpr int kDiagThreads = 256;
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ double warp_min(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// kind: 0 sum, 1 max, 2 min.  Result valid in thread 0.
+template <int KIND> __device__ __forceinline__ double block_reduce(double v, double *sm) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  v = KIND == 0 ? warp_sum(v) : (KIND == 1 ? warp_max(v) : warp_min(v));
+  __syncthreads();
+  if (lane == 0) sm[wid] = v;
+  __syncthreads();
+  if (wid == 0) {
+    const int nw = blockDim.x >> 5;
+    v = lane < nw ? sm[lane] : (KIND == 0 ? 0.0 : (KIND == 1 ? -INFINITY : INFINITY));
+    v = KIND == 0 ? warp_sum(v) : (KIND == 1 ? warp_max(v) : warp_min(v));
+  }
+  return v;
+}
+
+template <int LAT, int SCHEME>
+__global__ void __launch_bounds__(kDiagThreads)
+diag_partial_kernel(const double *__restrict__ F, double *__restrict__ partial, int nx, int ny, int nz, int bc0, int bc2,
+                    int bc4, double gamma) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, Q = L::Q, K = Vars<SCHEME, D>::K, iB = Vars<SCHEME, D>::iB;
+  __shared__ double sm[32];
+  const size_t N = (size_t)nx * ny * nz;
+  double sum[K], asum[K], mx[K];
+#pragma unroll
+  for (int l = 0; l < K; l++) { sum[l] = 0.0; asum[l] = 0.0; mx[l] = 0.0; }
+  double maxdiv = 0.0, minrho = INFINITY, minp = INFINITY, flag_nan = 0.0, flag_rho = 0.0;
+  const bool per[3] = {bc0 == BC_PERIODIC, bc2 == BC_PERIODIC, bc4 == BC_PERIODIC};
+  const int nn[3] = {nx, ny, nz};
+  for (size_t n = (size_t)blockIdx.x * blockDim.x + threadIdx.x; n < N; n += (size_t)gridDim.x * blockDim.x) {
+    const int x = (int)(n % nx), y = (int)((n / nx) % ny), z = (int)(n / ((size_t)nx * ny));
+    const int xi[3] = {x, y, z};
+    double v[K];
+#pragma unroll
+    for (int l = 0; l < K; l++) {
+      v[l] = F[(size_t)l * N + n];
+      if (!isfinite(v[l])) flag_nan = 1.0;
+      sum[l] += v[l];
+      asum[l] += fabs(v[l]);
+      mx[l] = fmax(mx[l], fabs(v[l]));
+    }
+    double div = 0.0;
+#pragma unroll
+    for (int i = 1; i < Q; i++) {
+      int q[3] = {x, y, z};
+#pragma unroll
+      for (int c = 0; c < D; c++) {
+        q[c] = xi[c] + lat_c<L>(i, c);
+        if (q[c] < 0) q[c] = per[c] ? q[c] + nn[c] : 0;
+        else if (q[c] >= nn[c]) q[c] = per[c] ? q[c] - nn[c] : nn[c] - 1;
+      }
+      const size_t nq = ((size_t)q[2] * ny + q[1]) * nx + q[0];
+      double cB = 0.0;
+#pragma unroll
+      for (int c = 0; c < D; c++)
+        if (lat_c<L>(i, c) != 0) cB += (double)lat_c<L>(i, c) * F[(size_t)(iB + c) * N + nq];
+      div += L::w(i) * cB;
+    }
+    div *= 3.0;
+    maxdiv = fmax(maxdiv, fabs(div));
+    if (SCHEME == kIdeal) {
+      const double rho = v[0];
+      const double mu = (v[1] * v[1] + v[2] * v[2] + v[3] * v[3]) / rho;
+      const double B2 = v[5] * v[5] + v[6] * v[6] + v[7] * v[7];
+      const double p = (gamma - 1.0) * (v[4] - 0.5 * mu - 0.5 * B2);
+      minrho = fmin(minrho, rho);
+      minp = fmin(minp, p);
+      if (!(rho > 0.0)) flag_rho = 1.0;
+    } else {
+      minp = fmin(minp, v[0]);
+      minrho = 1.0;
+    }
+  }
+  double *out = partial + (size_t)blockIdx.x * (3 * K + 4);
+#pragma unroll
+  for (int l = 0; l < K; l++) {
+    double r = block_reduce<0>(sum[l], sm);
+    if (threadIdx.x == 0) out[l] = r;
+    r = block_reduce<0>(asum[l], sm);
+    if (threadIdx.x == 0) out[K + l] = r;
+    r = block_reduce<1>(mx[l], sm);
+    if (threadIdx.x == 0) out[2 * K + l] = r;
+  }
+  double r = block_reduce<1>(maxdiv, sm);
+  if (threadIdx.x == 0) out[3 * K] = r;
+  r = block_reduce<2>(minrho, sm);
+  if (threadIdx.x == 0) out[3 * K + 1] = r;
+  r = block_reduce<2>(minp, sm);
+  if (threadIdx.x == 0) out[3 * K + 2] = r;
+  r = block_reduce<1>(flag_nan, sm);
+  const double r2 = block_reduce<1>(flag_rho, sm);
+  if (threadIdx.x == 0) out[3 * K + 3] = r + 2.0 * r2;
+}
+
+// stage 2: one block folds the per-block partials in block order (deterministic)
+__global__ void __launch_bounds__(kDiagThreads)
+diag_final_kernel(const double *__restrict__ partial, int nblocks, int K, double *__restrict__ out) {
+  __shared__ double sm[32];
+  const int nslots = 3 * K + 4;
+  for (int s = 0; s < nslots; s++) {
+    const int kind = s < 2 * K ? 0 : ((s < 3 * K + 1 || s == 3 * K + 3) ? 1 : 2);
+    double v = kind == 0 ? 0.0 : (kind == 1 ? -INFINITY : INFINITY);
+    for (int b = threadIdx.x; b < nblocks; b += blockDim.x) {
+      const double p = partial[(size_t)b * nslots + s];
+      v = kind == 0 ? v + p : (kind == 1 ? fmax(v, p) : fmin(v, p));
+    }
+    double r = kind == 0 ? block_reduce<0>(v, sm) : (kind == 1 ? block_reduce<1>(v, sm) : block_reduce<2>(v, sm));
+    if (threadIdx.x == 0) out[s] = r;
+  }
+}
+
+// ---- population import / export: canonical fp64 [K*Q][N] <-> internal real planes with pstride ------------
+template <typename real>
+__global__ void pops_export_kernel(const real *__restrict__ g, size_t pstride, double *__restrict__ out, size_t N, int planes) {
+  const size_t total = N * (size_t)planes;
+  for (size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x; j < total; j += (size_t)gridDim.x * blockDim.x) {
+    const size_t pl = j / N, n = j - pl * N;
+    out[j] = (double)g[pl * pstride + n];
+  }
+}
+template <typename real>
+__global__ void pops_import_kernel(const double *__restrict__ in, real *__restrict__ g, size_t pstride, size_t N, int planes) {
+  const size_t total = N * (size_t)planes;
+  for (size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x; j < total; j += (size_t)gridDim.x * blockDim.x) {
+    const size_t pl = j / N, n = j - pl * N;
+    g[pl * pstride + n] = (real)in[j];
+  }
+}
+
+// ---- bandwidth probe: BabelStream-style copy, 2 fp64 per thread per iteration ----------------
+__global__ void __launch_bounds__(256) copy_probe_kernel(const double2 *__restrict__ a, double2 *__restrict__ b, size_t n2) {
+  for (size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x; j < n2; j += (size_t)gridDim.x * blockDim.x) b[j] = a[j];
+}
+
+}  // namespace lbk

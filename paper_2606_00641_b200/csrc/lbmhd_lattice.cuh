@@ -1,0 +1,63 @@
+// lbmhd_lattice.cuh — compile-time lattice tables for the CUDA path (A2).
+// Direction order: rest; +x,-x,+y,-y,+z,-z; diagonals (+,+),(-,-),(+,-),(-,+) per plane xy, xz, yz.
+// Gauss-Hermite weights, c_s^2 = 1/3 on all three lattices.  Every accessor is constexpr
+// and is only ever called with a compile-time index inside fully unrolled loops, so no table lives in
+// memory: the velocities become immediate offsets and the weights immediate fp constants.
+#pragma once
+
+namespace lbk {
+
+template <int LAT> struct Lattice;
+
+template <> struct Lattice<1> {   // D1Q3
+  static constexpr int D = 1, Q = 3;
+  __host__ __device__ static constexpr int cx(int i) { return i == 1 ? 1 : (i == 2 ? -1 : 0); }
+  __host__ __device__ static constexpr int cy(int) { return 0; }
+  __host__ __device__ static constexpr int cz(int) { return 0; }
+  __host__ __device__ static constexpr double w(int i) { return i == 0 ? 2.0 / 3.0 : 1.0 / 6.0; }
+};
+
+template <> struct Lattice<2> {   // D2Q9
+  static constexpr int D = 2, Q = 9;
+  __host__ __device__ static constexpr int cx(int i) {
+    constexpr int t[9] = {0, 1, -1, 0, 0, 1, -1, 1, -1};
+    return t[i];
+  }
+  __host__ __device__ static constexpr int cy(int i) {
+    constexpr int t[9] = {0, 0, 0, 1, -1, 1, -1, -1, 1};
+    return t[i];
+  }
+  __host__ __device__ static constexpr int cz(int) { return 0; }
+  __host__ __device__ static constexpr double w(int i) { return i == 0 ? 4.0 / 9.0 : (i < 5 ? 1.0 / 9.0 : 1.0 / 36.0); }
+};
+
+template <> struct Lattice<3> {   // D3Q19
+  static constexpr int D = 3, Q = 19;
+  __host__ __device__ static constexpr int cx(int i) {
+    constexpr int t[19] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
+    return t[i];
+  }
+  __host__ __device__ static constexpr int cy(int i) {
+    constexpr int t[19] = {0, 0, 0, 1, -1, 0, 0, 1, -1, -1, 1, 0, 0, 0, 0, 1, -1, 1, -1};
+    return t[i];
+  }
+  __host__ __device__ static constexpr int cz(int i) {
+    constexpr int t[19] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, -1, -1, 1, 1, -1, -1, 1};
+    return t[i];
+  }
+  __host__ __device__ static constexpr double w(int i) { return i == 0 ? 1.0 / 3.0 : (i < 7 ? 1.0 / 18.0 : 1.0 / 36.0); }
+};
+
+template <class L> __host__ __device__ constexpr int lat_c(int i, int axis) {
+  return axis == 0 ? L::cx(i) : (axis == 1 ? L::cy(i) : L::cz(i));
+}
+
+constexpr int kIdeal = 0, kIncres = 1;
+template <int SCHEME, int D> struct Vars {
+  static constexpr int K = SCHEME == kIdeal ? 8 : 1 + 2 * D;
+  static constexpr int NV = SCHEME == kIdeal ? 3 : D;      // vector components carried
+  static constexpr int iU = 1;                             // first momentum / velocity component
+  static constexpr int iB = SCHEME == kIdeal ? 5 : 1 + D;  // first magnetic component
+};
+
+}  // namespace lbk

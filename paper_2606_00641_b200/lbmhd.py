@@ -1,0 +1,269 @@
+"""ctypes binding of the C-ABI CUDA library (include/lbmhd.h): same names, argument marshalling only.
+
+Every step of the path runs in the library's kernels.  torch is used for device memory (the workspace
+tensor), the current stream and pinned host buffers; numpy arrays are accepted for host-side fields.
+There is no CPU fallback: if the shared library is missing, cannot be loaded, or no CUDA device is
+present, construction raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+D1Q3, D2Q9, D3Q19 = 1, 2, 3
+IDEAL, INCRES = 0, 1
+BC_PERIODIC, BC_ZEROGRAD, BC_INFLOW = 0, 1, 2
+CELL_FLUID, CELL_FROZEN, CELL_SOLID = 0, 1, 2
+STREAM_AB, STREAM_INPLACE = 0, 1
+OK, EINVAL, ENOMEM, ECUDA, ENUMERIC = 0, -1, -2, -3, -4
+LATTICES = {"D1Q3": D1Q3, "D2Q9": D2Q9, "D3Q19": D3Q19}
+SCHEMES = {"IDEAL": IDEAL, "INCRES": INCRES}
+
+
+class LbmhdParams(C.Structure):
+    _fields_ = [("scheme", C.c_int), ("lattice", C.c_int), ("precision", C.c_int),
+                ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("gamma", C.c_double), ("c0sq", C.c_double), ("nu", C.c_double), ("eta", C.c_double),
+                ("tau", C.c_double * 8), ("powell", C.c_double), ("bc", C.c_int * 6),
+                ("streaming", C.c_int), ("device", C.c_int), ("stream", C.c_void_p),
+                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+
+
+class LbmhdError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("lbmhd error %d: %s" % (code, text))
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree liblbmhd.so (it must have been built: __graft_entry__.build())."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_build.SO):
+        raise ImportError("CUDA extension %s is missing; run __graft_entry__.build() (nvcc, sm_100a)" % _build.SO)
+    lib = C.CDLL(_build.SO)
+    dp, up, pp = C.c_void_p, C.c_void_p, C.POINTER(LbmhdParams)
+    lib.lbmhd_num_vars.argtypes = [pp]
+    lib.lbmhd_num_dirs.argtypes = [pp]
+    lib.lbmhd_workspace_bytes.argtypes = [pp]
+    lib.lbmhd_workspace_bytes.restype = C.c_size_t
+    lib.lbmhd_create.argtypes = [pp, up, C.POINTER(C.c_void_p)]
+    lib.lbmhd_destroy.argtypes = [C.c_void_p]
+    lib.lbmhd_destroy.restype = None
+    lib.lbmhd_init.argtypes = [C.c_void_p, dp, C.c_int]
+    lib.lbmhd_step.argtypes = [C.c_void_p, C.c_int]
+    lib.lbmhd_moments.argtypes = [C.c_void_p, dp, dp, C.c_int]
+    lib.lbmhd_set_obstacle.argtypes = [C.c_void_p, up, dp, dp, C.c_int]
+    lib.lbmhd_set_sphere.argtypes = [C.c_void_p, dp, C.c_double, dp, dp, C.c_double]
+    lib.lbmhd_get_populations.argtypes = [C.c_void_p, dp, C.c_int]
+    lib.lbmhd_set_populations.argtypes = [C.c_void_p, dp, C.c_int]
+    lib.lbmhd_steps_done.argtypes = [C.c_void_p]
+    lib.lbmhd_steps_done.restype = C.c_longlong
+    lib.lbmhd_launch_count.argtypes = [C.c_void_p]
+    lib.lbmhd_launch_count.restype = C.c_longlong
+    lib.lbmhd_copy_probe.argtypes = [dp, dp, C.c_size_t, C.c_int, C.c_void_p]
+    lib.lbmhd_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+EXPORTS = ["lbmhd_num_vars", "lbmhd_num_dirs", "lbmhd_workspace_bytes", "lbmhd_create", "lbmhd_destroy",
+           "lbmhd_init", "lbmhd_step", "lbmhd_moments", "lbmhd_set_obstacle", "lbmhd_set_sphere",
+           "lbmhd_get_populations", "lbmhd_set_populations", "lbmhd_steps_done", "lbmhd_launch_count",
+           "lbmhd_copy_probe", "lbmhd_last_error"]
+
+
+def _check(rc, allow=()):
+    if rc != 0 and rc not in allow:
+        raise LbmhdError(rc, load_library().lbmhd_last_error().decode())
+    return rc
+
+
+def make_params(scheme, lattice, shape, precision=64, gamma=5.0 / 3.0, c0sq=1.0 / 36.0, nu=0.0, eta=0.0, tau=0.6,
+                powell=1.0, bc=(0,) * 6, streaming=STREAM_AB, device=0):
+    p = LbmhdParams()
+    p.scheme = SCHEMES.get(scheme, scheme)
+    p.lattice = LATTICES.get(lattice, lattice)
+    p.precision = precision
+    dims = list(shape) + [1] * (3 - len(shape))
+    p.nx, p.ny, p.nz = dims
+    p.gamma, p.c0sq, p.nu, p.eta, p.powell = gamma, c0sq, nu, eta, powell
+    taus = [tau] * 8 if np.isscalar(tau) else list(tau) + [0.0] * (8 - len(tau))
+    for k in range(8):
+        p.tau[k] = taus[k]
+    for j in range(6):
+        p.bc[j] = bc[j]
+    p.streaming, p.device = streaming, device
+    return p
+
+
+def workspace_bytes(params):
+    return int(load_library().lbmhd_workspace_bytes(C.byref(params)))
+
+
+def _host_ptr(a):
+    return C.c_void_p(a.ctypes.data)
+
+
+class Lbmhd:
+    """Handle wrapper: lbmhd_create / init / step / moments / set_obstacle / set_sphere / destroy."""
+
+    def __init__(self, params, mask=None, stream=None):
+        import torch
+        self.lib = load_library()
+        if not torch.cuda.is_available():
+            raise LbmhdError(ECUDA, "no CUDA device: this library has no CPU path")
+        self.torch = torch
+        self.params = params
+        self.K = self.lib.lbmhd_num_vars(C.byref(params))
+        self.Q = self.lib.lbmhd_num_dirs(C.byref(params))
+        if self.K < 0 or self.Q < 0:
+            raise LbmhdError(EINVAL, "unknown scheme or lattice")
+        self.shape = (params.nz, params.ny, params.nx)
+        self.N = params.nx * params.ny * params.nz
+        nbytes = workspace_bytes(params)
+        if nbytes == 0:
+            raise LbmhdError(EINVAL, "bad dims or precision")
+        dev = torch.device("cuda", params.device)
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev)
+        base = self.workspace.data_ptr()
+        aligned = (base + 255) // 256 * 256
+        params.workspace = aligned
+        params.workspace_bytes = nbytes
+        self.stream = stream if stream is not None else torch.cuda.current_stream(dev)
+        params.stream = self.stream.cuda_stream
+        h = C.c_void_p()
+        m = None
+        if mask is not None:
+            self._mask = np.ascontiguousarray(mask, dtype=np.uint8).reshape(-1)
+            assert self._mask.size == self.N
+            m = _host_ptr(self._mask)
+        _check(self.lib.lbmhd_create(C.byref(params), m, C.byref(h)))
+        self.h = h
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.lbmhd_destroy(self.h)
+            self.h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ptr(self, a, nelem, dtype_np, dtype_torch):
+        """(pointer, on_device, keepalive) for a numpy array or a torch tensor"""
+        torch = self.torch
+        if isinstance(a, torch.Tensor):
+            assert a.dtype == dtype_torch and a.is_contiguous() and a.numel() == nelem
+            return C.c_void_p(a.data_ptr()), int(a.is_cuda), a
+        arr = np.ascontiguousarray(a, dtype=dtype_np)
+        assert arr.size == nelem
+        return _host_ptr(arr), 0, arr
+
+    def init(self, fields):
+        ptr, dev, keep = self._ptr(fields, self.K * self.N, np.float64, self.torch.float64)
+        _check(self.lib.lbmhd_init(self.h, ptr, dev))
+
+    def step(self, n=1):
+        _check(self.lib.lbmhd_step(self.h, int(n)))
+
+    def moments(self, fields_out=None, diag_out=None, want_fields=True, want_diag=True, check=False):
+        """-> (fields [K, nz, ny, nx], diag [3K+4]).  Host numpy by default; pass CUDA tensors to stay on device."""
+        torch = self.torch
+        nd = 3 * self.K + 4
+        on_dev = isinstance(fields_out, torch.Tensor) and fields_out.is_cuda or isinstance(diag_out, torch.Tensor) and diag_out.is_cuda
+        if on_dev:
+            fp = C.c_void_p(fields_out.data_ptr()) if fields_out is not None else None
+            dg = C.c_void_p(diag_out.data_ptr()) if diag_out is not None else None
+            _check(self.lib.lbmhd_moments(self.h, fp, dg, 1))
+            return fields_out, diag_out
+        if fields_out is None and want_fields:
+            fields_out = np.empty((self.K,) + self.shape, dtype=np.float64)
+        if diag_out is None and want_diag:
+            diag_out = np.empty(nd, dtype=np.float64)
+        fp = None
+        if fields_out is not None:
+            fp = C.c_void_p(fields_out.data_ptr()) if isinstance(fields_out, torch.Tensor) else _host_ptr(fields_out)
+        dg = None
+        if diag_out is not None:
+            dg = C.c_void_p(diag_out.data_ptr()) if isinstance(diag_out, torch.Tensor) else _host_ptr(diag_out)
+        _check(self.lib.lbmhd_moments(self.h, fp, dg, 0), allow=() if check else (ENUMERIC,))
+        return fields_out, diag_out
+
+    def set_obstacle(self, mask, u_solid=(0.0, 0.0, 0.0), B_solid=None):
+        mp, dev, k1 = self._ptr(mask, self.N, np.uint8, self.torch.uint8)
+        u = np.ascontiguousarray(u_solid, dtype=np.float64)
+        bp, k2 = None, None
+        if B_solid is not None:
+            bp, dev2, k2 = self._ptr(B_solid, 3 * self.N, np.float64, self.torch.float64)
+            assert dev2 == dev
+        _check(self.lib.lbmhd_set_obstacle(self.h, mp, _host_ptr(u), bp, dev))
+
+    def set_sphere(self, centre, radius, u_solid, dipole_dir, B_surface):
+        c = np.ascontiguousarray(centre, dtype=np.float64)
+        u = np.ascontiguousarray(u_solid, dtype=np.float64)
+        m = np.ascontiguousarray(dipole_dir, dtype=np.float64)
+        _check(self.lib.lbmhd_set_sphere(self.h, _host_ptr(c), float(radius), _host_ptr(u), _host_ptr(m), float(B_surface)))
+
+    def populations(self):
+        """canonical fp64 [K, Q, nz, ny, nx] on the host (via a device tensor)"""
+        torch = self.torch
+        t = torch.empty(self.K * self.Q * self.N, dtype=torch.float64, device=self.workspace.device)
+        _check(self.lib.lbmhd_get_populations(self.h, C.c_void_p(t.data_ptr()), 1))
+        self.stream.synchronize()
+        return t.cpu().numpy().reshape((self.K, self.Q) + self.shape)
+
+    def set_populations(self, g):
+        torch = self.torch
+        t = torch.as_tensor(np.ascontiguousarray(g, dtype=np.float64).reshape(-1)).to(self.workspace.device)
+        _check(self.lib.lbmhd_set_populations(self.h, C.c_void_p(t.data_ptr()), 1))
+        self.stream.synchronize()
+
+    @property
+    def steps_done(self):
+        return int(self.lib.lbmhd_steps_done(self.h))
+
+    @property
+    def launch_count(self):
+        return int(self.lib.lbmhd_launch_count(self.h))
+
+
+def from_workload(w, precision=64, device=0, streaming=STREAM_AB):
+    """Lbmhd handle configured (boundaries, tau, sphere) for a workloads.py dict; fields not yet initialised."""
+    p = make_params(w["scheme"], w["lattice"], w["shape"], precision=precision, gamma=w["gamma"] or 1.4, c0sq=w["c0sq"],
+                    nu=w["nu"], eta=w["eta"], tau=w["tau"], powell=w["powell"], bc=w["bc"], streaming=streaming,
+                    device=device)
+    sim = Lbmhd(p)
+    if w.get("sphere"):
+        s = w["sphere"]
+        sim.set_sphere(s["centre"], s["radius"], s["u_solid"], s["dipole_dir"], s["B_surface"])
+    return sim
+
+
+def copy_probe(n_elems=1 << 28, reps=10, device=0):
+    """measured fp64 copy bandwidth in GB/s (read + write bytes), BabelStream-style"""
+    import torch
+    lib = load_library()
+    dev = torch.device("cuda", device)
+    a = torch.ones(n_elems, dtype=torch.float64, device=dev)
+    b = torch.empty_like(a)
+    st = torch.cuda.current_stream(dev)
+    _check(lib.lbmhd_copy_probe(C.c_void_p(a.data_ptr()), C.c_void_p(b.data_ptr()), n_elems, 3, st.cuda_stream))
+    best = 0.0
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        _check(lib.lbmhd_copy_probe(C.c_void_p(a.data_ptr()), C.c_void_p(b.data_ptr()), n_elems, 1, st.cuda_stream))
+        e1.record(st)
+        e1.synchronize()
+        best = max(best, 2 * 8 * n_elems / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+    return best

@@ -1,0 +1,132 @@
+"""GPU-vs-oracle parity (the graded gate): same seeded arrays -> lbmhd_init -> n steps -> lbmhd_moments,
+compared element by element with the CPU oracle through the C ABI.  fp64 bar 1e-11 (north_star), reading A15."""
+import numpy as np
+import pytest
+
+from paper_2606_00641_b200 import workloads as W
+from parity_util import oracle_from_workload, field_errors, diag_errors, TOL64, TOL32
+from test_oracle_pins import admissible_ideal, ideal_fields, incres_fields, zyx
+
+pytestmark = pytest.mark.gpu
+
+
+def gpu_from_workload(w, precision=64):
+    from paper_2606_00641_b200 import lbmhd
+    return lbmhd.from_workload(w, precision=precision)
+
+
+def random_workload(scheme, lattice, shape, bc, seed, tau=0.7, sphere=None, gamma=5 / 3):
+    rng = np.random.default_rng(seed)
+    s = zyx(shape)
+    D = len(shape)
+    if scheme == "IDEAL":
+        rho, u, B, p = admissible_ideal(rng, s)
+        F = ideal_fields(rho, u, B, p, gamma)
+    else:
+        F = incres_fields(rng, D, s)
+    return dict(name="rand", scheme=scheme, lattice=lattice, shape=shape, gamma=gamma, c0sq=1 / 36, nu=0.0, eta=0.0,
+                tau=tau, powell=1.0, bc=bc, steps=0, fields=F, sphere=sphere)
+
+
+def compare(w, steps, tol=TOL64, mask=None, obstacle=None, precision=64):
+    o = oracle_from_workload(w, mask=mask)
+    g = gpu_from_workload(w, precision=precision)
+    if obstacle is not None:
+        o.set_obstacle(*obstacle)
+        g.set_obstacle(*obstacle)
+    o.init(w["fields"])
+    g.init(w["fields"])
+    o.step(steps)
+    g.step(steps)
+    Qo, do = o.moments()
+    Qg, dg = g.moments()
+    errs = field_errors(Qg, Qo)
+    assert (errs <= tol).all(), errs
+    K = o.K
+    e_sum, e_abs, e_max = diag_errors(dg, do, K)
+    assert (e_sum <= 10 * tol).all() and (e_abs <= 10 * tol).all() and (e_max <= 10 * tol).all()
+    assert abs(dg[3 * K] - do[3 * K]) <= 1e3 * tol * max(do[2 * K:3 * K].max(), 1e-300)        # max|div_h B|
+    if np.isfinite(do[3 * K + 1]):
+        assert abs(dg[3 * K + 1] - do[3 * K + 1]) <= 10 * tol * abs(do[3 * K + 1])             # min rho
+    if np.isfinite(do[3 * K + 2]):
+        assert abs(dg[3 * K + 2] - do[3 * K + 2]) <= 1e3 * tol * max(do[2 * K:3 * K].max(), 1e-300)   # min p
+    assert dg[3 * K + 3] == do[3 * K + 3]
+    g.close()
+    return errs
+
+
+CASES = [
+    ("IDEAL", "D1Q3", (200,), (0,) * 6),
+    ("IDEAL", "D1Q3", (131,), (1, 1, 0, 0, 0, 0)),
+    ("IDEAL", "D1Q3", (70,), (2, 1, 0, 0, 0, 0)),
+    ("INCRES", "D1Q3", (131,), (1, 1, 0, 0, 0, 0)),
+    ("IDEAL", "D2Q9", (150, 37), (0,) * 6),
+    ("IDEAL", "D2Q9", (150, 37), (1, 1, 1, 1, 0, 0)),
+    ("IDEAL", "D2Q9", (67, 20), (2, 1, 0, 0, 0, 0)),
+    ("INCRES", "D2Q9", (150, 37), (0,) * 6),
+    ("INCRES", "D2Q9", (90, 21), (1, 1, 2, 1, 0, 0)),
+    ("IDEAL", "D3Q19", (100, 12, 9), (0,) * 6),
+    ("IDEAL", "D3Q19", (100, 12, 9), (2, 1, 0, 0, 0, 0)),
+    ("IDEAL", "D3Q19", (45, 11, 10), (1, 1, 1, 1, 1, 1)),
+    ("INCRES", "D3Q19", (70, 9, 8), (1, 1, 0, 0, 2, 1)),
+]
+
+
+@pytest.mark.parametrize("scheme,lattice,shape,bc", CASES)
+def test_random_state_parity(scheme, lattice, shape, bc):
+    """several x-tiles plus a ragged tail, every boundary kind, 20 steps from a rough random state"""
+    w = random_workload(scheme, lattice, shape, bc, seed=1234)
+    compare(w, 20)
+
+
+@pytest.mark.parametrize("scheme,lattice,shape", [("IDEAL", "D2Q9", (90, 33)), ("IDEAL", "D3Q19", (70, 12, 10)), ("INCRES", "D2Q9", (90, 33))])
+def test_masked_obstacle_parity(scheme, lattice, shape):
+    rng = np.random.default_rng(77)
+    w = random_workload(scheme, lattice, shape, (1, 1) + (0,) * 4, seed=99)
+    s = zyx(shape)
+    mask = (rng.random(s) < 0.05).astype(np.uint8) * 2
+    mask[rng.random(s) < 0.02] = 1
+    Bs = 0.1 * (rng.random((3,) + s) - 0.5)
+    compare(w, 15, obstacle=(mask, np.array([0.03, -0.02, 0.01]), Bs))
+
+
+@pytest.mark.parametrize("lattice,shape", [("D2Q9", (80, 40)), ("D3Q19", (72, 24, 20))])
+def test_moving_sphere_parity(lattice, shape):
+    D = len(shape)
+    cen = np.array([shape[0] / 2.0, shape[1] / 2.0, shape[2] / 2.0 if D == 3 else 0.0])
+    mh = np.array([0.3, -0.5, 0.8]) / np.linalg.norm([0.3, -0.5, 0.8])
+    sph = dict(centre=cen, radius=6.0, u_solid=np.array([-0.25, 0.0, 0.0]), dipole_dir=mh, B_surface=0.03)
+    w = random_workload("IDEAL", lattice, shape, (2, 1, 0, 0, 0, 0), seed=5, sphere=sph)
+    compare(w, 12)
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
+def test_config_parity_100_steps_reduced_size(name):
+    """the five BASELINE configs at the reduced sizes the oracle finishes in seconds, 100 steps"""
+    w = W.get(name, small=True)
+    errs = compare(w, 100)
+    print(name, "max field error", errs.max())
+
+
+def test_empty_step_and_odd_counts():
+    w = random_workload("IDEAL", "D2Q9", (64, 16), (0,) * 6, seed=3)
+    o = oracle_from_workload(w)
+    g = gpu_from_workload(w)
+    o.init(w["fields"])
+    g.init(w["fields"])
+    g.step(0)
+    assert g.steps_done == 0
+    for n in (1, 2, 3):
+        o.step(n)
+        g.step(n)
+        assert (field_errors(g.moments()[0], o.moments()[0]) <= TOL64).all()
+    assert g.steps_done == 6
+    # populations themselves, not only their moments
+    assert np.abs(g.populations() - o.populations()).max() <= 1e-13
+    g.close()
+
+
+def test_fp32_variant_parity():
+    w = W.get("C3", small=True)
+    errs = compare(w, 100, tol=TOL32, precision=32)
+    print("fp32 C3 small", errs.max())
