@@ -1,0 +1,246 @@
+#!/usr/bin/env python
+"""bench.py — MLUPS and achieved HBM GB/s of the fused VLBM MHD step (BASELINE.json metric).
+
+  python bench.py --gpus N --steps K --warmup W [--impl reference] [--workload C5]
+
+One "step" = one pass of the whole hot path (one lbmhd_step launch) over the resident workload.
+N = 1 runs BASELINE config 5 (3D ideal MHD, D3Q19 x 8 sets, fp64, 384x256x256, moving magnetised sphere):
+the configuration the north_star target is quoted on.  N > 1 (torchrun): every rank runs the same
+workload on its own GPU with no data-path collective ("scaling": "weak").
+Prints ONE JSON line on rank 0.  --impl reference times the CPU oracle (oracle/) on the host cores.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "MLUPS (fused VLBM MHD stream-collide step)"
+SAMPLE_SHAPE = (96, 64, 64)      # bounded sample of the same workload for the CPU oracle legs
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy_)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler(threading.Thread):
+    """samples SM clock and throttle reasons of one GPU during the timed region (NVML)"""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.sm, self.reasons, self.sm_max = index, False, [], set(), None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap", nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self.stop_flag:
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.05)
+
+    def result(self):
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.sm_max,
+                "reasons": sorted(self.reasons)}
+
+
+def oracle_leg(workload_name, steps, warmup, budget_s=None):
+    """the CPU oracle, as it stands, on a bounded sample of the workload; -> (MLUPS, cores, sample text, ms/step)"""
+    from oracle import oracle as orc
+    from paper_2606_00641_b200 import workloads as W
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from parity_util import oracle_from_workload
+    w = W.config5(shape=SAMPLE_SHAPE) if workload_name == "C5" else W.get(workload_name, small=True)
+    o = oracle_from_workload(w)
+    o.init(w["fields"])
+    o.step(max(warmup, 1))
+    N = int(np.prod(w["shape"]))
+    t0 = time.perf_counter()
+    done = 0
+    while done < steps:
+        o.step(1)
+        done += 1
+        if budget_s is not None and done >= 3 and time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    sample = "%s at %s (same recipe, reduced size), %d steps after %d warm-up" % (
+        workload_name, "x".join(str(s) for s in w["shape"]), done, max(warmup, 1))
+    return N * done / dt / 1e6, orc.get_threads(), sample, dt / done * 1e3, w
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    mlups, cores, sample, ms, w = oracle_leg(args.workload, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": mlups, "unit": "MLUPS", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "%s (CPU oracle on a bounded sample)" % args.workload, "sample": sample},
+            "cpu_baseline": {"value": mlups, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": mlups, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_native(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_00641_b200 import lbmhd, workloads as W
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device and no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    w = W.get(args.workload)
+    N = int(np.prod(w["shape"]))
+    prec = args.precision
+    sim = lbmhd.from_workload(w, precision=prec, device=local_rank)
+    K, Q = sim.K, sim.Q
+    bytes_per_cell = 2 * K * Q * (8 if prec == 64 else 4) + (0 if w.get("sphere") else 0)
+    st = sim.stream
+
+    # ---- device-resident timing: inputs already in HBM -------------------------------------------------
+    F_dev = torch.as_tensor(w["fields"]).to(dev)
+    sim.init(F_dev)
+    sim.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    l0 = sim.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(st)
+    sim.step(args.steps)
+    e1.record(st)
+    barrier()
+    launches = sim.launch_count - l0
+    sampler.stop_flag = True
+    sampler.join()
+    ms_total = e0.elapsed_time(e1)
+    _, dg = sim.moments(want_fields=False)
+    if dg[-1] != 0:
+        raise SystemExit("bench.py: numerical failure flag %g after the timed run" % dg[-1])
+
+    # ---- end to end through the C ABI with HOST buffers: init (H2D) + K steps + moments (D2H) ----------
+    F_host = torch.as_tensor(w["fields"]).pin_memory()
+    out_host = torch.empty_like(F_host).pin_memory()
+    diag_host = torch.empty(3 * K + 4, dtype=torch.float64).pin_memory()
+    del F_dev
+    sim.init(F_host)               # warm the path once
+    sim.moments(out_host, diag_host)
+    barrier()
+    t0 = torch.cuda.Event(enable_timing=True)
+    t1 = torch.cuda.Event(enable_timing=True)
+    t0.record(st)
+    sim.init(F_host)
+    sim.step(args.steps)
+    sim.moments(out_host, diag_host)
+    t1.record(st)
+    barrier()
+    ms_e2e = t0.elapsed_time(t1)
+    h2d = F_host.numel() * 8
+    d2h = out_host.numel() * 8 + diag_host.numel() * 8
+
+    times = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    ms_total, ms_e2e = [float(v) for v in times.cpu()]
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = load_peaks()
+    ms_step = ms_total / args.steps
+    value = world * N * args.steps / (ms_total * 1e-3) / 1e6
+    achieved = N * bytes_per_cell / (ms_step * 1e-3) / 1e9
+    e2e_val = world * N * args.steps / (ms_e2e * 1e-3) / 1e6
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic_%s.json" % args.workload)
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get("dram_bytes_per_launch")
+    line = {
+        "metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64" if prec == 64 else "f32", "data": "synthetic",
+        "config": {"workload": "%s: %s %s x %d sets, %s, %s, %d B/cell/step; replicas per GPU, no collective" % (
+                       w["name"], w["scheme"], w["lattice"], K, "x".join(str(s) for s in w["shape"]),
+                       "fp64" if prec == 64 else "fp32", bytes_per_cell),
+                   "cells": N, "streaming": "A/B double buffer",
+                   "l2": "working set %.1f GB >> 126 MB L2, no flush needed" % (2 * N * bytes_per_cell / 2 / 1e9)},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": traffic, "peak_source": peak_src, "kernel": "step_kernel",
+                     "frac_of_nominal_8TBs": achieved / 8000.0,
+                     "paper_context": "98.9% (2D) / 75.8% (3D) of 680 GB/s BabelStream, RTX A5000 fp32 (PAPER.md:269)"},
+        "e2e": {"value": e2e_val, "unit": "MLUPS", "h2d_bytes_per_step": h2d / args.steps,
+                "d2h_bytes_per_step": d2h / args.steps,
+                "what": "lbmhd_init(pinned host fields) + %d x lbmhd_step + lbmhd_moments(pinned host out)" % args.steps},
+        "gpu_launches": int(launches), "clocks": sampler.result(),
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        mlups, cores, sample, _, _ = oracle_leg(args.workload, 10 ** 9, 1, budget_s=args.cpu_seconds)
+        line["cpu_baseline"] = {"value": mlups, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": sample}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="native", choices=["native", "reference"])
+    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "native" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_native(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -102,7 +102,7 @@ struct lbmhd {
   bool has_sphere;
   double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs;
   long long sph_t0;
-  int tx;                // x-tile of the step kernel
+  int tx, minb;          // x-tile and min blocks/SM (launch bound) of the step kernel
 };
 
 extern "C" {
@@ -176,11 +176,9 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
   }
   h->ws = (char *)p->workspace;
   h->stream = (cudaStream_t)p->stream;
-  h->tx = 64;
-  if (const char *e = getenv("LBMHD_TX")) {
-    const int v = atoi(e);
-    if (v == 32 || v == 64 || v == 128) h->tx = v;
-  }
+  h->tx = 32; h->minb = 3;
+  if (const char *e = getenv("LBMHD_TX")) h->tx = atoi(e);        // tuning knobs; unknown pairs fall back to 32/2
+  if (const char *e = getenv("LBMHD_MINB")) h->minb = atoi(e);
   cudaError_t e = cudaSetDevice(p->device);
   if (e != cudaSuccess) { delete h; return fail(LBMHD_ECUDA, "cudaSetDevice(%d): %s", p->device, cudaGetErrorString(e)); }
   h->have_mask = cell_mask != nullptr;
@@ -202,15 +200,15 @@ namespace {
 
 template <int LAT, int SCHEME, typename real> struct Ops {
   using L = Lattice<LAT>;
-  static constexpr int D = L::D, Q = L::Q, K = Vars<SCHEME, L::D>::K;
+  static constexpr int Q = L::Q, K = Vars<SCHEME, L::D>::K;
   static constexpr int TXAUX = 64;   // x-tile of init / moments
 
   static real *pops(lbmhd_t *h, int which) { return (real *)(h->ws + h->L.off_pop[which]); }
 
   static dim3 grid(const lbmhd_t *h, int tx) { return dim3((h->p.nx + tx - 1) / tx, h->p.ny, h->p.nz); }
 
-  template <int TX> static cudaError_t launch_step(lbmhd_t *h, const StepArgs<real> &a) {
-    step_kernel<LAT, SCHEME, real, TX><<<grid(h, TX), dim3(TX, K), 0, h->stream>>>(a);
+  template <int TX, int MINB> static cudaError_t launch_step(lbmhd_t *h, const StepArgs<real> &a) {
+    step_kernel<LAT, SCHEME, real, TX, MINB><<<grid(h, TX), dim3(TX, K), 0, h->stream>>>(a);
     return cudaGetLastError();
   }
 
@@ -245,10 +243,15 @@ template <int LAT, int SCHEME, typename real> struct Ops {
         }
       }
       cudaError_t e;
-      switch (h->tx) {
-        case 32: e = launch_step<32>(h, a); break;
-        case 128: e = launch_step<128>(h, a); break;
-        default: e = launch_step<64>(h, a); break;
+      switch (h->tx * 10 + h->minb) {
+        case 321: e = launch_step<32, 1>(h, a); break;
+        case 322: e = launch_step<32, 2>(h, a); break;
+        case 323: e = launch_step<32, 3>(h, a); break;
+        case 324: e = launch_step<32, 4>(h, a); break;
+        case 641: e = launch_step<64, 1>(h, a); break;
+        case 642: e = launch_step<64, 2>(h, a); break;
+        case 1281: e = launch_step<128, 1>(h, a); break;
+        default: e = launch_step<32, 3>(h, a); break;
       }
       if (e != cudaSuccess) return fail(LBMHD_ECUDA, "step kernel launch: %s", cudaGetErrorString(e));
       h->cur = 1 - h->cur;

@@ -217,8 +217,8 @@ __device__ __forceinline__ void solid_blend(const real *Qv, real gamma, const do
 // Fused step kernel, A/B buffers: pull-stream + moments + div-B estimate + Powell source + solid blend +
 // flux + BGK + direct injection + store (DESIGN.md §2 steps S1-S8; Eq.2-4, 8, 11-14).
 // =====================================================================================================
-template <int LAT, int SCHEME, typename real, int TX>
-__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K)
+template <int LAT, int SCHEME, typename real, int TX, int MINB>
+__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
 step_kernel(const StepArgs<real> a) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
@@ -333,24 +333,23 @@ step_kernel(const StepArgs<real> a) {
   for (int b = 0; b < D; b++) tr += sTr[b][tx];
   const real delta = -tr * a.inv_tauB_cs2;                      // A6
 
-  // S4 Powell source, S5 solid blend
-  real S = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
-  real Qh[K];
-#pragma unroll
-  for (int l = 0; l < K; l++) Qh[l] = Qv[l];
-  real dQh = real(0);
+  // S4 Powell source, S5 solid blend (rare: own branch so the blended copy of the state costs no registers
+  // on the fluid path), S6 flux row of this variable
+  real Phi[3];
+  real inj;
   double uS[3], BS[3];
   if (solid_state<real, D>(a, x, y, z, n, uS, BS)) {
+    real Qh[K];
     solid_blend<SCHEME, D, real>(Qv, a.gamma, uS, BS, Qh);
-    dQh = pick<K, real>(Qh, k) - Qk;
-    S = real(0);
+    flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, Phi);
+    inj = pick<K, real>(Qh, k) - Qk;                            // dQh; the Powell source is scaled by d = 0
+  } else {
+    flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, Phi);
+    inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
   }
 
-  // S6 flux row of this variable, S7 BGK + direct injection, S8 store
-  real Phi[3];
-  flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, Phi);
+  // S7 BGK + direct injection, S8 store
   const real om = a.omega[k];
-  const real inj = dQh + S;
 #pragma unroll
   for (int i = 0; i < Q; i++) {
     const real cPhi = real(L::cx(i)) * Phi[0] + real(L::cy(i)) * Phi[1] + real(L::cz(i)) * Phi[2];
