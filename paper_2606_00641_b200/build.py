@@ -6,6 +6,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SO = os.path.join(_HERE, "liblbmhd.so")
 SRC = os.path.join(_HERE, "csrc", "lbmhd_api.cu")
 DEPS = [SRC, os.path.join(_HERE, "csrc", "lbmhd_kernels.cuh"), os.path.join(_HERE, "csrc", "lbmhd_lattice.cuh"),
+        os.path.join(_HERE, "csrc", "lbmhd_tma.cuh"),
         os.path.join(os.path.dirname(_HERE), "include", "lbmhd.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]

@@ -13,6 +13,7 @@
 #include <string>
 
 #include "lbmhd_kernels.cuh"
+#include "lbmhd_tma.cuh"
 
 using namespace lbk;
 
@@ -102,8 +103,44 @@ struct lbmhd {
   bool has_sphere;
   double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs;
   long long sph_t0;
-  int tx, minb;          // x-tile and min blocks/SM (launch bound) of the step kernel
+  int tx, minb;          // x-tile and min blocks/SM (launch bound) of the plain step kernel
+  bool use_tma;          // TMA-staged persistent step kernel (needs nx * sizeof(real) % 16 == 0)
+  int num_sms;
+  CUtensorMap tmap[2][2];   // [copy][0: tile-wide box, 1: box 16 bytes wider] 5D views (x, y, z, i, k) of the populations
 };
+
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+constexpr int kTmaTX = 32, kTmaStages = 5;
+
+// 5D view of one population copy: x, y, z, direction i, variable k; box = [K][1][1][1][kTmaTX]
+int make_tensor_maps(lbmhd *h) {
+  void *fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+  if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn)
+    return fail(LBMHD_ECUDA, "cuTensorMapEncodeTiled is not available from the driver");
+  const size_t es = h->p.precision == 64 ? 8 : 4;
+  const cuuint64_t dims[5] = {(cuuint64_t)h->p.nx, (cuuint64_t)h->p.ny, (cuuint64_t)h->p.nz, (cuuint64_t)h->g.Q, (cuuint64_t)h->g.K};
+  const cuuint64_t strides[4] = {(cuuint64_t)h->p.nx * es, (cuuint64_t)h->p.nx * h->p.ny * es, (cuuint64_t)h->L.pstride * es,
+                                 (cuuint64_t)h->L.pstride * h->g.Q * es};
+  const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  for (int b = 0; b < 4; b++) {
+    const cuuint32_t box[5] = {(cuuint32_t)(kTmaTX + (b & 1) * (16 / es)), 1, 1, 1, (cuuint32_t)h->g.K};
+    CUresult r = ((EncodeTiledFn)fn)(&h->tmap[b >> 1][b & 1], es == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5,
+                                     h->ws + h->L.off_pop[b >> 1], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(LBMHD_ECUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+  }
+  return LBMHD_OK;
+}
+
+}  // namespace
 
 extern "C" {
 
@@ -145,6 +182,8 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
   if (g.D < 2 && p->ny != 1) return fail(LBMHD_EINVAL, "ny must be 1 on a 1D lattice");
   if (g.D < 3 && p->nz != 1) return fail(LBMHD_EINVAL, "nz must be 1 on a 1D/2D lattice");
   if ((size_t)p->ny > 65535 || (size_t)p->nz > 65535) return fail(LBMHD_EINVAL, "ny, nz must be <= 65535");
+  if ((unsigned long long)g.Q * L.pstride >= (1ull << 32))
+    return fail(LBMHD_EINVAL, "grid too large: Q * cells must stay below 2^32 (32-bit plane offsets in the kernels)");
   const int nn[3] = {p->nx, p->ny, p->nz};
   for (int a = 0; a < g.D; a++) {
     const int lo = p->bc[2 * a], hi = p->bc[2 * a + 1];
@@ -181,6 +220,20 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
   if (const char *e = getenv("LBMHD_MINB")) h->minb = atoi(e);
   cudaError_t e = cudaSetDevice(p->device);
   if (e != cudaSuccess) { delete h; return fail(LBMHD_ECUDA, "cudaSetDevice(%d): %s", p->device, cudaGetErrorString(e)); }
+  {
+    int sms = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
+    if (e != cudaSuccess) { delete h; return fail(LBMHD_ECUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e)); }
+    h->num_sms = sms;
+    const char *path = getenv("LBMHD_PATH");      // tuning knob: "plain" forces the register-pull kernel
+    const size_t es = p->precision == 64 ? 8 : 4;
+    const long long tiles = (long long)((p->nx + kTmaTX - 1) / kTmaTX) * p->ny * p->nz;
+    h->use_tma = !(path && strcmp(path, "plain") == 0) && ((size_t)p->nx * es) % 16 == 0 && tiles < 2000000000LL;
+    if (h->use_tma) {
+      const int rc = make_tensor_maps(h);
+      if (rc) { delete h; return rc; }
+    }
+  }
   h->have_mask = cell_mask != nullptr;
   if (cell_mask) {
     e = cudaMemcpyAsync(h->ws + L.off_mask, cell_mask, h->N, cudaMemcpyHostToDevice, h->stream);
@@ -212,6 +265,22 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     return cudaGetLastError();
   }
 
+  static cudaError_t launch_step_tma(lbmhd_t *h, const StepArgs<real> &a) {
+    using C = TmaCfg<LAT, SCHEME, real, kTmaTX, kTmaStages>;
+    auto kern = step_kernel_tma<LAT, SCHEME, real, kTmaTX, kTmaStages>;
+    static bool attr_set = false;
+    if (!attr_set) {
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
+      if (e != cudaSuccess) return e;
+      attr_set = true;
+    }
+    const int tiles_x = (h->p.nx + kTmaTX - 1) / kTmaTX;
+    const long long n_rows = (long long)h->p.ny * h->p.nz;                 // < 2^31 - SMs checked at create
+    const int grid = (int)(n_rows < (long long)h->num_sms ? n_rows : (long long)h->num_sms);
+    kern<<<grid, C::THREADS, C::SMEM_BYTES, h->stream>>>(a, h->tmap[h->cur][0], h->tmap[h->cur][1], tiles_x, (int)n_rows);
+    return cudaGetLastError();
+  }
+
   static int step(lbmhd_t *h, int n_steps) {
     StepArgs<real> a;
     memset(&a, 0, sizeof a);
@@ -224,7 +293,16 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     a.mask = h->have_mask ? (const unsigned char *)(h->ws + h->L.off_mask) : nullptr;
     a.Bsolid = h->have_bsolid ? (const double *)(h->ws + h->L.off_bsolid) : nullptr;
     for (int c = 0; c < 3; c++) a.usolid[c] = h->usolid[c];
+    {
+      const long long es = (long long)sizeof(real);
+      for (int i = 0; i < Q; i++) {
+        const long long shift = lat_c<L>(i, 0) + (long long)lat_c<L>(i, 1) * h->p.nx + (long long)lat_c<L>(i, 2) * h->p.nx * h->p.ny;
+        a.ld_off[i] = ((long long)i * (long long)h->L.pstride - shift) * es;
+        a.st_off[i] = (long long)i * (long long)h->L.pstride * es;
+      }
+    }
     a.has_sphere = h->has_sphere ? 1 : 0;
+    if (const char *e = getenv("LBMHD_DBG")) a.dbg = atoi(e);
     if (h->has_sphere) {
       a.sph_R = h->sph_R;
       a.sph_R2 = h->sph_R * h->sph_R;
@@ -243,7 +321,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
         }
       }
       cudaError_t e;
-      switch (h->tx * 10 + h->minb) {
+      if (h->use_tma) e = launch_step_tma(h, a);
+      else switch (h->tx * 10 + h->minb) {
         case 321: e = launch_step<32, 1>(h, a); break;
         case 322: e = launch_step<32, 2>(h, a); break;
         case 323: e = launch_step<32, 3>(h, a); break;

@@ -34,6 +34,10 @@ template <typename real> struct StepArgs {
   const unsigned char *mask;    // [N] or nullptr
   const double *Bsolid;         // [3][N] or nullptr
   double usolid[3];
+  long long ld_off[19];         // bytes from a cell's own slot in plane (k,0) to its pull source in plane (k,i), no wrap:
+                                //   (i*pstride - (c_x + c_y nx + c_z nx ny)) * sizeof(real)
+  long long st_off[19];         // i * pstride * sizeof(real)
+  int dbg;                      // experiments only (LBMHD_DBG): 1 = TMA kernel skips the math and the stores
   int has_sphere;
   double sph_c[3], sph_R, sph_R2, sph_m[3], sph_Bs, sph_u[3];
 };
@@ -213,82 +217,58 @@ __device__ __forceinline__ void solid_blend(const real *Qv, real gamma, const do
   }
 }
 
+// per-cell context shared by the load front ends (plain pulls / TMA-staged pulls) and finish_cell
+struct CellCtx {
+  int tx, k, x, y, z;
+  uint32_t n;                                   // cell index (N < 2^32 is checked at create)
+  bool work;                                    // active and not frozen
+  bool out_xm, out_xp, out_ym, out_yp, out_zm, out_zp;   // source x - c would be outside a non-periodic face
+};
+
+// Conservative, tile-uniform test: can the sphere touch cells [x0, x0+tx_cells) of row (y, z)?
+template <typename real, int D>
+__device__ __forceinline__ bool sphere_may_touch(const StepArgs<real> &a, int x0, int tx_cells, int y, int z) {
+  if (!a.has_sphere) return false;
+  const double lo = (double)x0 - a.sph_c[0], hi = a.sph_c[0] - (double)(x0 + tx_cells - 1);
+  const double dx = fmax(0.0, fmax(lo, hi));
+  const double dy = D > 1 ? (double)y - a.sph_c[1] : 0.0;
+  const double dz = D > 2 ? (double)z - a.sph_c[2] : 0.0;
+  return dx * dx + dy * dy + dz * dz <= a.sph_R2 * (1.0 + 1e-9) + 1e-9;
+}
+
 // =====================================================================================================
-// Fused step kernel, A/B buffers: pull-stream + moments + div-B estimate + Powell source + solid blend +
-// flux + BGK + direct injection + store (DESIGN.md §2 steps S1-S8; Eq.2-4, 8, 11-14).
+// Everything after the pull: boundary substitution (A9), moments exchange, div-B estimate, Powell source,
+// solid blend, flux, BGK + direct injection, store (DESIGN.md §2 steps S2-S8; Eq.2-4, 8, 11-14).
+// sQ[K][TX], sTr[D][TX] are shared arrays of the TX*K threads that call this together; `sync` is their
+// barrier (__syncthreads or a named barrier).  BND / SOLID are tile-uniform: the interior fluid tile (both
+// false) is the hot path and carries no boundary predicates, no mask or sphere test.
 // =====================================================================================================
-template <int LAT, int SCHEME, typename real, int TX, int MINB>
-__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
-step_kernel(const StepArgs<real> a) {
+template <int LAT, int SCHEME, typename real, int TX, bool BND, bool SOLID, class Sync>
+__device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellCtx &c, real (&f)[Lattice<LAT>::Q],
+                                            real (*sQ)[TX], real (*sTr)[TX], Sync sync) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
   using V = Vars<SCHEME, D>;
   constexpr int K = V::K, iB = V::iB;
-  __shared__ real sQ[K][TX];
-  __shared__ real sTr[D][TX];
+  const int tx = c.tx, k = c.k;
+  const uint32_t ps = (uint32_t)a.pstride;
+  const bool work = c.work;
+  const real *__restrict__ srck = a.src + (size_t)k * Q * a.pstride;
 
-  const int tx = threadIdx.x, k = threadIdx.y;
-  const int x = blockIdx.x * TX + tx, y = blockIdx.y, z = blockIdx.z;
-  const int nx = a.nx, ny = a.ny, nz = a.nz;
-  const bool active = x < nx;
-  const size_t n = ((size_t)z * ny + y) * nx + (active ? x : 0);
-  const size_t ps = a.pstride;
-  const real *__restrict__ srck = a.src + (size_t)k * Q * ps;
-  real *__restrict__ dstk = a.dst + (size_t)k * Q * ps;
-
-  const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
-  const bool x_lo = x == 0, x_hi = x == nx - 1;
-  const bool y_lo = D > 1 && y == 0, y_hi = D > 1 && y == ny - 1;
-  const bool z_lo = D > 2 && z == 0, z_hi = D > 2 && z == nz - 1;
-
-  // frozen cells keep their populations: mask FROZEN or on an INFLOW face (A10)
-  bool frozen = false;
-  if (active) {
-    frozen = (a.mask != nullptr && a.mask[n] == CELL_FROZEN) || (x_lo && a.bc[0] == BC_INFLOW) ||
-             (x_hi && a.bc[1] == BC_INFLOW) || (y_lo && a.bc[2] == BC_INFLOW) || (y_hi && a.bc[3] == BC_INFLOW) ||
-             (z_lo && a.bc[4] == BC_INFLOW) || (z_hi && a.bc[5] == BC_INFLOW);
-    if (frozen) {
-#pragma unroll
-      for (int i = 0; i < Q; i++) dstk[(size_t)i * ps + n] = srck[(size_t)i * ps + n];
-    }
-  }
-  const bool work = active && !frozen;
-
-  // S1 pull: f_i(x) = g_i(x - c_i), periodic wrap; sources outside a non-periodic face are filled below
-  const int xm = x_lo ? nx - 1 : x - 1, xp = x_hi ? 0 : x + 1;
-  const int ym = y_lo ? ny - 1 : y - 1, yp = y_hi ? 0 : y + 1;
-  const int zm = z_lo ? nz - 1 : z - 1, zp = z_hi ? 0 : z + 1;
-  const bool out_xm = npx && x_lo, out_xp = npx && x_hi;
-  const bool out_ym = npy && y_lo, out_yp = npy && y_hi;
-  const bool out_zm = npz && z_lo, out_zp = npz && z_hi;
-
-  real f[Q];
-#pragma unroll
-  for (int i = 0; i < Q; i++) {
-    const int cx = L::cx(i), cy = L::cy(i), cz = L::cz(i);
-    const int sx = cx == 1 ? xm : (cx == -1 ? xp : x);
-    const int sy = cy == 1 ? ym : (cy == -1 ? yp : y);
-    const int sz = cz == 1 ? zm : (cz == -1 ? zp : z);
-    const bool outside = (cx == 1 && out_xm) || (cx == -1 && out_xp) || (cy == 1 && out_ym) || (cy == -1 && out_yp) ||
-                         (cz == 1 && out_zm) || (cz == -1 && out_zp);
-    f[i] = (work && !outside) ? srck[(size_t)i * ps + ((size_t)sz * ny + sy) * nx + sx] : real(0);
-  }
-
-  // A9 / PAPER.md:154: directions whose source is outside take the equilibrium of the inward neighbour's state
-  const bool block_bnd = out_ym || out_yp || out_zm || out_zp || (npx && (blockIdx.x == 0 || blockIdx.x == gridDim.x - 1));
-  if (block_bnd) {
-    const bool cell_bnd = work && (out_xm || out_xp || out_ym || out_yp || out_zm || out_zp);
+  if (BND) {
+    // A9 / PAPER.md:154: directions whose source is outside take the equilibrium of the inward neighbour's state
+    const bool cell_bnd = work && (c.out_xm || c.out_xp || c.out_ym || c.out_yp || c.out_zm || c.out_zp);
     if (cell_bnd) {
-      const int qx = out_xm ? x + 1 : (out_xp ? x - 1 : x);
-      const int qy = out_ym ? y + 1 : (out_yp ? y - 1 : y);
-      const int qz = out_zm ? z + 1 : (out_zp ? z - 1 : z);
-      const size_t nb = ((size_t)qz * ny + qy) * nx + qx;
+      const int qx = c.out_xm ? c.x + 1 : (c.out_xp ? c.x - 1 : c.x);
+      const int qy = c.out_ym ? c.y + 1 : (c.out_yp ? c.y - 1 : c.y);
+      const int qz = c.out_zm ? c.z + 1 : (c.out_zp ? c.z - 1 : c.z);
+      const uint32_t nb = ((uint32_t)qz * a.ny + qy) * a.nx + qx;
       real s = real(0);
 #pragma unroll
-      for (int j = 0; j < Q; j++) s += srck[(size_t)j * ps + nb];
+      for (int j = 0; j < Q; j++) s += srck[(uint32_t)j * ps + nb];
       sQ[k][tx] = s;
     }
-    __syncthreads();
+    sync();
     if (cell_bnd) {
       real Qnb[K], Phi[3];
 #pragma unroll
@@ -298,13 +278,13 @@ step_kernel(const StepArgs<real> a) {
 #pragma unroll
       for (int i = 0; i < Q; i++) {
         const int cx = L::cx(i), cy = L::cy(i), cz = L::cz(i);
-        const bool outside = (cx == 1 && out_xm) || (cx == -1 && out_xp) || (cy == 1 && out_ym) ||
-                             (cy == -1 && out_yp) || (cz == 1 && out_zm) || (cz == -1 && out_zp);
+        const bool outside = (cx == 1 && c.out_xm) || (cx == -1 && c.out_xp) || (cy == 1 && c.out_ym) ||
+                             (cy == -1 && c.out_yp) || (cz == 1 && c.out_zm) || (cz == -1 && c.out_zp);
         const real cPhi = real(cx) * Phi[0] + real(cy) * Phi[1] + real(cz) * Phi[2];
         if (outside) f[i] = real(L::w(i)) * (Qnbk + real(3) * cPhi);
       }
     }
-    __syncthreads();
+    sync();
   }
 
   // S2 zeroth moment of this set (index order) and S3 this set's share of tr Pi_B
@@ -313,16 +293,24 @@ step_kernel(const StepArgs<real> a) {
   for (int i = 0; i < Q; i++) Qk += f[i];
   sQ[k][tx] = Qk;
   if (k >= iB && k < iB + D) {
-    const int b = k - iB;
+    const int b = k - iB;   // warp-uniform
     real t = real(0);
+    if (b == 0) {
 #pragma unroll
-    for (int i = 0; i < Q; i++) {
-      const int cb = b == 0 ? L::cx(i) : (b == 1 ? L::cy(i) : L::cz(i));   // b is warp-uniform
-      t += real(cb) * f[i];
+      for (int i = 0; i < Q; i++)
+        if (L::cx(i) != 0) t += real(L::cx(i)) * f[i];
+    } else if (b == 1) {
+#pragma unroll
+      for (int i = 0; i < Q; i++)
+        if (L::cy(i) != 0) t += real(L::cy(i)) * f[i];
+    } else {
+#pragma unroll
+      for (int i = 0; i < Q; i++)
+        if (L::cz(i) != 0) t += real(L::cz(i)) * f[i];
     }
     sTr[b][tx] = t;
   }
-  __syncthreads();
+  sync();
   if (!work) return;
 
   real Qv[K];
@@ -337,25 +325,115 @@ step_kernel(const StepArgs<real> a) {
   // on the fluid path), S6 flux row of this variable
   real Phi[3];
   real inj;
-  double uS[3], BS[3];
-  if (solid_state<real, D>(a, x, y, z, n, uS, BS)) {
-    real Qh[K];
-    solid_blend<SCHEME, D, real>(Qv, a.gamma, uS, BS, Qh);
-    flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, Phi);
-    inj = pick<K, real>(Qh, k) - Qk;                            // dQh; the Powell source is scaled by d = 0
-  } else {
+  bool solid = false;
+  if (SOLID) {
+    double uS[3], BS[3];
+    if (solid_state<real, D>(a, c.x, c.y, c.z, c.n, uS, BS)) {
+      real Qh[K];
+      solid_blend<SCHEME, D, real>(Qv, a.gamma, uS, BS, Qh);
+      flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, Phi);
+      inj = pick<K, real>(Qh, k) - Qk;                          // dQh; the Powell source is scaled by d = 0
+      solid = true;
+    }
+  }
+  if (!solid) {
     flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, Phi);
     inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
   }
 
-  // S7 BGK + direct injection, S8 store
+  // S7 BGK + direct injection, S8 store:
+  //   g'_i = (1 - w) f_i + w_i [ w Q_k + inj ] + w_i (c_i . 3 w Phi)       (w = omega_k; Eq.2-3 with c_s^2 = 1/3)
   const real om = a.omega[k];
+  const real omc = real(1) - om;
+  const real b0 = om * Qk + inj;
+  const real P0 = real(3) * om * Phi[0], P1 = real(3) * om * Phi[1], P2 = real(3) * om * Phi[2];
+  char *__restrict__ dp = reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + c.n));
 #pragma unroll
   for (int i = 0; i < Q; i++) {
-    const real cPhi = real(L::cx(i)) * Phi[0] + real(L::cy(i)) * Phi[1] + real(L::cz(i)) * Phi[2];
-    const real feq = real(L::w(i)) * (Qk + real(3) * cPhi);
-    dstk[(size_t)i * ps + n] = f[i] + om * (feq - f[i]) + real(L::w(i)) * inj;
+    real t = real(L::w(i)) * b0;
+    if (L::cx(i) != 0) t = fma(real(L::cx(i) * L::w(i)), P0, t);
+    if (L::cy(i) != 0) t = fma(real(L::cy(i) * L::w(i)), P1, t);
+    if (L::cz(i) != 0) t = fma(real(L::cz(i) * L::w(i)), P2, t);
+    *reinterpret_cast<real *>(dp + a.st_off[i]) = fma(f[i], omc, t);
   }
+}
+
+// =====================================================================================================
+// Fused step kernel, A/B buffers, plain coalesced pulls (S1) + finish_cell.
+// =====================================================================================================
+template <int LAT, int SCHEME, typename real, int TX, int MINB>
+__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
+step_kernel(const StepArgs<real> a) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, Q = L::Q;
+  using V = Vars<SCHEME, D>;
+  constexpr int K = V::K;
+  __shared__ real sQ[K][TX];
+  __shared__ real sTr[D][TX];
+
+  const int tx = threadIdx.x, k = threadIdx.y;
+  const int x0 = blockIdx.x * TX;
+  const int x = x0 + tx, y = blockIdx.y, z = blockIdx.z;
+  const int nx = a.nx, ny = a.ny, nz = a.nz;
+  const bool active = x < nx;
+  const uint32_t ps = (uint32_t)a.pstride;
+  const uint32_t n = ((uint32_t)z * ny + y) * nx + (active ? x : 0);
+  const real *__restrict__ srck = a.src + (size_t)k * Q * a.pstride;
+
+  const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
+  const bool x_lo = x == 0, x_hi = x == nx - 1;
+  const bool y_lo = D > 1 && y == 0, y_hi = D > 1 && y == ny - 1;
+  const bool z_lo = D > 2 && z == 0, z_hi = D > 2 && z == nz - 1;
+  const int xm = x_lo ? nx - 1 : x - 1, xp = x_hi ? 0 : x + 1;
+  const int ym = y_lo ? ny - 1 : y - 1, yp = y_hi ? 0 : y + 1;
+  const int zm = z_lo ? nz - 1 : z - 1, zp = z_hi ? 0 : z + 1;
+  const auto sync = [] { __syncthreads(); };
+
+  // block-uniform classification.  Interior tile: no face, no wrap in any direction, every thread active, no
+  // mask, sphere out of reach -> the lean path: one base pointer per thread plus per-direction byte offsets
+  // from the constant bank, no predicates.
+  const bool interior = x0 >= 1 && x0 + TX <= nx - 1 && (D < 2 || (y >= 1 && y <= ny - 2)) && (D < 3 || (z >= 1 && z <= nz - 2)) &&
+                        a.mask == nullptr && !sphere_may_touch<real, D>(a, x0, TX, y, z);
+  real f[Q];
+  if (interior) {
+    const char *__restrict__ pb = reinterpret_cast<const char *>(a.src + ((size_t)k * Q * a.pstride + n));
+#pragma unroll
+    for (int i = 0; i < Q; i++) f[i] = *reinterpret_cast<const real *>(pb + a.ld_off[i]);
+    CellCtx c{tx, k, x, y, z, n, true, false, false, false, false, false, false};
+    finish_cell<LAT, SCHEME, real, TX, false, false>(a, c, f, sQ, sTr, sync);
+    return;
+  }
+
+  // frozen cells keep their populations: mask FROZEN or on an INFLOW face (A10)
+  bool frozen = false;
+  if (active) {
+    frozen = (a.mask != nullptr && a.mask[n] == CELL_FROZEN) || (x_lo && a.bc[0] == BC_INFLOW) ||
+             (x_hi && a.bc[1] == BC_INFLOW) || (y_lo && a.bc[2] == BC_INFLOW) || (y_hi && a.bc[3] == BC_INFLOW) ||
+             (z_lo && a.bc[4] == BC_INFLOW) || (z_hi && a.bc[5] == BC_INFLOW);
+    if (frozen) {
+      real *__restrict__ dstk = a.dst + (size_t)k * Q * a.pstride;
+#pragma unroll
+      for (int i = 0; i < Q; i++) dstk[(uint32_t)i * ps + n] = srck[(uint32_t)i * ps + n];
+    }
+  }
+  const bool work = active && !frozen;
+  const bool out_xm = npx && x_lo, out_xp = npx && x_hi;
+  const bool out_ym = npy && y_lo, out_yp = npy && y_hi;
+  const bool out_zm = npz && z_lo, out_zp = npz && z_hi;
+
+  // S1 pull: f_i(x) = g_i(x - c_i), periodic wrap; sources outside a non-periodic face are filled in finish_cell
+#pragma unroll
+  for (int i = 0; i < Q; i++) {
+    const int cx = L::cx(i), cy = L::cy(i), cz = L::cz(i);
+    const int sx = cx == 1 ? xm : (cx == -1 ? xp : x);
+    const int sy = cy == 1 ? ym : (cy == -1 ? yp : y);
+    const int sz = cz == 1 ? zm : (cz == -1 ? zp : z);
+    const bool outside = (cx == 1 && out_xm) || (cx == -1 && out_xp) || (cy == 1 && out_ym) || (cy == -1 && out_yp) ||
+                         (cz == 1 && out_zm) || (cz == -1 && out_zp);
+    f[i] = (work && !outside) ? srck[(uint32_t)i * ps + ((uint32_t)sz * ny + sy) * nx + sx] : real(0);
+  }
+  CellCtx c{tx, k, x, y, z, n, work, out_xm, out_xp, out_ym, out_yp, out_zm, out_zp};
+  finish_cell<LAT, SCHEME, real, TX, true, true>(a, c, f, sQ, sTr, sync);
 }
 
 // ---- S10 init: g_{k,i} = w_i (Q_k + c_i.Phi_k(Q)/c_s^2) (Eq.3) from fp64 fields [K][N] ---------
