@@ -72,6 +72,7 @@ bool layout(const lbmhd_params *p, const Geometry &g, Layout *L) {
   const size_t N = (size_t)p->nx * p->ny * p->nz;
   const size_t es = p->precision == 64 ? 8 : 4;
   L->pstride = align_up(N, 32);
+  if (const char *e = getenv("LBMHD_PAD")) L->pstride += 32 * (size_t)atoi(e);   // experiment: skew planes across DRAM channels
   L->pop_bytes = align_up((size_t)g.K * g.Q * L->pstride * es, 256);
   size_t off = 0;
   L->off_pop[0] = off; off += L->pop_bytes;
@@ -104,6 +105,7 @@ struct lbmhd {
   double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs;
   long long sph_t0;
   int tx, minb;          // x-tile and min blocks/SM (launch bound) of the plain step kernel
+  bool split;            // interior / edge launches split (large grids); LBMHD_SPLIT=0/1 overrides
   bool use_tma;          // TMA-staged persistent step kernel (needs nx * sizeof(real) % 16 == 0)
   int num_sms;
   CUtensorMap tmap[2][2];   // [copy][0: tile-wide box, 1: box 16 bytes wider] 5D views (x, y, z, i, k) of the populations
@@ -215,7 +217,7 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
   }
   h->ws = (char *)p->workspace;
   h->stream = (cudaStream_t)p->stream;
-  h->tx = 32; h->minb = 3;
+  h->tx = 32; h->minb = g.Q > 9 ? 3 : 4;     // measured best on B200: D3Q19 80 regs x 3 blocks/SM, D2Q9/D1Q3 64 regs x 4
   if (const char *e = getenv("LBMHD_TX")) h->tx = atoi(e);        // tuning knobs; unknown pairs fall back to 32/2
   if (const char *e = getenv("LBMHD_MINB")) h->minb = atoi(e);
   cudaError_t e = cudaSetDevice(p->device);
@@ -225,10 +227,12 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
     if (e != cudaSuccess) { delete h; return fail(LBMHD_ECUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e)); }
     h->num_sms = sms;
+    h->split = false;   // measured slower on config 5: edge tiles lose DRAM page locality when launched apart from their rows
+    if (const char *e2 = getenv("LBMHD_SPLIT")) h->split = atoi(e2) != 0;
     const char *path = getenv("LBMHD_PATH");      // tuning knob: "plain" forces the register-pull kernel
     const size_t es = p->precision == 64 ? 8 : 4;
     const long long tiles = (long long)((p->nx + kTmaTX - 1) / kTmaTX) * p->ny * p->nz;
-    h->use_tma = !(path && strcmp(path, "plain") == 0) && ((size_t)p->nx * es) % 16 == 0 && tiles < 2000000000LL;
+    h->use_tma = path && strcmp(path, "tma") == 0 && ((size_t)p->nx * es) % 16 == 0 && tiles < 2000000000LL;
     if (h->use_tma) {
       const int rc = make_tensor_maps(h);
       if (rc) { delete h; return rc; }
@@ -260,8 +264,48 @@ template <int LAT, int SCHEME, typename real> struct Ops {
 
   static dim3 grid(const lbmhd_t *h, int tx) { return dim3((h->p.nx + tx - 1) / tx, h->p.ny, h->p.nz); }
 
+  // One launch over all tiles (small grids, masked obstacles), or the split form: a lean interior launch plus
+  // general launches over the x-edge columns, the y/z-edge rows and the sphere's bounding box.
   template <int TX, int MINB> static cudaError_t launch_step(lbmhd_t *h, const StepArgs<real> &a) {
-    step_kernel<LAT, SCHEME, real, TX, MINB><<<grid(h, TX), dim3(TX, K), 0, h->stream>>>(a);
+    constexpr int D = L::D;
+    const int nx = h->p.nx, ny = h->p.ny, nz = h->p.nz;
+    const int tiles_x = (nx + TX - 1) / TX;
+    const dim3 block(TX, K);
+    const bool split = h->split && !h->have_mask && tiles_x >= 3 && (D < 2 || ny >= 3) && (D < 3 || nz >= 3);
+    if (!split) {
+      step_kernel<LAT, SCHEME, real, TX, MINB, 0><<<dim3(tiles_x, ny, nz), block, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
+      h->launches += 1;
+      return cudaGetLastError();
+    }
+    const int iy0 = D > 1 ? 1 : 0, iny = D > 1 ? ny - 2 : 1;
+    const int iz0 = D > 2 ? 1 : 0, inz = D > 2 ? nz - 2 : 1;
+    // interior tiles (x-edge tiles excluded even when their cells are interior: they need wrap or face handling)
+    step_kernel<LAT, SCHEME, real, TX, MINB, 1><<<dim3(tiles_x - 2, iny, inz), block, 0, h->stream>>>(a, Region{1, 1, iy0, 1, iz0, 1}, 0);
+    // x-edge columns, all rows
+    step_kernel<LAT, SCHEME, real, TX, 2, 2><<<dim3(2, ny, nz), block, 0, h->stream>>>(a, Region{0, tiles_x - 1, 0, 1, 0, 1}, 0);
+    h->launches += 2;
+    if (D > 1) {   // y-edge rows of the remaining columns
+      step_kernel<LAT, SCHEME, real, TX, 2, 2><<<dim3(tiles_x - 2, 2, nz), block, 0, h->stream>>>(a, Region{1, 1, 0, ny - 1, 0, 1}, 0);
+      h->launches += 1;
+    }
+    if (D > 2) {   // z-edge planes of what is left
+      step_kernel<LAT, SCHEME, real, TX, 2, 2><<<dim3(tiles_x - 2, ny - 2, 2), block, 0, h->stream>>>(a, Region{1, 1, 1, 1, 0, nz - 1}, 0);
+      h->launches += 1;
+    }
+    if (a.has_sphere) {   // interior-positioned tiles inside the sphere's bounding box
+      const double R = a.sph_R + 1.0;
+      int bx_lo = (int)floor((a.sph_c[0] - R) / TX), bx_hi = (int)floor((a.sph_c[0] + R) / TX);
+      int y_lo = D > 1 ? (int)floor(a.sph_c[1] - R) : 0, y_hi = D > 1 ? (int)ceil(a.sph_c[1] + R) : 0;
+      int z_lo = D > 2 ? (int)floor(a.sph_c[2] - R) : 0, z_hi = D > 2 ? (int)ceil(a.sph_c[2] + R) : 0;
+      bx_lo = bx_lo < 1 ? 1 : bx_lo; bx_hi = bx_hi > tiles_x - 2 ? tiles_x - 2 : bx_hi;
+      y_lo = y_lo < iy0 ? iy0 : y_lo; y_hi = y_hi > iy0 + iny - 1 ? iy0 + iny - 1 : y_hi;
+      z_lo = z_lo < iz0 ? iz0 : z_lo; z_hi = z_hi > iz0 + inz - 1 ? iz0 + inz - 1 : z_hi;
+      if (bx_lo <= bx_hi && y_lo <= y_hi && z_lo <= z_hi) {
+        step_kernel<LAT, SCHEME, real, TX, 2, 2><<<dim3(bx_hi - bx_lo + 1, y_hi - y_lo + 1, z_hi - z_lo + 1), block, 0, h->stream>>>(
+            a, Region{bx_lo, 1, y_lo, 1, z_lo, 1}, 1);
+        h->launches += 1;
+      }
+    }
     return cudaGetLastError();
   }
 
@@ -278,6 +322,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     const long long n_rows = (long long)h->p.ny * h->p.nz;                 // < 2^31 - SMs checked at create
     const int grid = (int)(n_rows < (long long)h->num_sms ? n_rows : (long long)h->num_sms);
     kern<<<grid, C::THREADS, C::SMEM_BYTES, h->stream>>>(a, h->tmap[h->cur][0], h->tmap[h->cur][1], tiles_x, (int)n_rows);
+    h->launches += 1;
     return cudaGetLastError();
   }
 
@@ -335,7 +380,6 @@ template <int LAT, int SCHEME, typename real> struct Ops {
       if (e != cudaSuccess) return fail(LBMHD_ECUDA, "step kernel launch: %s", cudaGetErrorString(e));
       h->cur = 1 - h->cur;
       h->t += 1;
-      h->launches += 1;
     }
     return LBMHD_OK;
   }

@@ -243,9 +243,9 @@ __device__ __forceinline__ bool sphere_may_touch(const StepArgs<real> &a, int x0
 // barrier (__syncthreads or a named barrier).  BND / SOLID are tile-uniform: the interior fluid tile (both
 // false) is the hot path and carries no boundary predicates, no mask or sphere test.
 // =====================================================================================================
-template <int LAT, int SCHEME, typename real, int TX, bool BND, bool SOLID, class Sync>
-__device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellCtx &c, real (&f)[Lattice<LAT>::Q],
-                                            real (*sQ)[TX], real (*sTr)[TX], Sync sync) {
+template <int LAT, int SCHEME, typename real, int TX, bool BND, bool SOLID, class FArr, class Sync>
+__device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellCtx &c, FArr &f, real (*sQ)[TX],
+                                            real (*sTr)[TX], Sync sync) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
   using V = Vars<SCHEME, D>;
@@ -255,7 +255,7 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   const bool work = c.work;
   const real *__restrict__ srck = a.src + (size_t)k * Q * a.pstride;
 
-  if (BND) {
+  if constexpr (BND) {
     // A9 / PAPER.md:154: directions whose source is outside take the equilibrium of the inward neighbour's state
     const bool cell_bnd = work && (c.out_xm || c.out_xp || c.out_ym || c.out_yp || c.out_zm || c.out_zp);
     if (cell_bnd) {
@@ -326,7 +326,7 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   real Phi[3];
   real inj;
   bool solid = false;
-  if (SOLID) {
+  if constexpr (SOLID) {
     double uS[3], BS[3];
     if (solid_state<real, D>(a, c.x, c.y, c.z, c.n, uS, BS)) {
       real Qh[K];
@@ -359,27 +359,20 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
 }
 
 // =====================================================================================================
-// Fused step kernel, A/B buffers, plain coalesced pulls (S1) + finish_cell.
+// General tile (faces, periodic wrap, mask, sphere): register pulls with per-direction predicates, then
+// finish_cell with boundary and solid handling compiled in.  Used by every step kernel for the tiles that are
+// not interior; the TX*K threads of the tile call it together.
 // =====================================================================================================
-template <int LAT, int SCHEME, typename real, int TX, int MINB>
-__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
-step_kernel(const StepArgs<real> a) {
+template <int LAT, int SCHEME, typename real, int TX, class Sync>
+__device__ __forceinline__ void general_tile(const StepArgs<real> &a, int tx, int k, int x, int y, int z, real (*sQ)[TX],
+                                          real (*sTr)[TX], Sync sync) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
-  using V = Vars<SCHEME, D>;
-  constexpr int K = V::K;
-  __shared__ real sQ[K][TX];
-  __shared__ real sTr[D][TX];
-
-  const int tx = threadIdx.x, k = threadIdx.y;
-  const int x0 = blockIdx.x * TX;
-  const int x = x0 + tx, y = blockIdx.y, z = blockIdx.z;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
   const bool active = x < nx;
   const uint32_t ps = (uint32_t)a.pstride;
   const uint32_t n = ((uint32_t)z * ny + y) * nx + (active ? x : 0);
   const real *__restrict__ srck = a.src + (size_t)k * Q * a.pstride;
-
   const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
   const bool x_lo = x == 0, x_hi = x == nx - 1;
   const bool y_lo = D > 1 && y == 0, y_hi = D > 1 && y == ny - 1;
@@ -387,22 +380,7 @@ step_kernel(const StepArgs<real> a) {
   const int xm = x_lo ? nx - 1 : x - 1, xp = x_hi ? 0 : x + 1;
   const int ym = y_lo ? ny - 1 : y - 1, yp = y_hi ? 0 : y + 1;
   const int zm = z_lo ? nz - 1 : z - 1, zp = z_hi ? 0 : z + 1;
-  const auto sync = [] { __syncthreads(); };
-
-  // block-uniform classification.  Interior tile: no face, no wrap in any direction, every thread active, no
-  // mask, sphere out of reach -> the lean path: one base pointer per thread plus per-direction byte offsets
-  // from the constant bank, no predicates.
-  const bool interior = x0 >= 1 && x0 + TX <= nx - 1 && (D < 2 || (y >= 1 && y <= ny - 2)) && (D < 3 || (z >= 1 && z <= nz - 2)) &&
-                        a.mask == nullptr && !sphere_may_touch<real, D>(a, x0, TX, y, z);
   real f[Q];
-  if (interior) {
-    const char *__restrict__ pb = reinterpret_cast<const char *>(a.src + ((size_t)k * Q * a.pstride + n));
-#pragma unroll
-    for (int i = 0; i < Q; i++) f[i] = *reinterpret_cast<const real *>(pb + a.ld_off[i]);
-    CellCtx c{tx, k, x, y, z, n, true, false, false, false, false, false, false};
-    finish_cell<LAT, SCHEME, real, TX, false, false>(a, c, f, sQ, sTr, sync);
-    return;
-  }
 
   // frozen cells keep their populations: mask FROZEN or on an INFLOW face (A10)
   bool frozen = false;
@@ -434,6 +412,120 @@ step_kernel(const StepArgs<real> a) {
   }
   CellCtx c{tx, k, x, y, z, n, work, out_xm, out_xp, out_ym, out_yp, out_zm, out_zp};
   finish_cell<LAT, SCHEME, real, TX, true, true>(a, c, f, sQ, sTr, sync);
+}
+
+// Which tiles a launch covers: block (bx, by, bz) -> tile (bx0 + bx*bxs, y0 + by*ys, z0 + bz*zs).
+struct Region {
+  int bx0, bxs, y0, ys, z0, zs;
+};
+
+// =====================================================================================================
+// Fused step kernel, A/B buffers, plain coalesced pulls into registers (S1) + finish_cell.
+// MODE 0: one launch over all tiles; interior tiles take the lean path, the others general_tile().
+// MODE 1: interior tiles only (the launch covers bx in [1, tiles_x-2], y in [1, ny-2], z in [1, nz-2]); tiles the
+//         sphere may touch are left to a MODE 2 launch.  No general path is compiled in, so the register
+//         budget is that of the lean path alone.
+// MODE 2: general tiles only, over a Region (x-edge columns, y/z-edge rows, sphere bounding box); with
+//         sphere_only the launch handles exactly the interior-positioned tiles that MODE 1 skipped.
+// =====================================================================================================
+template <int LAT, int SCHEME, typename real, int TX, int MINB, int MODE>
+__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
+step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int sphere_only) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, Q = L::Q;
+  using V = Vars<SCHEME, D>;
+  constexpr int K = V::K;
+  __shared__ real sQ[K][TX];
+  __shared__ real sTr[D][TX];
+
+  const int tx = threadIdx.x, k = threadIdx.y;
+  const int x0 = (r.bx0 + (int)blockIdx.x * r.bxs) * TX;
+  const int x = x0 + tx, y = r.y0 + (int)blockIdx.y * r.ys, z = r.z0 + (int)blockIdx.z * r.zs;
+  const int nx = a.nx, ny = a.ny, nz = a.nz;
+  const auto sync = [] { __syncthreads(); };
+
+  // block-uniform classification.  Interior tile: no face, no wrap in any direction, every thread active, no
+  // mask, sphere out of reach -> the lean path: one base pointer per thread plus per-direction byte offsets
+  // from the constant bank, no predicates.
+  const bool inner_pos = x0 >= 1 && x0 + TX <= nx - 1 && (D < 2 || (y >= 1 && y <= ny - 2)) && (D < 3 || (z >= 1 && z <= nz - 2));
+  const bool touched = sphere_may_touch<real, D>(a, x0, TX, y, z);
+  const bool interior = inner_pos && a.mask == nullptr && !touched;
+  if (MODE == 1 && !interior) return;
+  if (MODE == 2 && sphere_only && !(inner_pos && touched)) return;
+  if (MODE != 2 && interior) {
+    const uint32_t n = ((uint32_t)z * ny + y) * nx + x;
+    const char *__restrict__ pb = reinterpret_cast<const char *>(a.src + ((size_t)k * Q * a.pstride + n));
+    real f[Q];
+#pragma unroll
+    for (int i = 0; i < Q; i++) f[i] = *reinterpret_cast<const real *>(pb + a.ld_off[i]);
+    CellCtx c{tx, k, x, y, z, n, true, false, false, false, false, false, false};
+    finish_cell<LAT, SCHEME, real, TX, false, false>(a, c, f, sQ, sTr, sync);
+    return;
+  }
+  if (MODE == 1) return;
+
+  // x-edge tile of an otherwise interior row (no mask, sphere out of reach, not both ends in one tile): lean
+  // loads for every thread; only the thread ON the face differs (A9-A11):
+  //   periodic x   its c_x != 0 sources come from the other end of the row (offset +- nx);
+  //   INFLOW face  it is frozen: it re-stores its own populations;
+  //   ZEROGRAD     its outside directions take f^eq of the inward neighbour's state Q^nb = sum_j g_j(x +- 1); the Q
+  //                values g_j(nb) are fetched one per lane together with the pulls and summed by shuffles, so the
+  //                face costs no second memory round trip.
+  const bool row_inner = (D < 2 || (y >= 1 && y <= ny - 2)) && (D < 3 || (z >= 1 && z <= nz - 2));
+  const bool edge_lo = x0 == 0, edge_hi = x0 + TX >= nx;
+  if (TX == 32 && row_inner && a.mask == nullptr && !touched && (edge_lo != edge_hi) && nx >= 3) {
+    const bool active = x < nx;
+    const int xe = active ? x : nx - 1;                      // inactive tail threads shadow the last cell, store nothing
+    const uint32_t n = ((uint32_t)z * ny + y) * nx + xe;
+    const bool on_face = active && (edge_lo ? x == 0 : x == nx - 1);
+    const int bcf = edge_lo ? a.bc[0] : a.bc[1];
+    const bool frozen = on_face && bcf == BC_INFLOW;
+    const bool zg = on_face && bcf == BC_ZEROGRAD;
+    const bool wrap = on_face && bcf == BC_PERIODIC;
+    const long long wrap_adj = (long long)nx * (long long)sizeof(real) * (edge_lo ? 1 : -1);
+    const char *__restrict__ pb = reinterpret_cast<const char *>(a.src + ((size_t)k * Q * a.pstride + n));
+    real f[Q];
+#pragma unroll
+    for (int i = 0; i < Q; i++) {
+      long long off = frozen ? a.st_off[i] : a.ld_off[i];
+      if ((edge_lo && L::cx(i) == 1) || (!edge_lo && L::cx(i) == -1)) off += wrap ? wrap_adj : 0;   // only these cross the face
+      f[i] = *reinterpret_cast<const real *>(pb + off);
+    }
+    __shared__ real sNb[K];
+    const bool tile_zg = bcf == BC_ZEROGRAD;                 // tile-uniform
+    if (tile_zg) {
+      // lane j < Q fetches g_{k,j}(nb), nb = the face cell's inward neighbour; butterfly sum -> Q^nb_k in every lane
+      const uint32_t nb = ((uint32_t)z * ny + y) * nx + (edge_lo ? 1 : nx - 2);
+      real v = tx < Q ? a.src[(size_t)k * Q * a.pstride + (size_t)tx * a.pstride + nb] : real(0);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+      if (tx == 0) sNb[k] = v;
+      __syncthreads();
+      if (zg) {
+        real Qnb[K], Phi[3];
+#pragma unroll
+        for (int l = 0; l < K; l++) Qnb[l] = sNb[l];
+        flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, Phi);
+        const real Qnbk = pick<K, real>(Qnb, k);
+#pragma unroll
+        for (int i = 0; i < Q; i++) {
+          if ((edge_lo && L::cx(i) == 1) || (!edge_lo && L::cx(i) == -1)) {
+            const real cPhi = real(L::cx(i)) * Phi[0] + real(L::cy(i)) * Phi[1] + real(L::cz(i)) * Phi[2];
+            f[i] = real(L::w(i)) * (Qnbk + real(3) * cPhi);
+          }
+        }
+      }
+    }
+    if (frozen) {
+      char *dp = reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + n));
+#pragma unroll
+      for (int i = 0; i < Q; i++) *reinterpret_cast<real *>(dp + a.st_off[i]) = f[i];
+    }
+    CellCtx c{tx, k, x, y, z, n, active && !frozen, false, false, false, false, false, false};
+    finish_cell<LAT, SCHEME, real, TX, false, false>(a, c, f, sQ, sTr, sync);
+    return;
+  }
+  general_tile<LAT, SCHEME, real, TX>(a, tx, k, x, y, z, sQ, sTr, sync);
 }
 
 // ---- S10 init: g_{k,i} = w_i (Q_k + c_i.Phi_k(Q)/c_s^2) (Eq.3) from fp64 fields [K][N] ---------

@@ -84,7 +84,7 @@ template <int LAT, int SCHEME, typename real, int TXT, int NSTAGE> struct TmaCfg
 
 template <int LAT, int SCHEME, typename real, int TXT, int NSTAGE>
 __global__ void __launch_bounds__(TmaCfg<LAT, SCHEME, real, TXT, NSTAGE>::THREADS, 1)
-step_kernel_tma(const StepArgs<real> a, const __grid_constant__ CUtensorMap map_tile, const __grid_constant__ CUtensorMap map_wide,
+step_kernel_tma(const __grid_constant__ StepArgs<real> a, const __grid_constant__ CUtensorMap map_tile, const __grid_constant__ CUtensorMap map_wide,
                 int tiles_x, int n_rows) {
   using C = TmaCfg<LAT, SCHEME, real, TXT, NSTAGE>;
   using L = Lattice<LAT>;
