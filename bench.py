@@ -191,10 +191,13 @@ def run_native(args, rank, world, local_rank):
     achieved = N * bytes_per_cell / (ms_step * 1e-3) / 1e9
     e2e_val = world * N * args.steps / (ms_e2e * 1e-3) / 1e6
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic_%s.json" % args.workload)
-    if os.path.exists(tpath):
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")      # dram__bytes_read/write.sum of one ncu --set full capture
+    if os.path.exists(tpath) and prec == 64:
         with open(tpath) as f:
-            traffic = json.load(f).get("dram_bytes_per_launch")
+            for row in f.read().splitlines()[1:]:
+                cols = row.split(",")
+                if cols[0] == args.workload:
+                    traffic = float(cols[1]) + float(cols[2])
     line = {
         "metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

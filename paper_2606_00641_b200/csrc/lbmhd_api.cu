@@ -72,7 +72,6 @@ bool layout(const lbmhd_params *p, const Geometry &g, Layout *L) {
   const size_t N = (size_t)p->nx * p->ny * p->nz;
   const size_t es = p->precision == 64 ? 8 : 4;
   L->pstride = align_up(N, 32);
-  if (const char *e = getenv("LBMHD_PAD")) L->pstride += 32 * (size_t)atoi(e);   // experiment: skew planes across DRAM channels
   L->pop_bytes = align_up((size_t)g.K * g.Q * L->pstride * es, 256);
   size_t off = 0;
   L->off_pop[0] = off; off += L->pop_bytes;
@@ -347,7 +346,6 @@ template <int LAT, int SCHEME, typename real> struct Ops {
       }
     }
     a.has_sphere = h->has_sphere ? 1 : 0;
-    if (const char *e = getenv("LBMHD_DBG")) a.dbg = atoi(e);
     if (h->has_sphere) {
       a.sph_R = h->sph_R;
       a.sph_R2 = h->sph_R * h->sph_R;

@@ -37,7 +37,6 @@ template <typename real> struct StepArgs {
   long long ld_off[19];         // bytes from a cell's own slot in plane (k,0) to its pull source in plane (k,i), no wrap:
                                 //   (i*pstride - (c_x + c_y nx + c_z nx ny)) * sizeof(real)
   long long st_off[19];         // i * pstride * sizeof(real)
-  int dbg;                      // experiments only (LBMHD_DBG): 1 = TMA kernel skips the math and the stores
   int has_sphere;
   double sph_c[3], sph_R, sph_R2, sph_m[3], sph_Bs, sph_u[3];
 };

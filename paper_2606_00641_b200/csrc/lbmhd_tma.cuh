@@ -123,7 +123,7 @@ step_kernel_tma(const __grid_constant__ StepArgs<real> a, const __grid_constant_
       uint32_t ph = 0;
       while (row < n_rows) {
         mbar_wait(&empty[s], ph ^ 1u);
-        mbar_expect_tx(&full[s], a.dbg == 2 ? (uint32_t)(Q * K * TXT * sizeof(real)) : (uint32_t)C::tx_bytes());
+        mbar_expect_tx(&full[s], (uint32_t)C::tx_bytes());
         unsigned char *dst = smem + (size_t)s * C::STAGE_BYTES;
 #pragma unroll
         for (int i = 0; i < Q; i++) {
@@ -132,10 +132,6 @@ step_kernel_tma(const __grid_constant__ StepArgs<real> a, const __grid_constant_
           if (!npz && D > 2) sz = sz < 0 ? nz - 1 : (sz >= nz ? 0 : sz);
           // aligned window: c_x = +1 needs x0-1.. -> start x0-PAD; c_x = -1 needs ..x0+TXT -> start x0, PAD wider
           const int c0 = L::cx(i) == 1 ? bx * TXT - C::PAD : bx * TXT;
-          if (a.dbg == 2) {   // experiment: every box tile-aligned (wrong data, timing only)
-            tma_load_5d(dst + C::slot_off(i), &map_tile, &full[s], bx * TXT, sy, sz, i, 0);
-            continue;
-          }
           tma_load_5d(dst + C::slot_off(i), L::cx(i) == 0 ? &map_tile : &map_wide, &full[s], c0, sy, sz, i, 0);
         }
         if (++s == NSTAGE) { s = 0; ph ^= 1u; }
@@ -231,12 +227,7 @@ step_kernel_tma(const __grid_constant__ StepArgs<real> a, const __grid_constant_
 #pragma unroll
       for (int i = 0; i < Q; i++) f[i] = real(0);
     }
-    if (a.dbg >= 1) {
-      real acc = real(0);
-#pragma unroll
-      for (int i = 0; i < Q; i++) acc += f[i];
-      if (acc == real(1.2345e-300)) dstk[n] = acc;
-    } else if (!special) {
+    if (!special) {
       CellCtx c{tx, k, x, y, z, n, work, false, false, false, false, false, false};
       finish_cell<LAT, SCHEME, real, TXT, false, false>(a, c, f, sQ, sTr, gsync);
     } else {
