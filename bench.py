@@ -72,6 +72,22 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons)}
 
 
+def max_over_ranks(values, world, device=None):
+    """element-wise MAX of a list of floats over all ranks (the contract's max-over-ranks timing); identity at world 1"""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(values, dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def aggregate_mlups(cells_per_rank, steps, ms, world):
+    """whole-job throughput: every rank advanced its own replica `steps` times in `ms` (max over ranks)"""
+    return world * cells_per_rank * steps / (ms * 1e-3) / 1e6
+
+
 def oracle_leg(workload_name, steps, warmup, budget_s=None):
     """the CPU oracle, as it stands, on a bounded sample of the workload; -> (MLUPS, cores, sample text, ms/step)"""
     from oracle import oracle as orc
@@ -176,10 +192,7 @@ def run_native(args, rank, world, local_rank):
     h2d = F_host.numel() * 8
     d2h = out_host.numel() * 8 + diag_host.numel() * 8
 
-    times = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    ms_total, ms_e2e = [float(v) for v in times.cpu()]
+    ms_total, ms_e2e = max_over_ranks([ms_total, ms_e2e], world, dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -187,9 +200,9 @@ def run_native(args, rank, world, local_rank):
 
     peak, peak_src = load_peaks()
     ms_step = ms_total / args.steps
-    value = world * N * args.steps / (ms_total * 1e-3) / 1e6
+    value = aggregate_mlups(N, args.steps, ms_total, world)
     achieved = N * bytes_per_cell / (ms_step * 1e-3) / 1e9
-    e2e_val = world * N * args.steps / (ms_e2e * 1e-3) / 1e6
+    e2e_val = aggregate_mlups(N, args.steps, ms_e2e, world)
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.csv")      # dram__bytes_read/write.sum of one ncu --set full capture
     if os.path.exists(tpath) and prec == 64:

@@ -1,0 +1,107 @@
+"""Parity at BASELINE's full sizes, in the launch configuration bench.py times, on SAMPLED outputs: the value of a
+cell after n steps depends only on the initial fields within n cells (|c_i| <= 1), so the oracle recomputes each
+sampled cell on a small sub-box cut out of the same seeded input (true boundary kinds on faces the box shares with
+the domain, a zero-gradient cut elsewhere, kept > n cells away from the sample)."""
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2606_00641_b200 import workloads as W
+from parity_util import LAT_ORC, TOL64
+
+pytestmark = pytest.mark.gpu
+NSTEPS = 4
+MARGIN = NSTEPS + 2
+
+
+def subbox_oracle(w, centre_xyz, nsteps):
+    """-> oracle fields on the sub-box and the index of the sample inside it"""
+    shape = w["shape"]
+    D = len(shape)
+    F = w["fields"]
+    lo, hi, bc, idx = [], [], list(w["bc"]), []
+    for a in range(3):
+        if a >= D:
+            lo.append(0); hi.append(1); idx.append(np.array([0])); continue
+        n, c = shape[a], centre_xyz[a]
+        periodic = w["bc"][2 * a] == 0
+        l, h = c - MARGIN, c + MARGIN + 1
+        if not periodic:
+            l, h = max(l, 0), min(h, n)
+        lo.append(l); hi.append(h)
+        idx.append(np.arange(l, h) % n)
+        # faces shared with the domain keep their kind; cuts are zero-gradient
+        bc[2 * a] = w["bc"][2 * a] if (not periodic and l == 0) else 1
+        bc[2 * a + 1] = w["bc"][2 * a + 1] if (not periodic and h == n) else 1
+    sub = F[:, idx[2]][:, :, idx[1]][:, :, :, idx[0]]
+    sub_shape = tuple(len(idx[a]) for a in range(D))
+    p = orc.make_params(orc.IDEAL if w["scheme"] == "IDEAL" else orc.INCRES, LAT_ORC[w["lattice"]], sub_shape,
+                        gamma=w["gamma"] or 1.4, c0sq=w["c0sq"], nu=w["nu"], eta=w["eta"], tau=w["tau"], powell=w["powell"], bc=bc)
+    o = orc.Oracle(p)
+    if w.get("sphere"):
+        s = w["sphere"]
+        cen = np.array(s["centre"], dtype=np.float64) - np.array([lo[0], lo[1], lo[2]], dtype=np.float64)
+        o.set_sphere(cen, s["radius"], s["u_solid"], s["dipole_dir"], s["B_surface"])
+    o.init(np.ascontiguousarray(sub))
+    o.step(nsteps)
+    Q = o.moments(diag=False)
+    loc = tuple(centre_xyz[a] - lo[a] if a < D else 0 for a in range(3))
+    return Q[:, loc[2], loc[1], loc[0]]
+
+
+def run_fullsize(name, samples):
+    from paper_2606_00641_b200 import lbmhd
+    w = W.get(name)
+    sim = lbmhd.from_workload(w)
+    sim.init(w["fields"])
+    sim.step(NSTEPS)
+    Q, dg = sim.moments()
+    assert dg[-1] == 0
+    scale = np.abs(Q).reshape(Q.shape[0], -1).max(1)
+    worst = 0.0
+    for c in samples:
+        ref = subbox_oracle(w, c, NSTEPS)
+        z = c[2] if len(w["shape"]) > 2 else 0
+        y = c[1] if len(w["shape"]) > 1 else 0
+        got = Q[:, z, y, c[0]]
+        for k in range(Q.shape[0]):
+            err = abs(got[k] - ref[k]) / scale[k] if scale[k] > 0 else abs(got[k] - ref[k])
+            worst = max(worst, err)
+            assert err <= TOL64, (name, c, k, got[k], ref[k])
+    sim.close()
+    return worst
+
+
+def test_config5_fullsize_sampled():
+    """384x256x256: inflow and outflow faces, periodic seams, the moving sphere's surface, centre and wake, interior"""
+    rng = np.random.default_rng(55)
+    S = [(0, 10, 10), (1, 100, 200), (383, 5, 250), (382, 128, 128), (200, 0, 0), (200, 255, 255), (31, 0, 128), (32, 255, 17),
+         (383, 0, 0), (0, 255, 255), (128, 128, 128), (127, 128, 128), (128, 152, 128), (128, 153, 128), (152, 128, 128),
+         (153, 128, 128), (104, 128, 128), (128, 128, 104), (140, 140, 140), (160, 128, 128), (96, 128, 128)]
+    S += [tuple(int(v) for v in (rng.integers(0, 384), rng.integers(0, 256), rng.integers(0, 256))) for _ in range(12)]
+    print("C5 full size, worst sampled error", run_fullsize("C5", S))
+
+
+def test_config4_fullsize_sampled():
+    """2048^2 with zero-gradient sides: corners, edges, rotor rim, interior"""
+    rng = np.random.default_rng(44)
+    S = [(0, 0, 0), (2047, 2047, 0), (0, 2047, 0), (2047, 0, 0), (0, 1000, 0), (1000, 0, 0), (2047, 777, 0), (31, 5, 0), (32, 2046, 0),
+         (1024, 1024, 0), (1228, 1024, 0), (1024, 1259, 0), (1200, 1200, 0)]
+    S += [(int(rng.integers(0, 2048)), int(rng.integers(0, 2048)), 0) for _ in range(10)]
+    print("C4 full size, worst sampled error", run_fullsize("C4", S))
+
+
+def test_config3_and_2_fullsize_sampled():
+    rng = np.random.default_rng(33)
+    for name, n in (("C3", 1024), ("C2", 512)):
+        S = [(0, 0, 0), (n - 1, n - 1, 0), (0, n // 2, 0), (n // 2, n - 1, 0), (31, 31, 0), (32, 32, 0)]
+        S += [(int(rng.integers(0, n)), int(rng.integers(0, n)), 0) for _ in range(8)]
+        print(name, "full size, worst sampled error", run_fullsize(name, S))
+
+
+def test_config1_full_size_all_cells_500_steps():
+    """config 1 IS small: the whole 800-cell tube, all 500 steps, element by element"""
+    from test_parity_gpu import compare
+    w = W.get("C1")
+    errs = compare(w, 500)
+    print("C1 full run", errs.max())
