@@ -63,7 +63,7 @@ constexpr int kMaxDiagBlocks = 1184;   // 8 x 148 SMs
 struct Layout {
   size_t pstride;        // elements per population plane (N rounded up to 32)
   size_t pop_bytes;      // one population copy
-  size_t off_pop[2], off_fields, off_mask, off_bsolid, off_partial, off_diag, total;
+  size_t off_pop[2], off_fields, off_M[2], off_mask, off_bsolid, off_partial, off_diag, total;
 };
 
 bool layout(const lbmhd_params *p, const Geometry &g, Layout *L) {
@@ -77,6 +77,9 @@ bool layout(const lbmhd_params *p, const Geometry &g, Layout *L) {
   L->off_pop[0] = off; off += L->pop_bytes;
   L->off_pop[1] = off; off += p->streaming == LBMHD_STREAM_AB ? L->pop_bytes : 0;
   L->off_fields = off; off += align_up((size_t)g.K * N * 8, 256);
+  // in place: two ping-pong arrays of published post-collision moments (Q^nb of face cells, state of frozen cells)
+  L->off_M[0] = off; off += p->streaming == LBMHD_STREAM_INPLACE ? align_up((size_t)g.K * N * 8, 256) : 0;
+  L->off_M[1] = off; off += p->streaming == LBMHD_STREAM_INPLACE ? align_up((size_t)g.K * N * 8, 256) : 0;
   L->off_mask = off; off += align_up(N, 256);
   L->off_bsolid = off; off += align_up(3 * N * 8, 256);
   L->off_partial = off; off += align_up((size_t)kMaxDiagBlocks * (3 * g.K + 4) * 8, 256);
@@ -95,7 +98,9 @@ struct lbmhd {
   double tau[8];
   cudaStream_t stream;
   char *ws;
-  int cur;               // which population copy holds the current state
+  int cur;               // A/B: which population copy holds the current state (in place: always 0)
+  int parity;            // in place: 0 = layout P0 (g_j(x) at (x, j)), 1 = layout P1 (after a pull-push step)
+  int mcur;              // in place: which M array holds the moments published by the last step
   long long t;           // steps done since init
   long long launches;
   bool have_mask, have_bsolid;
@@ -178,8 +183,8 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
   if (!geometry(p->scheme, p->lattice, &g)) return fail(LBMHD_EINVAL, "unknown scheme %d or lattice %d", p->scheme, p->lattice);
   Layout L;
   if (!layout(p, g, &L)) return fail(LBMHD_EINVAL, "bad dims %d x %d x %d or precision %d", p->nx, p->ny, p->nz, p->precision);
-  if (p->streaming != LBMHD_STREAM_AB)
-    return fail(LBMHD_EINVAL, "streaming mode %d is not built yet (only LBMHD_STREAM_AB)", p->streaming);
+  if (p->streaming != LBMHD_STREAM_AB && p->streaming != LBMHD_STREAM_INPLACE)
+    return fail(LBMHD_EINVAL, "unknown streaming mode %d", p->streaming);
   if (g.D < 2 && p->ny != 1) return fail(LBMHD_EINVAL, "ny must be 1 on a 1D lattice");
   if (g.D < 3 && p->nz != 1) return fail(LBMHD_EINVAL, "nz must be 1 on a 1D/2D lattice");
   if ((size_t)p->ny > 65535 || (size_t)p->nz > 65535) return fail(LBMHD_EINVAL, "ny, nz must be <= 65535");
@@ -231,7 +236,7 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     const char *path = getenv("LBMHD_PATH");      // tuning knob: "plain" forces the register-pull kernel
     const size_t es = p->precision == 64 ? 8 : 4;
     const long long tiles = (long long)((p->nx + kTmaTX - 1) / kTmaTX) * p->ny * p->nz;
-    h->use_tma = path && strcmp(path, "tma") == 0 && ((size_t)p->nx * es) % 16 == 0 && tiles < 2000000000LL;
+    h->use_tma = p->streaming == LBMHD_STREAM_AB && path && strcmp(path, "tma") == 0 && ((size_t)p->nx * es) % 16 == 0 && tiles < 2000000000LL;
     if (h->use_tma) {
       const int rc = make_tensor_maps(h);
       if (rc) { delete h; return rc; }
@@ -267,28 +272,35 @@ template <int LAT, int SCHEME, typename real> struct Ops {
   // general launches over the x-edge columns, the y/z-edge rows and the sphere's bounding box.
   template <int TX, int MINB> static cudaError_t launch_step(lbmhd_t *h, const StepArgs<real> &a) {
     constexpr int D = L::D;
+    if (h->p.streaming == LBMHD_STREAM_INPLACE) {
+      const dim3 g((h->p.nx + TX - 1) / TX, h->p.ny, h->p.nz), b(TX, K);
+      if (h->parity == 0) step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_PP><<<g, b, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
+      else step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_LOC><<<g, b, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
+      h->launches += 1;
+      return cudaGetLastError();
+    }
     const int nx = h->p.nx, ny = h->p.ny, nz = h->p.nz;
     const int tiles_x = (nx + TX - 1) / TX;
     const dim3 block(TX, K);
     const bool split = h->split && !h->have_mask && tiles_x >= 3 && (D < 2 || ny >= 3) && (D < 3 || nz >= 3);
     if (!split) {
-      step_kernel<LAT, SCHEME, real, TX, MINB, 0><<<dim3(tiles_x, ny, nz), block, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
+      step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_AB><<<dim3(tiles_x, ny, nz), block, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
       h->launches += 1;
       return cudaGetLastError();
     }
     const int iy0 = D > 1 ? 1 : 0, iny = D > 1 ? ny - 2 : 1;
     const int iz0 = D > 2 ? 1 : 0, inz = D > 2 ? nz - 2 : 1;
     // interior tiles (x-edge tiles excluded even when their cells are interior: they need wrap or face handling)
-    step_kernel<LAT, SCHEME, real, TX, MINB, 1><<<dim3(tiles_x - 2, iny, inz), block, 0, h->stream>>>(a, Region{1, 1, iy0, 1, iz0, 1}, 0);
+    step_kernel<LAT, SCHEME, real, TX, MINB, 1, ST_AB><<<dim3(tiles_x - 2, iny, inz), block, 0, h->stream>>>(a, Region{1, 1, iy0, 1, iz0, 1}, 0);
     // x-edge columns, all rows
-    step_kernel<LAT, SCHEME, real, TX, 2, 2><<<dim3(2, ny, nz), block, 0, h->stream>>>(a, Region{0, tiles_x - 1, 0, 1, 0, 1}, 0);
+    step_kernel<LAT, SCHEME, real, TX, 2, 2, ST_AB><<<dim3(2, ny, nz), block, 0, h->stream>>>(a, Region{0, tiles_x - 1, 0, 1, 0, 1}, 0);
     h->launches += 2;
     if (D > 1) {   // y-edge rows of the remaining columns
-      step_kernel<LAT, SCHEME, real, TX, 2, 2><<<dim3(tiles_x - 2, 2, nz), block, 0, h->stream>>>(a, Region{1, 1, 0, ny - 1, 0, 1}, 0);
+      step_kernel<LAT, SCHEME, real, TX, 2, 2, ST_AB><<<dim3(tiles_x - 2, 2, nz), block, 0, h->stream>>>(a, Region{1, 1, 0, ny - 1, 0, 1}, 0);
       h->launches += 1;
     }
     if (D > 2) {   // z-edge planes of what is left
-      step_kernel<LAT, SCHEME, real, TX, 2, 2><<<dim3(tiles_x - 2, ny - 2, 2), block, 0, h->stream>>>(a, Region{1, 1, 1, 1, 0, nz - 1}, 0);
+      step_kernel<LAT, SCHEME, real, TX, 2, 2, ST_AB><<<dim3(tiles_x - 2, ny - 2, 2), block, 0, h->stream>>>(a, Region{1, 1, 1, 1, 0, nz - 1}, 0);
       h->launches += 1;
     }
     if (a.has_sphere) {   // interior-positioned tiles inside the sphere's bounding box
@@ -300,7 +312,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
       y_lo = y_lo < iy0 ? iy0 : y_lo; y_hi = y_hi > iy0 + iny - 1 ? iy0 + iny - 1 : y_hi;
       z_lo = z_lo < iz0 ? iz0 : z_lo; z_hi = z_hi > iz0 + inz - 1 ? iz0 + inz - 1 : z_hi;
       if (bx_lo <= bx_hi && y_lo <= y_hi && z_lo <= z_hi) {
-        step_kernel<LAT, SCHEME, real, TX, 2, 2><<<dim3(bx_hi - bx_lo + 1, y_hi - y_lo + 1, z_hi - z_lo + 1), block, 0, h->stream>>>(
+        step_kernel<LAT, SCHEME, real, TX, 2, 2, ST_AB><<<dim3(bx_hi - bx_lo + 1, y_hi - y_lo + 1, z_hi - z_lo + 1), block, 0, h->stream>>>(
             a, Region{bx_lo, 1, y_lo, 1, z_lo, 1}, 1);
         h->launches += 1;
       }
@@ -353,8 +365,13 @@ template <int LAT, int SCHEME, typename real> struct Ops {
       for (int c = 0; c < 3; c++) { a.sph_m[c] = h->sph_m[c]; a.sph_u[c] = h->sph_u[c]; }
     }
     for (int s = 0; s < n_steps; s++) {
+      const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
       a.src = pops(h, h->cur);
-      a.dst = pops(h, 1 - h->cur);
+      a.dst = pops(h, inplace ? h->cur : 1 - h->cur);
+      if (inplace) {
+        a.M_cur = (const double *)(h->ws + h->L.off_M[h->mcur]);
+        a.M_next = (double *)(h->ws + h->L.off_M[1 - h->mcur]);
+      }
       if (h->has_sphere) {
         // A12: centre before step t is c0 + (t - t0) u^B; product and sum rounded separately, like the oracle
         const volatile double dt = (double)(h->t - h->sph_t0);
@@ -364,7 +381,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
         }
       }
       cudaError_t e;
-      if (h->use_tma) e = launch_step_tma(h, a);
+      if (inplace) e = h->minb == 4 ? launch_step<32, 4>(h, a) : launch_step<32, 3>(h, a);
+      else if (h->use_tma) e = launch_step_tma(h, a);
       else switch (h->tx * 10 + h->minb) {
         case 321: e = launch_step<32, 1>(h, a); break;
         case 322: e = launch_step<32, 2>(h, a); break;
@@ -376,7 +394,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
         default: e = launch_step<32, 3>(h, a); break;
       }
       if (e != cudaSuccess) return fail(LBMHD_ECUDA, "step kernel launch: %s", cudaGetErrorString(e));
-      h->cur = 1 - h->cur;
+      if (inplace) { h->parity ^= 1; h->mcur ^= 1; }
+      else h->cur = 1 - h->cur;
       h->t += 1;
     }
     return LBMHD_OK;
@@ -387,14 +406,29 @@ template <int LAT, int SCHEME, typename real> struct Ops {
         fields_dev, pops(h, 0), h->L.pstride, h->p.nx, h->p.ny, h->p.nz, (real)h->p.gamma, (real)h->p.c0sq);
     CUDA_TRY(cudaGetLastError());
     h->launches += 1;
-    return LBMHD_OK;
+    h->parity = 0;
+    return refresh_published(h);
   }
 
   static int moments(lbmhd_t *h, double *fields_dev) {
-    moments_kernel<LAT, SCHEME, real, TXAUX><<<grid(h, TXAUX), dim3(TXAUX, K), 0, h->stream>>>(
-        pops(h, h->cur), h->L.pstride, fields_dev, h->p.nx, h->p.ny, h->p.nz);
+    if (h->p.streaming == LBMHD_STREAM_INPLACE && h->parity == 1)
+      moments_p1_kernel<LAT, SCHEME, real, TXAUX><<<grid(h, TXAUX), dim3(TXAUX, K), 0, h->stream>>>(
+          pops(h, h->cur), h->L.pstride, fields_dev, h->p.nx, h->p.ny, h->p.nz, h->p.bc[0], h->p.bc[2], h->p.bc[4]);
+    else
+      moments_kernel<LAT, SCHEME, real, TXAUX><<<grid(h, TXAUX), dim3(TXAUX, K), 0, h->stream>>>(
+          pops(h, h->cur), h->L.pstride, fields_dev, h->p.nx, h->p.ny, h->p.nz);
     CUDA_TRY(cudaGetLastError());
     h->launches += 1;
+    return LBMHD_OK;
+  }
+
+  // in place: (re)publish the moments of every cell in both M arrays — after init, set_populations, set_obstacle
+  static int refresh_published(lbmhd_t *h) {
+    if (h->p.streaming != LBMHD_STREAM_INPLACE) return LBMHD_OK;
+    double *m0 = (double *)(h->ws + h->L.off_M[0]), *m1 = (double *)(h->ws + h->L.off_M[1]);
+    if (int rc = moments(h, m0)) return rc;
+    CUDA_TRY(cudaMemcpyAsync(m1, m0, (size_t)K * h->N * 8, cudaMemcpyDeviceToDevice, h->stream));
+    h->mcur = 0;
     return LBMHD_OK;
   }
 
@@ -412,7 +446,11 @@ template <int LAT, int SCHEME, typename real> struct Ops {
   }
 
   static int pops_export(lbmhd_t *h, double *out_dev) {
-    pops_export_kernel<real><<<1184, 256, 0, h->stream>>>(pops(h, h->cur), h->L.pstride, out_dev, h->N, K * Q);
+    if (h->p.streaming == LBMHD_STREAM_INPLACE && h->parity == 1)
+      pops_export_p1_kernel<LAT, real><<<1184, 256, 0, h->stream>>>(pops(h, h->cur), h->L.pstride, out_dev, h->p.nx, h->p.ny, h->p.nz,
+                                                                    K * Q, h->p.bc[0], h->p.bc[2], h->p.bc[4]);
+    else
+      pops_export_kernel<real><<<1184, 256, 0, h->stream>>>(pops(h, h->cur), h->L.pstride, out_dev, h->N, K * Q);
     CUDA_TRY(cudaGetLastError());
     h->launches += 1;
     return LBMHD_OK;
@@ -421,7 +459,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     pops_import_kernel<real><<<1184, 256, 0, h->stream>>>(in_dev, pops(h, h->cur), h->L.pstride, h->N, K * Q);
     CUDA_TRY(cudaGetLastError());
     h->launches += 1;
-    return LBMHD_OK;
+    h->parity = 0;                      // canonical order is layout P0
+    return refresh_published(h);
   }
 };
 
@@ -432,11 +471,12 @@ struct OpTable {
   int (*diag)(lbmhd_t *, const double *, double *);
   int (*pops_export)(lbmhd_t *, double *);
   int (*pops_import)(lbmhd_t *, const double *);
+  int (*refresh_published)(lbmhd_t *);
 };
 
 template <int LAT, int SCHEME, typename real> OpTable make_table() {
   using O = Ops<LAT, SCHEME, real>;
-  return OpTable{O::step, O::init, O::moments, O::diag, O::pops_export, O::pops_import};
+  return OpTable{O::step, O::init, O::moments, O::diag, O::pops_export, O::pops_import, O::refresh_published};
 }
 
 template <int LAT> OpTable pick2(int scheme, int precision) {
@@ -514,6 +554,7 @@ int lbmhd_set_obstacle(lbmhd_t *h, const unsigned char *mask, const double u_sol
   h->have_bsolid = B_solid != nullptr;
   if (B_solid) CUDA_TRY(cudaMemcpyAsync(h->ws + h->L.off_bsolid, B_solid, 3 * h->N * 8, kind, h->stream));
   for (int c = 0; c < 3; c++) h->usolid[c] = u_solid ? u_solid[c] : 0.0;
+  if (int rc = pick(h).refresh_published(h)) return rc;      // in place: newly FROZEN cells keep their current moments
   CUDA_TRY(cudaStreamSynchronize(h->stream));
   return LBMHD_OK;
 }
@@ -536,7 +577,8 @@ static int pops_io(lbmhd_t *h, double *out, const double *in, int on_device) {
   const size_t bytes = (size_t)h->g.K * h->g.Q * h->N * 8;
   if (on_device) return out ? op.pops_export(h, out) : op.pops_import(h, in);
   // host path: stage through the not-current population copy when it is large enough (fp64 A/B), plane by plane otherwise
-  if (h->p.precision != 64) return fail(LBMHD_EINVAL, "host population I/O needs precision 64 (use device pointers for fp32)");
+  if (h->p.precision != 64 || h->p.streaming != LBMHD_STREAM_AB)
+    return fail(LBMHD_EINVAL, "host population I/O needs precision 64 and A/B streaming (use device pointers otherwise)");
   double *stage = (double *)(h->ws + h->L.off_pop[1 - h->cur]);
   if (bytes > h->L.pop_bytes) return fail(LBMHD_ENOMEM, "staging buffer too small");
   if (out) {

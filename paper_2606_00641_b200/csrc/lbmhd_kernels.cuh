@@ -37,6 +37,9 @@ template <typename real> struct StepArgs {
   long long ld_off[19];         // bytes from a cell's own slot in plane (k,0) to its pull source in plane (k,i), no wrap:
                                 //   (i*pstride - (c_x + c_y nx + c_z nx ny)) * sizeof(real)
   long long st_off[19];         // i * pstride * sizeof(real)
+  const double *M_cur;          // in-place modes: post-collision moments [K][N] published last step (and the constant
+                                //   state of frozen cells); nullptr in A/B mode
+  double *M_next;               // in-place modes: moments published by this step
   int has_sphere;
   double sph_c[3], sph_R, sph_R2, sph_m[3], sph_Bs, sph_u[3];
 };
@@ -216,12 +219,69 @@ __device__ __forceinline__ void solid_blend(const real *Qv, real gamma, const do
   }
 }
 
+// ---- streaming layouts -------------------------------------------------------------------
+// ST_AB   two population copies; step reads src, writes dst:            g'_j(x) -> dst (x, slot j)
+// ST_PP   one copy, AA pattern, layout P0 -> P1 ("pull-push"): the cell reads f_i from (x - c_i, slot i), exactly
+//         the A/B pull, and writes g'_j back into the location it read for the opposite direction:
+//         g'_j(x) -> (x + c_j, slot opp(j)); if x + c_j is outside a non-periodic face, -> (x, slot j).
+// ST_LOC  one copy, layout P1 -> P0 (local): f_i(x) is at (x, slot opp(i)); g'_j(x) -> (x, slot j).
+// In both in-place steps a cell only touches locations no other cell touches, so there is no race.
+enum { ST_AB = 0, ST_PP = 1, ST_LOC = 2 };
+
+__host__ __device__ constexpr int opp(int i) { return i == 0 ? 0 : ((i & 1) ? i + 1 : i - 1); }
+
 // per-cell context shared by the load front ends (plain pulls / TMA-staged pulls) and finish_cell
 struct CellCtx {
   int tx, k, x, y, z;
   uint32_t n;                                   // cell index (N < 2^32 is checked at create)
   bool work;                                    // active and not frozen
   bool out_xm, out_xp, out_ym, out_yp, out_zm, out_zp;   // source x - c would be outside a non-periodic face
+  bool writeM;                                  // in-place modes: publish this cell's post-collision moment (see M_next)
+};
+
+// ---- where result j of a cell goes --------------------------------------------------------------------------
+// own slot: A/B (base in the dst copy) and ST_LOC (base in the single copy)
+template <typename real> struct StoreOwn {
+  char *base;                 // address of (k, 0, cell)
+  const long long *st_off;
+  __device__ __forceinline__ void put(int j, real v) const { *reinterpret_cast<real *>(base + st_off[j]) = v; }
+};
+// ST_PP, interior tile: the location read for direction opp(j)
+template <typename real> struct StorePPInterior {
+  char *base;
+  const long long *ld_off;
+  __device__ __forceinline__ void put(int j, real v) const { *reinterpret_cast<real *>(base + ld_off[opp(j)]) = v; }
+};
+// ST_PP, x-edge tile of an interior row: only the thread on the face differs (wrap, or own slot when outside)
+template <class L, typename real> struct StorePPEdge {
+  char *base;
+  const long long *ld_off, *st_off;
+  bool edge_lo, on_face, wrap;
+  long long wrap_adj;
+  __device__ __forceinline__ void put(int j, real v) const {
+    const int i = opp(j);
+    long long off = ld_off[i];
+    if ((L::cx(i) == 1 || L::cx(i) == -1) && on_face && ((edge_lo && L::cx(i) == 1) || (!edge_lo && L::cx(i) == -1)))
+      off = wrap ? off + wrap_adj : st_off[j];
+    *reinterpret_cast<real *>(base + off) = v;
+  }
+};
+// ST_PP, general tile: full index arithmetic with wrap and outside tests
+template <class L, typename real> struct StorePPGeneral {
+  real *basek;                // (k, 0, cell 0)
+  uint32_t ps, n;
+  int x, y, z, nx, ny, nz;
+  bool npx, npy, npz;
+  __device__ __forceinline__ void put(int j, real v) const {
+    const int i = opp(j);
+    int sx = x - L::cx(i), sy = y - L::cy(i), sz = z - L::cz(i);
+    bool outside = false;
+    if (sx < 0) { if (npx) outside = true; else sx += nx; } else if (sx >= nx) { if (npx) outside = true; else sx -= nx; }
+    if (sy < 0) { if (npy) outside = true; else sy += ny; } else if (sy >= ny) { if (npy) outside = true; else sy -= ny; }
+    if (sz < 0) { if (npz) outside = true; else sz += nz; } else if (sz >= nz) { if (npz) outside = true; else sz -= nz; }
+    if (outside) basek[(uint32_t)j * ps + n] = v;
+    else basek[(uint32_t)i * ps + ((uint32_t)sz * ny + sy) * nx + sx] = v;
+  }
 };
 
 // Conservative, tile-uniform test: can the sphere touch cells [x0, x0+tx_cells) of row (y, z)?
@@ -235,24 +295,41 @@ __device__ __forceinline__ bool sphere_may_touch(const StepArgs<real> &a, int x0
   return dx * dx + dy * dy + dz * dz <= a.sph_R2 * (1.0 + 1e-9) + 1e-9;
 }
 
+// frozen cell in the in-place modes (A10): its populations are f^eq of its constant state, kept in M_cur
+template <int LAT, int SCHEME, typename real, class Store>
+__device__ __forceinline__ void frozen_rematerialise(const StepArgs<real> &a, int k, uint32_t n, const Store &store) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, Q = L::Q, K = Vars<SCHEME, D>::K;
+  const size_t N = (size_t)a.nx * a.ny * a.nz;
+  real Qf[K], Phi[3];
+#pragma unroll
+  for (int l = 0; l < K; l++) Qf[l] = (real)a.M_cur[(size_t)l * N + n];
+  flux_row<SCHEME, D, real>(k, Qf, a.gamma, a.c0sq, Phi);
+  const real Qfk = pick<K, real>(Qf, k);
+#pragma unroll
+  for (int j = 0; j < Q; j++) {
+    const real cPhi = real(L::cx(j)) * Phi[0] + real(L::cy(j)) * Phi[1] + real(L::cz(j)) * Phi[2];
+    store.put(j, real(L::w(j)) * (Qfk + real(3) * cPhi));
+  }
+}
+
 // =====================================================================================================
 // Everything after the pull: boundary substitution (A9), moments exchange, div-B estimate, Powell source,
 // solid blend, flux, BGK + direct injection, store (DESIGN.md §2 steps S2-S8; Eq.2-4, 8, 11-14).
 // sQ[K][TX], sTr[D][TX] are shared arrays of the TX*K threads that call this together; `sync` is their
 // barrier (__syncthreads or a named barrier).  BND / SOLID are tile-uniform: the interior fluid tile (both
-// false) is the hot path and carries no boundary predicates, no mask or sphere test.
+// false) is the hot path and carries no boundary predicates, no mask or sphere test.  `store` says where
+// result j goes (streaming layout); STREAM only selects where Q^nb comes from.
 // =====================================================================================================
-template <int LAT, int SCHEME, typename real, int TX, bool BND, bool SOLID, class FArr, class Sync>
-__device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellCtx &c, FArr &f, real (*sQ)[TX],
-                                            real (*sTr)[TX], Sync sync) {
+template <int LAT, int SCHEME, typename real, int TX, bool BND, bool SOLID, int STREAM, class FArr, class Store, class Sync>
+__device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellCtx &c, FArr &f, const Store &store,
+                                            real (*sQ)[TX], real (*sTr)[TX], Sync sync) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
   using V = Vars<SCHEME, D>;
   constexpr int K = V::K, iB = V::iB;
   const int tx = c.tx, k = c.k;
-  const uint32_t ps = (uint32_t)a.pstride;
   const bool work = c.work;
-  const real *__restrict__ srck = a.src + (size_t)k * Q * a.pstride;
 
   if constexpr (BND) {
     // A9 / PAPER.md:154: directions whose source is outside take the equilibrium of the inward neighbour's state
@@ -263,8 +340,14 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
       const int qz = c.out_zm ? c.z + 1 : (c.out_zp ? c.z - 1 : c.z);
       const uint32_t nb = ((uint32_t)qz * a.ny + qy) * a.nx + qx;
       real s = real(0);
+      if (STREAM == ST_AB) {      // stored populations of the neighbour, index order
+        const uint32_t ps = (uint32_t)a.pstride;
+        const real *__restrict__ srck = a.src + (size_t)k * Q * a.pstride;
 #pragma unroll
-      for (int j = 0; j < Q; j++) s += srck[(uint32_t)j * ps + nb];
+        for (int j = 0; j < Q; j++) s += srck[(uint32_t)j * ps + nb];
+      } else {                    // in place the neighbour's slots are in flux: it published its moment last step
+        s = (real)a.M_cur[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + nb];
+      }
       sQ[k][tx] = s;
     }
     sync();
@@ -339,6 +422,8 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
     flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, Phi);
     inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
   }
+  // in place: cells next to a non-periodic face publish their post-collision moment (sum_i g'_i = Q_k + inj)
+  if (STREAM != ST_AB && c.writeM) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + c.n] = (double)(Qk + inj);
 
   // S7 BGK + direct injection, S8 store:
   //   g'_i = (1 - w) f_i + w_i [ w Q_k + inj ] + w_i (c_i . 3 w Phi)       (w = omega_k; Eq.2-3 with c_s^2 = 1/3)
@@ -346,14 +431,13 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   const real omc = real(1) - om;
   const real b0 = om * Qk + inj;
   const real P0 = real(3) * om * Phi[0], P1 = real(3) * om * Phi[1], P2 = real(3) * om * Phi[2];
-  char *__restrict__ dp = reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + c.n));
 #pragma unroll
   for (int i = 0; i < Q; i++) {
     real t = real(L::w(i)) * b0;
     if (L::cx(i) != 0) t = fma(real(L::cx(i) * L::w(i)), P0, t);
     if (L::cy(i) != 0) t = fma(real(L::cy(i) * L::w(i)), P1, t);
     if (L::cz(i) != 0) t = fma(real(L::cz(i) * L::w(i)), P2, t);
-    *reinterpret_cast<real *>(dp + a.st_off[i]) = fma(f[i], omc, t);
+    store.put(i, fma(f[i], omc, t));
   }
 }
 
@@ -362,9 +446,9 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
 // finish_cell with boundary and solid handling compiled in.  Used by every step kernel for the tiles that are
 // not interior; the TX*K threads of the tile call it together.
 // =====================================================================================================
-template <int LAT, int SCHEME, typename real, int TX, class Sync>
+template <int LAT, int SCHEME, typename real, int TX, int STREAM, class Sync>
 __device__ __forceinline__ void general_tile(const StepArgs<real> &a, int tx, int k, int x, int y, int z, real (*sQ)[TX],
-                                          real (*sTr)[TX], Sync sync) {
+                                             real (*sTr)[TX], Sync sync) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
@@ -372,6 +456,7 @@ __device__ __forceinline__ void general_tile(const StepArgs<real> &a, int tx, in
   const uint32_t ps = (uint32_t)a.pstride;
   const uint32_t n = ((uint32_t)z * ny + y) * nx + (active ? x : 0);
   const real *__restrict__ srck = a.src + (size_t)k * Q * a.pstride;
+  real *__restrict__ dstk = a.dst + (size_t)k * Q * a.pstride;       // ST_AB: the other copy; in place: the same copy
   const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
   const bool x_lo = x == 0, x_hi = x == nx - 1;
   const bool y_lo = D > 1 && y == 0, y_hi = D > 1 && y == ny - 1;
@@ -379,7 +464,8 @@ __device__ __forceinline__ void general_tile(const StepArgs<real> &a, int tx, in
   const int xm = x_lo ? nx - 1 : x - 1, xp = x_hi ? 0 : x + 1;
   const int ym = y_lo ? ny - 1 : y - 1, yp = y_hi ? 0 : y + 1;
   const int zm = z_lo ? nz - 1 : z - 1, zp = z_hi ? 0 : z + 1;
-  real f[Q];
+  const StoreOwn<real> own{reinterpret_cast<char *>(dstk + n), a.st_off};
+  const StorePPGeneral<L, real> pp{dstk, ps, n, x, y, z, nx, ny, nz, npx, npy, npz};
 
   // frozen cells keep their populations: mask FROZEN or on an INFLOW face (A10)
   bool frozen = false;
@@ -388,9 +474,14 @@ __device__ __forceinline__ void general_tile(const StepArgs<real> &a, int tx, in
              (x_hi && a.bc[1] == BC_INFLOW) || (y_lo && a.bc[2] == BC_INFLOW) || (y_hi && a.bc[3] == BC_INFLOW) ||
              (z_lo && a.bc[4] == BC_INFLOW) || (z_hi && a.bc[5] == BC_INFLOW);
     if (frozen) {
-      real *__restrict__ dstk = a.dst + (size_t)k * Q * a.pstride;
+      if (STREAM == ST_AB) {
 #pragma unroll
-      for (int i = 0; i < Q; i++) dstk[(uint32_t)i * ps + n] = srck[(uint32_t)i * ps + n];
+        for (int i = 0; i < Q; i++) dstk[(uint32_t)i * ps + n] = srck[(uint32_t)i * ps + n];
+      } else if (STREAM == ST_PP) {
+        frozen_rematerialise<LAT, SCHEME, real>(a, k, n, pp);
+      } else {
+        frozen_rematerialise<LAT, SCHEME, real>(a, k, n, own);
+      }
     }
   }
   const bool work = active && !frozen;
@@ -399,6 +490,7 @@ __device__ __forceinline__ void general_tile(const StepArgs<real> &a, int tx, in
   const bool out_zm = npz && z_lo, out_zp = npz && z_hi;
 
   // S1 pull: f_i(x) = g_i(x - c_i), periodic wrap; sources outside a non-periodic face are filled in finish_cell
+  real f[Q];
 #pragma unroll
   for (int i = 0; i < Q; i++) {
     const int cx = L::cx(i), cy = L::cy(i), cz = L::cz(i);
@@ -407,10 +499,12 @@ __device__ __forceinline__ void general_tile(const StepArgs<real> &a, int tx, in
     const int sz = cz == 1 ? zm : (cz == -1 ? zp : z);
     const bool outside = (cx == 1 && out_xm) || (cx == -1 && out_xp) || (cy == 1 && out_ym) || (cy == -1 && out_yp) ||
                          (cz == 1 && out_zm) || (cz == -1 && out_zp);
-    f[i] = (work && !outside) ? srck[(uint32_t)i * ps + ((uint32_t)sz * ny + sy) * nx + sx] : real(0);
+    const uint32_t at = STREAM == ST_LOC ? (uint32_t)opp(i) * ps + n : (uint32_t)i * ps + ((uint32_t)sz * ny + sy) * nx + sx;
+    f[i] = (work && !outside) ? srck[at] : real(0);
   }
-  CellCtx c{tx, k, x, y, z, n, work, out_xm, out_xp, out_ym, out_yp, out_zm, out_zp};
-  finish_cell<LAT, SCHEME, real, TX, true, true>(a, c, f, sQ, sTr, sync);
+  CellCtx c{tx, k, x, y, z, n, work, out_xm, out_xp, out_ym, out_yp, out_zm, out_zp, true};
+  if (STREAM == ST_PP) finish_cell<LAT, SCHEME, real, TX, true, true, STREAM>(a, c, f, pp, sQ, sTr, sync);
+  else finish_cell<LAT, SCHEME, real, TX, true, true, STREAM>(a, c, f, own, sQ, sTr, sync);
 }
 
 // Which tiles a launch covers: block (bx, by, bz) -> tile (bx0 + bx*bxs, y0 + by*ys, z0 + bz*zs).
@@ -419,15 +513,13 @@ struct Region {
 };
 
 // =====================================================================================================
-// Fused step kernel, A/B buffers, plain coalesced pulls into registers (S1) + finish_cell.
-// MODE 0: one launch over all tiles; interior tiles take the lean path, the others general_tile().
-// MODE 1: interior tiles only (the launch covers bx in [1, tiles_x-2], y in [1, ny-2], z in [1, nz-2]); tiles the
-//         sphere may touch are left to a MODE 2 launch.  No general path is compiled in, so the register
-//         budget is that of the lean path alone.
-// MODE 2: general tiles only, over a Region (x-edge columns, y/z-edge rows, sphere bounding box); with
-//         sphere_only the launch handles exactly the interior-positioned tiles that MODE 1 skipped.
+// Fused step kernel: coalesced pulls into registers (S1) + finish_cell.  STREAM: ST_AB | ST_PP | ST_LOC.
+// MODE 0: one launch over all tiles; interior tiles take the lean path, x-edge tiles of interior rows the lean
+//         edge path, the others general_tile().
+// MODE 1: interior tiles only (no general path compiled in); MODE 2: general tiles only, over a Region.
+//         (split launches: measured slower, kept behind LBMHD_SPLIT=1, A/B only.)
 // =====================================================================================================
-template <int LAT, int SCHEME, typename real, int TX, int MINB, int MODE>
+template <int LAT, int SCHEME, typename real, int TX, int MINB, int MODE, int STREAM>
 __global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
 step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int sphere_only) {
   using L = Lattice<LAT>;
@@ -442,23 +534,37 @@ step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int 
   const int x = x0 + tx, y = r.y0 + (int)blockIdx.y * r.ys, z = r.z0 + (int)blockIdx.z * r.zs;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
   const auto sync = [] { __syncthreads(); };
+  const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
 
   // block-uniform classification.  Interior tile: no face, no wrap in any direction, every thread active, no
   // mask, sphere out of reach -> the lean path: one base pointer per thread plus per-direction byte offsets
   // from the constant bank, no predicates.
-  const bool inner_pos = x0 >= 1 && x0 + TX <= nx - 1 && (D < 2 || (y >= 1 && y <= ny - 2)) && (D < 3 || (z >= 1 && z <= nz - 2));
+  const bool row_inner = (D < 2 || (y >= 1 && y <= ny - 2)) && (D < 3 || (z >= 1 && z <= nz - 2));
+  const bool inner_pos = x0 >= 1 && x0 + TX <= nx - 1 && row_inner;
   const bool touched = sphere_may_touch<real, D>(a, x0, TX, y, z);
   const bool interior = inner_pos && a.mask == nullptr && !touched;
+  // in place: rows next to a non-periodic y/z face publish their moments (Q^nb of the face cells, A9)
+  const bool rowM = STREAM != ST_AB && ((npy && (y == 1 || y == ny - 2)) || (npz && (z == 1 || z == nz - 2)));
   if (MODE == 1 && !interior) return;
   if (MODE == 2 && sphere_only && !(inner_pos && touched)) return;
   if (MODE != 2 && interior) {
     const uint32_t n = ((uint32_t)z * ny + y) * nx + x;
-    const char *__restrict__ pb = reinterpret_cast<const char *>(a.src + ((size_t)k * Q * a.pstride + n));
+    char *__restrict__ pb = reinterpret_cast<char *>(const_cast<real *>(a.src) + ((size_t)k * Q * a.pstride + n));
     real f[Q];
 #pragma unroll
-    for (int i = 0; i < Q; i++) f[i] = *reinterpret_cast<const real *>(pb + a.ld_off[i]);
-    CellCtx c{tx, k, x, y, z, n, true, false, false, false, false, false, false};
-    finish_cell<LAT, SCHEME, real, TX, false, false>(a, c, f, sQ, sTr, sync);
+    for (int i = 0; i < Q; i++) f[i] = *reinterpret_cast<const real *>(pb + (STREAM == ST_LOC ? a.st_off[opp(i)] : a.ld_off[i]));
+    const bool writeM = STREAM != ST_AB && (rowM || (npx && (x == 1 || x == nx - 2)));
+    CellCtx c{tx, k, x, y, z, n, true, false, false, false, false, false, false, writeM};
+    if (STREAM == ST_AB) {
+      const StoreOwn<real> st{reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + n)), a.st_off};
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sQ, sTr, sync);
+    } else if (STREAM == ST_PP) {
+      const StorePPInterior<real> st{pb, a.ld_off};
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sQ, sTr, sync);
+    } else {
+      const StoreOwn<real> st{pb, a.st_off};
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sQ, sTr, sync);
+    }
     return;
   }
   if (MODE == 1) return;
@@ -466,11 +572,10 @@ step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int 
   // x-edge tile of an otherwise interior row (no mask, sphere out of reach, not both ends in one tile): lean
   // loads for every thread; only the thread ON the face differs (A9-A11):
   //   periodic x   its c_x != 0 sources come from the other end of the row (offset +- nx);
-  //   INFLOW face  it is frozen: it re-stores its own populations;
-  //   ZEROGRAD     its outside directions take f^eq of the inward neighbour's state Q^nb = sum_j g_j(x +- 1); the Q
-  //                values g_j(nb) are fetched one per lane together with the pulls and summed by shuffles, so the
-  //                face costs no second memory round trip.
-  const bool row_inner = (D < 2 || (y >= 1 && y <= ny - 2)) && (D < 3 || (z >= 1 && z <= nz - 2));
+  //   INFLOW face  it is frozen: it re-stores its own populations (in place: f^eq of its constant state);
+  //   ZEROGRAD     its outside directions take f^eq of the inward neighbour's state Q^nb.  A/B: the Q values
+  //                g_j(nb) are fetched one per lane together with the pulls and summed by shuffles, so the
+  //                face costs no second memory round trip.  In place: Q^nb was published in M_cur.
   const bool edge_lo = x0 == 0, edge_hi = x0 + TX >= nx;
   if (TX == 32 && row_inner && a.mask == nullptr && !touched && (edge_lo != edge_hi) && nx >= 3) {
     const bool active = x < nx;
@@ -482,23 +587,32 @@ step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int 
     const bool zg = on_face && bcf == BC_ZEROGRAD;
     const bool wrap = on_face && bcf == BC_PERIODIC;
     const long long wrap_adj = (long long)nx * (long long)sizeof(real) * (edge_lo ? 1 : -1);
-    const char *__restrict__ pb = reinterpret_cast<const char *>(a.src + ((size_t)k * Q * a.pstride + n));
+    char *__restrict__ pb = reinterpret_cast<char *>(const_cast<real *>(a.src) + ((size_t)k * Q * a.pstride + n));
     real f[Q];
 #pragma unroll
     for (int i = 0; i < Q; i++) {
-      long long off = frozen ? a.st_off[i] : a.ld_off[i];
-      if ((edge_lo && L::cx(i) == 1) || (!edge_lo && L::cx(i) == -1)) off += wrap ? wrap_adj : 0;   // only these cross the face
+      long long off;
+      if (STREAM == ST_LOC) {
+        off = a.st_off[opp(i)];
+      } else {
+        off = (STREAM == ST_AB && frozen) ? a.st_off[i] : a.ld_off[i];
+        if ((edge_lo && L::cx(i) == 1) || (!edge_lo && L::cx(i) == -1)) off += wrap ? wrap_adj : 0;   // only these cross the face
+      }
       f[i] = *reinterpret_cast<const real *>(pb + off);
     }
     __shared__ real sNb[K];
     const bool tile_zg = bcf == BC_ZEROGRAD;                 // tile-uniform
     if (tile_zg) {
-      // lane j < Q fetches g_{k,j}(nb), nb = the face cell's inward neighbour; butterfly sum -> Q^nb_k in every lane
       const uint32_t nb = ((uint32_t)z * ny + y) * nx + (edge_lo ? 1 : nx - 2);
-      real v = tx < Q ? a.src[(size_t)k * Q * a.pstride + (size_t)tx * a.pstride + nb] : real(0);
+      if (STREAM == ST_AB) {
+        // lane j < Q fetches g_{k,j}(nb); butterfly sum -> Q^nb_k in every lane
+        real v = tx < Q ? a.src[(size_t)k * Q * a.pstride + (size_t)tx * a.pstride + nb] : real(0);
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-      if (tx == 0) sNb[k] = v;
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (tx == 0) sNb[k] = v;
+      } else {
+        if (tx == 0) sNb[k] = (real)a.M_cur[(size_t)k * ((size_t)nx * ny * nz) + nb];
+      }
       __syncthreads();
       if (zg) {
         real Qnb[K], Phi[3];
@@ -515,16 +629,26 @@ step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int 
         }
       }
     }
-    if (frozen) {
-      char *dp = reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + n));
+    CellCtx c{tx, k, x, y, z, n, active && !frozen, false, false, false, false, false, false, true};
+    if (STREAM == ST_AB) {
+      const StoreOwn<real> st{reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + n)), a.st_off};
+      if (frozen) {
 #pragma unroll
-      for (int i = 0; i < Q; i++) *reinterpret_cast<real *>(dp + a.st_off[i]) = f[i];
+        for (int i = 0; i < Q; i++) st.put(i, f[i]);
+      }
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sQ, sTr, sync);
+    } else if (STREAM == ST_PP) {
+      const StorePPEdge<L, real> st{pb, a.ld_off, a.st_off, edge_lo, on_face, wrap, wrap_adj};
+      if (frozen) frozen_rematerialise<LAT, SCHEME, real>(a, k, n, st);
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sQ, sTr, sync);
+    } else {
+      const StoreOwn<real> st{pb, a.st_off};
+      if (frozen) frozen_rematerialise<LAT, SCHEME, real>(a, k, n, st);
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sQ, sTr, sync);
     }
-    CellCtx c{tx, k, x, y, z, n, active && !frozen, false, false, false, false, false, false};
-    finish_cell<LAT, SCHEME, real, TX, false, false>(a, c, f, sQ, sTr, sync);
     return;
   }
-  general_tile<LAT, SCHEME, real, TX>(a, tx, k, x, y, z, sQ, sTr, sync);
+  general_tile<LAT, SCHEME, real, TX, STREAM>(a, tx, k, x, y, z, sQ, sTr, sync);
 }
 
 // ---- S10 init: g_{k,i} = w_i (Q_k + c_i.Phi_k(Q)/c_s^2) (Eq.3) from fp64 fields [K][N] ---------
@@ -568,6 +692,53 @@ moments_kernel(const real *__restrict__ g, size_t pstride, double *__restrict__ 
 #pragma unroll
   for (int i = 0; i < Q; i++) s += gk[(size_t)i * pstride + n];
   out[(size_t)k * N + n] = (double)s;
+}
+
+// ---- in-place layout P1 (after a pull-push step): g_{k,j}(x) lives at (x + c_j, slot opp(j)), or at (x, slot j) when
+// x + c_j is outside a non-periodic face.  Element fetch used by the P1 moments and export kernels. ----------------
+template <class L, typename real>
+__device__ __forceinline__ real p1_fetch(const real *__restrict__ gk, size_t pstride, int j, int x, int y, int z, int nx, int ny,
+                                         int nz, bool npx, bool npy, bool npz) {
+  int sx = x + lat_c<L>(j, 0), sy = y + lat_c<L>(j, 1), sz = z + lat_c<L>(j, 2);
+  bool outside = false;
+  if (sx < 0) { if (npx) outside = true; else sx += nx; } else if (sx >= nx) { if (npx) outside = true; else sx -= nx; }
+  if (sy < 0) { if (npy) outside = true; else sy += ny; } else if (sy >= ny) { if (npy) outside = true; else sy -= ny; }
+  if (sz < 0) { if (npz) outside = true; else sz += nz; } else if (sz >= nz) { if (npz) outside = true; else sz -= nz; }
+  if (outside) return gk[(size_t)j * pstride + ((size_t)z * ny + y) * nx + x];
+  return gk[(size_t)opp(j) * pstride + ((size_t)sz * ny + sy) * nx + sx];
+}
+
+template <int LAT, int SCHEME, typename real, int TX>
+__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K)
+moments_p1_kernel(const real *__restrict__ g, size_t pstride, double *__restrict__ out, int nx, int ny, int nz, int bc0, int bc2, int bc4) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, Q = L::Q;
+  const int k = threadIdx.y;
+  const int x = blockIdx.x * TX + threadIdx.x, y = blockIdx.y, z = blockIdx.z;
+  if (x >= nx) return;
+  const size_t N = (size_t)nx * ny * nz;
+  const size_t n = ((size_t)z * ny + y) * nx + x;
+  const real *gk = g + (size_t)k * Q * pstride;
+  const bool npx = bc0 != BC_PERIODIC, npy = D > 1 && bc2 != BC_PERIODIC, npz = D > 2 && bc4 != BC_PERIODIC;
+  real s = real(0);
+#pragma unroll
+  for (int j = 0; j < Q; j++) s += p1_fetch<L, real>(gk, pstride, j, x, y, z, nx, ny, nz, npx, npy, npz);
+  out[(size_t)k * N + n] = (double)s;
+}
+
+template <int LAT, typename real>
+__global__ void pops_export_p1_kernel(const real *__restrict__ g, size_t pstride, double *__restrict__ out, int nx, int ny, int nz,
+                                      int planes, int bc0, int bc2, int bc4) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, Q = L::Q;
+  const size_t N = (size_t)nx * ny * nz, total = N * (size_t)planes;
+  const bool npx = bc0 != BC_PERIODIC, npy = D > 1 && bc2 != BC_PERIODIC, npz = D > 2 && bc4 != BC_PERIODIC;
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
+    const size_t pl = e / N, n = e - pl * N;
+    const int k = (int)(pl / Q), j = (int)(pl % Q);
+    const int x = (int)(n % nx), y = (int)((n / nx) % ny), z = (int)(n / ((size_t)nx * ny));
+    out[e] = (double)p1_fetch<L, real>(g + (size_t)k * Q * pstride, pstride, j, x, y, z, nx, ny, nz, npx, npy, npz);
+  }
 }
 
 // ---- S9b diagnostics: two-stage deterministic reduction with warp shuffles --------------------------------

@@ -227,12 +227,13 @@ step_kernel_tma(const __grid_constant__ StepArgs<real> a, const __grid_constant_
 #pragma unroll
       for (int i = 0; i < Q; i++) f[i] = real(0);
     }
+    const StoreOwn<real> sto{reinterpret_cast<char *>(dstk + n), a.st_off};
     if (!special) {
-      CellCtx c{tx, k, x, y, z, n, work, false, false, false, false, false, false};
-      finish_cell<LAT, SCHEME, real, TXT, false, false>(a, c, f, sQ, sTr, gsync);
+      CellCtx c{tx, k, x, y, z, n, work, false, false, false, false, false, false, false};
+      finish_cell<LAT, SCHEME, real, TXT, false, false, ST_AB>(a, c, f, sto, sQ, sTr, gsync);
     } else {
-      CellCtx c{tx, k, x, y, z, n, work, npx && x_lo, npx && x_hi, npy && y_lo, npy && y_hi, npz && z_lo, npz && z_hi};
-      finish_cell<LAT, SCHEME, real, TXT, true, true>(a, c, f, sQ, sTr, gsync);
+      CellCtx c{tx, k, x, y, z, n, work, npx && x_lo, npx && x_hi, npy && y_lo, npy && y_hi, npz && z_lo, npz && z_hi, false};
+      finish_cell<LAT, SCHEME, real, TXT, true, true, ST_AB>(a, c, f, sto, sQ, sTr, gsync);
     }
     gsync();      // sQ / sTr are reused by this group's next tile
     s += 2;

@@ -67,7 +67,7 @@ def test_create_validates_before_touching_a_device(lib):
         (mk("IDEAL", "D1Q3", (16, 2)), "ny must be 1"),
         (mk("IDEAL", "D2Q9", (16, 16, 2)), "nz must be 1"),
         (mk("IDEAL", "D2Q9", (16, 16), precision=16), "precision"),
-        (mk("IDEAL", "D2Q9", (16, 16), streaming=1), "not built"),
+        (mk("IDEAL", "D2Q9", (16, 16), streaming=2), "streaming"),
         (mk("IDEAL", "D2Q9", (16, 16), bc=(0, 0, 5, 5, 0, 0)), "boundary"),
     ]
     for p, word in cases:

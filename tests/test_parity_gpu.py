@@ -10,9 +10,9 @@ from test_oracle_pins import admissible_ideal, ideal_fields, incres_fields, zyx
 pytestmark = pytest.mark.gpu
 
 
-def gpu_from_workload(w, precision=64):
+def gpu_from_workload(w, precision=64, streaming=0):
     from paper_2606_00641_b200 import lbmhd
-    return lbmhd.from_workload(w, precision=precision)
+    return lbmhd.from_workload(w, precision=precision, streaming=streaming)
 
 
 def random_workload(scheme, lattice, shape, bc, seed, tau=0.7, sphere=None, gamma=5 / 3):
@@ -28,9 +28,9 @@ def random_workload(scheme, lattice, shape, bc, seed, tau=0.7, sphere=None, gamm
                 tau=tau, powell=1.0, bc=bc, steps=0, fields=F, sphere=sphere)
 
 
-def compare(w, steps, tol=TOL64, mask=None, obstacle=None, precision=64):
+def compare(w, steps, tol=TOL64, mask=None, obstacle=None, precision=64, streaming=0):
     o = oracle_from_workload(w, mask=mask)
-    g = gpu_from_workload(w, precision=precision)
+    g = gpu_from_workload(w, precision=precision, streaming=streaming)
     if obstacle is not None:
         o.set_obstacle(*obstacle)
         g.set_obstacle(*obstacle)
