@@ -59,7 +59,9 @@ typedef struct {
   double tau[8];        /* per variable, > 1/2, order of `scheme`; all magnetic sets must share one value (A7) */
   double powell;        /* kappa: 0 = off, 1 = Eq.12 */
   int    bc[6];         /* xmin, xmax, ymin, ymax, zmin, zmax; periodic must be paired per axis */
-  int    streaming;     /* LBMHD_STREAM_AB (two population copies) | LBMHD_STREAM_INPLACE (one copy) */
+  int    streaming;     /* LBMHD_STREAM_AB (two population copies) | LBMHD_STREAM_INPLACE (one copy, AA pattern:
+                           same results; a FROZEN cell is re-emitted as f^eq of its moments, which is what it holds
+                           after lbmhd_init; host-pointer population I/O needs LBMHD_STREAM_AB) */
   int    device;        /* CUDA device ordinal */
   void  *stream;        /* cudaStream_t to enqueue on (0 = default stream) */
   void  *workspace;     /* DEVICE pointer, 256-byte aligned, >= lbmhd_workspace_bytes() bytes */
