@@ -146,7 +146,7 @@ def run_native(args, rank, world, local_rank):
     w = W.get(args.workload)
     N = int(np.prod(w["shape"]))
     prec = args.precision
-    sim = lbmhd.from_workload(w, precision=prec, device=local_rank)
+    sim = lbmhd.from_workload(w, precision=prec, device=local_rank, streaming=1 if args.streaming == "inplace" else 0)
     K, Q = sim.K, sim.Q
     bytes_per_cell = 2 * K * Q * (8 if prec == 64 else 4) + (0 if w.get("sphere") else 0)
     st = sim.stream
@@ -205,7 +205,7 @@ def run_native(args, rank, world, local_rank):
     e2e_val = aggregate_mlups(N, args.steps, ms_e2e, world)
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.csv")      # dram__bytes_read/write.sum of one ncu --set full capture
-    if os.path.exists(tpath) and prec == 64:
+    if os.path.exists(tpath) and prec == 64 and args.streaming == "ab":
         with open(tpath) as f:
             for row in f.read().splitlines()[1:]:
                 cols = row.split(",")
@@ -218,8 +218,10 @@ def run_native(args, rank, world, local_rank):
         "config": {"workload": "%s: %s %s x %d sets, %s, %s, %d B/cell/step; replicas per GPU, no collective" % (
                        w["name"], w["scheme"], w["lattice"], K, "x".join(str(s) for s in w["shape"]),
                        "fp64" if prec == 64 else "fp32", bytes_per_cell),
-                   "cells": N, "streaming": "A/B double buffer",
-                   "l2": "working set %.1f GB >> 126 MB L2, no flush needed" % (2 * N * bytes_per_cell / 2 / 1e9)},
+                   "cells": N, "streaming": "in-place AA pattern, one copy" if args.streaming == "inplace" else "A/B double buffer",
+                   "workspace_GB": round(sim.workspace.numel() / 1e9, 2),
+                   "l2": "populations %.1f GB >> 126 MB L2, no flush needed" % (
+                       (1 if args.streaming == "inplace" else 2) * N * bytes_per_cell / 2 / 1e9)},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "peak_source": peak_src, "kernel": "step_kernel",
                      "frac_of_nominal_8TBs": achieved / 8000.0,
@@ -245,6 +247,7 @@ def main():
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
+    ap.add_argument("--streaming", default="ab", choices=["ab", "inplace"])
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -8,7 +8,7 @@ SRC = os.path.join(_HERE, "csrc", "lbmhd_api.cu")
 DEPS = [SRC, os.path.join(_HERE, "csrc", "lbmhd_kernels.cuh"), os.path.join(_HERE, "csrc", "lbmhd_lattice.cuh"),
         os.path.join(_HERE, "csrc", "lbmhd_tma.cuh"),
         os.path.join(os.path.dirname(_HERE), "include", "lbmhd.h")]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--split-compile", "0",
               "-shared", "-Xcompiler", "-fPIC"]
 
 

@@ -270,15 +270,25 @@ template <int LAT, int SCHEME, typename real> struct Ops {
 
   // One launch over all tiles (small grids, masked obstacles), or the split form: a lean interior launch plus
   // general launches over the x-edge columns, the y/z-edge rows and the sphere's bounding box.
+  // in place: pull-push step from layout P0, local step from layout P1
+  template <int MINB> static cudaError_t launch_step_inplace(lbmhd_t *h, const StepArgs<real> &a) {
+    constexpr int TX = 32;
+    const dim3 g((h->p.nx + TX - 1) / TX, h->p.ny, h->p.nz), b(TX, K);
+    if (h->parity == 0) step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_PP><<<g, b, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
+    else step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_LOC><<<g, b, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
+    h->launches += 1;
+    return cudaGetLastError();
+  }
+
+  template <int TX, int MINB> static cudaError_t launch_step_whole(lbmhd_t *h, const StepArgs<real> &a) {
+    step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_AB><<<dim3((h->p.nx + TX - 1) / TX, h->p.ny, h->p.nz), dim3(TX, K), 0, h->stream>>>(
+        a, Region{0, 1, 0, 1, 0, 1}, 0);
+    h->launches += 1;
+    return cudaGetLastError();
+  }
+
   template <int TX, int MINB> static cudaError_t launch_step(lbmhd_t *h, const StepArgs<real> &a) {
     constexpr int D = L::D;
-    if (h->p.streaming == LBMHD_STREAM_INPLACE) {
-      const dim3 g((h->p.nx + TX - 1) / TX, h->p.ny, h->p.nz), b(TX, K);
-      if (h->parity == 0) step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_PP><<<g, b, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
-      else step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_LOC><<<g, b, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
-      h->launches += 1;
-      return cudaGetLastError();
-    }
     const int nx = h->p.nx, ny = h->p.ny, nz = h->p.nz;
     const int tiles_x = (nx + TX - 1) / TX;
     const dim3 block(TX, K);
@@ -381,16 +391,14 @@ template <int LAT, int SCHEME, typename real> struct Ops {
         }
       }
       cudaError_t e;
-      if (inplace) e = h->minb == 4 ? launch_step<32, 4>(h, a) : launch_step<32, 3>(h, a);
+      if (inplace) e = h->minb == 4 ? launch_step_inplace<4>(h, a) : launch_step_inplace<3>(h, a);
       else if (h->use_tma) e = launch_step_tma(h, a);
       else switch (h->tx * 10 + h->minb) {
-        case 321: e = launch_step<32, 1>(h, a); break;
-        case 322: e = launch_step<32, 2>(h, a); break;
-        case 323: e = launch_step<32, 3>(h, a); break;
+        case 322: e = launch_step_whole<32, 2>(h, a); break;
+        case 323: e = launch_step<32, 3>(h, a); break;          // split launches exist for the two default bounds only
         case 324: e = launch_step<32, 4>(h, a); break;
-        case 641: e = launch_step<64, 1>(h, a); break;
-        case 642: e = launch_step<64, 2>(h, a); break;
-        case 1281: e = launch_step<128, 1>(h, a); break;
+        case 642: e = launch_step_whole<64, 2>(h, a); break;
+        case 1281: e = launch_step_whole<128, 1>(h, a); break;
         default: e = launch_step<32, 3>(h, a); break;
       }
       if (e != cudaSuccess) return fail(LBMHD_ECUDA, "step kernel launch: %s", cudaGetErrorString(e));
