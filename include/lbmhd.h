@@ -35,7 +35,8 @@ extern "C" {
 
 typedef struct lbmhd lbmhd_t;
 
-enum { LBMHD_D1Q3 = 1, LBMHD_D2Q9 = 2, LBMHD_D3Q19 = 3 };
+enum { LBMHD_D1Q3 = 1, LBMHD_D2Q9 = 2, LBMHD_D3Q19 = 3,
+       LBMHD_D2Q5 = 4, LBMHD_D3Q7 = 5 /* the paper's own lattices; D3Q7 has c_s^2 = 1/4 */ };
 enum { LBMHD_IDEAL = 0, LBMHD_INCRES = 1 };
 enum { LBMHD_BC_PERIODIC = 0, LBMHD_BC_ZEROGRAD = 1, LBMHD_BC_INFLOW = 2 };
 enum { LBMHD_CELL_FLUID = 0, LBMHD_CELL_FROZEN = 1, LBMHD_CELL_SOLID = 2 };
@@ -50,7 +51,7 @@ enum {
 
 typedef struct {
   int    scheme;        /* LBMHD_IDEAL | LBMHD_INCRES */
-  int    lattice;       /* LBMHD_D1Q3 | LBMHD_D2Q9 | LBMHD_D3Q19 */
+  int    lattice;       /* LBMHD_D1Q3 | LBMHD_D2Q9 | LBMHD_D3Q19 | LBMHD_D2Q5 | LBMHD_D3Q7 */
   int    precision;     /* 64 (fp64 populations and arithmetic) or 32 (fp32 populations and arithmetic) */
   int    nx, ny, nz;    /* unused dims = 1 */
   double gamma;         /* IDEAL: adiabatic index, Eq.8 */

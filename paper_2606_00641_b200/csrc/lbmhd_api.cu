@@ -39,14 +39,18 @@ int fail(int code, const char *fmt, ...) {
 
 struct Geometry {
   int D, Q, K, NV, iU, iB;
+  double cs2;
 };
 
 bool geometry(int scheme, int lattice, Geometry *g) {
   if (scheme != LBMHD_IDEAL && scheme != LBMHD_INCRES) return false;
+  g->cs2 = 1.0 / 3.0;
   switch (lattice) {
     case LBMHD_D1Q3: g->D = 1; g->Q = 3; break;
     case LBMHD_D2Q9: g->D = 2; g->Q = 9; break;
     case LBMHD_D3Q19: g->D = 3; g->Q = 19; break;
+    case LBMHD_D2Q5: g->D = 2; g->Q = 5; break;
+    case LBMHD_D3Q7: g->D = 3; g->Q = 7; g->cs2 = 0.25; break;
     default: return false;
   }
   g->K = scheme == LBMHD_IDEAL ? 8 : 1 + 2 * g->D;
@@ -201,7 +205,7 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
   h->p = *p; h->g = g; h->L = L;
   h->N = (size_t)p->nx * p->ny * p->nz;
   for (int k = 0; k < g.K; k++) h->tau[k] = p->tau[k];
-  const double cs2 = 1.0 / 3.0;
+  const double cs2 = g.cs2;
   if (p->nu > 0.0) {    // Eq.5
     for (int b = 0; b < g.NV; b++) h->tau[g.iU + b] = 0.5 + p->nu / cs2;
     if (p->scheme == LBMHD_INCRES) h->tau[0] = 0.5 + p->nu / cs2;
@@ -354,7 +358,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     a.nx = h->p.nx; a.ny = h->p.ny; a.nz = h->p.nz;
     for (int j = 0; j < 6; j++) a.bc[j] = h->p.bc[j];
     for (int k = 0; k < K; k++) a.omega[k] = (real)(1.0 / h->tau[k]);
-    a.inv_tauB_cs2 = (real)(1.0 / (h->tau[h->g.iB] * (1.0 / 3.0)));
+    a.inv_tauB_cs2 = (real)(1.0 / (h->tau[h->g.iB] * h->g.cs2));
     a.kappa = (real)h->p.powell; a.gamma = (real)h->p.gamma; a.c0sq = (real)h->p.c0sq;
     a.mask = h->have_mask ? (const unsigned char *)(h->ws + h->L.off_mask) : nullptr;
     a.Bsolid = h->have_bsolid ? (const double *)(h->ws + h->L.off_bsolid) : nullptr;
@@ -496,6 +500,8 @@ OpTable pick(const lbmhd_t *h) {
   switch (h->p.lattice) {
     case LBMHD_D1Q3: return pick2<1>(h->p.scheme, h->p.precision);
     case LBMHD_D2Q9: return pick2<2>(h->p.scheme, h->p.precision);
+    case LBMHD_D2Q5: return pick2<4>(h->p.scheme, h->p.precision);
+    case LBMHD_D3Q7: return pick2<5>(h->p.scheme, h->p.precision);
     default: return pick2<3>(h->p.scheme, h->p.precision);
   }
 }

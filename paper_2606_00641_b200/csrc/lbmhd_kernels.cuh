@@ -309,7 +309,7 @@ __device__ __forceinline__ void frozen_rematerialise(const StepArgs<real> &a, in
 #pragma unroll
   for (int j = 0; j < Q; j++) {
     const real cPhi = real(L::cx(j)) * Phi[0] + real(L::cy(j)) * Phi[1] + real(L::cz(j)) * Phi[2];
-    store.put(j, real(L::w(j)) * (Qfk + real(3) * cPhi));
+    store.put(j, real(L::w(j)) * (Qfk + real(L::inv_cs2) * cPhi));
   }
 }
 
@@ -363,7 +363,7 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
         const bool outside = (cx == 1 && c.out_xm) || (cx == -1 && c.out_xp) || (cy == 1 && c.out_ym) ||
                              (cy == -1 && c.out_yp) || (cz == 1 && c.out_zm) || (cz == -1 && c.out_zp);
         const real cPhi = real(cx) * Phi[0] + real(cy) * Phi[1] + real(cz) * Phi[2];
-        if (outside) f[i] = real(L::w(i)) * (Qnbk + real(3) * cPhi);
+        if (outside) f[i] = real(L::w(i)) * (Qnbk + real(L::inv_cs2) * cPhi);
       }
     }
     sync();
@@ -426,11 +426,11 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   if (STREAM != ST_AB && c.writeM) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + c.n] = (double)(Qk + inj);
 
   // S7 BGK + direct injection, S8 store:
-  //   g'_i = (1 - w) f_i + w_i [ w Q_k + inj ] + w_i (c_i . 3 w Phi)       (w = omega_k; Eq.2-3 with c_s^2 = 1/3)
+  //   g'_i = (1 - w) f_i + w_i [ w Q_k + inj ] + w_i (c_i . 3 w Phi)       (w = omega_k; Eq.2-3, 3 = 1/c_s^2)
   const real om = a.omega[k];
   const real omc = real(1) - om;
   const real b0 = om * Qk + inj;
-  const real P0 = real(3) * om * Phi[0], P1 = real(3) * om * Phi[1], P2 = real(3) * om * Phi[2];
+  const real P0 = real(L::inv_cs2) * om * Phi[0], P1 = real(L::inv_cs2) * om * Phi[1], P2 = real(L::inv_cs2) * om * Phi[2];
 #pragma unroll
   for (int i = 0; i < Q; i++) {
     real t = real(L::w(i)) * b0;
@@ -624,7 +624,7 @@ step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int 
         for (int i = 0; i < Q; i++) {
           if ((edge_lo && L::cx(i) == 1) || (!edge_lo && L::cx(i) == -1)) {
             const real cPhi = real(L::cx(i)) * Phi[0] + real(L::cy(i)) * Phi[1] + real(L::cz(i)) * Phi[2];
-            f[i] = real(L::w(i)) * (Qnbk + real(3) * cPhi);
+            f[i] = real(L::w(i)) * (Qnbk + real(L::inv_cs2) * cPhi);
           }
         }
       }
@@ -672,7 +672,7 @@ init_kernel(const double *__restrict__ fields, real *__restrict__ g, size_t pstr
 #pragma unroll
   for (int i = 0; i < Q; i++) {
     const real cPhi = real(L::cx(i)) * Phi[0] + real(L::cy(i)) * Phi[1] + real(L::cz(i)) * Phi[2];
-    gk[(size_t)i * pstride + n] = real(L::w(i)) * (Qk + real(3) * cPhi);
+    gk[(size_t)i * pstride + n] = real(L::w(i)) * (Qk + real(L::inv_cs2) * cPhi);
   }
 }
 
@@ -819,7 +819,7 @@ diag_partial_kernel(const double *__restrict__ F, double *__restrict__ partial, 
         if (lat_c<L>(i, c) != 0) cB += (double)lat_c<L>(i, c) * F[(size_t)(iB + c) * N + nq];
       div += L::w(i) * cB;
     }
-    div *= 3.0;
+    div *= L::inv_cs2;
     maxdiv = fmax(maxdiv, fabs(div));
     if (SCHEME == kIdeal) {
       const double rho = v[0];

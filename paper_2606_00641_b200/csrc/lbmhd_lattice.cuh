@@ -11,6 +11,7 @@ template <int LAT> struct Lattice;
 
 template <> struct Lattice<1> {   // D1Q3
   static constexpr int D = 1, Q = 3;
+  static constexpr double inv_cs2 = 3.0;
   __host__ __device__ static constexpr int cx(int i) { return i == 1 ? 1 : (i == 2 ? -1 : 0); }
   __host__ __device__ static constexpr int cy(int) { return 0; }
   __host__ __device__ static constexpr int cz(int) { return 0; }
@@ -19,6 +20,7 @@ template <> struct Lattice<1> {   // D1Q3
 
 template <> struct Lattice<2> {   // D2Q9
   static constexpr int D = 2, Q = 9;
+  static constexpr double inv_cs2 = 3.0;
   __host__ __device__ static constexpr int cx(int i) {
     constexpr int t[9] = {0, 1, -1, 0, 0, 1, -1, 1, -1};
     return t[i];
@@ -33,6 +35,7 @@ template <> struct Lattice<2> {   // D2Q9
 
 template <> struct Lattice<3> {   // D3Q19
   static constexpr int D = 3, Q = 19;
+  static constexpr double inv_cs2 = 3.0;
   __host__ __device__ static constexpr int cx(int i) {
     constexpr int t[19] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
     return t[i];
@@ -46,6 +49,27 @@ template <> struct Lattice<3> {   // D3Q19
     return t[i];
   }
   __host__ __device__ static constexpr double w(int i) { return i == 0 ? 1.0 / 3.0 : (i < 7 ? 1.0 / 18.0 : 1.0 / 36.0); }
+};
+
+// The paper's own lattices (PAPER.md:183 D2Q5 in all validation cases, :300 D3Q7 in the showcase): axis directions only.
+// Rest weight and c_s^2 follow from sum_i w_i = 1 and sum_i w_i c_ia c_ib = c_s^2 delta_ab with the textbook choice
+// c_s^2 = 1/3 (D2Q5: w = 1/3, 1/6) resp. c_s^2 = 1/4 (D3Q7: w = 1/4, 1/8).
+template <> struct Lattice<4> {   // D2Q5
+  static constexpr int D = 2, Q = 5;
+  static constexpr double inv_cs2 = 3.0;
+  __host__ __device__ static constexpr int cx(int i) { return i == 1 ? 1 : (i == 2 ? -1 : 0); }
+  __host__ __device__ static constexpr int cy(int i) { return i == 3 ? 1 : (i == 4 ? -1 : 0); }
+  __host__ __device__ static constexpr int cz(int) { return 0; }
+  __host__ __device__ static constexpr double w(int i) { return i == 0 ? 1.0 / 3.0 : 1.0 / 6.0; }
+};
+
+template <> struct Lattice<5> {   // D3Q7
+  static constexpr int D = 3, Q = 7;
+  static constexpr double inv_cs2 = 4.0;
+  __host__ __device__ static constexpr int cx(int i) { return i == 1 ? 1 : (i == 2 ? -1 : 0); }
+  __host__ __device__ static constexpr int cy(int i) { return i == 3 ? 1 : (i == 4 ? -1 : 0); }
+  __host__ __device__ static constexpr int cz(int i) { return i == 5 ? 1 : (i == 6 ? -1 : 0); }
+  __host__ __device__ static constexpr double w(int i) { return i == 0 ? 1.0 / 4.0 : 1.0 / 8.0; }
 };
 
 template <class L> __host__ __device__ constexpr int lat_c(int i, int axis) {

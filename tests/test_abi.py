@@ -32,7 +32,8 @@ def test_exports_every_declared_symbol(lib):
 def test_geometry_and_workspace_arithmetic(lib):
     for scheme, lat, shape, K, Q in [("IDEAL", "D1Q3", (800,), 8, 3), ("INCRES", "D2Q9", (512, 512), 5, 9),
                                      ("IDEAL", "D2Q9", (1024, 1024), 8, 9), ("IDEAL", "D3Q19", (384, 256, 256), 8, 19),
-                                     ("INCRES", "D3Q19", (10, 10, 10), 7, 19), ("INCRES", "D1Q3", (10,), 3, 3)]:
+                                     ("INCRES", "D3Q19", (10, 10, 10), 7, 19), ("INCRES", "D1Q3", (10,), 3, 3),
+                                     ("IDEAL", "D2Q5", (64, 64), 8, 5), ("INCRES", "D3Q7", (10, 10, 10), 7, 7)]:
         p = lbmhd.make_params(scheme, lat, shape)
         assert lib.lbmhd_num_vars(C.byref(p)) == K and lib.lbmhd_num_dirs(C.byref(p)) == Q
         N = int(np.prod(shape))

@@ -19,11 +19,12 @@ def random_workload(scheme, lattice, shape, bc, seed, tau=0.7, sphere=None, gamm
     rng = np.random.default_rng(seed)
     s = zyx(shape)
     D = len(shape)
+    slow = lattice in ("D2Q5", "D3Q7")        # axis-only lattices: lower speed limit (A16)
     if scheme == "IDEAL":
-        rho, u, B, p = admissible_ideal(rng, s)
-        F = ideal_fields(rho, u, B, p, gamma)
+        rho, u, B, p = admissible_ideal(rng, s, amp=0.06 if slow else 0.2)
+        F = ideal_fields(rho, u, B, p * (0.1 if slow else 1.0), gamma)
     else:
-        F = incres_fields(rng, D, s)
+        F = incres_fields(rng, D, s, amp=0.02 if slow else 0.05)
     return dict(name="rand", scheme=scheme, lattice=lattice, shape=shape, gamma=gamma, c0sq=1 / 36, nu=0.0, eta=0.0,
                 tau=tau, powell=1.0, bc=bc, steps=0, fields=F, sphere=sphere)
 
@@ -69,6 +70,12 @@ CASES = [
     ("IDEAL", "D3Q19", (100, 12, 9), (2, 1, 0, 0, 0, 0)),
     ("IDEAL", "D3Q19", (45, 11, 10), (1, 1, 1, 1, 1, 1)),
     ("INCRES", "D3Q19", (70, 9, 8), (1, 1, 0, 0, 2, 1)),
+    ("IDEAL", "D2Q5", (150, 37), (0,) * 6),
+    ("IDEAL", "D2Q5", (67, 20), (2, 1, 1, 1, 0, 0)),
+    ("INCRES", "D2Q5", (90, 21), (1, 1, 0, 0, 0, 0)),
+    ("IDEAL", "D3Q7", (100, 12, 9), (0,) * 6),
+    ("IDEAL", "D3Q7", (100, 12, 9), (2, 1, 1, 1, 0, 0)),
+    ("INCRES", "D3Q7", (45, 11, 10), (1, 1, 1, 1, 1, 1)),
 ]
 
 
