@@ -55,6 +55,8 @@ def _load():
         lib.oracle_moments.argtypes = [C.c_void_p, dp, dp]
         lib.oracle_set_obstacle.argtypes = [C.c_void_p, up, dp, dp]
         lib.oracle_set_sphere.argtypes = [C.c_void_p, dp, C.c_double, dp, dp, C.c_double]
+        lib.oracle_set_porosity.argtypes = [C.c_void_p, dp]
+        lib.oracle_set_sphere_width.argtypes = [C.c_void_p, C.c_double]
         lib.oracle_get_populations.argtypes = [C.c_void_p, dp]
         lib.oracle_set_populations.argtypes = [C.c_void_p, dp]
         lib.oracle_source_log.argtypes = [C.c_void_p, dp]
@@ -190,6 +192,15 @@ class Oracle:
         c, u, m = _f64(centre), _f64(u_solid), _f64(dipole_dir)
         if self.lib.oracle_set_sphere(self.h, _dptr(c), float(radius), _dptr(u), _dptr(m), float(B_surface)):
             raise RuntimeError("oracle_set_sphere")
+
+    def set_porosity(self, d_field):
+        d = None if d_field is None else _f64(d_field).reshape(-1)
+        if self.lib.oracle_set_porosity(self.h, None if d is None else _dptr(d)):
+            raise RuntimeError("oracle_set_porosity")
+
+    def set_sphere_width(self, eps):
+        if self.lib.oracle_set_sphere_width(self.h, float(eps)):
+            raise RuntimeError("oracle_set_sphere_width")
 
     def populations(self):
         g = np.zeros((self.K, self.Q) + self.shape)

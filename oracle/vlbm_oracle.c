@@ -203,6 +203,8 @@ struct oracle {
   int has_sphere;
   double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs;
   long sph_t0;         /* step count at which the centre was sph_c0 */
+  double sph_eps;      /* width eps_h of the linear porosity ramp across the sphere surface (Eq.15-16), 0 = sharp */
+  double *dfield;      /* lattice porosity d in [0,1] per cell (Eq.15), or NULL: d from the mask (SOLID -> 0) */
   long t;              /* steps done so far */
   double srclog[MAXK];
 };
@@ -265,7 +267,7 @@ int oracle_create(const oracle_params *p, const unsigned char *cell_mask, oracle
 void oracle_destroy(oracle_t *o)
 {
   if (!o) return;
-  free(o->g[0]); free(o->g[1]); free(o->mask); free(o->Bsolid); free(o);
+  free(o->g[0]); free(o->g[1]); free(o->mask); free(o->Bsolid); free(o->dfield); free(o);
 }
 
 int oracle_set_obstacle(oracle_t *o, const unsigned char *mask, const double u_solid[3], const double *B_solid)
@@ -292,6 +294,25 @@ int oracle_set_sphere(oracle_t *o, const double centre[3], double radius, const 
     o->sph_u[a] = u_solid[a]; o->sph_m[a] = dipole_dir[a];
   }
   o->sph_R = radius; o->sph_Bs = B_surface; o->sph_t0 = o->t;
+  return 0;
+}
+
+int oracle_set_porosity(oracle_t *o, const double *d_field)
+{
+  if (!o) return -1;
+  free(o->dfield); o->dfield = NULL;
+  if (d_field) {
+    o->dfield = (double *)malloc((size_t)o->N * sizeof(double));
+    if (!o->dfield) return -2;
+    for (long n = 0; n < o->N; n++) { if (!(d_field[n] >= 0.0 && d_field[n] <= 1.0)) return -1; o->dfield[n] = d_field[n]; }
+  }
+  return 0;
+}
+
+int oracle_set_sphere_width(oracle_t *o, double eps)
+{
+  if (!o || !(eps >= 0.0)) return -1;
+  o->sph_eps = eps;
   return 0;
 }
 
@@ -333,11 +354,14 @@ int oracle_source_log(oracle_t *o, double *acc)
   return 0;
 }
 
-/* ---- solid state at a cell (A8, A11, A12) ----
- * returns porosity d in {0,1}; fills uB[3], BB[3] when d < 1.
- * Sphere: SOLID iff |x - c(t)|^2 <= R^2 with x the integer cell coordinates and
- * c(t) = c0 + (t - t0) u^B; dipole B^B(r) = 1/2 B_s (R / max(|r|, R/2))^3 [3 (m.r^) r^ - m],
- * r^ = r/|r| (0 at r = 0). */
+/* ---- solid state at a cell (A8, A11, A12; Eq.15-16) ----
+ * returns the lattice porosity d in [0,1]; fills uB[3], BB[3] when d < 1.
+ * Sphere, c(t) = c0 + (t - t0) u^B, x the integer cell coordinates:
+ *   sharp (eps = 0): d = 0 iff |x - c|^2 <= R^2;
+ *   ramp  (eps > 0): d = clamp(phi/eps + 1/2, 0, 1), phi = |x - c| - R the signed distance (Eq.15 with the linear
+ *                    profile Eq.16; eps_b read as eps_h, A14).
+ * dipole B^B(r) = 1/2 B_s (R / max(|r|, R/2))^3 [3 (m.r^) r^ - m], r^ = r/|r| (0 at r = 0).
+ * Mask / porosity field: d = dfield[n] if given, else 0 for SOLID cells; u^B uniform, B^B per cell. */
 static double solid_state(const oracle_t *o, int x, int y, int z, long n, double uB[3], double BB[3])
 {
   if (o->has_sphere) {
@@ -349,22 +373,32 @@ static double solid_state(const oracle_t *o, int x, int y, int z, long n, double
       r[a] = a < o->L.D ? xi[a] - c : 0.0;
       r2 = r2 + r[a] * r[a];
     }
-    if (r2 <= o->sph_R * o->sph_R) {
-      double rn = sqrt(r2);
+    double rn = sqrt(r2);
+    double d;
+    if (o->sph_eps > 0.0) {
+      d = (rn - o->sph_R) / o->sph_eps + 0.5;
+      if (d < 0.0) d = 0.0;
+      if (d > 1.0) d = 1.0;
+    } else {
+      d = r2 <= o->sph_R * o->sph_R ? 0.0 : 1.0;
+    }
+    if (d < 1.0) {
       double rc = rn > 0.5 * o->sph_R ? rn : 0.5 * o->sph_R;
       double q = o->sph_R / rc;
       double amp = 0.5 * o->sph_Bs * (q * q * q);
       double rh[3], mr = 0.0;
       for (int a = 0; a < 3; a++) { rh[a] = rn > 0.0 ? r[a] / rn : 0.0; mr += o->sph_m[a] * rh[a]; }
       for (int a = 0; a < 3; a++) { BB[a] = amp * (3.0 * mr * rh[a] - o->sph_m[a]); uB[a] = o->sph_u[a]; }
-      return 0.0;
+      return d;
     }
   }
-  if (o->mask[n] == ORC_CELL_SOLID) {
+  double d = 1.0;
+  if (o->dfield) d = o->dfield[n];
+  else if (o->mask[n] == ORC_CELL_SOLID) d = 0.0;
+  if (d < 1.0) {
     for (int a = 0; a < 3; a++) { uB[a] = o->usolid[a]; BB[a] = o->Bsolid ? o->Bsolid[(long)a * o->N + n] : 0.0; }
-    return 0.0;
   }
-  return 1.0;
+  return d;
 }
 
 /* ---- one cell of one step ---- */

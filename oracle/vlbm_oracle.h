@@ -56,6 +56,11 @@ int  oracle_set_obstacle(oracle_t *o, const unsigned char *mask /* [N] */, const
 int  oracle_set_sphere(oracle_t *o, const double centre[3], double radius, const double u_solid[3],
                        const double dipole_dir[3], double B_surface);
 
+/* fractional porosity (Eq.15-16): per-cell d in [0,1] for the masked solid (NULL = back to the mask),
+ * linear ramp of width eps across the sphere surface (0 = sharp) */
+int  oracle_set_porosity(oracle_t *o, const double *d_field /* [N] or NULL */);
+int  oracle_set_sphere_width(oracle_t *o, double eps);
+
 /* test hooks */
 int  oracle_get_populations(oracle_t *o, double *g_out /* [K][Q][N] */);
 int  oracle_set_populations(oracle_t *o, const double *g_in /* [K][Q][N] */);

@@ -94,6 +94,8 @@ class NpVLBM:
         self.u_solid = np.zeros(3)
         self.B_solid = None
         self.sphere = None
+        self.sphere_eps = 0.0
+        self.d_field = None
         self.t = 0
         self.src_acc = np.zeros(self.K)
         zz, yy, xx = np.meshgrid(*[np.arange(n) for n in self.shape], indexing="ij")
@@ -141,9 +143,12 @@ class NpVLBM:
         d = np.ones(self.shape)
         uB = np.zeros((3,) + self.shape)
         BB = np.zeros((3,) + self.shape)
-        sol = self.mask == SOLID
+        if self.d_field is not None:
+            d = np.asarray(self.d_field, dtype=float).reshape(self.shape).copy()
+        else:
+            d[self.mask == SOLID] = 0.0
+        sol = d < 1.0
         if sol.any():
-            d[sol] = 0.0
             for a in range(3):
                 uB[a][sol] = self.u_solid[a]
                 if self.B_solid is not None:
@@ -155,14 +160,18 @@ class NpVLBM:
             for a in range(self.D):
                 r[a] = self.coord[a] - cen[a]
             r2 = (r * r).sum(0)
-            ins = r2 <= R * R
             rn = np.sqrt(r2)
+            if self.sphere_eps > 0:
+                ds = np.clip((rn - R) / self.sphere_eps + 0.5, 0.0, 1.0)
+            else:
+                ds = np.where(r2 <= R * R, 0.0, 1.0)
+            ins = ds < 1.0
             rc = np.maximum(rn, 0.5 * R)
             with np.errstate(invalid="ignore", divide="ignore"):
                 rh = np.where(rn > 0, r / np.where(rn > 0, rn, 1.0), 0.0)
             mr = (mh.reshape(3, 1, 1, 1) * rh).sum(0)
             dip = 0.5 * Bs * (R / rc) ** 3 * (3.0 * mr * rh - mh.reshape(3, 1, 1, 1))
-            d[ins] = 0.0
+            d[ins] = ds[ins]
             for a in range(3):
                 uB[a][ins] = us[a]
                 BB[a][ins] = dip[a][ins]

@@ -247,3 +247,92 @@ class _at:
     def __init__(self, n, t):
         self.__dict__.update(n.__dict__)
         self.t = t
+
+
+# ---------------------------------------------------------------- fractional porosity (Eq.13-16, NEXT-3)
+@pytest.mark.parametrize("lat,scheme", [("D2Q9", "IDEAL"), ("D3Q19", "IDEAL"), ("D2Q9", "INCRES"), ("D3Q7", "IDEAL")])
+def test_P6_numpy_bruteforce_fractional_porosity(lat, scheme):
+    rng = np.random.default_rng(404)
+    shape = (7, 6) if lattice_np(lat)[0] == 2 else (7, 6, 5)
+    s = zyx(shape)
+    o, n = make_pair(scheme, lat, shape, 0.8, bc=(1, 1) + (0,) * 4)
+    d = np.clip(1.6 * rng.random(s) - 0.3, 0.0, 1.0)          # zeros, ones and everything between
+    us = np.array([0.03, -0.02, 0.01])
+    Bs = 0.1 * (rng.random((3,) + s) - 0.5)
+    o.set_obstacle(np.zeros(s, dtype=np.uint8), us, Bs)
+    o.set_porosity(d)
+    n.u_solid, n.B_solid, n.d_field = us, Bs, d
+    F = random_fields(rng, scheme, lat, shape)
+    if lat == "D3Q7":
+        F[1:4] *= 0.3
+        F[5:8] *= 0.3
+    o.init(F)
+    n.init(F)
+    for st in range(6):
+        o.step(1)
+        n.step(1)
+        assert np.abs(o.populations() - n.g).max() < 1e-14, st
+    assert np.abs(o.source_log() - n.src_acc).max() < 1e-13
+
+
+def test_P6_numpy_bruteforce_smooth_sphere():
+    rng = np.random.default_rng(505)
+    shape = (14, 12, 10)
+    o, n = make_pair("IDEAL", "D3Q19", shape, 0.7, bc=(2, 1, 0, 0, 0, 0))
+    cen, us = np.array([7.3, 6.1, 5.2]), np.array([-0.2, 0.05, 0.0])
+    mh = np.array([0.3, -0.5, 0.8]) / np.linalg.norm([0.3, -0.5, 0.8])
+    o.set_sphere(cen, 3.0, us, mh, 0.03)
+    o.set_sphere_width(1.5)
+    n.sphere, n.sphere_eps = (cen, 3.0, us, mh, 0.03, 0), 1.5
+    F = random_fields(rng, "IDEAL", "D3Q19", shape)
+    o.init(F)
+    n.init(F)
+    for st in range(6):
+        o.step(1)
+        n.step(1)
+        assert np.abs(o.populations() - n.g).max() < 1e-14, st
+    d, _, _ = n._solid()
+    assert ((d > 0) & (d < 1)).sum() > 20 and (d == 0).sum() > 20      # the ramp and the core were both exercised
+
+
+def test_porosity_limits_and_half_cell():
+    """d = 1 everywhere is the fluid run bit for bit; d in {0,1} equals the mask; a d = 1/2 cell in a state at rest takes
+    exactly half the solid velocity and the mean of the fields (Eq.13-14)."""
+    rng = np.random.default_rng(606)
+    shape = (8, 7, 6)
+    s = zyx(shape)
+    F = random_fields(rng, "IDEAL", "D3Q19", shape)
+    par = orc.make_params(orc.IDEAL, orc.D3Q19, shape, gamma=5 / 3, tau=0.7, powell=1.0)
+    a, b, c = orc.Oracle(par), orc.Oracle(par), orc.Oracle(par)
+    us, Bs = np.array([0.02, -0.01, 0.03]), 0.1 * (rng.random((3,) + s) - 0.5)
+    mask = (rng.random(s) < 0.1).astype(np.uint8) * 2
+    b.set_obstacle(np.zeros(s, dtype=np.uint8), us, Bs)
+    b.set_porosity(np.ones(s))
+    for o in (a, b):
+        o.init(F)
+        o.step(4)
+    assert np.array_equal(a.populations(), b.populations())
+    b.set_obstacle(mask, us, Bs)
+    b.set_porosity(None)
+    c.set_obstacle(np.zeros(s, dtype=np.uint8), us, Bs)
+    c.set_porosity(np.where(mask == 2, 0.0, 1.0))
+    b.init(F)
+    c.init(F)
+    b.step(4)
+    c.step(4)
+    assert np.array_equal(b.populations(), c.populations())
+    # half cell
+    B0 = np.array([0.05, -0.02, 0.03])
+    one = np.ones(s)
+    Fu = ideal_fields(1.3 * one, np.zeros((3,) + s), B0.reshape(3, 1, 1, 1) * one, 0.03 * one, 5 / 3)
+    d = np.ones(s)
+    d[2, 3, 4] = 0.5
+    h = orc.Oracle(par)
+    h.set_obstacle(np.zeros(s, dtype=np.uint8), us, np.zeros((3,) + s))
+    h.set_porosity(d)
+    h.init(Fu)
+    h.step(1)
+    Q = h.moments(diag=False)
+    assert np.allclose(Q[1:4, 2, 3, 4], 1.3 * 0.5 * us, rtol=0, atol=1e-16)
+    assert np.allclose(Q[5:8, 2, 3, 4], 0.5 * B0, rtol=0, atol=1e-16)
+    assert abs(Q[0, 2, 3, 4] - 1.3) < 1e-15
