@@ -114,6 +114,13 @@ int lbmhd_set_obstacle(lbmhd_t *h, const unsigned char *mask, const double u_sol
 int lbmhd_set_sphere(lbmhd_t *h, const double centre[3], double radius, const double u_solid[3],
                      const double dipole_dir[3], double B_surface);
 
+/* Fractional lattice porosity (Eq.15-16).  lbmhd_set_porosity: d in [0,1] per cell (fp64 [N], HOST or
+ * DEVICE per on_device; NULL = back to the mask) for the masked solid: u^ = d u + (1-d) u_solid, B^ likewise (Eq.13-14),
+ * u_solid / B_solid as given to lbmhd_set_obstacle.  lbmhd_set_sphere_width: linear ramp d = clamp(phi/eps + 1/2, 0, 1)
+ * of width eps (cells) across the sphere surface, phi the signed distance; eps = 0 (default) is the sharp sphere. */
+int lbmhd_set_porosity(lbmhd_t *h, const double *d_field, int on_device);
+int lbmhd_set_sphere_width(lbmhd_t *h, double eps);
+
 /* Raw population access (checkpoint / tests): fp64 [K][Q][N] at this boundary in both precisions, in
  * canonical (k, i, cell) order whatever the streaming layout.  HOST or DEVICE pointer per on_device. */
 int lbmhd_get_populations(lbmhd_t *h, double *g_out, int on_device);

@@ -67,7 +67,7 @@ constexpr int kMaxDiagBlocks = 1184;   // 8 x 148 SMs
 struct Layout {
   size_t pstride;        // elements per population plane (N rounded up to 32)
   size_t pop_bytes;      // one population copy
-  size_t off_pop[2], off_fields, off_M[2], off_mask, off_bsolid, off_partial, off_diag, total;
+  size_t off_pop[2], off_fields, off_M[2], off_mask, off_bsolid, off_dfield, off_partial, off_diag, total;
 };
 
 bool layout(const lbmhd_params *p, const Geometry &g, Layout *L) {
@@ -86,6 +86,7 @@ bool layout(const lbmhd_params *p, const Geometry &g, Layout *L) {
   L->off_M[1] = off; off += p->streaming == LBMHD_STREAM_INPLACE ? align_up((size_t)g.K * N * 8, 256) : 0;
   L->off_mask = off; off += align_up(N, 256);
   L->off_bsolid = off; off += align_up(3 * N * 8, 256);
+  L->off_dfield = off; off += align_up(N * 8, 256);
   L->off_partial = off; off += align_up((size_t)kMaxDiagBlocks * (3 * g.K + 4) * 8, 256);
   L->off_diag = off; off += 256;
   L->total = off;
@@ -107,10 +108,10 @@ struct lbmhd {
   int mcur;              // in place: which M array holds the moments published by the last step
   long long t;           // steps done since init
   long long launches;
-  bool have_mask, have_bsolid;
+  bool have_mask, have_bsolid, have_dfield;
   double usolid[3];
   bool has_sphere;
-  double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs;
+  double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs, sph_eps;
   long long sph_t0;
   int tx, minb;          // x-tile and min blocks/SM (launch bound) of the plain step kernel
   bool split;            // interior / edge launches split (large grids); LBMHD_SPLIT=0/1 overrides
@@ -318,7 +319,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
       h->launches += 1;
     }
     if (a.has_sphere) {   // interior-positioned tiles inside the sphere's bounding box
-      const double R = a.sph_R + 1.0;
+      const double R = a.sph_R + 0.5 * a.sph_eps + 1.0;
       int bx_lo = (int)floor((a.sph_c[0] - R) / TX), bx_hi = (int)floor((a.sph_c[0] + R) / TX);
       int y_lo = D > 1 ? (int)floor(a.sph_c[1] - R) : 0, y_hi = D > 1 ? (int)ceil(a.sph_c[1] + R) : 0;
       int z_lo = D > 2 ? (int)floor(a.sph_c[2] - R) : 0, z_hi = D > 2 ? (int)ceil(a.sph_c[2] + R) : 0;
@@ -362,6 +363,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     a.kappa = (real)h->p.powell; a.gamma = (real)h->p.gamma; a.c0sq = (real)h->p.c0sq;
     a.mask = h->have_mask ? (const unsigned char *)(h->ws + h->L.off_mask) : nullptr;
     a.Bsolid = h->have_bsolid ? (const double *)(h->ws + h->L.off_bsolid) : nullptr;
+    a.dfield = h->have_dfield ? (const double *)(h->ws + h->L.off_dfield) : nullptr;
     for (int c = 0; c < 3; c++) a.usolid[c] = h->usolid[c];
     {
       const long long es = (long long)sizeof(real);
@@ -375,6 +377,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     if (h->has_sphere) {
       a.sph_R = h->sph_R;
       a.sph_R2 = h->sph_R * h->sph_R;
+      a.sph_eps = h->sph_eps;
+      a.sph_touch2 = h->sph_eps > 0.0 ? (h->sph_R + 0.5 * h->sph_eps) * (h->sph_R + 0.5 * h->sph_eps) : a.sph_R2;
       a.sph_Bs = h->sph_Bs;
       for (int c = 0; c < 3; c++) { a.sph_m[c] = h->sph_m[c]; a.sph_u[c] = h->sph_u[c]; }
     }
@@ -581,6 +585,27 @@ int lbmhd_set_sphere(lbmhd_t *h, const double centre[3], double radius, const do
   h->has_sphere = true;
   for (int c = 0; c < 3; c++) { h->sph_c0[c] = centre[c]; h->sph_u[c] = u_solid[c]; h->sph_m[c] = dipole_dir[c]; }
   h->sph_R = radius; h->sph_Bs = B_surface; h->sph_t0 = h->t;
+  return LBMHD_OK;
+}
+
+int lbmhd_set_porosity(lbmhd_t *h, const double *d_field, int on_device) {
+  if (!h) return fail(LBMHD_EINVAL, "NULL handle");
+  if (int rc = use_device(h)) return rc;
+  if (!d_field) { h->have_dfield = false; return LBMHD_OK; }
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  CUDA_TRY(cudaMemcpyAsync(h->ws + h->L.off_dfield, d_field, h->N * 8, kind, h->stream));
+  if (!h->have_mask) {       // the kernels route tiles to the general path on "a mask exists"
+    CUDA_TRY(cudaMemsetAsync(h->ws + h->L.off_mask, 0, h->N, h->stream));
+    h->have_mask = true;
+  }
+  h->have_dfield = true;
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LBMHD_OK;
+}
+
+int lbmhd_set_sphere_width(lbmhd_t *h, double eps) {
+  if (!h || !(eps >= 0.0)) return fail(LBMHD_EINVAL, "bad handle or width");
+  h->sph_eps = eps;
   return LBMHD_OK;
 }
 

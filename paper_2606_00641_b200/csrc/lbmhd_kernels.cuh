@@ -33,6 +33,7 @@ template <typename real> struct StepArgs {
   real kappa, gamma, c0sq;
   const unsigned char *mask;    // [N] or nullptr
   const double *Bsolid;         // [3][N] or nullptr
+  const double *dfield;         // lattice porosity d in [0,1] per cell (Eq.15) or nullptr: d from the mask (SOLID -> 0)
   double usolid[3];
   long long ld_off[19];         // bytes from a cell's own slot in plane (k,0) to its pull source in plane (k,i), no wrap:
                                 //   (i*pstride - (c_x + c_y nx + c_z nx ny)) * sizeof(real)
@@ -42,15 +43,16 @@ template <typename real> struct StepArgs {
   double *M_next;               // in-place modes: moments published by this step
   int has_sphere;
   double sph_c[3], sph_R, sph_R2, sph_m[3], sph_Bs, sph_u[3];
+  double sph_eps, sph_touch2;   // width of the linear porosity ramp (Eq.15-16), 0 = sharp; (R + eps/2)^2
 };
 
-// ---- homogenised solid state at a cell (Eq.13-14; A8, A11, A12) ----------
-// Returns true when the cell is solid (porosity d = 0) and fills uS, BS.  The sphere decision
+// ---- homogenised solid state at a cell (Eq.13-16; A8, A11, A12) ----------
+// Returns the lattice porosity d in [0,1] and fills uS, BS when d < 1.  The sharp-sphere decision
 // |x - c|^2 <= R^2 is taken in fp64 with separately rounded products and sums, the order the oracle uses,
-// so both sides agree on the integer outcome.
+// so both sides agree on the integer outcome; the ramp d = clamp(phi/eps + 1/2, 0, 1) is continuous.
 template <typename real, int D>
-__device__ __forceinline__ bool solid_state(const StepArgs<real> &a, int x, int y, int z, size_t n, double uS[3],
-                                            double BS[3]) {
+__device__ __forceinline__ double solid_state(const StepArgs<real> &a, int x, int y, int z, size_t n, double uS[3],
+                                              double BS[3]) {
   if (a.has_sphere) {
     double r[3];
     r[0] = __dsub_rn((double)x, a.sph_c[0]);
@@ -59,34 +61,41 @@ __device__ __forceinline__ bool solid_state(const StepArgs<real> &a, int x, int 
     double r2 = __dmul_rn(r[0], r[0]);
     r2 = __dadd_rn(r2, __dmul_rn(r[1], r[1]));
     r2 = __dadd_rn(r2, __dmul_rn(r[2], r[2]));
-    if (r2 <= a.sph_R2) {
+    if (r2 <= a.sph_touch2) {
       const double rn = sqrt(r2);
-      const double rc = rn > 0.5 * a.sph_R ? rn : 0.5 * a.sph_R;
-      const double q = a.sph_R / rc;
-      const double amp = 0.5 * a.sph_Bs * (q * q * q);
-      double rh[3], mr = 0.0;
+      double d;
+      if (a.sph_eps > 0.0) d = fmin(fmax((rn - a.sph_R) / a.sph_eps + 0.5, 0.0), 1.0);
+      else d = r2 <= a.sph_R2 ? 0.0 : 1.0;
+      if (d < 1.0) {
+        const double rc = rn > 0.5 * a.sph_R ? rn : 0.5 * a.sph_R;
+        const double q = a.sph_R / rc;
+        const double amp = 0.5 * a.sph_Bs * (q * q * q);
+        double rh[3], mr = 0.0;
 #pragma unroll
-      for (int c = 0; c < 3; c++) {
-        rh[c] = rn > 0.0 ? r[c] / rn : 0.0;
-        mr += a.sph_m[c] * rh[c];
-      }
+        for (int c = 0; c < 3; c++) {
+          rh[c] = rn > 0.0 ? r[c] / rn : 0.0;
+          mr += a.sph_m[c] * rh[c];
+        }
 #pragma unroll
-      for (int c = 0; c < 3; c++) {
-        BS[c] = amp * (3.0 * mr * rh[c] - a.sph_m[c]);
-        uS[c] = a.sph_u[c];
+        for (int c = 0; c < 3; c++) {
+          BS[c] = amp * (3.0 * mr * rh[c] - a.sph_m[c]);
+          uS[c] = a.sph_u[c];
+        }
+        return d;
       }
-      return true;
     }
   }
-  if (a.mask != nullptr && a.mask[n] == CELL_SOLID) {
+  double d = 1.0;
+  if (a.dfield != nullptr) d = a.dfield[n];
+  else if (a.mask != nullptr && a.mask[n] == CELL_SOLID) d = 0.0;
+  if (d < 1.0) {
 #pragma unroll
     for (int c = 0; c < 3; c++) {
       uS[c] = a.usolid[c];
       BS[c] = a.Bsolid != nullptr ? a.Bsolid[(size_t)c * ((size_t)a.nx * a.ny * a.nz) + n] : 0.0;
     }
-    return true;
   }
-  return false;
+  return d;
 }
 
 // ---- flux row of variable k: Phi_k,alpha(Qh), alpha < D (Eq.11, Eq.8; A3) -------
@@ -189,9 +198,10 @@ __device__ __forceinline__ real powell_row(int k, const real *Qv) {
   }
 }
 
-// ---- blended state Q^ of a solid cell with porosity d = 0 (A8): rho and p kept, u = u^B, B = B^B -----------
+// ---- blended state Q^ of a cell with porosity d < 1 (Eq.13-14, A8): rho and p kept, u^ = d u + (1-d) u^B, B^ likewise -----
 template <int SCHEME, int D, typename real>
-__device__ __forceinline__ void solid_blend(const real *Qv, real gamma, const double uS[3], const double BS[3], real *Qh) {
+__device__ __forceinline__ void solid_blend(const real *Qv, real gamma, real d, const double uS[3], const double BS[3], real *Qh) {
+  const real e = real(1) - d;
   if (SCHEME == kIdeal) {
     const real rho = Qv[0];
     const real ir = real(1) / rho;
@@ -201,7 +211,7 @@ __device__ __forceinline__ void solid_blend(const real *Qv, real gamma, const do
     real uh2 = real(0), Bh2 = real(0);
 #pragma unroll
     for (int c = 0; c < 3; c++) {
-      const real uh = (real)uS[c], Bh = (real)BS[c];
+      const real uh = d * (Qv[1 + c] * ir) + e * (real)uS[c], Bh = d * Qv[5 + c] + e * (real)BS[c];
       Qh[1 + c] = rho * uh;
       Qh[5 + c] = Bh;
       uh2 += uh * uh;
@@ -213,8 +223,8 @@ __device__ __forceinline__ void solid_blend(const real *Qv, real gamma, const do
     Qh[0] = Qv[0];
 #pragma unroll
     for (int c = 0; c < D; c++) {
-      Qh[1 + c] = (real)uS[c];
-      Qh[1 + D + c] = (real)BS[c];
+      Qh[1 + c] = d * Qv[1 + c] + e * (real)uS[c];
+      Qh[1 + D + c] = d * Qv[1 + D + c] + e * (real)BS[c];
     }
   }
 }
@@ -292,7 +302,7 @@ __device__ __forceinline__ bool sphere_may_touch(const StepArgs<real> &a, int x0
   const double dx = fmax(0.0, fmax(lo, hi));
   const double dy = D > 1 ? (double)y - a.sph_c[1] : 0.0;
   const double dz = D > 2 ? (double)z - a.sph_c[2] : 0.0;
-  return dx * dx + dy * dy + dz * dz <= a.sph_R2 * (1.0 + 1e-9) + 1e-9;
+  return dx * dx + dy * dy + dz * dz <= a.sph_touch2 * (1.0 + 1e-9) + 1e-9;
 }
 
 // frozen cell in the in-place modes (A10): its populations are f^eq of its constant state, kept in M_cur
@@ -410,11 +420,13 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   bool solid = false;
   if constexpr (SOLID) {
     double uS[3], BS[3];
-    if (solid_state<real, D>(a, c.x, c.y, c.z, c.n, uS, BS)) {
+    const real d = (real)solid_state<real, D>(a, c.x, c.y, c.z, c.n, uS, BS);
+    if (d < real(1)) {
       real Qh[K];
-      solid_blend<SCHEME, D, real>(Qv, a.gamma, uS, BS, Qh);
+      solid_blend<SCHEME, D, real>(Qv, a.gamma, d, uS, BS, Qh);
       flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, Phi);
-      inj = pick<K, real>(Qh, k) - Qk;                          // dQh; the Powell source is scaled by d = 0
+      // dQh plus the Powell source scaled by the porosity d (A8)
+      inj = (pick<K, real>(Qh, k) - Qk) - d * (a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
       solid = true;
     }
   }

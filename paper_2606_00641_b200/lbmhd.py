@@ -61,6 +61,8 @@ def load_library():
     lib.lbmhd_moments.argtypes = [C.c_void_p, dp, dp, C.c_int]
     lib.lbmhd_set_obstacle.argtypes = [C.c_void_p, up, dp, dp, C.c_int]
     lib.lbmhd_set_sphere.argtypes = [C.c_void_p, dp, C.c_double, dp, dp, C.c_double]
+    lib.lbmhd_set_porosity.argtypes = [C.c_void_p, dp, C.c_int]
+    lib.lbmhd_set_sphere_width.argtypes = [C.c_void_p, C.c_double]
     lib.lbmhd_get_populations.argtypes = [C.c_void_p, dp, C.c_int]
     lib.lbmhd_set_populations.argtypes = [C.c_void_p, dp, C.c_int]
     lib.lbmhd_steps_done.argtypes = [C.c_void_p]
@@ -75,7 +77,7 @@ def load_library():
 
 EXPORTS = ["lbmhd_num_vars", "lbmhd_num_dirs", "lbmhd_workspace_bytes", "lbmhd_create", "lbmhd_destroy",
            "lbmhd_init", "lbmhd_step", "lbmhd_moments", "lbmhd_set_obstacle", "lbmhd_set_sphere",
-           "lbmhd_get_populations", "lbmhd_set_populations", "lbmhd_steps_done", "lbmhd_launch_count",
+           "lbmhd_set_porosity", "lbmhd_set_sphere_width", "lbmhd_get_populations", "lbmhd_set_populations", "lbmhd_steps_done", "lbmhd_launch_count",
            "lbmhd_copy_probe", "lbmhd_last_error"]
 
 
@@ -214,6 +216,16 @@ class Lbmhd:
         m = np.ascontiguousarray(dipole_dir, dtype=np.float64)
         _check(self.lib.lbmhd_set_sphere(self.h, _host_ptr(c), float(radius), _host_ptr(u), _host_ptr(m), float(B_surface)))
 
+    def set_porosity(self, d_field):
+        if d_field is None:
+            _check(self.lib.lbmhd_set_porosity(self.h, None, 0))
+            return
+        dp_, dev, keep = self._ptr(d_field, self.N, np.float64, self.torch.float64)
+        _check(self.lib.lbmhd_set_porosity(self.h, dp_, dev))
+
+    def set_sphere_width(self, eps):
+        _check(self.lib.lbmhd_set_sphere_width(self.h, float(eps)))
+
     def populations(self):
         """canonical fp64 [K, Q, nz, ny, nx] on the host (via a device tensor)"""
         torch = self.torch
@@ -246,6 +258,8 @@ def from_workload(w, precision=64, device=0, streaming=STREAM_AB):
     if w.get("sphere"):
         s = w["sphere"]
         sim.set_sphere(s["centre"], s["radius"], s["u_solid"], s["dipole_dir"], s["B_surface"])
+        if s.get("width"):
+            sim.set_sphere_width(s["width"])
     return sim
 
 

@@ -16,6 +16,8 @@ def oracle_from_workload(w, mask=None):
     if w.get("sphere"):
         s = w["sphere"]
         o.set_sphere(s["centre"], s["radius"], s["u_solid"], s["dipole_dir"], s["B_surface"])
+        if s.get("width"):
+            o.set_sphere_width(s["width"])
     return o
 
 

@@ -137,3 +137,28 @@ def test_fp32_variant_parity():
     w = W.get("C3", small=True)
     errs = compare(w, 100, tol=TOL32, precision=32)
     print("fp32 C3 small", errs.max())
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+def test_fractional_porosity_parity(streaming):
+    """Eq.13-16: per-cell porosity field for the masked solid and a ramp of width 1.5 cells across the moving sphere"""
+    rng = np.random.default_rng(808)
+    shape = (70, 12, 10)
+    s = zyx(shape)
+    w = random_workload("IDEAL", "D3Q19", shape, (1, 1) + (0,) * 4, seed=12)
+    d = np.clip(1.6 * rng.random(s) - 0.3, 0.0, 1.0)
+    us, Bs = np.array([0.03, -0.02, 0.01]), 0.1 * (rng.random((3,) + s) - 0.5)
+    o = oracle_from_workload(w)
+    g = gpu_from_workload(w, streaming=streaming)
+    for sim in (o, g):
+        sim.set_obstacle(np.zeros(s, dtype=np.uint8), us, Bs)
+        sim.set_porosity(d)
+        sim.init(w["fields"])
+        sim.step(15)
+    assert (field_errors(g.moments()[0], o.moments()[0]) <= TOL64).all()
+    g.close()
+    cen = np.array([36.3, 12.1, 10.2])
+    mh = np.array([0.3, -0.5, 0.8]) / np.linalg.norm([0.3, -0.5, 0.8])
+    sph = dict(centre=cen, radius=6.0, u_solid=np.array([-0.25, 0.0, 0.0]), dipole_dir=mh, B_surface=0.03, width=1.5)
+    w2 = random_workload("IDEAL", "D3Q19", (72, 24, 20), (2, 1, 0, 0, 0, 0), seed=13, sphere=sph)
+    compare(w2, 13, streaming=streaming)
