@@ -114,6 +114,7 @@ struct lbmhd {
   double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs, sph_eps;
   long long sph_t0;
   int tx, minb;          // x-tile and min blocks/SM (launch bound) of the plain step kernel
+  bool pair;             // fp32: two cells per thread (even nx); LBMHD_PAIR=0 turns it off
   bool split;            // interior / edge launches split (large grids); LBMHD_SPLIT=0/1 overrides
   bool use_tma;          // TMA-staged persistent step kernel (needs nx * sizeof(real) % 16 == 0)
   int num_sms;
@@ -236,6 +237,8 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
     if (e != cudaSuccess) { delete h; return fail(LBMHD_ECUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e)); }
     h->num_sms = sms;
+    h->pair = p->precision == 32 && p->nx % 2 == 0;
+    if (const char *e3 = getenv("LBMHD_PAIR")) h->pair = h->pair && atoi(e3) != 0;
     h->split = false;   // measured slower on config 5: edge tiles lose DRAM page locality when launched apart from their rows
     if (const char *e2 = getenv("LBMHD_SPLIT")) h->split = atoi(e2) != 0;
     const char *path = getenv("LBMHD_PATH");      // tuning knob: "plain" forces the register-pull kernel
@@ -283,6 +286,23 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     else step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_LOC><<<g, b, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
     h->launches += 1;
     return cudaGetLastError();
+  }
+
+  // fp32: two cells per thread (64-cell tiles); needs an even nx for the 8-byte alignment of the float2 accesses
+  template <int MINB> static cudaError_t launch_step_pair(lbmhd_t *h, const StepArgs<real> &a) {
+    if constexpr (sizeof(real) == 4) {
+      const int npair = h->p.nx >= 128 ? (h->p.nx - 64) / 64 : 0;      // pair tiles at x0 = 32 + 64 j, all interior in x
+      const int ntail = (h->p.nx - (32 + 64 * npair) + 31) / 32;         // 32-cell tiles after the pair tiles (>= 0)
+      const dim3 g(npair + 1 + (ntail > 0 ? ntail : 0), h->p.ny, h->p.nz), b(32, K);
+      const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
+      if (!inplace) step_kernel_pair<LAT, SCHEME, MINB, ST_AB><<<g, b, 0, h->stream>>>(a, npair);
+      else if (h->parity == 0) step_kernel_pair<LAT, SCHEME, MINB, ST_PP><<<g, b, 0, h->stream>>>(a, npair);
+      else step_kernel_pair<LAT, SCHEME, MINB, ST_LOC><<<g, b, 0, h->stream>>>(a, npair);
+      h->launches += 1;
+      return cudaGetLastError();
+    } else {
+      return cudaErrorInvalidValue;
+    }
   }
 
   template <int TX, int MINB> static cudaError_t launch_step_whole(lbmhd_t *h, const StepArgs<real> &a) {
@@ -399,7 +419,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
         }
       }
       cudaError_t e;
-      if (inplace) e = h->minb == 4 ? launch_step_inplace<4>(h, a) : launch_step_inplace<3>(h, a);
+      if (sizeof(real) == 4 && h->pair) e = h->minb == 2 ? launch_step_pair<2>(h, a) : (h->minb == 4 ? launch_step_pair<4>(h, a) : launch_step_pair<3>(h, a));
+      else if (inplace) e = h->minb == 4 ? launch_step_inplace<4>(h, a) : launch_step_inplace<3>(h, a);
       else if (h->use_tma) e = launch_step_tma(h, a);
       else switch (h->tx * 10 + h->minb) {
         case 322: e = launch_step_whole<32, 2>(h, a); break;

@@ -531,19 +531,16 @@ struct Region {
 // MODE 1: interior tiles only (no general path compiled in); MODE 2: general tiles only, over a Region.
 //         (split launches: measured slower, kept behind LBMHD_SPLIT=1, A/B only.)
 // =====================================================================================================
-template <int LAT, int SCHEME, typename real, int TX, int MINB, int MODE, int STREAM>
-__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
-step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int sphere_only) {
+// One TX-cell tile of row (y, z) starting at x0: classification and the three paths (interior / x-edge / general).
+// Called by all TX*K threads of a block together (it contains block barriers).
+template <int LAT, int SCHEME, typename real, int TX, int MODE, int STREAM>
+__device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, const int k, const int x0, const int y, const int z,
+                                         const int sphere_only, real (*sQ)[TX], real (*sTr)[TX]) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
   using V = Vars<SCHEME, D>;
   constexpr int K = V::K;
-  __shared__ real sQ[K][TX];
-  __shared__ real sTr[D][TX];
-
-  const int tx = threadIdx.x, k = threadIdx.y;
-  const int x0 = (r.bx0 + (int)blockIdx.x * r.bxs) * TX;
-  const int x = x0 + tx, y = r.y0 + (int)blockIdx.y * r.ys, z = r.z0 + (int)blockIdx.z * r.zs;
+  const int x = x0 + tx;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
   const auto sync = [] { __syncthreads(); };
   const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
@@ -661,6 +658,170 @@ step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int 
     return;
   }
   general_tile<LAT, SCHEME, real, TX, STREAM>(a, tx, k, x, y, z, sQ, sTr, sync);
+}
+
+template <int LAT, int SCHEME, typename real, int TX, int MINB, int MODE, int STREAM>
+__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
+step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int sphere_only) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, K = Vars<SCHEME, D>::K;
+  __shared__ real sQ[K][TX];
+  __shared__ real sTr[D][TX];
+  run_tile<LAT, SCHEME, real, TX, MODE, STREAM>(a, threadIdx.x, threadIdx.y, (r.bx0 + (int)blockIdx.x * r.bxs) * TX,
+                                                r.y0 + (int)blockIdx.y * r.ys, r.z0 + (int)blockIdx.z * r.zs, sphere_only, sQ, sTr);
+}
+
+// =====================================================================================================
+// fp32 variant with TWO adjacent cells per thread.  With 4-byte populations a warp's row
+// segment is only 128 bytes, so the one-cell mapping needs twice the instructions per byte and is issue-bound
+// (measured 4.4-4.9 TB/s).  Here a block owns 64 x-cells x K sets with the same 32 x K threads; thread tx
+// holds cells x0 + 2 tx and x0 + 2 tx + 1: float2 loads for the 9 unshifted directions and float2 stores
+// for all, two scalar loads where the x-shift breaks the 8-byte alignment.  Interior tiles only; every
+// other tile is handed to run_tile() in 32-cell pieces.
+// =====================================================================================================
+template <typename real> struct StorePairOwn {
+  char *base;
+  const long long *st_off;
+  __device__ __forceinline__ void put2(int j, real v0, real v1) const {
+    *reinterpret_cast<float2 *>(base + st_off[j]) = make_float2(v0, v1);
+  }
+};
+template <class L, typename real> struct StorePairPP {
+  char *base;
+  const long long *ld_off;
+  __device__ __forceinline__ void put2(int j, real v0, real v1) const {
+    const int i = opp(j);
+    if (L::cx(i) == 0) {
+      *reinterpret_cast<float2 *>(base + ld_off[i]) = make_float2(v0, v1);
+    } else {
+      *reinterpret_cast<real *>(base + ld_off[i]) = v0;
+      *reinterpret_cast<real *>(base + ld_off[i] + (long long)sizeof(real)) = v1;
+    }
+  }
+};
+
+template <int LAT, int SCHEME, int STREAM, class Store>
+__device__ __forceinline__ void finish_pair(const StepArgs<float> &a, int tx, int k, uint32_t n, bool writeM0, bool writeM1,
+                                            float (&f0)[Lattice<LAT>::Q], float (&f1)[Lattice<LAT>::Q], const Store &store,
+                                            float (*sQ)[64], float (*sTr)[64]) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, Q = L::Q;
+  using V = Vars<SCHEME, D>;
+  constexpr int K = V::K, iB = V::iB;
+  float Qk0 = 0.f, Qk1 = 0.f;
+#pragma unroll
+  for (int i = 0; i < Q; i++) { Qk0 += f0[i]; Qk1 += f1[i]; }
+  *reinterpret_cast<float2 *>(&sQ[k][2 * tx]) = make_float2(Qk0, Qk1);
+  if (k >= iB && k < iB + D) {
+    const int b = k - iB;
+    float t0 = 0.f, t1 = 0.f;
+#pragma unroll
+    for (int i = 0; i < Q; i++) {
+      const int cb = lat_c<L>(i, 0) * (b == 0) + lat_c<L>(i, 1) * (b == 1) + lat_c<L>(i, 2) * (b == 2);
+      if (lat_c<L>(i, 0) != 0 || lat_c<L>(i, 1) != 0 || lat_c<L>(i, 2) != 0) { t0 += float(cb) * f0[i]; t1 += float(cb) * f1[i]; }
+    }
+    *reinterpret_cast<float2 *>(&sTr[b][2 * tx]) = make_float2(t0, t1);
+  }
+  __syncthreads();
+  float Qv0[K], Qv1[K];
+#pragma unroll
+  for (int l = 0; l < K; l++) {
+    const float2 q = *reinterpret_cast<const float2 *>(&sQ[l][2 * tx]);
+    Qv0[l] = q.x; Qv1[l] = q.y;
+  }
+  float tr0 = 0.f, tr1 = 0.f;
+#pragma unroll
+  for (int b = 0; b < D; b++) {
+    const float2 t = *reinterpret_cast<const float2 *>(&sTr[b][2 * tx]);
+    tr0 += t.x; tr1 += t.y;
+  }
+  float Phi0[3], Phi1[3];
+  flux_row<SCHEME, D, float>(k, Qv0, a.gamma, a.c0sq, Phi0);
+  flux_row<SCHEME, D, float>(k, Qv1, a.gamma, a.c0sq, Phi1);
+  const float kd = a.kappa * a.inv_tauB_cs2;
+  const float inj0 = (kd * tr0) * powell_row<SCHEME, D, float>(k, Qv0);      // -kappa delta S_row, delta = -tr/(tau_B cs2)
+  const float inj1 = (kd * tr1) * powell_row<SCHEME, D, float>(k, Qv1);
+  if (STREAM != ST_AB) {
+    const size_t N = (size_t)a.nx * a.ny * a.nz;
+    if (writeM0) a.M_next[(size_t)k * N + n] = (double)(Qk0 + inj0);
+    if (writeM1) a.M_next[(size_t)k * N + n + 1] = (double)(Qk1 + inj1);
+  }
+  const float om = a.omega[k], omc = 1.f - om;
+  const float b00 = om * Qk0 + inj0, b01 = om * Qk1 + inj1;
+  const float ic = float(L::inv_cs2) * om;
+  const float P00 = ic * Phi0[0], P01 = ic * Phi0[1], P02 = ic * Phi0[2];
+  const float P10 = ic * Phi1[0], P11 = ic * Phi1[1], P12 = ic * Phi1[2];
+#pragma unroll
+  for (int i = 0; i < Q; i++) {
+    float t0 = float(L::w(i)) * b00, t1 = float(L::w(i)) * b01;
+    if (L::cx(i) != 0) { t0 = fmaf(float(L::cx(i) * L::w(i)), P00, t0); t1 = fmaf(float(L::cx(i) * L::w(i)), P10, t1); }
+    if (L::cy(i) != 0) { t0 = fmaf(float(L::cy(i) * L::w(i)), P01, t0); t1 = fmaf(float(L::cy(i) * L::w(i)), P11, t1); }
+    if (L::cz(i) != 0) { t0 = fmaf(float(L::cz(i) * L::w(i)), P02, t0); t1 = fmaf(float(L::cz(i) * L::w(i)), P12, t1); }
+    store.put2(i, fmaf(f0[i], omc, t0), fmaf(f1[i], omc, t1));
+  }
+}
+
+template <int LAT, int SCHEME, int MINB, int STREAM>
+__global__ void __launch_bounds__(32 * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
+step_kernel_pair(const __grid_constant__ StepArgs<float> a, const int npair) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, Q = L::Q;
+  using V = Vars<SCHEME, D>;
+  constexpr int K = V::K;
+  __shared__ float sQ[K][64];
+  __shared__ float sTr[D][64];
+  const int tx = threadIdx.x, k = threadIdx.y;
+  // row layout: [32-cell edge tile][npair 64-cell pair tiles][rest in 32-cell tiles], one block each, so that the pair
+  // tiles are all interior when the row is; blocks 0..npair-1 are the pair tiles, block npair the first edge tile
+  const int nx = a.nx, ny = a.ny, nz = a.nz;
+  const int y = blockIdx.y, z = blockIdx.z;
+  float(*sQ32)[32] = reinterpret_cast<float(*)[32]>(&sQ[0][0]);
+  float(*sTr32)[32] = reinterpret_cast<float(*)[32]>(&sTr[0][0]);
+  if ((int)blockIdx.x >= npair) {
+    const int t = (int)blockIdx.x - npair;
+    run_tile<LAT, SCHEME, float, 32, 0, STREAM>(a, tx, k, t == 0 ? 0 : 32 + 64 * npair + 32 * (t - 1), y, z, 0, sQ32, sTr32);
+    return;
+  }
+  const int x0 = 32 + (int)blockIdx.x * 64;
+  const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
+  const bool row_inner = (D < 2 || (y >= 1 && y <= ny - 2)) && (D < 3 || (z >= 1 && z <= nz - 2));
+  const bool interior = x0 >= 1 && x0 + 64 <= nx - 1 && row_inner && a.mask == nullptr && !sphere_may_touch<float, D>(a, x0, 64, y, z);
+  if (interior) {
+    const int x = x0 + 2 * tx;
+    const uint32_t n = ((uint32_t)z * ny + y) * nx + x;
+    char *__restrict__ pb = reinterpret_cast<char *>(const_cast<float *>(a.src) + ((size_t)k * Q * a.pstride + n));
+    float f0[Q], f1[Q];
+#pragma unroll
+    for (int i = 0; i < Q; i++) {
+      if (STREAM == ST_LOC) {
+        const float2 v = *reinterpret_cast<const float2 *>(pb + a.st_off[opp(i)]);
+        f0[i] = v.x; f1[i] = v.y;
+      } else if (L::cx(i) == 0) {
+        const float2 v = *reinterpret_cast<const float2 *>(pb + a.ld_off[i]);
+        f0[i] = v.x; f1[i] = v.y;
+      } else {
+        f0[i] = *reinterpret_cast<const float *>(pb + a.ld_off[i]);
+        f1[i] = *reinterpret_cast<const float *>(pb + a.ld_off[i] + 4);
+      }
+    }
+    const bool rowM = STREAM != ST_AB && ((npy && (y == 1 || y == ny - 2)) || (npz && (z == 1 || z == nz - 2)));
+    const bool wM0 = rowM || (npx && (x == 1 || x == nx - 2)), wM1 = rowM || (npx && (x + 1 == 1 || x + 1 == nx - 2));
+    if (STREAM == ST_AB) {
+      const StorePairOwn<float> st{reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + n)), a.st_off};
+      finish_pair<LAT, SCHEME, STREAM>(a, tx, k, n, wM0, wM1, f0, f1, st, sQ, sTr);
+    } else if (STREAM == ST_PP) {
+      const StorePairPP<L, float> st{pb, a.ld_off};
+      finish_pair<LAT, SCHEME, STREAM>(a, tx, k, n, wM0, wM1, f0, f1, st, sQ, sTr);
+    } else {
+      const StorePairOwn<float> st{pb, a.st_off};
+      finish_pair<LAT, SCHEME, STREAM>(a, tx, k, n, wM0, wM1, f0, f1, st, sQ, sTr);
+    }
+    return;
+  }
+  // anything else: the two 32-cell halves through the one-cell paths (they share sQ / sTr rows 0..31)
+  run_tile<LAT, SCHEME, float, 32, 0, STREAM>(a, tx, k, x0, y, z, 0, sQ32, sTr32);
+  __syncthreads();
+  if (x0 + 32 < nx) run_tile<LAT, SCHEME, float, 32, 0, STREAM>(a, tx, k, x0 + 32, y, z, 0, sQ32, sTr32);
 }
 
 // ---- S10 init: g_{k,i} = w_i (Q_k + c_i.Phi_k(Q)/c_s^2) (Eq.3) from fp64 fields [K][N] ---------

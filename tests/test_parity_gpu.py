@@ -45,7 +45,11 @@ def compare(w, steps, tol=TOL64, mask=None, obstacle=None, precision=64, streami
     assert (errs <= tol).all(), errs
     K = o.K
     e_sum, e_abs, e_max = diag_errors(dg, do, K)
-    assert (e_sum <= 10 * tol).all() and (e_abs <= 10 * tol).all() and (e_max <= 10 * tol).all()
+    # a sum over N cells, each within tol * max|Q_k|, can be off by tol * N * max|Q_k|; relative to sum|Q_k| that is
+    # tol * N max / sum|.| (>= tol; large for a field that lives in a small part of the domain)
+    N = Qo[0].size
+    bound = tol * np.maximum(1.0, N * do[2 * K:3 * K] / np.maximum(do[K:2 * K], 1e-300))
+    assert (e_sum <= bound).all() and (e_abs <= bound).all() and (e_max <= 10 * tol).all()
     assert abs(dg[3 * K] - do[3 * K]) <= 1e3 * tol * max(do[2 * K:3 * K].max(), 1e-300)        # max|div_h B|
     if np.isfinite(do[3 * K + 1]):
         assert abs(dg[3 * K + 1] - do[3 * K + 1]) <= 10 * tol * abs(do[3 * K + 1])             # min rho
@@ -162,3 +166,22 @@ def test_fractional_porosity_parity(streaming):
     sph = dict(centre=cen, radius=6.0, u_solid=np.array([-0.25, 0.0, 0.0]), dipole_dir=mh, B_surface=0.03, width=1.5)
     w2 = random_workload("IDEAL", "D3Q19", (72, 24, 20), (2, 1, 0, 0, 0, 0), seed=13, sphere=sph)
     compare(w2, 13, streaming=streaming)
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+@pytest.mark.parametrize("scheme,lattice,shape,bc", [
+    ("IDEAL", "D3Q19", (200, 12, 9), (0,) * 6), ("IDEAL", "D3Q19", (200, 12, 9), (2, 1, 0, 0, 0, 0)),
+    ("IDEAL", "D2Q9", (300, 37), (1, 1, 1, 1, 0, 0)), ("INCRES", "D2Q9", (300, 37), (0,) * 6),
+    ("IDEAL", "D3Q7", (200, 12, 9), (2, 1, 1, 1, 0, 0)), ("IDEAL", "D1Q3", (400,), (1, 1, 0, 0, 0, 0)),
+    ("IDEAL", "D2Q9", (131, 20), (0,) * 6),          # odd nx: one cell per thread
+])
+def test_fp32_paths_parity(scheme, lattice, shape, bc, streaming):
+    """fp32: two cells per thread on interior tiles (even nx), one-cell paths elsewhere; bar 1e-5 (north_star)"""
+    w = random_workload(scheme, lattice, shape, bc, seed=77)
+    compare(w, 20, tol=TOL32, precision=32, streaming=streaming)
+    compare(w, 7, tol=TOL32, precision=32, streaming=streaming)
+
+
+def test_fp32_config5_small_with_sphere():
+    compare(W.get("C5", small=True), 60, tol=TOL32, precision=32)
+    compare(W.get("C5", small=True), 61, tol=TOL32, precision=32, streaming=1)
