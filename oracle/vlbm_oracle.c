@@ -23,7 +23,7 @@
 #include <omp.h>
 #endif
 
-#define MAXK 8
+#define MAXK 9
 #define MAXQ 19
 
 /* ---- lattice tables (A2): rest; +x,-x,+y,-y,+z,-z; diagonals (+,+),(-,-),(+,-),(-,+) per plane
@@ -89,7 +89,8 @@ int oracle_lattice(int lattice, int *D, int *Q, int *c, double *w, double *cs2)
   return 0;
 }
 
-static int num_vars(int scheme, int D) { return scheme == ORC_IDEAL ? 8 : 1 + 2 * D; }
+static int is_ideal(int scheme) { return scheme == ORC_IDEAL || scheme == ORC_IDEAL_DIVB; }
+static int num_vars(int scheme, int D) { return scheme == ORC_IDEAL ? 8 : (scheme == ORC_IDEAL_DIVB ? 9 : 1 + 2 * D); }
 
 int oracle_num_vars(const oracle_params *p)
 {
@@ -122,7 +123,7 @@ int oracle_get_threads(void)
 static void flux_eval(int scheme, int D, double gamma, double c0sq, const double *Q, double Phi[MAXK][3])
 {
   int a, b;
-  if (scheme == ORC_IDEAL) {
+  if (is_ideal(scheme)) {
     double rho = Q[0], E = Q[4];
     const double *m = Q + 1, *B = Q + 5;
     double u[3];
@@ -137,6 +138,8 @@ static void flux_eval(int scheme, int D, double gamma, double c0sq, const double
       for (b = 0; b < 3; b++) Phi[1 + b][a] = m[b] * u[a] + (a == b ? pt : 0.0) - B[b] * B[a];
       Phi[4][a] = (E + pt) * u[a] - B[a] * uB;
       for (b = 0; b < 3; b++) Phi[5 + b][a] = u[a] * B[b] - B[a] * u[b];
+      /* Eq.10 PAPER.md:136 traced: the relaxation variable D = tr G has the flux D u - B */
+      if (scheme == ORC_IDEAL_DIVB) Phi[8][a] = Q[8] * u[a] - B[a];
     }
   } else {
     double P = Q[0];
@@ -220,7 +223,8 @@ int oracle_create(const oracle_params *p, const unsigned char *cell_mask, oracle
   lattice_t L;
   *out = NULL;
   if (lattice_make(p->lattice, &L)) return -1;
-  if (p->scheme != ORC_IDEAL && p->scheme != ORC_INCRES) return -1;
+  if (p->scheme != ORC_IDEAL && p->scheme != ORC_INCRES && p->scheme != ORC_IDEAL_DIVB) return -1;
+  if (p->scheme == ORC_IDEAL_DIVB && !(p->tau_relax > 0.0)) return -1;
   if (p->nx < 1 || p->ny < 1 || p->nz < 1) return -1;
   if (L.D < 2 && p->ny != 1) return -1;
   if (L.D < 3 && p->nz != 1) return -1;
@@ -237,8 +241,8 @@ int oracle_create(const oracle_params *p, const unsigned char *cell_mask, oracle
   o->K = num_vars(p->scheme, L.D);
   o->N = (long)p->nx * p->ny * p->nz;
   o->iU = 1;
-  o->iB = p->scheme == ORC_IDEAL ? 5 : 1 + L.D;
-  int nvec = p->scheme == ORC_IDEAL ? 3 : L.D;
+  o->iB = is_ideal(p->scheme) ? 5 : 1 + L.D;
+  int nvec = is_ideal(p->scheme) ? 3 : L.D;
   double tau[MAXK] = { 0 };
   for (int k = 0; k < o->K; k++) tau[k] = p->tau[k];
   /* Eq.5: tau = 1/2 + D / c_s^2 for the sets that carry a physical diffusivity (A3) */
@@ -253,7 +257,7 @@ int oracle_create(const oracle_params *p, const unsigned char *cell_mask, oracle
   }
   o->tauB = tau[o->iB];
   for (int b = 1; b < nvec; b++) if (tau[o->iB + b] != o->tauB) { free(o); return -1; }   /* A7 */
-  if (p->scheme == ORC_IDEAL && !(p->gamma > 1.0)) { free(o); return -1; }
+  if (is_ideal(p->scheme) && !(p->gamma > 1.0)) { free(o); return -1; }
   size_t bytes = (size_t)o->K * L.Q * o->N * sizeof(double);
   o->g[0] = (double *)calloc(1, bytes);
   o->g[1] = (double *)calloc(1, bytes);
@@ -467,16 +471,19 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
   double tr = 0.0;
   for (b = 0; b < D; b++) for (i = 0; i < Qn; i++) tr += (double)L->c[i][b] * f[o->iB + b][i];
   double delta = -tr / (o->tauB * L->cs2);
+  /* IDEAL_DIVB: div B from the relaxation variable instead, D ~ tau_M div B (Eq.7) */
+  if (o->p.scheme == ORC_IDEAL_DIVB) delta = Qv[8] / o->p.tau_relax;
 
   /* 4. Powell source (Eq.12), direct injection (A5) */
   double S[MAXK];
   for (k = 0; k < K; k++) S[k] = 0.0;
   double kd = o->p.powell * delta;
-  if (o->p.scheme == ORC_IDEAL) {
+  if (is_ideal(o->p.scheme)) {
     double u[3], uBdot = 0.0;
     for (b = 0; b < 3; b++) { u[b] = Qv[1 + b] / Qv[0]; uBdot += u[b] * Qv[5 + b]; }
     for (b = 0; b < 3; b++) { S[1 + b] = -kd * Qv[5 + b]; S[5 + b] = -kd * u[b]; }
     S[4] = -kd * uBdot;
+    if (o->p.scheme == ORC_IDEAL_DIVB) S[8] = -Qv[8] / o->p.tau_relax;      /* relaxation source of Eq.6 */
   } else {
     for (b = 0; b < D; b++) { S[1 + b] = -kd * Qv[1 + D + b]; S[1 + D + b] = -kd * Qv[1 + b]; }
   }
@@ -487,7 +494,7 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
   double uSol[3], BSol[3];
   double d = solid_state(o, x, y, z, n, uSol, BSol);
   if (d < 1.0) {
-    if (o->p.scheme == ORC_IDEAL) {
+    if (is_ideal(o->p.scheme)) {
       double rho = Qv[0], u[3], uh[3], Bh[3], mu = 0.0, B2 = 0.0, uh2 = 0.0, Bh2 = 0.0;
       for (b = 0; b < 3; b++) {
         u[b] = Qv[1 + b] / rho;
@@ -509,7 +516,8 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
         Qh[1 + D + b] = d * Qv[1 + D + b] + (1.0 - d) * BSol[b];
       }
     }
-    for (k = 0; k < K; k++) { dQh[k] = Qh[k] - Qv[k]; S[k] *= d; }
+    /* the Powell rows are scaled by the porosity (A8); the relaxation of D is intrinsic and is not */
+    for (k = 0; k < K; k++) { dQh[k] = Qh[k] - Qv[k]; if (!(o->p.scheme == ORC_IDEAL_DIVB && k == 8)) S[k] *= d; }
   }
   if (srcacc) for (k = 0; k < K; k++) srcacc[k] += S[k];
 
@@ -616,7 +624,7 @@ int oracle_moments(oracle_t *o, double *fields_out, double *diag_out)
       }
       div /= L->cs2;
       if (fabs(div) > maxdiv) maxdiv = fabs(div);
-      if (o->p.scheme == ORC_IDEAL) {
+      if (is_ideal(o->p.scheme)) {
         double rho = F[n], mu = 0.0, B2 = 0.0;
         for (int b = 0; b < 3; b++) {
           double m = F[(long)(1 + b) * N + n], B = F[(long)(5 + b) * N + n];

@@ -64,6 +64,16 @@ def flux_ideal(Q, gamma, D):
     return Phi
 
 
+def flux_ideal_divb(Q, gamma, D):
+    """IDEAL plus the traced gradient variable D = tr G of PAPER.md:104-138: flux D u - B (Eq.10 traced)."""
+    Phi = np.zeros((9, 3) + Q.shape[1:])
+    Phi[:8] = flux_ideal(Q[:8], gamma, D)
+    u = Q[1:4] / Q[0]
+    Phi[8] = Q[8][None] * u - Q[5:8]
+    Phi[8, D:] = 0.0
+    return Phi
+
+
 def flux_incres(Q, c0sq, D):
     """A3. Q: [1+2D, ...] = (P, u, B)."""
     P, u, B = Q[0], Q[1:1 + D], Q[1 + D:1 + 2 * D]
@@ -80,16 +90,18 @@ class NpVLBM:
     """fields / populations are indexed [k, (i,) z, y, x]."""
 
     def __init__(self, scheme, lat, shape_zyx, tau, gamma=5 / 3, c0sq=1 / 12, powell=1.0,
-                 bc=(0,) * 6, mask=None):
+                 bc=(0,) * 6, mask=None, tau_relax=0.0):
         self.scheme = scheme
         self.D, self.c, self.w, self.cs2 = lattice_np(lat)
         self.Qn = len(self.w)
         self.shape = tuple(shape_zyx)
-        self.K = 8 if scheme == "IDEAL" else 1 + 2 * self.D
+        self.K = 8 if scheme == "IDEAL" else (9 if scheme == "IDEAL_DIVB" else 1 + 2 * self.D)
+        self.ideal = scheme in ("IDEAL", "IDEAL_DIVB")
+        self.tau_relax = tau_relax
         self.tau = np.broadcast_to(np.asarray(tau, dtype=float), (self.K,)).copy()
         self.gamma, self.c0sq, self.kappa = gamma, c0sq, powell
         self.bc = tuple(bc)
-        self.iB = 5 if scheme == "IDEAL" else 1 + self.D
+        self.iB = 5 if self.ideal else 1 + self.D
         self.mask = np.zeros(self.shape, dtype=np.uint8) if mask is None else np.asarray(mask, dtype=np.uint8).reshape(self.shape)
         self.u_solid = np.zeros(3)
         self.B_solid = None
@@ -103,7 +115,11 @@ class NpVLBM:
         self.n_axis = (self.shape[2], self.shape[1], self.shape[0])
 
     def flux(self, Q):
-        return flux_ideal(Q, self.gamma, self.D) if self.scheme == "IDEAL" else flux_incres(Q, self.c0sq, self.D)
+        if self.scheme == "IDEAL":
+            return flux_ideal(Q, self.gamma, self.D)
+        if self.scheme == "IDEAL_DIVB":
+            return flux_ideal_divb(Q, self.gamma, self.D)
+        return flux_incres(Q, self.c0sq, self.D)
 
     def feq(self, Q, Phi):
         # Eq.3: w_i (Q_k + c_i.Phi_k / cs2) -> [K, Qn, ...]
@@ -214,14 +230,18 @@ class NpVLBM:
         for b in range(D):
             tr += np.tensordot(self.c[:, b].astype(float), f[self.iB + b], axes=([0], [0]))
         delta = -tr / (self.tau[self.iB] * self.cs2)
+        if self.scheme == "IDEAL_DIVB":
+            delta = Q[8] / self.tau_relax            # Eq.7: D ~ tau_M div B
         # 4. Powell source
         S = np.zeros_like(Q)
-        if self.scheme == "IDEAL":
+        if self.ideal:
             u = Q[1:4] / Q[0]
             B = Q[5:8]
             S[1:4] = -self.kappa * delta * B
             S[4] = -self.kappa * delta * (u * B).sum(0)
             S[5:8] = -self.kappa * delta * u
+            if self.scheme == "IDEAL_DIVB":
+                S[8] = -Q[8] / self.tau_relax        # relaxation source of Eq.6
         else:
             u, B = Q[1:1 + D], Q[1 + D:]
             S[1:1 + D] = -self.kappa * delta * B
@@ -229,7 +249,7 @@ class NpVLBM:
         # 5. homogenised solid
         d, uB, BB = self._solid()
         Qh = Q.copy()
-        if self.scheme == "IDEAL":
+        if self.ideal:
             rho = Q[0]
             u = Q[1:4] / rho
             B = Q[5:8]
@@ -248,7 +268,10 @@ class NpVLBM:
                 Qh[1 + b] = np.where(sol, d * Q[1 + b] + (1 - d) * uB[b], Q[1 + b])
                 Qh[1 + D + b] = np.where(sol, d * Q[1 + D + b] + (1 - d) * BB[b], Q[1 + D + b])
         dQh = Qh - Q
-        S = S * d
+        if self.scheme == "IDEAL_DIVB":
+            S[:8] = S[:8] * d
+        else:
+            S = S * d
         # 6./7. flux, BGK, injection
         feq = self.feq(Q, self.flux(Qh))
         om = (1.0 / self.tau).reshape((K, 1) + (1,) * len(self.shape))
