@@ -15,6 +15,7 @@
  *  - Macroscopic fields are fp64 SoA [K][nz][ny][nx], x fastest, at this boundary in both precisions.
  *    IDEAL: K = 8 in every dimension, order rho, m_x, m_y, m_z, E, B_x, B_y, B_z.
  *    INCRES: K = 1 + 2D, order P, u_1..u_D, B_1..B_D (P = kinematic pressure carrier, A3).
+ *    IDEAL_DIVB: K = 9, the IDEAL order followed by D.
  *  - Direction order: rest; +x,-x,+y,-y,+z,-z; diagonals (+,+),(-,-),(+,-),(-,+) per plane xy, xz, yz.
  *  - Every pointer argument says whether it is a HOST or a DEVICE pointer.  The caller owns every
  *    buffer it passes, including `workspace` (device memory, e.g. a torch tensor): the library never
@@ -37,7 +38,9 @@ typedef struct lbmhd lbmhd_t;
 
 enum { LBMHD_D1Q3 = 1, LBMHD_D2Q9 = 2, LBMHD_D3Q19 = 3,
        LBMHD_D2Q5 = 4, LBMHD_D3Q7 = 5 /* the paper's own lattices; D3Q7 has c_s^2 = 1/4 */ };
-enum { LBMHD_IDEAL = 0, LBMHD_INCRES = 1 };
+enum { LBMHD_IDEAL = 0, LBMHD_INCRES = 1,
+       LBMHD_IDEAL_DIVB = 2 /* IDEAL + the paper's local gradient evolution in traced form: a 9th set
+                               D = tr G with flux D u - B and source -D/tau_relax; div B in Eq.12 := D/tau_relax */ };
 enum { LBMHD_BC_PERIODIC = 0, LBMHD_BC_ZEROGRAD = 1, LBMHD_BC_INFLOW = 2 };
 enum { LBMHD_CELL_FLUID = 0, LBMHD_CELL_FROZEN = 1, LBMHD_CELL_SOLID = 2 };
 enum { LBMHD_STREAM_AB = 0, LBMHD_STREAM_INPLACE = 1 };
@@ -50,14 +53,15 @@ enum {
 };
 
 typedef struct {
-  int    scheme;        /* LBMHD_IDEAL | LBMHD_INCRES */
+  int    scheme;        /* LBMHD_IDEAL | LBMHD_INCRES | LBMHD_IDEAL_DIVB */
   int    lattice;       /* LBMHD_D1Q3 | LBMHD_D2Q9 | LBMHD_D3Q19 | LBMHD_D2Q5 | LBMHD_D3Q7 */
   int    precision;     /* 64 (fp64 populations and arithmetic) or 32 (fp32 populations and arithmetic) */
   int    nx, ny, nz;    /* unused dims = 1 */
   double gamma;         /* IDEAL: adiabatic index, Eq.8 */
   double c0sq;          /* INCRES: artificial sound speed squared (A3) */
   double nu, eta;       /* if > 0: tau of the velocity (and P) / magnetic sets := 1/2 + D/c_s^2, Eq.5 */
-  double tau[8];        /* per variable, > 1/2, order of `scheme`; all magnetic sets must share one value (A7) */
+  double tau[16];       /* per variable (first K used), > 1/2, order of `scheme`; all magnetic sets must share one value (A7) */
+  double tau_relax;     /* IDEAL_DIVB: relaxation time tau_M of D (Eq.6) in lattice units, > 0 */
   double powell;        /* kappa: 0 = off, 1 = Eq.12 */
   int    bc[6];         /* xmin, xmax, ymin, ymax, zmin, zmax; periodic must be paired per axis */
   int    streaming;     /* LBMHD_STREAM_AB (two population copies) | LBMHD_STREAM_INPLACE (one copy, AA pattern:

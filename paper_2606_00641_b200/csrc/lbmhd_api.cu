@@ -43,7 +43,7 @@ struct Geometry {
 };
 
 bool geometry(int scheme, int lattice, Geometry *g) {
-  if (scheme != LBMHD_IDEAL && scheme != LBMHD_INCRES) return false;
+  if (scheme != LBMHD_IDEAL && scheme != LBMHD_INCRES && scheme != LBMHD_IDEAL_DIVB) return false;
   g->cs2 = 1.0 / 3.0;
   switch (lattice) {
     case LBMHD_D1Q3: g->D = 1; g->Q = 3; break;
@@ -53,10 +53,11 @@ bool geometry(int scheme, int lattice, Geometry *g) {
     case LBMHD_D3Q7: g->D = 3; g->Q = 7; g->cs2 = 0.25; break;
     default: return false;
   }
-  g->K = scheme == LBMHD_IDEAL ? 8 : 1 + 2 * g->D;
-  g->NV = scheme == LBMHD_IDEAL ? 3 : g->D;
+  const bool ideal = scheme != LBMHD_INCRES;
+  g->K = scheme == LBMHD_IDEAL ? 8 : (scheme == LBMHD_IDEAL_DIVB ? 9 : 1 + 2 * g->D);
+  g->NV = ideal ? 3 : g->D;
   g->iU = 1;
-  g->iB = scheme == LBMHD_IDEAL ? 5 : 1 + g->D;
+  g->iB = ideal ? 5 : 1 + g->D;
   return true;
 }
 
@@ -100,7 +101,7 @@ struct lbmhd {
   Geometry g;
   Layout L;
   size_t N;
-  double tau[8];
+  double tau[16];
   cudaStream_t stream;
   char *ws;
   int cur;               // A/B: which population copy holds the current state (in place: always 0)
@@ -218,7 +219,8 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     if (!(h->tau[k] > 0.5)) { delete h; return fail(LBMHD_EINVAL, "tau[%d] = %g must be > 1/2", k, p->tau[k]); }
   for (int b = 1; b < g.NV; b++)
     if (h->tau[g.iB + b] != h->tau[g.iB]) { delete h; return fail(LBMHD_EINVAL, "all magnetic sets must share one tau (A7)"); }
-  if (p->scheme == LBMHD_IDEAL && !(p->gamma > 1.0)) { delete h; return fail(LBMHD_EINVAL, "gamma must be > 1"); }
+  if (p->scheme != LBMHD_INCRES && !(p->gamma > 1.0)) { delete h; return fail(LBMHD_EINVAL, "gamma must be > 1"); }
+  if (p->scheme == LBMHD_IDEAL_DIVB && !(p->tau_relax > 0.0)) { delete h; return fail(LBMHD_EINVAL, "tau_relax must be > 0"); }
   if (!p->workspace) { delete h; return fail(LBMHD_EINVAL, "workspace is NULL"); }
   if (((uintptr_t)p->workspace & 255) != 0) { delete h; return fail(LBMHD_ENOMEM, "workspace must be 256-byte aligned"); }
   if (p->workspace_bytes < L.total) {
@@ -381,6 +383,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     for (int k = 0; k < K; k++) a.omega[k] = (real)(1.0 / h->tau[k]);
     a.inv_tauB_cs2 = (real)(1.0 / (h->tau[h->g.iB] * h->g.cs2));
     a.kappa = (real)h->p.powell; a.gamma = (real)h->p.gamma; a.c0sq = (real)h->p.c0sq;
+    a.inv_tau_relax = h->p.tau_relax > 0.0 ? (real)(1.0 / h->p.tau_relax) : real(0);
     a.mask = h->have_mask ? (const unsigned char *)(h->ws + h->L.off_mask) : nullptr;
     a.Bsolid = h->have_bsolid ? (const double *)(h->ws + h->L.off_bsolid) : nullptr;
     a.dfield = h->have_dfield ? (const double *)(h->ws + h->L.off_dfield) : nullptr;
@@ -518,6 +521,7 @@ template <int LAT, int SCHEME, typename real> OpTable make_table() {
 
 template <int LAT> OpTable pick2(int scheme, int precision) {
   if (scheme == LBMHD_IDEAL) return precision == 64 ? make_table<LAT, kIdeal, double>() : make_table<LAT, kIdeal, float>();
+  if (scheme == LBMHD_IDEAL_DIVB) return precision == 64 ? make_table<LAT, kIdealD, double>() : make_table<LAT, kIdealD, float>();
   return precision == 64 ? make_table<LAT, kIncres, double>() : make_table<LAT, kIncres, float>();
 }
 

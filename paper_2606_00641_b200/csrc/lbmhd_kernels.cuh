@@ -28,9 +28,10 @@ template <typename real> struct StepArgs {
   size_t pstride;               // elements between planes
   int nx, ny, nz;
   int bc[6];
-  real omega[8];                // 1 / tau_k
+  real omega[16];               // 1 / tau_k
   real inv_tauB_cs2;            // 1 / (tau_B c_s^2)
   real kappa, gamma, c0sq;
+  real inv_tau_relax;           // kIdealD: 1 / tau_M of the relaxation variable D (Eq.6)
   const unsigned char *mask;    // [N] or nullptr
   const double *Bsolid;         // [3][N] or nullptr
   const double *dfield;         // lattice porosity d in [0,1] per cell (Eq.15) or nullptr: d from the mask (SOLID -> 0)
@@ -104,7 +105,7 @@ __device__ __forceinline__ double solid_state(const StepArgs<real> &a, int x, in
 template <int SCHEME, int D, typename real>
 __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real c0sq, real Phi[3]) {
   Phi[0] = Phi[1] = Phi[2] = real(0);
-  if (SCHEME == kIdeal) {
+  if (is_ideal(SCHEME)) {
     const real rho = Qh[0], E = Qh[4];
     const real *m = Qh + 1, *B = Qh + 5;
     if (k == 0) {
@@ -114,6 +115,11 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
     }
     const real ir = real(1) / rho;
     const real u[3] = {m[0] * ir, m[1] * ir, m[2] * ir};
+    if (SCHEME == kIdealD && k == 8) {   // relaxation variable D = tr G: D u - B (Eq.10, traced)
+#pragma unroll
+      for (int a = 0; a < D; a++) Phi[a] = Qh[8] * u[a] - B[a];
+      return;
+    }
     if (k >= 5) {   // induction: u_a B_b - B_a u_b
       const int b = k - 5;
       const real Bb = b == 0 ? B[0] : (b == 1 ? B[1] : B[2]);
@@ -182,7 +188,8 @@ template <int K, typename real> __device__ __forceinline__ real pick(const real 
 template <int SCHEME, int D, typename real>
 __device__ __forceinline__ real powell_row(int k, const real *Qv) {
   if (k == 0) return real(0);
-  if (SCHEME == kIdeal) {
+  if (is_ideal(SCHEME)) {
+    if (SCHEME == kIdealD && k == 8) return real(0);
     if (k <= 3) return k == 1 ? Qv[5] : (k == 2 ? Qv[6] : Qv[7]);
     const real ir = real(1) / Qv[0];
     if (k == 4) return (Qv[1] * Qv[5] + Qv[2] * Qv[6] + Qv[3] * Qv[7]) * ir;
@@ -202,7 +209,8 @@ __device__ __forceinline__ real powell_row(int k, const real *Qv) {
 template <int SCHEME, int D, typename real>
 __device__ __forceinline__ void solid_blend(const real *Qv, real gamma, real d, const double uS[3], const double BS[3], real *Qh) {
   const real e = real(1) - d;
-  if (SCHEME == kIdeal) {
+  if (SCHEME == kIdealD) Qh[8] = Qv[8];
+  if (is_ideal(SCHEME)) {
     const real rho = Qv[0];
     const real ir = real(1) / rho;
     const real mu = (Qv[1] * Qv[1] + Qv[2] * Qv[2] + Qv[3] * Qv[3]) * ir;
@@ -411,7 +419,8 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   real tr = real(0);
 #pragma unroll
   for (int b = 0; b < D; b++) tr += sTr[b][tx];
-  const real delta = -tr * a.inv_tauB_cs2;                      // A6
+  // A6: local estimate from tr Pi_B; kIdealD: from the relaxation variable, D ~ tau_M div B (Eq.7)
+  const real delta = SCHEME == kIdealD ? Qv[K - 1] * a.inv_tau_relax : -tr * a.inv_tauB_cs2;
 
   // S4 Powell source, S5 solid blend (rare: own branch so the blended copy of the state costs no registers
   // on the fluid path), S6 flux row of this variable
@@ -427,12 +436,14 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
       flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, Phi);
       // dQh plus the Powell source scaled by the porosity d (A8)
       inj = (pick<K, real>(Qh, k) - Qk) - d * (a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
+      if (SCHEME == kIdealD && k == K - 1) inj = -Qk * a.inv_tau_relax;      // relaxation source of Eq.6, not porosity-scaled
       solid = true;
     }
   }
   if (!solid) {
     flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, Phi);
     inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
+    if (SCHEME == kIdealD && k == K - 1) inj = -Qk * a.inv_tau_relax;        // relaxation source of Eq.6
   }
   // in place: cells next to a non-periodic face publish their post-collision moment (sum_i g'_i = Q_k + inj)
   if (STREAM != ST_AB && c.writeM) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + c.n] = (double)(Qk + inj);
@@ -738,9 +749,12 @@ __device__ __forceinline__ void finish_pair(const StepArgs<float> &a, int tx, in
   float Phi0[3], Phi1[3];
   flux_row<SCHEME, D, float>(k, Qv0, a.gamma, a.c0sq, Phi0);
   flux_row<SCHEME, D, float>(k, Qv1, a.gamma, a.c0sq, Phi1);
-  const float kd = a.kappa * a.inv_tauB_cs2;
-  const float inj0 = (kd * tr0) * powell_row<SCHEME, D, float>(k, Qv0);      // -kappa delta S_row, delta = -tr/(tau_B cs2)
-  const float inj1 = (kd * tr1) * powell_row<SCHEME, D, float>(k, Qv1);
+  // -kappa delta S_row with delta = -tr/(tau_B cs2) (A6) or D/tau_M (kIdealD)
+  const float d0 = SCHEME == kIdealD ? Qv0[K - 1] * a.inv_tau_relax : -tr0 * a.inv_tauB_cs2;
+  const float d1 = SCHEME == kIdealD ? Qv1[K - 1] * a.inv_tau_relax : -tr1 * a.inv_tauB_cs2;
+  float inj0 = -(a.kappa * d0) * powell_row<SCHEME, D, float>(k, Qv0);
+  float inj1 = -(a.kappa * d1) * powell_row<SCHEME, D, float>(k, Qv1);
+  if (SCHEME == kIdealD && k == K - 1) { inj0 = -Qk0 * a.inv_tau_relax; inj1 = -Qk1 * a.inv_tau_relax; }
   if (STREAM != ST_AB) {
     const size_t N = (size_t)a.nx * a.ny * a.nz;
     if (writeM0) a.M_next[(size_t)k * N + n] = (double)(Qk0 + inj0);
@@ -994,7 +1008,7 @@ diag_partial_kernel(const double *__restrict__ F, double *__restrict__ partial, 
     }
     div *= L::inv_cs2;
     maxdiv = fmax(maxdiv, fabs(div));
-    if (SCHEME == kIdeal) {
+    if (is_ideal(SCHEME)) {
       const double rho = v[0];
       const double mu = (v[1] * v[1] + v[2] * v[2] + v[3] * v[3]) / rho;
       const double B2 = v[5] * v[5] + v[6] * v[6] + v[7] * v[7];

@@ -76,12 +76,14 @@ template <class L> __host__ __device__ constexpr int lat_c(int i, int axis) {
   return axis == 0 ? L::cx(i) : (axis == 1 ? L::cy(i) : L::cz(i));
 }
 
-constexpr int kIdeal = 0, kIncres = 1;
+// kIdealD: ideal MHD plus the traced gradient-relaxation variable D = tr G (A19), K = 9
+constexpr int kIdeal = 0, kIncres = 1, kIdealD = 2;
+__host__ __device__ constexpr bool is_ideal(int scheme) { return scheme == kIdeal || scheme == kIdealD; }
 template <int SCHEME, int D> struct Vars {
-  static constexpr int K = SCHEME == kIdeal ? 8 : 1 + 2 * D;
-  static constexpr int NV = SCHEME == kIdeal ? 3 : D;      // vector components carried
+  static constexpr int K = SCHEME == kIdeal ? 8 : (SCHEME == kIdealD ? 9 : 1 + 2 * D);
+  static constexpr int NV = is_ideal(SCHEME) ? 3 : D;      // vector components carried
   static constexpr int iU = 1;                             // first momentum / velocity component
-  static constexpr int iB = SCHEME == kIdeal ? 5 : 1 + D;  // first magnetic component
+  static constexpr int iB = is_ideal(SCHEME) ? 5 : 1 + D;  // first magnetic component
 };
 
 }  // namespace lbk

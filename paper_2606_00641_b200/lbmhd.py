@@ -13,20 +13,20 @@ import numpy as np
 from . import build as _build
 
 D1Q3, D2Q9, D3Q19, D2Q5, D3Q7 = 1, 2, 3, 4, 5
-IDEAL, INCRES = 0, 1
+IDEAL, INCRES, IDEAL_DIVB = 0, 1, 2
 BC_PERIODIC, BC_ZEROGRAD, BC_INFLOW = 0, 1, 2
 CELL_FLUID, CELL_FROZEN, CELL_SOLID = 0, 1, 2
 STREAM_AB, STREAM_INPLACE = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC = 0, -1, -2, -3, -4
 LATTICES = {"D1Q3": D1Q3, "D2Q9": D2Q9, "D3Q19": D3Q19, "D2Q5": D2Q5, "D3Q7": D3Q7}
-SCHEMES = {"IDEAL": IDEAL, "INCRES": INCRES}
+SCHEMES = {"IDEAL": IDEAL, "INCRES": INCRES, "IDEAL_DIVB": IDEAL_DIVB}
 
 
 class LbmhdParams(C.Structure):
     _fields_ = [("scheme", C.c_int), ("lattice", C.c_int), ("precision", C.c_int),
                 ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
                 ("gamma", C.c_double), ("c0sq", C.c_double), ("nu", C.c_double), ("eta", C.c_double),
-                ("tau", C.c_double * 8), ("powell", C.c_double), ("bc", C.c_int * 6),
+                ("tau", C.c_double * 16), ("tau_relax", C.c_double), ("powell", C.c_double), ("bc", C.c_int * 6),
                 ("streaming", C.c_int), ("device", C.c_int), ("stream", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
 
@@ -88,7 +88,7 @@ def _check(rc, allow=()):
 
 
 def make_params(scheme, lattice, shape, precision=64, gamma=5.0 / 3.0, c0sq=1.0 / 36.0, nu=0.0, eta=0.0, tau=0.6,
-                powell=1.0, bc=(0,) * 6, streaming=STREAM_AB, device=0):
+                powell=1.0, bc=(0,) * 6, streaming=STREAM_AB, device=0, tau_relax=0.0):
     p = LbmhdParams()
     p.scheme = SCHEMES.get(scheme, scheme)
     p.lattice = LATTICES.get(lattice, lattice)
@@ -96,9 +96,10 @@ def make_params(scheme, lattice, shape, precision=64, gamma=5.0 / 3.0, c0sq=1.0 
     dims = list(shape) + [1] * (3 - len(shape))
     p.nx, p.ny, p.nz = dims
     p.gamma, p.c0sq, p.nu, p.eta, p.powell = gamma, c0sq, nu, eta, powell
-    taus = [tau] * 8 if np.isscalar(tau) else list(tau) + [0.0] * (8 - len(tau))
-    for k in range(8):
+    taus = [tau] * 16 if np.isscalar(tau) else list(tau) + [0.0] * (16 - len(tau))
+    for k in range(16):
         p.tau[k] = taus[k]
+    p.tau_relax = tau_relax
     for j in range(6):
         p.bc[j] = bc[j]
     p.streaming, p.device = streaming, device
@@ -253,7 +254,7 @@ def from_workload(w, precision=64, device=0, streaming=STREAM_AB):
     """Lbmhd handle configured (boundaries, tau, sphere) for a workloads.py dict; fields not yet initialised."""
     p = make_params(w["scheme"], w["lattice"], w["shape"], precision=precision, gamma=w["gamma"] or 1.4, c0sq=w["c0sq"],
                     nu=w["nu"], eta=w["eta"], tau=w["tau"], powell=w["powell"], bc=w["bc"], streaming=streaming,
-                    device=device)
+                    device=device, tau_relax=w.get("tau_relax", 0.0))
     sim = Lbmhd(p)
     if w.get("sphere"):
         s = w["sphere"]

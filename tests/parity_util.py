@@ -4,14 +4,15 @@ import numpy as np
 from oracle import oracle as orc
 
 LAT_ORC = {"D1Q3": orc.D1Q3, "D2Q9": orc.D2Q9, "D3Q19": orc.D3Q19, "D2Q5": orc.D2Q5, "D3Q7": orc.D3Q7}
+ORC_SCHEME = {"IDEAL": orc.IDEAL, "INCRES": orc.INCRES, "IDEAL_DIVB": orc.IDEAL_DIVB}
 TOL64 = 1e-11      # BASELINE.json north_star: max relative error on all macroscopic fields, fp64
 TOL32 = 1e-5       # fp32
 
 
 def oracle_from_workload(w, mask=None):
-    p = orc.make_params(orc.IDEAL if w["scheme"] == "IDEAL" else orc.INCRES, LAT_ORC[w["lattice"]], w["shape"],
+    p = orc.make_params(ORC_SCHEME[w["scheme"]], LAT_ORC[w["lattice"]], w["shape"],
                         gamma=w["gamma"] or 1.4, c0sq=w["c0sq"], nu=w["nu"], eta=w["eta"], tau=w["tau"],
-                        powell=w["powell"], bc=w["bc"])
+                        powell=w["powell"], bc=w["bc"], tau_relax=w.get("tau_relax", 0.0))
     o = orc.Oracle(p, mask=mask)
     if w.get("sphere"):
         s = w["sphere"]

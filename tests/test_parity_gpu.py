@@ -185,3 +185,37 @@ def test_fp32_paths_parity(scheme, lattice, shape, bc, streaming):
 def test_fp32_config5_small_with_sphere():
     compare(W.get("C5", small=True), 60, tol=TOL32, precision=32)
     compare(W.get("C5", small=True), 61, tol=TOL32, precision=32, streaming=1)
+
+
+def divb_workload(lattice, shape, bc, seed, sphere=None):
+    """IDEAL_DIVB (K = 9): random ideal state plus a random D field"""
+    w = random_workload("IDEAL", lattice, shape, bc, seed=seed, sphere=sphere)
+    rng = np.random.default_rng(seed + 1)
+    w["scheme"] = "IDEAL_DIVB"
+    w["tau_relax"] = 7.5
+    w["fields"] = np.concatenate([w["fields"], 0.05 * (rng.random((1,) + zyx(shape)) - 0.5)])
+    return w
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+@pytest.mark.parametrize("precision,tol", [(64, TOL64), (32, TOL32)])
+@pytest.mark.parametrize("lattice,shape,bc", [("D1Q3", (200,), (1, 1, 0, 0, 0, 0)), ("D2Q9", (150, 37), (0,) * 6),
+                                              ("D3Q19", (200, 12, 9), (2, 1, 0, 0, 0, 0)), ("D3Q7", (100, 12, 9), (1, 1, 1, 1, 0, 0))])
+def test_ideal_divb_scheme_parity(lattice, shape, bc, precision, tol, streaming):
+    """the paper's local gradient evolution (traced): 9th set D, div B = D / tau_M in the Powell source"""
+    w = divb_workload(lattice, shape, bc, seed=21)
+    compare(w, 20, tol=tol, precision=precision, streaming=streaming)
+    compare(w, 7, tol=tol, precision=precision, streaming=streaming)
+
+
+def test_ideal_divb_with_sphere_and_mask():
+    cen = np.array([36.0, 12.0, 10.0])
+    mh = np.array([0.3, -0.5, 0.8]) / np.linalg.norm([0.3, -0.5, 0.8])
+    sph = dict(centre=cen, radius=6.0, u_solid=np.array([-0.25, 0.0, 0.0]), dipole_dir=mh, B_surface=0.03)
+    compare(divb_workload("D3Q19", (72, 24, 20), (2, 1, 0, 0, 0, 0), seed=31, sphere=sph), 12)
+    rng = np.random.default_rng(9)
+    shape = (70, 12, 10)
+    s = zyx(shape)
+    mask = (rng.random(s) < 0.05).astype(np.uint8) * 2
+    compare(divb_workload("D3Q19", shape, (1, 1) + (0,) * 4, seed=41), 12,
+            obstacle=(mask, np.array([0.03, -0.02, 0.01]), 0.1 * (rng.random((3,) + s) - 0.5)), streaming=1)
