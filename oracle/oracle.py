@@ -34,7 +34,7 @@ class OracleParams(C.Structure):
                 ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
                 ("gamma", C.c_double), ("c0sq", C.c_double),
                 ("nu", C.c_double), ("eta", C.c_double),
-                ("tau", C.c_double * 16), ("tau_relax", C.c_double), ("powell", C.c_double), ("bc", C.c_int * 6)]
+                ("tau", C.c_double * 16), ("tau_relax", C.c_double), ("eta_jc", C.c_double), ("powell", C.c_double), ("bc", C.c_int * 6)]
 
 
 _lib = None
@@ -65,6 +65,8 @@ def _load():
         lib.oracle_equilibrium.argtypes = [pp, dp, dp]
         lib.oracle_num_vars.argtypes = [pp]
         lib.oracle_num_dirs.argtypes = [pp]
+        lib.oracle_tau_of_current.argtypes = [C.c_double] * 4
+        lib.oracle_tau_of_current.restype = C.c_double
         lib.oracle_set_threads.argtypes = [C.c_int]
         lib.oracle_set_threads.restype = None
         lib.oracle_get_threads.restype = C.c_int
@@ -81,7 +83,7 @@ def _f64(a):
 
 
 def make_params(scheme, lattice, shape, gamma=5.0 / 3.0, c0sq=1.0 / 12.0, nu=0.0, eta=0.0, tau=0.6,
-                powell=1.0, bc=(0, 0, 0, 0, 0, 0), tau_relax=0.0):
+                powell=1.0, bc=(0, 0, 0, 0, 0, 0), tau_relax=0.0, eta_jc=0.0):
     """shape = (nx,), (nx, ny) or (nx, ny, nz)."""
     p = OracleParams()
     p.scheme, p.lattice = scheme, lattice
@@ -92,6 +94,7 @@ def make_params(scheme, lattice, shape, gamma=5.0 / 3.0, c0sq=1.0 / 12.0, nu=0.0
     for k in range(16):
         p.tau[k] = taus[k]
     p.tau_relax = tau_relax
+    p.eta_jc = eta_jc
     for j in range(6):
         p.bc[j] = bc[j]
     return p
@@ -125,6 +128,10 @@ def equilibrium(params, Qv):
     out = np.zeros((K, Q))
     lib.oracle_equilibrium(C.byref(params), _dptr(Qv), _dptr(out))
     return out
+
+
+def tau_of_current(tau0, e0, a2, jc):
+    return float(_load().oracle_tau_of_current(tau0, e0, a2, jc))
 
 
 def set_threads(n):

@@ -188,6 +188,28 @@ int oracle_equilibrium(const oracle_params *p, const double *Qv, double *feq)
   return 0;
 }
 
+/* ---- current-dependent resistivity (eta(j) = eta0 (1 + (j/j_c)^2); reading A20) ----
+ * The B sets relax with a cell-local tau_B = 1/2 + eta(j)/c_s^2 (Eq.5).  The current comes from the antisymmetric part
+ * of the non-equilibrium first moment of the B sets, N_ab = sum_i c_ia f_{B_b,i} - Phi_{B_b,a} ~ -tau_B c_s^2 d_a B_b:
+ *   a2 := sum_{a<b} (N_ab - N_ba)^2 / c_s^4 = (tau_B |j|)^2.
+ * tau_B then solves  tau = tau0 + e0 a2 / (j_c^2 tau^2),  tau0 = 1/2 + e0, e0 = eta0/c_s^2:  the cubic
+ *   g(tau) = tau^3 - tau0 tau^2 - c = 0,  c = e0 a2 / j_c^2 >= 0,
+ * whose only root >= tau0 is found by NEWTON_ITERS Newton steps from tau0 + cbrt(c) (g >= 0 there, g convex increasing). */
+#define NEWTON_ITERS 6
+static double tau_of_current(double tau0, double e0, double a2, double jc)
+{
+  double c = e0 * a2 / (jc * jc);
+  double t = tau0 + cbrt(c);
+  for (int it = 0; it < NEWTON_ITERS; it++) {
+    double g = (t - tau0) * t * t - c;
+    double dg = t * (3.0 * t - 2.0 * tau0);
+    t = t - g / dg;
+  }
+  return t;
+}
+
+double oracle_tau_of_current(double tau0, double e0, double a2, double jc) { return tau_of_current(tau0, e0, a2, jc); }
+
 /* ---- state ---- */
 struct oracle {
   oracle_params p;
@@ -225,6 +247,7 @@ int oracle_create(const oracle_params *p, const unsigned char *cell_mask, oracle
   if (lattice_make(p->lattice, &L)) return -1;
   if (p->scheme != ORC_IDEAL && p->scheme != ORC_INCRES && p->scheme != ORC_IDEAL_DIVB) return -1;
   if (p->scheme == ORC_IDEAL_DIVB && !(p->tau_relax > 0.0)) return -1;
+  if (p->eta_jc != 0.0 && !(p->scheme == ORC_INCRES && p->eta_jc > 0.0)) return -1;
   if (p->nx < 1 || p->ny < 1 || p->nz < 1) return -1;
   if (L.D < 2 && p->ny != 1) return -1;
   if (L.D < 3 && p->nz != 1) return -1;
@@ -470,7 +493,22 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
   /* 3. local div B estimate (A6): delta = - tr Pi_B / (tau_B c_s^2) */
   double tr = 0.0;
   for (b = 0; b < D; b++) for (i = 0; i < Qn; i++) tr += (double)L->c[i][b] * f[o->iB + b][i];
-  double delta = -tr / (o->tauB * L->cs2);
+  /* A20: cell-local tau_B from the current (INCRES with eta_jc > 0) */
+  double tauB = o->tauB;
+  if (o->p.scheme == ORC_INCRES && o->p.eta_jc > 0.0) {
+    double Phieq[MAXK][3], Pi[3][3], a2 = 0.0;
+    memset(Phieq, 0, sizeof Phieq);
+    flux_eval(o->p.scheme, D, o->p.gamma, o->p.c0sq, Qv, Phieq);
+    for (a = 0; a < D; a++) for (b = 0; b < D; b++) {
+      double m = 0.0;
+      for (i = 0; i < Qn; i++) m += (double)L->c[i][a] * f[o->iB + b][i];
+      Pi[a][b] = m - Phieq[o->iB + b][a];
+    }
+    for (a = 0; a < D; a++) for (b = a + 1; b < D; b++) { double w2 = Pi[a][b] - Pi[b][a]; a2 += w2 * w2; }
+    a2 /= L->cs2 * L->cs2;
+    tauB = tau_of_current(o->tauB, o->tauB - 0.5, a2, o->p.eta_jc);
+  }
+  double delta = -tr / (tauB * L->cs2);
   /* IDEAL_DIVB: div B from the relaxation variable instead, D ~ tau_M div B (Eq.7) */
   if (o->p.scheme == ORC_IDEAL_DIVB) delta = Qv[8] / o->p.tau_relax;
 
@@ -530,7 +568,8 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
   for (k = 0; k < K; k++)
     for (i = 0; i < Qn; i++) {
       double feq = feq_eval(L, i, Qv[k], Phi[k]);
-      dst[((long)k * Qn + i) * N + n] = f[k][i] + o->omega[k] * (feq - f[k][i]) + L->w[i] * (dQh[k] + S[k]);
+      double om = (k >= o->iB && k < o->iB + (is_ideal(o->p.scheme) ? 3 : D) && tauB != o->tauB) ? 1.0 / tauB : o->omega[k];
+      dst[((long)k * Qn + i) * N + n] = f[k][i] + om * (feq - f[k][i]) + L->w[i] * (dQh[k] + S[k]);
     }
 }
 

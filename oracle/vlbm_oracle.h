@@ -38,6 +38,7 @@ typedef struct {
   double nu, eta;  /* if > 0: tau of the velocity / magnetic sets := 1/2 + D / c_s^2 (Eq.5) */
   double tau[16];  /* per variable, > 1/2, variable order of `scheme` */
   double tau_relax; /* IDEAL_DIVB: relaxation time tau_M of the gradient variable D (Eq.6), lattice units, > 0 */
+  double eta_jc;   /* INCRES: critical current j_c of eta(j) = eta0 (1 + (j/j_c)^2), lattice units; 0 = constant eta */
   double powell;   /* kappa: 0 = off, 1 = Eq.12 */
   int bc[6];       /* xmin, xmax, ymin, ymax, zmin, zmax */
 } oracle_params;
@@ -64,6 +65,7 @@ int  oracle_set_porosity(oracle_t *o, const double *d_field /* [N] or NULL */);
 int  oracle_set_sphere_width(oracle_t *o, double eps);
 
 /* test hooks */
+double oracle_tau_of_current(double tau0, double e0, double a2, double jc);
 int  oracle_get_populations(oracle_t *o, double *g_out /* [K][Q][N] */);
 int  oracle_set_populations(oracle_t *o, const double *g_in /* [K][Q][N] */);
 int  oracle_source_log(oracle_t *o, double *acc /* [K]: accumulated sum_x d*S_k over all steps so far */);

@@ -90,7 +90,7 @@ class NpVLBM:
     """fields / populations are indexed [k, (i,) z, y, x]."""
 
     def __init__(self, scheme, lat, shape_zyx, tau, gamma=5 / 3, c0sq=1 / 12, powell=1.0,
-                 bc=(0,) * 6, mask=None, tau_relax=0.0):
+                 bc=(0,) * 6, mask=None, tau_relax=0.0, eta_jc=0.0):
         self.scheme = scheme
         self.D, self.c, self.w, self.cs2 = lattice_np(lat)
         self.Qn = len(self.w)
@@ -98,6 +98,7 @@ class NpVLBM:
         self.K = 8 if scheme == "IDEAL" else (9 if scheme == "IDEAL_DIVB" else 1 + 2 * self.D)
         self.ideal = scheme in ("IDEAL", "IDEAL_DIVB")
         self.tau_relax = tau_relax
+        self.eta_jc = eta_jc
         self.tau = np.broadcast_to(np.asarray(tau, dtype=float), (self.K,)).copy()
         self.gamma, self.c0sq, self.kappa = gamma, c0sq, powell
         self.bc = tuple(bc)
@@ -229,7 +230,27 @@ class NpVLBM:
         tr = np.zeros(self.shape)
         for b in range(D):
             tr += np.tensordot(self.c[:, b].astype(float), f[self.iB + b], axes=([0], [0]))
-        delta = -tr / (self.tau[self.iB] * self.cs2)
+        tauB = self.tau[self.iB] * np.ones(self.shape)
+        if self.scheme == "INCRES" and self.eta_jc > 0:
+            # PAPER.md:215 eta(j) = eta0 (1 + (j/jc)^2): local tau_B from the antisymmetric non-equilibrium moment (A20)
+            Pieq = self.flux(Q)
+            cf = self.c.astype(float)
+            Nab = np.zeros((D, D) + self.shape)
+            for a_ in range(D):
+                for b in range(D):
+                    Nab[a_, b] = np.tensordot(cf[:, a_], f[self.iB + b], axes=([0], [0])) - Pieq[self.iB + b, a_]
+            a2 = np.zeros(self.shape)
+            for a_ in range(D):
+                for b in range(a_ + 1, D):
+                    a2 += (Nab[a_, b] - Nab[b, a_]) ** 2
+            a2 /= self.cs2 ** 2
+            tau0 = self.tau[self.iB]
+            cc = (tau0 - 0.5) * a2 / self.eta_jc ** 2
+            t = tau0 + np.cbrt(cc)
+            for _ in range(60):                       # converged root of t^3 - tau0 t^2 - c (the oracle does 6 Newton steps)
+                t = t - ((t - tau0) * t * t - cc) / (t * (3 * t - 2 * tau0))
+            tauB = t
+        delta = -tr / (tauB * self.cs2)
         if self.scheme == "IDEAL_DIVB":
             delta = Q[8] / self.tau_relax            # Eq.7: D ~ tau_M div B
         # 4. Powell source
@@ -274,7 +295,9 @@ class NpVLBM:
             S = S * d
         # 6./7. flux, BGK, injection
         feq = self.feq(Q, self.flux(Qh))
-        om = (1.0 / self.tau).reshape((K, 1) + (1,) * len(self.shape))
+        om = (1.0 / self.tau).reshape((K, 1) + (1,) * len(self.shape)) * np.ones((K, 1) + self.shape)
+        if self.scheme == "INCRES" and self.eta_jc > 0:
+            om[self.iB:self.iB + D, 0] = 1.0 / tauB
         wv = self.w.reshape((1, Qn) + (1,) * len(self.shape))
         gnew = f + om * (feq - f) + wv * (dQh + S)[:, None]
         fr = self._frozen()
