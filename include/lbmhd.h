@@ -62,6 +62,8 @@ typedef struct {
   double nu, eta;       /* if > 0: tau of the velocity (and P) / magnetic sets := 1/2 + D/c_s^2, Eq.5 */
   double tau[16];       /* per variable (first K used), > 1/2, order of `scheme`; all magnetic sets must share one value (A7) */
   double tau_relax;     /* IDEAL_DIVB: relaxation time tau_M of D (Eq.6) in lattice units, > 0 */
+  double eta_jc;        /* INCRES: critical current j_c of eta(j) = eta0 (1 + (j/j_c)^2) (eta0 from `eta` or tau),
+                           lattice units; 0 = constant resistivity */
   double powell;        /* kappa: 0 = off, 1 = Eq.12 */
   int    bc[6];         /* xmin, xmax, ymin, ymax, zmin, zmax; periodic must be paired per axis */
   int    streaming;     /* LBMHD_STREAM_AB (two population copies) | LBMHD_STREAM_INPLACE (one copy, AA pattern:

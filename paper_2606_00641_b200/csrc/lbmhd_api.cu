@@ -221,6 +221,7 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     if (h->tau[g.iB + b] != h->tau[g.iB]) { delete h; return fail(LBMHD_EINVAL, "all magnetic sets must share one tau (A7)"); }
   if (p->scheme != LBMHD_INCRES && !(p->gamma > 1.0)) { delete h; return fail(LBMHD_EINVAL, "gamma must be > 1"); }
   if (p->scheme == LBMHD_IDEAL_DIVB && !(p->tau_relax > 0.0)) { delete h; return fail(LBMHD_EINVAL, "tau_relax must be > 0"); }
+  if (p->eta_jc != 0.0 && !(p->scheme == LBMHD_INCRES && p->eta_jc > 0.0)) { delete h; return fail(LBMHD_EINVAL, "eta_jc needs the INCRES scheme and must be > 0"); }
   if (!p->workspace) { delete h; return fail(LBMHD_EINVAL, "workspace is NULL"); }
   if (((uintptr_t)p->workspace & 255) != 0) { delete h; return fail(LBMHD_ENOMEM, "workspace must be 256-byte aligned"); }
   if (p->workspace_bytes < L.total) {
@@ -239,7 +240,7 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
     if (e != cudaSuccess) { delete h; return fail(LBMHD_ECUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e)); }
     h->num_sms = sms;
-    h->pair = p->precision == 32 && p->nx % 2 == 0;
+    h->pair = p->precision == 32 && p->nx % 2 == 0 && p->eta_jc == 0.0;      // eta(j) runs on the one-cell kernels
     if (const char *e3 = getenv("LBMHD_PAIR")) h->pair = h->pair && atoi(e3) != 0;
     h->split = false;   // measured slower on config 5: edge tiles lose DRAM page locality when launched apart from their rows
     if (const char *e2 = getenv("LBMHD_SPLIT")) h->split = atoi(e2) != 0;
@@ -384,6 +385,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     a.inv_tauB_cs2 = (real)(1.0 / (h->tau[h->g.iB] * h->g.cs2));
     a.kappa = (real)h->p.powell; a.gamma = (real)h->p.gamma; a.c0sq = (real)h->p.c0sq;
     a.inv_tau_relax = h->p.tau_relax > 0.0 ? (real)(1.0 / h->p.tau_relax) : real(0);
+    a.etaj_inv_jc2 = h->p.eta_jc > 0.0 ? (real)(1.0 / (h->p.eta_jc * h->p.eta_jc)) : real(0);
+    a.tauB0 = (real)h->tau[h->g.iB];
     a.mask = h->have_mask ? (const unsigned char *)(h->ws + h->L.off_mask) : nullptr;
     a.Bsolid = h->have_bsolid ? (const double *)(h->ws + h->L.off_bsolid) : nullptr;
     a.dfield = h->have_dfield ? (const double *)(h->ws + h->L.off_dfield) : nullptr;

@@ -32,6 +32,8 @@ template <typename real> struct StepArgs {
   real inv_tauB_cs2;            // 1 / (tau_B c_s^2)
   real kappa, gamma, c0sq;
   real inv_tau_relax;           // kIdealD: 1 / tau_M of the relaxation variable D (Eq.6)
+  real etaj_inv_jc2;            // kIncres: 1 / j_c^2 of eta(j) = eta0 (1 + (j/j_c)^2), 0 = constant eta
+  real tauB0;                   // tau of the magnetic sets at zero current
   const unsigned char *mask;    // [N] or nullptr
   const double *Bsolid;         // [3][N] or nullptr
   const double *dfield;         // lattice porosity d in [0,1] per cell (Eq.15) or nullptr: d from the mask (SOLID -> 0)
@@ -334,7 +336,7 @@ __device__ __forceinline__ void frozen_rematerialise(const StepArgs<real> &a, in
 // =====================================================================================================
 // Everything after the pull: boundary substitution (A9), moments exchange, div-B estimate, Powell source,
 // solid blend, flux, BGK + direct injection, store (DESIGN.md §2 steps S2-S8; Eq.2-4, 8, 11-14).
-// sQ[K][TX], sTr[D][TX] are shared arrays of the TX*K threads that call this together; `sync` is their
+// sQ[K][TX], sTr[D*D][TX] are shared arrays of the TX*K threads that call this together; `sync` is their
 // barrier (__syncthreads or a named barrier).  BND / SOLID are tile-uniform: the interior fluid tile (both
 // false) is the hot path and carries no boundary predicates, no mask or sphere test.  `store` says where
 // result j goes (streaming layout); STREAM only selects where Q^nb comes from.
@@ -394,21 +396,27 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   sQ[k][tx] = Qk;
   if (k >= iB && k < iB + D) {
     const int b = k - iB;   // warp-uniform
-    real t = real(0);
-    if (b == 0) {
+    // first moment of this B set, Pi_{a,b} = sum_i c_ia f_i: the diagonal entry is its share of tr Pi_B (A6); the
+    // resistive scheme keeps all D entries, their antisymmetric part gives the current (A20)
+    real m[3] = {real(0), real(0), real(0)};
+    if (SCHEME == kIncres || b == 0) {
 #pragma unroll
       for (int i = 0; i < Q; i++)
-        if (L::cx(i) != 0) t += real(L::cx(i)) * f[i];
-    } else if (b == 1) {
-#pragma unroll
-      for (int i = 0; i < Q; i++)
-        if (L::cy(i) != 0) t += real(L::cy(i)) * f[i];
-    } else {
-#pragma unroll
-      for (int i = 0; i < Q; i++)
-        if (L::cz(i) != 0) t += real(L::cz(i)) * f[i];
+        if (L::cx(i) != 0) m[0] += real(L::cx(i)) * f[i];
     }
-    sTr[b][tx] = t;
+    if (D > 1 && (SCHEME == kIncres || b == 1)) {
+#pragma unroll
+      for (int i = 0; i < Q; i++)
+        if (L::cy(i) != 0) m[1] += real(L::cy(i)) * f[i];
+    }
+    if (D > 2 && (SCHEME == kIncres || b == 2)) {
+#pragma unroll
+      for (int i = 0; i < Q; i++)
+        if (L::cz(i) != 0) m[2] += real(L::cz(i)) * f[i];
+    }
+#pragma unroll
+    for (int al = 0; al < D; al++)
+      if (SCHEME == kIncres || al == b) sTr[b * D + al][tx] = m[al];
   }
   sync();
   if (!work) return;
@@ -418,9 +426,32 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   for (int l = 0; l < K; l++) Qv[l] = sQ[l][tx];
   real tr = real(0);
 #pragma unroll
-  for (int b = 0; b < D; b++) tr += sTr[b][tx];
+  for (int b = 0; b < D; b++) tr += sTr[b * D + b][tx];
+  // A20: current-dependent resistivity -> cell-local tau_B (6 Newton steps on tau^3 - tau0 tau^2 - c = 0 from tau0 + cbrt(c))
+  real inv_tauB_cs2 = a.inv_tauB_cs2;
+  real omB = real(0);
+  if (SCHEME == kIncres && a.etaj_inv_jc2 > real(0)) {
+    real a2 = real(0);
+#pragma unroll
+    for (int al = 0; al < D; al++)
+#pragma unroll
+      for (int be = al + 1; be < D; be++) {
+        // N_ab = Pi_ab - Phi_{B_b,a},  Phi_{B_b,a} = u_a B_b - B_a u_b  (antisymmetric in a <-> b)
+        const real phi = Qv[1 + al] * Qv[1 + D + be] - Qv[1 + D + al] * Qv[1 + be];
+        const real w2 = (sTr[be * D + al][tx] - phi) - (sTr[al * D + be][tx] + phi);
+        a2 += w2 * w2;
+      }
+    a2 *= real(L::inv_cs2 * L::inv_cs2);
+    const real tau0 = a.tauB0;
+    const real cc = (tau0 - real(0.5)) * a2 * a.etaj_inv_jc2;
+    real t = tau0 + cbrt(cc);
+#pragma unroll
+    for (int it = 0; it < 6; it++) t = t - ((t - tau0) * t * t - cc) / (t * (real(3) * t - real(2) * tau0));
+    omB = real(1) / t;
+    inv_tauB_cs2 = omB * real(L::inv_cs2);
+  }
   // A6: local estimate from tr Pi_B; kIdealD: from the relaxation variable, D ~ tau_M div B (Eq.7)
-  const real delta = SCHEME == kIdealD ? Qv[K - 1] * a.inv_tau_relax : -tr * a.inv_tauB_cs2;
+  const real delta = SCHEME == kIdealD ? Qv[K - 1] * a.inv_tau_relax : -tr * inv_tauB_cs2;
 
   // S4 Powell source, S5 solid blend (rare: own branch so the blended copy of the state costs no registers
   // on the fluid path), S6 flux row of this variable
@@ -450,7 +481,7 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
 
   // S7 BGK + direct injection, S8 store:
   //   g'_i = (1 - w) f_i + w_i [ w Q_k + inj ] + w_i (c_i . 3 w Phi)       (w = omega_k; Eq.2-3, 3 = 1/c_s^2)
-  const real om = a.omega[k];
+  const real om = (SCHEME == kIncres && omB > real(0) && k >= iB) ? omB : a.omega[k];
   const real omc = real(1) - om;
   const real b0 = om * Qk + inj;
   const real P0 = real(L::inv_cs2) * om * Phi[0], P1 = real(L::inv_cs2) * om * Phi[1], P2 = real(L::inv_cs2) * om * Phi[2];
@@ -677,7 +708,7 @@ step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int 
   using L = Lattice<LAT>;
   constexpr int D = L::D, K = Vars<SCHEME, D>::K;
   __shared__ real sQ[K][TX];
-  __shared__ real sTr[D][TX];
+  __shared__ real sTr[D * D][TX];
   run_tile<LAT, SCHEME, real, TX, MODE, STREAM>(a, threadIdx.x, threadIdx.y, (r.bx0 + (int)blockIdx.x * r.bxs) * TX,
                                                 r.y0 + (int)blockIdx.y * r.ys, r.z0 + (int)blockIdx.z * r.zs, sphere_only, sQ, sTr);
 }
@@ -731,7 +762,7 @@ __device__ __forceinline__ void finish_pair(const StepArgs<float> &a, int tx, in
       const int cb = lat_c<L>(i, 0) * (b == 0) + lat_c<L>(i, 1) * (b == 1) + lat_c<L>(i, 2) * (b == 2);
       if (lat_c<L>(i, 0) != 0 || lat_c<L>(i, 1) != 0 || lat_c<L>(i, 2) != 0) { t0 += float(cb) * f0[i]; t1 += float(cb) * f1[i]; }
     }
-    *reinterpret_cast<float2 *>(&sTr[b][2 * tx]) = make_float2(t0, t1);
+    *reinterpret_cast<float2 *>(&sTr[b * D + b][2 * tx]) = make_float2(t0, t1);
   }
   __syncthreads();
   float Qv0[K], Qv1[K];
@@ -743,7 +774,7 @@ __device__ __forceinline__ void finish_pair(const StepArgs<float> &a, int tx, in
   float tr0 = 0.f, tr1 = 0.f;
 #pragma unroll
   for (int b = 0; b < D; b++) {
-    const float2 t = *reinterpret_cast<const float2 *>(&sTr[b][2 * tx]);
+    const float2 t = *reinterpret_cast<const float2 *>(&sTr[b * D + b][2 * tx]);
     tr0 += t.x; tr1 += t.y;
   }
   float Phi0[3], Phi1[3];
@@ -783,7 +814,7 @@ step_kernel_pair(const __grid_constant__ StepArgs<float> a, const int npair) {
   using V = Vars<SCHEME, D>;
   constexpr int K = V::K;
   __shared__ float sQ[K][64];
-  __shared__ float sTr[D][64];
+  __shared__ float sTr[D * D][64];
   const int tx = threadIdx.x, k = threadIdx.y;
   // row layout: [32-cell edge tile][npair 64-cell pair tiles][rest in 32-cell tiles], one block each, so that the pair
   // tiles are all interior when the row is; blocks 0..npair-1 are the pair tiles, block npair the first edge tile

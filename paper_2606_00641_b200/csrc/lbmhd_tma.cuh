@@ -78,7 +78,7 @@ template <int LAT, int SCHEME, typename real, int TXT, int NSTAGE> struct TmaCfg
   static constexpr size_t STAGE_BYTES = slot_off(Q);
   static constexpr size_t OFF_SQ = (size_t)NSTAGE * STAGE_BYTES;
   static constexpr size_t OFF_STR = OFF_SQ + (size_t)NGROUP * K * TXT * sizeof(real);
-  static constexpr size_t OFF_BAR = OFF_STR + (size_t)NGROUP * D * TXT * sizeof(real);
+  static constexpr size_t OFF_BAR = OFF_STR + (size_t)NGROUP * D * D * TXT * sizeof(real);
   static constexpr size_t SMEM_BYTES = OFF_BAR + 2 * NSTAGE * sizeof(uint64_t) + 128;   // + alignment slack
 };
 
@@ -149,7 +149,7 @@ step_kernel_tma(const __grid_constant__ StepArgs<real> a, const __grid_constant_
   const int lt = tid - g * C::GROUP;
   const int tx = lt % TXT, k = lt / TXT;
   real(*sQ)[TXT] = (real(*)[TXT])(smem + C::OFF_SQ + (size_t)g * K * TXT * sizeof(real));
-  real(*sTr)[TXT] = (real(*)[TXT])(smem + C::OFF_STR + (size_t)g * D * TXT * sizeof(real));
+  real(*sTr)[TXT] = (real(*)[TXT])(smem + C::OFF_STR + (size_t)g * D * D * TXT * sizeof(real));
   const uint32_t ps = (uint32_t)a.pstride;
   const real *__restrict__ srck = a.src + (size_t)k * Q * a.pstride;
   real *__restrict__ dstk = a.dst + (size_t)k * Q * a.pstride;

@@ -26,7 +26,7 @@ class LbmhdParams(C.Structure):
     _fields_ = [("scheme", C.c_int), ("lattice", C.c_int), ("precision", C.c_int),
                 ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
                 ("gamma", C.c_double), ("c0sq", C.c_double), ("nu", C.c_double), ("eta", C.c_double),
-                ("tau", C.c_double * 16), ("tau_relax", C.c_double), ("powell", C.c_double), ("bc", C.c_int * 6),
+                ("tau", C.c_double * 16), ("tau_relax", C.c_double), ("eta_jc", C.c_double), ("powell", C.c_double), ("bc", C.c_int * 6),
                 ("streaming", C.c_int), ("device", C.c_int), ("stream", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
 
@@ -88,7 +88,7 @@ def _check(rc, allow=()):
 
 
 def make_params(scheme, lattice, shape, precision=64, gamma=5.0 / 3.0, c0sq=1.0 / 36.0, nu=0.0, eta=0.0, tau=0.6,
-                powell=1.0, bc=(0,) * 6, streaming=STREAM_AB, device=0, tau_relax=0.0):
+                powell=1.0, bc=(0,) * 6, streaming=STREAM_AB, device=0, tau_relax=0.0, eta_jc=0.0):
     p = LbmhdParams()
     p.scheme = SCHEMES.get(scheme, scheme)
     p.lattice = LATTICES.get(lattice, lattice)
@@ -100,6 +100,7 @@ def make_params(scheme, lattice, shape, precision=64, gamma=5.0 / 3.0, c0sq=1.0 
     for k in range(16):
         p.tau[k] = taus[k]
     p.tau_relax = tau_relax
+    p.eta_jc = eta_jc
     for j in range(6):
         p.bc[j] = bc[j]
     p.streaming, p.device = streaming, device
@@ -254,7 +255,7 @@ def from_workload(w, precision=64, device=0, streaming=STREAM_AB):
     """Lbmhd handle configured (boundaries, tau, sphere) for a workloads.py dict; fields not yet initialised."""
     p = make_params(w["scheme"], w["lattice"], w["shape"], precision=precision, gamma=w["gamma"] or 1.4, c0sq=w["c0sq"],
                     nu=w["nu"], eta=w["eta"], tau=w["tau"], powell=w["powell"], bc=w["bc"], streaming=streaming,
-                    device=device, tau_relax=w.get("tau_relax", 0.0))
+                    device=device, tau_relax=w.get("tau_relax", 0.0), eta_jc=w.get("eta_jc", 0.0))
     sim = Lbmhd(p)
     if w.get("sphere"):
         s = w["sphere"]

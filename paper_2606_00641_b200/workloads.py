@@ -82,7 +82,7 @@ def _fourier_potential(rng, n, nmodes=8, kmax=4):
     return psi
 
 
-def config2(n=512, steps=1000, rms=0.02, nu=1e-3, eta=1e-3, c0sq=1.0 / 36.0):
+def config2(n=512, steps=1000, rms=0.02, nu=1e-3, eta=1e-3, c0sq=1.0 / 36.0, eta_jc=0.0):
     """C2: 2D incompressible resistive MHD, D2Q9, periodic, 8 random Fourier modes |k| <= 4, lattice units."""
     rng = _rng(2)
     ux, uy = _curl_h(_fourier_potential(rng, n))
@@ -92,7 +92,7 @@ def config2(n=512, steps=1000, rms=0.02, nu=1e-3, eta=1e-3, c0sq=1.0 / 36.0):
     F = np.stack([np.zeros_like(ux), su * ux, su * uy, sb * Bx, sb * By])[:, None]
     return dict(name="C2", scheme="INCRES", lattice="D2Q9", shape=(n, n), gamma=0.0, c0sq=c0sq, nu=nu, eta=eta,
                 tau=0.5 + 3.0 * nu, powell=1.0, bc=(0,) * 6, steps=steps, fields=np.ascontiguousarray(F), sphere=None,
-                scale=1.0)
+                scale=1.0, eta_jc=eta_jc)      # eta_jc > 0: the paper's eta(j) = eta0 (1 + (j/j_c)^2), lattice units
 
 
 def config3(n=1024, steps=2000, cfl=0.1, tau=0.505):

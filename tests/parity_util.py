@@ -12,7 +12,7 @@ TOL32 = 1e-5       # fp32
 def oracle_from_workload(w, mask=None):
     p = orc.make_params(ORC_SCHEME[w["scheme"]], LAT_ORC[w["lattice"]], w["shape"],
                         gamma=w["gamma"] or 1.4, c0sq=w["c0sq"], nu=w["nu"], eta=w["eta"], tau=w["tau"],
-                        powell=w["powell"], bc=w["bc"], tau_relax=w.get("tau_relax", 0.0))
+                        powell=w["powell"], bc=w["bc"], tau_relax=w.get("tau_relax", 0.0), eta_jc=w.get("eta_jc", 0.0))
     o = orc.Oracle(p, mask=mask)
     if w.get("sphere"):
         s = w["sphere"]

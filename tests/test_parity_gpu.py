@@ -219,3 +219,24 @@ def test_ideal_divb_with_sphere_and_mask():
     mask = (rng.random(s) < 0.05).astype(np.uint8) * 2
     compare(divb_workload("D3Q19", shape, (1, 1) + (0,) * 4, seed=41), 12,
             obstacle=(mask, np.array([0.03, -0.02, 0.01]), 0.1 * (rng.random((3,) + s) - 0.5)), streaming=1)
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+@pytest.mark.parametrize("precision,tol", [(64, TOL64), (32, TOL32)])
+@pytest.mark.parametrize("lattice,shape,bc", [("D2Q9", (150, 37), (0,) * 6), ("D2Q9", (90, 21), (1, 1, 2, 1, 0, 0)),
+                                              ("D3Q19", (100, 12, 9), (0,) * 6), ("D2Q5", (150, 37), (1, 1, 0, 0, 0, 0))])
+def test_eta_of_j_parity(lattice, shape, bc, precision, tol, streaming):
+    """INCRES with current-dependent resistivity: cell-local tau_B from the local current (A20)"""
+    w = random_workload("INCRES", lattice, shape, bc, seed=51)
+    w["eta_jc"] = 0.02
+    w["tau"] = [0.7] + [0.6] * len(shape) + [0.55] * len(shape)
+    compare(w, 20, tol=tol, precision=precision, streaming=streaming)
+    # the feature is live on this data: the constant-eta run differs
+    w0 = dict(w, eta_jc=0.0)
+    a, b = gpu_from_workload(w), gpu_from_workload(w0)
+    for sim in (a, b):
+        sim.init(w["fields"])
+        sim.step(5)
+    assert np.abs(a.moments()[0] - b.moments()[0]).max() > 1e-7
+    a.close()
+    b.close()
