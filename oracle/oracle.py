@@ -57,6 +57,7 @@ def _load():
         lib.oracle_set_sphere.argtypes = [C.c_void_p, dp, C.c_double, dp, dp, C.c_double]
         lib.oracle_set_porosity.argtypes = [C.c_void_p, dp]
         lib.oracle_set_sphere_width.argtypes = [C.c_void_p, C.c_double]
+        lib.oracle_set_sphere_rotation.argtypes = [C.c_void_p, dp]
         lib.oracle_get_populations.argtypes = [C.c_void_p, dp]
         lib.oracle_set_populations.argtypes = [C.c_void_p, dp]
         lib.oracle_source_log.argtypes = [C.c_void_p, dp]
@@ -209,6 +210,11 @@ class Oracle:
     def set_sphere_width(self, eps):
         if self.lib.oracle_set_sphere_width(self.h, float(eps)):
             raise RuntimeError("oracle_set_sphere_width")
+
+    def set_sphere_rotation(self, omega):
+        om = _f64(omega)
+        if self.lib.oracle_set_sphere_rotation(self.h, _dptr(om)):
+            raise RuntimeError("oracle_set_sphere_rotation")
 
     def populations(self):
         g = np.zeros((self.K, self.Q) + self.shape)

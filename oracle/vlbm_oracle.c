@@ -228,6 +228,7 @@ struct oracle {
   int has_sphere;
   double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs;
   long sph_t0;         /* step count at which the centre was sph_c0 */
+  double sph_om[3];    /* angular velocity Omega of the body (rad per step): u^B(x) = u_s + Omega x r, dipole axis co-rotates */
   double sph_eps;      /* width eps_h of the linear porosity ramp across the sphere surface (Eq.15-16), 0 = sharp */
   double *dfield;      /* lattice porosity d in [0,1] per cell (Eq.15), or NULL: d from the mask (SOLID -> 0) */
   long t;              /* steps done so far */
@@ -336,6 +337,13 @@ int oracle_set_porosity(oracle_t *o, const double *d_field)
   return 0;
 }
 
+int oracle_set_sphere_rotation(oracle_t *o, const double omega[3])
+{
+  if (!o || !omega) return -1;
+  for (int a = 0; a < 3; a++) o->sph_om[a] = omega[a];
+  return 0;
+}
+
 int oracle_set_sphere_width(oracle_t *o, double eps)
 {
   if (!o || !(eps >= 0.0)) return -1;
@@ -400,6 +408,16 @@ static double solid_state(const oracle_t *o, int x, int y, int z, long n, double
       r[a] = a < o->L.D ? xi[a] - c : 0.0;
       r2 = r2 + r[a] * r[a];
     }
+    /* dipole axis at this step: m0 rotated about Omega by |Omega| (t - t0) (Rodrigues) */
+    double mt[3] = { o->sph_m[0], o->sph_m[1], o->sph_m[2] };
+    double om2 = o->sph_om[0] * o->sph_om[0] + o->sph_om[1] * o->sph_om[1] + o->sph_om[2] * o->sph_om[2];
+    if (om2 > 0.0) {
+      double omn = sqrt(om2), th = omn * dt, cth = cos(th), sth = sin(th);
+      double e[3] = { o->sph_om[0] / omn, o->sph_om[1] / omn, o->sph_om[2] / omn };
+      double em = e[0] * mt[0] + e[1] * mt[1] + e[2] * mt[2];
+      double ex[3] = { e[1] * mt[2] - e[2] * mt[1], e[2] * mt[0] - e[0] * mt[2], e[0] * mt[1] - e[1] * mt[0] };
+      for (int a = 0; a < 3; a++) mt[a] = o->sph_m[a] * cth + ex[a] * sth + e[a] * em * (1.0 - cth);
+    }
     double rn = sqrt(r2);
     double d;
     if (o->sph_eps > 0.0) {
@@ -414,8 +432,12 @@ static double solid_state(const oracle_t *o, int x, int y, int z, long n, double
       double q = o->sph_R / rc;
       double amp = 0.5 * o->sph_Bs * (q * q * q);
       double rh[3], mr = 0.0;
-      for (int a = 0; a < 3; a++) { rh[a] = rn > 0.0 ? r[a] / rn : 0.0; mr += o->sph_m[a] * rh[a]; }
-      for (int a = 0; a < 3; a++) { BB[a] = amp * (3.0 * mr * rh[a] - o->sph_m[a]); uB[a] = o->sph_u[a]; }
+      for (int a = 0; a < 3; a++) { rh[a] = rn > 0.0 ? r[a] / rn : 0.0; mr += mt[a] * rh[a]; }
+      for (int a = 0; a < 3; a++) BB[a] = amp * (3.0 * mr * rh[a] - mt[a]);
+      /* rigid body: u^B = u_s + Omega x r ("rotated around a ... tilt vector") */
+      uB[0] = o->sph_u[0] + (o->sph_om[1] * r[2] - o->sph_om[2] * r[1]);
+      uB[1] = o->sph_u[1] + (o->sph_om[2] * r[0] - o->sph_om[0] * r[2]);
+      uB[2] = o->sph_u[2] + (o->sph_om[0] * r[1] - o->sph_om[1] * r[0]);
       return d;
     }
   }

@@ -63,6 +63,8 @@ int  oracle_set_sphere(oracle_t *o, const double centre[3], double radius, const
  * linear ramp of width eps across the sphere surface (0 = sharp) */
 int  oracle_set_porosity(oracle_t *o, const double *d_field /* [N] or NULL */);
 int  oracle_set_sphere_width(oracle_t *o, double eps);
+/* rigid rotation of the sphere: u^B(x) = u_solid + omega x (x - c), dipole axis rotates with the body */
+int  oracle_set_sphere_rotation(oracle_t *o, const double omega[3]);
 
 /* test hooks */
 double oracle_tau_of_current(double tau0, double e0, double a2, double jc);

@@ -108,6 +108,7 @@ class NpVLBM:
         self.B_solid = None
         self.sphere = None
         self.sphere_eps = 0.0
+        self.sphere_omega = np.zeros(3)
         self.d_field = None
         self.t = 0
         self.src_acc = np.zeros(self.K)
@@ -186,11 +187,18 @@ class NpVLBM:
             rc = np.maximum(rn, 0.5 * R)
             with np.errstate(invalid="ignore", divide="ignore"):
                 rh = np.where(rn > 0, r / np.where(rn > 0, rn, 1.0), 0.0)
+            om = np.asarray(self.sphere_omega, dtype=float)
+            omn = np.linalg.norm(om)
+            if omn > 0:                                  # Rodrigues rotation of the dipole axis by |Omega| (t - t0)
+                e, th = om / omn, omn * (self.t - t0)
+                mh = mh * np.cos(th) + np.cross(e, mh) * np.sin(th) + e * (e @ mh) * (1 - np.cos(th))
+            urot = np.cross(om.reshape(1, 1, 1, 3), np.moveaxis(r, 0, -1))     # Omega x r
+            urot = np.moveaxis(urot, -1, 0)
             mr = (mh.reshape(3, 1, 1, 1) * rh).sum(0)
             dip = 0.5 * Bs * (R / rc) ** 3 * (3.0 * mr * rh - mh.reshape(3, 1, 1, 1))
             d[ins] = ds[ins]
             for a in range(3):
-                uB[a][ins] = us[a]
+                uB[a][ins] = us[a] + urot[a][ins]
                 BB[a][ins] = dip[a][ins]
         return d, uB, BB
 

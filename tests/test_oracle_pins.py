@@ -336,3 +336,31 @@ def test_porosity_limits_and_half_cell():
     assert np.allclose(Q[1:4, 2, 3, 4], 1.3 * 0.5 * us, rtol=0, atol=1e-16)
     assert np.allclose(Q[5:8, 2, 3, 4], 0.5 * B0, rtol=0, atol=1e-16)
     assert abs(Q[0, 2, 3, 4] - 1.3) < 1e-15
+
+
+def test_P6_numpy_bruteforce_rotating_smooth_sphere():
+    """rigid rotation: u^B = u_s + Omega x r, dipole axis co-rotating; against the array writing"""
+    rng = np.random.default_rng(707)
+    shape = (14, 12, 10)
+    o, n = make_pair("IDEAL", "D3Q19", shape, 0.7, bc=(2, 1, 0, 0, 0, 0))
+    cen, us = np.array([7.3, 6.1, 5.2]), np.array([-0.2, 0.05, 0.0])
+    mh = np.array([0.3, -0.5, 0.8]) / np.linalg.norm([0.3, -0.5, 0.8])
+    om = np.array([0.02, 0.0, 0.02])
+    o.set_sphere(cen, 3.0, us, mh, 0.03)
+    o.set_sphere_width(1.0)
+    o.set_sphere_rotation(om)
+    n.sphere, n.sphere_eps, n.sphere_omega = (cen, 3.0, us, mh, 0.03, 0), 1.0, om
+    F = random_fields(rng, "IDEAL", "D3Q19", shape)
+    o.init(F)
+    n.init(F)
+    for st in range(6):
+        o.step(1)
+        n.step(1)
+        assert np.abs(o.populations() - n.g).max() < 1e-14, st
+    # a fully solid cell moves with u_s + Omega x r exactly (post-collision momentum = rho u^B)
+    Q = o.moments(diag=False)
+    d, uB, BB = n._solid.__func__(_at(n, n.t - 1))
+    core = d == 0
+    assert core.sum() > 10 and np.abs(uB[:, core] - us.reshape(3, 1)).max() > 1e-3
+    for b in range(3):
+        assert np.abs(Q[1 + b][core] - Q[0][core] * uB[b][core]).max() < 1e-15
