@@ -127,6 +127,10 @@ int lbmhd_set_sphere(lbmhd_t *h, const double centre[3], double radius, const do
 int lbmhd_set_porosity(lbmhd_t *h, const double *d_field, int on_device);
 int lbmhd_set_sphere_width(lbmhd_t *h, double eps);
 
+/* Rigid rotation of the sphere: u^B(x) = u_solid + omega x (x - c), omega HOST double[3] in radians per
+ * step; the dipole axis rotates with the body about omega, counted from the step lbmhd_set_sphere was called at. */
+int lbmhd_set_sphere_rotation(lbmhd_t *h, const double omega[3]);
+
 /* Raw population access (checkpoint / tests): fp64 [K][Q][N] at this boundary in both precisions, in
  * canonical (k, i, cell) order whatever the streaming layout.  HOST or DEVICE pointer per on_device. */
 int lbmhd_get_populations(lbmhd_t *h, double *g_out, int on_device);

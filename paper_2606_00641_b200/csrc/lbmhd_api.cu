@@ -112,7 +112,7 @@ struct lbmhd {
   bool have_mask, have_bsolid, have_dfield;
   double usolid[3];
   bool has_sphere;
-  double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs, sph_eps;
+  double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs, sph_eps, sph_om[3];
   long long sph_t0;
   int tx, minb;          // x-tile and min blocks/SM (launch bound) of the plain step kernel
   bool pair;             // fp32: two cells per thread (even nx); LBMHD_PAIR=0 turns it off
@@ -422,6 +422,17 @@ template <int LAT, int SCHEME, typename real> struct Ops {
         for (int c = 0; c < 3; c++) {
           const volatile double prod = dt * h->sph_u[c];
           a.sph_c[c] = h->sph_c0[c] + prod;
+          a.sph_om[c] = h->sph_om[c];
+          a.sph_m[c] = h->sph_m[c];
+        }
+        const double om2 = h->sph_om[0] * h->sph_om[0] + h->sph_om[1] * h->sph_om[1] + h->sph_om[2] * h->sph_om[2];
+        if (om2 > 0.0) {      // dipole axis co-rotates: Rodrigues rotation of m0 about Omega by |Omega| (t - t0)
+          const double omn = sqrt(om2), th = omn * dt, cth = cos(th), sth = sin(th);
+          const double e[3] = {h->sph_om[0] / omn, h->sph_om[1] / omn, h->sph_om[2] / omn};
+          const double *m0 = h->sph_m;
+          const double em = e[0] * m0[0] + e[1] * m0[1] + e[2] * m0[2];
+          const double ex[3] = {e[1] * m0[2] - e[2] * m0[1], e[2] * m0[0] - e[0] * m0[2], e[0] * m0[1] - e[1] * m0[0]};
+          for (int c = 0; c < 3; c++) a.sph_m[c] = m0[c] * cth + ex[c] * sth + e[c] * em * (1.0 - cth);
         }
       }
       cudaError_t e;
@@ -628,6 +639,12 @@ int lbmhd_set_porosity(lbmhd_t *h, const double *d_field, int on_device) {
   }
   h->have_dfield = true;
   CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LBMHD_OK;
+}
+
+int lbmhd_set_sphere_rotation(lbmhd_t *h, const double omega[3]) {
+  if (!h || !omega) return fail(LBMHD_EINVAL, "NULL argument");
+  for (int c = 0; c < 3; c++) h->sph_om[c] = omega[c];
   return LBMHD_OK;
 }
 

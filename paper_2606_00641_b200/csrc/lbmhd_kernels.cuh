@@ -46,6 +46,7 @@ template <typename real> struct StepArgs {
   double *M_next;               // in-place modes: moments published by this step
   int has_sphere;
   double sph_c[3], sph_R, sph_R2, sph_m[3], sph_Bs, sph_u[3];
+  double sph_om[3];             // angular velocity of the body: u^B = sph_u + sph_om x r; sph_m is already rotated by the host
   double sph_eps, sph_touch2;   // width of the linear porosity ramp (Eq.15-16), 0 = sharp; (R + eps/2)^2
 };
 
@@ -82,8 +83,10 @@ __device__ __forceinline__ double solid_state(const StepArgs<real> &a, int x, in
 #pragma unroll
         for (int c = 0; c < 3; c++) {
           BS[c] = amp * (3.0 * mr * rh[c] - a.sph_m[c]);
-          uS[c] = a.sph_u[c];
         }
+        uS[0] = a.sph_u[0] + (a.sph_om[1] * r[2] - a.sph_om[2] * r[1]);
+        uS[1] = a.sph_u[1] + (a.sph_om[2] * r[0] - a.sph_om[0] * r[2]);
+        uS[2] = a.sph_u[2] + (a.sph_om[0] * r[1] - a.sph_om[1] * r[0]);
         return d;
       }
     }

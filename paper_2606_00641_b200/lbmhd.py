@@ -63,6 +63,7 @@ def load_library():
     lib.lbmhd_set_sphere.argtypes = [C.c_void_p, dp, C.c_double, dp, dp, C.c_double]
     lib.lbmhd_set_porosity.argtypes = [C.c_void_p, dp, C.c_int]
     lib.lbmhd_set_sphere_width.argtypes = [C.c_void_p, C.c_double]
+    lib.lbmhd_set_sphere_rotation.argtypes = [C.c_void_p, dp]
     lib.lbmhd_get_populations.argtypes = [C.c_void_p, dp, C.c_int]
     lib.lbmhd_set_populations.argtypes = [C.c_void_p, dp, C.c_int]
     lib.lbmhd_steps_done.argtypes = [C.c_void_p]
@@ -77,7 +78,7 @@ def load_library():
 
 EXPORTS = ["lbmhd_num_vars", "lbmhd_num_dirs", "lbmhd_workspace_bytes", "lbmhd_create", "lbmhd_destroy",
            "lbmhd_init", "lbmhd_step", "lbmhd_moments", "lbmhd_set_obstacle", "lbmhd_set_sphere",
-           "lbmhd_set_porosity", "lbmhd_set_sphere_width", "lbmhd_get_populations", "lbmhd_set_populations", "lbmhd_steps_done", "lbmhd_launch_count",
+           "lbmhd_set_porosity", "lbmhd_set_sphere_width", "lbmhd_set_sphere_rotation", "lbmhd_get_populations", "lbmhd_set_populations", "lbmhd_steps_done", "lbmhd_launch_count",
            "lbmhd_copy_probe", "lbmhd_last_error"]
 
 
@@ -228,6 +229,10 @@ class Lbmhd:
     def set_sphere_width(self, eps):
         _check(self.lib.lbmhd_set_sphere_width(self.h, float(eps)))
 
+    def set_sphere_rotation(self, omega):
+        om = np.ascontiguousarray(omega, dtype=np.float64)
+        _check(self.lib.lbmhd_set_sphere_rotation(self.h, _host_ptr(om)))
+
     def populations(self):
         """canonical fp64 [K, Q, nz, ny, nx] on the host (via a device tensor)"""
         torch = self.torch
@@ -262,6 +267,8 @@ def from_workload(w, precision=64, device=0, streaming=STREAM_AB):
         sim.set_sphere(s["centre"], s["radius"], s["u_solid"], s["dipole_dir"], s["B_surface"])
         if s.get("width"):
             sim.set_sphere_width(s["width"])
+        if s.get("omega") is not None:
+            sim.set_sphere_rotation(s["omega"])
     return sim
 
 

@@ -19,6 +19,8 @@ def oracle_from_workload(w, mask=None):
         o.set_sphere(s["centre"], s["radius"], s["u_solid"], s["dipole_dir"], s["B_surface"])
         if s.get("width"):
             o.set_sphere_width(s["width"])
+        if s.get("omega") is not None:
+            o.set_sphere_rotation(s["omega"])
     return o
 
 

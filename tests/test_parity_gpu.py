@@ -166,6 +166,9 @@ def test_fractional_porosity_parity(streaming):
     sph = dict(centre=cen, radius=6.0, u_solid=np.array([-0.25, 0.0, 0.0]), dipole_dir=mh, B_surface=0.03, width=1.5)
     w2 = random_workload("IDEAL", "D3Q19", (72, 24, 20), (2, 1, 0, 0, 0, 0), seed=13, sphere=sph)
     compare(w2, 13, streaming=streaming)
+    sph["omega"] = np.array([0.02, 0.0, 0.02])        # tumbling body, dipole co-rotating
+    w3 = random_workload("IDEAL", "D3Q19", (72, 24, 20), (2, 1, 0, 0, 0, 0), seed=14, sphere=sph)
+    compare(w3, 13, streaming=streaming)
 
 
 @pytest.mark.parametrize("streaming", [0, 1])
