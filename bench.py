@@ -133,10 +133,16 @@ def run_native(args, rank, world, local_rank):
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device and no CPU fallback (use --impl reference for the oracle)")
+    local_rank = local_rank % torch.cuda.device_count()
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        if args.backend == "nccl":
+            dist.init_process_group("nccl", device_id=dev)
+        else:
+            dist.init_process_group(args.backend)
+    if args.decomp == "slab" and world > 1:
+        return run_slab(args, rank, world, local_rank, dev)
 
     def barrier():
         if world > 1:
@@ -239,6 +245,74 @@ def run_native(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_slab(args, rank, world, local_rank, dev):
+    """N > 1 with a real exchange: ONE lattice, config 5 stacked `world` times along z (weak scaling: 384x256x256 owned
+    cells per rank), cut into z-slabs with one ghost plane per cut face; per step one paired send/recv of the 5 x 8
+    crossing populations per face.  Opt-in: this path could not be run on more than one GPU here."""
+    import torch
+    import torch.distributed as dist
+    from paper_2606_00641_b200 import slab, workloads as W
+    nx, ny, nz1 = (384, 256, 256) if args.shape is None else tuple(int(v) for v in args.shape.split("x"))
+    shape = (nx, ny, nz1 * world)
+    meta = W.config5(shape=(nx, ny, 4), planes=[0])          # parameters only; the fields are built per slab below
+    meta["shape"] = shape
+    meta["sphere"]["centre"] = np.array([nx / 3.0, ny / 2.0, shape[2] / 2.0])
+    geo = slab.local_geometry(shape, meta["bc"], rank, world)
+    local = W.config5(shape=shape, planes=geo["take"])
+    meta["sphere"] = local["sphere"]
+    sl = slab.Slab(meta, rank, world, precision=args.precision, device=local_rank)
+    via_host = args.backend != "nccl"
+    F = torch.as_tensor(local["fields"]).to(dev)
+    sl.init_local(F)
+    for _ in range(args.warmup):
+        slab.exchange_distributed(sl, dist, via_host=via_host)
+        sl.sim.step(1)
+    dist.barrier()
+    torch.cuda.synchronize(dev)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    l0 = sl.sim.launch_count
+    st = sl.sim.stream
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(st)
+    for _ in range(args.steps):
+        slab.exchange_distributed(sl, dist, via_host=via_host)
+        sl.sim.step(1)
+    e1.record(st)
+    dist.barrier()
+    torch.cuda.synchronize(dev)
+    sampler.stop_flag = True
+    sampler.join()
+    launches = sl.sim.launch_count - l0
+    ms_total = max_over_ranks([e0.elapsed_time(e1)], world, dev if args.backend == "nccl" else None)[0]
+    slab.exchange_distributed(sl, dist, full=True, via_host=via_host)
+    _, dg = sl.sim.moments(want_fields=False)
+    flag = max_over_ranks([float(dg[-1])], world, dev if args.backend == "nccl" else None)[0]
+    if rank == 0:
+        if flag != 0:
+            raise SystemExit("bench.py: numerical failure flag %g after the timed run" % flag)
+        N = nx * ny * nz1
+        K, Q = sl.sim.K, sl.sim.Q
+        bpc = 2 * K * Q * (8 if args.precision == 64 else 4)
+        peak, peak_src = load_peaks()
+        ms_step = ms_total / args.steps
+        halo = int(sl.sim.lib.lbmhd_halo_bytes(sl.sim.h, 0))
+        line = {"metric": METRIC, "value": aggregate_mlups(N, args.steps, ms_total, world), "unit": "MLUPS", "n_gpus": world,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32", "data": "synthetic",
+                "config": {"workload": "C5 stacked %d x along z: one %dx%dx%d lattice in %d z-slabs, halo exchange of %d B per face "
+                                       "per step (%s)" % (world, nx, ny, shape[2], world, halo, args.backend),
+                           "cells": N * world, "streaming": "A/B double buffer"},
+                "roofline": {"bound": "hbm", "achieved": N * bpc / (ms_step * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                             "frac": N * bpc / (ms_step * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                             "kernel": "step_kernel (per rank, exchange included in the step time)"},
+                "e2e": {"value": None, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                        "what": "not measured in slab mode"},
+                "gpu_launches": int(launches), "clocks": sampler.result()}
+        print(json.dumps(line), flush=True)
+    dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -248,6 +322,10 @@ def main():
     ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--streaming", default="ab", choices=["ab", "inplace"])
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (default) or one lattice in z-slabs with halo exchange")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="gloo + host staging is for tests only")
+    ap.add_argument("--shape", default=None, help="slab mode: per-rank owned shape nx x ny x nz (default 384x256x256)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

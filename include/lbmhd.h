@@ -41,7 +41,8 @@ enum { LBMHD_D1Q3 = 1, LBMHD_D2Q9 = 2, LBMHD_D3Q19 = 3,
 enum { LBMHD_IDEAL = 0, LBMHD_INCRES = 1,
        LBMHD_IDEAL_DIVB = 2 /* IDEAL + the paper's local gradient evolution in traced form: a 9th set
                                D = tr G with flux D u - B and source -D/tau_relax; div B in Eq.12 := D/tau_relax */ };
-enum { LBMHD_BC_PERIODIC = 0, LBMHD_BC_ZEROGRAD = 1, LBMHD_BC_INFLOW = 2 };
+enum { LBMHD_BC_PERIODIC = 0, LBMHD_BC_ZEROGRAD = 1, LBMHD_BC_INFLOW = 2,
+       LBMHD_BC_HALO = 3 /* slab decomposition, slowest lattice axis only: the plane on this face is a ghost plane */ };
 enum { LBMHD_CELL_FLUID = 0, LBMHD_CELL_FROZEN = 1, LBMHD_CELL_SOLID = 2 };
 enum { LBMHD_STREAM_AB = 0, LBMHD_STREAM_INPLACE = 1 };
 enum {
@@ -66,6 +67,8 @@ typedef struct {
                            lattice units; 0 = constant resistivity */
   double powell;        /* kappa: 0 = off, 1 = Eq.12 */
   int    bc[6];         /* xmin, xmax, ymin, ymax, zmin, zmax; periodic must be paired per axis */
+  int    halo_offset;   /* slab decomposition: global index of local plane 0 along the slowest lattice axis (0 otherwise);
+                           only the analytic sphere looks at it */
   int    streaming;     /* LBMHD_STREAM_AB (two population copies) | LBMHD_STREAM_INPLACE (one copy, AA pattern:
                            same results; a FROZEN cell is re-emitted as f^eq of its moments, which is what it holds
                            after lbmhd_init; host-pointer population I/O needs LBMHD_STREAM_AB) */
@@ -130,6 +133,18 @@ int lbmhd_set_sphere_width(lbmhd_t *h, double eps);
 /* Rigid rotation of the sphere: u^B(x) = u_solid + omega x (x - c), omega HOST double[3] in radians per
  * step; the dipole axis rotates with the body about omega, counted from the step lbmhd_set_sphere was called at. */
 int lbmhd_set_sphere_rotation(lbmhd_t *h, const double omega[3]);
+
+/* Slab decomposition along the slowest lattice axis (z in 3D, y in 2D), one slab per GPU, A/B streaming.
+ * A face of kind LBMHD_BC_HALO carries a ghost plane: its cells are never updated or counted here, owned cells pull from
+ * them.  Before EVERY step the caller refreshes both ghost planes with the neighbour's data:
+ *   lbmhd_halo_pack(h, side, full, buf)    owned plane next to the ghost on `side` (0 low, 1 high) -> DEVICE buf
+ *   lbmhd_halo_unpack(h, side, full, buf)  DEVICE buf (packed by the neighbour on its opposite side) -> ghost plane on `side`
+ * full = 0 moves only the Q/3-ish directions that cross the face (what a step needs: 5 of 19 on D3Q19), full = 1 all Q
+ * directions (needed before lbmhd_moments so that div_h B sees the neighbour's field).  Buffer layout [K][ndir][plane],
+ * element type = `precision`, lbmhd_halo_bytes(h, full) bytes.  All calls are asynchronous on the stream. */
+size_t lbmhd_halo_bytes(const lbmhd_t *h, int full);
+int lbmhd_halo_pack(lbmhd_t *h, int side, int full, void *buf);
+int lbmhd_halo_unpack(lbmhd_t *h, int side, int full, const void *buf);
 
 /* Raw population access (checkpoint / tests): fp64 [K][Q][N] at this boundary in both precisions, in
  * canonical (k, i, cell) order whatever the streaming layout.  HOST or DEVICE pointer per on_device. */

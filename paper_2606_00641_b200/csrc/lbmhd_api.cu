@@ -68,7 +68,7 @@ constexpr int kMaxDiagBlocks = 1184;   // 8 x 148 SMs
 struct Layout {
   size_t pstride;        // elements per population plane (N rounded up to 32)
   size_t pop_bytes;      // one population copy
-  size_t off_pop[2], off_fields, off_M[2], off_mask, off_bsolid, off_dfield, off_partial, off_diag, total;
+  size_t off_pop[2], off_fields, off_M[2], off_mask, off_bsolid, off_dfield, off_partial, off_diag, off_dirs, total;
 };
 
 bool layout(const lbmhd_params *p, const Geometry &g, Layout *L) {
@@ -90,6 +90,7 @@ bool layout(const lbmhd_params *p, const Geometry &g, Layout *L) {
   L->off_dfield = off; off += align_up(N * 8, 256);
   L->off_partial = off; off += align_up((size_t)kMaxDiagBlocks * (3 * g.K + 4) * 8, 256);
   L->off_diag = off; off += 256;
+  L->off_dirs = off; off += 512;       // direction lists of the halo pack kernels (3 x 32 ints)
   L->total = off;
   return true;
 }
@@ -114,6 +115,7 @@ struct lbmhd {
   bool has_sphere;
   double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs, sph_eps, sph_om[3];
   long long sph_t0;
+  int *halo_dirs;        // device: direction lists for halo packing (in the workspace)
   int tx, minb;          // x-tile and min blocks/SM (launch bound) of the plain step kernel
   bool pair;             // fp32: two cells per thread (even nx); LBMHD_PAIR=0 turns it off
   bool split;            // interior / edge launches split (large grids); LBMHD_SPLIT=0/1 overrides
@@ -200,7 +202,9 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
   const int nn[3] = {p->nx, p->ny, p->nz};
   for (int a = 0; a < g.D; a++) {
     const int lo = p->bc[2 * a], hi = p->bc[2 * a + 1];
-    if (lo < 0 || lo > 2 || hi < 0 || hi > 2) return fail(LBMHD_EINVAL, "bad boundary kind on axis %d", a);
+    const int top = (a == g.D - 1 && g.D >= 2 && p->streaming == LBMHD_STREAM_AB) ? LBMHD_BC_HALO : LBMHD_BC_INFLOW;
+    if (lo < 0 || lo > top || hi < 0 || hi > top)
+      return fail(LBMHD_EINVAL, "bad boundary kind on axis %d (HALO: slowest lattice axis, D >= 2, A/B streaming only)", a);
     if ((lo == LBMHD_BC_PERIODIC) != (hi == LBMHD_BC_PERIODIC)) return fail(LBMHD_EINVAL, "periodic must be paired on axis %d", a);
     if (lo != LBMHD_BC_PERIODIC && nn[a] < 3) return fail(LBMHD_EINVAL, "non-periodic axis %d needs >= 3 cells", a);
   }
@@ -242,12 +246,14 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     h->num_sms = sms;
     h->pair = p->precision == 32 && p->nx % 2 == 0 && p->eta_jc == 0.0;      // eta(j) runs on the one-cell kernels
     if (const char *e3 = getenv("LBMHD_PAIR")) h->pair = h->pair && atoi(e3) != 0;
-    h->split = false;   // measured slower on config 5: edge tiles lose DRAM page locality when launched apart from their rows
+    h->split = false;
+    h->halo_dirs = nullptr;   // measured slower on config 5: edge tiles lose DRAM page locality when launched apart from their rows
     if (const char *e2 = getenv("LBMHD_SPLIT")) h->split = atoi(e2) != 0;
     const char *path = getenv("LBMHD_PATH");      // tuning knob: "plain" forces the register-pull kernel
     const size_t es = p->precision == 64 ? 8 : 4;
     const long long tiles = (long long)((p->nx + kTmaTX - 1) / kTmaTX) * p->ny * p->nz;
-    h->use_tma = p->streaming == LBMHD_STREAM_AB && path && strcmp(path, "tma") == 0 && ((size_t)p->nx * es) % 16 == 0 && tiles < 2000000000LL;
+    const bool halo = g.D >= 2 && (p->bc[2 * (g.D - 1)] == LBMHD_BC_HALO || p->bc[2 * (g.D - 1) + 1] == LBMHD_BC_HALO);
+    h->use_tma = !halo && p->streaming == LBMHD_STREAM_AB && path && strcmp(path, "tma") == 0 && ((size_t)p->nx * es) % 16 == 0 && tiles < 2000000000LL;
     if (h->use_tma) {
       const int rc = make_tensor_maps(h);
       if (rc) { delete h; return rc; }
@@ -399,6 +405,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
         a.st_off[i] = (long long)i * (long long)h->L.pstride * es;
       }
     }
+    a.hoff = h->p.halo_offset;
     a.has_sphere = h->has_sphere ? 1 : 0;
     if (h->has_sphere) {
       a.sph_R = h->sph_R;
@@ -491,12 +498,22 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     const int nb = (int)(want < (size_t)kMaxDiagBlocks ? want : (size_t)kMaxDiagBlocks);
     double *partial = (double *)(h->ws + h->L.off_partial);
     diag_partial_kernel<LAT, SCHEME><<<nb, kDiagThreads, 0, h->stream>>>(fields_dev, partial, h->p.nx, h->p.ny, h->p.nz,
-                                                                          h->p.bc[0], h->p.bc[2], h->p.bc[4], h->p.gamma);
+                                                                          h->p.bc[0], h->p.bc[2], h->p.bc[4], h->p.gamma,
+                                                                          h->g.D >= 2 && h->p.bc[2 * (h->g.D - 1)] == LBMHD_BC_HALO,
+                                                                          h->g.D >= 2 && h->p.bc[2 * (h->g.D - 1) + 1] == LBMHD_BC_HALO);
     CUDA_TRY(cudaGetLastError());
     diag_final_kernel<<<1, kDiagThreads, 0, h->stream>>>(partial, nb, K, diag_dev);
     CUDA_TRY(cudaGetLastError());
     h->launches += 2;
     return LBMHD_OK;
+  }
+
+  // directions whose component along the slowest lattice axis equals `sign` (all directions if sign == 0)
+  static int halo_dirs(int sign, int *dirs) {
+    int n = 0;
+    for (int i = 0; i < Q; i++)
+      if (sign == 0 || lat_c<L>(i, L::D - 1) == sign) dirs[n++] = i;
+    return n;
   }
 
   static int pops_export(lbmhd_t *h, double *out_dev) {
@@ -526,11 +543,12 @@ struct OpTable {
   int (*pops_export)(lbmhd_t *, double *);
   int (*pops_import)(lbmhd_t *, const double *);
   int (*refresh_published)(lbmhd_t *);
+  int (*halo_dirs)(int, int *);
 };
 
 template <int LAT, int SCHEME, typename real> OpTable make_table() {
   using O = Ops<LAT, SCHEME, real>;
-  return OpTable{O::step, O::init, O::moments, O::diag, O::pops_export, O::pops_import, O::refresh_published};
+  return OpTable{O::step, O::init, O::moments, O::diag, O::pops_export, O::pops_import, O::refresh_published, O::halo_dirs};
 }
 
 template <int LAT> OpTable pick2(int scheme, int precision) {
@@ -653,6 +671,51 @@ int lbmhd_set_sphere_width(lbmhd_t *h, double eps) {
   h->sph_eps = eps;
   return LBMHD_OK;
 }
+
+// ---- slab halo exchange: side 0 = low face of the slowest lattice axis, 1 = high face -----------------
+static int halo_dir_list(const lbmhd_t *h, int sign, int *dirs) {      // directions with c_H == sign (all if sign == 0)
+  return pick(h).halo_dirs(sign, dirs);
+}
+
+size_t lbmhd_halo_bytes(const lbmhd_t *h, int full) {
+  if (!h || h->g.D < 2) return 0;
+  int dirs[32];
+  const int nd = halo_dir_list(h, full ? 0 : 1, dirs);
+  const size_t plane = h->g.D == 3 ? (size_t)h->p.nx * h->p.ny : (size_t)h->p.nx;
+  return (size_t)h->g.K * nd * plane * (h->p.precision == 64 ? 8 : 4);
+}
+
+static int halo_move(lbmhd_t *h, int side, int full, void *buf, bool pack) {
+  if (!h || !buf || side < 0 || side > 1) return fail(LBMHD_EINVAL, "bad argument");
+  if (h->g.D < 2 || h->p.streaming != LBMHD_STREAM_AB) return fail(LBMHD_EINVAL, "halo exchange needs D >= 2 and A/B streaming");
+  if (int rc = use_device(h)) return rc;
+  const int nH = h->g.D == 3 ? h->p.nz : h->p.ny;
+  const size_t plane = h->g.D == 3 ? (size_t)h->p.nx * h->p.ny : (size_t)h->p.nx;
+  // pack: the owned plane next to the ghost, directions that leave through that face (the neighbour pulls them);
+  // unpack: the ghost plane itself, directions that enter through that face
+  const int sign = full ? 0 : (pack ? (side == 0 ? -1 : 1) : (side == 0 ? 1 : -1));
+  const int hidx = pack ? (side == 0 ? 1 : nH - 2) : (side == 0 ? 0 : nH - 1);
+  int dirs[32];
+  const int nd = halo_dir_list(h, sign, dirs);
+  int *ddev = (int *)(h->ws + h->L.off_dirs) + 32 * (full ? 2 : (sign > 0 ? 1 : 0));
+  CUDA_TRY(cudaMemcpyAsync(ddev, dirs, nd * sizeof(int), cudaMemcpyHostToDevice, h->stream));
+  const size_t total = (size_t)h->g.K * nd * plane;
+  const int blocks = (int)((total + 255) / 256 < 1184 ? (total + 255) / 256 : 1184);
+  char *pops = h->ws + h->L.off_pop[h->cur];
+  if (h->p.precision == 64) {
+    if (pack) halo_plane_kernel<double, true><<<blocks, 256, 0, h->stream>>>((double *)pops, h->L.pstride, (double *)buf, plane, (size_t)hidx * plane, h->g.K, h->g.Q, nd, ddev);
+    else halo_plane_kernel<double, false><<<blocks, 256, 0, h->stream>>>((double *)pops, h->L.pstride, (double *)buf, plane, (size_t)hidx * plane, h->g.K, h->g.Q, nd, ddev);
+  } else {
+    if (pack) halo_plane_kernel<float, true><<<blocks, 256, 0, h->stream>>>((float *)pops, h->L.pstride, (float *)buf, plane, (size_t)hidx * plane, h->g.K, h->g.Q, nd, ddev);
+    else halo_plane_kernel<float, false><<<blocks, 256, 0, h->stream>>>((float *)pops, h->L.pstride, (float *)buf, plane, (size_t)hidx * plane, h->g.K, h->g.Q, nd, ddev);
+  }
+  CUDA_TRY(cudaGetLastError());
+  h->launches += 1;
+  return LBMHD_OK;
+}
+
+int lbmhd_halo_pack(lbmhd_t *h, int side, int full, void *buf) { return halo_move(h, side, full, buf, true); }
+int lbmhd_halo_unpack(lbmhd_t *h, int side, int full, const void *buf) { return halo_move(h, side, full, (void *)buf, false); }
 
 static int pops_io(lbmhd_t *h, double *out, const double *in, int on_device) {
   if (!h || (!out && !in)) return fail(LBMHD_EINVAL, "NULL argument");

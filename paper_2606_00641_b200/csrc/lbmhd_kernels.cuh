@@ -19,7 +19,7 @@
 
 namespace lbk {
 
-enum { BC_PERIODIC = 0, BC_ZEROGRAD = 1, BC_INFLOW = 2 };
+enum { BC_PERIODIC = 0, BC_ZEROGRAD = 1, BC_INFLOW = 2, BC_HALO = 3 };
 enum { CELL_FLUID = 0, CELL_FROZEN = 1, CELL_SOLID = 2 };
 
 template <typename real> struct StepArgs {
@@ -44,6 +44,7 @@ template <typename real> struct StepArgs {
   const double *M_cur;          // in-place modes: post-collision moments [K][N] published last step (and the constant
                                 //   state of frozen cells); nullptr in A/B mode
   double *M_next;               // in-place modes: moments published by this step
+  int hoff;                     // slab decomposition: global index of local plane 0 along the slowest lattice axis
   int has_sphere;
   double sph_c[3], sph_R, sph_R2, sph_m[3], sph_Bs, sph_u[3];
   double sph_om[3];             // angular velocity of the body: u^B = sph_u + sph_om x r; sph_m is already rotated by the host
@@ -60,8 +61,8 @@ __device__ __forceinline__ double solid_state(const StepArgs<real> &a, int x, in
   if (a.has_sphere) {
     double r[3];
     r[0] = __dsub_rn((double)x, a.sph_c[0]);
-    r[1] = D > 1 ? __dsub_rn((double)y, a.sph_c[1]) : 0.0;
-    r[2] = D > 2 ? __dsub_rn((double)z, a.sph_c[2]) : 0.0;
+    r[1] = D > 1 ? __dsub_rn((double)(y + (D == 2 ? a.hoff : 0)), a.sph_c[1]) : 0.0;
+    r[2] = D > 2 ? __dsub_rn((double)(z + a.hoff), a.sph_c[2]) : 0.0;
     double r2 = __dmul_rn(r[0], r[0]);
     r2 = __dadd_rn(r2, __dmul_rn(r[1], r[1]));
     r2 = __dadd_rn(r2, __dmul_rn(r[2], r[2]));
@@ -307,14 +308,24 @@ template <class L, typename real> struct StorePPGeneral {
   }
 };
 
+// Slab decomposition: the plane on a HALO face of the slowest lattice axis is a ghost plane owned by the
+// neighbouring slab: it is never updated here (the caller refreshes it before every step) and its cells are pulled from
+// like any other in-range cell.
+template <typename real, int D>
+__device__ __forceinline__ bool ghost_row(const StepArgs<real> &a, int y, int z) {
+  if (D < 2) return false;
+  const int hc = D == 3 ? z : y, hn = D == 3 ? a.nz : a.ny;
+  return (hc == 0 && a.bc[2 * (D - 1)] == BC_HALO) || (hc == hn - 1 && a.bc[2 * (D - 1) + 1] == BC_HALO);
+}
+
 // Conservative, tile-uniform test: can the sphere touch cells [x0, x0+tx_cells) of row (y, z)?
 template <typename real, int D>
 __device__ __forceinline__ bool sphere_may_touch(const StepArgs<real> &a, int x0, int tx_cells, int y, int z) {
   if (!a.has_sphere) return false;
   const double lo = (double)x0 - a.sph_c[0], hi = a.sph_c[0] - (double)(x0 + tx_cells - 1);
   const double dx = fmax(0.0, fmax(lo, hi));
-  const double dy = D > 1 ? (double)y - a.sph_c[1] : 0.0;
-  const double dz = D > 2 ? (double)z - a.sph_c[2] : 0.0;
+  const double dy = D > 1 ? (double)(y + (D == 2 ? a.hoff : 0)) - a.sph_c[1] : 0.0;
+  const double dz = D > 2 ? (double)(z + a.hoff) - a.sph_c[2] : 0.0;
   return dx * dx + dy * dy + dz * dz <= a.sph_touch2 * (1.0 + 1e-9) + 1e-9;
 }
 
@@ -587,6 +598,7 @@ __device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, 
   constexpr int K = V::K;
   const int x = x0 + tx;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
+  if (ghost_row<real, D>(a, y, z)) return;
   const auto sync = [] { __syncthreads(); };
   const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
 
@@ -823,6 +835,7 @@ step_kernel_pair(const __grid_constant__ StepArgs<float> a, const int npair) {
   // tiles are all interior when the row is; blocks 0..npair-1 are the pair tiles, block npair the first edge tile
   const int nx = a.nx, ny = a.ny, nz = a.nz;
   const int y = blockIdx.y, z = blockIdx.z;
+  if (ghost_row<float, D>(a, y, z)) return;
   float(*sQ32)[32] = reinterpret_cast<float(*)[32]>(&sQ[0][0]);
   float(*sTr32)[32] = reinterpret_cast<float(*)[32]>(&sTr[0][0]);
   if ((int)blockIdx.x >= npair) {
@@ -1000,7 +1013,7 @@ template <int KIND> __device__ __forceinline__ double block_reduce(double v, dou
 template <int LAT, int SCHEME>
 __global__ void __launch_bounds__(kDiagThreads)
 diag_partial_kernel(const double *__restrict__ F, double *__restrict__ partial, int nx, int ny, int nz, int bc0, int bc2,
-                    int bc4, double gamma) {
+                    int bc4, double gamma, int ghost_lo, int ghost_hi) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q, K = Vars<SCHEME, D>::K, iB = Vars<SCHEME, D>::iB;
   __shared__ double sm[32];
@@ -1014,6 +1027,10 @@ diag_partial_kernel(const double *__restrict__ F, double *__restrict__ partial, 
   for (size_t n = (size_t)blockIdx.x * blockDim.x + threadIdx.x; n < N; n += (size_t)gridDim.x * blockDim.x) {
     const int x = (int)(n % nx), y = (int)((n / nx) % ny), z = (int)(n / ((size_t)nx * ny));
     const int xi[3] = {x, y, z};
+    if (D >= 2) {      // ghost planes of a slab belong to the neighbour: not counted
+      const int hc = D == 3 ? z : y, hn = D == 3 ? nz : ny;
+      if ((ghost_lo && hc == 0) || (ghost_hi && hc == hn - 1)) continue;
+    }
     double v[K];
 #pragma unroll
     for (int l = 0; l < K; l++) {
@@ -1108,6 +1125,21 @@ __global__ void pops_import_kernel(const double *__restrict__ in, real *__restri
   for (size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x; j < total; j += (size_t)gridDim.x * blockDim.x) {
     const size_t pl = j / N, n = j - pl * N;
     g[pl * pstride + n] = (real)in[j];
+  }
+}
+
+// ---- slab halo: pack the populations of one plane of the slowest axis (the listed directions, all K sets) into a
+// contiguous buffer [K][ndir][plane cells], or write such a buffer into a plane ------------------------------
+template <typename real, bool PACK>
+__global__ void halo_plane_kernel(real *__restrict__ g, size_t pstride, real *__restrict__ buf, size_t plane_cells, size_t plane_first,
+                                  int K, int Q, int ndir, const int *__restrict__ dirs) {
+  const size_t total = (size_t)K * ndir * plane_cells;
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
+    const size_t c = e % plane_cells, kd = e / plane_cells;
+    const int d = (int)(kd % ndir), k = (int)(kd / ndir);
+    real *slot = g + ((size_t)k * Q + dirs[d]) * pstride + plane_first + c;
+    if (PACK) buf[e] = *slot;
+    else *slot = buf[e];
   }
 }
 

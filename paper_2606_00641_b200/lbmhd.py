@@ -14,7 +14,7 @@ from . import build as _build
 
 D1Q3, D2Q9, D3Q19, D2Q5, D3Q7 = 1, 2, 3, 4, 5
 IDEAL, INCRES, IDEAL_DIVB = 0, 1, 2
-BC_PERIODIC, BC_ZEROGRAD, BC_INFLOW = 0, 1, 2
+BC_PERIODIC, BC_ZEROGRAD, BC_INFLOW, BC_HALO = 0, 1, 2, 3
 CELL_FLUID, CELL_FROZEN, CELL_SOLID = 0, 1, 2
 STREAM_AB, STREAM_INPLACE = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC = 0, -1, -2, -3, -4
@@ -27,7 +27,7 @@ class LbmhdParams(C.Structure):
                 ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
                 ("gamma", C.c_double), ("c0sq", C.c_double), ("nu", C.c_double), ("eta", C.c_double),
                 ("tau", C.c_double * 16), ("tau_relax", C.c_double), ("eta_jc", C.c_double), ("powell", C.c_double), ("bc", C.c_int * 6),
-                ("streaming", C.c_int), ("device", C.c_int), ("stream", C.c_void_p),
+                ("halo_offset", C.c_int), ("streaming", C.c_int), ("device", C.c_int), ("stream", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
 
 
@@ -64,6 +64,10 @@ def load_library():
     lib.lbmhd_set_porosity.argtypes = [C.c_void_p, dp, C.c_int]
     lib.lbmhd_set_sphere_width.argtypes = [C.c_void_p, C.c_double]
     lib.lbmhd_set_sphere_rotation.argtypes = [C.c_void_p, dp]
+    lib.lbmhd_halo_bytes.argtypes = [C.c_void_p, C.c_int]
+    lib.lbmhd_halo_bytes.restype = C.c_size_t
+    lib.lbmhd_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
+    lib.lbmhd_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
     lib.lbmhd_get_populations.argtypes = [C.c_void_p, dp, C.c_int]
     lib.lbmhd_set_populations.argtypes = [C.c_void_p, dp, C.c_int]
     lib.lbmhd_steps_done.argtypes = [C.c_void_p]
@@ -78,7 +82,8 @@ def load_library():
 
 EXPORTS = ["lbmhd_num_vars", "lbmhd_num_dirs", "lbmhd_workspace_bytes", "lbmhd_create", "lbmhd_destroy",
            "lbmhd_init", "lbmhd_step", "lbmhd_moments", "lbmhd_set_obstacle", "lbmhd_set_sphere",
-           "lbmhd_set_porosity", "lbmhd_set_sphere_width", "lbmhd_set_sphere_rotation", "lbmhd_get_populations", "lbmhd_set_populations", "lbmhd_steps_done", "lbmhd_launch_count",
+           "lbmhd_set_porosity", "lbmhd_set_sphere_width", "lbmhd_set_sphere_rotation", "lbmhd_halo_bytes", "lbmhd_halo_pack",
+           "lbmhd_halo_unpack", "lbmhd_get_populations", "lbmhd_set_populations", "lbmhd_steps_done", "lbmhd_launch_count",
            "lbmhd_copy_probe", "lbmhd_last_error"]
 
 
@@ -89,7 +94,7 @@ def _check(rc, allow=()):
 
 
 def make_params(scheme, lattice, shape, precision=64, gamma=5.0 / 3.0, c0sq=1.0 / 36.0, nu=0.0, eta=0.0, tau=0.6,
-                powell=1.0, bc=(0,) * 6, streaming=STREAM_AB, device=0, tau_relax=0.0, eta_jc=0.0):
+                powell=1.0, bc=(0,) * 6, streaming=STREAM_AB, device=0, tau_relax=0.0, eta_jc=0.0, halo_offset=0):
     p = LbmhdParams()
     p.scheme = SCHEMES.get(scheme, scheme)
     p.lattice = LATTICES.get(lattice, lattice)
@@ -104,7 +109,7 @@ def make_params(scheme, lattice, shape, precision=64, gamma=5.0 / 3.0, c0sq=1.0 
     p.eta_jc = eta_jc
     for j in range(6):
         p.bc[j] = bc[j]
-    p.streaming, p.device = streaming, device
+    p.streaming, p.device, p.halo_offset = streaming, device, halo_offset
     return p
 
 
@@ -246,6 +251,18 @@ class Lbmhd:
         t = torch.as_tensor(np.ascontiguousarray(g, dtype=np.float64).reshape(-1)).to(self.workspace.device)
         _check(self.lib.lbmhd_set_populations(self.h, C.c_void_p(t.data_ptr()), 1))
         self.stream.synchronize()
+
+    def halo_buffer(self, full=False):
+        """device tensor sized for one packed face (element type = precision)"""
+        torch = self.torch
+        nbytes = int(self.lib.lbmhd_halo_bytes(self.h, int(full)))
+        return torch.empty(nbytes, dtype=torch.uint8, device=self.workspace.device)
+
+    def halo_pack(self, side, buf, full=False):
+        _check(self.lib.lbmhd_halo_pack(self.h, int(side), int(full), C.c_void_p(buf.data_ptr())))
+
+    def halo_unpack(self, side, buf, full=False):
+        _check(self.lib.lbmhd_halo_unpack(self.h, int(side), int(full), C.c_void_p(buf.data_ptr())))
 
     @property
     def steps_done(self):

@@ -141,13 +141,15 @@ def config4(n=2048, steps=1000, cfl=0.1, tau=0.51):
                 fields=_ideal_Q(rho, u, B, p, gamma), sphere=None, scale=s)
 
 
-def dipole_field(shape_zyx, centre, R, mhat, Bs, dtype=np.float64):
-    """input data only: capped dipole 1/2 Bs (R / max(|r|, R/2))^3 [3 (m.r^) r^ - m] on integer cell coordinates"""
+def dipole_field(shape_zyx, centre, R, mhat, Bs, dtype=np.float64, planes=None):
+    """input data only: capped dipole 1/2 Bs (R / max(|r|, R/2))^3 [3 (m.r^) r^ - m] on integer cell coordinates;
+    planes = global z indices to build (default: all nz)"""
     nz, ny, nx = shape_zyx
-    out = np.zeros((3, nz, ny, nx), dtype=dtype)
+    zs = np.arange(nz) if planes is None else np.asarray(planes)
+    out = np.zeros((3, len(zs), ny, nx), dtype=dtype)
     xs = np.arange(nx, dtype=np.float64) - centre[0]
     ys = np.arange(ny, dtype=np.float64) - centre[1]
-    for z in range(nz):                                   # plane by plane: bounded temporaries at full size
+    for iz, z in enumerate(zs):                           # plane by plane: bounded temporaries at full size
         rz = float(z) - centre[2]
         X, Y = np.meshgrid(xs, ys, indexing="xy")
         r2 = X * X + Y * Y + rz * rz
@@ -157,14 +159,15 @@ def dipole_field(shape_zyx, centre, R, mhat, Bs, dtype=np.float64):
         hx, hy, hz = X * inv, Y * inv, rz * inv
         mr = mhat[0] * hx + mhat[1] * hy + mhat[2] * hz
         amp = 0.5 * Bs * (R / rc) ** 3
-        out[0, z] = amp * (3 * mr * hx - mhat[0])
-        out[1, z] = amp * (3 * mr * hy - mhat[1])
-        out[2, z] = amp * (3 * mr * hz - mhat[2])
+        out[0, iz] = amp * (3 * mr * hx - mhat[0])
+        out[1, iz] = amp * (3 * mr * hy - mhat[1])
+        out[2, iz] = amp * (3 * mr * hz - mhat[2])
     return out
 
 
-def config5(shape=(384, 256, 256), steps=500, tau=0.7, radius=None):
-    """C5: 3D supersonic flow (Mach 4) past a moving magnetised sphere, D3Q19, lattice units directly."""
+def config5(shape=(384, 256, 256), steps=500, tau=0.7, radius=None, planes=None):
+    """C5: 3D supersonic flow (Mach 4) past a moving magnetised sphere, D3Q19, lattice units directly.
+    planes: build the fields of these global z planes only (slab decomposition: each rank makes its own slab)."""
     rng = _rng(5)
     gamma = 5.0 / 3.0
     nx, ny, nz = shape
@@ -175,8 +178,8 @@ def config5(shape=(384, 256, 256), steps=500, tau=0.7, radius=None):
     m = rng.normal(size=3)
     mhat = m / np.linalg.norm(m)
     Bs = 0.03
-    F = np.empty((8, nz, ny, nx), dtype=np.float64)
-    B = dipole_field((nz, ny, nx), centre, R, mhat, Bs)
+    F = np.empty((8, nz if planes is None else len(planes), ny, nx), dtype=np.float64)
+    B = dipole_field((nz, ny, nx), centre, R, mhat, Bs, planes=planes)
     B[2] += 0.1 * a / np.sqrt(gamma)
     ux = 4.0 * a
     F[0] = 1.0
