@@ -115,7 +115,6 @@ struct lbmhd {
   bool has_sphere;
   double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs, sph_eps, sph_om[3];
   long long sph_t0;
-  int *halo_dirs;        // device: direction lists for halo packing (in the workspace)
   int tx, minb;          // x-tile and min blocks/SM (launch bound) of the plain step kernel
   bool pair;             // fp32: two cells per thread (even nx); LBMHD_PAIR=0 turns it off
   bool split;            // interior / edge launches split (large grids); LBMHD_SPLIT=0/1 overrides
@@ -235,7 +234,7 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
   h->ws = (char *)p->workspace;
   h->stream = (cudaStream_t)p->stream;
   h->tx = 32; h->minb = g.Q > 9 ? 3 : 4;     // measured best on B200: D3Q19 80 regs x 3 blocks/SM, D2Q9/D1Q3 64 regs x 4
-  if (const char *e = getenv("LBMHD_TX")) h->tx = atoi(e);        // tuning knobs; unknown pairs fall back to 32/2
+  if (const char *e = getenv("LBMHD_TX")) h->tx = atoi(e);        // tuning knobs; unknown pairs fall back to 32/3
   if (const char *e = getenv("LBMHD_MINB")) h->minb = atoi(e);
   cudaError_t e = cudaSetDevice(p->device);
   if (e != cudaSuccess) { delete h; return fail(LBMHD_ECUDA, "cudaSetDevice(%d): %s", p->device, cudaGetErrorString(e)); }
@@ -246,8 +245,7 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     h->num_sms = sms;
     h->pair = p->precision == 32 && p->nx % 2 == 0 && p->eta_jc == 0.0;      // eta(j) runs on the one-cell kernels
     if (const char *e3 = getenv("LBMHD_PAIR")) h->pair = h->pair && atoi(e3) != 0;
-    h->split = false;
-    h->halo_dirs = nullptr;   // measured slower on config 5: edge tiles lose DRAM page locality when launched apart from their rows
+    h->split = false;   // measured slower on config 5: edge tiles lose DRAM page locality when launched apart from their rows
     if (const char *e2 = getenv("LBMHD_SPLIT")) h->split = atoi(e2) != 0;
     const char *path = getenv("LBMHD_PATH");      // tuning knob: "plain" forces the register-pull kernel
     const size_t es = p->precision == 64 ? 8 : 4;
