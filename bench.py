@@ -199,6 +199,7 @@ def run_native(args, rank, world, local_rank):
     d2h = out_host.numel() * 8 + diag_host.numel() * 8
 
     ms_total, ms_e2e = max_over_ranks([ms_total, ms_e2e], world, dev)
+    own_copy = lbmhd.copy_probe(1 << 27, reps=5, device=local_rank) if rank == 0 else None   # fp64 copy, this library's grid style
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -231,6 +232,7 @@ def run_native(args, rank, world, local_rank):
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "peak_source": peak_src, "kernel": "step_kernel",
                      "frac_of_nominal_8TBs": achieved / 8000.0,
+                     "own_fp64_copy_GBs": own_copy, "frac_of_own_copy": achieved / own_copy,
                      "paper_context": "98.9% (2D) / 75.8% (3D) of 680 GB/s BabelStream, RTX A5000 fp32 (PAPER.md:269)"},
         "e2e": {"value": e2e_val, "unit": "MLUPS", "h2d_bytes_per_step": h2d / args.steps,
                 "d2h_bytes_per_step": d2h / args.steps,

@@ -61,6 +61,8 @@ def _load():
         lib.oracle_get_populations.argtypes = [C.c_void_p, dp]
         lib.oracle_set_populations.argtypes = [C.c_void_p, dp]
         lib.oracle_source_log.argtypes = [C.c_void_p, dp]
+        lib.oracle_body_read.argtypes = [C.c_void_p, dp, C.c_int]
+        lib.oracle_set_body_reference.argtypes = [C.c_void_p, dp]
         lib.oracle_lattice.argtypes = [C.c_int, ip, ip, ip, dp, dp]
         lib.oracle_flux.argtypes = [pp, dp, dp]
         lib.oracle_equilibrium.argtypes = [pp, dp, dp]
@@ -230,3 +232,13 @@ class Oracle:
         acc = np.zeros(self.K)
         self.lib.oracle_source_log(self.h, _dptr(acc))
         return acc
+
+    def body_read(self, reset=False):
+        """body integrals accumulated since init / the last reset: F[3] | T[3] | W | I_B[3] | sum (1-d) B [3] | sum (1-d)"""
+        out = np.zeros(14)
+        assert self.lib.oracle_body_read(self.h, _dptr(out), int(reset)) == 0
+        return out
+
+    def set_body_reference(self, ref):
+        ref = np.ascontiguousarray(ref, dtype=np.float64)
+        assert self.lib.oracle_set_body_reference(self.h, _dptr(ref)) == 0

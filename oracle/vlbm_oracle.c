@@ -24,6 +24,8 @@
 #endif
 
 #define MAXK 9
+#define NBODY 14          /* body integrals, oracle_body_read */
+#define ACCW (MAXK + NBODY) /* per-row accumulator: source log | body integrals */
 #define MAXQ 19
 
 /* ---- lattice tables (A2): rest; +x,-x,+y,-y,+z,-z; diagonals (+,+),(-,-),(+,-),(-,+) per plane
@@ -233,6 +235,8 @@ struct oracle {
   double *dfield;      /* lattice porosity d in [0,1] per cell (Eq.15), or NULL: d from the mask (SOLID -> 0) */
   long t;              /* steps done so far */
   double srclog[MAXK];
+  double body[NBODY];  /* body integrals accumulated over the steps since the last reset (A21) */
+  double body_ref[3];  /* torque reference point of masked bodies; an analytic sphere uses its own centre */
 };
 
 static long cell_index(const oracle_t *o, int x, int y, int z)
@@ -370,6 +374,7 @@ int oracle_init(oracle_t *o, const double *fields)
   }
   o->cur = 0; o->t = 0; o->sph_t0 = 0;
   memset(o->srclog, 0, sizeof o->srclog);
+  memset(o->body, 0, sizeof o->body);
   return 0;
 }
 
@@ -386,6 +391,30 @@ int oracle_set_populations(oracle_t *o, const double *g_in)
 int oracle_source_log(oracle_t *o, double *acc)
 {
   for (int k = 0; k < o->K; k++) acc[k] = o->srclog[k];
+  return 0;
+}
+
+/* ---- body integrals (A21) ----
+ * The blend of Eq.13-14 injects dQh = Q^ - Q into the fluid at every cell with d < 1 (A8); what the fluid receives the body
+ * gives.  Summed over those cells and accumulated over steps, r = x - (sphere centre at this step, else body_ref):
+ *   [0..2] F = - sum dQh_m            momentum the fluid hands to the body per step (aerodynamic + Maxwell)
+ *   [3..5] T = - sum r x dQh_m        its moment about the reference point
+ *   [6]    W = - sum dQh_E            energy handed to the body (IDEAL; 0 for INCRES)
+ *   [7..9] I =   sum dQh_B            magnetic field injected into the fluid
+ *   [10..12]     sum (1-d) B          volume integral of the fluid's pre-blend B over the body (flux x length)
+ *   [13]         sum (1-d)            body volume in cells
+ * INCRES: the velocity sets stand for momentum (rho = 1). */
+int oracle_body_read(oracle_t *o, double *out, int reset)
+{
+  if (!o) return -1;
+  if (out) for (int j = 0; j < NBODY; j++) out[j] = o->body[j];
+  if (reset) memset(o->body, 0, sizeof o->body);
+  return 0;
+}
+int oracle_set_body_reference(oracle_t *o, const double ref[3])
+{
+  if (!o || !ref) return -1;
+  for (int a = 0; a < 3; a++) o->body_ref[a] = ref[a];
   return 0;
 }
 
@@ -578,6 +607,26 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
     }
     /* the Powell rows are scaled by the porosity (A8); the relaxation of D is intrinsic and is not */
     for (k = 0; k < K; k++) { dQh[k] = Qh[k] - Qv[k]; if (!(o->p.scheme == ORC_IDEAL_DIVB && k == 8)) S[k] *= d; }
+    if (srcacc) {   /* body integrals (A21) */
+      double *bd = srcacc + MAXK;
+      const int nvec = is_ideal(o->p.scheme) ? 3 : D;
+      double r[3] = { 0.0, 0.0, 0.0 }, Fm[3] = { 0.0, 0.0, 0.0 };
+      for (a = 0; a < D; a++) {
+        double ref = o->has_sphere ? o->sph_c0[a] + (double)(o->t - o->sph_t0) * o->sph_u[a] : o->body_ref[a];
+        r[a] = (double)xi[a] - ref;
+      }
+      for (b = 0; b < nvec; b++) {
+        Fm[b] = -dQh[o->iU + b];
+        bd[b] += Fm[b];
+        bd[7 + b] += dQh[o->iB + b];
+        bd[10 + b] += (1.0 - d) * Qv[o->iB + b];
+      }
+      bd[3] += r[1] * Fm[2] - r[2] * Fm[1];
+      bd[4] += r[2] * Fm[0] - r[0] * Fm[2];
+      bd[5] += r[0] * Fm[1] - r[1] * Fm[0];
+      if (is_ideal(o->p.scheme)) bd[6] += -dQh[4];
+      bd[13] += 1.0 - d;
+    }
   }
   if (srcacc) for (k = 0; k < K; k++) srcacc[k] += S[k];
 
@@ -600,31 +649,34 @@ int oracle_step(oracle_t *o, int n_steps)
   if (!o || n_steps < 0) return -1;
   const int nx = o->p.nx, ny = o->p.ny, nz = o->p.nz;
   const long rows = (long)ny * nz;
-  double *rowacc = (double *)calloc((size_t)rows * MAXK, sizeof(double));
+  double *rowacc = (double *)calloc((size_t)rows * ACCW, sizeof(double));
   if (!rowacc) return -2;
   for (int s = 0; s < n_steps; s++) {
     const double *src = o->g[o->cur];
     double *dst = o->g[1 - o->cur];
-    memset(rowacc, 0, (size_t)rows * MAXK * sizeof(double));
+    memset(rowacc, 0, (size_t)rows * ACCW * sizeof(double));
     if (rows >= 4) {
 #pragma omp parallel for schedule(static) num_threads(oracle_get_threads())
       for (long r = 0; r < rows; r++) {
         int z = (int)(r / ny), y = (int)(r % ny);
-        for (int x = 0; x < nx; x++) cell_update(o, src, dst, x, y, z, rowacc + r * MAXK);
+        for (int x = 0; x < nx; x++) cell_update(o, src, dst, x, y, z, rowacc + r * ACCW);
       }
     } else {
       /* 1D / thin domains: parallelise over x, source log kept serial-free by per-cell slots */
-      double *cellacc = (double *)calloc((size_t)o->N * MAXK, sizeof(double));
+      double *cellacc = (double *)calloc((size_t)o->N * ACCW, sizeof(double));
       if (!cellacc) { free(rowacc); return -2; }
 #pragma omp parallel for schedule(static) num_threads(oracle_get_threads())
       for (long n = 0; n < o->N; n++) {
         int x = (int)(n % nx), y = (int)((n / nx) % ny), z = (int)(n / ((long)nx * ny));
-        cell_update(o, src, dst, x, y, z, cellacc + n * MAXK);
+        cell_update(o, src, dst, x, y, z, cellacc + n * ACCW);
       }
-      for (long n = 0; n < o->N; n++) for (int k = 0; k < o->K; k++) rowacc[k] += cellacc[n * MAXK + k];
+      for (long n = 0; n < o->N; n++) for (int k = 0; k < ACCW; k++) rowacc[k] += cellacc[n * ACCW + k];
       free(cellacc);
     }
-    for (long r = 0; r < rows; r++) for (int k = 0; k < o->K; k++) o->srclog[k] += rowacc[r * MAXK + k];
+    for (long r = 0; r < rows; r++) {
+      for (int k = 0; k < o->K; k++) o->srclog[k] += rowacc[r * ACCW + k];
+      for (int j = 0; j < NBODY; j++) o->body[j] += rowacc[r * ACCW + MAXK + j];
+    }
     o->cur = 1 - o->cur;
     o->t += 1;
   }

@@ -11,7 +11,7 @@
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): P1 equilibrium moments, P2 uniform invariance,
  * P3 conservation, P4 div B, P5/P5b linear waves (closed form + exact Fourier symbol), P6 numpy
- * brute force, P7 symmetries, P8 hydrodynamic limits, P9 obstacle, P10 boundaries.
+ * brute force, P7 symmetries, P8 hydrodynamic limits, P9 obstacle, P10 boundaries, P12 body integrals (tests/test_oracle_body.py).
  * Parity unpinned: absolute accuracy against the paper's figures (data not available) and the
  * readings A3, A6, A8-A12 themselves (choices, not facts of the paper) — see DESIGN.md §3.
  */
@@ -65,6 +65,11 @@ int  oracle_set_porosity(oracle_t *o, const double *d_field /* [N] or NULL */);
 int  oracle_set_sphere_width(oracle_t *o, double eps);
 /* rigid rotation of the sphere: u^B(x) = u_solid + omega x (x - c), dipole axis rotates with the body */
 int  oracle_set_sphere_rotation(oracle_t *o, const double omega[3]);
+
+/* body integrals (A21), accumulated over the steps since init or the last reset:
+ * out[14] = F[3] | T[3] | W | I_B[3] | sum (1-d) B [3] | sum (1-d);  see vlbm_oracle.c */
+int  oracle_body_read(oracle_t *o, double *out /* [14] or NULL */, int reset);
+int  oracle_set_body_reference(oracle_t *o, const double ref[3]);   /* torque reference of masked bodies (default 0) */
 
 /* test hooks */
 double oracle_tau_of_current(double tau0, double e0, double a2, double jc);

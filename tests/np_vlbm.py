@@ -112,6 +112,8 @@ class NpVLBM:
         self.d_field = None
         self.t = 0
         self.src_acc = np.zeros(self.K)
+        self.body = np.zeros(14)
+        self.body_ref = np.zeros(3)
         zz, yy, xx = np.meshgrid(*[np.arange(n) for n in self.shape], indexing="ij")
         self.coord = (xx, yy, zz)
         self.n_axis = (self.shape[2], self.shape[1], self.shape[0])
@@ -313,5 +315,24 @@ class NpVLBM:
             gnew = np.where(fr[None, None], g, gnew)
             S = np.where(fr[None], 0.0, S)
         self.src_acc += S.reshape(K, -1).sum(1)
+        # body integrals (A21): what the blend hands over at the cells with d < 1
+        body_cells = (d < 1.0) & ~fr
+        if body_cells.any():
+            nvec = 3 if self.ideal else D
+            ref = self.body_ref if self.sphere is None else self.sphere[0] + (self.t - self.sphere[5]) * self.sphere[2]
+            r = np.zeros((3,) + self.shape)
+            Fm = np.zeros((3,) + self.shape)
+            for a in range(D):
+                r[a] = self.coord[a] - ref[a]
+            Fm[:nvec] = -dQh[1:1 + nvec]
+            Tq = np.cross(np.moveaxis(r, 0, -1), np.moveaxis(Fm, 0, -1))
+            sel = body_cells
+            self.body[0:3] += Fm[:, sel].sum(1)
+            self.body[3:6] += Tq[sel].sum(0)
+            if self.ideal:
+                self.body[6] += -dQh[4][sel].sum()
+            self.body[7:7 + nvec] += dQh[self.iB:self.iB + nvec][:, sel].sum(1)
+            self.body[10:10 + nvec] += ((1.0 - d) * Q[self.iB:self.iB + nvec])[:, sel].sum(1)
+            self.body[13] += (1.0 - d)[sel].sum()
         self.g = gnew
         self.t += 1
