@@ -146,6 +146,22 @@ size_t lbmhd_halo_bytes(const lbmhd_t *h, int full);
 int lbmhd_halo_pack(lbmhd_t *h, int side, int full, void *buf);
 int lbmhd_halo_unpack(lbmhd_t *h, int side, int full, const void *buf);
 
+/* Body integrals ("per-timestep surface integrals of net magnetic flux, forces, torques,
+ * electromagnetic work"; the paper prints no formulas: DESIGN.md reading A21 takes them from what the blend of
+ * Eq.13-14 hands over).  While enabled every lbmhd_step adds, over the cells with d < 1,
+ *   out[0..2]   F = - sum dQh_m         momentum the fluid gives the body per step (aerodynamic + Maxwell)
+ *   out[3..5]   T = - sum r x dQh_m     its moment about the sphere centre (analytic sphere) or `ref` (masked bodies)
+ *   out[6]      W = - sum dQh_E         energy given to the body (0 for INCRES)
+ *   out[7..9]       sum dQh_B           magnetic field injected into the fluid
+ *   out[10..12]     sum (1-d) B         volume integral of the fluid's B over the body (flux x length)
+ *   out[13]         sum (1-d)           body volume in cells
+ * in lattice units (INCRES: the velocity sets stand for momentum).  lbmhd_body_enable zeroes the accumulator (so does
+ * lbmhd_init); `ref` HOST [3] or NULL (0,0,0), global cell coordinates.  lbmhd_body_read copies the 14 fp64 sums to
+ * HOST (synchronises) or DEVICE (stays asynchronous on the stream) memory, then zeroes them if `reset`: one read per
+ * step gives the per-step series.  The order of the additions across thread blocks is not fixed (atomics). */
+int lbmhd_body_enable(lbmhd_t *h, int enable, const double ref[3]);
+int lbmhd_body_read(lbmhd_t *h, double *out, int reset, int on_device);
+
 /* Raw population access (checkpoint / tests): fp64 [K][Q][N] at this boundary in both precisions, in
  * canonical (k, i, cell) order whatever the streaming layout.  HOST or DEVICE pointer per on_device. */
 int lbmhd_get_populations(lbmhd_t *h, double *g_out, int on_device);

@@ -1,27 +1,53 @@
-"""Builds the C-ABI CUDA library in-tree for sm_100a with nvcc (no torch in the build)."""
+"""Builds the C-ABI CUDA library in-tree for sm_100a with nvcc (no torch in the build).
+
+The kernel templates are instantiated once per (lattice, precision) in csrc/lbmhd_inst.cu; those ten translation units and
+csrc/lbmhd_api.cu compile in parallel into build/*.o and link into liblbmhd.so."""
 import os
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
+_CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "liblbmhd.so")
-SRC = os.path.join(_HERE, "csrc", "lbmhd_api.cu")
-DEPS = [SRC, os.path.join(_HERE, "csrc", "lbmhd_kernels.cuh"), os.path.join(_HERE, "csrc", "lbmhd_lattice.cuh"),
-        os.path.join(_HERE, "csrc", "lbmhd_tma.cuh"),
-        os.path.join(os.path.dirname(_HERE), "include", "lbmhd.h")]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--split-compile", "0",
-              "-shared", "-Xcompiler", "-fPIC"]
+OBJ_DIR = os.path.join(_HERE, "build")
+DEPS = [os.path.join(_CSRC, f) for f in ("lbmhd_api.cu", "lbmhd_inst.cu", "lbmhd_host.h", "lbmhd_ops.cuh", "lbmhd_kernels.cuh",
+                                         "lbmhd_lattice.cuh", "lbmhd_tma.cuh")] + \
+       [os.path.join(os.path.dirname(_HERE), "include", "lbmhd.h")]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
+LATTICES = (3, 2, 5, 4, 1)          # heaviest first: D3Q19, D2Q9, D3Q7, D2Q5, D1Q3
+PRECISIONS = (64, 32)
 
 
 def needs_build():
     return (not os.path.exists(SO)) or os.path.getmtime(SO) < max(os.path.getmtime(d) for d in DEPS)
 
 
-def build(force=False, verbose=False):
+def _units():
+    units = [("api", os.path.join(_CSRC, "lbmhd_api.cu"), [])]
+    for lat in LATTICES:
+        for bits in PRECISIONS:
+            units.append(("inst_%d_%d" % (lat, bits), os.path.join(_CSRC, "lbmhd_inst.cu"),
+                          ["-DLBMHD_INST_LAT=%d" % lat, "-DLBMHD_INST_BITS=%d" % bits]))
+    return units
+
+
+def build(force=False, verbose=False, jobs=None):
     if not force and not needs_build():
         return SO
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + [SRC, "-o", SO]
-    subprocess.run(cmd, check=True, cwd=os.path.join(_HERE, "csrc"))
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    jobs = jobs or int(os.environ.get("LBMHD_BUILD_JOBS", "0")) or min(os.cpu_count() or 1, 11)
+    extra = ["-Xptxas", "-v"] if verbose else []
+
+    def compile_one(unit):
+        name, src, defs = unit
+        obj = os.path.join(OBJ_DIR, name + ".o")
+        subprocess.run([nvcc] + NVCC_FLAGS + extra + defs + ["-c", src, "-o", obj], check=True, cwd=_CSRC)
+        return obj
+
+    with ThreadPoolExecutor(max_workers=jobs) as pool:
+        objs = list(pool.map(compile_one, _units()))
+    subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a"] + objs + ["-o", SO], check=True, cwd=_CSRC)
     return SO
 
 

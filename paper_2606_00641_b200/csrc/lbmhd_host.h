@@ -1,0 +1,92 @@
+// lbmhd_host.h — what the host-side translation units of the library share: the handle behind lbmhd_t, the workspace
+// layout, the per-(lattice, scheme, precision) operation table and the error helpers.  Private to csrc/.
+// The kernel templates are instantiated in lbmhd_inst.cu, once per (lattice, precision) and in parallel; lbmhd_api.cu
+// holds the C entry points and dispatches through OpTable.
+#pragma once
+#include "../../include/lbmhd.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+namespace lbh {
+
+int fail(int code, const char *fmt, ...);      // records the message lbmhd_last_error returns (thread-local), returns code
+
+#define CUDA_TRY(expr)                                                                              \
+  do {                                                                                              \
+    cudaError_t e_ = (expr);                                                                        \
+    if (e_ != cudaSuccess) return ::lbh::fail(LBMHD_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_));      \
+  } while (0)
+struct Geometry {
+  int D, Q, K, NV, iU, iB;
+  double cs2;
+};
+
+constexpr int kMaxDiagBlocks = 1184;   // 8 x 148 SMs
+constexpr int kBodyInts = 14;          // lbmhd_body_read
+constexpr int kTmaTX = 32, kTmaStages = 5;
+
+struct Layout {
+  size_t pstride;        // elements per population plane (N rounded up to 32)
+  size_t pop_bytes;      // one population copy
+  size_t off_pop[2], off_fields, off_M[2], off_mask, off_bsolid, off_dfield, off_partial, off_diag, off_dirs, off_body, total;
+};
+
+}  // namespace lbh
+
+struct lbmhd {
+  lbmhd_params p;
+  lbh::Geometry g;
+  lbh::Layout L;
+  size_t N;
+  double tau[16];
+  cudaStream_t stream;
+  char *ws;
+  int cur;               // A/B: which population copy holds the current state (in place: always 0)
+  int parity;            // in place: 0 = layout P0 (g_j(x) at (x, j)), 1 = layout P1 (after a pull-push step)
+  int mcur;              // in place: which M array holds the moments published by the last step
+  long long t;           // steps done since init
+  long long launches;
+  bool have_mask, have_bsolid, have_dfield;
+  bool body_on;          // body integrals accumulate during the steps
+  double body_ref[3];
+  double usolid[3];
+  bool has_sphere;
+  double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs, sph_eps, sph_om[3];
+  long long sph_t0;
+  int tx, minb;          // x-tile and min blocks/SM (launch bound) of the plain step kernel
+  bool pair;             // fp32: two cells per thread (even nx); LBMHD_PAIR=0 turns it off
+  bool split;            // interior / edge launches split (large grids); LBMHD_SPLIT=0/1 overrides
+  bool use_tma;          // TMA-staged persistent step kernel (needs nx * sizeof(real) % 16 == 0)
+  int num_sms;
+  CUtensorMap tmap[2][2];   // [copy][0: tile-wide box, 1: box 16 bytes wider] 5D views (x, y, z, i, k) of the populations
+};
+
+namespace lbh {
+
+struct OpTable {
+  int (*step)(lbmhd_t *, int);
+  int (*init)(lbmhd_t *, const double *);
+  int (*moments)(lbmhd_t *, double *);
+  int (*diag)(lbmhd_t *, const double *, double *);
+  int (*pops_export)(lbmhd_t *, double *);
+  int (*pops_import)(lbmhd_t *, const double *);
+  int (*refresh_published)(lbmhd_t *);
+  int (*halo_dirs)(int, int *);
+};
+
+// defined by lbmhd_inst.cu, one translation unit per (lattice, precision)
+#define LBH_DECLARE_TABLES(P) \
+  OpTable ops_table_1_##P(int scheme); OpTable ops_table_2_##P(int scheme); OpTable ops_table_3_##P(int scheme); \
+  OpTable ops_table_4_##P(int scheme); OpTable ops_table_5_##P(int scheme);
+LBH_DECLARE_TABLES(64)
+LBH_DECLARE_TABLES(32)
+#undef LBH_DECLARE_TABLES
+
+inline int use_device(const lbmhd_t *h) {
+  CUDA_TRY(cudaSetDevice(h->p.device));
+  return LBMHD_OK;
+}
+
+}  // namespace lbh

@@ -12,6 +12,8 @@
 // scheme: population (k,i) at x - c_i is read only by cell x).  Shifts in x misalign a warp's 256-byte
 // segment by one element; the straddled 32-byte sector is re-read from L2/L1, not from DRAM.
 #pragma once
+#include <cooperative_groups.h>
+#include <cooperative_groups/reduce.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -49,6 +51,8 @@ template <typename real> struct StepArgs {
   double sph_c[3], sph_R, sph_R2, sph_m[3], sph_Bs, sph_u[3];
   double sph_om[3];             // angular velocity of the body: u^B = sph_u + sph_om x r; sph_m is already rotated by the host
   double sph_eps, sph_touch2;   // width of the linear porosity ramp (Eq.15-16), 0 = sharp; (R + eps/2)^2
+  double *body;                 // body integrals accumulator [14] (A21) or nullptr = off
+  double body_ref[3];           // torque reference of masked bodies; an analytic sphere uses its centre
 };
 
 // ---- homogenised solid state at a cell (Eq.13-16; A8, A11, A12) ----------
@@ -347,6 +351,57 @@ __device__ __forceinline__ void frozen_rematerialise(const StepArgs<real> &a, in
   }
 }
 
+// ---- body integrals (A21) ------------------------------------------------
+// What the blend hands over at a cell with d < 1, summed over the body and accumulated over steps:
+//   [0..2] F = -sum dQh_m | [3..5] T = -sum r x dQh_m | [6] W = -sum dQh_E | [7..9] sum dQh_B |
+//   [10..12] sum (1-d) B | [13] sum (1-d).
+// Thread (cell, k) owns dQh_k; k is warp-uniform, so the slots are: the lanes that are here reduce their values
+// and one lane adds to the accumulator (solid cells are 0.2 % of config 5; fluid tiles never get here).
+// One out-of-line copy for every kernel: the lanes that are here reduce up to three values and one lane adds them.
+static __device__ __noinline__ void body_add(double *body, bool solid, int s0, double v0, int s1, double v1, int s2, double v2) {
+  namespace cg = cooperative_groups;
+  const cg::coalesced_group g = cg::coalesced_threads();
+  if (!g.any(solid)) return;
+  if (!solid) v0 = v1 = v2 = 0.0;
+  const double t0 = cg::reduce(g, v0, cg::plus<double>());
+  const double t1 = s1 >= 0 ? cg::reduce(g, v1, cg::plus<double>()) : 0.0;       // slots are warp-uniform (k is)
+  const double t2 = s2 >= 0 ? cg::reduce(g, v2, cg::plus<double>()) : 0.0;
+  if (g.thread_rank() == 0) {
+    atomicAdd(body + s0, t0);
+    if (s1 >= 0) atomicAdd(body + s1, t1);
+    if (s2 >= 0) atomicAdd(body + s2, t2);
+  }
+}
+
+template <int SCHEME, int D, typename real>
+__device__ __forceinline__ void body_accumulate(const StepArgs<real> &a, const CellCtx &c, int k, bool solid, double dq, double d,
+                                                double Qk) {
+  constexpr int nvec = is_ideal(SCHEME) ? 3 : D;
+  constexpr int iB = Vars<SCHEME, D>::iB;
+  int s0 = -1, s1 = -1, s2 = -1;
+  double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+  if (k == 0) {
+    s0 = 13; v0 = 1.0 - d;
+  } else if (k >= 1 && k < 1 + nvec) {
+    const int b = k - 1;
+    const double *ref = a.has_sphere ? a.sph_c : a.body_ref;
+    const double rx = (double)c.x - ref[0];
+    const double ry = D > 1 ? (double)(c.y + (D == 2 ? a.hoff : 0)) - ref[1] : 0.0;
+    const double rz = D > 2 ? (double)(c.z + a.hoff) - ref[2] : 0.0;
+    const double F = -dq;
+    // (r x F)_{b+1} += r_{b+2} F_b,  (r x F)_{b+2} -= r_{b+1} F_b   (indices mod 3)
+    s0 = b; v0 = F;
+    s1 = 3 + (b + 1) % 3; v1 = (b == 0 ? rz : (b == 1 ? rx : ry)) * F;
+    s2 = 3 + (b + 2) % 3; v2 = -(b == 0 ? ry : (b == 1 ? rz : rx)) * F;
+  } else if (is_ideal(SCHEME) && k == 4) {
+    s0 = 6; v0 = -dq;
+  } else if (k >= iB && k < iB + nvec) {
+    s0 = 7 + (k - iB); v0 = dq;
+    s1 = 10 + (k - iB); v1 = (1.0 - d) * Qk;
+  }
+  if (s0 >= 0) body_add(a.body, solid, s0, v0, s1, v1, s2, v2);
+}
+
 // =====================================================================================================
 // Everything after the pull: boundary substitution (A9), moments exchange, div-B estimate, Powell source,
 // solid blend, flux, BGK + direct injection, store (DESIGN.md §2 steps S2-S8; Eq.2-4, 8, 11-14).
@@ -475,15 +530,18 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   if constexpr (SOLID) {
     double uS[3], BS[3];
     const real d = (real)solid_state<real, D>(a, c.x, c.y, c.z, c.n, uS, BS);
+    real dq = real(0);
     if (d < real(1)) {
       real Qh[K];
       solid_blend<SCHEME, D, real>(Qv, a.gamma, d, uS, BS, Qh);
       flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, Phi);
       // dQh plus the Powell source scaled by the porosity d (A8)
-      inj = (pick<K, real>(Qh, k) - Qk) - d * (a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
+      dq = pick<K, real>(Qh, k) - Qk;
+      inj = dq - d * (a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
       if (SCHEME == kIdealD && k == K - 1) inj = -Qk * a.inv_tau_relax;      // relaxation source of Eq.6, not porosity-scaled
       solid = true;
     }
+    if (a.body != nullptr) body_accumulate<SCHEME, D, real>(a, c, k, solid, (double)dq, (double)d, (double)Qk);
   }
   if (!solid) {
     flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, Phi);
@@ -1094,7 +1152,7 @@ diag_partial_kernel(const double *__restrict__ F, double *__restrict__ partial, 
 }
 
 // stage 2: one block folds the per-block partials in block order (deterministic)
-__global__ void __launch_bounds__(kDiagThreads)
+static __global__ void __launch_bounds__(kDiagThreads)
 diag_final_kernel(const double *__restrict__ partial, int nblocks, int K, double *__restrict__ out) {
   __shared__ double sm[32];
   const int nslots = 3 * K + 4;
@@ -1144,7 +1202,7 @@ __global__ void halo_plane_kernel(real *__restrict__ g, size_t pstride, real *__
 }
 
 // ---- bandwidth probe: BabelStream-style copy, 2 fp64 per thread per iteration ----------------
-__global__ void __launch_bounds__(256) copy_probe_kernel(const double2 *__restrict__ a, double2 *__restrict__ b, size_t n2) {
+static __global__ void __launch_bounds__(256) copy_probe_kernel(const double2 *__restrict__ a, double2 *__restrict__ b, size_t n2) {
   for (size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x; j < n2; j += (size_t)gridDim.x * blockDim.x) b[j] = a[j];
 }
 

@@ -74,6 +74,8 @@ def load_library():
     lib.lbmhd_steps_done.restype = C.c_longlong
     lib.lbmhd_launch_count.argtypes = [C.c_void_p]
     lib.lbmhd_launch_count.restype = C.c_longlong
+    lib.lbmhd_body_enable.argtypes = [C.c_void_p, C.c_int, dp]
+    lib.lbmhd_body_read.argtypes = [C.c_void_p, dp, C.c_int, C.c_int]
     lib.lbmhd_copy_probe.argtypes = [dp, dp, C.c_size_t, C.c_int, C.c_void_p]
     lib.lbmhd_last_error.restype = C.c_char_p
     _lib = lib
@@ -84,7 +86,7 @@ EXPORTS = ["lbmhd_num_vars", "lbmhd_num_dirs", "lbmhd_workspace_bytes", "lbmhd_c
            "lbmhd_init", "lbmhd_step", "lbmhd_moments", "lbmhd_set_obstacle", "lbmhd_set_sphere",
            "lbmhd_set_porosity", "lbmhd_set_sphere_width", "lbmhd_set_sphere_rotation", "lbmhd_halo_bytes", "lbmhd_halo_pack",
            "lbmhd_halo_unpack", "lbmhd_get_populations", "lbmhd_set_populations", "lbmhd_steps_done", "lbmhd_launch_count",
-           "lbmhd_copy_probe", "lbmhd_last_error"]
+           "lbmhd_copy_probe", "lbmhd_last_error", "lbmhd_body_enable", "lbmhd_body_read"]
 
 
 def _check(rc, allow=()):
@@ -237,6 +239,22 @@ class Lbmhd:
     def set_sphere_rotation(self, omega):
         om = np.ascontiguousarray(omega, dtype=np.float64)
         _check(self.lib.lbmhd_set_sphere_rotation(self.h, _host_ptr(om)))
+
+    def body_enable(self, enable=True, ref=None):
+        """accumulate the body integrals during the steps (lbmhd_body_enable); ref: torque reference of masked bodies"""
+        r = None if ref is None else np.ascontiguousarray(ref, dtype=np.float64)
+        _check(self.lib.lbmhd_body_enable(self.h, int(bool(enable)), None if r is None else _host_ptr(r)))
+
+    def body_read(self, reset=False, out=None):
+        """F[3] | T[3] | W | I_B[3] | sum (1-d) B [3] | sum (1-d) since init / the last reset.  `out`: a device fp64 tensor
+        of 14 elements (asynchronous), else a numpy array is returned (synchronises)"""
+        if out is not None:
+            assert out.is_cuda and out.dtype == self.torch.float64 and out.numel() >= 14 and out.is_contiguous()
+            _check(self.lib.lbmhd_body_read(self.h, C.c_void_p(out.data_ptr()), int(reset), 1))
+            return out
+        res = np.zeros(14)
+        _check(self.lib.lbmhd_body_read(self.h, _host_ptr(res), int(reset), 0))
+        return res
 
     def populations(self):
         """canonical fp64 [K, Q, nz, ny, nx] on the host (via a device tensor)"""

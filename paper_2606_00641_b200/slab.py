@@ -203,6 +203,14 @@ class LocalSlabGroup:
         axis = 1 if len(self.w["shape"]) == 3 else 2
         return np.concatenate(parts, axis=axis), combine_diag(diags, self.K)
 
+    def body_enable(self, enable=True, ref=None):
+        for s in self.slabs:
+            s.sim.body_enable(enable, ref)
+
+    def body_read(self, reset=False):
+        """body integrals of the whole lattice: every slab sums over its owned cells, the sums add"""
+        return sum(s.sim.body_read(reset) for s in self.slabs)
+
     def close(self):
         for s in self.slabs:
             s.sim.close()

@@ -29,12 +29,23 @@ def random_workload(scheme, lattice, shape, bc, seed, tau=0.7, sphere=None, gamm
                 tau=tau, powell=1.0, bc=bc, steps=0, fields=F, sphere=sphere)
 
 
+def assert_body_close(bg, bo, tol, qmax, extent):
+    """body integrals (A21): sums over the body cells and the steps of terms that are each within ~tol * max|Q|;
+    bo[13] = sum (1 - d) counts cells x steps; torques carry a lever arm of up to the domain extent"""
+    scale = 10 * tol * max(1.0, bo[13]) * qmax
+    bound = np.full(14, scale)
+    bound[3:6] *= extent
+    bound[13] = 10 * tol * max(1.0, bo[13])
+    assert (np.abs(bg - bo) <= bound).all(), (bg, bo, bound)
+
+
 def compare(w, steps, tol=TOL64, mask=None, obstacle=None, precision=64, streaming=0):
     o = oracle_from_workload(w, mask=mask)
     g = gpu_from_workload(w, precision=precision, streaming=streaming)
     if obstacle is not None:
         o.set_obstacle(*obstacle)
         g.set_obstacle(*obstacle)
+    g.body_enable(True)
     o.init(w["fields"])
     g.init(w["fields"])
     o.step(steps)
@@ -44,6 +55,7 @@ def compare(w, steps, tol=TOL64, mask=None, obstacle=None, precision=64, streami
     errs = field_errors(Qg, Qo)
     assert (errs <= tol).all(), errs
     K = o.K
+    assert_body_close(g.body_read(), o.body_read(), tol, do[2 * K:3 * K].max(), max(w["shape"]))
     e_sum, e_abs, e_max = diag_errors(dg, do, K)
     # a sum over N cells, each within tol * max|Q_k|, can be off by tol * N * max|Q_k|; relative to sum|Q_k| that is
     # tol * N max / sum|.| (>= tol; large for a field that lives in a small part of the domain)
