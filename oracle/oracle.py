@@ -61,6 +61,8 @@ def _load():
         lib.oracle_get_populations.argtypes = [C.c_void_p, dp]
         lib.oracle_set_populations.argtypes = [C.c_void_p, dp]
         lib.oracle_source_log.argtypes = [C.c_void_p, dp]
+        lib.oracle_set_sphere_dipoles.argtypes = [C.c_void_p, C.c_int, dp, dp, dp, dp]
+        lib.oracle_set_obstacle_rotation.argtypes = [C.c_void_p, dp, dp]
         lib.oracle_body_read.argtypes = [C.c_void_p, dp, C.c_int]
         lib.oracle_set_body_reference.argtypes = [C.c_void_p, dp]
         lib.oracle_lattice.argtypes = [C.c_int, ip, ip, ip, dp, dp]
@@ -217,6 +219,16 @@ class Oracle:
         om = _f64(omega)
         if self.lib.oracle_set_sphere_rotation(self.h, _dptr(om)):
             raise RuntimeError("oracle_set_sphere_rotation")
+
+    def set_sphere_dipoles(self, offsets, dirs, B_surface, cores):
+        off, m, bs, co = _f64(offsets).reshape(-1, 3), _f64(dirs).reshape(-1, 3), _f64(B_surface).reshape(-1), _f64(cores).reshape(-1)
+        if self.lib.oracle_set_sphere_dipoles(self.h, len(bs), _dptr(off), _dptr(m), _dptr(bs), _dptr(co)):
+            raise RuntimeError("oracle_set_sphere_dipoles")
+
+    def set_obstacle_rotation(self, omega, centre):
+        om, c = _f64(omega), _f64(centre)
+        if self.lib.oracle_set_obstacle_rotation(self.h, _dptr(om), _dptr(c)):
+            raise RuntimeError("oracle_set_obstacle_rotation")
 
     def populations(self):
         g = np.zeros((self.K, self.Q) + self.shape)

@@ -24,6 +24,7 @@
 #endif
 
 #define MAXK 9
+#define MAXDIP 4
 #define NBODY 14          /* body integrals, oracle_body_read */
 #define ACCW (MAXK + NBODY) /* per-row accumulator: source log | body integrals */
 #define MAXQ 19
@@ -232,6 +233,9 @@ struct oracle {
   long sph_t0;         /* step count at which the centre was sph_c0 */
   double sph_om[3];    /* angular velocity Omega of the body (rad per step): u^B(x) = u_s + Omega x r, dipole axis co-rotates */
   double sph_eps;      /* width eps_h of the linear porosity ramp across the sphere surface (Eq.15-16), 0 = sharp */
+  int n_dip;           /* dipole ensemble of the sphere ("four independent, shifted, and smoothed magnetic dipoles"): */
+  double dip_off[MAXDIP][3], dip_m[MAXDIP][3], dip_Bs[MAXDIP], dip_core[MAXDIP];   /* body-frame offset, axis, strength, core radius */
+  double obs_om[3], obs_c[3];   /* masked bodies: u^B(x) = usolid + obs_om x (x - obs_c) */
   double *dfield;      /* lattice porosity d in [0,1] per cell (Eq.15), or NULL: d from the mask (SOLID -> 0) */
   long t;              /* steps done so far */
   double srclog[MAXK];
@@ -326,6 +330,32 @@ int oracle_set_sphere(oracle_t *o, const double centre[3], double radius, const 
     o->sph_u[a] = u_solid[a]; o->sph_m[a] = dipole_dir[a];
   }
   o->sph_R = radius; o->sph_Bs = B_surface; o->sph_t0 = o->t;
+  /* A12: one centred dipole capped at R/2 */
+  o->n_dip = 1;
+  for (int a = 0; a < 3; a++) { o->dip_off[0][a] = 0.0; o->dip_m[0][a] = dipole_dir[a]; }
+  o->dip_Bs[0] = B_surface; o->dip_core[0] = 0.5 * radius;
+  return 0;
+}
+
+/* ensemble of n <= 4 shifted, smoothed dipoles in the body frame; replaces the single dipole of set_sphere:
+ *   B^B(x) = sum_j 1/2 Bs_j (R / max(|r_j|, core_j))^3 [3 (m_j.r^_j) r^_j - m_j],  r_j = x - c(t) - Rot(t) off_j,  m_j -> Rot(t) m_j */
+int oracle_set_sphere_dipoles(oracle_t *o, int n, const double *offset, const double *dir, const double *B_surface, const double *core)
+{
+  if (!o || !o->has_sphere || n < 1 || n > MAXDIP || !offset || !dir || !B_surface || !core) return -1;
+  for (int j = 0; j < n; j++) {
+    if (!(core[j] > 0.0)) return -1;
+    for (int a = 0; a < 3; a++) { o->dip_off[j][a] = offset[3 * j + a]; o->dip_m[j][a] = dir[3 * j + a]; }
+    o->dip_Bs[j] = B_surface[j]; o->dip_core[j] = core[j];
+  }
+  o->n_dip = n;
+  return 0;
+}
+
+/* rigid rotation of the masked / porosity body about `centre`: u^B(x) = u_solid + omega x (x - centre) */
+int oracle_set_obstacle_rotation(oracle_t *o, const double omega[3], const double centre[3])
+{
+  if (!o || !omega || !centre) return -1;
+  for (int a = 0; a < 3; a++) { o->obs_om[a] = omega[a]; o->obs_c[a] = centre[a]; }
   return 0;
 }
 
@@ -426,6 +456,20 @@ int oracle_set_body_reference(oracle_t *o, const double ref[3])
  *                    profile Eq.16; eps_b read as eps_h, A14).
  * dipole B^B(r) = 1/2 B_s (R / max(|r|, R/2))^3 [3 (m.r^) r^ - m], r^ = r/|r| (0 at r = 0).
  * Mask / porosity field: d = dfield[n] if given, else 0 for SOLID cells; u^B uniform, B^B per cell. */
+/* v rotated about the axis Omega by the angle |Omega| dt (Rodrigues); v itself when Omega = 0 */
+static void rotate_about(const double om[3], double dt, const double v[3], double out[3])
+{
+  double om2 = om[0] * om[0] + om[1] * om[1] + om[2] * om[2];
+  out[0] = v[0]; out[1] = v[1]; out[2] = v[2];
+  if (om2 > 0.0) {
+    double omn = sqrt(om2), th = omn * dt, cth = cos(th), sth = sin(th);
+    double e[3] = { om[0] / omn, om[1] / omn, om[2] / omn };
+    double ev = e[0] * v[0] + e[1] * v[1] + e[2] * v[2];
+    double ex[3] = { e[1] * v[2] - e[2] * v[1], e[2] * v[0] - e[0] * v[2], e[0] * v[1] - e[1] * v[0] };
+    for (int a = 0; a < 3; a++) out[a] = v[a] * cth + ex[a] * sth + e[a] * ev * (1.0 - cth);
+  }
+}
+
 static double solid_state(const oracle_t *o, int x, int y, int z, long n, double uB[3], double BB[3])
 {
   if (o->has_sphere) {
@@ -437,16 +481,6 @@ static double solid_state(const oracle_t *o, int x, int y, int z, long n, double
       r[a] = a < o->L.D ? xi[a] - c : 0.0;
       r2 = r2 + r[a] * r[a];
     }
-    /* dipole axis at this step: m0 rotated about Omega by |Omega| (t - t0) (Rodrigues) */
-    double mt[3] = { o->sph_m[0], o->sph_m[1], o->sph_m[2] };
-    double om2 = o->sph_om[0] * o->sph_om[0] + o->sph_om[1] * o->sph_om[1] + o->sph_om[2] * o->sph_om[2];
-    if (om2 > 0.0) {
-      double omn = sqrt(om2), th = omn * dt, cth = cos(th), sth = sin(th);
-      double e[3] = { o->sph_om[0] / omn, o->sph_om[1] / omn, o->sph_om[2] / omn };
-      double em = e[0] * mt[0] + e[1] * mt[1] + e[2] * mt[2];
-      double ex[3] = { e[1] * mt[2] - e[2] * mt[1], e[2] * mt[0] - e[0] * mt[2], e[0] * mt[1] - e[1] * mt[0] };
-      for (int a = 0; a < 3; a++) mt[a] = o->sph_m[a] * cth + ex[a] * sth + e[a] * em * (1.0 - cth);
-    }
     double rn = sqrt(r2);
     double d;
     if (o->sph_eps > 0.0) {
@@ -457,12 +491,21 @@ static double solid_state(const oracle_t *o, int x, int y, int z, long n, double
       d = r2 <= o->sph_R * o->sph_R ? 0.0 : 1.0;
     }
     if (d < 1.0) {
-      double rc = rn > 0.5 * o->sph_R ? rn : 0.5 * o->sph_R;
-      double q = o->sph_R / rc;
-      double amp = 0.5 * o->sph_Bs * (q * q * q);
-      double rh[3], mr = 0.0;
-      for (int a = 0; a < 3; a++) { rh[a] = rn > 0.0 ? r[a] / rn : 0.0; mr += mt[a] * rh[a]; }
-      for (int a = 0; a < 3; a++) BB[a] = amp * (3.0 * mr * rh[a] - mt[a]);
+      BB[0] = BB[1] = BB[2] = 0.0;
+      for (int j = 0; j < o->n_dip; j++) {
+        /* offset and axis at this step: body-frame vectors rotated about Omega by |Omega| (t - t0) */
+        double mt[3], ot[3], rj[3], rj2 = 0.0;
+        rotate_about(o->sph_om, dt, o->dip_m[j], mt);
+        rotate_about(o->sph_om, dt, o->dip_off[j], ot);
+        for (int a = 0; a < 3; a++) { rj[a] = a < o->L.D ? r[a] - ot[a] : 0.0; rj2 = rj2 + rj[a] * rj[a]; }
+        double rjn = sqrt(rj2);
+        double rc = rjn > o->dip_core[j] ? rjn : o->dip_core[j];
+        double q = o->sph_R / rc;
+        double amp = 0.5 * o->dip_Bs[j] * (q * q * q);
+        double rh[3], mr = 0.0;
+        for (int a = 0; a < 3; a++) { rh[a] = rjn > 0.0 ? rj[a] / rjn : 0.0; mr += mt[a] * rh[a]; }
+        for (int a = 0; a < 3; a++) BB[a] += amp * (3.0 * mr * rh[a] - mt[a]);
+      }
       /* rigid body: u^B = u_s + Omega x r ("rotated around a ... tilt vector") */
       uB[0] = o->sph_u[0] + (o->sph_om[1] * r[2] - o->sph_om[2] * r[1]);
       uB[1] = o->sph_u[1] + (o->sph_om[2] * r[0] - o->sph_om[0] * r[2]);
@@ -474,7 +517,12 @@ static double solid_state(const oracle_t *o, int x, int y, int z, long n, double
   if (o->dfield) d = o->dfield[n];
   else if (o->mask[n] == ORC_CELL_SOLID) d = 0.0;
   if (d < 1.0) {
-    for (int a = 0; a < 3; a++) { uB[a] = o->usolid[a]; BB[a] = o->Bsolid ? o->Bsolid[(long)a * o->N + n] : 0.0; }
+    double xi[3] = { (double)x, (double)y, (double)z }, r[3];
+    for (int a = 0; a < 3; a++) r[a] = a < o->L.D ? xi[a] - o->obs_c[a] : 0.0;
+    uB[0] = o->usolid[0] + (o->obs_om[1] * r[2] - o->obs_om[2] * r[1]);
+    uB[1] = o->usolid[1] + (o->obs_om[2] * r[0] - o->obs_om[0] * r[2]);
+    uB[2] = o->usolid[2] + (o->obs_om[0] * r[1] - o->obs_om[1] * r[0]);
+    for (int a = 0; a < 3; a++) BB[a] = o->Bsolid ? o->Bsolid[(long)a * o->N + n] : 0.0;
   }
   return d;
 }

@@ -66,6 +66,13 @@ int  oracle_set_sphere_width(oracle_t *o, double eps);
 /* rigid rotation of the sphere: u^B(x) = u_solid + omega x (x - c), dipole axis rotates with the body */
 int  oracle_set_sphere_rotation(oracle_t *o, const double omega[3]);
 
+/* ensemble of n <= 4 shifted, smoothed dipoles fixed in the body frame of the sphere, replacing the single
+ * dipole of oracle_set_sphere: offset[n][3] from the centre, dir[n][3], B_surface[n], core[n] (cap radius, > 0) */
+int  oracle_set_sphere_dipoles(oracle_t *o, int n, const double *offset, const double *dir, const double *B_surface,
+                               const double *core);
+/* masked / porosity bodies: u^B(x) = u_solid + omega x (x - centre) */
+int  oracle_set_obstacle_rotation(oracle_t *o, const double omega[3], const double centre[3]);
+
 /* body integrals (A21), accumulated over the steps since init or the last reset:
  * out[14] = F[3] | T[3] | W | I_B[3] | sum (1-d) B [3] | sum (1-d);  see vlbm_oracle.c */
 int  oracle_body_read(oracle_t *o, double *out /* [14] or NULL */, int reset);

@@ -110,6 +110,8 @@ class NpVLBM:
         self.sphere_eps = 0.0
         self.sphere_omega = np.zeros(3)
         self.d_field = None
+        self.dipoles = None            # [(offset[3], axis[3], B_surface, core)] in the body frame, replaces the sphere's own dipole
+        self.obst_omega, self.obst_centre = np.zeros(3), np.zeros(3)
         self.t = 0
         self.src_acc = np.zeros(self.K)
         self.body = np.zeros(14)
@@ -169,8 +171,12 @@ class NpVLBM:
             d[self.mask == SOLID] = 0.0
         sol = d < 1.0
         if sol.any():
+            rr = np.zeros(self.shape + (3,))
+            for a in range(self.D):
+                rr[..., a] = self.coord[a] - self.obst_centre[a]
+            urot = np.cross(np.asarray(self.obst_omega, dtype=float), rr)
             for a in range(3):
-                uB[a][sol] = self.u_solid[a]
+                uB[a][sol] = self.u_solid[a] + urot[..., a][sol]
                 if self.B_solid is not None:
                     BB[a][sol] = self.B_solid[a][sol]
         if self.sphere is not None:
@@ -186,18 +192,29 @@ class NpVLBM:
             else:
                 ds = np.where(r2 <= R * R, 0.0, 1.0)
             ins = ds < 1.0
-            rc = np.maximum(rn, 0.5 * R)
-            with np.errstate(invalid="ignore", divide="ignore"):
-                rh = np.where(rn > 0, r / np.where(rn > 0, rn, 1.0), 0.0)
             om = np.asarray(self.sphere_omega, dtype=float)
             omn = np.linalg.norm(om)
-            if omn > 0:                                  # Rodrigues rotation of the dipole axis by |Omega| (t - t0)
+
+            def rot(v):                                  # Rodrigues rotation about Omega by |Omega| (t - t0)
+                v = np.asarray(v, dtype=float)
+                if omn == 0:
+                    return v
                 e, th = om / omn, omn * (self.t - t0)
-                mh = mh * np.cos(th) + np.cross(e, mh) * np.sin(th) + e * (e @ mh) * (1 - np.cos(th))
+                return v * np.cos(th) + np.cross(e, v) * np.sin(th) + e * (e @ v) * (1 - np.cos(th))
             urot = np.cross(om.reshape(1, 1, 1, 3), np.moveaxis(r, 0, -1))     # Omega x r
             urot = np.moveaxis(urot, -1, 0)
-            mr = (mh.reshape(3, 1, 1, 1) * rh).sum(0)
-            dip = 0.5 * Bs * (R / rc) ** 3 * (3.0 * mr * rh - mh.reshape(3, 1, 1, 1))
+            ensemble = self.dipoles if self.dipoles is not None else [(np.zeros(3), mh, Bs, 0.5 * R)]
+            dip = np.zeros((3,) + self.shape)
+            for off, axis, bsj, core in ensemble:
+                oj, mj = rot(off), rot(axis)
+                rj = np.zeros((3,) + self.shape)
+                for a in range(self.D):
+                    rj[a] = r[a] - oj[a]
+                rjn = np.sqrt((rj * rj).sum(0))
+                with np.errstate(invalid="ignore", divide="ignore"):
+                    rh = np.where(rjn > 0, rj / np.where(rjn > 0, rjn, 1.0), 0.0)
+                mr = (mj.reshape(3, 1, 1, 1) * rh).sum(0)
+                dip += 0.5 * bsj * (R / np.maximum(rjn, core)) ** 3 * (3.0 * mr * rh - mj.reshape(3, 1, 1, 1))
             d[ins] = ds[ins]
             for a in range(3):
                 uB[a][ins] = us[a] + urot[a][ins]
