@@ -146,6 +146,19 @@ size_t lbmhd_halo_bytes(const lbmhd_t *h, int full);
 int lbmhd_halo_pack(lbmhd_t *h, int side, int full, void *buf);
 int lbmhd_halo_unpack(lbmhd_t *h, int side, int full, const void *buf);
 
+/* Dipole ensemble of the sphere ("an analytical ensemble of four independent, shifted, and smoothed magnetic
+ * dipoles"): replaces the single dipole of lbmhd_set_sphere (call that first) by n in 1..4 dipoles fixed in the body frame,
+ *   B^B(x) = sum_j 1/2 B_surface[j] (R / max(|r_j|, core[j]))^3 [3 (m_j.r^_j) r^_j - m_j],  r_j = x - c(t) - Rot(t) offset[j],
+ * m_j = Rot(t) dir[j], Rot(t) the rotation of lbmhd_set_sphere_rotation since the sphere was set.  HOST arrays offset[n][3],
+ * dir[n][3] (used as given, not normalised), B_surface[n], core[n] (> 0, the smoothing radius); copied. */
+int lbmhd_set_sphere_dipoles(lbmhd_t *h, int n, const double *offset, const double *dir, const double *B_surface,
+                             const double *core);
+
+/* Rigid rotation of the masked / porosity body: u^B(x) = u_solid + omega x (x - centre), global cell
+ * coordinates, HOST [3] each, lattice units (radians per step).  The mask itself is the caller's: re-voxelise and pass it
+ * with lbmhd_set_obstacle / lbmhd_set_porosity (device pointers keep that asynchronous) as the body turns. */
+int lbmhd_set_obstacle_rotation(lbmhd_t *h, const double omega[3], const double centre[3]);
+
 /* Body integrals ("per-timestep surface integrals of net magnetic flux, forces, torques,
  * electromagnetic work"; the paper prints no formulas: DESIGN.md reading A21 takes them from what the blend of
  * Eq.13-14 hands over).  While enabled every lbmhd_step adds, over the cells with d < 1,

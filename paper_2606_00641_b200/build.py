@@ -3,6 +3,7 @@
 The kernel templates are instantiated once per (lattice, precision) in csrc/lbmhd_inst.cu; those ten translation units and
 csrc/lbmhd_api.cu compile in parallel into build/*.o and link into liblbmhd.so."""
 import os
+import shutil
 import subprocess
 from concurrent.futures import ThreadPoolExecutor
 
@@ -48,6 +49,7 @@ def build(force=False, verbose=False, jobs=None):
     with ThreadPoolExecutor(max_workers=jobs) as pool:
         objs = list(pool.map(compile_one, _units()))
     subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a"] + objs + ["-o", SO], check=True, cwd=_CSRC)
+    shutil.rmtree(OBJ_DIR, ignore_errors=True)      # intermediates only: every unit depends on the same headers
     return SO
 
 

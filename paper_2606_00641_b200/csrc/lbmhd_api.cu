@@ -304,8 +304,11 @@ int lbmhd_set_sphere(lbmhd_t *h, const double centre[3], double radius, const do
   if (!(radius > 0.0)) { h->has_sphere = false; return LBMHD_OK; }
   if (!centre || !u_solid || !dipole_dir) return fail(LBMHD_EINVAL, "NULL argument");
   h->has_sphere = true;
-  for (int c = 0; c < 3; c++) { h->sph_c0[c] = centre[c]; h->sph_u[c] = u_solid[c]; h->sph_m[c] = dipole_dir[c]; }
-  h->sph_R = radius; h->sph_Bs = B_surface; h->sph_t0 = h->t;
+  for (int c = 0; c < 3; c++) { h->sph_c0[c] = centre[c]; h->sph_u[c] = u_solid[c]; }
+  h->sph_R = radius; h->sph_t0 = h->t;
+  h->n_dip = 1;                                  // A12: one centred dipole capped at R/2
+  for (int c = 0; c < 3; c++) { h->dip_off[0][c] = 0.0; h->dip_m[0][c] = dipole_dir[c]; }
+  h->dip_Bs[0] = B_surface; h->dip_core[0] = 0.5 * radius;
   return LBMHD_OK;
 }
 
@@ -321,6 +324,26 @@ int lbmhd_set_porosity(lbmhd_t *h, const double *d_field, int on_device) {
   }
   h->have_dfield = true;
   CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LBMHD_OK;
+}
+
+int lbmhd_set_sphere_dipoles(lbmhd_t *h, int n, const double *offset, const double *dir, const double *B_surface, const double *core) {
+  if (!h || !offset || !dir || !B_surface || !core) return fail(LBMHD_EINVAL, "NULL argument");
+  if (!h->has_sphere) return fail(LBMHD_EINVAL, "lbmhd_set_sphere first");
+  if (n < 1 || n > 4) return fail(LBMHD_EINVAL, "1 to 4 dipoles, got %d", n);
+  for (int j = 0; j < n; j++)
+    if (!(core[j] > 0.0)) return fail(LBMHD_EINVAL, "core radius of dipole %d must be > 0", j);
+  for (int j = 0; j < n; j++) {
+    for (int c = 0; c < 3; c++) { h->dip_off[j][c] = offset[3 * j + c]; h->dip_m[j][c] = dir[3 * j + c]; }
+    h->dip_Bs[j] = B_surface[j]; h->dip_core[j] = core[j];
+  }
+  h->n_dip = n;
+  return LBMHD_OK;
+}
+
+int lbmhd_set_obstacle_rotation(lbmhd_t *h, const double omega[3], const double centre[3]) {
+  if (!h || !omega || !centre) return fail(LBMHD_EINVAL, "NULL argument");
+  for (int c = 0; c < 3; c++) { h->obs_om[c] = omega[c]; h->obs_c[c] = centre[c]; }
   return LBMHD_OK;
 }
 

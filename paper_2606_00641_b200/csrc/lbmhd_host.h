@@ -53,7 +53,10 @@ struct lbmhd {
   double body_ref[3];
   double usolid[3];
   bool has_sphere;
-  double sph_c0[3], sph_R, sph_u[3], sph_m[3], sph_Bs, sph_eps, sph_om[3];
+  double sph_c0[3], sph_R, sph_u[3], sph_eps, sph_om[3];
+  int n_dip;             // dipole ensemble in the body frame (lbmhd_set_sphere: one centred dipole capped at R/2)
+  double dip_off[4][3], dip_m[4][3], dip_Bs[4], dip_core[4];
+  double obs_om[3], obs_c[3];   // rigid rotation of masked bodies
   long long sph_t0;
   int tx, minb;          // x-tile and min blocks/SM (launch bound) of the plain step kernel
   bool pair;             // fp32: two cells per thread (even nx); LBMHD_PAIR=0 turns it off

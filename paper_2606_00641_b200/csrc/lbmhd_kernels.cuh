@@ -48,8 +48,11 @@ template <typename real> struct StepArgs {
   double *M_next;               // in-place modes: moments published by this step
   int hoff;                     // slab decomposition: global index of local plane 0 along the slowest lattice axis
   int has_sphere;
-  double sph_c[3], sph_R, sph_R2, sph_m[3], sph_Bs, sph_u[3];
-  double sph_om[3];             // angular velocity of the body: u^B = sph_u + sph_om x r; sph_m is already rotated by the host
+  double sph_c[3], sph_R, sph_R2, sph_u[3];
+  double sph_om[3];             // angular velocity of the body: u^B = sph_u + sph_om x r
+  int n_dip;                    // dipole ensemble of the sphere, offsets and axes already rotated by the host
+  double dip_off[4][3], dip_m[4][3], dip_Bs[4], dip_core[4];
+  double obs_om[3], obs_c[3];   // masked bodies: u^B = usolid + obs_om x (x - obs_c)
   double sph_eps, sph_touch2;   // width of the linear porosity ramp (Eq.15-16), 0 = sharp; (R + eps/2)^2
   double *body;                 // body integrals accumulator [14] (A21) or nullptr = off
   double body_ref[3];           // torque reference of masked bodies; an analytic sphere uses its centre
@@ -76,18 +79,26 @@ __device__ __forceinline__ double solid_state(const StepArgs<real> &a, int x, in
       if (a.sph_eps > 0.0) d = fmin(fmax((rn - a.sph_R) / a.sph_eps + 0.5, 0.0), 1.0);
       else d = r2 <= a.sph_R2 ? 0.0 : 1.0;
       if (d < 1.0) {
-        const double rc = rn > 0.5 * a.sph_R ? rn : 0.5 * a.sph_R;
-        const double q = a.sph_R / rc;
-        const double amp = 0.5 * a.sph_Bs * (q * q * q);
-        double rh[3], mr = 0.0;
+        BS[0] = BS[1] = BS[2] = 0.0;
+        for (int j = 0; j < a.n_dip; j++) {     // 1/2 Bs_j (R / max(|r_j|, core_j))^3 [3 (m_j.r^_j) r^_j - m_j]
+          double rj[3], rj2 = 0.0;
 #pragma unroll
-        for (int c = 0; c < 3; c++) {
-          rh[c] = rn > 0.0 ? r[c] / rn : 0.0;
-          mr += a.sph_m[c] * rh[c];
-        }
+          for (int c = 0; c < 3; c++) {
+            rj[c] = c < D ? r[c] - a.dip_off[j][c] : 0.0;
+            rj2 = rj2 + rj[c] * rj[c];
+          }
+          const double rjn = sqrt(rj2);
+          const double rc = rjn > a.dip_core[j] ? rjn : a.dip_core[j];
+          const double q = a.sph_R / rc;
+          const double amp = 0.5 * a.dip_Bs[j] * (q * q * q);
+          double rh[3], mr = 0.0;
 #pragma unroll
-        for (int c = 0; c < 3; c++) {
-          BS[c] = amp * (3.0 * mr * rh[c] - a.sph_m[c]);
+          for (int c = 0; c < 3; c++) {
+            rh[c] = rjn > 0.0 ? rj[c] / rjn : 0.0;
+            mr += a.dip_m[j][c] * rh[c];
+          }
+#pragma unroll
+          for (int c = 0; c < 3; c++) BS[c] += amp * (3.0 * mr * rh[c] - a.dip_m[j][c]);
         }
         uS[0] = a.sph_u[0] + (a.sph_om[1] * r[2] - a.sph_om[2] * r[1]);
         uS[1] = a.sph_u[1] + (a.sph_om[2] * r[0] - a.sph_om[0] * r[2]);
@@ -100,11 +111,14 @@ __device__ __forceinline__ double solid_state(const StepArgs<real> &a, int x, in
   if (a.dfield != nullptr) d = a.dfield[n];
   else if (a.mask != nullptr && a.mask[n] == CELL_SOLID) d = 0.0;
   if (d < 1.0) {
+    const double rx = (double)x - a.obs_c[0];
+    const double ry = D > 1 ? (double)(y + (D == 2 ? a.hoff : 0)) - a.obs_c[1] : 0.0;
+    const double rz = D > 2 ? (double)(z + a.hoff) - a.obs_c[2] : 0.0;
+    uS[0] = a.usolid[0] + (a.obs_om[1] * rz - a.obs_om[2] * ry);
+    uS[1] = a.usolid[1] + (a.obs_om[2] * rx - a.obs_om[0] * rz);
+    uS[2] = a.usolid[2] + (a.obs_om[0] * ry - a.obs_om[1] * rx);
 #pragma unroll
-    for (int c = 0; c < 3; c++) {
-      uS[c] = a.usolid[c];
-      BS[c] = a.Bsolid != nullptr ? a.Bsolid[(size_t)c * ((size_t)a.nx * a.ny * a.nz) + n] : 0.0;
-    }
+    for (int c = 0; c < 3; c++) BS[c] = a.Bsolid != nullptr ? a.Bsolid[(size_t)c * ((size_t)a.nx * a.ny * a.nz) + n] : 0.0;
   }
   return d;
 }

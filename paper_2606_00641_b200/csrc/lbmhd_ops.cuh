@@ -132,7 +132,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     a.mask = h->have_mask ? (const unsigned char *)(h->ws + h->L.off_mask) : nullptr;
     a.Bsolid = h->have_bsolid ? (const double *)(h->ws + h->L.off_bsolid) : nullptr;
     a.dfield = h->have_dfield ? (const double *)(h->ws + h->L.off_dfield) : nullptr;
-    for (int c = 0; c < 3; c++) a.usolid[c] = h->usolid[c];
+    for (int c = 0; c < 3; c++) { a.usolid[c] = h->usolid[c]; a.obs_om[c] = h->obs_om[c]; a.obs_c[c] = h->obs_c[c]; }
     {
       const long long es = (long long)sizeof(real);
       for (int i = 0; i < Q; i++) {
@@ -150,8 +150,9 @@ template <int LAT, int SCHEME, typename real> struct Ops {
       a.sph_R2 = h->sph_R * h->sph_R;
       a.sph_eps = h->sph_eps;
       a.sph_touch2 = h->sph_eps > 0.0 ? (h->sph_R + 0.5 * h->sph_eps) * (h->sph_R + 0.5 * h->sph_eps) : a.sph_R2;
-      a.sph_Bs = h->sph_Bs;
-      for (int c = 0; c < 3; c++) { a.sph_m[c] = h->sph_m[c]; a.sph_u[c] = h->sph_u[c]; }
+      a.n_dip = h->n_dip;
+      for (int j = 0; j < h->n_dip; j++) { a.dip_Bs[j] = h->dip_Bs[j]; a.dip_core[j] = h->dip_core[j]; }
+      for (int c = 0; c < 3; c++) a.sph_u[c] = h->sph_u[c];
     }
     for (int s = 0; s < n_steps; s++) {
       const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
@@ -168,17 +169,22 @@ template <int LAT, int SCHEME, typename real> struct Ops {
           const volatile double prod = dt * h->sph_u[c];
           a.sph_c[c] = h->sph_c0[c] + prod;
           a.sph_om[c] = h->sph_om[c];
-          a.sph_m[c] = h->sph_m[c];
         }
+        // body-frame offsets and axes of the dipoles at this step: Rodrigues rotation about Omega by |Omega| (t - t0)
         const double om2 = h->sph_om[0] * h->sph_om[0] + h->sph_om[1] * h->sph_om[1] + h->sph_om[2] * h->sph_om[2];
-        if (om2 > 0.0) {      // dipole axis co-rotates: Rodrigues rotation of m0 about Omega by |Omega| (t - t0)
-          const double omn = sqrt(om2), th = omn * dt, cth = cos(th), sth = sin(th);
-          const double e[3] = {h->sph_om[0] / omn, h->sph_om[1] / omn, h->sph_om[2] / omn};
-          const double *m0 = h->sph_m;
-          const double em = e[0] * m0[0] + e[1] * m0[1] + e[2] * m0[2];
-          const double ex[3] = {e[1] * m0[2] - e[2] * m0[1], e[2] * m0[0] - e[0] * m0[2], e[0] * m0[1] - e[1] * m0[0]};
-          for (int c = 0; c < 3; c++) a.sph_m[c] = m0[c] * cth + ex[c] * sth + e[c] * em * (1.0 - cth);
-        }
+        for (int j = 0; j < h->n_dip; j++)
+          for (int which = 0; which < 2; which++) {
+            const double *v = which ? h->dip_off[j] : h->dip_m[j];
+            double *out = which ? a.dip_off[j] : a.dip_m[j];
+            for (int c = 0; c < 3; c++) out[c] = v[c];
+            if (om2 > 0.0) {
+              const double omn = sqrt(om2), th = omn * dt, cth = cos(th), sth = sin(th);
+              const double e[3] = {h->sph_om[0] / omn, h->sph_om[1] / omn, h->sph_om[2] / omn};
+              const double ev = e[0] * v[0] + e[1] * v[1] + e[2] * v[2];
+              const double ex[3] = {e[1] * v[2] - e[2] * v[1], e[2] * v[0] - e[0] * v[2], e[0] * v[1] - e[1] * v[0]};
+              for (int c = 0; c < 3; c++) out[c] = v[c] * cth + ex[c] * sth + e[c] * ev * (1.0 - cth);
+            }
+          }
       }
       cudaError_t e;
       if (sizeof(real) == 4 && h->pair) e = h->minb == 2 ? launch_step_pair<2>(h, a) : (h->minb == 4 ? launch_step_pair<4>(h, a) : launch_step_pair<3>(h, a));

@@ -74,6 +74,8 @@ def load_library():
     lib.lbmhd_steps_done.restype = C.c_longlong
     lib.lbmhd_launch_count.argtypes = [C.c_void_p]
     lib.lbmhd_launch_count.restype = C.c_longlong
+    lib.lbmhd_set_sphere_dipoles.argtypes = [C.c_void_p, C.c_int, dp, dp, dp, dp]
+    lib.lbmhd_set_obstacle_rotation.argtypes = [C.c_void_p, dp, dp]
     lib.lbmhd_body_enable.argtypes = [C.c_void_p, C.c_int, dp]
     lib.lbmhd_body_read.argtypes = [C.c_void_p, dp, C.c_int, C.c_int]
     lib.lbmhd_copy_probe.argtypes = [dp, dp, C.c_size_t, C.c_int, C.c_void_p]
@@ -86,7 +88,8 @@ EXPORTS = ["lbmhd_num_vars", "lbmhd_num_dirs", "lbmhd_workspace_bytes", "lbmhd_c
            "lbmhd_init", "lbmhd_step", "lbmhd_moments", "lbmhd_set_obstacle", "lbmhd_set_sphere",
            "lbmhd_set_porosity", "lbmhd_set_sphere_width", "lbmhd_set_sphere_rotation", "lbmhd_halo_bytes", "lbmhd_halo_pack",
            "lbmhd_halo_unpack", "lbmhd_get_populations", "lbmhd_set_populations", "lbmhd_steps_done", "lbmhd_launch_count",
-           "lbmhd_copy_probe", "lbmhd_last_error", "lbmhd_body_enable", "lbmhd_body_read"]
+           "lbmhd_copy_probe", "lbmhd_last_error", "lbmhd_body_enable", "lbmhd_body_read",
+           "lbmhd_set_sphere_dipoles", "lbmhd_set_obstacle_rotation"]
 
 
 def _check(rc, allow=()):
@@ -240,6 +243,19 @@ class Lbmhd:
         om = np.ascontiguousarray(omega, dtype=np.float64)
         _check(self.lib.lbmhd_set_sphere_rotation(self.h, _host_ptr(om)))
 
+    def set_sphere_dipoles(self, offsets, dirs, B_surface, cores):
+        off = np.ascontiguousarray(offsets, dtype=np.float64).reshape(-1, 3)
+        m = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
+        bs = np.ascontiguousarray(B_surface, dtype=np.float64).reshape(-1)
+        co = np.ascontiguousarray(cores, dtype=np.float64).reshape(-1)
+        assert len(off) == len(m) == len(bs) == len(co)
+        _check(self.lib.lbmhd_set_sphere_dipoles(self.h, len(bs), _host_ptr(off), _host_ptr(m), _host_ptr(bs), _host_ptr(co)))
+
+    def set_obstacle_rotation(self, omega, centre):
+        om = np.ascontiguousarray(omega, dtype=np.float64)
+        c = np.ascontiguousarray(centre, dtype=np.float64)
+        _check(self.lib.lbmhd_set_obstacle_rotation(self.h, _host_ptr(om), _host_ptr(c)))
+
     def body_enable(self, enable=True, ref=None):
         """accumulate the body integrals during the steps (lbmhd_body_enable); ref: torque reference of masked bodies"""
         r = None if ref is None else np.ascontiguousarray(ref, dtype=np.float64)
@@ -304,6 +320,9 @@ def from_workload(w, precision=64, device=0, streaming=STREAM_AB):
             sim.set_sphere_width(s["width"])
         if s.get("omega") is not None:
             sim.set_sphere_rotation(s["omega"])
+        if s.get("dipoles"):
+            dp = s["dipoles"]
+            sim.set_sphere_dipoles(dp["offsets"], dp["dirs"], dp["B_surface"], dp["cores"])
     return sim
 
 

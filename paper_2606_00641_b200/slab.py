@@ -83,6 +83,9 @@ class Slab:
                 self.sim.set_sphere_width(s["width"])
             if s.get("omega") is not None:
                 self.sim.set_sphere_rotation(s["omega"])
+            if s.get("dipoles"):
+                dp = s["dipoles"]
+                self.sim.set_sphere_dipoles(dp["offsets"], dp["dirs"], dp["B_surface"], dp["cores"])
         self.lo, self.hi = self.geo["lo"], self.geo["hi"]
 
     def local_fields(self, fields):

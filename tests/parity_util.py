@@ -21,6 +21,9 @@ def oracle_from_workload(w, mask=None):
             o.set_sphere_width(s["width"])
         if s.get("omega") is not None:
             o.set_sphere_rotation(s["omega"])
+        if s.get("dipoles"):
+            dp = s["dipoles"]
+            o.set_sphere_dipoles(dp["offsets"], dp["dirs"], dp["B_surface"], dp["cores"])
     return o
 
 

@@ -107,3 +107,71 @@ def test_sharded_body_integrals_add_up(parts):
     _, do = o.moments()
     assert_body_close(grp.body_read(), o.body_read(), TOL64, do[2 * o.K:3 * o.K].max(), 48)
     grp.close()
+
+
+def dipoles(R):
+    """four dipoles inside a body of radius R; cores >= 0.45 R keep the capped field below ~0.1 (lattice units)"""
+    return dict(offsets=R / 5.0 * np.array([[1.5, 0.0, 0.5], [-1.0, 2.0, 0.0], [0.0, -1.5, -2.0], [0.5, 0.5, 2.5]]),
+                dirs=np.array([[0.0, 0.0, 1.0], [0.6, 0.0, 0.8], [1.0, 0.0, 0.0], [0.0, -0.8, 0.6]]),
+                B_surface=np.array([0.01, -0.008, 0.006, 0.009]), cores=R * np.array([0.5, 0.6, 0.45, 0.7]))
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+@pytest.mark.parametrize("precision,tol", [(64, TOL64), (32, TOL32)])
+@pytest.mark.parametrize("lattice,shape", [("D3Q19", (72, 24, 20)), ("D2Q9", (90, 40))])
+def test_dipole_ensemble_parity(lattice, shape, precision, tol, streaming):
+    """four shifted, capped dipoles fixed in the frame of the tumbling sphere"""
+    from test_parity_gpu import compare
+    w = sphere_workload("IDEAL", lattice, shape, seed=61)
+    w["sphere"]["dipoles"] = dipoles(w["sphere"]["radius"])
+    compare(w, 11, tol=tol, precision=precision, streaming=streaming)
+
+
+def test_dipole_ensemble_sharded():
+    w = sphere_workload("IDEAL", "D3Q19", (48, 16, 18), seed=62)
+    w["sphere"]["dipoles"] = dipoles(w["sphere"]["radius"])
+    o = oracle_from_workload(w)
+    grp = slab.LocalSlabGroup(w, 3)
+    o.init(w["fields"])
+    grp.init(w["fields"])
+    o.step(6)
+    grp.step(6)
+    Qo, _ = o.moments()
+    Qg, _ = grp.moments()
+    from parity_util import field_errors
+    assert (field_errors(Qg, Qo) <= TOL64).all()
+    grp.close()
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+@pytest.mark.parametrize("scheme,lattice,shape", [("IDEAL", "D3Q19", (70, 14, 12)), ("INCRES", "D2Q9", (80, 30))])
+def test_rotating_masked_body_parity(scheme, lattice, shape, streaming):
+    """u^B = u_solid + omega x (x - centre) at the cells of a masked body with porosity"""
+    from parity_util import field_errors
+    rng = np.random.default_rng(71)
+    D = len(shape)
+    s = zyx(shape)
+    w = random_workload(scheme, lattice, shape, (1, 1) + (0,) * 4, seed=72)
+    mask = np.zeros(s, dtype=np.uint8)
+    mask[..., 4:11, 20:41] = 2
+    d = np.ones(s)
+    d[mask == 2] = rng.random(int((mask == 2).sum())) * 0.9
+    Bs = 0.05 * (rng.random((3,) + s) - 0.5)
+    cen = np.array([30.5, 7.25, 6.0 if D == 3 else 0.0])
+    om = np.array([0.002, -0.003, 0.004]) if D == 3 else np.array([0.0, 0.0, 0.004])
+    o = oracle_from_workload(w)
+    g = gpu_from_workload(w, streaming=streaming)
+    for sim in (o, g):
+        sim.set_obstacle(mask, np.array([0.02, -0.01, 0.015 if D == 3 else 0.0]), Bs)
+        sim.set_porosity(d)
+        sim.set_obstacle_rotation(om, cen)
+    o.set_body_reference(cen)
+    g.body_enable(True, cen)
+    o.init(w["fields"])
+    g.init(w["fields"])
+    o.step(8)
+    g.step(8)
+    Qo, do = o.moments()
+    assert (field_errors(g.moments()[0], Qo) <= TOL64).all()
+    assert_body_close(g.body_read(), o.body_read(), TOL64, do[2 * o.K:3 * o.K].max(), max(shape))
+    g.close()
