@@ -14,7 +14,7 @@ _SRC = os.path.join(_HERE, "vlbm_oracle.c")
 _HDR = os.path.join(_HERE, "vlbm_oracle.h")
 
 D1Q3, D2Q9, D3Q19, D2Q5, D3Q7 = 1, 2, 3, 4, 5
-IDEAL, INCRES, IDEAL_DIVB = 0, 1, 2
+IDEAL, INCRES, IDEAL_DIVB, RESIST = 0, 1, 2, 3
 BC_PERIODIC, BC_ZEROGRAD, BC_INFLOW = 0, 1, 2
 CELL_FLUID, CELL_FROZEN, CELL_SOLID = 0, 1, 2
 
@@ -34,7 +34,7 @@ class OracleParams(C.Structure):
                 ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
                 ("gamma", C.c_double), ("c0sq", C.c_double),
                 ("nu", C.c_double), ("eta", C.c_double),
-                ("tau", C.c_double * 16), ("tau_relax", C.c_double), ("eta_jc", C.c_double), ("powell", C.c_double), ("bc", C.c_int * 6)]
+                ("tau", C.c_double * 32), ("tau_relax", C.c_double), ("eta_jc", C.c_double), ("powell", C.c_double), ("bc", C.c_int * 6)]
 
 
 _lib = None
@@ -95,8 +95,8 @@ def make_params(scheme, lattice, shape, gamma=5.0 / 3.0, c0sq=1.0 / 12.0, nu=0.0
     dims = list(shape) + [1] * (3 - len(shape))
     p.nx, p.ny, p.nz = dims
     p.gamma, p.c0sq, p.nu, p.eta, p.powell = gamma, c0sq, nu, eta, powell
-    taus = [tau] * 16 if np.isscalar(tau) else list(tau) + [0.0] * (16 - len(tau))
-    for k in range(16):
+    taus = [tau] * 32 if np.isscalar(tau) else list(tau) + [0.0] * (32 - len(tau))
+    for k in range(32):
         p.tau[k] = taus[k]
     p.tau_relax = tau_relax
     p.eta_jc = eta_jc

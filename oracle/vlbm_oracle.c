@@ -23,7 +23,7 @@
 #include <omp.h>
 #endif
 
-#define MAXK 9
+#define MAXK 17
 #define MAXDIP 4
 #define NBODY 14          /* body integrals, oracle_body_read */
 #define ACCW (MAXK + NBODY) /* per-row accumulator: source log | body integrals */
@@ -92,8 +92,14 @@ int oracle_lattice(int lattice, int *D, int *Q, int *c, double *w, double *cs2)
   return 0;
 }
 
-static int is_ideal(int scheme) { return scheme == ORC_IDEAL || scheme == ORC_IDEAL_DIVB; }
-static int num_vars(int scheme, int D) { return scheme == ORC_IDEAL ? 8 : (scheme == ORC_IDEAL_DIVB ? 9 : 1 + 2 * D); }
+static int is_ideal(int scheme) { return scheme == ORC_IDEAL || scheme == ORC_IDEAL_DIVB || scheme == ORC_RESIST; }   /* first 8 variables (rho, m, E, B) */
+static int num_vars(int scheme, int D)
+{
+  if (scheme == ORC_IDEAL) return 8;
+  if (scheme == ORC_IDEAL_DIVB) return 9;
+  if (scheme == ORC_RESIST) return 8 + 3 * D;       /* + G_ab = tau_M d_a B_b, a < D, b < 3, index 8 + 3 a + b */
+  return 1 + 2 * D;
+}
 
 int oracle_num_vars(const oracle_params *p)
 {
@@ -123,8 +129,10 @@ int oracle_get_threads(void)
 /* IDEAL: Eq.11 PAPER.md:142 with the EOS Eq.8; magnetic pressure |B|^2/2.
  * INCRES (A3): P carries kinematic pressure, dP/dt + c0^2 div u = 0; momentum flux u u + (P + B^2/2) I - B B;
  * induction flux u B - B u. */
-static void flux_eval(int scheme, int D, double gamma, double c0sq, const double *Q, double Phi[MAXK][3])
+static void flux_eval(const oracle_params *prm, int D, const double *Q, double Phi[MAXK][3])
 {
+  const int scheme = prm->scheme;
+  const double gamma = prm->gamma, c0sq = prm->c0sq;
   int a, b;
   if (is_ideal(scheme)) {
     double rho = Q[0], E = Q[4];
@@ -143,6 +151,27 @@ static void flux_eval(int scheme, int D, double gamma, double c0sq, const double
       for (b = 0; b < 3; b++) Phi[5 + b][a] = u[a] * B[b] - B[a] * u[b];
       /* Eq.10 PAPER.md:136 traced: the relaxation variable D = tr G has the flux D u - B */
       if (scheme == ORC_IDEAL_DIVB) Phi[8][a] = Q[8] * u[a] - B[a];
+    }
+    if (scheme == ORC_RESIST) {
+      /* dissipative system, PAPER.md:122 with the transported gradients of Eq.9-10 PAPER.md:132-136 (A22):
+       *   g_cb = G_cb / tau_M ~ d_c B_b;  current j = curl B: j_e = eps_ecb g_cb (c < D);
+       *   Phi_{B_b},a -= eta g_ab;  Phi_E,a += eta (j x B)_a;  Phi_{G_cb},a = G_cb u_a - delta_ca B_b */
+      const double *Gv = Q + 8;
+      const double eta = prm->eta, itm = 1.0 / prm->tau_relax;
+      double g[3][3], j[3], jxB[3];
+      int c;
+      for (c = 0; c < 3; c++) for (b = 0; b < 3; b++) g[c][b] = c < D ? Gv[3 * c + b] * itm : 0.0;
+      j[0] = g[1][2] - g[2][1];
+      j[1] = g[2][0] - g[0][2];
+      j[2] = g[0][1] - g[1][0];
+      jxB[0] = j[1] * B[2] - j[2] * B[1];
+      jxB[1] = j[2] * B[0] - j[0] * B[2];
+      jxB[2] = j[0] * B[1] - j[1] * B[0];
+      for (a = 0; a < D; a++) {
+        Phi[4][a] += eta * jxB[a];
+        for (b = 0; b < 3; b++) Phi[5 + b][a] -= eta * g[a][b];
+        for (c = 0; c < D; c++) for (b = 0; b < 3; b++) Phi[8 + 3 * c + b][a] = Gv[3 * c + b] * u[a] - (c == a ? B[b] : 0.0);
+      }
     }
   } else {
     double P = Q[0];
@@ -173,7 +202,7 @@ int oracle_flux(const oracle_params *p, const double *Qv, double *Phi)
   int K = num_vars(p->scheme, L.D);
   double F[MAXK][3];
   memset(F, 0, sizeof F);
-  flux_eval(p->scheme, L.D, p->gamma, p->c0sq, Qv, F);
+  flux_eval(p, L.D, Qv, F);
   for (int k = 0; k < K; k++) for (int a = 0; a < 3; a++) Phi[3 * k + a] = a < L.D ? F[k][a] : 0.0;
   return 0;
 }
@@ -185,7 +214,7 @@ int oracle_equilibrium(const oracle_params *p, const double *Qv, double *feq)
   int K = num_vars(p->scheme, L.D);
   double F[MAXK][3];
   memset(F, 0, sizeof F);
-  flux_eval(p->scheme, L.D, p->gamma, p->c0sq, Qv, F);
+  flux_eval(p, L.D, Qv, F);
   for (int k = 0; k < K; k++)
     for (int i = 0; i < L.Q; i++) feq[k * L.Q + i] = feq_eval(&L, i, Qv[k], F[k]);
   return 0;
@@ -254,8 +283,9 @@ int oracle_create(const oracle_params *p, const unsigned char *cell_mask, oracle
   lattice_t L;
   *out = NULL;
   if (lattice_make(p->lattice, &L)) return -1;
-  if (p->scheme != ORC_IDEAL && p->scheme != ORC_INCRES && p->scheme != ORC_IDEAL_DIVB) return -1;
-  if (p->scheme == ORC_IDEAL_DIVB && !(p->tau_relax > 0.0)) return -1;
+  if (p->scheme != ORC_IDEAL && p->scheme != ORC_INCRES && p->scheme != ORC_IDEAL_DIVB && p->scheme != ORC_RESIST) return -1;
+  if ((p->scheme == ORC_IDEAL_DIVB || p->scheme == ORC_RESIST) && !(p->tau_relax > 0.0)) return -1;
+  if (p->scheme == ORC_RESIST && !(p->eta >= 0.0)) return -1;
   if (p->eta_jc != 0.0 && !(p->scheme == ORC_INCRES && p->eta_jc > 0.0)) return -1;
   if (p->nx < 1 || p->ny < 1 || p->nz < 1) return -1;
   if (L.D < 2 && p->ny != 1) return -1;
@@ -282,7 +312,8 @@ int oracle_create(const oracle_params *p, const unsigned char *cell_mask, oracle
     for (int b = 0; b < nvec; b++) tau[o->iU + b] = 0.5 + p->nu / L.cs2;
     if (p->scheme == ORC_INCRES) tau[0] = 0.5 + p->nu / L.cs2;
   }
-  if (p->eta > 0.0) for (int b = 0; b < nvec; b++) tau[o->iB + b] = 0.5 + p->eta / L.cs2;
+  /* RESIST carries eta in the flux (-eta grad B): tau_B stays the stabilisation parameter */
+  if (p->eta > 0.0 && p->scheme != ORC_RESIST) for (int b = 0; b < nvec; b++) tau[o->iB + b] = 0.5 + p->eta / L.cs2;
   for (int k = 0; k < o->K; k++) {
     if (!(tau[k] > 0.5)) { free(o); return -1; }
     o->omega[k] = 1.0 / tau[k];
@@ -394,7 +425,7 @@ int oracle_init(oracle_t *o, const double *fields)
     double Qv[MAXK], Phi[MAXK][3];
     for (int k = 0; k < K; k++) Qv[k] = fields[(long)k * o->N + n];
     memset(Phi, 0, sizeof Phi);
-    flux_eval(o->p.scheme, o->L.D, o->p.gamma, o->p.c0sq, Qv, Phi);
+    flux_eval(&o->p, o->L.D, Qv, Phi);
     for (int k = 0; k < K; k++)
       for (int i = 0; i < Qn; i++) {
         double v = feq_eval(&o->L, i, Qv[k], Phi[k]);
@@ -578,7 +609,7 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
           Qnb[k] = sum;
         }
         memset(Phinb, 0, sizeof Phinb);
-        flux_eval(o->p.scheme, D, o->p.gamma, o->p.c0sq, Qnb, Phinb);
+        flux_eval(&o->p, D, Qnb, Phinb);
         have_nb = 1;
       }
       for (k = 0; k < K; k++) f[k][i] = feq_eval(L, i, Qnb[k], Phinb[k]);
@@ -597,7 +628,7 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
   if (o->p.scheme == ORC_INCRES && o->p.eta_jc > 0.0) {
     double Phieq[MAXK][3], Pi[3][3], a2 = 0.0;
     memset(Phieq, 0, sizeof Phieq);
-    flux_eval(o->p.scheme, D, o->p.gamma, o->p.c0sq, Qv, Phieq);
+    flux_eval(&o->p, D, Qv, Phieq);
     for (a = 0; a < D; a++) for (b = 0; b < D; b++) {
       double m = 0.0;
       for (i = 0; i < Qn; i++) m += (double)L->c[i][a] * f[o->iB + b][i];
@@ -610,6 +641,11 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
   double delta = -tr / (tauB * L->cs2);
   /* IDEAL_DIVB: div B from the relaxation variable instead, D ~ tau_M div B (Eq.7) */
   if (o->p.scheme == ORC_IDEAL_DIVB) delta = Qv[8] / o->p.tau_relax;
+  /* RESIST: div B = tr g = sum_a G_aa / tau_M */
+  if (o->p.scheme == ORC_RESIST) {
+    delta = 0.0;
+    for (a = 0; a < D; a++) delta += Qv[8 + 3 * a + a] / o->p.tau_relax;
+  }
 
   /* 4. Powell source (Eq.12), direct injection (A5) */
   double S[MAXK];
@@ -621,6 +657,7 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
     for (b = 0; b < 3; b++) { S[1 + b] = -kd * Qv[5 + b]; S[5 + b] = -kd * u[b]; }
     S[4] = -kd * uBdot;
     if (o->p.scheme == ORC_IDEAL_DIVB) S[8] = -Qv[8] / o->p.tau_relax;      /* relaxation source of Eq.6 */
+    if (o->p.scheme == ORC_RESIST) for (k = 8; k < K; k++) S[k] = -Qv[k] / o->p.tau_relax;
   } else {
     for (b = 0; b < D; b++) { S[1 + b] = -kd * Qv[1 + D + b]; S[1 + D + b] = -kd * Qv[1 + b]; }
   }
@@ -654,7 +691,7 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
       }
     }
     /* the Powell rows are scaled by the porosity (A8); the relaxation of D is intrinsic and is not */
-    for (k = 0; k < K; k++) { dQh[k] = Qh[k] - Qv[k]; if (!(o->p.scheme == ORC_IDEAL_DIVB && k == 8)) S[k] *= d; }
+    for (k = 0; k < K; k++) { dQh[k] = Qh[k] - Qv[k]; if (k < 8 || !is_ideal(o->p.scheme)) S[k] *= d; }
     if (srcacc) {   /* body integrals (A21) */
       double *bd = srcacc + MAXK;
       const int nvec = is_ideal(o->p.scheme) ? 3 : D;
@@ -681,7 +718,7 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
   /* 6. flux of the (blended) state (Eq.11) */
   double Phi[MAXK][3];
   memset(Phi, 0, sizeof Phi);
-  flux_eval(o->p.scheme, D, o->p.gamma, o->p.c0sq, Qh, Phi);
+  flux_eval(&o->p, D, Qh, Phi);
 
   /* 7./8. BGK + direct injection (Eq.2-3), store */
   for (k = 0; k < K; k++)

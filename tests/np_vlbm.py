@@ -74,6 +74,32 @@ def flux_ideal_divb(Q, gamma, D):
     return Phi
 
 
+LEVI = np.zeros((3, 3, 3))
+for _a, _b, _c in ((0, 1, 2), (1, 2, 0), (2, 0, 1)):
+    LEVI[_a, _b, _c], LEVI[_a, _c, _b] = 1.0, -1.0
+
+
+def flux_resist(Q, gamma, D, eta, tau_m):
+    """dissipative system with transported gradients G (Eq.9-10): Q = (rho, m, E, B, G[a<D][b<3]).
+    Tensor form: g = G / tau_M ~ grad B; j = curl B = eps : g; Phi_B -= eta g; Phi_E += eta j x B; Phi_G = G (x) u - I (x) B."""
+    K = 8 + 3 * D
+    tail = Q.shape[1:]
+    Phi = np.zeros((K, 3) + tail)
+    Phi[:8] = flux_ideal(Q[:8], gamma, D)
+    u, B = Q[1:4] / Q[0], Q[5:8]
+    G = np.zeros((3, 3) + tail)
+    G[:D] = Q[8:].reshape((D, 3) + tail)
+    g = G / tau_m
+    j = np.einsum("ecb,cb...->e...", LEVI, g)
+    jxB = np.einsum("aef,e...,f...->a...", LEVI, j, B)
+    Phi[4] += eta * jxB
+    Phi[5:8] -= eta * np.swapaxes(g, 0, 1)                      # Phi[5+b, a] -= eta g[a, b]
+    PhiG = G[:, :, None] * u[None, None] - np.einsum("ca,b...->cba...", np.eye(3), B)     # [c, b, a]
+    Phi[8:] = PhiG[:D].reshape((3 * D, 3) + tail)
+    Phi[:, D:] = 0.0
+    return Phi
+
+
 def flux_incres(Q, c0sq, D):
     """A3. Q: [1+2D, ...] = (P, u, B)."""
     P, u, B = Q[0], Q[1:1 + D], Q[1 + D:1 + 2 * D]
@@ -95,8 +121,9 @@ class NpVLBM:
         self.D, self.c, self.w, self.cs2 = lattice_np(lat)
         self.Qn = len(self.w)
         self.shape = tuple(shape_zyx)
-        self.K = 8 if scheme == "IDEAL" else (9 if scheme == "IDEAL_DIVB" else 1 + 2 * self.D)
-        self.ideal = scheme in ("IDEAL", "IDEAL_DIVB")
+        self.K = {"IDEAL": 8, "IDEAL_DIVB": 9, "RESIST": 8 + 3 * self.D, "INCRES": 1 + 2 * self.D}[scheme]
+        self.ideal = scheme in ("IDEAL", "IDEAL_DIVB", "RESIST")
+        self.eta = 0.0                 # RESIST: magnetic diffusivity of the flux terms
         self.tau_relax = tau_relax
         self.eta_jc = eta_jc
         self.tau = np.broadcast_to(np.asarray(tau, dtype=float), (self.K,)).copy()
@@ -125,6 +152,8 @@ class NpVLBM:
             return flux_ideal(Q, self.gamma, self.D)
         if self.scheme == "IDEAL_DIVB":
             return flux_ideal_divb(Q, self.gamma, self.D)
+        if self.scheme == "RESIST":
+            return flux_resist(Q, self.gamma, self.D, self.eta, self.tau_relax)
         return flux_incres(Q, self.c0sq, self.D)
 
     def feq(self, Q, Phi):
@@ -278,6 +307,8 @@ class NpVLBM:
                 t = t - ((t - tau0) * t * t - cc) / (t * (3 * t - 2 * tau0))
             tauB = t
         delta = -tr / (tauB * self.cs2)
+        if self.scheme == "RESIST":
+            delta = sum(Q[8 + 3 * a + a] for a in range(D)) / self.tau_relax        # div B = tr G / tau_M
         if self.scheme == "IDEAL_DIVB":
             delta = Q[8] / self.tau_relax            # Eq.7: D ~ tau_M div B
         # 4. Powell source
@@ -288,8 +319,8 @@ class NpVLBM:
             S[1:4] = -self.kappa * delta * B
             S[4] = -self.kappa * delta * (u * B).sum(0)
             S[5:8] = -self.kappa * delta * u
-            if self.scheme == "IDEAL_DIVB":
-                S[8] = -Q[8] / self.tau_relax        # relaxation source of Eq.6
+            if self.scheme in ("IDEAL_DIVB", "RESIST"):
+                S[8:] = -Q[8:] / self.tau_relax      # relaxation source of Eq.6
         else:
             u, B = Q[1:1 + D], Q[1 + D:]
             S[1:1 + D] = -self.kappa * delta * B
@@ -316,7 +347,7 @@ class NpVLBM:
                 Qh[1 + b] = np.where(sol, d * Q[1 + b] + (1 - d) * uB[b], Q[1 + b])
                 Qh[1 + D + b] = np.where(sol, d * Q[1 + D + b] + (1 - d) * BB[b], Q[1 + D + b])
         dQh = Qh - Q
-        if self.scheme == "IDEAL_DIVB":
+        if self.scheme in ("IDEAL_DIVB", "RESIST"):
             S[:8] = S[:8] * d
         else:
             S = S * d
