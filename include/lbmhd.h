@@ -16,6 +16,7 @@
  *    IDEAL: K = 8 in every dimension, order rho, m_x, m_y, m_z, E, B_x, B_y, B_z.
  *    INCRES: K = 1 + 2D, order P, u_1..u_D, B_1..B_D (P = kinematic pressure carrier, A3).
  *    IDEAL_DIVB: K = 9, the IDEAL order followed by D.
+ *    RESIST: K = 8 + 3 D, the IDEAL order followed by G_ab, a-major (variable 8 + 3 a + b).
  *  - Direction order: rest; +x,-x,+y,-y,+z,-z; diagonals (+,+),(-,-),(+,-),(-,+) per plane xy, xz, yz.
  *  - Every pointer argument says whether it is a HOST or a DEVICE pointer.  The caller owns every
  *    buffer it passes, including `workspace` (device memory, e.g. a torch tensor): the library never
@@ -40,7 +41,11 @@ enum { LBMHD_D1Q3 = 1, LBMHD_D2Q9 = 2, LBMHD_D3Q19 = 3,
        LBMHD_D2Q5 = 4, LBMHD_D3Q7 = 5 /* the paper's own lattices; D3Q7 has c_s^2 = 1/4 */ };
 enum { LBMHD_IDEAL = 0, LBMHD_INCRES = 1,
        LBMHD_IDEAL_DIVB = 2 /* IDEAL + the paper's local gradient evolution in traced form: a 9th set
-                               D = tr G with flux D u - B and source -D/tau_relax; div B in Eq.12 := D/tau_relax */ };
+                               D = tr G with flux D u - B and source -D/tau_relax; div B in Eq.12 := D/tau_relax */,
+       LBMHD_RESIST = 3 /* dissipative MHD with the magnetic gradients transported (Eq.9-10 PAPER.md:132-136;
+                           DESIGN.md A22): IDEAL + G_ab ~ tau_relax d_a B_b (a < D lattice axes, b < 3), flux G (x) u - I (x) B,
+                           source -G/tau_relax; induction flux - eta G/tau_relax, energy flux + eta j x B with j = curl B
+                           from G; div B in Eq.12 := tr G / tau_relax.  No viscous stress, no heat flux */ };
 enum { LBMHD_BC_PERIODIC = 0, LBMHD_BC_ZEROGRAD = 1, LBMHD_BC_INFLOW = 2,
        LBMHD_BC_HALO = 3 /* slab decomposition, slowest lattice axis only: the plane on this face is a ghost plane */ };
 enum { LBMHD_CELL_FLUID = 0, LBMHD_CELL_FROZEN = 1, LBMHD_CELL_SOLID = 2 };
@@ -54,15 +59,16 @@ enum {
 };
 
 typedef struct {
-  int    scheme;        /* LBMHD_IDEAL | LBMHD_INCRES | LBMHD_IDEAL_DIVB */
+  int    scheme;        /* LBMHD_IDEAL | LBMHD_INCRES | LBMHD_IDEAL_DIVB | LBMHD_RESIST */
   int    lattice;       /* LBMHD_D1Q3 | LBMHD_D2Q9 | LBMHD_D3Q19 | LBMHD_D2Q5 | LBMHD_D3Q7 */
   int    precision;     /* 64 (fp64 populations and arithmetic) or 32 (fp32 populations and arithmetic) */
   int    nx, ny, nz;    /* unused dims = 1 */
   double gamma;         /* IDEAL: adiabatic index, Eq.8 */
   double c0sq;          /* INCRES: artificial sound speed squared (A3) */
-  double nu, eta;       /* if > 0: tau of the velocity (and P) / magnetic sets := 1/2 + D/c_s^2, Eq.5 */
-  double tau[16];       /* per variable (first K used), > 1/2, order of `scheme`; all magnetic sets must share one value (A7) */
-  double tau_relax;     /* IDEAL_DIVB: relaxation time tau_M of D (Eq.6) in lattice units, > 0 */
+  double nu, eta;       /* if > 0: tau of the velocity (and P) / magnetic sets := 1/2 + D/c_s^2, Eq.5 PAPER.md:98.
+                           RESIST: eta (>= 0) is the magnetic diffusivity of the flux terms instead and leaves tau alone */
+  double tau[32];       /* per variable (first K <= 17 used), > 1/2, order of `scheme`; all magnetic sets must share one value (A7) */
+  double tau_relax;     /* IDEAL_DIVB, RESIST: relaxation time tau_M of the gradient variables (Eq.6), lattice units, > 0 */
   double eta_jc;        /* INCRES: critical current j_c of eta(j) = eta0 (1 + (j/j_c)^2) (eta0 from `eta` or tau),
                            lattice units; 0 = constant resistivity */
   double powell;        /* kappa: 0 = off, 1 = Eq.12 */

@@ -40,7 +40,7 @@ struct lbmhd {
   lbh::Geometry g;
   lbh::Layout L;
   size_t N;
-  double tau[16];
+  double tau[32];
   cudaStream_t stream;
   char *ws;
   int cur;               // A/B: which population copy holds the current state (in place: always 0)

@@ -30,10 +30,11 @@ template <typename real> struct StepArgs {
   size_t pstride;               // elements between planes
   int nx, ny, nz;
   int bc[6];
-  real omega[16];               // 1 / tau_k
+  real omega[20];               // 1 / tau_k (K <= 17)
   real inv_tauB_cs2;            // 1 / (tau_B c_s^2)
   real kappa, gamma, c0sq;
-  real inv_tau_relax;           // kIdealD: 1 / tau_M of the relaxation variable D (Eq.6)
+  real inv_tau_relax;           // kIdealD, kResist: 1 / tau_M of the relaxation variables (Eq.6)
+  real eta;                     // kResist: magnetic diffusivity of the flux terms -eta grad B, eta j x B
   real etaj_inv_jc2;            // kIncres: 1 / j_c^2 of eta(j) = eta0 (1 + (j/j_c)^2), 0 = constant eta
   real tauB0;                   // tau of the magnetic sets at zero current
   const unsigned char *mask;    // [N] or nullptr
@@ -123,11 +124,20 @@ __device__ __forceinline__ double solid_state(const StepArgs<real> &a, int x, in
   return d;
 }
 
+// register-array element by a runtime (warp-uniform) index without spilling the array to local memory
+template <int K, typename real> __device__ __forceinline__ real pick(const real *v, int k) {
+  real r = v[0];
+#pragma unroll
+  for (int l = 1; l < K; l++)
+    if (k == l) r = v[l];
+  return r;
+}
+
 // ---- flux row of variable k: Phi_k,alpha(Qh), alpha < D (Eq.11, Eq.8; A3) -------
 // Qh is the (possibly solid-blended) state; `p` the gas pressure of the unblended state (A8 keeps p).
 // k is warp-uniform, so the switch does not diverge.
 template <int SCHEME, int D, typename real>
-__device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real c0sq, real Phi[3]) {
+__device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real c0sq, real eta, real itm, real Phi[3]) {
   Phi[0] = Phi[1] = Phi[2] = real(0);
   if (is_ideal(SCHEME)) {
     const real rho = Qh[0], E = Qh[4];
@@ -144,12 +154,27 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
       for (int a = 0; a < D; a++) Phi[a] = Qh[8] * u[a] - B[a];
       return;
     }
-    if (k >= 5) {   // induction: u_a B_b - B_a u_b
+    if (SCHEME == kResist && k >= 8) {   // G_cb: G_cb u_a - delta_ca B_b (Eq.10)
+      const int c = (k - 8) / 3, b = (k - 8) - 3 * c;
+      const real Gk = pick<8 + 3 * D, real>(Qh, k);
+      const real Bb = b == 0 ? B[0] : (b == 1 ? B[1] : B[2]);
+#pragma unroll
+      for (int a = 0; a < D; a++) Phi[a] = Gk * u[a] - (a == c ? Bb : real(0));
+      return;
+    }
+    if (k >= 5) {   // induction: u_a B_b - B_a u_b  (kResist: - eta g_ab, g = G / tau_M ~ grad B)
       const int b = k - 5;
       const real Bb = b == 0 ? B[0] : (b == 1 ? B[1] : B[2]);
       const real ub = b == 0 ? u[0] : (b == 1 ? u[1] : u[2]);
 #pragma unroll
       for (int a = 0; a < D; a++) Phi[a] = u[a] * Bb - B[a] * ub;
+      if (SCHEME == kResist) {
+#pragma unroll
+        for (int a = 0; a < D; a++) {
+          const real Gab = b == 0 ? Qh[8 + 3 * a] : (b == 1 ? Qh[8 + 3 * a + 1] : Qh[8 + 3 * a + 2]);
+          Phi[a] -= eta * (Gab * itm);
+        }
+      }
       return;
     }
     const real B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
@@ -160,6 +185,17 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
       const real uB = u[0] * B[0] + u[1] * B[1] + u[2] * B[2];
 #pragma unroll
       for (int a = 0; a < D; a++) Phi[a] = (E + pt) * u[a] - B[a] * uB;
+      if (SCHEME == kResist) {   // + eta (j x B)_a,  j = curl B: j_e = eps_ecb g_cb over the lattice axes c < D
+        real g[3][3];
+#pragma unroll
+        for (int c = 0; c < 3; c++)
+#pragma unroll
+          for (int b = 0; b < 3; b++) g[c][b] = c < D ? Qh[8 + 3 * (c < D ? c : 0) + b] * itm : real(0);
+        const real j0 = g[1][2] - g[2][1], j1 = g[2][0] - g[0][2], j2 = g[0][1] - g[1][0];
+        const real jxB[3] = {j1 * B[2] - j2 * B[1], j2 * B[0] - j0 * B[2], j0 * B[1] - j1 * B[0]};
+#pragma unroll
+        for (int a = 0; a < D; a++) Phi[a] += eta * jxB[a];
+      }
       return;
     }
     const int b = k - 1;   // momentum: m_b u_a + pt delta_ab - B_b B_a
@@ -199,21 +235,12 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
   }
 }
 
-// register-array element by a runtime (warp-uniform) index without spilling the array to local memory
-template <int K, typename real> __device__ __forceinline__ real pick(const real *v, int k) {
-  real r = v[0];
-#pragma unroll
-  for (int l = 1; l < K; l++)
-    if (k == l) r = v[l];
-  return r;
-}
-
 // ---- Powell source row S_k / (-kappa delta) (Eq.12): (0, B, u.B, u) resp. (0, B, u) ----------
 template <int SCHEME, int D, typename real>
 __device__ __forceinline__ real powell_row(int k, const real *Qv) {
   if (k == 0) return real(0);
   if (is_ideal(SCHEME)) {
-    if (SCHEME == kIdealD && k == 8) return real(0);
+    if (has_relax(SCHEME) && k >= 8) return real(0);
     if (k <= 3) return k == 1 ? Qv[5] : (k == 2 ? Qv[6] : Qv[7]);
     const real ir = real(1) / Qv[0];
     if (k == 4) return (Qv[1] * Qv[5] + Qv[2] * Qv[6] + Qv[3] * Qv[7]) * ir;
@@ -233,7 +260,10 @@ __device__ __forceinline__ real powell_row(int k, const real *Qv) {
 template <int SCHEME, int D, typename real>
 __device__ __forceinline__ void solid_blend(const real *Qv, real gamma, real d, const double uS[3], const double BS[3], real *Qh) {
   const real e = real(1) - d;
-  if (SCHEME == kIdealD) Qh[8] = Qv[8];
+  if (has_relax(SCHEME)) {      // gradient variables are not blended
+#pragma unroll
+    for (int l = 8; l < Vars<SCHEME, D>::K; l++) Qh[l] = Qv[l];
+  }
   if (is_ideal(SCHEME)) {
     const real rho = Qv[0];
     const real ir = real(1) / rho;
@@ -356,7 +386,7 @@ __device__ __forceinline__ void frozen_rematerialise(const StepArgs<real> &a, in
   real Qf[K], Phi[3];
 #pragma unroll
   for (int l = 0; l < K; l++) Qf[l] = (real)a.M_cur[(size_t)l * N + n];
-  flux_row<SCHEME, D, real>(k, Qf, a.gamma, a.c0sq, Phi);
+  flux_row<SCHEME, D, real>(k, Qf, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
   const real Qfk = pick<K, real>(Qf, k);
 #pragma unroll
   for (int j = 0; j < Q; j++) {
@@ -458,7 +488,7 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
       real Qnb[K], Phi[3];
 #pragma unroll
       for (int l = 0; l < K; l++) Qnb[l] = sQ[l][tx];
-      flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, Phi);
+      flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
       const real Qnbk = pick<K, real>(Qnb, k);
 #pragma unroll
       for (int i = 0; i < Q; i++) {
@@ -534,7 +564,13 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
     inv_tauB_cs2 = omB * real(L::inv_cs2);
   }
   // A6: local estimate from tr Pi_B; kIdealD: from the relaxation variable, D ~ tau_M div B (Eq.7)
-  const real delta = SCHEME == kIdealD ? Qv[K - 1] * a.inv_tau_relax : -tr * inv_tauB_cs2;
+  real delta;
+  if (SCHEME == kIdealD) delta = Qv[K - 1] * a.inv_tau_relax;
+  else if (SCHEME == kResist) {         // div B = tr g = sum_a G_aa / tau_M
+    delta = real(0);
+#pragma unroll
+    for (int al = 0; al < D; al++) delta += Qv[8 + 3 * al + al] * a.inv_tau_relax;
+  } else delta = -tr * inv_tauB_cs2;
 
   // S4 Powell source, S5 solid blend (rare: own branch so the blended copy of the state costs no registers
   // on the fluid path), S6 flux row of this variable
@@ -548,19 +584,19 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
     if (d < real(1)) {
       real Qh[K];
       solid_blend<SCHEME, D, real>(Qv, a.gamma, d, uS, BS, Qh);
-      flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, Phi);
+      flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
       // dQh plus the Powell source scaled by the porosity d (A8)
       dq = pick<K, real>(Qh, k) - Qk;
       inj = dq - d * (a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
-      if (SCHEME == kIdealD && k == K - 1) inj = -Qk * a.inv_tau_relax;      // relaxation source of Eq.6, not porosity-scaled
+      if (has_relax(SCHEME) && k >= 8) inj = -Qk * a.inv_tau_relax;      // relaxation source of Eq.6, not porosity-scaled
       solid = true;
     }
     if (a.body != nullptr) body_accumulate<SCHEME, D, real>(a, c, k, solid, (double)dq, (double)d, (double)Qk);
   }
   if (!solid) {
-    flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, Phi);
+    flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
     inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
-    if (SCHEME == kIdealD && k == K - 1) inj = -Qk * a.inv_tau_relax;        // relaxation source of Eq.6
+    if (has_relax(SCHEME) && k >= 8) inj = -Qk * a.inv_tau_relax;        // relaxation source of Eq.6
   }
   // in place: cells next to a non-periodic face publish their post-collision moment (sum_i g'_i = Q_k + inj)
   if (STREAM != ST_AB && c.writeM) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + c.n] = (double)(Qk + inj);
@@ -756,7 +792,7 @@ __device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, 
         real Qnb[K], Phi[3];
 #pragma unroll
         for (int l = 0; l < K; l++) Qnb[l] = sNb[l];
-        flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, Phi);
+        flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
         const real Qnbk = pick<K, real>(Qnb, k);
 #pragma unroll
         for (int i = 0; i < Q; i++) {
@@ -865,8 +901,8 @@ __device__ __forceinline__ void finish_pair(const StepArgs<float> &a, int tx, in
     tr0 += t.x; tr1 += t.y;
   }
   float Phi0[3], Phi1[3];
-  flux_row<SCHEME, D, float>(k, Qv0, a.gamma, a.c0sq, Phi0);
-  flux_row<SCHEME, D, float>(k, Qv1, a.gamma, a.c0sq, Phi1);
+  flux_row<SCHEME, D, float>(k, Qv0, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi0);
+  flux_row<SCHEME, D, float>(k, Qv1, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi1);
   // -kappa delta S_row with delta = -tr/(tau_B cs2) (A6) or D/tau_M (kIdealD)
   const float d0 = SCHEME == kIdealD ? Qv0[K - 1] * a.inv_tau_relax : -tr0 * a.inv_tauB_cs2;
   const float d1 = SCHEME == kIdealD ? Qv1[K - 1] * a.inv_tau_relax : -tr1 * a.inv_tauB_cs2;
@@ -961,7 +997,7 @@ step_kernel_pair(const __grid_constant__ StepArgs<float> a, const int npair) {
 template <int LAT, int SCHEME, typename real, int TX>
 __global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K)
 init_kernel(const double *__restrict__ fields, real *__restrict__ g, size_t pstride, int nx, int ny, int nz, real gamma,
-            real c0sq) {
+            real c0sq, real eta, real itm) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q, K = Vars<SCHEME, D>::K;
   const int k = threadIdx.y;
@@ -972,7 +1008,7 @@ init_kernel(const double *__restrict__ fields, real *__restrict__ g, size_t pstr
   real Qv[K], Phi[3];
 #pragma unroll
   for (int l = 0; l < K; l++) Qv[l] = (real)fields[(size_t)l * N + n];
-  flux_row<SCHEME, D, real>(k, Qv, gamma, c0sq, Phi);
+  flux_row<SCHEME, D, real>(k, Qv, gamma, c0sq, eta, itm, Phi);
   const real Qk = pick<K, real>(Qv, k);
   real *gk = g + (size_t)k * Q * pstride;
 #pragma unroll

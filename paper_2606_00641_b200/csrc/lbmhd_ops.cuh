@@ -15,7 +15,9 @@ using namespace lbk;
 template <int LAT, int SCHEME, typename real> struct Ops {
   using L = Lattice<LAT>;
   static constexpr int Q = L::Q, K = Vars<SCHEME, L::D>::K;
-  static constexpr int TXAUX = 64;   // x-tile of init / moments
+  static constexpr int TXAUX = K > 16 ? 32 : 64;   // x-tile of init / moments (TXAUX * K threads <= 1024)
+  // launch bound of the step kernels of kResist (K = 11 / 14 / 17 variable rows per block): registers, not threads, limit it
+  static constexpr int MINB_R = K >= 17 ? 1 : 2;
 
   static real *pops(lbmhd_t *h, int which) { return (real *)(h->ws + h->L.off_pop[which]); }
 
@@ -128,6 +130,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     a.kappa = (real)h->p.powell; a.gamma = (real)h->p.gamma; a.c0sq = (real)h->p.c0sq;
     a.inv_tau_relax = h->p.tau_relax > 0.0 ? (real)(1.0 / h->p.tau_relax) : real(0);
     a.etaj_inv_jc2 = h->p.eta_jc > 0.0 ? (real)(1.0 / (h->p.eta_jc * h->p.eta_jc)) : real(0);
+    a.eta = SCHEME == kResist ? (real)h->p.eta : real(0);
     a.tauB0 = (real)h->tau[h->g.iB];
     a.mask = h->have_mask ? (const unsigned char *)(h->ws + h->L.off_mask) : nullptr;
     a.Bsolid = h->have_bsolid ? (const double *)(h->ws + h->L.off_bsolid) : nullptr;
@@ -187,16 +190,18 @@ template <int LAT, int SCHEME, typename real> struct Ops {
           }
       }
       cudaError_t e;
-      if (sizeof(real) == 4 && h->pair) e = h->minb == 2 ? launch_step_pair<2>(h, a) : (h->minb == 4 ? launch_step_pair<4>(h, a) : launch_step_pair<3>(h, a));
-      else if (inplace) e = h->minb == 4 ? launch_step_inplace<4>(h, a) : launch_step_inplace<3>(h, a);
-      else if (h->use_tma) e = launch_step_tma(h, a);
-      else switch (h->tx * 10 + h->minb) {
-        case 322: e = launch_step_whole<32, 2>(h, a); break;
-        case 323: e = launch_step<32, 3>(h, a); break;          // split launches exist for the two default bounds only
-        case 324: e = launch_step<32, 4>(h, a); break;
-        case 642: e = launch_step_whole<64, 2>(h, a); break;
-        case 1281: e = launch_step_whole<128, 1>(h, a); break;
-        default: e = launch_step<32, 3>(h, a); break;
+      if constexpr (SCHEME == kResist) {     // one launch configuration: one-cell kernels, one launch over all tiles
+        e = inplace ? launch_step_inplace<MINB_R>(h, a) : launch_step_whole<32, MINB_R>(h, a);
+      } else {
+        if (sizeof(real) == 4 && h->pair) e = h->minb == 2 ? launch_step_pair<2>(h, a) : (h->minb == 4 ? launch_step_pair<4>(h, a) : launch_step_pair<3>(h, a));
+        else if (inplace) e = h->minb == 4 ? launch_step_inplace<4>(h, a) : launch_step_inplace<3>(h, a);
+        else if (h->use_tma) e = launch_step_tma(h, a);
+        else switch (h->tx * 10 + h->minb) {
+          case 322: e = launch_step_whole<32, 2>(h, a); break;
+          case 323: e = launch_step<32, 3>(h, a); break;          // split launches exist for the two default bounds only
+          case 324: e = launch_step<32, 4>(h, a); break;
+          default: e = launch_step<32, 3>(h, a); break;
+        }
       }
       if (e != cudaSuccess) return fail(LBMHD_ECUDA, "step kernel launch: %s", cudaGetErrorString(e));
       if (inplace) { h->parity ^= 1; h->mcur ^= 1; }
@@ -208,7 +213,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
 
   static int init(lbmhd_t *h, const double *fields_dev) {
     init_kernel<LAT, SCHEME, real, TXAUX><<<grid(h, TXAUX), dim3(TXAUX, K), 0, h->stream>>>(
-        fields_dev, pops(h, 0), h->L.pstride, h->p.nx, h->p.ny, h->p.nz, (real)h->p.gamma, (real)h->p.c0sq);
+        fields_dev, pops(h, 0), h->L.pstride, h->p.nx, h->p.ny, h->p.nz, (real)h->p.gamma, (real)h->p.c0sq,
+        SCHEME == kResist ? (real)h->p.eta : real(0), h->p.tau_relax > 0.0 ? (real)(1.0 / h->p.tau_relax) : real(0));
     CUDA_TRY(cudaGetLastError());
     h->launches += 1;
     h->parity = 0;
@@ -287,6 +293,7 @@ template <int LAT, int SCHEME, typename real> OpTable make_table() {
 template <int LAT, typename real> OpTable table_for(int scheme) {
   if (scheme == LBMHD_IDEAL) return make_table<LAT, kIdeal, real>();
   if (scheme == LBMHD_IDEAL_DIVB) return make_table<LAT, kIdealD, real>();
+  if (scheme == LBMHD_RESIST) return make_table<LAT, kResist, real>();
   return make_table<LAT, kIncres, real>();
 }
 

@@ -13,20 +13,20 @@ import numpy as np
 from . import build as _build
 
 D1Q3, D2Q9, D3Q19, D2Q5, D3Q7 = 1, 2, 3, 4, 5
-IDEAL, INCRES, IDEAL_DIVB = 0, 1, 2
+IDEAL, INCRES, IDEAL_DIVB, RESIST = 0, 1, 2, 3
 BC_PERIODIC, BC_ZEROGRAD, BC_INFLOW, BC_HALO = 0, 1, 2, 3
 CELL_FLUID, CELL_FROZEN, CELL_SOLID = 0, 1, 2
 STREAM_AB, STREAM_INPLACE = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC = 0, -1, -2, -3, -4
 LATTICES = {"D1Q3": D1Q3, "D2Q9": D2Q9, "D3Q19": D3Q19, "D2Q5": D2Q5, "D3Q7": D3Q7}
-SCHEMES = {"IDEAL": IDEAL, "INCRES": INCRES, "IDEAL_DIVB": IDEAL_DIVB}
+SCHEMES = {"IDEAL": IDEAL, "INCRES": INCRES, "IDEAL_DIVB": IDEAL_DIVB, "RESIST": RESIST}
 
 
 class LbmhdParams(C.Structure):
     _fields_ = [("scheme", C.c_int), ("lattice", C.c_int), ("precision", C.c_int),
                 ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
                 ("gamma", C.c_double), ("c0sq", C.c_double), ("nu", C.c_double), ("eta", C.c_double),
-                ("tau", C.c_double * 16), ("tau_relax", C.c_double), ("eta_jc", C.c_double), ("powell", C.c_double), ("bc", C.c_int * 6),
+                ("tau", C.c_double * 32), ("tau_relax", C.c_double), ("eta_jc", C.c_double), ("powell", C.c_double), ("bc", C.c_int * 6),
                 ("halo_offset", C.c_int), ("streaming", C.c_int), ("device", C.c_int), ("stream", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
 
@@ -107,8 +107,8 @@ def make_params(scheme, lattice, shape, precision=64, gamma=5.0 / 3.0, c0sq=1.0 
     dims = list(shape) + [1] * (3 - len(shape))
     p.nx, p.ny, p.nz = dims
     p.gamma, p.c0sq, p.nu, p.eta, p.powell = gamma, c0sq, nu, eta, powell
-    taus = [tau] * 16 if np.isscalar(tau) else list(tau) + [0.0] * (16 - len(tau))
-    for k in range(16):
+    taus = [tau] * 32 if np.isscalar(tau) else list(tau) + [0.0] * (32 - len(tau))
+    for k in range(32):
         p.tau[k] = taus[k]
     p.tau_relax = tau_relax
     p.eta_jc = eta_jc

@@ -3,7 +3,7 @@ boundary combination, both streaming modes, all lattices and schemes — a seede
 import numpy as np
 import pytest
 
-from test_parity_gpu import compare, random_workload, divb_workload
+from test_parity_gpu import compare, random_workload, divb_workload, resist_workload
 from parity_util import TOL64, TOL32
 
 pytestmark = pytest.mark.gpu
@@ -12,7 +12,7 @@ pytestmark = pytest.mark.gpu
 def random_case(rng):
     lattice = rng.choice(["D1Q3", "D2Q9", "D3Q19", "D2Q5", "D3Q7"])
     D = {"D1Q3": 1, "D2Q9": 2, "D3Q19": 3, "D2Q5": 2, "D3Q7": 3}[lattice]
-    scheme = rng.choice(["IDEAL", "INCRES", "IDEAL_DIVB"])
+    scheme = rng.choice(["IDEAL", "INCRES", "IDEAL_DIVB", "RESIST"])
     bc = [0] * 6
     shape = []
     for a in range(D):
@@ -26,7 +26,7 @@ def random_case(rng):
     return scheme, lattice, tuple(shape), tuple(bc)
 
 
-@pytest.mark.parametrize("seed", range(40))
+@pytest.mark.parametrize("seed", range(60))
 def test_random_small_shapes(seed):
     rng = np.random.default_rng(9000 + seed)
     scheme, lattice, shape, bc = random_case(rng)
@@ -34,6 +34,8 @@ def test_random_small_shapes(seed):
     precision = 64 if rng.random() < 0.75 else 32
     if scheme == "IDEAL_DIVB":
         w = divb_workload(lattice, shape, bc, seed=seed)
+    elif scheme == "RESIST":
+        w = resist_workload(lattice, shape, bc, seed=seed)
     else:
         w = random_workload(scheme, lattice, shape, bc, seed=seed)
     steps = int(rng.integers(1, 7))

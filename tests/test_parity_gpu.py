@@ -236,6 +236,68 @@ def test_ideal_divb_with_sphere_and_mask():
             obstacle=(mask, np.array([0.03, -0.02, 0.01]), 0.1 * (rng.random((3,) + s) - 0.5)), streaming=1)
 
 
+def resist_workload(lattice, shape, bc, seed, sphere=None, eta=0.02, tau_relax=3.0):
+    """RESIST (K = 8 + 3 D): random ideal state plus random gradient variables G"""
+    w = random_workload("IDEAL", lattice, shape, bc, seed=seed, sphere=sphere)
+    rng = np.random.default_rng(seed + 2)
+    w["scheme"], w["tau_relax"], w["eta"] = "RESIST", tau_relax, eta
+    w["fields"] = np.concatenate([w["fields"], 0.05 * (rng.random((3 * len(shape),) + zyx(shape)) - 0.5)])
+    return w
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+@pytest.mark.parametrize("precision,tol", [(64, TOL64), (32, TOL32)])
+@pytest.mark.parametrize("lattice,shape,bc", [("D1Q3", (200,), (1, 1, 0, 0, 0, 0)), ("D2Q9", (150, 37), (0,) * 6),
+                                              ("D2Q9", (90, 21), (1, 1, 2, 1, 0, 0)), ("D3Q19", (200, 12, 9), (2, 1, 0, 0, 0, 0)),
+                                              ("D3Q19", (45, 11, 10), (1, 1, 1, 1, 1, 1)), ("D3Q7", (100, 12, 9), (1, 1, 1, 1, 0, 0)),
+                                              ("D2Q5", (150, 37), (0,) * 6)])
+def test_resist_scheme_parity(lattice, shape, bc, precision, tol, streaming):
+    """dissipative MHD with transported gradients (Eq.9-10): K = 8 + 3 D sets, resistive fluxes from G"""
+    w = resist_workload(lattice, shape, bc, seed=71)
+    compare(w, 20, tol=tol, precision=precision, streaming=streaming)
+    compare(w, 7, tol=tol, precision=precision, streaming=streaming)
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+def test_resist_with_sphere_and_mask(streaming):
+    cen = np.array([36.0, 12.0, 10.0])
+    mh = np.array([0.3, -0.5, 0.8]) / np.linalg.norm([0.3, -0.5, 0.8])
+    sph = dict(centre=cen, radius=6.0, u_solid=np.array([-0.25, 0.0, 0.0]), dipole_dir=mh, B_surface=0.03, width=1.5,
+               omega=np.array([0.02, 0.0, 0.02]))
+    compare(resist_workload("D3Q19", (72, 24, 20), (2, 1, 0, 0, 0, 0), seed=81, sphere=sph), 12, streaming=streaming)
+    rng = np.random.default_rng(19)
+    shape = (70, 33)
+    s = zyx(shape)
+    mask = (rng.random(s) < 0.05).astype(np.uint8) * 2
+    mask[rng.random(s) < 0.02] = 1
+    compare(resist_workload("D2Q9", shape, (1, 1) + (0,) * 4, seed=82), 12,
+            obstacle=(mask, np.array([0.03, -0.02, 0.01]), 0.1 * (rng.random((3,) + s) - 0.5)), streaming=streaming)
+
+
+def test_resist_physics_on_gpu():
+    """the CUDA path alone: a magnetic shear mode decays at (eta + (tau_B - 1/2) c_s^2) k^2 (the oracle's pin, re-run here)"""
+    from test_oracle_pins import ideal_fields
+    from paper_2606_00641_b200 import lbmhd
+    nx, tauB, eta, tau_m = 128, 0.6, 0.03, 4.0
+    k = 2 * np.pi / nx
+    x = np.arange(nx)
+    B = np.zeros((3, 1, 1, nx))
+    B[1, 0, 0] = 1e-4 * np.sin(k * x)
+    F8 = ideal_fields(np.ones((1, 1, nx)), np.zeros((3, 1, 1, nx)), B, 0.02 * np.ones((1, 1, nx)), 5 / 3)
+    F = np.concatenate([F8, np.zeros((3, 1, 1, nx))])
+    p = lbmhd.make_params("RESIST", "D1Q3", (nx,), gamma=5 / 3, tau=[0.6] * 5 + [tauB] * 3 + [0.6] * 3, powell=1.0, eta=eta,
+                          tau_relax=tau_m)
+    g = lbmhd.Lbmhd(p)
+    g.init(F)
+    g.step(200)
+    a1 = 2 * (g.moments()[0][6].reshape(-1) @ np.sin(k * x)) / nx
+    g.step(400)
+    a2 = 2 * (g.moments()[0][6].reshape(-1) @ np.sin(k * x)) / nx
+    rate = -np.log(a2 / a1) / 400
+    assert abs(rate / ((eta + (tauB - 0.5) / 3.0) * k * k) - 1) < 0.02
+    g.close()
+
+
 @pytest.mark.parametrize("streaming", [0, 1])
 @pytest.mark.parametrize("precision,tol", [(64, TOL64), (32, TOL32)])
 @pytest.mark.parametrize("lattice,shape,bc", [("D2Q9", (150, 37), (0,) * 6), ("D2Q9", (90, 21), (1, 1, 2, 1, 0, 0)),
