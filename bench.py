@@ -88,13 +88,14 @@ def aggregate_mlups(cells_per_rank, steps, ms, world):
     return world * cells_per_rank * steps / (ms * 1e-3) / 1e6
 
 
-def oracle_leg(workload_name, steps, warmup, budget_s=None):
+def oracle_leg(workload_name, steps, warmup, budget_s=None, scheme=None, lattice=None):
     """the CPU oracle, as it stands, on a bounded sample of the workload; -> (MLUPS, cores, sample text, ms/step)"""
     from oracle import oracle as orc
     from paper_2606_00641_b200 import workloads as W
     sys.path.insert(0, os.path.join(ROOT, "tests"))
     from parity_util import oracle_from_workload
     w = W.config5(shape=SAMPLE_SHAPE) if workload_name == "C5" else W.get(workload_name, small=True)
+    w = W.variant(w, scheme=scheme, lattice=lattice)
     o = oracle_from_workload(w)
     o.init(w["fields"])
     o.step(max(warmup, 1))
@@ -115,7 +116,7 @@ def oracle_leg(workload_name, steps, warmup, budget_s=None):
 def run_reference(args, rank):
     if rank != 0:
         return
-    mlups, cores, sample, ms, w = oracle_leg(args.workload, args.steps, args.warmup)
+    mlups, cores, sample, ms, w = oracle_leg(args.workload, args.steps, args.warmup, scheme=args.scheme, lattice=args.lattice)
     line = {"impl": "reference", "metric": METRIC, "value": mlups, "unit": "MLUPS", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -149,7 +150,7 @@ def run_native(args, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    w = W.get(args.workload)
+    w = W.variant(W.get(args.workload), scheme=args.scheme, lattice=args.lattice)
     N = int(np.prod(w["shape"]))
     prec = args.precision
     sim = lbmhd.from_workload(w, precision=prec, device=local_rank, streaming=1 if args.streaming == "inplace" else 0)
@@ -212,7 +213,7 @@ def run_native(args, rank, world, local_rank):
     e2e_val = aggregate_mlups(N, args.steps, ms_e2e, world)
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.csv")      # dram__bytes_read/write.sum of one ncu --set full capture
-    if os.path.exists(tpath) and prec == 64 and args.streaming == "ab":
+    if os.path.exists(tpath) and prec == 64 and args.streaming == "ab" and args.scheme is None and args.lattice is None:
         with open(tpath) as f:
             for row in f.read().splitlines()[1:]:
                 cols = row.split(",")
@@ -240,7 +241,7 @@ def run_native(args, rank, world, local_rank):
         "gpu_launches": int(launches), "clocks": sampler.result(),
     }
     if world == 1 and not args.no_cpu_baseline:
-        mlups, cores, sample, _, _ = oracle_leg(args.workload, 10 ** 9, 1, budget_s=args.cpu_seconds)
+        mlups, cores, sample, _, _ = oracle_leg(args.workload, 10 ** 9, 1, budget_s=args.cpu_seconds, scheme=args.scheme, lattice=args.lattice)
         line["cpu_baseline"] = {"value": mlups, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": sample}
     print(json.dumps(line), flush=True)
     if world > 1:
@@ -322,6 +323,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--scheme", default=None, choices=["IDEAL_DIVB", "RESIST"],
+                    help="run the ideal-MHD workload on a scheme with transported gradient sets (DESIGN.md A19, A22)")
+    ap.add_argument("--lattice", default=None, choices=["D2Q5", "D3Q7"], help="the paper's own lattice instead of D2Q9 / D3Q19")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--streaming", default="ab", choices=["ab", "inplace"])
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],

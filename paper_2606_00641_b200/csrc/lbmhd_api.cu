@@ -187,9 +187,6 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
   }
   h->ws = (char *)p->workspace;
   h->stream = (cudaStream_t)p->stream;
-  h->tx = 32; h->minb = g.Q > 9 ? 3 : 4;     // measured best on B200: D3Q19 80 regs x 3 blocks/SM, D2Q9/D1Q3 64 regs x 4
-  if (const char *e = getenv("LBMHD_TX")) h->tx = atoi(e);        // tuning knobs; unknown pairs fall back to 32/3
-  if (const char *e = getenv("LBMHD_MINB")) h->minb = atoi(e);
   cudaError_t e = cudaSetDevice(p->device);
   if (e != cudaSuccess) { delete h; return fail(LBMHD_ECUDA, "cudaSetDevice(%d): %s", p->device, cudaGetErrorString(e)); }
   {
@@ -197,10 +194,10 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
     if (e != cudaSuccess) { delete h; return fail(LBMHD_ECUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e)); }
     h->num_sms = sms;
-    h->pair = p->precision == 32 && p->nx % 2 == 0 && p->eta_jc == 0.0 && p->scheme != LBMHD_RESIST;   // eta(j), RESIST: one-cell kernels
+    h->pair = p->eta_jc == 0.0;      // several cells per thread where the lattice has a multi-cell kernel; eta(j): one-cell kernels
     if (const char *e3 = getenv("LBMHD_PAIR")) h->pair = h->pair && atoi(e3) != 0;
-    h->split = false;   // measured slower on config 5: edge tiles lose DRAM page locality when launched apart from their rows
-    if (const char *e2 = getenv("LBMHD_SPLIT")) h->split = atoi(e2) != 0;
+    h->cluster = p->scheme == LBMHD_RESIST && g.Q > 9;      // measured: pays on D3Q19 only
+    if (const char *e4 = getenv("LBMHD_CLUSTER")) h->cluster = h->cluster && atoi(e4) != 0;
     const char *path = getenv("LBMHD_PATH");      // tuning knob: "plain" forces the register-pull kernel
     const size_t es = p->precision == 64 ? 8 : 4;
     const long long tiles = (long long)((p->nx + kTmaTX - 1) / kTmaTX) * p->ny * p->nz;

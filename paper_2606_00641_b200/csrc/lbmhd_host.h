@@ -58,9 +58,8 @@ struct lbmhd {
   double dip_off[4][3], dip_m[4][3], dip_Bs[4], dip_core[4];
   double obs_om[3], obs_c[3];   // rigid rotation of masked bodies
   long long sph_t0;
-  int tx, minb;          // x-tile and min blocks/SM (launch bound) of the plain step kernel
-  bool pair;             // fp32: two cells per thread (even nx); LBMHD_PAIR=0 turns it off
-  bool split;            // interior / edge launches split (large grids); LBMHD_SPLIT=0/1 overrides
+  bool cluster;          // RESIST: variable rows of a tile split over a 2-CTA cluster; LBMHD_CLUSTER=0 turns it off
+  bool pair;             // several cells per thread on interior tiles (fp32; fp64 on the short lattices); LBMHD_PAIR=0 turns it off
   bool use_tma;          // TMA-staged persistent step kernel (needs nx * sizeof(real) % 16 == 0)
   int num_sms;
   CUtensorMap tmap[2][2];   // [copy][0: tile-wide box, 1: box 16 bytes wider] 5D views (x, y, z, i, k) of the populations

@@ -447,16 +447,74 @@ __device__ __forceinline__ void body_accumulate(const StepArgs<real> &a, const C
 }
 
 // =====================================================================================================
+// How the K variable rows of a tile exchange their moments.  The threads of a tile write the K zeroth moments
+// (sQ), the first moments of the B sets (sTr) and, on a zero-gradient x face, the neighbour state (sNb) for
+// each other and meet at a barrier.
+//   CL = false  one CTA holds all K rows: shared memory + a block barrier (`Sync`: __syncthreads or a named barrier).
+//   CL = true   a 2-CTA cluster splits the rows (RESIST: K = 11 / 14 / 17 rows in one block would leave an SM with
+//               one or two blocks, i.e. no other block's loads in flight while one computes): each CTA keeps a full
+//               copy of the arrays, every value is written into both copies (the partner's through distributed
+//               shared memory) and the barrier is the cluster's (release / acquire, so the remote writes are
+//               visible).  begin() waits for the start barrier the kernel arrived at on entry: the partner CTA is
+//               resident before its shared memory is written.  All remote writes precede a barrier both CTAs
+//               pass, so neither can exit while the other still writes into it.
+// =====================================================================================================
+struct SyncBlock {
+  __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_arrive_release() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait_acquire() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
+template <typename real, int W, bool CL, class Sync = SyncBlock> struct Share {
+  real (*sQ)[W];
+  real (*sTr)[W];
+  real *sNb;
+  real (*rQ)[W];      // the partner CTA's copies (CL only)
+  real (*rTr)[W];
+  real *rNb;
+  Sync sync_;
+  __device__ __forceinline__ void begin() const {
+    if (CL) cluster_wait_acquire();
+  }
+  __device__ __forceinline__ void putQ(int l, int tx, real v) const {
+    sQ[l][tx] = v;
+    if (CL) rQ[l][tx] = v;
+  }
+  __device__ __forceinline__ void putTr(int j, int tx, real v) const {
+    sTr[j][tx] = v;
+    if (CL) rTr[j][tx] = v;
+  }
+  __device__ __forceinline__ void putNb(int l, real v) const {
+    sNb[l] = v;
+    if (CL) rNb[l] = v;
+  }
+  __device__ __forceinline__ void sync() const {
+    if (CL) {
+      cluster_arrive_release();
+      cluster_wait_acquire();
+    } else {
+      sync_();
+    }
+  }
+  // the same arrays seen W2 cells wide (W2 <= W): the one-cell paths of the multi-cell kernels
+  template <int W2> __device__ __forceinline__ Share<real, W2, CL, Sync> narrow() const {
+    return Share<real, W2, CL, Sync>{reinterpret_cast<real(*)[W2]>(&sQ[0][0]), reinterpret_cast<real(*)[W2]>(&sTr[0][0]), sNb,
+                                    reinterpret_cast<real(*)[W2]>(CL ? &rQ[0][0] : nullptr),
+                                    reinterpret_cast<real(*)[W2]>(CL ? &rTr[0][0] : nullptr), rNb, sync_};
+  }
+};
+
+// =====================================================================================================
 // Everything after the pull: boundary substitution (A9), moments exchange, div-B estimate, Powell source,
 // solid blend, flux, BGK + direct injection, store (DESIGN.md §2 steps S2-S8; Eq.2-4, 8, 11-14).
-// sQ[K][TX], sTr[D*D][TX] are shared arrays of the TX*K threads that call this together; `sync` is their
-// barrier (__syncthreads or a named barrier).  BND / SOLID are tile-uniform: the interior fluid tile (both
+// `sh` (Share) holds the exchange arrays sQ[K][TX], sTr[D*D][TX] of the threads that call this together and their
+// barrier.  BND / SOLID are tile-uniform: the interior fluid tile (both
 // false) is the hot path and carries no boundary predicates, no mask or sphere test.  `store` says where
 // result j goes (streaming layout); STREAM only selects where Q^nb comes from.
 // =====================================================================================================
-template <int LAT, int SCHEME, typename real, int TX, bool BND, bool SOLID, int STREAM, class FArr, class Store, class Sync>
-__device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellCtx &c, FArr &f, const Store &store,
-                                            real (*sQ)[TX], real (*sTr)[TX], Sync sync) {
+template <int LAT, int SCHEME, typename real, int TX, bool BND, bool SOLID, int STREAM, class FArr, class Store, class Sh>
+__device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellCtx &c, FArr &f, const Store &store, const Sh &sh) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
   using V = Vars<SCHEME, D>;
@@ -481,13 +539,13 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
       } else {                    // in place the neighbour's slots are in flux: it published its moment last step
         s = (real)a.M_cur[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + nb];
       }
-      sQ[k][tx] = s;
+      sh.putQ(k, tx, s);
     }
-    sync();
+    sh.sync();
     if (cell_bnd) {
       real Qnb[K], Phi[3];
 #pragma unroll
-      for (int l = 0; l < K; l++) Qnb[l] = sQ[l][tx];
+      for (int l = 0; l < K; l++) Qnb[l] = sh.sQ[l][tx];
       flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
       const real Qnbk = pick<K, real>(Qnb, k);
 #pragma unroll
@@ -499,14 +557,14 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
         if (outside) f[i] = real(L::w(i)) * (Qnbk + real(L::inv_cs2) * cPhi);
       }
     }
-    sync();
+    sh.sync();
   }
 
   // S2 zeroth moment of this set (index order) and S3 this set's share of tr Pi_B
   real Qk = real(0);
 #pragma unroll
   for (int i = 0; i < Q; i++) Qk += f[i];
-  sQ[k][tx] = Qk;
+  sh.putQ(k, tx, Qk);
   if (k >= iB && k < iB + D) {
     const int b = k - iB;   // warp-uniform
     // first moment of this B set, Pi_{a,b} = sum_i c_ia f_i: the diagonal entry is its share of tr Pi_B (A6); the
@@ -529,17 +587,17 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
     }
 #pragma unroll
     for (int al = 0; al < D; al++)
-      if (SCHEME == kIncres || al == b) sTr[b * D + al][tx] = m[al];
+      if (SCHEME == kIncres || al == b) sh.putTr(b * D + al, tx, m[al]);
   }
-  sync();
+  sh.sync();
   if (!work) return;
 
   real Qv[K];
 #pragma unroll
-  for (int l = 0; l < K; l++) Qv[l] = sQ[l][tx];
+  for (int l = 0; l < K; l++) Qv[l] = sh.sQ[l][tx];
   real tr = real(0);
 #pragma unroll
-  for (int b = 0; b < D; b++) tr += sTr[b * D + b][tx];
+  for (int b = 0; b < D; b++) tr += sh.sTr[b * D + b][tx];
   // A20: current-dependent resistivity -> cell-local tau_B (6 Newton steps on tau^3 - tau0 tau^2 - c = 0 from tau0 + cbrt(c))
   real inv_tauB_cs2 = a.inv_tauB_cs2;
   real omB = real(0);
@@ -551,7 +609,7 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
       for (int be = al + 1; be < D; be++) {
         // N_ab = Pi_ab - Phi_{B_b,a},  Phi_{B_b,a} = u_a B_b - B_a u_b  (antisymmetric in a <-> b)
         const real phi = Qv[1 + al] * Qv[1 + D + be] - Qv[1 + D + al] * Qv[1 + be];
-        const real w2 = (sTr[be * D + al][tx] - phi) - (sTr[al * D + be][tx] + phi);
+        const real w2 = (sh.sTr[be * D + al][tx] - phi) - (sh.sTr[al * D + be][tx] + phi);
         a2 += w2 * w2;
       }
     a2 *= real(L::inv_cs2 * L::inv_cs2);
@@ -622,9 +680,8 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
 // finish_cell with boundary and solid handling compiled in.  Used by every step kernel for the tiles that are
 // not interior; the TX*K threads of the tile call it together.
 // =====================================================================================================
-template <int LAT, int SCHEME, typename real, int TX, int STREAM, class Sync>
-__device__ __forceinline__ void general_tile(const StepArgs<real> &a, int tx, int k, int x, int y, int z, real (*sQ)[TX],
-                                             real (*sTr)[TX], Sync sync) {
+template <int LAT, int SCHEME, typename real, int TX, int STREAM, class Sh>
+__device__ __forceinline__ void general_tile(const StepArgs<real> &a, int tx, int k, int x, int y, int z, const Sh &sh) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
@@ -679,8 +736,9 @@ __device__ __forceinline__ void general_tile(const StepArgs<real> &a, int tx, in
     f[i] = (work && !outside) ? srck[at] : real(0);
   }
   CellCtx c{tx, k, x, y, z, n, work, out_xm, out_xp, out_ym, out_yp, out_zm, out_zp, true};
-  if (STREAM == ST_PP) finish_cell<LAT, SCHEME, real, TX, true, true, STREAM>(a, c, f, pp, sQ, sTr, sync);
-  else finish_cell<LAT, SCHEME, real, TX, true, true, STREAM>(a, c, f, own, sQ, sTr, sync);
+  sh.begin();
+  if (STREAM == ST_PP) finish_cell<LAT, SCHEME, real, TX, true, true, STREAM>(a, c, f, pp, sh);
+  else finish_cell<LAT, SCHEME, real, TX, true, true, STREAM>(a, c, f, own, sh);
 }
 
 // Which tiles a launch covers: block (bx, by, bz) -> tile (bx0 + bx*bxs, y0 + by*ys, z0 + bz*zs).
@@ -693,21 +751,23 @@ struct Region {
 // MODE 0: one launch over all tiles; interior tiles take the lean path, x-edge tiles of interior rows the lean
 //         edge path, the others general_tile().
 // MODE 1: interior tiles only (no general path compiled in); MODE 2: general tiles only, over a Region.
-//         (split launches: measured slower, kept behind LBMHD_SPLIT=1, A/B only.)
+//         (split launches were measured slower; the modes remain for register-use checks.)
 // =====================================================================================================
 // One TX-cell tile of row (y, z) starting at x0: classification and the three paths (interior / x-edge / general).
 // Called by all TX*K threads of a block together (it contains block barriers).
-template <int LAT, int SCHEME, typename real, int TX, int MODE, int STREAM>
+template <int LAT, int SCHEME, typename real, int TX, int MODE, int STREAM, class Sh>
 __device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, const int k, const int x0, const int y, const int z,
-                                         const int sphere_only, real (*sQ)[TX], real (*sTr)[TX]) {
+                                         const int sphere_only, const Sh &sh) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
   using V = Vars<SCHEME, D>;
   constexpr int K = V::K;
   const int x = x0 + tx;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
-  if (ghost_row<real, D>(a, y, z)) return;
-  const auto sync = [] { __syncthreads(); };
+  if (ghost_row<real, D>(a, y, z)) {
+    sh.begin();      // cluster: consume the start barrier the kernel arrived at
+    return;
+  }
   const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
 
   // block-uniform classification.  Interior tile: no face, no wrap in any direction, every thread active, no
@@ -719,8 +779,10 @@ __device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, 
   const bool interior = inner_pos && a.mask == nullptr && !touched;
   // in place: rows next to a non-periodic y/z face publish their moments (Q^nb of the face cells, A9)
   const bool rowM = STREAM != ST_AB && ((npy && (y == 1 || y == ny - 2)) || (npz && (z == 1 || z == nz - 2)));
-  if (MODE == 1 && !interior) return;
-  if (MODE == 2 && sphere_only && !(inner_pos && touched)) return;
+  if ((MODE == 1 && !interior) || (MODE == 2 && sphere_only && !(inner_pos && touched))) {
+    sh.begin();
+    return;
+  }
   if (MODE != 2 && interior) {
     const uint32_t n = ((uint32_t)z * ny + y) * nx + x;
     char *__restrict__ pb = reinterpret_cast<char *>(const_cast<real *>(a.src) + ((size_t)k * Q * a.pstride + n));
@@ -729,19 +791,20 @@ __device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, 
     for (int i = 0; i < Q; i++) f[i] = *reinterpret_cast<const real *>(pb + (STREAM == ST_LOC ? a.st_off[opp(i)] : a.ld_off[i]));
     const bool writeM = STREAM != ST_AB && (rowM || (npx && (x == 1 || x == nx - 2)));
     CellCtx c{tx, k, x, y, z, n, true, false, false, false, false, false, false, writeM};
+    sh.begin();
     if (STREAM == ST_AB) {
       const StoreOwn<real> st{reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + n)), a.st_off};
-      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sQ, sTr, sync);
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sh);
     } else if (STREAM == ST_PP) {
       const StorePPInterior<real> st{pb, a.ld_off};
-      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sQ, sTr, sync);
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sh);
     } else {
       const StoreOwn<real> st{pb, a.st_off};
-      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sQ, sTr, sync);
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sh);
     }
     return;
   }
-  if (MODE == 1) return;
+  if (MODE == 1) return;      // (never reached: MODE 1 left above)
 
   // x-edge tile of an otherwise interior row (no mask, sphere out of reach, not both ends in one tile): lean
   // loads for every thread; only the thread ON the face differs (A9-A11):
@@ -774,8 +837,8 @@ __device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, 
       }
       f[i] = *reinterpret_cast<const real *>(pb + off);
     }
-    __shared__ real sNb[K];
     const bool tile_zg = bcf == BC_ZEROGRAD;                 // tile-uniform
+    sh.begin();
     if (tile_zg) {
       const uint32_t nb = ((uint32_t)z * ny + y) * nx + (edge_lo ? 1 : nx - 2);
       if (STREAM == ST_AB) {
@@ -783,15 +846,15 @@ __device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, 
         real v = tx < Q ? a.src[(size_t)k * Q * a.pstride + (size_t)tx * a.pstride + nb] : real(0);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if (tx == 0) sNb[k] = v;
+        if (tx == 0) sh.putNb(k, v);
       } else {
-        if (tx == 0) sNb[k] = (real)a.M_cur[(size_t)k * ((size_t)nx * ny * nz) + nb];
+        if (tx == 0) sh.putNb(k, (real)a.M_cur[(size_t)k * ((size_t)nx * ny * nz) + nb]);
       }
-      __syncthreads();
+      sh.sync();
       if (zg) {
         real Qnb[K], Phi[3];
 #pragma unroll
-        for (int l = 0; l < K; l++) Qnb[l] = sNb[l];
+        for (int l = 0; l < K; l++) Qnb[l] = sh.sNb[l];
         flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
         const real Qnbk = pick<K, real>(Qnb, k);
 #pragma unroll
@@ -810,19 +873,19 @@ __device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, 
 #pragma unroll
         for (int i = 0; i < Q; i++) st.put(i, f[i]);
       }
-      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sQ, sTr, sync);
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sh);
     } else if (STREAM == ST_PP) {
       const StorePPEdge<L, real> st{pb, a.ld_off, a.st_off, edge_lo, on_face, wrap, wrap_adj};
       if (frozen) frozen_rematerialise<LAT, SCHEME, real>(a, k, n, st);
-      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sQ, sTr, sync);
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sh);
     } else {
       const StoreOwn<real> st{pb, a.st_off};
       if (frozen) frozen_rematerialise<LAT, SCHEME, real>(a, k, n, st);
-      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sQ, sTr, sync);
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sh);
     }
     return;
   }
-  general_tile<LAT, SCHEME, real, TX, STREAM>(a, tx, k, x, y, z, sQ, sTr, sync);
+  general_tile<LAT, SCHEME, real, TX, STREAM>(a, tx, k, x, y, z, sh);
 }
 
 template <int LAT, int SCHEME, typename real, int TX, int MINB, int MODE, int STREAM>
@@ -832,165 +895,238 @@ step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int 
   constexpr int D = L::D, K = Vars<SCHEME, D>::K;
   __shared__ real sQ[K][TX];
   __shared__ real sTr[D * D][TX];
+  __shared__ real sNb[K];
+  const Share<real, TX, false> sh{sQ, sTr, sNb, nullptr, nullptr, nullptr, SyncBlock{}};
   run_tile<LAT, SCHEME, real, TX, MODE, STREAM>(a, threadIdx.x, threadIdx.y, (r.bx0 + (int)blockIdx.x * r.bxs) * TX,
-                                                r.y0 + (int)blockIdx.y * r.ys, r.z0 + (int)blockIdx.z * r.zs, sphere_only, sQ, sTr);
+                                                r.y0 + (int)blockIdx.y * r.ys, r.z0 + (int)blockIdx.z * r.zs, sphere_only, sh);
+}
+
+// The same step with the K rows of a tile split over a 2-CTA cluster (Share<.., CL = true>): CTA `rank` owns rows
+// rank*KH .. rank*KH + KH - 1 (KH = ceil(K/2)); for odd K the last warp of CTA 1 has no row and exits at once (exited
+// threads count as arrived at the cluster barrier).  grid.x = 2 * tiles_x.
+template <int LAT, int SCHEME, typename real, int MINB, int STREAM>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(32 * ((Vars<SCHEME, Lattice<LAT>::D>::K + 1) / 2), MINB)
+step_kernel_cl(const __grid_constant__ StepArgs<real> a) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, K = Vars<SCHEME, D>::K, KH = (K + 1) / 2;
+  __shared__ real sQ[K][32];
+  __shared__ real sTr[D * D][32];
+  __shared__ real sNb[K];
+  const unsigned rank = blockIdx.x & 1u;
+  const int k = (int)rank * KH + (int)threadIdx.y;
+  if (k >= K) return;
+  cluster_arrive_relaxed();      // start barrier; Share::begin() waits for it
+  namespace cg = cooperative_groups;
+  cg::cluster_group cl = cg::this_cluster();
+  const Share<real, 32, true> sh{sQ, sTr, sNb, cl.map_shared_rank(sQ, rank ^ 1u), cl.map_shared_rank(sTr, rank ^ 1u),
+                                 cl.map_shared_rank(sNb, rank ^ 1u), SyncBlock{}};
+  run_tile<LAT, SCHEME, real, 32, 0, STREAM>(a, threadIdx.x, k, (int)(blockIdx.x >> 1) * 32, blockIdx.y, blockIdx.z, 0, sh);
 }
 
 // =====================================================================================================
-// fp32 variant with TWO adjacent cells per thread.  With 4-byte populations a warp's row
-// segment is only 128 bytes, so the one-cell mapping needs twice the instructions per byte and is issue-bound
-// (measured 4.4-4.9 TB/s).  Here a block owns 64 x-cells x K sets with the same 32 x K threads; thread tx
-// holds cells x0 + 2 tx and x0 + 2 tx + 1: float2 loads for the 9 unshifted directions and float2 stores
-// for all, two scalar loads where the x-shift breaks the 8-byte alignment.  Interior tiles only; every
-// other tile is handed to run_tile() in 32-cell pieces.
+// Several adjacent cells per thread.  With one cell per thread a warp moves 32*sizeof(real)
+// bytes per load: 128 bytes in fp32, and only Q loads are in flight per thread, so the short lattices (D3Q7,
+// D2Q5, D1Q3) and fp32 run out of bytes in flight long before the SM runs out of warps (measured: fp32
+// D3Q19 4.9 TB/s, fp64 D3Q7 5.4, fp32 D3Q7 4.5 with one cell per thread).  Here a block owns 32*NC x-cells
+// x K sets with the same 32 x K threads; thread tx holds cells x0 + NC tx .. x0 + NC tx + NC - 1: one
+// NC-wide vector load (8 or 16 bytes) per direction without x-shift and one vector store per direction, NC
+// scalar loads where the x-shift breaks the vector alignment.  Interior tiles only; every other tile is
+// handed to run_tile() in 32-cell pieces.  Needs nx % NC == 0 (vector alignment of every row).
 // =====================================================================================================
-template <typename real> struct StorePairOwn {
+template <typename real, int NC> __device__ __forceinline__ void ldv(const char *p, real (&v)[NC]) {
+  static_assert(NC == 2 || (NC * sizeof(real)) % 16 == 0, "vector width");
+  if constexpr (NC * sizeof(real) == 8) {
+    const float2 t = *reinterpret_cast<const float2 *>(p);
+    v[0] = t.x; v[1] = t.y;
+  } else if constexpr (sizeof(real) == 4) {
+#pragma unroll
+    for (int j = 0; j < NC / 4; j++) {
+      const float4 t = *reinterpret_cast<const float4 *>(p + 16 * j);
+      v[4 * j] = t.x; v[4 * j + 1] = t.y; v[4 * j + 2] = t.z; v[4 * j + 3] = t.w;
+    }
+  } else {
+#pragma unroll
+    for (int j = 0; j < NC / 2; j++) {
+      const double2 t = *reinterpret_cast<const double2 *>(p + 16 * j);
+      v[2 * j] = t.x; v[2 * j + 1] = t.y;
+    }
+  }
+}
+template <typename real, int NC> __device__ __forceinline__ void stv(char *p, const real (&v)[NC]) {
+  if constexpr (NC * sizeof(real) == 8) {
+    *reinterpret_cast<float2 *>(p) = make_float2(v[0], v[1]);
+  } else if constexpr (sizeof(real) == 4) {
+#pragma unroll
+    for (int j = 0; j < NC / 4; j++) *reinterpret_cast<float4 *>(p + 16 * j) = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+  } else {
+#pragma unroll
+    for (int j = 0; j < NC / 2; j++) *reinterpret_cast<double2 *>(p + 16 * j) = make_double2(v[2 * j], v[2 * j + 1]);
+  }
+}
+
+template <typename real, int NC> struct StoreMultiOwn {
   char *base;
   const long long *st_off;
-  __device__ __forceinline__ void put2(int j, real v0, real v1) const {
-    *reinterpret_cast<float2 *>(base + st_off[j]) = make_float2(v0, v1);
-  }
+  __device__ __forceinline__ void put(int j, const real (&v)[NC]) const { stv<real, NC>(base + st_off[j], v); }
 };
-template <class L, typename real> struct StorePairPP {
+template <class L, typename real, int NC> struct StoreMultiPP {
   char *base;
   const long long *ld_off;
-  __device__ __forceinline__ void put2(int j, real v0, real v1) const {
+  __device__ __forceinline__ void put(int j, const real (&v)[NC]) const {
     const int i = opp(j);
     if (L::cx(i) == 0) {
-      *reinterpret_cast<float2 *>(base + ld_off[i]) = make_float2(v0, v1);
+      stv<real, NC>(base + ld_off[i], v);
     } else {
-      *reinterpret_cast<real *>(base + ld_off[i]) = v0;
-      *reinterpret_cast<real *>(base + ld_off[i] + (long long)sizeof(real)) = v1;
+#pragma unroll
+      for (int c = 0; c < NC; c++) *reinterpret_cast<real *>(base + ld_off[i] + (long long)(c * sizeof(real))) = v[c];
     }
   }
 };
 
-template <int LAT, int SCHEME, int STREAM, class Store>
-__device__ __forceinline__ void finish_pair(const StepArgs<float> &a, int tx, int k, uint32_t n, bool writeM0, bool writeM1,
-                                            float (&f0)[Lattice<LAT>::Q], float (&f1)[Lattice<LAT>::Q], const Store &store,
-                                            float (*sQ)[64], float (*sTr)[64]) {
+// S2-S8 of NC fluid cells of an interior tile (no boundary, no solid, constant eta).  sQ / sTr rows are laid out
+// [c][32] (cell c of lane tx at c*32 + tx): conflict-free scalar accesses.
+template <int LAT, int SCHEME, typename real, int NC, int STREAM, class Store>
+__device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, int k, uint32_t n, const bool (&writeM)[NC],
+                                             real (&f)[NC][Lattice<LAT>::Q], const Store &store, real (*sQ)[32 * NC],
+                                             real (*sTr)[32 * NC]) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
   using V = Vars<SCHEME, D>;
   constexpr int K = V::K, iB = V::iB;
-  float Qk0 = 0.f, Qk1 = 0.f;
+  constexpr bool use_tr = !has_relax(SCHEME);       // A6; the schemes with gradient sets take div B from them
+  real Qk[NC];
 #pragma unroll
-  for (int i = 0; i < Q; i++) { Qk0 += f0[i]; Qk1 += f1[i]; }
-  *reinterpret_cast<float2 *>(&sQ[k][2 * tx]) = make_float2(Qk0, Qk1);
-  if (k >= iB && k < iB + D) {
+  for (int c = 0; c < NC; c++) {
+    real s = real(0);
+#pragma unroll
+    for (int i = 0; i < Q; i++) s += f[c][i];
+    Qk[c] = s;
+    sQ[k][c * 32 + tx] = s;
+  }
+  if (use_tr && k >= iB && k < iB + D) {
     const int b = k - iB;
-    float t0 = 0.f, t1 = 0.f;
 #pragma unroll
-    for (int i = 0; i < Q; i++) {
-      const int cb = lat_c<L>(i, 0) * (b == 0) + lat_c<L>(i, 1) * (b == 1) + lat_c<L>(i, 2) * (b == 2);
-      if (lat_c<L>(i, 0) != 0 || lat_c<L>(i, 1) != 0 || lat_c<L>(i, 2) != 0) { t0 += float(cb) * f0[i]; t1 += float(cb) * f1[i]; }
+    for (int c = 0; c < NC; c++) {
+      real t = real(0);
+#pragma unroll
+      for (int i = 0; i < Q; i++) {
+        const int cb = lat_c<L>(i, 0) * (b == 0) + lat_c<L>(i, 1) * (b == 1) + lat_c<L>(i, 2) * (b == 2);
+        if (lat_c<L>(i, 0) != 0 || lat_c<L>(i, 1) != 0 || lat_c<L>(i, 2) != 0) t += real(cb) * f[c][i];
+      }
+      sTr[b * D + b][c * 32 + tx] = t;
     }
-    *reinterpret_cast<float2 *>(&sTr[b * D + b][2 * tx]) = make_float2(t0, t1);
   }
   __syncthreads();
-  float Qv0[K], Qv1[K];
+  const real om = a.omega[k], omc = real(1) - om;
+  const real ic = real(L::inv_cs2) * om;
+  real b0[NC], P[NC][3];
 #pragma unroll
-  for (int l = 0; l < K; l++) {
-    const float2 q = *reinterpret_cast<const float2 *>(&sQ[l][2 * tx]);
-    Qv0[l] = q.x; Qv1[l] = q.y;
-  }
-  float tr0 = 0.f, tr1 = 0.f;
+  for (int c = 0; c < NC; c++) {
+    real Qv[K];
 #pragma unroll
-  for (int b = 0; b < D; b++) {
-    const float2 t = *reinterpret_cast<const float2 *>(&sTr[b * D + b][2 * tx]);
-    tr0 += t.x; tr1 += t.y;
+    for (int l = 0; l < K; l++) Qv[l] = sQ[l][c * 32 + tx];
+    real delta;
+    if (SCHEME == kIdealD) {
+      delta = Qv[K - 1] * a.inv_tau_relax;
+    } else if (SCHEME == kResist) {
+      delta = real(0);
+#pragma unroll
+      for (int al = 0; al < D; al++) delta += Qv[8 + 3 * al + al] * a.inv_tau_relax;
+    } else {
+      real tr = real(0);
+#pragma unroll
+      for (int b = 0; b < D; b++) tr += sTr[b * D + b][c * 32 + tx];
+      delta = -tr * a.inv_tauB_cs2;
+    }
+    real Phi[3];
+    flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
+    real inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
+    if (has_relax(SCHEME) && k >= 8) inj = -Qk[c] * a.inv_tau_relax;      // relaxation source of Eq.6
+    if (STREAM != ST_AB && writeM[c]) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + n + c] = (double)(Qk[c] + inj);
+    b0[c] = om * Qk[c] + inj;
+    P[c][0] = ic * Phi[0]; P[c][1] = ic * Phi[1]; P[c][2] = ic * Phi[2];
   }
-  float Phi0[3], Phi1[3];
-  flux_row<SCHEME, D, float>(k, Qv0, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi0);
-  flux_row<SCHEME, D, float>(k, Qv1, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi1);
-  // -kappa delta S_row with delta = -tr/(tau_B cs2) (A6) or D/tau_M (kIdealD)
-  const float d0 = SCHEME == kIdealD ? Qv0[K - 1] * a.inv_tau_relax : -tr0 * a.inv_tauB_cs2;
-  const float d1 = SCHEME == kIdealD ? Qv1[K - 1] * a.inv_tau_relax : -tr1 * a.inv_tauB_cs2;
-  float inj0 = -(a.kappa * d0) * powell_row<SCHEME, D, float>(k, Qv0);
-  float inj1 = -(a.kappa * d1) * powell_row<SCHEME, D, float>(k, Qv1);
-  if (SCHEME == kIdealD && k == K - 1) { inj0 = -Qk0 * a.inv_tau_relax; inj1 = -Qk1 * a.inv_tau_relax; }
-  if (STREAM != ST_AB) {
-    const size_t N = (size_t)a.nx * a.ny * a.nz;
-    if (writeM0) a.M_next[(size_t)k * N + n] = (double)(Qk0 + inj0);
-    if (writeM1) a.M_next[(size_t)k * N + n + 1] = (double)(Qk1 + inj1);
-  }
-  const float om = a.omega[k], omc = 1.f - om;
-  const float b00 = om * Qk0 + inj0, b01 = om * Qk1 + inj1;
-  const float ic = float(L::inv_cs2) * om;
-  const float P00 = ic * Phi0[0], P01 = ic * Phi0[1], P02 = ic * Phi0[2];
-  const float P10 = ic * Phi1[0], P11 = ic * Phi1[1], P12 = ic * Phi1[2];
 #pragma unroll
   for (int i = 0; i < Q; i++) {
-    float t0 = float(L::w(i)) * b00, t1 = float(L::w(i)) * b01;
-    if (L::cx(i) != 0) { t0 = fmaf(float(L::cx(i) * L::w(i)), P00, t0); t1 = fmaf(float(L::cx(i) * L::w(i)), P10, t1); }
-    if (L::cy(i) != 0) { t0 = fmaf(float(L::cy(i) * L::w(i)), P01, t0); t1 = fmaf(float(L::cy(i) * L::w(i)), P11, t1); }
-    if (L::cz(i) != 0) { t0 = fmaf(float(L::cz(i) * L::w(i)), P02, t0); t1 = fmaf(float(L::cz(i) * L::w(i)), P12, t1); }
-    store.put2(i, fmaf(f0[i], omc, t0), fmaf(f1[i], omc, t1));
+    real out[NC];
+#pragma unroll
+    for (int c = 0; c < NC; c++) {
+      real t = real(L::w(i)) * b0[c];
+      if (L::cx(i) != 0) t = fma(real(L::cx(i) * L::w(i)), P[c][0], t);
+      if (L::cy(i) != 0) t = fma(real(L::cy(i) * L::w(i)), P[c][1], t);
+      if (L::cz(i) != 0) t = fma(real(L::cz(i) * L::w(i)), P[c][2], t);
+      out[c] = fma(f[c][i], omc, t);
+    }
+    store.put(i, out);
   }
 }
 
-template <int LAT, int SCHEME, int MINB, int STREAM>
+// Row layout: [32-cell edge tile][nmulti tiles of 32*NC cells][rest in 32-cell tiles], one block each, so that the
+// multi-cell tiles are all interior in x; blocks 0..nmulti-1 are those tiles, block nmulti the first edge tile.
+template <int LAT, int SCHEME, typename real, int NC, int MINB, int STREAM>
 __global__ void __launch_bounds__(32 * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
-step_kernel_pair(const __grid_constant__ StepArgs<float> a, const int npair) {
+step_kernel_multi(const __grid_constant__ StepArgs<real> a, const int nmulti) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
   using V = Vars<SCHEME, D>;
-  constexpr int K = V::K;
-  __shared__ float sQ[K][64];
-  __shared__ float sTr[D * D][64];
+  constexpr int K = V::K, W = 32 * NC;
+  __shared__ real sQ[K][W];
+  __shared__ real sTr[D * D][W];
+  __shared__ real sNb[K];
   const int tx = threadIdx.x, k = threadIdx.y;
-  // row layout: [32-cell edge tile][npair 64-cell pair tiles][rest in 32-cell tiles], one block each, so that the pair
-  // tiles are all interior when the row is; blocks 0..npair-1 are the pair tiles, block npair the first edge tile
   const int nx = a.nx, ny = a.ny, nz = a.nz;
   const int y = blockIdx.y, z = blockIdx.z;
-  if (ghost_row<float, D>(a, y, z)) return;
-  float(*sQ32)[32] = reinterpret_cast<float(*)[32]>(&sQ[0][0]);
-  float(*sTr32)[32] = reinterpret_cast<float(*)[32]>(&sTr[0][0]);
-  if ((int)blockIdx.x >= npair) {
-    const int t = (int)blockIdx.x - npair;
-    run_tile<LAT, SCHEME, float, 32, 0, STREAM>(a, tx, k, t == 0 ? 0 : 32 + 64 * npair + 32 * (t - 1), y, z, 0, sQ32, sTr32);
+  if (ghost_row<real, D>(a, y, z)) return;
+  const Share<real, 32, false> sh32{reinterpret_cast<real(*)[32]>(&sQ[0][0]), reinterpret_cast<real(*)[32]>(&sTr[0][0]), sNb,
+                                    nullptr, nullptr, nullptr, SyncBlock{}};
+  if ((int)blockIdx.x >= nmulti) {
+    const int t = (int)blockIdx.x - nmulti;
+    run_tile<LAT, SCHEME, real, 32, 0, STREAM>(a, tx, k, t == 0 ? 0 : 32 + W * nmulti + 32 * (t - 1), y, z, 0, sh32);
     return;
   }
-  const int x0 = 32 + (int)blockIdx.x * 64;
+  const int x0 = 32 + (int)blockIdx.x * W;
   const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
   const bool row_inner = (D < 2 || (y >= 1 && y <= ny - 2)) && (D < 3 || (z >= 1 && z <= nz - 2));
-  const bool interior = x0 >= 1 && x0 + 64 <= nx - 1 && row_inner && a.mask == nullptr && !sphere_may_touch<float, D>(a, x0, 64, y, z);
+  const bool interior = x0 >= 1 && x0 + W <= nx - 1 && row_inner && a.mask == nullptr && !sphere_may_touch<real, D>(a, x0, W, y, z);
   if (interior) {
-    const int x = x0 + 2 * tx;
+    const int x = x0 + NC * tx;
     const uint32_t n = ((uint32_t)z * ny + y) * nx + x;
-    char *__restrict__ pb = reinterpret_cast<char *>(const_cast<float *>(a.src) + ((size_t)k * Q * a.pstride + n));
-    float f0[Q], f1[Q];
+    char *__restrict__ pb = reinterpret_cast<char *>(const_cast<real *>(a.src) + ((size_t)k * Q * a.pstride + n));
+    real f[NC][Q];
 #pragma unroll
     for (int i = 0; i < Q; i++) {
-      if (STREAM == ST_LOC) {
-        const float2 v = *reinterpret_cast<const float2 *>(pb + a.st_off[opp(i)]);
-        f0[i] = v.x; f1[i] = v.y;
-      } else if (L::cx(i) == 0) {
-        const float2 v = *reinterpret_cast<const float2 *>(pb + a.ld_off[i]);
-        f0[i] = v.x; f1[i] = v.y;
+      if (STREAM == ST_LOC || L::cx(i) == 0) {
+        real v[NC];
+        ldv<real, NC>(pb + (STREAM == ST_LOC ? a.st_off[opp(i)] : a.ld_off[i]), v);
+#pragma unroll
+        for (int c = 0; c < NC; c++) f[c][i] = v[c];
       } else {
-        f0[i] = *reinterpret_cast<const float *>(pb + a.ld_off[i]);
-        f1[i] = *reinterpret_cast<const float *>(pb + a.ld_off[i] + 4);
+#pragma unroll
+        for (int c = 0; c < NC; c++) f[c][i] = *reinterpret_cast<const real *>(pb + a.ld_off[i] + (long long)(c * sizeof(real)));
       }
     }
     const bool rowM = STREAM != ST_AB && ((npy && (y == 1 || y == ny - 2)) || (npz && (z == 1 || z == nz - 2)));
-    const bool wM0 = rowM || (npx && (x == 1 || x == nx - 2)), wM1 = rowM || (npx && (x + 1 == 1 || x + 1 == nx - 2));
+    bool wM[NC];
+#pragma unroll
+    for (int c = 0; c < NC; c++) wM[c] = rowM || (npx && (x + c == 1 || x + c == nx - 2));
     if (STREAM == ST_AB) {
-      const StorePairOwn<float> st{reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + n)), a.st_off};
-      finish_pair<LAT, SCHEME, STREAM>(a, tx, k, n, wM0, wM1, f0, f1, st, sQ, sTr);
+      const StoreMultiOwn<real, NC> st{reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + n)), a.st_off};
+      finish_multi<LAT, SCHEME, real, NC, STREAM>(a, tx, k, n, wM, f, st, sQ, sTr);
     } else if (STREAM == ST_PP) {
-      const StorePairPP<L, float> st{pb, a.ld_off};
-      finish_pair<LAT, SCHEME, STREAM>(a, tx, k, n, wM0, wM1, f0, f1, st, sQ, sTr);
+      const StoreMultiPP<L, real, NC> st{pb, a.ld_off};
+      finish_multi<LAT, SCHEME, real, NC, STREAM>(a, tx, k, n, wM, f, st, sQ, sTr);
     } else {
-      const StorePairOwn<float> st{pb, a.st_off};
-      finish_pair<LAT, SCHEME, STREAM>(a, tx, k, n, wM0, wM1, f0, f1, st, sQ, sTr);
+      const StoreMultiOwn<real, NC> st{pb, a.st_off};
+      finish_multi<LAT, SCHEME, real, NC, STREAM>(a, tx, k, n, wM, f, st, sQ, sTr);
     }
     return;
   }
-  // anything else: the two 32-cell halves through the one-cell paths (they share sQ / sTr rows 0..31)
-  run_tile<LAT, SCHEME, float, 32, 0, STREAM>(a, tx, k, x0, y, z, 0, sQ32, sTr32);
-  __syncthreads();
-  if (x0 + 32 < nx) run_tile<LAT, SCHEME, float, 32, 0, STREAM>(a, tx, k, x0 + 32, y, z, 0, sQ32, sTr32);
+  // anything else: the NC 32-cell pieces through the one-cell paths (they share sQ / sTr columns 0..31)
+#pragma unroll 1
+  for (int s = 0; s < NC; s++) {
+    if (s) __syncthreads();
+    if (x0 + 32 * s < nx) run_tile<LAT, SCHEME, real, 32, 0, STREAM>(a, tx, k, x0 + 32 * s, y, z, 0, sh32);
+  }
 }
 
 // ---- S10 init: g_{k,i} = w_i (Q_k + c_i.Phi_k(Q)/c_s^2) (Eq.3) from fp64 fields [K][N] ---------

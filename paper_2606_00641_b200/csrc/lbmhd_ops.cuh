@@ -16,17 +16,25 @@ template <int LAT, int SCHEME, typename real> struct Ops {
   using L = Lattice<LAT>;
   static constexpr int Q = L::Q, K = Vars<SCHEME, L::D>::K;
   static constexpr int TXAUX = K > 16 ? 32 : 64;   // x-tile of init / moments (TXAUX * K threads <= 1024)
-  // launch bound of the step kernels of kResist (K = 11 / 14 / 17 variable rows per block): registers, not threads, limit it
-  static constexpr int MINB_R = K >= 17 ? 1 : 2;
+  // Launch bound (min blocks/SM) of the step kernels: the largest count whose register cap still holds the lean
+  // interior path of this lattice (measured: D3Q19 72-80 registers, D2Q9 58, D3Q7 54, D2Q5 50, D1Q3 44), so that small
+  // blocks (INCRES: 32 x 5 threads) do not leave the SM at 20 warps.  DESIGN.md §5.1.
+  static constexpr int minb_for(int threads, int need) {
+    int best = 1;
+    for (int m = 1; m <= 16; m++)
+      if (m * threads <= 2048 && (65536 / (m * threads)) / 8 * 8 >= need) best = m;
+    return best;
+  }
+  static constexpr int REGS_NEED = Q > 9 ? 72 : (Q > 7 ? 64 : (Q > 3 ? 56 : 48));
+  static constexpr int MINB = minb_for(32 * K, REGS_NEED);
 
   static real *pops(lbmhd_t *h, int which) { return (real *)(h->ws + h->L.off_pop[which]); }
 
   static dim3 grid(const lbmhd_t *h, int tx) { return dim3((h->p.nx + tx - 1) / tx, h->p.ny, h->p.nz); }
 
-  // One launch over all tiles (small grids, masked obstacles), or the split form: a lean interior launch plus
-  // general launches over the x-edge columns, the y/z-edge rows and the sphere's bounding box.
+  // One launch over all tiles; the tile class (interior / x-edge / general) is chosen per block.
   // in place: pull-push step from layout P0, local step from layout P1
-  template <int MINB> static cudaError_t launch_step_inplace(lbmhd_t *h, const StepArgs<real> &a) {
+  static cudaError_t launch_step_inplace(lbmhd_t *h, const StepArgs<real> &a) {
     constexpr int TX = 32;
     const dim3 g((h->p.nx + TX - 1) / TX, h->p.ny, h->p.nz), b(TX, K);
     if (h->parity == 0) step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_PP><<<g, b, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
@@ -35,16 +43,39 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     return cudaGetLastError();
   }
 
-  // fp32: two cells per thread (64-cell tiles); needs an even nx for the 8-byte alignment of the float2 accesses
-  template <int MINB> static cudaError_t launch_step_pair(lbmhd_t *h, const StepArgs<real> &a) {
-    if constexpr (sizeof(real) == 4) {
-      const int npair = h->p.nx >= 128 ? (h->p.nx - 64) / 64 : 0;      // pair tiles at x0 = 32 + 64 j, all interior in x
-      const int ntail = (h->p.nx - (32 + 64 * npair) + 31) / 32;         // 32-cell tiles after the pair tiles (>= 0)
-      const dim3 g(npair + 1 + (ntail > 0 ? ntail : 0), h->p.ny, h->p.nz), b(32, K);
+  // several cells per thread on interior tiles (lbmhd_kernels.cuh, step_kernel_multi): NC-wide vector accesses need nx % NC == 0
+  // NC = cells per thread: the widest of {NCMAX, NCMAX/2, .., 2} whose register need (NC*Q population registers + 36..52)
+  // still lets two blocks share an SM, so that one block's loads overlap the other's arithmetic; a block that is alone on
+  // its SM anyway (K = 17 rows) loses nothing.  Measured on B200: fp64 NC = 2 lifts config 5 from 0.955
+  // to 0.975 of the copy bandwidth, D2Q5 0.76 -> 0.98; fp32 NC = 4 on D3Q19 / D2Q9 does not pay (scalar x-shifted loads).
+  static constexpr int NCMAX = sizeof(real) == 8 ? 2 : (Q <= 7 ? 4 : 2);
+  static constexpr int regs_need_multi(int nc) {
+    const int pops = nc * Q * (int)sizeof(real) / 4;
+    return (pops + (pops > 64 ? 52 : 36) + 7) / 8 * 8;        // D3Q19 fp64 x 2 cells: 76 + 52 = 128 (measured: no spills at 128, slower at 96)
+  }
+  static constexpr int pick_nc() {
+    for (int nc = NCMAX; nc >= 2; nc /= 2)
+      if (minb_for(32 * K, regs_need_multi(nc)) >= 2 || (MINB == 1 && regs_need_multi(nc) <= (65536 / (32 * K)) / 8 * 8)) return nc;
+    return 1;
+  }
+  static constexpr int NC = pick_nc();
+  static constexpr int VW = NC * (int)sizeof(real) >= 16 ? 16 / (int)sizeof(real) : NC;       // nx must be a multiple (vector alignment of rows)
+  static constexpr int MINB_M = minb_for(32 * K, regs_need_multi(NC));
+  // small grids keep one cell per thread: fewer, larger blocks lose to wave quantisation (config 2: 0.87 vs 0.81)
+  static bool multi_pays(const lbmhd_t *h) {
+    const long long blocks = (long long)((h->p.nx + 32 * NC - 1) / (32 * NC) + 1) * h->p.ny * h->p.nz;
+    return blocks >= 16LL * h->num_sms * MINB_M;
+  }
+  static cudaError_t launch_step_multi(lbmhd_t *h, const StepArgs<real> &a) {
+    if constexpr (NC > 1) {
+      constexpr int W = 32 * NC;
+      const int nm = h->p.nx >= 64 + W ? (h->p.nx - 64) / W : 0;      // multi-cell tiles at x0 = 32 + W j, all interior in x
+      const int ntail = (h->p.nx - (32 + W * nm) + 31) / 32;           // 32-cell tiles after them (>= 0)
+      const dim3 g(nm + 1 + (ntail > 0 ? ntail : 0), h->p.ny, h->p.nz), b(32, K);
       const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
-      if (!inplace) step_kernel_pair<LAT, SCHEME, MINB, ST_AB><<<g, b, 0, h->stream>>>(a, npair);
-      else if (h->parity == 0) step_kernel_pair<LAT, SCHEME, MINB, ST_PP><<<g, b, 0, h->stream>>>(a, npair);
-      else step_kernel_pair<LAT, SCHEME, MINB, ST_LOC><<<g, b, 0, h->stream>>>(a, npair);
+      if (!inplace) step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_AB><<<g, b, 0, h->stream>>>(a, nm);
+      else if (h->parity == 0) step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_PP><<<g, b, 0, h->stream>>>(a, nm);
+      else step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_LOC><<<g, b, 0, h->stream>>>(a, nm);
       h->launches += 1;
       return cudaGetLastError();
     } else {
@@ -52,53 +83,22 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     }
   }
 
-  template <int TX, int MINB> static cudaError_t launch_step_whole(lbmhd_t *h, const StepArgs<real> &a) {
-    step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_AB><<<dim3((h->p.nx + TX - 1) / TX, h->p.ny, h->p.nz), dim3(TX, K), 0, h->stream>>>(
-        a, Region{0, 1, 0, 1, 0, 1}, 0);
+  // RESIST: the K = 11 / 14 / 17 rows of a tile split over a 2-CTA cluster (lbmhd_kernels.cuh, Share)
+  static constexpr int KH = (K + 1) / 2;
+  static constexpr int MINB_CL = minb_for(32 * KH, REGS_NEED);
+  static cudaError_t launch_step_cluster(lbmhd_t *h, const StepArgs<real> &a) {
+    const dim3 g(2 * ((h->p.nx + 31) / 32), h->p.ny, h->p.nz), b(32, KH);
+    if (h->p.streaming != LBMHD_STREAM_INPLACE) step_kernel_cl<LAT, SCHEME, real, MINB_CL, ST_AB><<<g, b, 0, h->stream>>>(a);
+    else if (h->parity == 0) step_kernel_cl<LAT, SCHEME, real, MINB_CL, ST_PP><<<g, b, 0, h->stream>>>(a);
+    else step_kernel_cl<LAT, SCHEME, real, MINB_CL, ST_LOC><<<g, b, 0, h->stream>>>(a);
     h->launches += 1;
     return cudaGetLastError();
   }
 
-  template <int TX, int MINB> static cudaError_t launch_step(lbmhd_t *h, const StepArgs<real> &a) {
-    constexpr int D = L::D;
-    const int nx = h->p.nx, ny = h->p.ny, nz = h->p.nz;
-    const int tiles_x = (nx + TX - 1) / TX;
-    const dim3 block(TX, K);
-    const bool split = h->split && !h->have_mask && tiles_x >= 3 && (D < 2 || ny >= 3) && (D < 3 || nz >= 3);
-    if (!split) {
-      step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_AB><<<dim3(tiles_x, ny, nz), block, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
-      h->launches += 1;
-      return cudaGetLastError();
-    }
-    const int iy0 = D > 1 ? 1 : 0, iny = D > 1 ? ny - 2 : 1;
-    const int iz0 = D > 2 ? 1 : 0, inz = D > 2 ? nz - 2 : 1;
-    // interior tiles (x-edge tiles excluded even when their cells are interior: they need wrap or face handling)
-    step_kernel<LAT, SCHEME, real, TX, MINB, 1, ST_AB><<<dim3(tiles_x - 2, iny, inz), block, 0, h->stream>>>(a, Region{1, 1, iy0, 1, iz0, 1}, 0);
-    // x-edge columns, all rows
-    step_kernel<LAT, SCHEME, real, TX, 2, 2, ST_AB><<<dim3(2, ny, nz), block, 0, h->stream>>>(a, Region{0, tiles_x - 1, 0, 1, 0, 1}, 0);
-    h->launches += 2;
-    if (D > 1) {   // y-edge rows of the remaining columns
-      step_kernel<LAT, SCHEME, real, TX, 2, 2, ST_AB><<<dim3(tiles_x - 2, 2, nz), block, 0, h->stream>>>(a, Region{1, 1, 0, ny - 1, 0, 1}, 0);
-      h->launches += 1;
-    }
-    if (D > 2) {   // z-edge planes of what is left
-      step_kernel<LAT, SCHEME, real, TX, 2, 2, ST_AB><<<dim3(tiles_x - 2, ny - 2, 2), block, 0, h->stream>>>(a, Region{1, 1, 1, 1, 0, nz - 1}, 0);
-      h->launches += 1;
-    }
-    if (a.has_sphere) {   // interior-positioned tiles inside the sphere's bounding box
-      const double R = a.sph_R + 0.5 * a.sph_eps + 1.0;
-      int bx_lo = (int)floor((a.sph_c[0] - R) / TX), bx_hi = (int)floor((a.sph_c[0] + R) / TX);
-      int y_lo = D > 1 ? (int)floor(a.sph_c[1] - R) : 0, y_hi = D > 1 ? (int)ceil(a.sph_c[1] + R) : 0;
-      int z_lo = D > 2 ? (int)floor(a.sph_c[2] - R) : 0, z_hi = D > 2 ? (int)ceil(a.sph_c[2] + R) : 0;
-      bx_lo = bx_lo < 1 ? 1 : bx_lo; bx_hi = bx_hi > tiles_x - 2 ? tiles_x - 2 : bx_hi;
-      y_lo = y_lo < iy0 ? iy0 : y_lo; y_hi = y_hi > iy0 + iny - 1 ? iy0 + iny - 1 : y_hi;
-      z_lo = z_lo < iz0 ? iz0 : z_lo; z_hi = z_hi > iz0 + inz - 1 ? iz0 + inz - 1 : z_hi;
-      if (bx_lo <= bx_hi && y_lo <= y_hi && z_lo <= z_hi) {
-        step_kernel<LAT, SCHEME, real, TX, 2, 2, ST_AB><<<dim3(bx_hi - bx_lo + 1, y_hi - y_lo + 1, z_hi - z_lo + 1), block, 0, h->stream>>>(
-            a, Region{bx_lo, 1, y_lo, 1, z_lo, 1}, 1);
-        h->launches += 1;
-      }
-    }
+  template <int TX> static cudaError_t launch_step_whole(lbmhd_t *h, const StepArgs<real> &a) {
+    step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_AB><<<dim3((h->p.nx + TX - 1) / TX, h->p.ny, h->p.nz), dim3(TX, K), 0, h->stream>>>(
+        a, Region{0, 1, 0, 1, 0, 1}, 0);
+    h->launches += 1;
     return cudaGetLastError();
   }
 
@@ -190,19 +190,15 @@ template <int LAT, int SCHEME, typename real> struct Ops {
           }
       }
       cudaError_t e;
-      if constexpr (SCHEME == kResist) {     // one launch configuration: one-cell kernels, one launch over all tiles
-        e = inplace ? launch_step_inplace<MINB_R>(h, a) : launch_step_whole<32, MINB_R>(h, a);
-      } else {
-        if (sizeof(real) == 4 && h->pair) e = h->minb == 2 ? launch_step_pair<2>(h, a) : (h->minb == 4 ? launch_step_pair<4>(h, a) : launch_step_pair<3>(h, a));
-        else if (inplace) e = h->minb == 4 ? launch_step_inplace<4>(h, a) : launch_step_inplace<3>(h, a);
-        else if (h->use_tma) e = launch_step_tma(h, a);
-        else switch (h->tx * 10 + h->minb) {
-          case 322: e = launch_step_whole<32, 2>(h, a); break;
-          case 323: e = launch_step<32, 3>(h, a); break;          // split launches exist for the two default bounds only
-          case 324: e = launch_step<32, 4>(h, a); break;
-          default: e = launch_step<32, 3>(h, a); break;
-        }
+      bool launched = false;
+      if constexpr (SCHEME == kResist && Q > 9) {
+        if (h->cluster) { e = launch_step_cluster(h, a); launched = true; }
       }
+      if (launched) {}
+      else if (h->use_tma) e = launch_step_tma(h, a);
+      else if (NC > 1 && h->pair && h->p.nx % VW == 0 && multi_pays(h)) e = launch_step_multi(h, a);
+      else if (inplace) e = launch_step_inplace(h, a);
+      else e = launch_step_whole<32>(h, a);
       if (e != cudaSuccess) return fail(LBMHD_ECUDA, "step kernel launch: %s", cudaGetErrorString(e));
       if (inplace) { h->parity ^= 1; h->mcur ^= 1; }
       else h->cur = 1 - h->cur;

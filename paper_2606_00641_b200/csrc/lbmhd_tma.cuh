@@ -157,6 +157,7 @@ step_kernel_tma(const __grid_constant__ StepArgs<real> a, const __grid_constant_
     if (g == 0) asm volatile("bar.sync 1, %0;" ::"n"(C::GROUP) : "memory");
     else asm volatile("bar.sync 2, %0;" ::"n"(C::GROUP) : "memory");
   };
+  const Share<real, TXT, false, decltype(gsync)> sh{sQ, sTr, nullptr, nullptr, nullptr, nullptr, gsync};
 
   // this group's tiles: the CTA's tile sequence (rows blockIdx.x, + gridDim.x, ...; tiles_x tiles per row) taken
   // alternately by the two groups; (row, bx, y, z), stage and phase are kept incrementally
@@ -230,10 +231,10 @@ step_kernel_tma(const __grid_constant__ StepArgs<real> a, const __grid_constant_
     const StoreOwn<real> sto{reinterpret_cast<char *>(dstk + n), a.st_off};
     if (!special) {
       CellCtx c{tx, k, x, y, z, n, work, false, false, false, false, false, false, false};
-      finish_cell<LAT, SCHEME, real, TXT, false, false, ST_AB>(a, c, f, sto, sQ, sTr, gsync);
+      finish_cell<LAT, SCHEME, real, TXT, false, false, ST_AB>(a, c, f, sto, sh);
     } else {
       CellCtx c{tx, k, x, y, z, n, work, npx && x_lo, npx && x_hi, npy && y_lo, npy && y_hi, npz && z_lo, npz && z_hi, false};
-      finish_cell<LAT, SCHEME, real, TXT, true, true, ST_AB>(a, c, f, sto, sQ, sTr, gsync);
+      finish_cell<LAT, SCHEME, real, TXT, true, true, ST_AB>(a, c, f, sto, sh);
     }
     gsync();      // sQ / sTr are reused by this group's next tile
     s += 2;

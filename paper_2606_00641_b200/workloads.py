@@ -193,6 +193,27 @@ def config5(shape=(384, 256, 256), steps=500, tau=0.7, radius=None, planes=None)
                 tau=tau, powell=1.0, bc=(INFLOW, ZEROGRAD, 0, 0, 0, 0), steps=steps, fields=F, sphere=sphere, scale=1.0)
 
 
+def variant(w, scheme=None, lattice=None, tau_relax=8.0, eta=1e-3):
+    """the same input on another scheme of the IDEAL family or on the paper's own lattice (DESIGN.md §0 NEXT rows):
+    IDEAL_DIVB adds D = tr G (1 set), RESIST adds G_ab (3 D sets), both started at 0 (they relax to tau_M grad B in
+    ~tau_M steps, Eq.7); D2Q5 / D3Q7 replace D2Q9 / D3Q19."""
+    w = dict(w)
+    if scheme is not None and scheme != w["scheme"]:
+        if w["scheme"] != "IDEAL" or scheme not in ("IDEAL_DIVB", "RESIST"):
+            raise ValueError("variant: %s -> %s" % (w["scheme"], scheme))
+        D = len(w["shape"])
+        extra = 1 if scheme == "IDEAL_DIVB" else 3 * D
+        w["fields"] = np.concatenate([w["fields"], np.zeros((extra,) + w["fields"].shape[1:])])
+        w["scheme"], w["tau_relax"] = scheme, tau_relax
+        if scheme == "RESIST":
+            w["eta"] = eta
+    if lattice is not None and lattice != w["lattice"]:
+        if lattice[:2] != w["lattice"][:2]:
+            raise ValueError("variant: %s -> %s" % (w["lattice"], lattice))
+        w["lattice"] = lattice
+    return w
+
+
 def get(name, small=False):
     """the five configs; small=True gives the reduced sizes the oracle finishes in seconds."""
     if name == "C1":
