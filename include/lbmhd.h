@@ -190,6 +190,13 @@ int lbmhd_set_populations(lbmhd_t *h, const double *g_in, int on_device);
 long long lbmhd_steps_done(const lbmhd_t *h);
 long long lbmhd_launch_count(const lbmhd_t *h);
 
+/* Which step kernel the last lbmhd_step launch used: LBMHD_PATH_ONE one cell per thread, LBMHD_PATH_MULTI
+ * several cells per thread on interior tiles, LBMHD_PATH_CLUSTER variable rows split over a 2-CTA cluster, LBMHD_PATH_TMA
+ * the TMA-staged persistent kernel; -1 before the first step or for a NULL handle.  The choice is made per lattice,
+ * scheme, precision and grid size; every path computes the same update. */
+enum { LBMHD_PATH_ONE = 0, LBMHD_PATH_MULTI = 1, LBMHD_PATH_CLUSTER = 2, LBMHD_PATH_TMA = 3 };
+int lbmhd_step_path(const lbmhd_t *h);
+
 /* Measured-bandwidth probe (BabelStream-style copy b[i] = a[i] over n fp64 elements, the paper's roofline
  * denominator is such a measurement).  a, b DEVICE pointers; enqueues `reps` launches. */
 int lbmhd_copy_probe(const double *a, double *b, size_t n, int reps, void *stream);

@@ -135,6 +135,7 @@ void lbmhd_destroy(lbmhd_t *h) { delete h; }
 
 long long lbmhd_steps_done(const lbmhd_t *h) { return h ? h->t : -1; }
 long long lbmhd_launch_count(const lbmhd_t *h) { return h ? h->launches : -1; }
+int lbmhd_step_path(const lbmhd_t *h) { return h ? h->last_path : -1; }
 
 int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t **out) {
   if (!out) return fail(LBMHD_EINVAL, "out is NULL");
@@ -196,8 +197,11 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     h->num_sms = sms;
     h->pair = p->eta_jc == 0.0;      // several cells per thread where the lattice has a multi-cell kernel; eta(j): one-cell kernels
     if (const char *e3 = getenv("LBMHD_PAIR")) h->pair = h->pair && atoi(e3) != 0;
-    h->cluster = p->scheme == LBMHD_RESIST && g.Q > 9;      // measured: pays on D3Q19 only
+    h->cluster = p->scheme == LBMHD_RESIST && g.Q > 9 && p->precision == 64;      // measured: pays there only
     if (const char *e4 = getenv("LBMHD_CLUSTER")) h->cluster = h->cluster && atoi(e4) != 0;
+    h->last_path = -1;
+    h->multi_force = false;
+    if (const char *e5 = getenv("LBMHD_MULTI")) h->multi_force = atoi(e5) != 0;
     const char *path = getenv("LBMHD_PATH");      // tuning knob: "plain" forces the register-pull kernel
     const size_t es = p->precision == 64 ? 8 : 4;
     const long long tiles = (long long)((p->nx + kTmaTX - 1) / kTmaTX) * p->ny * p->nz;

@@ -48,6 +48,7 @@ struct lbmhd {
   int mcur;              // in place: which M array holds the moments published by the last step
   long long t;           // steps done since init
   long long launches;
+  int last_path;         // LBMHD_PATH_* of the last step launch, -1 before the first
   bool have_mask, have_bsolid, have_dfield;
   bool body_on;          // body integrals accumulate during the steps
   double body_ref[3];
@@ -58,7 +59,8 @@ struct lbmhd {
   double dip_off[4][3], dip_m[4][3], dip_Bs[4], dip_core[4];
   double obs_om[3], obs_c[3];   // rigid rotation of masked bodies
   long long sph_t0;
-  bool cluster;          // RESIST: variable rows of a tile split over a 2-CTA cluster; LBMHD_CLUSTER=0 turns it off
+  bool multi_force;      // LBMHD_MULTI=1: take the multi-cell kernel on small grids too (tests)
+  bool cluster;          // RESIST on D3Q19, fp64: variable rows of a tile split over a 2-CTA cluster; LBMHD_CLUSTER=0 turns it off
   bool pair;             // several cells per thread on interior tiles (fp32; fp64 on the short lattices); LBMHD_PAIR=0 turns it off
   bool use_tma;          // TMA-staged persistent step kernel (needs nx * sizeof(real) % 16 == 0)
   int num_sms;

@@ -399,12 +399,13 @@ __device__ __forceinline__ void frozen_rematerialise(const StepArgs<real> &a, in
 // What the blend hands over at a cell with d < 1, summed over the body and accumulated over steps:
 //   [0..2] F = -sum dQh_m | [3..5] T = -sum r x dQh_m | [6] W = -sum dQh_E | [7..9] sum dQh_B |
 //   [10..12] sum (1-d) B | [13] sum (1-d).
-// Thread (cell, k) owns dQh_k; k is warp-uniform, so the slots are: the lanes that are here reduce their values
+// Thread (cell, k) owns dQh_k; k and so the slots are uniform over the lanes of a group: they reduce their values
 // and one lane adds to the accumulator (solid cells are 0.2 % of config 5; fluid tiles never get here).
 // One out-of-line copy for every kernel: the lanes that are here reduce up to three values and one lane adds them.
 static __device__ __noinline__ void body_add(double *body, bool solid, int s0, double v0, int s1, double v1, int s2, double v2) {
   namespace cg = cooperative_groups;
-  const cg::coalesced_group g = cg::coalesced_threads();
+  // the lanes that are here, grouped by slot: with 16-cell tiles a warp holds two variables (two slot sets)
+  const cg::coalesced_group g = cg::labeled_partition(cg::coalesced_threads(), s0);
   if (!g.any(solid)) return;
   if (!solid) v0 = v1 = v2 = 0.0;
   const double t0 = cg::reduce(g, v0, cg::plus<double>());

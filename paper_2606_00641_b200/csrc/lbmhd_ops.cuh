@@ -33,12 +33,14 @@ template <int LAT, int SCHEME, typename real> struct Ops {
   static dim3 grid(const lbmhd_t *h, int tx) { return dim3((h->p.nx + tx - 1) / tx, h->p.ny, h->p.nz); }
 
   // One launch over all tiles; the tile class (interior / x-edge / general) is chosen per block.
-  // in place: pull-push step from layout P0, local step from layout P1
-  static cudaError_t launch_step_inplace(lbmhd_t *h, const StepArgs<real> &a) {
+  // One cell per thread: A/B, or in place the pull-push step from layout P0 and the local step from P1.
+  static cudaError_t launch_step_one(lbmhd_t *h, const StepArgs<real> &a) {
     constexpr int TX = 32;
     const dim3 g((h->p.nx + TX - 1) / TX, h->p.ny, h->p.nz), b(TX, K);
-    if (h->parity == 0) step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_PP><<<g, b, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
-    else step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_LOC><<<g, b, 0, h->stream>>>(a, Region{0, 1, 0, 1, 0, 1}, 0);
+    const Region all{0, 1, 0, 1, 0, 1};
+    if (h->p.streaming != LBMHD_STREAM_INPLACE) step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_AB><<<g, b, 0, h->stream>>>(a, all, 0);
+    else if (h->parity == 0) step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_PP><<<g, b, 0, h->stream>>>(a, all, 0);
+    else step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_LOC><<<g, b, 0, h->stream>>>(a, all, 0);
     h->launches += 1;
     return cudaGetLastError();
   }
@@ -64,7 +66,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
   // small grids keep one cell per thread: fewer, larger blocks lose to wave quantisation (config 2: 0.87 vs 0.81)
   static bool multi_pays(const lbmhd_t *h) {
     const long long blocks = (long long)((h->p.nx + 32 * NC - 1) / (32 * NC) + 1) * h->p.ny * h->p.nz;
-    return blocks >= 16LL * h->num_sms * MINB_M;
+    return h->multi_force || blocks >= 16LL * h->num_sms * MINB_M;
   }
   static cudaError_t launch_step_multi(lbmhd_t *h, const StepArgs<real> &a) {
     if constexpr (NC > 1) {
@@ -91,13 +93,6 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     if (h->p.streaming != LBMHD_STREAM_INPLACE) step_kernel_cl<LAT, SCHEME, real, MINB_CL, ST_AB><<<g, b, 0, h->stream>>>(a);
     else if (h->parity == 0) step_kernel_cl<LAT, SCHEME, real, MINB_CL, ST_PP><<<g, b, 0, h->stream>>>(a);
     else step_kernel_cl<LAT, SCHEME, real, MINB_CL, ST_LOC><<<g, b, 0, h->stream>>>(a);
-    h->launches += 1;
-    return cudaGetLastError();
-  }
-
-  template <int TX> static cudaError_t launch_step_whole(lbmhd_t *h, const StepArgs<real> &a) {
-    step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_AB><<<dim3((h->p.nx + TX - 1) / TX, h->p.ny, h->p.nz), dim3(TX, K), 0, h->stream>>>(
-        a, Region{0, 1, 0, 1, 0, 1}, 0);
     h->launches += 1;
     return cudaGetLastError();
   }
@@ -191,14 +186,13 @@ template <int LAT, int SCHEME, typename real> struct Ops {
       }
       cudaError_t e;
       bool launched = false;
-      if constexpr (SCHEME == kResist && Q > 9) {
-        if (h->cluster) { e = launch_step_cluster(h, a); launched = true; }
+      if constexpr (SCHEME == kResist && Q > 9 && sizeof(real) == 8) {
+        if (h->cluster) { e = launch_step_cluster(h, a); launched = true; h->last_path = LBMHD_PATH_CLUSTER; }
       }
       if (launched) {}
-      else if (h->use_tma) e = launch_step_tma(h, a);
-      else if (NC > 1 && h->pair && h->p.nx % VW == 0 && multi_pays(h)) e = launch_step_multi(h, a);
-      else if (inplace) e = launch_step_inplace(h, a);
-      else e = launch_step_whole<32>(h, a);
+      else if (h->use_tma) { e = launch_step_tma(h, a); h->last_path = LBMHD_PATH_TMA; }
+      else if (NC > 1 && h->pair && h->p.nx % VW == 0 && multi_pays(h)) { e = launch_step_multi(h, a); h->last_path = LBMHD_PATH_MULTI; }
+      else { e = launch_step_one(h, a); h->last_path = LBMHD_PATH_ONE; }
       if (e != cudaSuccess) return fail(LBMHD_ECUDA, "step kernel launch: %s", cudaGetErrorString(e));
       if (inplace) { h->parity ^= 1; h->mcur ^= 1; }
       else h->cur = 1 - h->cur;

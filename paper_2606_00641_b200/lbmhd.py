@@ -74,6 +74,7 @@ def load_library():
     lib.lbmhd_steps_done.restype = C.c_longlong
     lib.lbmhd_launch_count.argtypes = [C.c_void_p]
     lib.lbmhd_launch_count.restype = C.c_longlong
+    lib.lbmhd_step_path.argtypes = [C.c_void_p]
     lib.lbmhd_set_sphere_dipoles.argtypes = [C.c_void_p, C.c_int, dp, dp, dp, dp]
     lib.lbmhd_set_obstacle_rotation.argtypes = [C.c_void_p, dp, dp]
     lib.lbmhd_body_enable.argtypes = [C.c_void_p, C.c_int, dp]
@@ -89,7 +90,7 @@ EXPORTS = ["lbmhd_num_vars", "lbmhd_num_dirs", "lbmhd_workspace_bytes", "lbmhd_c
            "lbmhd_set_porosity", "lbmhd_set_sphere_width", "lbmhd_set_sphere_rotation", "lbmhd_halo_bytes", "lbmhd_halo_pack",
            "lbmhd_halo_unpack", "lbmhd_get_populations", "lbmhd_set_populations", "lbmhd_steps_done", "lbmhd_launch_count",
            "lbmhd_copy_probe", "lbmhd_last_error", "lbmhd_body_enable", "lbmhd_body_read",
-           "lbmhd_set_sphere_dipoles", "lbmhd_set_obstacle_rotation"]
+           "lbmhd_set_sphere_dipoles", "lbmhd_set_obstacle_rotation", "lbmhd_step_path"]
 
 
 def _check(rc, allow=()):
@@ -305,6 +306,14 @@ class Lbmhd:
     @property
     def launch_count(self):
         return int(self.lib.lbmhd_launch_count(self.h))
+
+    @property
+    def step_path(self):
+        """PATH_ONE / PATH_MULTI / PATH_CLUSTER / PATH_TMA of the last step launch (-1 before the first)"""
+        return int(self.lib.lbmhd_step_path(self.h))
+
+
+PATH_ONE, PATH_MULTI, PATH_CLUSTER, PATH_TMA = 0, 1, 2, 3
 
 
 def from_workload(w, precision=64, device=0, streaming=STREAM_AB):

@@ -49,12 +49,14 @@ def subbox_oracle(w, centre_xyz, nsteps):
     return Q[:, loc[2], loc[1], loc[0]]
 
 
-def run_fullsize(name, samples):
+def run_fullsize(name, samples, streaming=0, path=None):
     from paper_2606_00641_b200 import lbmhd
     w = W.get(name)
-    sim = lbmhd.from_workload(w)
+    sim = lbmhd.from_workload(w, streaming=streaming)
     sim.init(w["fields"])
     sim.step(NSTEPS)
+    if path is not None:        # the kernel bench.py times for this config (large grids take several cells per thread)
+        assert sim.step_path == getattr(lbmhd, path), sim.step_path
     Q, dg = sim.moments()
     assert dg[-1] == 0
     scale = np.abs(Q).reshape(Q.shape[0], -1).max(1)
@@ -79,7 +81,10 @@ def test_config5_fullsize_sampled():
          (383, 0, 0), (0, 255, 255), (128, 128, 128), (127, 128, 128), (128, 152, 128), (128, 153, 128), (152, 128, 128),
          (153, 128, 128), (104, 128, 128), (128, 128, 104), (140, 140, 140), (160, 128, 128), (96, 128, 128)]
     S += [tuple(int(v) for v in (rng.integers(0, 384), rng.integers(0, 256), rng.integers(0, 256))) for _ in range(12)]
-    print("C5 full size, worst sampled error", run_fullsize("C5", S))
+    # seams of the two-cell tiles (x0 = 32 + 64 j, last one ends at 352) and of the thread pairs inside them
+    S += [(32, 77, 33), (33, 77, 33), (95, 77, 33), (96, 77, 33), (97, 200, 100), (351, 200, 100), (352, 200, 100), (223, 1, 254)]
+    print("C5 full size, worst sampled error", run_fullsize("C5", S, path="PATH_MULTI"))
+    print("C5 full size in place, worst sampled error", run_fullsize("C5", S, streaming=1, path="PATH_MULTI"))
 
 
 def test_config4_fullsize_sampled():
@@ -88,7 +93,9 @@ def test_config4_fullsize_sampled():
     S = [(0, 0, 0), (2047, 2047, 0), (0, 2047, 0), (2047, 0, 0), (0, 1000, 0), (1000, 0, 0), (2047, 777, 0), (31, 5, 0), (32, 2046, 0),
          (1024, 1024, 0), (1228, 1024, 0), (1024, 1259, 0), (1200, 1200, 0)]
     S += [(int(rng.integers(0, 2048)), int(rng.integers(0, 2048)), 0) for _ in range(10)]
-    print("C4 full size, worst sampled error", run_fullsize("C4", S))
+    S += [(95, 1024, 0), (96, 1024, 0), (1951, 3, 0), (1952, 3, 0), (2015, 2044, 0), (2016, 2044, 0)]
+    print("C4 full size, worst sampled error", run_fullsize("C4", S, path="PATH_MULTI"))
+    print("C4 full size in place, worst sampled error", run_fullsize("C4", S, streaming=1, path="PATH_MULTI"))
 
 
 def test_config3_and_2_fullsize_sampled():
@@ -96,7 +103,8 @@ def test_config3_and_2_fullsize_sampled():
     for name, n in (("C3", 1024), ("C2", 512)):
         S = [(0, 0, 0), (n - 1, n - 1, 0), (0, n // 2, 0), (n // 2, n - 1, 0), (31, 31, 0), (32, 32, 0)]
         S += [(int(rng.integers(0, n)), int(rng.integers(0, n)), 0) for _ in range(8)]
-        print(name, "full size, worst sampled error", run_fullsize(name, S))
+        # config 2 is small (8192 tiles): it stays on the one-cell kernel
+        print(name, "full size, worst sampled error", run_fullsize(name, S, path="PATH_MULTI" if name == "C3" else "PATH_ONE"))
 
 
 def test_config1_full_size_all_cells_500_steps():
