@@ -14,7 +14,7 @@ _SRC = os.path.join(_HERE, "vlbm_oracle.c")
 _HDR = os.path.join(_HERE, "vlbm_oracle.h")
 
 D1Q3, D2Q9, D3Q19, D2Q5, D3Q7 = 1, 2, 3, 4, 5
-IDEAL, INCRES, IDEAL_DIVB, RESIST = 0, 1, 2, 3
+IDEAL, INCRES, IDEAL_DIVB, RESIST, FULL = 0, 1, 2, 3, 4
 BC_PERIODIC, BC_ZEROGRAD, BC_INFLOW = 0, 1, 2
 CELL_FLUID, CELL_FROZEN, CELL_SOLID = 0, 1, 2
 

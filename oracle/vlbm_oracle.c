@@ -23,7 +23,7 @@
 #include <omp.h>
 #endif
 
-#define MAXK 17
+#define MAXK 26
 #define MAXDIP 4
 #define NBODY 14          /* body integrals, oracle_body_read */
 #define ACCW (MAXK + NBODY) /* per-row accumulator: source log | body integrals */
@@ -92,12 +92,13 @@ int oracle_lattice(int lattice, int *D, int *Q, int *c, double *w, double *cs2)
   return 0;
 }
 
-static int is_ideal(int scheme) { return scheme == ORC_IDEAL || scheme == ORC_IDEAL_DIVB || scheme == ORC_RESIST; }   /* first 8 variables (rho, m, E, B) */
+static int is_ideal(int scheme) { return scheme == ORC_IDEAL || scheme == ORC_IDEAL_DIVB || scheme == ORC_RESIST || scheme == ORC_FULL; }   /* first 8 variables (rho, m, E, B) */
 static int num_vars(int scheme, int D)
 {
   if (scheme == ORC_IDEAL) return 8;
   if (scheme == ORC_IDEAL_DIVB) return 9;
   if (scheme == ORC_RESIST) return 8 + 3 * D;       /* + G_ab = tau_M d_a B_b, a < D, b < 3, index 8 + 3 a + b */
+  if (scheme == ORC_FULL) return 8 + 6 * D;         /* + H_ab = tau_M d_a u_b, index 8 + 3 D + 3 a + b */
   return 1 + 2 * D;
 }
 
@@ -152,7 +153,7 @@ static void flux_eval(const oracle_params *prm, int D, const double *Q, double P
       /* Eq.10 PAPER.md:136 traced: the relaxation variable D = tr G has the flux D u - B */
       if (scheme == ORC_IDEAL_DIVB) Phi[8][a] = Q[8] * u[a] - B[a];
     }
-    if (scheme == ORC_RESIST) {
+    if (scheme == ORC_RESIST || scheme == ORC_FULL) {
       /* dissipative system, PAPER.md:122 with the transported gradients of Eq.9-10 PAPER.md:132-136 (A22):
        *   g_cb = G_cb / tau_M ~ d_c B_b;  current j = curl B: j_e = eps_ecb g_cb (c < D);
        *   Phi_{B_b},a -= eta g_ab;  Phi_E,a += eta (j x B)_a;  Phi_{G_cb},a = G_cb u_a - delta_ca B_b */
@@ -171,6 +172,25 @@ static void flux_eval(const oracle_params *prm, int D, const double *Q, double P
         Phi[4][a] += eta * jxB[a];
         for (b = 0; b < 3; b++) Phi[5 + b][a] -= eta * g[a][b];
         for (c = 0; c < D; c++) for (b = 0; b < 3; b++) Phi[8 + 3 * c + b][a] = Gv[3 * c + b] * u[a] - (c == a ? B[b] : 0.0);
+      }
+    }
+    if (scheme == ORC_FULL) {
+      /* viscous stress as transported variables (PAPER.md:132 Eq.9, :138 "a similar expansion logic is applied to the viscous
+       * stress tensor"; reading A23): H_cb = tau_M d_c u_b with flux H_cb u_a - delta_ca u_b (Eq.10 with B -> u);
+       *   h = H / tau_M ~ grad u;  sigma_ab = mu (h_ab + h_ba - 2/3 delta_ab tr h)   (Newtonian, mu = prm->nu);
+       *   Phi_{m_b},a -= sigma_ab;  Phi_E,a -= u_b sigma_ab   (the -tau and -u.tau of PAPER.md:122; q = 0) */
+      const double *Hv = Q + 8 + 3 * D;
+      const double mu = prm->nu, itm = 1.0 / prm->tau_relax;
+      double h[3][3], sig[3][3], trh = 0.0;
+      int c;
+      for (c = 0; c < 3; c++) for (b = 0; b < 3; b++) h[c][b] = c < D ? Hv[3 * c + b] * itm : 0.0;
+      for (c = 0; c < 3; c++) trh += h[c][c];
+      for (c = 0; c < 3; c++) for (b = 0; b < 3; b++) sig[c][b] = mu * (h[c][b] + h[b][c] - (c == b ? 2.0 / 3.0 * trh : 0.0));
+      for (a = 0; a < D; a++) {
+        double us = 0.0;
+        for (b = 0; b < 3; b++) { Phi[1 + b][a] -= sig[a][b]; us += u[b] * sig[a][b]; }
+        Phi[4][a] -= us;
+        for (c = 0; c < D; c++) for (b = 0; b < 3; b++) Phi[8 + 3 * D + 3 * c + b][a] = Hv[3 * c + b] * u[a] - (c == a ? u[b] : 0.0);
       }
     }
   } else {
@@ -283,9 +303,10 @@ int oracle_create(const oracle_params *p, const unsigned char *cell_mask, oracle
   lattice_t L;
   *out = NULL;
   if (lattice_make(p->lattice, &L)) return -1;
-  if (p->scheme != ORC_IDEAL && p->scheme != ORC_INCRES && p->scheme != ORC_IDEAL_DIVB && p->scheme != ORC_RESIST) return -1;
-  if ((p->scheme == ORC_IDEAL_DIVB || p->scheme == ORC_RESIST) && !(p->tau_relax > 0.0)) return -1;
-  if (p->scheme == ORC_RESIST && !(p->eta >= 0.0)) return -1;
+  if (p->scheme != ORC_IDEAL && p->scheme != ORC_INCRES && p->scheme != ORC_IDEAL_DIVB && p->scheme != ORC_RESIST && p->scheme != ORC_FULL) return -1;
+  if ((p->scheme == ORC_IDEAL_DIVB || p->scheme == ORC_RESIST || p->scheme == ORC_FULL) && !(p->tau_relax > 0.0)) return -1;
+  if ((p->scheme == ORC_RESIST || p->scheme == ORC_FULL) && !(p->eta >= 0.0)) return -1;
+  if (p->scheme == ORC_FULL && !(p->nu >= 0.0)) return -1;
   if (p->eta_jc != 0.0 && !(p->scheme == ORC_INCRES && p->eta_jc > 0.0)) return -1;
   if (p->nx < 1 || p->ny < 1 || p->nz < 1) return -1;
   if (L.D < 2 && p->ny != 1) return -1;
@@ -308,12 +329,13 @@ int oracle_create(const oracle_params *p, const unsigned char *cell_mask, oracle
   double tau[MAXK] = { 0 };
   for (int k = 0; k < o->K; k++) tau[k] = p->tau[k];
   /* Eq.5: tau = 1/2 + D / c_s^2 for the sets that carry a physical diffusivity (A3) */
-  if (p->nu > 0.0) {
+  /* FULL carries nu (the shear viscosity mu) in the flux like eta: tau_u stays the stabilisation parameter */
+  if (p->nu > 0.0 && p->scheme != ORC_FULL) {
     for (int b = 0; b < nvec; b++) tau[o->iU + b] = 0.5 + p->nu / L.cs2;
     if (p->scheme == ORC_INCRES) tau[0] = 0.5 + p->nu / L.cs2;
   }
   /* RESIST carries eta in the flux (-eta grad B): tau_B stays the stabilisation parameter */
-  if (p->eta > 0.0 && p->scheme != ORC_RESIST) for (int b = 0; b < nvec; b++) tau[o->iB + b] = 0.5 + p->eta / L.cs2;
+  if (p->eta > 0.0 && p->scheme != ORC_RESIST && p->scheme != ORC_FULL) for (int b = 0; b < nvec; b++) tau[o->iB + b] = 0.5 + p->eta / L.cs2;
   for (int k = 0; k < o->K; k++) {
     if (!(tau[k] > 0.5)) { free(o); return -1; }
     o->omega[k] = 1.0 / tau[k];
@@ -642,7 +664,7 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
   /* IDEAL_DIVB: div B from the relaxation variable instead, D ~ tau_M div B (Eq.7) */
   if (o->p.scheme == ORC_IDEAL_DIVB) delta = Qv[8] / o->p.tau_relax;
   /* RESIST: div B = tr g = sum_a G_aa / tau_M */
-  if (o->p.scheme == ORC_RESIST) {
+  if (o->p.scheme == ORC_RESIST || o->p.scheme == ORC_FULL) {
     delta = 0.0;
     for (a = 0; a < D; a++) delta += Qv[8 + 3 * a + a] / o->p.tau_relax;
   }
@@ -657,7 +679,7 @@ static void cell_update(const oracle_t *o, const double *src, double *dst, int x
     for (b = 0; b < 3; b++) { S[1 + b] = -kd * Qv[5 + b]; S[5 + b] = -kd * u[b]; }
     S[4] = -kd * uBdot;
     if (o->p.scheme == ORC_IDEAL_DIVB) S[8] = -Qv[8] / o->p.tau_relax;      /* relaxation source of Eq.6 */
-    if (o->p.scheme == ORC_RESIST) for (k = 8; k < K; k++) S[k] = -Qv[k] / o->p.tau_relax;
+    if (o->p.scheme == ORC_RESIST || o->p.scheme == ORC_FULL) for (k = 8; k < K; k++) S[k] = -Qv[k] / o->p.tau_relax;
   } else {
     for (b = 0; b < D; b++) { S[1 + b] = -kd * Qv[1 + D + b]; S[1 + D + b] = -kd * Qv[1 + b]; }
   }

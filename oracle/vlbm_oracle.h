@@ -23,7 +23,7 @@ extern "C" {
 #endif
 
 enum { ORC_D1Q3 = 1, ORC_D2Q9 = 2, ORC_D3Q19 = 3, ORC_D2Q5 = 4, ORC_D3Q7 = 5 };
-enum { ORC_IDEAL = 0, ORC_INCRES = 1, ORC_IDEAL_DIVB = 2, ORC_RESIST = 3 };
+enum { ORC_IDEAL = 0, ORC_INCRES = 1, ORC_IDEAL_DIVB = 2, ORC_RESIST = 3, ORC_FULL = 4 };
 enum { ORC_BC_PERIODIC = 0, ORC_BC_ZEROGRAD = 1, ORC_BC_INFLOW = 2 };
 enum { ORC_CELL_FLUID = 0, ORC_CELL_FROZEN = 1, ORC_CELL_SOLID = 2 };
 
@@ -32,15 +32,18 @@ typedef struct {
                       ORC_INCRES: Q = (P, u_1..u_D, B_1..B_D), K = 1 + 2 D                  (A2, A3)
                       ORC_IDEAL_DIVB: IDEAL + D = tr G, K = 9             (A19)
                       ORC_RESIST: IDEAL + G_ab = tau_M d_a B_b (a < D, b < 3; index 8 + 3a + b), K = 8 + 3 D, resistive
-                                  fluxes -eta grad B and eta j x B from G (Eq.9-10)  (A22) */
+                                  fluxes -eta grad B and eta j x B from G (Eq.9-10)  (A22)
+                      ORC_FULL: RESIST + H_ab = tau_M d_a u_b (index 8 + 3 D + 3a + b), K = 8 + 6 D: the full dissipative system of
+                                PAPER.md:122 with the viscous stress -tau, -u.tau from H (Eq.9)          (A23) */
   int lattice;     /* ORC_D1Q3 / D2Q9 / D3Q19 (A2); D2Q5 / D3Q7 are the paper's own */
   int nx, ny, nz;  /* unused dims = 1 */
   double gamma;    /* IDEAL: adiabatic index, Eq.8 */
   double c0sq;     /* INCRES: artificial sound speed squared (A3) */
   double nu, eta;  /* if > 0: tau of the velocity / magnetic sets := 1/2 + D / c_s^2 (Eq.5);
-                      ORC_RESIST: eta is the magnetic diffusivity of the flux terms instead and leaves tau alone */
+                      ORC_RESIST, ORC_FULL: eta is the magnetic diffusivity of the flux terms instead and leaves tau alone;
+                      ORC_FULL: nu is the shear viscosity mu of the flux terms likewise */
   double tau[32];  /* per variable, > 1/2, variable order of `scheme` */
-  double tau_relax; /* IDEAL_DIVB, RESIST: relaxation time tau_M of the gradient variables (Eq.6), lattice units, > 0 */
+  double tau_relax; /* IDEAL_DIVB, RESIST, FULL: relaxation time tau_M of the gradient variables (Eq.6), lattice units, > 0 */
   double eta_jc;   /* INCRES: critical current j_c of eta(j) = eta0 (1 + (j/j_c)^2), lattice units; 0 = constant eta */
   double powell;   /* kappa: 0 = off, 1 = Eq.12 */
   int bc[6];       /* xmin, xmax, ymin, ymax, zmin, zmax */

@@ -100,6 +100,28 @@ def flux_resist(Q, gamma, D, eta, tau_m):
     return Phi
 
 
+def flux_full(Q, gamma, D, eta, mu, tau_m):
+    """full dissipative system of PAPER.md:122 with transported gradients of B and of u (Eq.9; reading A23):
+    Q = (rho, m, E, B, G[a<D][b<3], H[a<D][b<3]), h = H / tau_M ~ grad u, sigma = mu (h + h^T - 2/3 tr h I);
+    Phi_m -= sigma; Phi_E -= u . sigma; Phi_H = H (x) u - I (x) u."""
+    K = 8 + 6 * D
+    tail = Q.shape[1:]
+    Phi = np.zeros((K, 3) + tail)
+    Phi[:8 + 3 * D] = flux_resist(Q[:8 + 3 * D], gamma, D, eta, tau_m)
+    u = Q[1:4] / Q[0]
+    H = np.zeros((3, 3) + tail)
+    H[:D] = Q[8 + 3 * D:].reshape((D, 3) + tail)
+    h = H / tau_m
+    eye = np.eye(3).reshape((3, 3) + (1,) * len(tail))
+    sigma = mu * (h + np.swapaxes(h, 0, 1) - (2.0 / 3.0) * np.einsum("cc...->...", h)[None, None] * eye)      # [a, b]
+    Phi[1:4] -= np.swapaxes(sigma, 0, 1)                         # Phi[1+b, a] -= sigma[a, b]
+    Phi[4] -= np.einsum("b...,ab...->a...", u, sigma)
+    PhiH = H[:, :, None] * u[None, None] - np.einsum("ca,b...->cba...", np.eye(3), u)     # [c, b, a]
+    Phi[8 + 3 * D:] = PhiH[:D].reshape((3 * D, 3) + tail)
+    Phi[:, D:] = 0.0
+    return Phi
+
+
 def flux_incres(Q, c0sq, D):
     """A3. Q: [1+2D, ...] = (P, u, B)."""
     P, u, B = Q[0], Q[1:1 + D], Q[1 + D:1 + 2 * D]
@@ -121,9 +143,10 @@ class NpVLBM:
         self.D, self.c, self.w, self.cs2 = lattice_np(lat)
         self.Qn = len(self.w)
         self.shape = tuple(shape_zyx)
-        self.K = {"IDEAL": 8, "IDEAL_DIVB": 9, "RESIST": 8 + 3 * self.D, "INCRES": 1 + 2 * self.D}[scheme]
-        self.ideal = scheme in ("IDEAL", "IDEAL_DIVB", "RESIST")
-        self.eta = 0.0                 # RESIST: magnetic diffusivity of the flux terms
+        self.K = {"IDEAL": 8, "IDEAL_DIVB": 9, "RESIST": 8 + 3 * self.D, "FULL": 8 + 6 * self.D, "INCRES": 1 + 2 * self.D}[scheme]
+        self.ideal = scheme in ("IDEAL", "IDEAL_DIVB", "RESIST", "FULL")
+        self.eta = 0.0                 # RESIST, FULL: magnetic diffusivity of the flux terms
+        self.mu = 0.0                  # FULL: shear viscosity of the flux terms
         self.tau_relax = tau_relax
         self.eta_jc = eta_jc
         self.tau = np.broadcast_to(np.asarray(tau, dtype=float), (self.K,)).copy()
@@ -154,6 +177,8 @@ class NpVLBM:
             return flux_ideal_divb(Q, self.gamma, self.D)
         if self.scheme == "RESIST":
             return flux_resist(Q, self.gamma, self.D, self.eta, self.tau_relax)
+        if self.scheme == "FULL":
+            return flux_full(Q, self.gamma, self.D, self.eta, self.mu, self.tau_relax)
         return flux_incres(Q, self.c0sq, self.D)
 
     def feq(self, Q, Phi):
@@ -307,7 +332,7 @@ class NpVLBM:
                 t = t - ((t - tau0) * t * t - cc) / (t * (3 * t - 2 * tau0))
             tauB = t
         delta = -tr / (tauB * self.cs2)
-        if self.scheme == "RESIST":
+        if self.scheme in ("RESIST", "FULL"):
             delta = sum(Q[8 + 3 * a + a] for a in range(D)) / self.tau_relax        # div B = tr G / tau_M
         if self.scheme == "IDEAL_DIVB":
             delta = Q[8] / self.tau_relax            # Eq.7: D ~ tau_M div B
@@ -319,7 +344,7 @@ class NpVLBM:
             S[1:4] = -self.kappa * delta * B
             S[4] = -self.kappa * delta * (u * B).sum(0)
             S[5:8] = -self.kappa * delta * u
-            if self.scheme in ("IDEAL_DIVB", "RESIST"):
+            if self.scheme in ("IDEAL_DIVB", "RESIST", "FULL"):
                 S[8:] = -Q[8:] / self.tau_relax      # relaxation source of Eq.6
         else:
             u, B = Q[1:1 + D], Q[1 + D:]
@@ -347,7 +372,7 @@ class NpVLBM:
                 Qh[1 + b] = np.where(sol, d * Q[1 + b] + (1 - d) * uB[b], Q[1 + b])
                 Qh[1 + D + b] = np.where(sol, d * Q[1 + D + b] + (1 - d) * BB[b], Q[1 + D + b])
         dQh = Qh - Q
-        if self.scheme in ("IDEAL_DIVB", "RESIST"):
+        if self.scheme in ("IDEAL_DIVB", "RESIST", "FULL"):
             S[:8] = S[:8] * d
         else:
             S = S * d
