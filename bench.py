@@ -231,7 +231,8 @@ def run_native(args, rank, world, local_rank):
                    "l2": "populations %.1f GB >> 126 MB L2, no flush needed" % (
                        (1 if args.streaming == "inplace" else 2) * N * bytes_per_cell / 2 / 1e9)},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "peak_source": peak_src, "kernel": "step_kernel",
+                     "traffic": traffic, "peak_source": peak_src,
+                     "kernel": {0: "step_kernel", 1: "step_kernel_multi", 2: "step_kernel_cl", 3: "step_kernel_tma"}.get(sim.step_path, "?"),
                      "frac_of_nominal_8TBs": achieved / 8000.0,
                      "own_fp64_copy_GBs": own_copy, "frac_of_own_copy": achieved / own_copy,
                      "paper_context": "98.9% (2D) / 75.8% (3D) of 680 GB/s BabelStream, RTX A5000 fp32 (PAPER.md:269)"},
