@@ -324,8 +324,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
-    ap.add_argument("--scheme", default=None, choices=["IDEAL_DIVB", "RESIST"],
-                    help="run the ideal-MHD workload on a scheme with transported gradient sets (DESIGN.md A19, A22)")
+    ap.add_argument("--scheme", default=None, choices=["IDEAL_DIVB", "RESIST", "FULL"],
+                    help="run the ideal-MHD workload on a scheme with transported gradient sets (DESIGN.md A19, A22, A23)")
     ap.add_argument("--lattice", default=None, choices=["D2Q5", "D3Q7"], help="the paper's own lattice instead of D2Q9 / D3Q19")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--streaming", default="ab", choices=["ab", "inplace"])

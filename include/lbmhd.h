@@ -17,6 +17,7 @@
  *    INCRES: K = 1 + 2D, order P, u_1..u_D, B_1..B_D (P = kinematic pressure carrier, A3).
  *    IDEAL_DIVB: K = 9, the IDEAL order followed by D.
  *    RESIST: K = 8 + 3 D, the IDEAL order followed by G_ab, a-major (variable 8 + 3 a + b).
+ *    FULL: K = 8 + 6 D, the RESIST order followed by H_ab, a-major (variable 8 + 3 D + 3 a + b).
  *  - Direction order: rest; +x,-x,+y,-y,+z,-z; diagonals (+,+),(-,-),(+,-),(-,+) per plane xy, xz, yz.
  *  - Every pointer argument says whether it is a HOST or a DEVICE pointer.  The caller owns every
  *    buffer it passes, including `workspace` (device memory, e.g. a torch tensor): the library never
@@ -45,7 +46,11 @@ enum { LBMHD_IDEAL = 0, LBMHD_INCRES = 1,
        LBMHD_RESIST = 3 /* dissipative MHD with the magnetic gradients transported (Eq.9-10 PAPER.md:132-136;
                            DESIGN.md A22): IDEAL + G_ab ~ tau_relax d_a B_b (a < D lattice axes, b < 3), flux G (x) u - I (x) B,
                            source -G/tau_relax; induction flux - eta G/tau_relax, energy flux + eta j x B with j = curl B
-                           from G; div B in Eq.12 := tr G / tau_relax.  No viscous stress, no heat flux */ };
+                           from G; div B in Eq.12 := tr G / tau_relax.  No viscous stress, no heat flux */,
+       LBMHD_FULL = 4 /* the full dissipative system of PAPER.md:122 (Eq.9; A23): RESIST + the velocity
+                         gradients H_ab ~ tau_relax d_a u_b transported the same way (flux H (x) u - I (x) u, source -H/tau_relax);
+                         Newtonian stress sigma = nu (h + h^T - 2/3 tr h I), h = H/tau_relax, enters the momentum flux as -sigma and
+                         the energy flux as -u.sigma.  Heat flux q = 0 */ };
 enum { LBMHD_BC_PERIODIC = 0, LBMHD_BC_ZEROGRAD = 1, LBMHD_BC_INFLOW = 2,
        LBMHD_BC_HALO = 3 /* slab decomposition, slowest lattice axis only: the plane on this face is a ghost plane */ };
 enum { LBMHD_CELL_FLUID = 0, LBMHD_CELL_FROZEN = 1, LBMHD_CELL_SOLID = 2 };
@@ -59,16 +64,17 @@ enum {
 };
 
 typedef struct {
-  int    scheme;        /* LBMHD_IDEAL | LBMHD_INCRES | LBMHD_IDEAL_DIVB | LBMHD_RESIST */
+  int    scheme;        /* LBMHD_IDEAL | LBMHD_INCRES | LBMHD_IDEAL_DIVB | LBMHD_RESIST | LBMHD_FULL */
   int    lattice;       /* LBMHD_D1Q3 | LBMHD_D2Q9 | LBMHD_D3Q19 | LBMHD_D2Q5 | LBMHD_D3Q7 */
   int    precision;     /* 64 (fp64 populations and arithmetic) or 32 (fp32 populations and arithmetic) */
   int    nx, ny, nz;    /* unused dims = 1 */
   double gamma;         /* IDEAL: adiabatic index, Eq.8 */
   double c0sq;          /* INCRES: artificial sound speed squared (A3) */
   double nu, eta;       /* if > 0: tau of the velocity (and P) / magnetic sets := 1/2 + D/c_s^2, Eq.5 PAPER.md:98.
-                           RESIST: eta (>= 0) is the magnetic diffusivity of the flux terms instead and leaves tau alone */
-  double tau[32];       /* per variable (first K <= 17 used), > 1/2, order of `scheme`; all magnetic sets must share one value (A7) */
-  double tau_relax;     /* IDEAL_DIVB, RESIST: relaxation time tau_M of the gradient variables (Eq.6), lattice units, > 0 */
+                           RESIST, FULL: eta (>= 0) is the magnetic diffusivity of the flux terms instead and leaves tau alone;
+                           FULL: nu (>= 0) is the shear viscosity mu of the flux terms likewise */
+  double tau[32];       /* per variable (first K <= 26 used), > 1/2, order of `scheme`; all magnetic sets must share one value (A7) */
+  double tau_relax;     /* IDEAL_DIVB, RESIST, FULL: relaxation time tau_M of the gradient variables (Eq.6), lattice units, > 0 */
   double eta_jc;        /* INCRES: critical current j_c of eta(j) = eta0 (1 + (j/j_c)^2) (eta0 from `eta` or tau),
                            lattice units; 0 = constant resistivity */
   double powell;        /* kappa: 0 = off, 1 = Eq.12 */

@@ -32,7 +32,7 @@ int lbh::fail(int code, const char *fmt, ...) {
 namespace {
 
 bool geometry(int scheme, int lattice, Geometry *g) {
-  if (scheme != LBMHD_IDEAL && scheme != LBMHD_INCRES && scheme != LBMHD_IDEAL_DIVB && scheme != LBMHD_RESIST) return false;
+  if (scheme != LBMHD_IDEAL && scheme != LBMHD_INCRES && scheme != LBMHD_IDEAL_DIVB && scheme != LBMHD_RESIST && scheme != LBMHD_FULL) return false;
   g->cs2 = 1.0 / 3.0;
   switch (lattice) {
     case LBMHD_D1Q3: g->D = 1; g->Q = 3; break;
@@ -43,7 +43,7 @@ bool geometry(int scheme, int lattice, Geometry *g) {
     default: return false;
   }
   const bool ideal = scheme != LBMHD_INCRES;
-  g->K = scheme == LBMHD_IDEAL ? 8 : (scheme == LBMHD_IDEAL_DIVB ? 9 : (scheme == LBMHD_RESIST ? 8 + 3 * g->D : 1 + 2 * g->D));
+  g->K = scheme == LBMHD_IDEAL ? 8 : (scheme == LBMHD_IDEAL_DIVB ? 9 : (scheme == LBMHD_RESIST ? 8 + 3 * g->D : (scheme == LBMHD_FULL ? 8 + 6 * g->D : 1 + 2 * g->D)));
   g->NV = ideal ? 3 : g->D;
   g->iU = 1;
   g->iB = ideal ? 5 : 1 + g->D;
@@ -166,19 +166,20 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
   h->N = (size_t)p->nx * p->ny * p->nz;
   for (int k = 0; k < g.K; k++) h->tau[k] = p->tau[k];
   const double cs2 = g.cs2;
-  if (p->nu > 0.0) {    // Eq.5
+  if (p->nu > 0.0 && p->scheme != LBMHD_FULL) {    // Eq.5; FULL carries nu (the shear viscosity) in the flux
     for (int b = 0; b < g.NV; b++) h->tau[g.iU + b] = 0.5 + p->nu / cs2;
     if (p->scheme == LBMHD_INCRES) h->tau[0] = 0.5 + p->nu / cs2;
   }
-  if (p->eta > 0.0 && p->scheme != LBMHD_RESIST)      // RESIST carries eta in the flux; tau_B stays the stabilisation parameter
+  if (p->eta > 0.0 && p->scheme != LBMHD_RESIST && p->scheme != LBMHD_FULL)      // RESIST, FULL carry eta in the flux; tau_B stays the stabilisation parameter
     for (int b = 0; b < g.NV; b++) h->tau[g.iB + b] = 0.5 + p->eta / cs2;
   for (int k = 0; k < g.K; k++)
     if (!(h->tau[k] > 0.5)) { delete h; return fail(LBMHD_EINVAL, "tau[%d] = %g must be > 1/2", k, p->tau[k]); }
   for (int b = 1; b < g.NV; b++)
     if (h->tau[g.iB + b] != h->tau[g.iB]) { delete h; return fail(LBMHD_EINVAL, "all magnetic sets must share one tau (A7)"); }
   if (p->scheme != LBMHD_INCRES && !(p->gamma > 1.0)) { delete h; return fail(LBMHD_EINVAL, "gamma must be > 1"); }
-  if ((p->scheme == LBMHD_IDEAL_DIVB || p->scheme == LBMHD_RESIST) && !(p->tau_relax > 0.0)) { delete h; return fail(LBMHD_EINVAL, "tau_relax must be > 0"); }
-  if (p->scheme == LBMHD_RESIST && !(p->eta >= 0.0)) { delete h; return fail(LBMHD_EINVAL, "eta must be >= 0"); }
+  if ((p->scheme == LBMHD_IDEAL_DIVB || p->scheme == LBMHD_RESIST || p->scheme == LBMHD_FULL) && !(p->tau_relax > 0.0)) { delete h; return fail(LBMHD_EINVAL, "tau_relax must be > 0"); }
+  if ((p->scheme == LBMHD_RESIST || p->scheme == LBMHD_FULL) && !(p->eta >= 0.0)) { delete h; return fail(LBMHD_EINVAL, "eta must be >= 0"); }
+  if (p->scheme == LBMHD_FULL && !(p->nu >= 0.0)) { delete h; return fail(LBMHD_EINVAL, "nu must be >= 0"); }
   if (p->eta_jc != 0.0 && !(p->scheme == LBMHD_INCRES && p->eta_jc > 0.0)) { delete h; return fail(LBMHD_EINVAL, "eta_jc needs the INCRES scheme and must be > 0"); }
   if (!p->workspace) { delete h; return fail(LBMHD_EINVAL, "workspace is NULL"); }
   if (((uintptr_t)p->workspace & 255) != 0) { delete h; return fail(LBMHD_ENOMEM, "workspace must be 256-byte aligned"); }
@@ -206,7 +207,7 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     const size_t es = p->precision == 64 ? 8 : 4;
     const long long tiles = (long long)((p->nx + kTmaTX - 1) / kTmaTX) * p->ny * p->nz;
     const bool halo = g.D >= 2 && (p->bc[2 * (g.D - 1)] == LBMHD_BC_HALO || p->bc[2 * (g.D - 1) + 1] == LBMHD_BC_HALO);
-    h->use_tma = !halo && p->scheme != LBMHD_RESIST && p->streaming == LBMHD_STREAM_AB && path && strcmp(path, "tma") == 0 && ((size_t)p->nx * es) % 16 == 0 && tiles < 2000000000LL;
+    h->use_tma = !halo && p->scheme != LBMHD_RESIST && p->scheme != LBMHD_FULL && p->streaming == LBMHD_STREAM_AB && path && strcmp(path, "tma") == 0 && ((size_t)p->nx * es) % 16 == 0 && tiles < 2000000000LL;
     if (h->use_tma) {
       const int rc = make_tensor_maps(h);
       if (rc) { delete h; return rc; }

@@ -30,11 +30,12 @@ template <typename real> struct StepArgs {
   size_t pstride;               // elements between planes
   int nx, ny, nz;
   int bc[6];
-  real omega[20];               // 1 / tau_k (K <= 17)
+  real omega[26];               // 1 / tau_k (K <= 26)
   real inv_tauB_cs2;            // 1 / (tau_B c_s^2)
   real kappa, gamma, c0sq;
   real inv_tau_relax;           // kIdealD, kResist: 1 / tau_M of the relaxation variables (Eq.6)
-  real eta;                     // kResist: magnetic diffusivity of the flux terms -eta grad B, eta j x B
+  real eta;                     // kResist, kFull: magnetic diffusivity of the flux terms -eta grad B, eta j x B
+  real mu;                      // kFull: shear viscosity of the flux terms -sigma, -u.sigma
   real etaj_inv_jc2;            // kIncres: 1 / j_c^2 of eta(j) = eta0 (1 + (j/j_c)^2), 0 = constant eta
   real tauB0;                   // tau of the magnetic sets at zero current
   const unsigned char *mask;    // [N] or nullptr
@@ -137,7 +138,7 @@ template <int K, typename real> __device__ __forceinline__ real pick(const real 
 // Qh is the (possibly solid-blended) state; `p` the gas pressure of the unblended state (A8 keeps p).
 // k is warp-uniform, so the switch does not diverge.
 template <int SCHEME, int D, typename real>
-__device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real c0sq, real eta, real itm, real Phi[3]) {
+__device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real c0sq, real eta, real visc, real itm, real Phi[3]) {
   Phi[0] = Phi[1] = Phi[2] = real(0);
   if (is_ideal(SCHEME)) {
     const real rho = Qh[0], E = Qh[4];
@@ -154,12 +155,16 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
       for (int a = 0; a < D; a++) Phi[a] = Qh[8] * u[a] - B[a];
       return;
     }
-    if (SCHEME == kResist && k >= 8) {   // G_cb: G_cb u_a - delta_ca B_b (Eq.10)
-      const int c = (k - 8) / 3, b = (k - 8) - 3 * c;
-      const real Gk = pick<8 + 3 * D, real>(Qh, k);
+    if (has_G(SCHEME) && k >= 8) {   // G_cb: G_cb u_a - delta_ca B_b (Eq.10); kFull H_cb: H_cb u_a - delta_ca u_b
+      const bool isH = SCHEME == kFull && k >= 8 + 3 * D;
+      const int kk = k - 8 - (isH ? 3 * D : 0);
+      const int c = kk / 3, b = kk - 3 * c;
+      const real Gk = pick<Vars<SCHEME, D>::K, real>(Qh, k);
       const real Bb = b == 0 ? B[0] : (b == 1 ? B[1] : B[2]);
+      const real ub = b == 0 ? u[0] : (b == 1 ? u[1] : u[2]);
+      const real Vb = isH ? ub : Bb;
 #pragma unroll
-      for (int a = 0; a < D; a++) Phi[a] = Gk * u[a] - (a == c ? Bb : real(0));
+      for (int a = 0; a < D; a++) Phi[a] = Gk * u[a] - (a == c ? Vb : real(0));
       return;
     }
     if (k >= 5) {   // induction: u_a B_b - B_a u_b  (kResist: - eta g_ab, g = G / tau_M ~ grad B)
@@ -168,7 +173,7 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
       const real ub = b == 0 ? u[0] : (b == 1 ? u[1] : u[2]);
 #pragma unroll
       for (int a = 0; a < D; a++) Phi[a] = u[a] * Bb - B[a] * ub;
-      if (SCHEME == kResist) {
+      if (has_G(SCHEME)) {
 #pragma unroll
         for (int a = 0; a < D; a++) {
           const real Gab = b == 0 ? Qh[8 + 3 * a] : (b == 1 ? Qh[8 + 3 * a + 1] : Qh[8 + 3 * a + 2]);
@@ -185,7 +190,7 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
       const real uB = u[0] * B[0] + u[1] * B[1] + u[2] * B[2];
 #pragma unroll
       for (int a = 0; a < D; a++) Phi[a] = (E + pt) * u[a] - B[a] * uB;
-      if (SCHEME == kResist) {   // + eta (j x B)_a,  j = curl B: j_e = eps_ecb g_cb over the lattice axes c < D
+      if (has_G(SCHEME)) {   // + eta (j x B)_a,  j = curl B: j_e = eps_ecb g_cb over the lattice axes c < D
         real g[3][3];
 #pragma unroll
         for (int c = 0; c < 3; c++)
@@ -196,13 +201,43 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
 #pragma unroll
         for (int a = 0; a < D; a++) Phi[a] += eta * jxB[a];
       }
+      if (SCHEME == kFull) {   // - u_b sigma_ab,  sigma = mu (h + h^T - 2/3 tr h I),  h = H / tau_M ~ grad u (A23)
+        real h[3][3];
+#pragma unroll
+        for (int c = 0; c < 3; c++)
+#pragma unroll
+          for (int b = 0; b < 3; b++) h[c][b] = c < D ? Qh[8 + 3 * D + 3 * (c < D ? c : 0) + b] * itm : real(0);
+        const real trh = h[0][0] + h[1][1] + h[2][2];
+#pragma unroll
+        for (int a = 0; a < D; a++) {
+          real us = real(0);
+#pragma unroll
+          for (int b = 0; b < 3; b++) us += u[b] * (visc * (h[a][b] + h[b][a] - (a == b ? real(2.0 / 3.0) * trh : real(0))));
+          Phi[a] -= us;
+        }
+      }
       return;
     }
-    const int b = k - 1;   // momentum: m_b u_a + pt delta_ab - B_b B_a
+    const int b = k - 1;   // momentum: m_b u_a + pt delta_ab - B_b B_a  (kFull: - sigma_ab)
     const real mb = b == 0 ? m[0] : (b == 1 ? m[1] : m[2]);
     const real Bb = b == 0 ? B[0] : (b == 1 ? B[1] : B[2]);
 #pragma unroll
     for (int a = 0; a < D; a++) Phi[a] = mb * u[a] + (a == b ? pt : real(0)) - Bb * B[a];
+    if (SCHEME == kFull) {
+      real trh = real(0);
+#pragma unroll
+      for (int c = 0; c < D; c++) trh += Qh[8 + 3 * D + 3 * c + c] * itm;
+#pragma unroll
+      for (int a = 0; a < D; a++) {
+        // h_ab = H_ab / tau_M (a < D), h_ba = H_ba / tau_M if b < D else 0
+        const real hab = (b == 0 ? Qh[8 + 3 * D + 3 * a] : (b == 1 ? Qh[8 + 3 * D + 3 * a + 1] : Qh[8 + 3 * D + 3 * a + 2])) * itm;
+        real hba = real(0);
+#pragma unroll
+        for (int c = 0; c < D; c++)
+          if (b == c) hba = Qh[8 + 3 * D + 3 * c + a] * itm;
+        Phi[a] -= visc * (hab + hba - (a == b ? real(2.0 / 3.0) * trh : real(0)));
+      }
+    }
   } else {
     const real P = Qh[0];
     const real *u = Qh + 1, *B = Qh + 1 + D;
@@ -386,7 +421,7 @@ __device__ __forceinline__ void frozen_rematerialise(const StepArgs<real> &a, in
   real Qf[K], Phi[3];
 #pragma unroll
   for (int l = 0; l < K; l++) Qf[l] = (real)a.M_cur[(size_t)l * N + n];
-  flux_row<SCHEME, D, real>(k, Qf, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
+  flux_row<SCHEME, D, real>(k, Qf, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
   const real Qfk = pick<K, real>(Qf, k);
 #pragma unroll
   for (int j = 0; j < Q; j++) {
@@ -547,7 +582,7 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
       real Qnb[K], Phi[3];
 #pragma unroll
       for (int l = 0; l < K; l++) Qnb[l] = sh.sQ[l][tx];
-      flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
+      flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
       const real Qnbk = pick<K, real>(Qnb, k);
 #pragma unroll
       for (int i = 0; i < Q; i++) {
@@ -625,7 +660,7 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   // A6: local estimate from tr Pi_B; kIdealD: from the relaxation variable, D ~ tau_M div B (Eq.7)
   real delta;
   if (SCHEME == kIdealD) delta = Qv[K - 1] * a.inv_tau_relax;
-  else if (SCHEME == kResist) {         // div B = tr g = sum_a G_aa / tau_M
+  else if (has_G(SCHEME)) {         // div B = tr g = sum_a G_aa / tau_M
     delta = real(0);
 #pragma unroll
     for (int al = 0; al < D; al++) delta += Qv[8 + 3 * al + al] * a.inv_tau_relax;
@@ -643,7 +678,7 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
     if (d < real(1)) {
       real Qh[K];
       solid_blend<SCHEME, D, real>(Qv, a.gamma, d, uS, BS, Qh);
-      flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
+      flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
       // dQh plus the Powell source scaled by the porosity d (A8)
       dq = pick<K, real>(Qh, k) - Qk;
       inj = dq - d * (a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
@@ -653,7 +688,7 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
     if (a.body != nullptr) body_accumulate<SCHEME, D, real>(a, c, k, solid, (double)dq, (double)d, (double)Qk);
   }
   if (!solid) {
-    flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
+    flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
     inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
     if (has_relax(SCHEME) && k >= 8) inj = -Qk * a.inv_tau_relax;        // relaxation source of Eq.6
   }
@@ -856,7 +891,7 @@ __device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, 
         real Qnb[K], Phi[3];
 #pragma unroll
         for (int l = 0; l < K; l++) Qnb[l] = sh.sNb[l];
-        flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
+        flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
         const real Qnbk = pick<K, real>(Qnb, k);
 #pragma unroll
         for (int i = 0; i < Q; i++) {
@@ -1029,7 +1064,7 @@ __device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, in
     real delta;
     if (SCHEME == kIdealD) {
       delta = Qv[K - 1] * a.inv_tau_relax;
-    } else if (SCHEME == kResist) {
+    } else if (has_G(SCHEME)) {
       delta = real(0);
 #pragma unroll
       for (int al = 0; al < D; al++) delta += Qv[8 + 3 * al + al] * a.inv_tau_relax;
@@ -1040,7 +1075,7 @@ __device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, in
       delta = -tr * a.inv_tauB_cs2;
     }
     real Phi[3];
-    flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, a.eta, a.inv_tau_relax, Phi);
+    flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
     real inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
     if (has_relax(SCHEME) && k >= 8) inj = -Qk[c] * a.inv_tau_relax;      // relaxation source of Eq.6
     if (STREAM != ST_AB && writeM[c]) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + n + c] = (double)(Qk[c] + inj);
@@ -1134,7 +1169,7 @@ step_kernel_multi(const __grid_constant__ StepArgs<real> a, const int nmulti) {
 template <int LAT, int SCHEME, typename real, int TX>
 __global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K)
 init_kernel(const double *__restrict__ fields, real *__restrict__ g, size_t pstride, int nx, int ny, int nz, real gamma,
-            real c0sq, real eta, real itm) {
+            real c0sq, real eta, real mu, real itm) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q, K = Vars<SCHEME, D>::K;
   const int k = threadIdx.y;
@@ -1145,7 +1180,7 @@ init_kernel(const double *__restrict__ fields, real *__restrict__ g, size_t pstr
   real Qv[K], Phi[3];
 #pragma unroll
   for (int l = 0; l < K; l++) Qv[l] = (real)fields[(size_t)l * N + n];
-  flux_row<SCHEME, D, real>(k, Qv, gamma, c0sq, eta, itm, Phi);
+  flux_row<SCHEME, D, real>(k, Qv, gamma, c0sq, eta, mu, itm, Phi);
   const real Qk = pick<K, real>(Qv, k);
   real *gk = g + (size_t)k * Q * pstride;
 #pragma unroll

@@ -79,11 +79,14 @@ template <class L> __host__ __device__ constexpr int lat_c(int i, int axis) {
 // kIdealD: ideal MHD plus the traced gradient-relaxation variable D = tr G (A19), K = 9
 // kResist: ideal MHD plus the transported gradients G_ab = tau_M d_a B_b (a < D, b < 3; variable 8 + 3a + b) with the
 //          resistive fluxes taken from them (Eq.9-10; A22), K = 8 + 3 D
-constexpr int kIdeal = 0, kIncres = 1, kIdealD = 2, kResist = 3;
+// kFull:   kResist plus the transported velocity gradients H_ab = tau_M d_a u_b (variable 8 + 3 D + 3a + b) with the viscous
+//          stress -sigma, -u.sigma taken from them: the full dissipative system (A23), K = 8 + 6 D
+constexpr int kIdeal = 0, kIncres = 1, kIdealD = 2, kResist = 3, kFull = 4;
+__host__ __device__ constexpr bool has_G(int scheme) { return scheme == kResist || scheme == kFull; }   // carries G_ab at 8 + 3a + b
 __host__ __device__ constexpr bool is_ideal(int scheme) { return scheme != kIncres; }          // first 8 variables (rho, m, E, B)
-__host__ __device__ constexpr bool has_relax(int scheme) { return scheme == kIdealD || scheme == kResist; }   // variables >= 8 relax
+__host__ __device__ constexpr bool has_relax(int scheme) { return scheme == kIdealD || scheme == kResist || scheme == kFull; }   // variables >= 8 relax
 template <int SCHEME, int D> struct Vars {
-  static constexpr int K = SCHEME == kIdeal ? 8 : (SCHEME == kIdealD ? 9 : (SCHEME == kResist ? 8 + 3 * D : 1 + 2 * D));
+  static constexpr int K = SCHEME == kIdeal ? 8 : (SCHEME == kIdealD ? 9 : (SCHEME == kResist ? 8 + 3 * D : (SCHEME == kFull ? 8 + 6 * D : 1 + 2 * D)));
   static constexpr int NV = is_ideal(SCHEME) ? 3 : D;      // vector components carried
   static constexpr int iU = 1;                             // first momentum / velocity component
   static constexpr int iB = is_ideal(SCHEME) ? 5 : 1 + D;  // first magnetic component

@@ -125,7 +125,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     a.kappa = (real)h->p.powell; a.gamma = (real)h->p.gamma; a.c0sq = (real)h->p.c0sq;
     a.inv_tau_relax = h->p.tau_relax > 0.0 ? (real)(1.0 / h->p.tau_relax) : real(0);
     a.etaj_inv_jc2 = h->p.eta_jc > 0.0 ? (real)(1.0 / (h->p.eta_jc * h->p.eta_jc)) : real(0);
-    a.eta = SCHEME == kResist ? (real)h->p.eta : real(0);
+    a.eta = has_G(SCHEME) ? (real)h->p.eta : real(0);
+    a.mu = SCHEME == kFull ? (real)h->p.nu : real(0);
     a.tauB0 = (real)h->tau[h->g.iB];
     a.mask = h->have_mask ? (const unsigned char *)(h->ws + h->L.off_mask) : nullptr;
     a.Bsolid = h->have_bsolid ? (const double *)(h->ws + h->L.off_bsolid) : nullptr;
@@ -204,7 +205,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
   static int init(lbmhd_t *h, const double *fields_dev) {
     init_kernel<LAT, SCHEME, real, TXAUX><<<grid(h, TXAUX), dim3(TXAUX, K), 0, h->stream>>>(
         fields_dev, pops(h, 0), h->L.pstride, h->p.nx, h->p.ny, h->p.nz, (real)h->p.gamma, (real)h->p.c0sq,
-        SCHEME == kResist ? (real)h->p.eta : real(0), h->p.tau_relax > 0.0 ? (real)(1.0 / h->p.tau_relax) : real(0));
+        has_G(SCHEME) ? (real)h->p.eta : real(0), SCHEME == kFull ? (real)h->p.nu : real(0), h->p.tau_relax > 0.0 ? (real)(1.0 / h->p.tau_relax) : real(0));
     CUDA_TRY(cudaGetLastError());
     h->launches += 1;
     h->parity = 0;
@@ -284,6 +285,7 @@ template <int LAT, typename real> OpTable table_for(int scheme) {
   if (scheme == LBMHD_IDEAL) return make_table<LAT, kIdeal, real>();
   if (scheme == LBMHD_IDEAL_DIVB) return make_table<LAT, kIdealD, real>();
   if (scheme == LBMHD_RESIST) return make_table<LAT, kResist, real>();
+  if (scheme == LBMHD_FULL) return make_table<LAT, kFull, real>();
   return make_table<LAT, kIncres, real>();
 }
 

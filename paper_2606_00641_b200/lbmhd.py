@@ -13,13 +13,13 @@ import numpy as np
 from . import build as _build
 
 D1Q3, D2Q9, D3Q19, D2Q5, D3Q7 = 1, 2, 3, 4, 5
-IDEAL, INCRES, IDEAL_DIVB, RESIST = 0, 1, 2, 3
+IDEAL, INCRES, IDEAL_DIVB, RESIST, FULL = 0, 1, 2, 3, 4
 BC_PERIODIC, BC_ZEROGRAD, BC_INFLOW, BC_HALO = 0, 1, 2, 3
 CELL_FLUID, CELL_FROZEN, CELL_SOLID = 0, 1, 2
 STREAM_AB, STREAM_INPLACE = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC = 0, -1, -2, -3, -4
 LATTICES = {"D1Q3": D1Q3, "D2Q9": D2Q9, "D3Q19": D3Q19, "D2Q5": D2Q5, "D3Q7": D3Q7}
-SCHEMES = {"IDEAL": IDEAL, "INCRES": INCRES, "IDEAL_DIVB": IDEAL_DIVB, "RESIST": RESIST}
+SCHEMES = {"IDEAL": IDEAL, "INCRES": INCRES, "IDEAL_DIVB": IDEAL_DIVB, "RESIST": RESIST, "FULL": FULL}
 
 
 class LbmhdParams(C.Structure):

@@ -193,20 +193,22 @@ def config5(shape=(384, 256, 256), steps=500, tau=0.7, radius=None, planes=None)
                 tau=tau, powell=1.0, bc=(INFLOW, ZEROGRAD, 0, 0, 0, 0), steps=steps, fields=F, sphere=sphere, scale=1.0)
 
 
-def variant(w, scheme=None, lattice=None, tau_relax=8.0, eta=1e-3):
+def variant(w, scheme=None, lattice=None, tau_relax=8.0, eta=1e-3, mu=1e-3):
     """the same input on another scheme of the IDEAL family or on the paper's own lattice (DESIGN.md §0 NEXT rows):
-    IDEAL_DIVB adds D = tr G (1 set), RESIST adds G_ab (3 D sets), both started at 0 (they relax to tau_M grad B in
+    IDEAL_DIVB adds D = tr G (1 set), RESIST adds G_ab (3 D sets), FULL adds G_ab and H_ab (6 D sets), all started at 0 (they relax to tau_M grad B in
     ~tau_M steps, Eq.7); D2Q5 / D3Q7 replace D2Q9 / D3Q19."""
     w = dict(w)
     if scheme is not None and scheme != w["scheme"]:
-        if w["scheme"] != "IDEAL" or scheme not in ("IDEAL_DIVB", "RESIST"):
+        if w["scheme"] != "IDEAL" or scheme not in ("IDEAL_DIVB", "RESIST", "FULL"):
             raise ValueError("variant: %s -> %s" % (w["scheme"], scheme))
         D = len(w["shape"])
-        extra = 1 if scheme == "IDEAL_DIVB" else 3 * D
+        extra = 1 if scheme == "IDEAL_DIVB" else (3 * D if scheme == "RESIST" else 6 * D)
         w["fields"] = np.concatenate([w["fields"], np.zeros((extra,) + w["fields"].shape[1:])])
         w["scheme"], w["tau_relax"] = scheme, tau_relax
-        if scheme == "RESIST":
+        if scheme in ("RESIST", "FULL"):
             w["eta"] = eta
+        if scheme == "FULL":
+            w["nu"] = mu
     if lattice is not None and lattice != w["lattice"]:
         if lattice[:2] != w["lattice"][:2]:
             raise ValueError("variant: %s -> %s" % (w["lattice"], lattice))

@@ -4,7 +4,7 @@ import numpy as np
 from oracle import oracle as orc
 
 LAT_ORC = {"D1Q3": orc.D1Q3, "D2Q9": orc.D2Q9, "D3Q19": orc.D3Q19, "D2Q5": orc.D2Q5, "D3Q7": orc.D3Q7}
-ORC_SCHEME = {"IDEAL": orc.IDEAL, "INCRES": orc.INCRES, "IDEAL_DIVB": orc.IDEAL_DIVB, "RESIST": orc.RESIST}
+ORC_SCHEME = {"IDEAL": orc.IDEAL, "INCRES": orc.INCRES, "IDEAL_DIVB": orc.IDEAL_DIVB, "RESIST": orc.RESIST, "FULL": orc.FULL}
 TOL64 = 1e-11      # BASELINE.json north_star: max relative error on all macroscopic fields, fp64
 TOL32 = 1e-5       # fp32
 

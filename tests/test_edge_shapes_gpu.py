@@ -3,7 +3,7 @@ boundary combination, both streaming modes, all lattices and schemes — a seede
 import numpy as np
 import pytest
 
-from test_parity_gpu import compare, random_workload, divb_workload, resist_workload
+from test_parity_gpu import compare, random_workload, divb_workload, resist_workload, full_workload
 from parity_util import TOL64, TOL32
 
 pytestmark = pytest.mark.gpu
@@ -40,6 +40,18 @@ def test_random_small_shapes(seed):
         w = random_workload(scheme, lattice, shape, bc, seed=seed)
     steps = int(rng.integers(1, 7))
     compare(w, steps, tol=TOL64 if precision == 64 else TOL32, precision=precision, streaming=streaming)
+
+
+@pytest.mark.parametrize("seed", range(20))
+def test_random_small_shapes_full_scheme(seed):
+    """the same sweep for the 8 + 6 D sets of the full dissipative scheme (blocks of up to 26 variable rows)"""
+    rng = np.random.default_rng(9500 + seed)
+    _, lattice, shape, bc = random_case(rng)
+    streaming = int(rng.integers(0, 2))
+    precision = 64 if rng.random() < 0.75 else 32
+    steps = int(rng.integers(1, 7))
+    compare(full_workload(lattice, shape, bc, seed=seed), steps, tol=TOL64 if precision == 64 else TOL32, precision=precision,
+            streaming=streaming)
 
 
 def test_single_cell_rows_and_zero_steps():

@@ -10,7 +10,7 @@ import numpy as np
 import pytest
 
 from parity_util import TOL64, TOL32
-from test_parity_gpu import compare, random_workload, divb_workload, resist_workload
+from test_parity_gpu import compare, random_workload, divb_workload, resist_workload, full_workload
 
 pytestmark = pytest.mark.gpu
 
@@ -47,6 +47,7 @@ def test_multi_cell_other_schemes(env, lattice, shape, bc, precision, tol, strea
     compare(random_workload("INCRES", lattice, shape, bc, seed=102), 7, tol=tol, precision=precision, streaming=streaming)
     compare(divb_workload(lattice, shape, bc, seed=103), 7, tol=tol, precision=precision, streaming=streaming)
     compare(resist_workload(lattice, shape, bc, seed=104), 7, tol=tol, precision=precision, streaming=streaming)
+    compare(full_workload(lattice, shape, bc, seed=111), 7, tol=tol, precision=precision, streaming=streaming)
 
 
 @pytest.mark.parametrize("streaming", [0, 1])

@@ -258,6 +258,60 @@ def test_resist_scheme_parity(lattice, shape, bc, precision, tol, streaming):
     compare(w, 7, tol=tol, precision=precision, streaming=streaming)
 
 
+def full_workload(lattice, shape, bc, seed, sphere=None, eta=0.02, mu=0.015, tau_relax=3.0):
+    """FULL (K = 8 + 6 D): random ideal state plus random gradient variables G (of B) and H (of u)"""
+    w = random_workload("IDEAL", lattice, shape, bc, seed=seed, sphere=sphere)
+    rng = np.random.default_rng(seed + 3)
+    w["scheme"], w["tau_relax"], w["eta"], w["nu"] = "FULL", tau_relax, eta, mu
+    w["fields"] = np.concatenate([w["fields"], 0.05 * (rng.random((6 * len(shape),) + zyx(shape)) - 0.5)])
+    return w
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+@pytest.mark.parametrize("precision,tol", [(64, TOL64), (32, TOL32)])
+@pytest.mark.parametrize("lattice,shape,bc", [("D1Q3", (200,), (1, 1, 0, 0, 0, 0)), ("D2Q9", (150, 37), (0,) * 6),
+                                              ("D2Q9", (90, 21), (1, 1, 2, 1, 0, 0)), ("D3Q19", (200, 12, 9), (2, 1, 0, 0, 0, 0)),
+                                              ("D3Q19", (45, 11, 10), (1, 1, 1, 1, 1, 1)), ("D3Q7", (100, 12, 9), (1, 1, 1, 1, 0, 0)),
+                                              ("D2Q5", (150, 37), (0,) * 6)])
+def test_full_scheme_parity(lattice, shape, bc, precision, tol, streaming):
+    """full dissipative MHD (Eq.9): K = 8 + 6 D sets, resistive fluxes from G, viscous stress from H (A23)"""
+    w = full_workload(lattice, shape, bc, seed=91)
+    compare(w, 20, tol=tol, precision=precision, streaming=streaming)
+    compare(w, 7, tol=tol, precision=precision, streaming=streaming)
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+def test_full_with_sphere_and_mask(streaming):
+    cen = np.array([36.0, 12.0, 10.0])
+    mh = np.array([0.3, -0.5, 0.8]) / np.linalg.norm([0.3, -0.5, 0.8])
+    sph = dict(centre=cen, radius=6.0, u_solid=np.array([-0.25, 0.0, 0.0]), dipole_dir=mh, B_surface=0.03, width=1.5,
+               omega=np.array([0.02, 0.0, 0.02]))
+    compare(full_workload("D3Q19", (72, 24, 20), (2, 1, 0, 0, 0, 0), seed=92, sphere=sph), 12, streaming=streaming)
+    rng = np.random.default_rng(23)
+    s = (9, 40)
+    mask = (rng.random(s) < 0.05).astype(np.uint8) * 2
+    mask[rng.random(s) < 0.02] = 1
+    compare(full_workload("D2Q9", (40, 9), (0,) * 6, seed=93), 10, mask=mask,
+            obstacle=(mask, np.array([0.03, -0.02, 0.0]), 0.1 * (rng.random((3,) + s) - 0.5)), streaming=streaming)
+
+
+def test_full_viscous_terms_are_live():
+    """mu changes the result (the H sets feed the momentum and energy fluxes), and mu = 0 reproduces RESIST on its variables"""
+    w = full_workload("D2Q9", (64, 16), (0,) * 6, seed=94)
+    a, b = gpu_from_workload(w), gpu_from_workload(dict(w, nu=0.0))
+    r = resist_workload("D2Q9", (64, 16), (0,) * 6, seed=94)
+    r["fields"] = w["fields"][:14].copy()
+    c = gpu_from_workload(r)
+    for g, F in ((a, w["fields"]), (b, w["fields"]), (c, r["fields"])):
+        g.init(F)
+        g.step(10)
+    Qa, Qb, Qc = a.moments()[0], b.moments()[0], c.moments()[0]
+    assert np.abs(Qa[1:5] - Qb[1:5]).max() > 1e-6
+    assert np.abs(Qb[:14] - Qc).max() <= 1e-13 * np.abs(Qc).max()
+    for g in (a, b, c):
+        g.close()
+
+
 @pytest.mark.parametrize("streaming", [0, 1])
 def test_resist_with_sphere_and_mask(streaming):
     cen = np.array([36.0, 12.0, 10.0])

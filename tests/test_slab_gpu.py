@@ -5,7 +5,7 @@ import pytest
 
 from paper_2606_00641_b200 import workloads as W
 from parity_util import field_errors, oracle_from_workload, TOL64, TOL32
-from test_parity_gpu import random_workload, gpu_from_workload, divb_workload, resist_workload
+from test_parity_gpu import random_workload, gpu_from_workload, divb_workload, resist_workload, full_workload
 
 pytestmark = pytest.mark.gpu
 
@@ -65,4 +65,7 @@ def test_slabs_fp32_and_divb_scheme():
     assert (field_errors(Qs, Qr) <= 1e-13).all()
     w = resist_workload("D2Q9", (100, 24), (0,) * 6, seed=65)
     Qr, dr, Qs, ds = run_both(w, 2, 10)
+    assert (field_errors(Qs, Qr) <= 1e-13).all()
+    w = full_workload("D3Q19", (64, 12, 12), (2, 1, 0, 0, 0, 0), seed=66)        # K = 26 sets across the cuts
+    Qr, dr, Qs, ds = run_both(w, 3, 8)
     assert (field_errors(Qs, Qr) <= 1e-13).all()
