@@ -135,39 +135,46 @@ template <int K, typename real> __device__ __forceinline__ real pick(const real 
 }
 
 // ---- flux row of variable k: Phi_k,alpha(Qh), alpha < D (Eq.11, Eq.8; A3) -------
-// Qh is the (possibly solid-blended) state; `p` the gas pressure of the unblended state (A8 keeps p).
-// k is warp-uniform, so the switch does not diverge.
-template <int SCHEME, int D, typename real>
-__device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real c0sq, real eta, real visc, real itm, real Phi[3]) {
+// Qh is the (possibly solid-blended) state: an array in registers or a column of the shared exchange array (QCol) — the
+// rows read only the entries they need (a gradient row of RESIST / FULL needs 5 of the 17 / 26).  `own` = Qh[k].
+// k is warp-uniform, so the branches do not diverge.
+template <typename real, int TX> struct QCol {
+  real (*s)[TX];
+  int tx;
+  __device__ __forceinline__ real operator[](int l) const { return s[l][tx]; }
+};
+template <class QA, typename real> __device__ __forceinline__ real pick3(const QA &Q, int base, int b) {
+  return b == 0 ? Q[base] : (b == 1 ? Q[base + 1] : Q[base + 2]);
+}
+
+template <int SCHEME, int D, typename real, class QA>
+__device__ __forceinline__ void flux_row(int k, const QA &Qh, real own, real gamma, real c0sq, real eta, real visc, real itm, real Phi[3]) {
   Phi[0] = Phi[1] = Phi[2] = real(0);
   if (is_ideal(SCHEME)) {
-    const real rho = Qh[0], E = Qh[4];
-    const real *m = Qh + 1, *B = Qh + 5;
     if (k == 0) {
 #pragma unroll
-      for (int a = 0; a < D; a++) Phi[a] = m[a];
+      for (int a = 0; a < D; a++) Phi[a] = Qh[1 + a];
       return;
     }
-    const real ir = real(1) / rho;
+    const real ir = real(1) / Qh[0];
+    const real m[3] = {Qh[1], Qh[2], Qh[3]};
     const real u[3] = {m[0] * ir, m[1] * ir, m[2] * ir};
     if (SCHEME == kIdealD && k == 8) {   // relaxation variable D = tr G: D u - B (Eq.10, traced)
 #pragma unroll
-      for (int a = 0; a < D; a++) Phi[a] = Qh[8] * u[a] - B[a];
+      for (int a = 0; a < D; a++) Phi[a] = own * u[a] - Qh[5 + a];
       return;
     }
     if (has_G(SCHEME) && k >= 8) {   // G_cb: G_cb u_a - delta_ca B_b (Eq.10); kFull H_cb: H_cb u_a - delta_ca u_b
       const bool isH = SCHEME == kFull && k >= 8 + 3 * D;
       const int kk = k - 8 - (isH ? 3 * D : 0);
       const int c = kk / 3, b = kk - 3 * c;
-      const real Gk = pick<Vars<SCHEME, D>::K, real>(Qh, k);
-      const real Bb = b == 0 ? B[0] : (b == 1 ? B[1] : B[2]);
-      const real ub = b == 0 ? u[0] : (b == 1 ? u[1] : u[2]);
-      const real Vb = isH ? ub : Bb;
+      const real Vb = isH ? (b == 0 ? u[0] : (b == 1 ? u[1] : u[2])) : pick3<QA, real>(Qh, 5, b);
 #pragma unroll
-      for (int a = 0; a < D; a++) Phi[a] = Gk * u[a] - (a == c ? Vb : real(0));
+      for (int a = 0; a < D; a++) Phi[a] = own * u[a] - (a == c ? Vb : real(0));
       return;
     }
-    if (k >= 5) {   // induction: u_a B_b - B_a u_b  (kResist: - eta g_ab, g = G / tau_M ~ grad B)
+    const real B[3] = {Qh[5], Qh[6], Qh[7]};
+    if (k >= 5) {   // induction: u_a B_b - B_a u_b  (kResist, kFull: - eta g_ab, g = G / tau_M ~ grad B)
       const int b = k - 5;
       const real Bb = b == 0 ? B[0] : (b == 1 ? B[1] : B[2]);
       const real ub = b == 0 ? u[0] : (b == 1 ? u[1] : u[2]);
@@ -175,13 +182,11 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
       for (int a = 0; a < D; a++) Phi[a] = u[a] * Bb - B[a] * ub;
       if (has_G(SCHEME)) {
 #pragma unroll
-        for (int a = 0; a < D; a++) {
-          const real Gab = b == 0 ? Qh[8 + 3 * a] : (b == 1 ? Qh[8 + 3 * a + 1] : Qh[8 + 3 * a + 2]);
-          Phi[a] -= eta * (Gab * itm);
-        }
+        for (int a = 0; a < D; a++) Phi[a] -= eta * (pick3<QA, real>(Qh, 8 + 3 * a, b) * itm);
       }
       return;
     }
+    const real E = Qh[4];
     const real B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
     const real mu = m[0] * u[0] + m[1] * u[1] + m[2] * u[2];
     const real p = (gamma - real(1)) * (E - real(0.5) * mu - real(0.5) * B2);
@@ -230,7 +235,7 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
 #pragma unroll
       for (int a = 0; a < D; a++) {
         // h_ab = H_ab / tau_M (a < D), h_ba = H_ba / tau_M if b < D else 0
-        const real hab = (b == 0 ? Qh[8 + 3 * D + 3 * a] : (b == 1 ? Qh[8 + 3 * D + 3 * a + 1] : Qh[8 + 3 * D + 3 * a + 2])) * itm;
+        const real hab = pick3<QA, real>(Qh, 8 + 3 * D + 3 * a, b) * itm;
         real hba = real(0);
 #pragma unroll
         for (int c = 0; c < D; c++)
@@ -239,13 +244,14 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
       }
     }
   } else {
-    const real P = Qh[0];
-    const real *u = Qh + 1, *B = Qh + 1 + D;
     if (k == 0) {
 #pragma unroll
-      for (int a = 0; a < D; a++) Phi[a] = c0sq * u[a];
+      for (int a = 0; a < D; a++) Phi[a] = c0sq * Qh[1 + a];
       return;
     }
+    real u[D], B[D];
+#pragma unroll
+    for (int c = 0; c < D; c++) { u[c] = Qh[1 + c]; B[c] = Qh[1 + D + c]; }
     if (k >= 1 + D) {
       const int b = k - 1 - D;
       real Bb = B[0], ub = u[0];
@@ -259,7 +265,7 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
     real B2 = real(0);
 #pragma unroll
     for (int c = 0; c < D; c++) B2 += B[c] * B[c];
-    const real pt = P + real(0.5) * B2;
+    const real pt = Qh[0] + real(0.5) * B2;
     const int b = k - 1;
     real Bb = B[0], ub = u[0];
 #pragma unroll
@@ -271,15 +277,15 @@ __device__ __forceinline__ void flux_row(int k, const real *Qh, real gamma, real
 }
 
 // ---- Powell source row S_k / (-kappa delta) (Eq.12): (0, B, u.B, u) resp. (0, B, u) ----------
-template <int SCHEME, int D, typename real>
-__device__ __forceinline__ real powell_row(int k, const real *Qv) {
+template <int SCHEME, int D, typename real, class QA>
+__device__ __forceinline__ real powell_row(int k, const QA &Qv) {
   if (k == 0) return real(0);
   if (is_ideal(SCHEME)) {
     if (has_relax(SCHEME) && k >= 8) return real(0);
-    if (k <= 3) return k == 1 ? Qv[5] : (k == 2 ? Qv[6] : Qv[7]);
+    if (k <= 3) return pick3<QA, real>(Qv, 5, k - 1);
     const real ir = real(1) / Qv[0];
     if (k == 4) return (Qv[1] * Qv[5] + Qv[2] * Qv[6] + Qv[3] * Qv[7]) * ir;
-    return (k == 5 ? Qv[1] : (k == 6 ? Qv[2] : Qv[3])) * ir;
+    return pick3<QA, real>(Qv, 1, k - 5) * ir;
   } else {
     real r = real(0);
 #pragma unroll
@@ -421,8 +427,8 @@ __device__ __forceinline__ void frozen_rematerialise(const StepArgs<real> &a, in
   real Qf[K], Phi[3];
 #pragma unroll
   for (int l = 0; l < K; l++) Qf[l] = (real)a.M_cur[(size_t)l * N + n];
-  flux_row<SCHEME, D, real>(k, Qf, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
   const real Qfk = pick<K, real>(Qf, k);
+  flux_row<SCHEME, D, real>(k, Qf, Qfk, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
 #pragma unroll
   for (int j = 0; j < Q; j++) {
     const real cPhi = real(L::cx(j)) * Phi[0] + real(L::cy(j)) * Phi[1] + real(L::cz(j)) * Phi[2];
@@ -582,8 +588,8 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
       real Qnb[K], Phi[3];
 #pragma unroll
       for (int l = 0; l < K; l++) Qnb[l] = sh.sQ[l][tx];
-      flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
       const real Qnbk = pick<K, real>(Qnb, k);
+      flux_row<SCHEME, D, real>(k, Qnb, Qnbk, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
 #pragma unroll
       for (int i = 0; i < Q; i++) {
         const int cx = L::cx(i), cy = L::cy(i), cz = L::cz(i);
@@ -628,16 +634,22 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   sh.sync();
   if (!work) return;
 
-  real Qv[K];
+  // The schemes with gradient sets (K = 11 .. 26) read the exchanged moments where a row needs them (a gradient row needs
+  // 5); the others keep the K moments in registers.
+  constexpr bool LAZY = has_G(SCHEME);
+  const QCol<real, TX> qc{sh.sQ, tx};
+  real Qv[LAZY ? 1 : K];
+  if constexpr (!LAZY) {
 #pragma unroll
-  for (int l = 0; l < K; l++) Qv[l] = sh.sQ[l][tx];
+    for (int l = 0; l < K; l++) Qv[l] = sh.sQ[l][tx];
+  }
   real tr = real(0);
 #pragma unroll
   for (int b = 0; b < D; b++) tr += sh.sTr[b * D + b][tx];
   // A20: current-dependent resistivity -> cell-local tau_B (6 Newton steps on tau^3 - tau0 tau^2 - c = 0 from tau0 + cbrt(c))
   real inv_tauB_cs2 = a.inv_tauB_cs2;
   real omB = real(0);
-  if (SCHEME == kIncres && a.etaj_inv_jc2 > real(0)) {
+  if constexpr (SCHEME == kIncres) if (a.etaj_inv_jc2 > real(0)) {
     real a2 = real(0);
 #pragma unroll
     for (int al = 0; al < D; al++)
@@ -659,11 +671,13 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   }
   // A6: local estimate from tr Pi_B; kIdealD: from the relaxation variable, D ~ tau_M div B (Eq.7)
   real delta;
-  if (SCHEME == kIdealD) delta = Qv[K - 1] * a.inv_tau_relax;
-  else if (has_G(SCHEME)) {         // div B = tr g = sum_a G_aa / tau_M
+  if constexpr (SCHEME == kIdealD) delta = Qv[K - 1] * a.inv_tau_relax;
+  else if constexpr (has_G(SCHEME)) {         // div B = tr g = sum_a G_aa / tau_M (only the 8 Powell rows use it)
     delta = real(0);
+    if (k < 8) {
 #pragma unroll
-    for (int al = 0; al < D; al++) delta += Qv[8 + 3 * al + al] * a.inv_tau_relax;
+      for (int al = 0; al < D; al++) delta += qc[8 + 3 * al + al] * a.inv_tau_relax;
+    }
   } else delta = -tr * inv_tauB_cs2;
 
   // S4 Powell source, S5 solid blend (rare: own branch so the blended copy of the state costs no registers
@@ -676,21 +690,29 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
     const real d = (real)solid_state<real, D>(a, c.x, c.y, c.z, c.n, uS, BS);
     real dq = real(0);
     if (d < real(1)) {
-      real Qh[K];
-      solid_blend<SCHEME, D, real>(Qv, a.gamma, d, uS, BS, Qh);
-      flux_row<SCHEME, D, real>(k, Qh, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
+      real Qh[K], Qs[K];
+#pragma unroll
+      for (int l = 0; l < K; l++) Qs[l] = LAZY ? sh.sQ[l][tx] : Qv[LAZY ? 0 : l];
+      solid_blend<SCHEME, D, real>(Qs, a.gamma, d, uS, BS, Qh);
+      const real Qhk = pick<K, real>(Qh, k);
+      flux_row<SCHEME, D, real>(k, Qh, Qhk, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
       // dQh plus the Powell source scaled by the porosity d (A8)
-      dq = pick<K, real>(Qh, k) - Qk;
-      inj = dq - d * (a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
+      dq = Qhk - Qk;
+      inj = dq - d * (a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qs);
       if (has_relax(SCHEME) && k >= 8) inj = -Qk * a.inv_tau_relax;      // relaxation source of Eq.6, not porosity-scaled
       solid = true;
     }
     if (a.body != nullptr) body_accumulate<SCHEME, D, real>(a, c, k, solid, (double)dq, (double)d, (double)Qk);
   }
   if (!solid) {
-    flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
-    inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
-    if (has_relax(SCHEME) && k >= 8) inj = -Qk * a.inv_tau_relax;        // relaxation source of Eq.6
+    if constexpr (LAZY) {
+      flux_row<SCHEME, D, real>(k, qc, Qk, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
+      inj = k < 8 ? -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, qc) : -Qk * a.inv_tau_relax;
+    } else {
+      flux_row<SCHEME, D, real>(k, Qv, Qk, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
+      inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
+      if (has_relax(SCHEME) && k >= 8) inj = -Qk * a.inv_tau_relax;        // relaxation source of Eq.6
+    }
   }
   // in place: cells next to a non-periodic face publish their post-collision moment (sum_i g'_i = Q_k + inj)
   if (STREAM != ST_AB && c.writeM) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + c.n] = (double)(Qk + inj);
@@ -891,8 +913,8 @@ __device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, 
         real Qnb[K], Phi[3];
 #pragma unroll
         for (int l = 0; l < K; l++) Qnb[l] = sh.sNb[l];
-        flux_row<SCHEME, D, real>(k, Qnb, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
         const real Qnbk = pick<K, real>(Qnb, k);
+        flux_row<SCHEME, D, real>(k, Qnb, Qnbk, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
 #pragma unroll
         for (int i = 0; i < Q; i++) {
           if ((edge_lo && L::cx(i) == 1) || (!edge_lo && L::cx(i) == -1)) {
@@ -1058,16 +1080,22 @@ __device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, in
   real b0[NC], P[NC][3];
 #pragma unroll
   for (int c = 0; c < NC; c++) {
-    real Qv[K];
+    constexpr bool LAZY = has_G(SCHEME);      // read the exchanged moments where a row needs them (see finish_cell)
+    const QCol<real, 32 * NC> qc{sQ, c * 32 + tx};
+    real Qv[LAZY ? 1 : K];
+    if constexpr (!LAZY) {
 #pragma unroll
-    for (int l = 0; l < K; l++) Qv[l] = sQ[l][c * 32 + tx];
+      for (int l = 0; l < K; l++) Qv[l] = sQ[l][c * 32 + tx];
+    }
     real delta;
-    if (SCHEME == kIdealD) {
+    if constexpr (SCHEME == kIdealD) {
       delta = Qv[K - 1] * a.inv_tau_relax;
-    } else if (has_G(SCHEME)) {
+    } else if constexpr (has_G(SCHEME)) {
       delta = real(0);
+      if (k < 8) {
 #pragma unroll
-      for (int al = 0; al < D; al++) delta += Qv[8 + 3 * al + al] * a.inv_tau_relax;
+        for (int al = 0; al < D; al++) delta += qc[8 + 3 * al + al] * a.inv_tau_relax;
+      }
     } else {
       real tr = real(0);
 #pragma unroll
@@ -1075,9 +1103,15 @@ __device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, in
       delta = -tr * a.inv_tauB_cs2;
     }
     real Phi[3];
-    flux_row<SCHEME, D, real>(k, Qv, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
-    real inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
-    if (has_relax(SCHEME) && k >= 8) inj = -Qk[c] * a.inv_tau_relax;      // relaxation source of Eq.6
+    real inj;
+    if constexpr (LAZY) {
+      flux_row<SCHEME, D, real>(k, qc, Qk[c], a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
+      inj = k < 8 ? -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, qc) : -Qk[c] * a.inv_tau_relax;
+    } else {
+      flux_row<SCHEME, D, real>(k, Qv, Qk[c], a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
+      inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
+      if (has_relax(SCHEME) && k >= 8) inj = -Qk[c] * a.inv_tau_relax;      // relaxation source of Eq.6
+    }
     if (STREAM != ST_AB && writeM[c]) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + n + c] = (double)(Qk[c] + inj);
     b0[c] = om * Qk[c] + inj;
     P[c][0] = ic * Phi[0]; P[c][1] = ic * Phi[1]; P[c][2] = ic * Phi[2];
@@ -1180,7 +1214,7 @@ init_kernel(const double *__restrict__ fields, real *__restrict__ g, size_t pstr
   real Qv[K], Phi[3];
 #pragma unroll
   for (int l = 0; l < K; l++) Qv[l] = (real)fields[(size_t)l * N + n];
-  flux_row<SCHEME, D, real>(k, Qv, gamma, c0sq, eta, mu, itm, Phi);
+  flux_row<SCHEME, D, real>(k, Qv, pick<K, real>(Qv, k), gamma, c0sq, eta, mu, itm, Phi);
   const real Qk = pick<K, real>(Qv, k);
   real *gk = g + (size_t)k * Q * pstride;
 #pragma unroll
