@@ -17,6 +17,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "lbmhd_lattice.cuh"
 
 namespace lbk {
@@ -138,6 +140,21 @@ template <int K, typename real> __device__ __forceinline__ real pick(const real 
 // Qh is the (possibly solid-blended) state: an array in registers or a column of the shared exchange array (QCol) — the
 // rows read only the entries they need (a gradient row of RESIST / FULL needs 5 of the 17 / 26).  `own` = Qh[k].
 // k is warp-uniform, so the branches do not diverge.
+// Calls f(integral_constant<int, k>) for the run-time row k in [LO, HI) by bisection (k is warp-uniform: no divergence), so
+// that the flux / source code of a row is compiled with k known: no selects, no unused terms.
+template <int LO, int HI, class F> __device__ __forceinline__ void dispatch_row(int k, F &&f) {
+  if constexpr (HI - LO == 1) {
+    f(std::integral_constant<int, LO>{});
+  } else {
+    constexpr int MID = (LO + HI) / 2;
+    if (k < MID) dispatch_row<LO, MID>(k, f);
+    else dispatch_row<MID, HI>(k, f);
+  }
+}
+
+template <int I> __device__ __forceinline__ constexpr int row_of(std::integral_constant<int, I>) { return I; }
+__device__ __forceinline__ constexpr int row_of(int k) { return k; }
+
 template <typename real, int TX> struct QCol {
   real (*s)[TX];
   int tx;
@@ -1078,44 +1095,55 @@ __device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, in
   const real om = a.omega[k], omc = real(1) - om;
   const real ic = real(L::inv_cs2) * om;
   real b0[NC], P[NC][3];
+  // The flux / source code of the NC cells, with the row either a compile-time constant (one copy of the code per row, chosen
+  // by dispatch_row: no selects, no unused terms, but K times the code) or the run-time k.  Measured on B200:
+  // the constant-row form pays where the kernel is bound by instruction issue (fp32; fp64 on the short lattices; the 20 / 26
+  // sets of FULL: +2 .. +6 %) and costs ~1 % where it is at the HBM roof (fp64 D3Q19 / D2Q9 with up to 17 sets); fp32 D3Q7 loses
+  // to spills (0.75 -> 0.70).
+  constexpr bool ROWCONST = sizeof(real) == 8 ? (Q <= 7 || K >= 20) : Q != 7;
+  const auto cells = [&](auto kc) {
+    const int KC = row_of(kc);      // == k
 #pragma unroll
-  for (int c = 0; c < NC; c++) {
-    constexpr bool LAZY = has_G(SCHEME);      // read the exchanged moments where a row needs them (see finish_cell)
-    const QCol<real, 32 * NC> qc{sQ, c * 32 + tx};
-    real Qv[LAZY ? 1 : K];
-    if constexpr (!LAZY) {
+    for (int c = 0; c < NC; c++) {
+      constexpr bool LAZY = has_G(SCHEME);      // read the exchanged moments where a row needs them (see finish_cell)
+      const QCol<real, 32 * NC> qc{sQ, c * 32 + tx};
+      real Qv[LAZY ? 1 : K];
+      if constexpr (!LAZY) {
 #pragma unroll
-      for (int l = 0; l < K; l++) Qv[l] = sQ[l][c * 32 + tx];
-    }
-    real delta;
-    if constexpr (SCHEME == kIdealD) {
-      delta = Qv[K - 1] * a.inv_tau_relax;
-    } else if constexpr (has_G(SCHEME)) {
-      delta = real(0);
-      if (k < 8) {
-#pragma unroll
-        for (int al = 0; al < D; al++) delta += qc[8 + 3 * al + al] * a.inv_tau_relax;
+        for (int l = 0; l < K; l++) Qv[l] = sQ[l][c * 32 + tx];
       }
-    } else {
-      real tr = real(0);
+      real delta;
+      if constexpr (SCHEME == kIdealD) {
+        delta = Qv[K - 1] * a.inv_tau_relax;
+      } else if constexpr (has_G(SCHEME)) {
+        delta = real(0);
+        if (KC < 8) {
 #pragma unroll
-      for (int b = 0; b < D; b++) tr += sTr[b * D + b][c * 32 + tx];
-      delta = -tr * a.inv_tauB_cs2;
+          for (int al = 0; al < D; al++) delta += qc[8 + 3 * al + al] * a.inv_tau_relax;
+        }
+      } else {
+        real tr = real(0);
+#pragma unroll
+        for (int b = 0; b < D; b++) tr += sTr[b * D + b][c * 32 + tx];
+        delta = -tr * a.inv_tauB_cs2;
+      }
+      real Phi[3];
+      real inj;
+      if constexpr (LAZY) {
+        flux_row<SCHEME, D, real>(KC, qc, Qk[c], a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
+        inj = KC < 8 ? -(a.kappa * delta) * powell_row<SCHEME, D, real>(KC, qc) : -Qk[c] * a.inv_tau_relax;
+      } else {
+        flux_row<SCHEME, D, real>(KC, Qv, Qk[c], a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
+        inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(KC, Qv);
+        if (has_relax(SCHEME) && KC >= 8) inj = -Qk[c] * a.inv_tau_relax;      // relaxation source of Eq.6
+      }
+      if (STREAM != ST_AB && writeM[c]) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + n + c] = (double)(Qk[c] + inj);
+      b0[c] = om * Qk[c] + inj;
+      P[c][0] = ic * Phi[0]; P[c][1] = ic * Phi[1]; P[c][2] = ic * Phi[2];
     }
-    real Phi[3];
-    real inj;
-    if constexpr (LAZY) {
-      flux_row<SCHEME, D, real>(k, qc, Qk[c], a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
-      inj = k < 8 ? -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, qc) : -Qk[c] * a.inv_tau_relax;
-    } else {
-      flux_row<SCHEME, D, real>(k, Qv, Qk[c], a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
-      inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(k, Qv);
-      if (has_relax(SCHEME) && k >= 8) inj = -Qk[c] * a.inv_tau_relax;      // relaxation source of Eq.6
-    }
-    if (STREAM != ST_AB && writeM[c]) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + n + c] = (double)(Qk[c] + inj);
-    b0[c] = om * Qk[c] + inj;
-    P[c][0] = ic * Phi[0]; P[c][1] = ic * Phi[1]; P[c][2] = ic * Phi[2];
-  }
+  };
+  if constexpr (ROWCONST) dispatch_row<0, K>(k, cells);
+  else cells(k);
 #pragma unroll
   for (int i = 0; i < Q; i++) {
     real out[NC];
