@@ -655,7 +655,7 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   // 5); the others keep the K moments in registers.
   constexpr bool LAZY = has_G(SCHEME);
   const QCol<real, TX> qc{sh.sQ, tx};
-  real Qv[LAZY ? 1 : K];
+  [[maybe_unused]] real Qv[LAZY ? 1 : K];
   if constexpr (!LAZY) {
 #pragma unroll
     for (int l = 0; l < K; l++) Qv[l] = sh.sQ[l][tx];
@@ -1107,7 +1107,7 @@ __device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, in
     for (int c = 0; c < NC; c++) {
       constexpr bool LAZY = has_G(SCHEME);      // read the exchanged moments where a row needs them (see finish_cell)
       const QCol<real, 32 * NC> qc{sQ, c * 32 + tx};
-      real Qv[LAZY ? 1 : K];
+      [[maybe_unused]] real Qv[LAZY ? 1 : K];
       if constexpr (!LAZY) {
 #pragma unroll
         for (int l = 0; l < K; l++) Qv[l] = sQ[l][c * 32 + tx];
