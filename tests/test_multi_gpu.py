@@ -26,7 +26,11 @@ def env():
 GRIDS = [("D1Q3", (292,), (1, 1, 0, 0, 0, 0)), ("D1Q3", (292,), (0,) * 6),
          ("D2Q5", (292, 9), (2, 1, 0, 0, 0, 0)), ("D2Q9", (292, 9), (0,) * 6), ("D2Q9", (292, 7), (1, 1, 1, 1, 0, 0)),
          ("D3Q7", (292, 6, 5), (0, 0, 1, 1, 0, 0)), ("D3Q19", (292, 6, 5), (2, 1, 0, 0, 0, 0)),
-         ("D3Q19", (292, 5, 6), (0, 0, 0, 0, 1, 1))]
+         ("D3Q19", (292, 5, 6), (0, 0, 0, 0, 1, 1)),
+         # nx a multiple of the tile widths (64, 128), every x-boundary kind
+         ("D1Q3", (384,), (1, 2, 0, 0, 0, 0)), ("D2Q5", (384, 6), (0,) * 6), ("D2Q9", (384, 6), (2, 1, 1, 1, 0, 0)),
+         ("D2Q9", (256, 7), (1, 2, 0, 0, 0, 0)), ("D3Q7", (384, 5, 4), (1, 1, 0, 0, 0, 0)), ("D3Q19", (384, 5, 4), (2, 1, 0, 0, 0, 0)),
+         ("D3Q19", (128, 5, 6), (0,) * 6), ("D3Q19", (256, 4, 5), (1, 2, 0, 0, 1, 1))]
 
 
 @pytest.mark.parametrize("streaming", [0, 1])
@@ -41,7 +45,7 @@ def test_multi_cell_ideal(env, lattice, shape, bc, precision, tol, streaming):
 
 @pytest.mark.parametrize("streaming", [0, 1])
 @pytest.mark.parametrize("precision,tol", [(64, TOL64), (32, TOL32)])
-@pytest.mark.parametrize("lattice,shape,bc", [GRIDS[0], GRIDS[2], GRIDS[4], GRIDS[5], GRIDS[6]])
+@pytest.mark.parametrize("lattice,shape,bc", [GRIDS[0], GRIDS[2], GRIDS[4], GRIDS[5], GRIDS[6], GRIDS[8], GRIDS[10], GRIDS[13], GRIDS[15]])
 def test_multi_cell_other_schemes(env, lattice, shape, bc, precision, tol, streaming):
     env["LBMHD_MULTI"] = "1"
     compare(random_workload("INCRES", lattice, shape, bc, seed=102), 7, tol=tol, precision=precision, streaming=streaming)
@@ -58,8 +62,9 @@ def test_multi_cell_with_sphere(env, precision, tol, streaming):
     sph = dict(centre=np.array([150.0, 8.0, 7.0]), radius=5.0, u_solid=np.array([-0.3, 0.0, 0.0]), dipole_dir=mh,
                B_surface=0.03, width=1.5)
     for lattice in ("D3Q19", "D3Q7"):
-        compare(random_workload("IDEAL", lattice, (292, 16, 14), (2, 1, 0, 0, 0, 0), seed=105, sphere=sph), 8, tol=tol,
-                precision=precision, streaming=streaming)
+        for nx in (292, 384):
+            compare(random_workload("IDEAL", lattice, (nx, 16, 14), (2, 1, 0, 0, 0, 0), seed=105, sphere=sph), 8, tol=tol,
+                    precision=precision, streaming=streaming)
 
 
 def test_multi_cell_is_taken_and_matches_one_cell(env):
