@@ -199,7 +199,9 @@ long long lbmhd_launch_count(const lbmhd_t *h);
 /* Which step kernel the last lbmhd_step launch used: LBMHD_PATH_ONE one cell per thread, LBMHD_PATH_MULTI
  * several cells per thread on interior tiles, LBMHD_PATH_CLUSTER variable rows split over a 2-CTA cluster, LBMHD_PATH_TMA
  * the TMA-staged persistent kernel; -1 before the first step or for a NULL handle.  The choice is made per lattice,
- * scheme, precision and grid size; every path computes the same update. */
+ * scheme, precision and grid size; every path computes the same update.  Environment variables read by lbmhd_create (test and
+ * measurement knobs, never needed for correct use): LBMHD_PAIR=0 one cell per thread everywhere; LBMHD_MULTI=1 the multi-cell
+ * kernel on small grids too; LBMHD_CLUSTER=0 no cluster split; LBMHD_PATH=tma the TMA-staged kernel (fp64 / fp32, A/B only). */
 enum { LBMHD_PATH_ONE = 0, LBMHD_PATH_MULTI = 1, LBMHD_PATH_CLUSTER = 2, LBMHD_PATH_TMA = 3 };
 int lbmhd_step_path(const lbmhd_t *h);
 
