@@ -254,3 +254,27 @@ class Oracle:
     def set_body_reference(self, ref):
         ref = np.ascontiguousarray(ref, dtype=np.float64)
         assert self.lib.oracle_set_body_reference(self.h, _dptr(ref)) == 0
+
+
+LATTICES = {"D1Q3": D1Q3, "D2Q9": D2Q9, "D3Q19": D3Q19, "D2Q5": D2Q5, "D3Q7": D3Q7}
+SCHEMES = {"IDEAL": IDEAL, "INCRES": INCRES, "IDEAL_DIVB": IDEAL_DIVB, "RESIST": RESIST, "FULL": FULL}
+
+
+def from_workload(w, mask=None):
+    """Oracle handle configured (boundaries, tau, sphere) for an input-recipe dict (keys: scheme, lattice, shape, gamma,
+    c0sq, nu, eta, tau, powell, bc, optional tau_relax, eta_jc, sphere); fields not yet initialised.  Marshalling only."""
+    p = make_params(SCHEMES[w["scheme"]], LATTICES[w["lattice"]], w["shape"],
+                    gamma=w["gamma"] or 1.4, c0sq=w["c0sq"], nu=w["nu"], eta=w["eta"], tau=w["tau"],
+                    powell=w["powell"], bc=w["bc"], tau_relax=w.get("tau_relax", 0.0), eta_jc=w.get("eta_jc", 0.0))
+    o = Oracle(p, mask=mask)
+    if w.get("sphere"):
+        s = w["sphere"]
+        o.set_sphere(s["centre"], s["radius"], s["u_solid"], s["dipole_dir"], s["B_surface"])
+        if s.get("width"):
+            o.set_sphere_width(s["width"])
+        if s.get("omega") is not None:
+            o.set_sphere_rotation(s["omega"])
+        if s.get("dipoles"):
+            dp = s["dipoles"]
+            o.set_sphere_dipoles(dp["offsets"], dp["dirs"], dp["B_surface"], dp["cores"])
+    return o

@@ -63,6 +63,7 @@ struct lbmhd {
   bool cluster;          // RESIST on D3Q19, fp64: variable rows of a tile split over a 2-CTA cluster; LBMHD_CLUSTER=0 turns it off
   bool pair;             // several cells per thread on interior tiles (fp32; fp64 on the short lattices); LBMHD_PAIR=0 turns it off
   bool use_tma;          // TMA-staged persistent step kernel (needs nx * sizeof(real) % 16 == 0)
+  bool tma_attr_set;     // its dynamic shared memory attribute has been set on this handle's device
   int num_sms;
   CUtensorMap tmap[2][2];   // [copy][0: tile-wide box, 1: box 16 bytes wider] 5D views (x, y, z, i, k) of the populations
 };

@@ -1435,13 +1435,15 @@ diag_partial_kernel(const double *__restrict__ F, double *__restrict__ partial, 
   if (threadIdx.x == 0) out[3 * K + 3] = r + 2.0 * r2;
 }
 
-// stage 2: one block folds the per-block partials in block order (deterministic)
+// stage 2: one block folds the per-block partials in block order (deterministic).  The flag slot is a bit mask
+// (1 = non-finite seen, 2 = rho <= 0 seen): its two bits fold separately (OR), so NaN in one block and rho <= 0 in
+// another give 3.
 static __global__ void __launch_bounds__(kDiagThreads)
 diag_final_kernel(const double *__restrict__ partial, int nblocks, int K, double *__restrict__ out) {
   __shared__ double sm[32];
   const int nslots = 3 * K + 4;
-  for (int s = 0; s < nslots; s++) {
-    const int kind = s < 2 * K ? 0 : ((s < 3 * K + 1 || s == 3 * K + 3) ? 1 : 2);
+  for (int s = 0; s < nslots - 1; s++) {
+    const int kind = s < 2 * K ? 0 : (s < 3 * K + 1 ? 1 : 2);
     double v = kind == 0 ? 0.0 : (kind == 1 ? -INFINITY : INFINITY);
     for (int b = threadIdx.x; b < nblocks; b += blockDim.x) {
       const double p = partial[(size_t)b * nslots + s];
@@ -1450,6 +1452,15 @@ diag_final_kernel(const double *__restrict__ partial, int nblocks, int K, double
     double r = kind == 0 ? block_reduce<0>(v, sm) : (kind == 1 ? block_reduce<1>(v, sm) : block_reduce<2>(v, sm));
     if (threadIdx.x == 0) out[s] = r;
   }
+  double f_nan = 0.0, f_rho = 0.0;
+  for (int b = threadIdx.x; b < nblocks; b += blockDim.x) {
+    const int bits = (int)partial[(size_t)b * nslots + nslots - 1];
+    if (bits & 1) f_nan = 1.0;
+    if (bits & 2) f_rho = 1.0;
+  }
+  f_nan = block_reduce<1>(f_nan, sm);
+  f_rho = block_reduce<1>(f_rho, sm);
+  if (threadIdx.x == 0) out[nslots - 1] = f_nan + 2.0 * f_rho;
 }
 
 // ---- population import / export: canonical fp64 [K*Q][N] <-> internal real planes with pstride ------------

@@ -100,11 +100,10 @@ template <int LAT, int SCHEME, typename real> struct Ops {
   static cudaError_t launch_step_tma(lbmhd_t *h, const StepArgs<real> &a) {
     using C = TmaCfg<LAT, SCHEME, real, kTmaTX, kTmaStages>;
     auto kern = step_kernel_tma<LAT, SCHEME, real, kTmaTX, kTmaStages>;
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!h->tma_attr_set) {      // the attribute is per device: tracked per handle (a handle is bound to one device)
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
       if (e != cudaSuccess) return e;
-      attr_set = true;
+      h->tma_attr_set = true;
     }
     const int tiles_x = (h->p.nx + kTmaTX - 1) / kTmaTX;
     const long long n_rows = (long long)h->p.ny * h->p.nz;                 // < 2^31 - SMs checked at create

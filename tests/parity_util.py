@@ -3,28 +3,14 @@ import numpy as np
 
 from oracle import oracle as orc
 
-LAT_ORC = {"D1Q3": orc.D1Q3, "D2Q9": orc.D2Q9, "D3Q19": orc.D3Q19, "D2Q5": orc.D2Q5, "D3Q7": orc.D3Q7}
-ORC_SCHEME = {"IDEAL": orc.IDEAL, "INCRES": orc.INCRES, "IDEAL_DIVB": orc.IDEAL_DIVB, "RESIST": orc.RESIST, "FULL": orc.FULL}
+LAT_ORC = orc.LATTICES
+ORC_SCHEME = orc.SCHEMES
 TOL64 = 1e-11      # BASELINE.json north_star: max relative error on all macroscopic fields, fp64
 TOL32 = 1e-5       # fp32
 
 
 def oracle_from_workload(w, mask=None):
-    p = orc.make_params(ORC_SCHEME[w["scheme"]], LAT_ORC[w["lattice"]], w["shape"],
-                        gamma=w["gamma"] or 1.4, c0sq=w["c0sq"], nu=w["nu"], eta=w["eta"], tau=w["tau"],
-                        powell=w["powell"], bc=w["bc"], tau_relax=w.get("tau_relax", 0.0), eta_jc=w.get("eta_jc", 0.0))
-    o = orc.Oracle(p, mask=mask)
-    if w.get("sphere"):
-        s = w["sphere"]
-        o.set_sphere(s["centre"], s["radius"], s["u_solid"], s["dipole_dir"], s["B_surface"])
-        if s.get("width"):
-            o.set_sphere_width(s["width"])
-        if s.get("omega") is not None:
-            o.set_sphere_rotation(s["omega"])
-        if s.get("dipoles"):
-            dp = s["dipoles"]
-            o.set_sphere_dipoles(dp["offsets"], dp["dirs"], dp["B_surface"], dp["cores"])
-    return o
+    return orc.from_workload(w, mask=mask)
 
 
 def field_errors(Q, Qref):

@@ -5,12 +5,11 @@ the domain, a zero-gradient cut elsewhere, kept > n cells away from the sample).
 import numpy as np
 import pytest
 
-from oracle import oracle as orc
 from paper_2606_00641_b200 import workloads as W
-from parity_util import LAT_ORC, TOL64
+from parity_util import oracle_from_workload, TOL64
 
 pytestmark = pytest.mark.gpu
-NSTEPS = 4
+NSTEPS = 20      # the sphere's surface (0.02 cells per step) crosses cell centres and the wake reaches tile seams meanwhile
 MARGIN = NSTEPS + 2
 
 
@@ -35,13 +34,10 @@ def subbox_oracle(w, centre_xyz, nsteps):
         bc[2 * a + 1] = w["bc"][2 * a + 1] if (not periodic and h == n) else 1
     sub = F[:, idx[2]][:, :, idx[1]][:, :, :, idx[0]]
     sub_shape = tuple(len(idx[a]) for a in range(D))
-    p = orc.make_params(orc.IDEAL if w["scheme"] == "IDEAL" else orc.INCRES, LAT_ORC[w["lattice"]], sub_shape,
-                        gamma=w["gamma"] or 1.4, c0sq=w["c0sq"], nu=w["nu"], eta=w["eta"], tau=w["tau"], powell=w["powell"], bc=bc)
-    o = orc.Oracle(p)
-    if w.get("sphere"):
-        s = w["sphere"]
-        cen = np.array(s["centre"], dtype=np.float64) - np.array([lo[0], lo[1], lo[2]], dtype=np.float64)
-        o.set_sphere(cen, s["radius"], s["u_solid"], s["dipole_dir"], s["B_surface"])
+    ws = dict(w, shape=sub_shape, bc=tuple(bc))
+    if w.get("sphere"):      # same body (width, rotation, dipoles included) with its centre in sub-box coordinates
+        ws["sphere"] = dict(w["sphere"], centre=np.array(w["sphere"]["centre"], dtype=np.float64) - np.array(lo, dtype=np.float64))
+    o = oracle_from_workload(ws)
     o.init(np.ascontiguousarray(sub))
     o.step(nsteps)
     Q = o.moments(diag=False)

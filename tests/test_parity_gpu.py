@@ -62,6 +62,12 @@ def compare(w, steps, tol=TOL64, mask=None, obstacle=None, precision=64, streami
     N = Qo[0].size
     bound = tol * np.maximum(1.0, N * do[2 * K:3 * K] / np.maximum(do[K:2 * K], 1e-300))
     assert (e_sum <= bound).all() and (e_abs <= bound).all() and (e_max <= 10 * tol).all()
+    # the reduction kernels themselves, with no oracle round-off in the way: against numpy sums of the fields this very call
+    # returned (deterministic two-stage fold vs numpy's pairwise sum: ~ sqrt(N) eps sum|.|), extrema exactly
+    Fg = Qg.reshape(K, -1)
+    rb = 8 * np.sqrt(N) * np.finfo(np.float64).eps * np.maximum(np.abs(Fg).sum(1), 1e-300)
+    assert (np.abs(dg[:K] - Fg.sum(1)) <= rb).all() and (np.abs(dg[K:2 * K] - np.abs(Fg).sum(1)) <= rb).all()
+    assert (dg[2 * K:3 * K] == np.abs(Fg).max(1)).all()
     assert abs(dg[3 * K] - do[3 * K]) <= 1e3 * tol * max(do[2 * K:3 * K].max(), 1e-300)        # max|div_h B|
     if np.isfinite(do[3 * K + 1]):
         assert abs(dg[3 * K + 1] - do[3 * K + 1]) <= 10 * tol * abs(do[3 * K + 1])             # min rho
