@@ -86,7 +86,7 @@ typedef struct {
                            after lbmhd_init; host-pointer population I/O needs LBMHD_STREAM_AB) */
   int    device;        /* CUDA device ordinal */
   void  *stream;        /* cudaStream_t to enqueue on (0 = default stream) */
-  void  *workspace;     /* DEVICE pointer, 256-byte aligned, >= lbmhd_workspace_bytes() bytes */
+  void  *workspace;     /* DEVICE pointer, 256-byte aligned, >= lbmhd_workspace_bytes() (or _min()) bytes */
   size_t workspace_bytes;
 } lbmhd_params;
 
@@ -94,9 +94,12 @@ typedef struct {
 int lbmhd_num_vars(const lbmhd_params *p);
 int lbmhd_num_dirs(const lbmhd_params *p);
 
-/* Device bytes the handle needs: populations (1 or 2 copies of K*Q planes), cell mask, solid field,
- * moments scratch, reduction scratch.  0 on bad input.  Needs no device. */
+/* Device bytes the handle needs: populations (1 or 2 copies of K*Q planes), cell mask, moments scratch, reduction scratch and,
+ * last, the per-cell solid field B_solid (3 N fp64) and porosity field (N fp64).  lbmhd_workspace_bytes_min leaves that
+ * optional tail out: a handle created on such a workspace refuses lbmhd_set_obstacle(B_solid != NULL) and
+ * lbmhd_set_porosity with LBMHD_ENOMEM and is otherwise identical (config 5: 0.8 GB less).  0 on bad input.  Needs no device. */
 size_t lbmhd_workspace_bytes(const lbmhd_params *p);
+size_t lbmhd_workspace_bytes_min(const lbmhd_params *p);
 
 /* Validates *p, lays the workspace out, uploads `cell_mask` (HOST uint8 [N], values LBMHD_CELL_*, or
  * NULL = all FLUID).  Cells on a face whose kind is LBMHD_BC_INFLOW are FROZEN whatever the mask says (A10). */
@@ -111,7 +114,9 @@ int lbmhd_init(lbmhd_t *h, const double *fields, int on_device);
 
 /* n_steps >= 0 applications of the fused update (pull-stream, moments, div-B estimate, Powell source,
  * solid blend, flux, BGK + injection, store: DESIGN.md §2), asynchronous on the stream.  A sphere set
- * by lbmhd_set_sphere advances its centre by u_solid per step. */
+ * by lbmhd_set_sphere advances its centre by u_solid per step.  On small lattices (launch-latency bound: BASELINE configs
+ * 1 and 2) a call with n_steps >= 2 runs all its steps in ONE cooperative launch (LBMHD_PATH_PERSIST);
+ * larger lattices launch one kernel per step.  The results do not depend on which. */
 int lbmhd_step(lbmhd_t *h, int n_steps);
 
 /* Q_k(x) = sum_i g_{k,i}(x) of the stored populations into fields_out (fp64 [K][N], NULL to skip) and the
@@ -146,17 +151,43 @@ int lbmhd_set_sphere_width(lbmhd_t *h, double eps);
  * step; the dipole axis rotates with the body about omega, counted from the step lbmhd_set_sphere was called at. */
 int lbmhd_set_sphere_rotation(lbmhd_t *h, const double omega[3]);
 
-/* Slab decomposition along the slowest lattice axis (z in 3D, y in 2D), one slab per GPU, A/B streaming.
- * A face of kind LBMHD_BC_HALO carries a ghost plane: its cells are never updated or counted here, owned cells pull from
- * them.  Before EVERY step the caller refreshes both ghost planes with the neighbour's data:
- *   lbmhd_halo_pack(h, side, full, buf)    owned plane next to the ghost on `side` (0 low, 1 high) -> DEVICE buf
- *   lbmhd_halo_unpack(h, side, full, buf)  DEVICE buf (packed by the neighbour on its opposite side) -> ghost plane on `side`
- * full = 0 moves only the Q/3-ish directions that cross the face (what a step needs: 5 of 19 on D3Q19), full = 1 all Q
- * directions (needed before lbmhd_moments so that div_h B sees the neighbour's field).  Buffer layout [K][ndir][plane],
- * element type = `precision`, lbmhd_halo_bytes(h, full) bytes.  All calls are asynchronous on the stream. */
-size_t lbmhd_halo_bytes(const lbmhd_t *h, int full);
-int lbmhd_halo_pack(lbmhd_t *h, int side, int full, void *buf);
-int lbmhd_halo_unpack(lbmhd_t *h, int side, int full, const void *buf);
+/* Slab decomposition along the slowest lattice axis (z in 3D, y in 2D), one slab per GPU (the paper's own runs use
+ * two GPUs).  A face of kind LBMHD_BC_HALO carries a ghost plane: its cells are never updated or counted here,
+ * owned cells pull from them.  The caller moves the crossing populations between neighbouring slabs:
+ *   lbmhd_halo_pack(h, side, what, buf)    plane on `side` (0 low, 1 high) -> DEVICE buf
+ *   lbmhd_halo_unpack(h, side, what, buf)  DEVICE buf (packed by the neighbour on its opposite side) -> plane on `side`
+ * `what`:
+ *   LBMHD_HALO_CROSSING  pack reads the owned plane next to the ghost, the directions that leave through the face (5 of 19 on
+ *                        D3Q19); unpack writes them into the ghost plane.  A/B streaming: before EVERY step.  In place: before
+ *                        every pull-push step (even step count since lbmhd_init / lbmhd_set_populations).
+ *   LBMHD_HALO_FULL      the same planes, all Q directions (A/B only; before lbmhd_moments so that div_h B sees the neighbour's
+ *                        field — or exchange the ghost planes of the FIELDS and call lbmhd_diagnostics, which works in both
+ *                        streaming modes).
+ *   LBMHD_HALO_RETURN    in place only, after every pull-push step and before the local step that follows: the boundary cells
+ *                        pushed their outgoing populations into the ghost plane; pack reads them there, unpack writes them
+ *                        into the neighbour's owned plane next to its ghost (the slots its local step reads).
+ * Buffer layout [K][ndir][plane], element type = `precision`, lbmhd_halo_bytes(h, what) bytes.  All calls are asynchronous on
+ * the handle's stream; the _on variants run on `stream` instead and, with next_copy != 0, act on the population copy the
+ * step IN PROGRESS writes (see lbmhd_step_part), so that the exchange overlaps the interior update. */
+enum { LBMHD_HALO_CROSSING = 0, LBMHD_HALO_FULL = 1, LBMHD_HALO_RETURN = 2 };
+size_t lbmhd_halo_bytes(const lbmhd_t *h, int what);
+int lbmhd_halo_pack(lbmhd_t *h, int side, int what, void *buf);
+int lbmhd_halo_unpack(lbmhd_t *h, int side, int what, const void *buf);
+int lbmhd_halo_pack_on(lbmhd_t *h, int side, int what, void *buf, int next_copy, void *stream);
+int lbmhd_halo_unpack_on(lbmhd_t *h, int side, int what, const void *buf, int next_copy, void *stream);
+
+/* One step in pieces: the fused update of lbmhd_step restricted to the planes [plane_lo, plane_hi) of the slowest lattice
+ * axis (local indices, ghost planes included in the count; an empty range launches nothing).  The pieces of one step must
+ * cover every owned plane exactly once; the call with last != 0 completes the step (flips the copies / the in-place layout,
+ * advances the step counter and the body).  Meant for slabs: update the two planes next to the ghosts first, start their
+ * exchange with lbmhd_halo_*_on(next_copy = 1) on another stream, update the interior planes meanwhile.
+ * Every piece reads only the state before the step, so the result is identical to one lbmhd_step(h, 1). */
+int lbmhd_step_part(lbmhd_t *h, int plane_lo, int plane_hi, int last);
+
+/* The diagnostics of lbmhd_moments (same 3K+4 slots) computed from a DEVICE fields array [K][N] the caller provides — e.g. the
+ * output of lbmhd_moments(on_device) after the ghost planes of the FIELDS were refreshed from the neighbouring slabs.
+ * diag_out HOST (synchronises, returns LBMHD_ENUMERIC on a flag) or DEVICE per on_device. */
+int lbmhd_diagnostics(lbmhd_t *h, const double *fields, double *diag_out, int on_device);
 
 /* Dipole ensemble of the sphere ("an analytical ensemble of four independent, shifted, and smoothed magnetic
  * dipoles"): replaces the single dipole of lbmhd_set_sphere (call that first) by n in 1..4 dipoles fixed in the body frame,
@@ -198,16 +229,24 @@ long long lbmhd_launch_count(const lbmhd_t *h);
 
 /* Which step kernel the last lbmhd_step launch used: LBMHD_PATH_ONE one cell per thread, LBMHD_PATH_MULTI
  * several cells per thread on interior tiles, LBMHD_PATH_CLUSTER variable rows split over a 2-CTA cluster, LBMHD_PATH_TMA
- * the TMA-staged persistent kernel; -1 before the first step or for a NULL handle.  The choice is made per lattice,
- * scheme, precision and grid size; every path computes the same update.  Environment variables read by lbmhd_create (test and
- * measurement knobs, never needed for correct use): LBMHD_PAIR=0 one cell per thread everywhere; LBMHD_MULTI=1 the multi-cell
- * kernel on small grids too; LBMHD_CLUSTER=0 no cluster split; LBMHD_PATH=tma the TMA-staged kernel (fp64 / fp32, A/B only). */
-enum { LBMHD_PATH_ONE = 0, LBMHD_PATH_MULTI = 1, LBMHD_PATH_CLUSTER = 2, LBMHD_PATH_TMA = 3 };
+ * the TMA-staged persistent kernel, LBMHD_PATH_PERSIST many steps in one cooperative launch; -1 before the first step or for
+ * a NULL handle.  The choice is made per lattice, scheme, precision, grid size and step count; every path computes the same
+ * update.  Environment variables read by lbmhd_create (test and measurement knobs, never needed for correct use):
+ * LBMHD_PAIR=0 one cell per thread everywhere; LBMHD_MULTI=1 the multi-cell kernel on small grids too; LBMHD_CLUSTER=0 no
+ * cluster split; LBMHD_PATH=tma the TMA-staged kernel (fp64 / fp32, A/B only); LBMHD_PERSIST=0 one launch per step
+ * everywhere, =2 the cooperative many-step launch whatever the grid size; LBMHD_PERSIST_WAVES=n its size threshold (tiles <=
+ * n x co-resident blocks); LBMHD_CELL=0 no cell-per-thread kernel, =2 that kernel on small grids too. */
+enum { LBMHD_PATH_ONE = 0, LBMHD_PATH_MULTI = 1, LBMHD_PATH_CLUSTER = 2, LBMHD_PATH_TMA = 3, LBMHD_PATH_PERSIST = 4,
+       LBMHD_PATH_CELL = 5 /* one thread per cell, all K sets in its registers: the short lattices D1Q3 / D2Q5 / D3Q7 */ };
 int lbmhd_step_path(const lbmhd_t *h);
 
 /* Measured-bandwidth probe (BabelStream-style copy b[i] = a[i] over n fp64 elements, the paper's roofline
  * denominator is such a measurement).  a, b DEVICE pointers; enqueues `reps` launches. */
 int lbmhd_copy_probe(const double *a, double *b, size_t n, int reps, void *stream);
+
+/* Its companion: BabelStream-style triad a[i] = b[i] + s * c[i] over n fp64 elements (two reads and one write per
+ * element: 24 n bytes per launch), the second probe SURVEY.md:546-549 asks for beside the copy.  DEVICE pointers. */
+int lbmhd_triad_probe(double *a, const double *b, const double *c, double s, size_t n, int reps, void *stream);
 
 /* Text of the last error on this thread ("" if none). */
 const char *lbmhd_last_error(void);

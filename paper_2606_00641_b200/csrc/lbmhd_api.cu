@@ -10,7 +10,7 @@
 #include <string>
 
 #include "lbmhd_host.h"
-#include "lbmhd_kernels.cuh"      // halo_plane_kernel, copy_probe_kernel
+#include "lbmhd_kernels.cuh"      // halo_plane_kernel, copy_probe_kernel, triad_probe_kernel
 
 using namespace lbk;
 using namespace lbh;
@@ -66,12 +66,13 @@ bool layout(const lbmhd_params *p, const Geometry &g, Layout *L) {
   L->off_M[0] = off; off += p->streaming == LBMHD_STREAM_INPLACE ? align_up((size_t)g.K * N * 8, 256) : 0;
   L->off_M[1] = off; off += p->streaming == LBMHD_STREAM_INPLACE ? align_up((size_t)g.K * N * 8, 256) : 0;
   L->off_mask = off; off += align_up(N, 256);
-  L->off_bsolid = off; off += align_up(3 * N * 8, 256);
-  L->off_dfield = off; off += align_up(N * 8, 256);
   L->off_partial = off; off += align_up((size_t)kMaxDiagBlocks * (3 * g.K + 4) * 8, 256);
   L->off_diag = off; off += 256;
-  L->off_dirs = off; off += 512;       // direction lists of the halo pack kernels (3 x 32 ints)
+  L->off_dirs = off; off += 1024;      // direction lists of the halo pack kernels (8 x 32 ints)
   L->off_body = off; off += 256;       // body integrals accumulator (14 doubles)
+  L->total_min = off;                  // everything a run without a per-cell solid field / porosity needs
+  L->off_bsolid = off; off += align_up(3 * N * 8, 256);     // optional tail: lbmhd_set_obstacle(B_solid), lbmhd_set_porosity
+  L->off_dfield = off; off += align_up(N * 8, 256);
   L->total = off;
   return true;
 }
@@ -130,6 +131,12 @@ size_t lbmhd_workspace_bytes(const lbmhd_params *p) {
   if (!p || !geometry(p->scheme, p->lattice, &g) || !layout(p, g, &L)) return 0;
   return L.total;
 }
+size_t lbmhd_workspace_bytes_min(const lbmhd_params *p) {
+  Geometry g;
+  Layout L;
+  if (!p || !geometry(p->scheme, p->lattice, &g) || !layout(p, g, &L)) return 0;
+  return L.total_min;
+}
 
 void lbmhd_destroy(lbmhd_t *h) { delete h; }
 
@@ -155,9 +162,10 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
   const int nn[3] = {p->nx, p->ny, p->nz};
   for (int a = 0; a < g.D; a++) {
     const int lo = p->bc[2 * a], hi = p->bc[2 * a + 1];
-    const int top = (a == g.D - 1 && g.D >= 2 && p->streaming == LBMHD_STREAM_AB) ? LBMHD_BC_HALO : LBMHD_BC_INFLOW;
+    const int top = (a == g.D - 1 && g.D >= 2) ? LBMHD_BC_HALO : LBMHD_BC_INFLOW;
     if (lo < 0 || lo > top || hi < 0 || hi > top)
-      return fail(LBMHD_EINVAL, "bad boundary kind on axis %d (HALO: slowest lattice axis, D >= 2, A/B streaming only)", a);
+      return fail(LBMHD_EINVAL, "bad boundary kind on axis %d (HALO: slowest lattice axis, D >= 2)", a);
+    if ((lo == LBMHD_BC_HALO || hi == LBMHD_BC_HALO) && nn[a] < 4) return fail(LBMHD_EINVAL, "a slab needs >= 4 planes (ghosts included)");
     if ((lo == LBMHD_BC_PERIODIC) != (hi == LBMHD_BC_PERIODIC)) return fail(LBMHD_EINVAL, "periodic must be paired on axis %d", a);
     if (lo != LBMHD_BC_PERIODIC && nn[a] < 3) return fail(LBMHD_EINVAL, "non-periodic axis %d needs >= 3 cells", a);
   }
@@ -183,10 +191,11 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
   if (p->eta_jc != 0.0 && !(p->scheme == LBMHD_INCRES && p->eta_jc > 0.0)) { delete h; return fail(LBMHD_EINVAL, "eta_jc needs the INCRES scheme and must be > 0"); }
   if (!p->workspace) { delete h; return fail(LBMHD_EINVAL, "workspace is NULL"); }
   if (((uintptr_t)p->workspace & 255) != 0) { delete h; return fail(LBMHD_ENOMEM, "workspace must be 256-byte aligned"); }
-  if (p->workspace_bytes < L.total) {
+  if (p->workspace_bytes < L.total_min) {
     delete h;
-    return fail(LBMHD_ENOMEM, "workspace has %zu bytes, need %zu", p->workspace_bytes, L.total);
+    return fail(LBMHD_ENOMEM, "workspace has %zu bytes, need %zu (%zu with per-cell solid fields)", p->workspace_bytes, L.total_min, L.total);
   }
+  h->have_solid_store = p->workspace_bytes >= L.total;
   h->ws = (char *)p->workspace;
   h->stream = (cudaStream_t)p->stream;
   cudaError_t e = cudaSetDevice(p->device);
@@ -201,6 +210,16 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     h->cluster = p->scheme == LBMHD_RESIST && g.Q > 9 && p->precision == 64;      // measured: pays there only
     if (const char *e4 = getenv("LBMHD_CLUSTER")) h->cluster = h->cluster && atoi(e4) != 0;
     h->last_path = -1;
+    h->cell = true;
+    h->cell_force = false;
+    if (const char *e8 = getenv("LBMHD_CELL")) { h->cell = atoi(e8) != 0; h->cell_force = atoi(e8) == 2; }
+    h->persist = true;
+    h->persist_force = false;
+    h->persist_waves = 2;
+    if (const char *e6 = getenv("LBMHD_PERSIST")) { h->persist = atoi(e6) != 0; h->persist_force = atoi(e6) == 2; }
+    if (const char *e7 = getenv("LBMHD_PERSIST_WAVES")) h->persist_waves = atoi(e7);
+    h->persist_cluster = true;
+    if (const char *e9 = getenv("LBMHD_PERSIST_CLUSTER")) h->persist_cluster = atoi(e9) != 0;
     h->multi_force = false;
     if (const char *e5 = getenv("LBMHD_MULTI")) h->multi_force = atoi(e5) != 0;
     const char *path = getenv("LBMHD_PATH");      // tuning knob: "plain" forces the register-pull kernel
@@ -265,6 +284,27 @@ int lbmhd_step(lbmhd_t *h, int n_steps) {
   return pick(h).step(h, n_steps);
 }
 
+int lbmhd_step_part(lbmhd_t *h, int plane_lo, int plane_hi, int last) {
+  if (!h) return fail(LBMHD_EINVAL, "NULL handle");
+  const int nH = h->g.D == 3 ? h->p.nz : (h->g.D == 2 ? h->p.ny : 1);
+  if (plane_lo < 0 || plane_hi > nH || plane_lo > plane_hi) return fail(LBMHD_EINVAL, "bad plane range [%d, %d) of %d", plane_lo, plane_hi, nH);
+  if (int rc = use_device(h)) return rc;
+  return pick(h).step_part(h, plane_lo, plane_hi, last);
+}
+
+int lbmhd_diagnostics(lbmhd_t *h, const double *fields, double *diag_out, int on_device) {
+  if (!h || !fields || !diag_out) return fail(LBMHD_EINVAL, "NULL argument");
+  if (int rc = use_device(h)) return rc;
+  const int nd = 3 * h->g.K + 4;
+  double *ddev = on_device ? diag_out : (double *)(h->ws + h->L.off_diag);
+  if (int rc = pick(h).diag(h, fields, ddev)) return rc;
+  if (on_device) return LBMHD_OK;
+  CUDA_TRY(cudaMemcpyAsync(diag_out, ddev, nd * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  if (diag_out[nd - 1] != 0.0) return fail(LBMHD_ENUMERIC, "non-finite value or rho <= 0 seen (flag %g)", diag_out[nd - 1]);
+  return LBMHD_OK;
+}
+
 int lbmhd_moments(lbmhd_t *h, double *fields_out, double *diag_out, int on_device) {
   if (!h) return fail(LBMHD_EINVAL, "NULL handle");
   if (int rc = use_device(h)) return rc;
@@ -292,6 +332,7 @@ int lbmhd_set_obstacle(lbmhd_t *h, const unsigned char *mask, const double u_sol
   if (int rc = use_device(h)) return rc;
   const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   CUDA_TRY(cudaMemcpyAsync(h->ws + h->L.off_mask, mask, h->N, kind, h->stream));
+  if (B_solid && !h->have_solid_store) return fail(LBMHD_ENOMEM, "workspace was sized with lbmhd_workspace_bytes_min: no room for B_solid");
   h->have_mask = true;
   h->have_bsolid = B_solid != nullptr;
   if (B_solid) CUDA_TRY(cudaMemcpyAsync(h->ws + h->L.off_bsolid, B_solid, 3 * h->N * 8, kind, h->stream));
@@ -319,6 +360,7 @@ int lbmhd_set_porosity(lbmhd_t *h, const double *d_field, int on_device) {
   if (!h) return fail(LBMHD_EINVAL, "NULL handle");
   if (int rc = use_device(h)) return rc;
   if (!d_field) { h->have_dfield = false; return LBMHD_OK; }
+  if (!h->have_solid_store) return fail(LBMHD_ENOMEM, "workspace was sized with lbmhd_workspace_bytes_min: no room for the porosity field");
   const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   CUDA_TRY(cudaMemcpyAsync(h->ws + h->L.off_dfield, d_field, h->N * 8, kind, h->stream));
   if (!h->have_mask) {       // the kernels route tiles to the general path on "a mask exists"
@@ -387,45 +429,70 @@ static int halo_dir_list(const lbmhd_t *h, int sign, int *dirs) {      // direct
   return pick(h).halo_dirs(sign, dirs);
 }
 
-size_t lbmhd_halo_bytes(const lbmhd_t *h, int full) {
+size_t lbmhd_halo_bytes(const lbmhd_t *h, int what) {
   if (!h || h->g.D < 2) return 0;
   int dirs[32];
-  const int nd = halo_dir_list(h, full ? 0 : 1, dirs);
+  const int nd = halo_dir_list(h, what == LBMHD_HALO_FULL ? 0 : 1, dirs);
   const size_t plane = h->g.D == 3 ? (size_t)h->p.nx * h->p.ny : (size_t)h->p.nx;
   return (size_t)h->g.K * nd * plane * (h->p.precision == 64 ? 8 : 4);
 }
 
-static int halo_move(lbmhd_t *h, int side, int full, void *buf, bool pack) {
-  if (!h || !buf || side < 0 || side > 1) return fail(LBMHD_EINVAL, "bad argument");
-  if (h->g.D < 2 || h->p.streaming != LBMHD_STREAM_AB) return fail(LBMHD_EINVAL, "halo exchange needs D >= 2 and A/B streaming");
+// LBMHD_HALO_CROSSING  pack: the owned plane next to the ghost, directions that leave through that face (the neighbour pulls
+//                      them); unpack: the ghost plane itself, directions that enter through that face.
+// LBMHD_HALO_FULL      the same planes, all Q directions.
+// LBMHD_HALO_RETURN    in place, after a pull-push step: this slab's boundary cells pushed g'_j (c_j leaving through the face)
+//                      into the ghost plane, at slot opp(j); those values belong in the NEIGHBOUR's owned plane next to its
+//                      ghost, same slots.  pack: the ghost plane, directions that enter through that face (the slots written);
+//                      unpack: the owned plane next to the ghost, directions that leave through that face.
+static int halo_move(lbmhd_t *h, int side, int what, void *buf, bool pack, int next_copy, cudaStream_t stream) {
+  if (!h || !buf || side < 0 || side > 1 || what < 0 || what > 2) return fail(LBMHD_EINVAL, "bad argument");
+  if (h->g.D < 2) return fail(LBMHD_EINVAL, "halo exchange needs D >= 2");
+  const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
+  if (what == LBMHD_HALO_RETURN && !inplace) return fail(LBMHD_EINVAL, "LBMHD_HALO_RETURN is the in-place exchange");
+  if (what == LBMHD_HALO_FULL && inplace) return fail(LBMHD_EINVAL, "LBMHD_HALO_FULL needs A/B streaming (in place: exchange fields, lbmhd_diagnostics)");
   if (int rc = use_device(h)) return rc;
   const int nH = h->g.D == 3 ? h->p.nz : h->p.ny;
   const size_t plane = h->g.D == 3 ? (size_t)h->p.nx * h->p.ny : (size_t)h->p.nx;
-  // pack: the owned plane next to the ghost, directions that leave through that face (the neighbour pulls them);
-  // unpack: the ghost plane itself, directions that enter through that face
-  const int sign = full ? 0 : (pack ? (side == 0 ? -1 : 1) : (side == 0 ? 1 : -1));
-  const int hidx = pack ? (side == 0 ? 1 : nH - 2) : (side == 0 ? 0 : nH - 1);
+  const bool ret = what == LBMHD_HALO_RETURN;
+  const bool from_owned = pack != ret;          // crossing / full: pack reads the owned plane, unpack writes the ghost; return: the reverse
+  const int sign = what == LBMHD_HALO_FULL ? 0 : (from_owned ? (side == 0 ? -1 : 1) : (side == 0 ? 1 : -1));
+  const int hidx = from_owned ? (side == 0 ? 1 : nH - 2) : (side == 0 ? 0 : nH - 1);
   int dirs[32];
   const int nd = halo_dir_list(h, sign, dirs);
-  int *ddev = (int *)(h->ws + h->L.off_dirs) + 32 * (full ? 2 : (sign > 0 ? 1 : 0));
-  CUDA_TRY(cudaMemcpyAsync(ddev, dirs, nd * sizeof(int), cudaMemcpyHostToDevice, h->stream));
+  // one list slot per (kind, sign): the lists are constant, but each call uploads its own so that no call depends on another
+  int *ddev = (int *)(h->ws + h->L.off_dirs) + 32 * (what == LBMHD_HALO_FULL ? 2 : (sign > 0 ? 1 : 0));
+  if (!h->dirs_uploaded[what == LBMHD_HALO_FULL ? 2 : (sign > 0 ? 1 : 0)]) {
+    CUDA_TRY(cudaMemcpyAsync(ddev, dirs, nd * sizeof(int), cudaMemcpyHostToDevice, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));      // once per handle and list: later calls may run on another stream
+    h->dirs_uploaded[what == LBMHD_HALO_FULL ? 2 : (sign > 0 ? 1 : 0)] = true;
+  }
   const size_t total = (size_t)h->g.K * nd * plane;
   const int blocks = (int)((total + 255) / 256 < 1184 ? (total + 255) / 256 : 1184);
-  char *pops = h->ws + h->L.off_pop[h->cur];
+  char *pops = h->ws + h->L.off_pop[inplace ? 0 : (next_copy ? 1 - h->cur : h->cur)];
+  // LBMHD_HALO_RETURN, unpack: skip the slots nobody pushed (the pusher would lie outside a non-periodic in-plane face)
+  const int fx = (ret && !pack && h->p.bc[0] != LBMHD_BC_PERIODIC) ? 1 : 0;
+  const int fy = (ret && !pack && h->g.D == 3 && h->p.bc[2] != LBMHD_BC_PERIODIC) ? 1 : 0;
+  const int pny = h->g.D == 3 ? h->p.ny : 1;
   if (h->p.precision == 64) {
-    if (pack) halo_plane_kernel<double, true><<<blocks, 256, 0, h->stream>>>((double *)pops, h->L.pstride, (double *)buf, plane, (size_t)hidx * plane, h->g.K, h->g.Q, nd, ddev);
-    else halo_plane_kernel<double, false><<<blocks, 256, 0, h->stream>>>((double *)pops, h->L.pstride, (double *)buf, plane, (size_t)hidx * plane, h->g.K, h->g.Q, nd, ddev);
+    if (pack) halo_plane_kernel<double, true><<<blocks, 256, 0, stream>>>((double *)pops, h->L.pstride, (double *)buf, plane, (size_t)hidx * plane, h->g.K, h->g.Q, nd, ddev, h->p.nx, pny, fx, fy);
+    else halo_plane_kernel<double, false><<<blocks, 256, 0, stream>>>((double *)pops, h->L.pstride, (double *)buf, plane, (size_t)hidx * plane, h->g.K, h->g.Q, nd, ddev, h->p.nx, pny, fx, fy);
   } else {
-    if (pack) halo_plane_kernel<float, true><<<blocks, 256, 0, h->stream>>>((float *)pops, h->L.pstride, (float *)buf, plane, (size_t)hidx * plane, h->g.K, h->g.Q, nd, ddev);
-    else halo_plane_kernel<float, false><<<blocks, 256, 0, h->stream>>>((float *)pops, h->L.pstride, (float *)buf, plane, (size_t)hidx * plane, h->g.K, h->g.Q, nd, ddev);
+    if (pack) halo_plane_kernel<float, true><<<blocks, 256, 0, stream>>>((float *)pops, h->L.pstride, (float *)buf, plane, (size_t)hidx * plane, h->g.K, h->g.Q, nd, ddev, h->p.nx, pny, fx, fy);
+    else halo_plane_kernel<float, false><<<blocks, 256, 0, stream>>>((float *)pops, h->L.pstride, (float *)buf, plane, (size_t)hidx * plane, h->g.K, h->g.Q, nd, ddev, h->p.nx, pny, fx, fy);
   }
   CUDA_TRY(cudaGetLastError());
   h->launches += 1;
   return LBMHD_OK;
 }
 
-int lbmhd_halo_pack(lbmhd_t *h, int side, int full, void *buf) { return halo_move(h, side, full, buf, true); }
-int lbmhd_halo_unpack(lbmhd_t *h, int side, int full, const void *buf) { return halo_move(h, side, full, (void *)buf, false); }
+int lbmhd_halo_pack(lbmhd_t *h, int side, int what, void *buf) { return halo_move(h, side, what, buf, true, 0, h ? h->stream : 0); }
+int lbmhd_halo_unpack(lbmhd_t *h, int side, int what, const void *buf) { return halo_move(h, side, what, (void *)buf, false, 0, h ? h->stream : 0); }
+int lbmhd_halo_pack_on(lbmhd_t *h, int side, int what, void *buf, int next_copy, void *stream) {
+  return halo_move(h, side, what, buf, true, next_copy, (cudaStream_t)stream);
+}
+int lbmhd_halo_unpack_on(lbmhd_t *h, int side, int what, const void *buf, int next_copy, void *stream) {
+  return halo_move(h, side, what, (void *)buf, false, next_copy, (cudaStream_t)stream);
+}
 
 static int pops_io(lbmhd_t *h, double *out, const double *in, int on_device) {
   if (!h || (!out && !in)) return fail(LBMHD_EINVAL, "NULL argument");
@@ -456,6 +523,15 @@ int lbmhd_copy_probe(const double *a, double *b, size_t n, int reps, void *strea
   if (!a || !b || reps < 0) return fail(LBMHD_EINVAL, "bad argument");
   for (int r = 0; r < reps; r++) {
     copy_probe_kernel<<<148 * 8, 256, 0, (cudaStream_t)stream>>>((const double2 *)a, (double2 *)b, n / 2);
+    CUDA_TRY(cudaGetLastError());
+  }
+  return LBMHD_OK;
+}
+
+int lbmhd_triad_probe(double *a, const double *b, const double *c, double s, size_t n, int reps, void *stream) {
+  if (!a || !b || !c || reps < 0) return fail(LBMHD_EINVAL, "bad argument");
+  for (int r = 0; r < reps; r++) {
+    triad_probe_kernel<<<148 * 8, 256, 0, (cudaStream_t)stream>>>((double2 *)a, (const double2 *)b, (const double2 *)c, s, n / 2);
     CUDA_TRY(cudaGetLastError());
   }
   return LBMHD_OK;

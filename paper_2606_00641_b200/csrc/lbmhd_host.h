@@ -30,7 +30,7 @@ constexpr int kTmaTX = 32, kTmaStages = 5;
 struct Layout {
   size_t pstride;        // elements per population plane (N rounded up to 32)
   size_t pop_bytes;      // one population copy
-  size_t off_pop[2], off_fields, off_M[2], off_mask, off_bsolid, off_dfield, off_partial, off_diag, off_dirs, off_body, total;
+  size_t off_pop[2], off_fields, off_M[2], off_mask, off_bsolid, off_dfield, off_partial, off_diag, off_dirs, off_body, total_min, total;
 };
 
 }  // namespace lbh
@@ -50,6 +50,8 @@ struct lbmhd {
   long long launches;
   int last_path;         // LBMHD_PATH_* of the last step launch, -1 before the first
   bool have_mask, have_bsolid, have_dfield;
+  bool have_solid_store; // the workspace holds the optional tail (B_solid, porosity field)
+  bool dirs_uploaded[3]; // halo direction lists present on the device
   bool body_on;          // body integrals accumulate during the steps
   double body_ref[3];
   double usolid[3];
@@ -62,6 +64,12 @@ struct lbmhd {
   bool multi_force;      // LBMHD_MULTI=1: take the multi-cell kernel on small grids too (tests)
   bool cluster;          // RESIST on D3Q19, fp64: variable rows of a tile split over a 2-CTA cluster; LBMHD_CLUSTER=0 turns it off
   bool pair;             // several cells per thread on interior tiles (fp32; fp64 on the short lattices); LBMHD_PAIR=0 turns it off
+  bool cell;             // one thread per cell on the short lattices (LBMHD_CELL=0 turns it off)
+  bool cell_force;       // LBMHD_CELL=2: on small grids too (tests)
+  bool persist;          // many steps of a small lattice in one cooperative launch (LBMHD_PERSIST=0 turns it off)
+  bool persist_force;    // LBMHD_PERSIST=2: take it whatever the lattice size (tests, measurements)
+  bool persist_cluster;  // lattices of <= 16 64-cell tiles: the one-cluster variant with the hardware barrier (LBMHD_PERSIST_CLUSTER=0 turns it off)
+  int persist_waves;     // taken when tiles <= persist_waves x co-resident blocks (LBMHD_PERSIST_WAVES)
   bool use_tma;          // TMA-staged persistent step kernel (needs nx * sizeof(real) % 16 == 0)
   bool tma_attr_set;     // its dynamic shared memory attribute has been set on this handle's device
   int num_sms;
@@ -72,6 +80,7 @@ namespace lbh {
 
 struct OpTable {
   int (*step)(lbmhd_t *, int);
+  int (*step_part)(lbmhd_t *, int, int, int);
   int (*init)(lbmhd_t *, const double *);
   int (*moments)(lbmhd_t *, double *);
   int (*diag)(lbmhd_t *, const double *, double *);

@@ -51,6 +51,8 @@ template <typename real> struct StepArgs {
                                 //   state of frozen cells); nullptr in A/B mode
   double *M_next;               // in-place modes: moments published by this step
   int hoff;                     // slab decomposition: global index of local plane 0 along the slowest lattice axis
+  int row0, row1;               // planes [row0, row1) of the slowest lattice axis this launch covers (lbmhd_step_part: a plane range)
+  long long kplane;             // Q * pstride * sizeof(real): bytes from plane (k, i) to plane (k + 1, i)
   int has_sphere;
   double sph_c[3], sph_R, sph_R2, sph_u[3];
   double sph_om[3];             // angular velocity of the body: u^B = sph_u + sph_om x r
@@ -973,7 +975,8 @@ step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int 
   __shared__ real sNb[K];
   const Share<real, TX, false> sh{sQ, sTr, sNb, nullptr, nullptr, nullptr, SyncBlock{}};
   run_tile<LAT, SCHEME, real, TX, MODE, STREAM>(a, threadIdx.x, threadIdx.y, (r.bx0 + (int)blockIdx.x * r.bxs) * TX,
-                                                r.y0 + (int)blockIdx.y * r.ys, r.z0 + (int)blockIdx.z * r.zs, sphere_only, sh);
+                                                r.y0 + (int)blockIdx.y * r.ys + (D == 2 ? a.row0 : 0),
+                                                r.z0 + (int)blockIdx.z * r.zs + (D == 3 ? a.row0 : 0), sphere_only, sh);
 }
 
 // The same step with the K rows of a tile split over a 2-CTA cluster (Share<.., CL = true>): CTA `rank` owns rows
@@ -995,7 +998,8 @@ step_kernel_cl(const __grid_constant__ StepArgs<real> a) {
   cg::cluster_group cl = cg::this_cluster();
   const Share<real, 32, true> sh{sQ, sTr, sNb, cl.map_shared_rank(sQ, rank ^ 1u), cl.map_shared_rank(sTr, rank ^ 1u),
                                  cl.map_shared_rank(sNb, rank ^ 1u), SyncBlock{}};
-  run_tile<LAT, SCHEME, real, 32, 0, STREAM>(a, threadIdx.x, k, (int)(blockIdx.x >> 1) * 32, blockIdx.y, blockIdx.z, 0, sh);
+  run_tile<LAT, SCHEME, real, 32, 0, STREAM>(a, threadIdx.x, k, (int)(blockIdx.x >> 1) * 32, (int)blockIdx.y + (D == 2 ? a.row0 : 0),
+                                             (int)blockIdx.z + (D == 3 ? a.row0 : 0), 0, sh);
 }
 
 // =====================================================================================================
@@ -1173,7 +1177,7 @@ step_kernel_multi(const __grid_constant__ StepArgs<real> a, const int nmulti) {
   __shared__ real sNb[K];
   const int tx = threadIdx.x, k = threadIdx.y;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
-  const int y = blockIdx.y, z = blockIdx.z;
+  const int y = (int)blockIdx.y + (D == 2 ? a.row0 : 0), z = (int)blockIdx.z + (D == 3 ? a.row0 : 0);
   if (ghost_row<real, D>(a, y, z)) return;
   const Share<real, 32, false> sh32{reinterpret_cast<real(*)[32]>(&sQ[0][0]), reinterpret_cast<real(*)[32]>(&sTr[0][0]), sNb,
                                     nullptr, nullptr, nullptr, SyncBlock{}};
@@ -1224,6 +1228,196 @@ step_kernel_multi(const __grid_constant__ StepArgs<real> a, const int nmulti) {
   for (int s = 0; s < NC; s++) {
     if (s) __syncthreads();
     if (x0 + 32 * s < nx) run_tile<LAT, SCHEME, real, 32, 0, STREAM>(a, tx, k, x0 + 32 * s, y, z, 0, sh32);
+  }
+}
+
+// =====================================================================================================
+// One thread per CELL on the short lattices: D2Q5 / D3Q7 / D1Q3 carry K*Q = 40 / 56 / 24 populations per
+// cell, which fit one thread's registers in both precisions, so the mapping north_star names applies: the flux, the Powell
+// source and the primitives (1/rho, u, p_tot, u.B) are evaluated ONCE per cell and shared by the K variable sets in registers
+// (the paper's CSE lesson), with no shared memory and no barrier.  With one thread per (cell, variable)
+// those lattices were bound by instruction issue (ncu: ~230 warp instructions per (cell, variable), K-fold repeated flux
+// arithmetic).  A block keeps the 32 x K thread shape of the other kernels and owns RY = 32 K / WX rows of WX cells; each warp
+// is 32 consecutive x of one row, so every access is a coalesced row segment of one plane.  Interior fluid tiles only:
+// everything else (faces, wrap, mask, sphere, the 32-cell end pieces of a row) goes through run_tile() piece by piece.
+// =====================================================================================================
+template <int LAT, int SCHEME, typename real, int WX, int MINB, int STREAM>
+__global__ void __launch_bounds__(32 * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
+step_kernel_cell(const __grid_constant__ StepArgs<real> a, const int ncell) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, Q = L::Q;
+  using V = Vars<SCHEME, D>;
+  constexpr int K = V::K, iB = V::iB, RY = 32 * K / WX;
+  static_assert((32 * K) % WX == 0 && WX % 32 == 0 && (D > 1 || RY == 1), "tile shape");
+  __shared__ real sQ[K][32];
+  __shared__ real sTr[D * D][32];
+  __shared__ real sNb[K];
+  const Share<real, 32, false> sh32{sQ, sTr, sNb, nullptr, nullptr, nullptr, SyncBlock{}};
+  const int tx = threadIdx.x, k = threadIdx.y;
+  const int nx = a.nx, ny = a.ny, nz = a.nz;
+  const int y0 = D == 1 ? 0 : (int)blockIdx.y * RY + (D == 2 ? a.row0 : 0);
+  const int yend = D == 1 ? 1 : (D == 2 ? a.row1 : ny);
+  const int z = D == 3 ? (int)blockIdx.z + a.row0 : 0;
+  if ((int)blockIdx.x >= ncell) {      // 32-cell pieces: the tile at the x = 0 end and what follows the cell tiles
+    const int t = (int)blockIdx.x - ncell;
+    const int x0 = t == 0 ? 0 : 32 + WX * ncell + 32 * (t - 1);
+#pragma unroll 1
+    for (int r = 0; r < RY; r++) {
+      if (y0 + r >= yend) break;
+      if (r) __syncthreads();
+      run_tile<LAT, SCHEME, real, 32, 0, STREAM>(a, tx, k, x0, y0 + r, z, 0, sh32);
+    }
+    return;
+  }
+  const int x0 = 32 + (int)blockIdx.x * WX;
+  const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
+  bool fast = a.mask == nullptr && x0 + WX <= nx - 1 && (D < 2 || (y0 >= 1 && y0 + RY - 1 <= ny - 2 && y0 + RY <= yend)) &&
+              (D < 3 || (z >= 1 && z <= nz - 2));
+  if (fast && a.has_sphere) {
+#pragma unroll 1
+    for (int r = 0; r < RY; r++) fast = fast && !sphere_may_touch<real, D>(a, x0, WX, y0 + r, z);
+  }
+  if (!fast) {
+#pragma unroll 1
+    for (int r = 0; r < RY; r++) {
+      if (y0 + r >= yend) break;
+#pragma unroll 1
+      for (int p = 0; p < WX / 32; p++) {
+        if (r || p) __syncthreads();
+        if (x0 + 32 * p < nx) run_tile<LAT, SCHEME, real, 32, 0, STREAM>(a, tx, k, x0 + 32 * p, y0 + r, z, 0, sh32);
+      }
+    }
+    return;
+  }
+  // ---- interior fluid tile: this thread owns one cell and all its K sets ----
+  const int tid = k * 32 + tx;
+  const int x = x0 + tid % WX, y = y0 + tid / WX;
+  const uint32_t n = ((uint32_t)z * ny + y) * nx + x;
+  char *__restrict__ pb = reinterpret_cast<char *>(const_cast<real *>(a.src) + n);
+  real f[K][Q];
+#pragma unroll
+  for (int l = 0; l < K; l++)
+#pragma unroll
+    for (int i = 0; i < Q; i++)
+      f[l][i] = *reinterpret_cast<const real *>(pb + (long long)l * a.kplane + (STREAM == ST_LOC ? a.st_off[opp(i)] : a.ld_off[i]));
+  real Qv[K];
+#pragma unroll
+  for (int l = 0; l < K; l++) {      // S2 zeroth moments, index order
+    real s = real(0);
+#pragma unroll
+    for (int i = 0; i < Q; i++) s += f[l][i];
+    Qv[l] = s;
+  }
+  real delta;                        // S3 (A6) or the relaxation variable (A19)
+  if constexpr (SCHEME == kIdealD) {
+    delta = Qv[K - 1] * a.inv_tau_relax;
+  } else {
+    real tr = real(0);
+#pragma unroll
+    for (int b = 0; b < D; b++) {
+      real m = real(0);
+#pragma unroll
+      for (int i = 0; i < Q; i++)
+        if (lat_c<L>(i, b) != 0) m += real(lat_c<L>(i, b)) * f[iB + b][i];
+      tr += m;
+    }
+    delta = -tr * a.inv_tauB_cs2;
+  }
+  const bool wM = STREAM != ST_AB && (((npy && (y == 1 || y == ny - 2)) || (npz && (z == 1 || z == nz - 2))) || (npx && x == nx - 2));
+  char *__restrict__ ob = STREAM == ST_AB ? reinterpret_cast<char *>(a.dst + n) : pb;
+#pragma unroll
+  for (int l = 0; l < K; l++) {      // S4, S6-S8 row by row; the compiler shares 1/rho, u, p_tot, u.B across the rows
+    real Phi[3];
+    flux_row<SCHEME, D, real>(l, Qv, Qv[l], a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
+    real inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(l, Qv);
+    if (has_relax(SCHEME) && l >= 8) inj = -Qv[l] * a.inv_tau_relax;
+    if (STREAM != ST_AB && wM) a.M_next[(size_t)l * ((size_t)nx * ny * nz) + n] = (double)(Qv[l] + inj);
+    const real om = a.omega[l], omc = real(1) - om;
+    const real b0 = om * Qv[l] + inj;
+    const real P0 = real(L::inv_cs2) * om * Phi[0], P1 = real(L::inv_cs2) * om * Phi[1], P2 = real(L::inv_cs2) * om * Phi[2];
+#pragma unroll
+    for (int i = 0; i < Q; i++) {
+      real t = real(L::w(i)) * b0;
+      if (L::cx(i) != 0) t = fma(real(L::cx(i) * L::w(i)), P0, t);
+      if (L::cy(i) != 0) t = fma(real(L::cy(i) * L::w(i)), P1, t);
+      if (L::cz(i) != 0) t = fma(real(L::cz(i) * L::w(i)), P2, t);
+      *reinterpret_cast<real *>(ob + (long long)l * a.kplane + (STREAM == ST_PP ? a.ld_off[opp(i)] : a.st_off[i])) = fma(f[l][i], omc, t);
+    }
+  }
+}
+
+// =====================================================================================================
+// Many steps in ONE launch: small lattices (config 1: 25 tiles, config 2: 8192) are bound by the
+// launch-to-launch latency and by the fill and drain of every launch, not by HBM.  A cooperative grid of at most the
+// co-resident block count loops over the tiles of a step (run_tile, the one-cell paths), meets at a grid barrier, flips the
+// population copies (A/B) or the step type (in place) and goes on.  The per-step part of the arguments (copies, published
+// moment arrays, sphere centre) lives in a shared-memory copy of StepArgs that thread 0 updates between steps.
+// =====================================================================================================
+template <typename real> struct PersistArgs {
+  int n_steps;
+  int inplace, parity0;         // in place: the first step is a pull-push step (parity 0) or a local step (1)
+  real *pop[2];                 // A/B: pop[0] is read by the first step; in place: both the single copy
+  double *M[2];                 // in place: M[0] is M_cur of the first step
+  long long t_rel0;             // sphere: steps since lbmhd_set_sphere at the first step
+  double sph_c0[3];             // sphere centre when it was set (A12: centre before step t is c0 + (t - t0) u)
+  int tiles_x;
+  long long n_tiles;            // tiles_x * ny * nz
+};
+
+// CLBAR = false: a cooperative launch of any size, grid barrier between the steps.
+// CLBAR = true:  the whole lattice fits ONE thread-block cluster (at most 16 CTAs of TX = 64 cells: config 1's 800 cells):
+//                the barrier between the steps is the cluster's hardware barrier (release / acquire: the stores of a step
+//                are visible to the pulls of the next), several times faster than a grid barrier through global memory.
+template <int LAT, int SCHEME, typename real, int TX, int MINB, bool INPLACE, bool CLBAR>
+__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
+step_kernel_persist(const __grid_constant__ StepArgs<real> a0, const __grid_constant__ PersistArgs<real> p) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, K = Vars<SCHEME, D>::K;
+  __shared__ real sQ[K][TX];
+  __shared__ real sTr[D * D][TX];
+  __shared__ real sNb[K];
+  __shared__ StepArgs<real> sa;
+  static_assert(sizeof(StepArgs<real>) % 4 == 0, "word copy");
+  namespace cg = cooperative_groups;
+  const int tid = threadIdx.y * TX + threadIdx.x, nthr = TX * K;
+  {
+    const uint32_t *src = reinterpret_cast<const uint32_t *>(&a0);
+    uint32_t *dst = reinterpret_cast<uint32_t *>(&sa);
+    for (int j = tid; j < (int)(sizeof(StepArgs<real>) / 4); j += nthr) dst[j] = src[j];
+  }
+  const Share<real, TX, false> sh{sQ, sTr, sNb, nullptr, nullptr, nullptr, SyncBlock{}};
+  for (int s = 0; s < p.n_steps; s++) {
+    __syncthreads();
+    if (tid == 0) {
+      sa.src = p.pop[s & 1];
+      sa.dst = p.pop[(s & 1) ^ 1];
+      sa.M_cur = INPLACE ? p.M[s & 1] : nullptr;
+      sa.M_next = INPLACE ? p.M[(s & 1) ^ 1] : nullptr;
+      if (a0.has_sphere) {
+        const double dt = (double)(p.t_rel0 + s);
+#pragma unroll
+        for (int c = 0; c < 3; c++) sa.sph_c[c] = __dadd_rn(p.sph_c0[c], __dmul_rn(dt, a0.sph_u[c]));
+      }
+    }
+    __syncthreads();
+    const bool pullpush = INPLACE && (((p.parity0 + s) & 1) == 0);
+    for (long long tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x) {
+      const int bx = (int)(tile % p.tiles_x);
+      const long long row = tile / p.tiles_x;
+      const int y = (int)(row % a0.ny), z = (int)(row / a0.ny);
+      if constexpr (!INPLACE) run_tile<LAT, SCHEME, real, TX, 0, ST_AB>(sa, threadIdx.x, threadIdx.y, bx * TX, y, z, 0, sh);
+      else if (pullpush) run_tile<LAT, SCHEME, real, TX, 0, ST_PP>(sa, threadIdx.x, threadIdx.y, bx * TX, y, z, 0, sh);
+      else run_tile<LAT, SCHEME, real, TX, 0, ST_LOC>(sa, threadIdx.x, threadIdx.y, bx * TX, y, z, 0, sh);
+      __syncthreads();      // the exchange arrays are reused by the next tile
+    }
+    if (s + 1 < p.n_steps) {      // every store of this step is visible before any pull of the next
+      if constexpr (CLBAR) {
+        cluster_arrive_release();
+        cluster_wait_acquire();
+      } else {
+        cg::this_grid().sync();
+      }
+    }
   }
 }
 
@@ -1482,15 +1676,26 @@ __global__ void pops_import_kernel(const double *__restrict__ in, real *__restri
 }
 
 // ---- slab halo: pack the populations of one plane of the slowest axis (the listed directions, all K sets) into a
-// contiguous buffer [K][ndir][plane cells], or write such a buffer into a plane ------------------------------
+// contiguous buffer [K][ndir][plane cells], or write such a buffer into a plane.  A list entry is the direction index plus
+// its in-plane components: dir | (c_x + 1) << 8 | (c_y + 1) << 10.
+// filt_x / filt_y (unpack of LBMHD_HALO_RETURN only): slot s of plane cell (x, y) was pushed by the cell at (x + c_sx,
+// y + c_sy) of the neighbouring slab's plane; where that cell would lie outside a non-periodic face nobody pushed, the
+// buffer holds no value for it, and the destination keeps what its own cell left there (a population that could not be
+// pushed out of the domain stays in its own slot). ------------------------------
 template <typename real, bool PACK>
 __global__ void halo_plane_kernel(real *__restrict__ g, size_t pstride, real *__restrict__ buf, size_t plane_cells, size_t plane_first,
-                                  int K, int Q, int ndir, const int *__restrict__ dirs) {
+                                  int K, int Q, int ndir, const int *__restrict__ dirs, int nx, int ny, int filt_x, int filt_y) {
   const size_t total = (size_t)K * ndir * plane_cells;
   for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
     const size_t c = e % plane_cells, kd = e / plane_cells;
     const int d = (int)(kd % ndir), k = (int)(kd / ndir);
-    real *slot = g + ((size_t)k * Q + dirs[d]) * pstride + plane_first + c;
+    const int entry = dirs[d], dir = entry & 255;
+    if (!PACK && (filt_x | filt_y)) {
+      const int x = (int)(c % nx), y = (int)(c / nx);
+      const int px = x + ((entry >> 8) & 3) - 1, py = y + ((entry >> 10) & 3) - 1;
+      if ((filt_x && (px < 0 || px >= nx)) || (filt_y && (py < 0 || py >= ny))) continue;
+    }
+    real *slot = g + ((size_t)k * Q + dir) * pstride + plane_first + c;
     if (PACK) buf[e] = *slot;
     else *slot = buf[e];
   }
@@ -1499,6 +1704,14 @@ __global__ void halo_plane_kernel(real *__restrict__ g, size_t pstride, real *__
 // ---- bandwidth probe: BabelStream-style copy, 2 fp64 per thread per iteration ----------------
 static __global__ void __launch_bounds__(256) copy_probe_kernel(const double2 *__restrict__ a, double2 *__restrict__ b, size_t n2) {
   for (size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x; j < n2; j += (size_t)gridDim.x * blockDim.x) b[j] = a[j];
+}
+
+static __global__ void __launch_bounds__(256) triad_probe_kernel(double2 *__restrict__ a, const double2 *__restrict__ b,
+                                                                const double2 *__restrict__ c, double s, size_t n2) {
+  for (size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x; j < n2; j += (size_t)gridDim.x * blockDim.x) {
+    const double2 bv = b[j], cv = c[j];
+    a[j] = make_double2(fma(s, cv.x, bv.x), fma(s, cv.y, bv.y));
+  }
 }
 
 }  // namespace lbk

@@ -34,9 +34,13 @@ template <int LAT, int SCHEME, typename real> struct Ops {
 
   // One launch over all tiles; the tile class (interior / x-edge / general) is chosen per block.
   // One cell per thread: A/B, or in place the pull-push step from layout P0 and the local step from P1.
-  static cudaError_t launch_step_one(lbmhd_t *h, const StepArgs<real> &a) {
+  // grid over the planes [lo, hi) of the slowest lattice axis (the whole lattice: 0 .. n)
+  static dim3 grid_planes(const lbmhd_t *h, int gx, int lo, int hi) {
+    return L::D == 3 ? dim3(gx, h->p.ny, hi - lo) : (L::D == 2 ? dim3(gx, hi - lo, 1) : dim3(gx, 1, 1));
+  }
+  static cudaError_t launch_step_one(lbmhd_t *h, const StepArgs<real> &a, int lo, int hi) {
     constexpr int TX = 32;
-    const dim3 g((h->p.nx + TX - 1) / TX, h->p.ny, h->p.nz), b(TX, K);
+    const dim3 g = grid_planes(h, (h->p.nx + TX - 1) / TX, lo, hi), b(TX, K);
     const Region all{0, 1, 0, 1, 0, 1};
     if (h->p.streaming != LBMHD_STREAM_INPLACE) step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_AB><<<g, b, 0, h->stream>>>(a, all, 0);
     else if (h->parity == 0) step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_PP><<<g, b, 0, h->stream>>>(a, all, 0);
@@ -68,12 +72,12 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     const long long blocks = (long long)((h->p.nx + 32 * NC - 1) / (32 * NC) + 1) * h->p.ny * h->p.nz;
     return h->multi_force || blocks >= 16LL * h->num_sms * MINB_M;
   }
-  static cudaError_t launch_step_multi(lbmhd_t *h, const StepArgs<real> &a) {
+  static cudaError_t launch_step_multi(lbmhd_t *h, const StepArgs<real> &a, int lo, int hi) {
     if constexpr (NC > 1) {
       constexpr int W = 32 * NC;
       const int nm = h->p.nx >= 64 + W ? (h->p.nx - 64) / W : 0;      // multi-cell tiles at x0 = 32 + W j, all interior in x
       const int ntail = (h->p.nx - (32 + W * nm) + 31) / 32;           // 32-cell tiles after them (>= 0)
-      const dim3 g(nm + 1 + (ntail > 0 ? ntail : 0), h->p.ny, h->p.nz), b(32, K);
+      const dim3 g = grid_planes(h, nm + 1 + (ntail > 0 ? ntail : 0), lo, hi), b(32, K);
       const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
       if (!inplace) step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_AB><<<g, b, 0, h->stream>>>(a, nm);
       else if (h->parity == 0) step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_PP><<<g, b, 0, h->stream>>>(a, nm);
@@ -85,11 +89,45 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     }
   }
 
+  // one thread per cell on the short lattices (lbmhd_kernels.cuh, step_kernel_cell): K * Q populations in one thread's registers
+  static constexpr bool CELL_OK = Q <= 7 && K <= 9;
+  static constexpr int cell_wx() {      // tile width: 32 x the smallest divisor >= 2 of K (a 1D lattice: the whole block in one row)
+    int g = 2;
+    while (g < K && K % g != 0) g++;
+    return L::D == 1 ? 32 * K : 32 * g;
+  }
+  static constexpr int WXC = cell_wx();
+  static constexpr int RYC = 32 * K / WXC;
+  static constexpr int regs_need_cell() { return (K * Q * (int)sizeof(real) / 4 + 48 + 7) / 8 * 8; }
+  static constexpr int MINB_C = minb_for(32 * K, regs_need_cell());
+  static bool cell_pays(const lbmhd_t *h) {
+    if (h->p.nx < 64 + WXC) return false;
+    const long long blocks = (long long)((h->p.nx - 64) / WXC + 2) * ((h->p.ny + RYC - 1) / RYC) * h->p.nz;
+    return h->cell_force || blocks >= 8LL * h->num_sms * MINB_C;
+  }
+  static cudaError_t launch_step_cell(lbmhd_t *h, const StepArgs<real> &a, int lo, int hi) {
+    if constexpr (CELL_OK) {
+      const int nc = (h->p.nx - 64) / WXC;                                 // cell tiles at x0 = 32 + WXC j, all interior in x
+      const int ntail = (h->p.nx - (32 + WXC * nc) + 31) / 32;             // 32-cell pieces after them
+      const int gx = nc + 1 + ntail;
+      const dim3 g = L::D == 3 ? dim3(gx, (h->p.ny + RYC - 1) / RYC, hi - lo) : (L::D == 2 ? dim3(gx, (hi - lo + RYC - 1) / RYC, 1) : dim3(gx, 1, 1));
+      const dim3 b(32, K);
+      const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
+      if (!inplace) step_kernel_cell<LAT, SCHEME, real, WXC, MINB_C, ST_AB><<<g, b, 0, h->stream>>>(a, nc);
+      else if (h->parity == 0) step_kernel_cell<LAT, SCHEME, real, WXC, MINB_C, ST_PP><<<g, b, 0, h->stream>>>(a, nc);
+      else step_kernel_cell<LAT, SCHEME, real, WXC, MINB_C, ST_LOC><<<g, b, 0, h->stream>>>(a, nc);
+      h->launches += 1;
+      return cudaGetLastError();
+    } else {
+      return cudaErrorInvalidValue;
+    }
+  }
+
   // RESIST: the K = 11 / 14 / 17 rows of a tile split over a 2-CTA cluster (lbmhd_kernels.cuh, Share)
   static constexpr int KH = (K + 1) / 2;
   static constexpr int MINB_CL = minb_for(32 * KH, REGS_NEED);
-  static cudaError_t launch_step_cluster(lbmhd_t *h, const StepArgs<real> &a) {
-    const dim3 g(2 * ((h->p.nx + 31) / 32), h->p.ny, h->p.nz), b(32, KH);
+  static cudaError_t launch_step_cluster(lbmhd_t *h, const StepArgs<real> &a, int lo, int hi) {
+    const dim3 g = grid_planes(h, 2 * ((h->p.nx + 31) / 32), lo, hi), b(32, KH);
     if (h->p.streaming != LBMHD_STREAM_INPLACE) step_kernel_cl<LAT, SCHEME, real, MINB_CL, ST_AB><<<g, b, 0, h->stream>>>(a);
     else if (h->parity == 0) step_kernel_cl<LAT, SCHEME, real, MINB_CL, ST_PP><<<g, b, 0, h->stream>>>(a);
     else step_kernel_cl<LAT, SCHEME, real, MINB_CL, ST_LOC><<<g, b, 0, h->stream>>>(a);
@@ -113,8 +151,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     return cudaGetLastError();
   }
 
-  static int step(lbmhd_t *h, int n_steps) {
-    StepArgs<real> a;
+  // the step-independent part of the kernel arguments
+  static void make_args(const lbmhd_t *h, StepArgs<real> &a) {
     memset(&a, 0, sizeof a);
     a.pstride = h->L.pstride;
     a.nx = h->p.nx; a.ny = h->p.ny; a.nz = h->p.nz;
@@ -139,6 +177,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
         a.st_off[i] = (long long)i * (long long)h->L.pstride * es;
       }
     }
+    a.kplane = (long long)Q * (long long)h->L.pstride * (long long)sizeof(real);
     a.hoff = h->p.halo_offset;
     a.body = h->body_on ? (double *)(h->ws + h->L.off_body) : nullptr;
     for (int c = 0; c < 3; c++) a.body_ref[c] = h->body_ref[c];
@@ -150,54 +189,195 @@ template <int LAT, int SCHEME, typename real> struct Ops {
       a.sph_touch2 = h->sph_eps > 0.0 ? (h->sph_R + 0.5 * h->sph_eps) * (h->sph_R + 0.5 * h->sph_eps) : a.sph_R2;
       a.n_dip = h->n_dip;
       for (int j = 0; j < h->n_dip; j++) { a.dip_Bs[j] = h->dip_Bs[j]; a.dip_core[j] = h->dip_core[j]; }
-      for (int c = 0; c < 3; c++) a.sph_u[c] = h->sph_u[c];
+      for (int c = 0; c < 3; c++) { a.sph_u[c] = h->sph_u[c]; a.sph_om[c] = h->sph_om[c]; }
+    }
+  }
+
+  // the part that changes every step: population copies, published moment arrays, the body's position
+  static void step_args(const lbmhd_t *h, StepArgs<real> &a) {
+    const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
+    a.src = pops(const_cast<lbmhd_t *>(h), h->cur);
+    a.dst = pops(const_cast<lbmhd_t *>(h), inplace ? h->cur : 1 - h->cur);
+    if (inplace) {
+      a.M_cur = (const double *)(h->ws + h->L.off_M[h->mcur]);
+      a.M_next = (double *)(h->ws + h->L.off_M[1 - h->mcur]);
+    }
+    if (h->has_sphere) {
+      // A12: centre before step t is c0 + (t - t0) u^B; product and sum rounded separately, like the oracle
+      const volatile double dt = (double)(h->t - h->sph_t0);
+      for (int c = 0; c < 3; c++) {
+        const volatile double prod = dt * h->sph_u[c];
+        a.sph_c[c] = h->sph_c0[c] + prod;
+      }
+      // body-frame offsets and axes of the dipoles at this step: Rodrigues rotation about Omega by |Omega| (t - t0)
+      const double om2 = h->sph_om[0] * h->sph_om[0] + h->sph_om[1] * h->sph_om[1] + h->sph_om[2] * h->sph_om[2];
+      for (int j = 0; j < h->n_dip; j++)
+        for (int which = 0; which < 2; which++) {
+          const double *v = which ? h->dip_off[j] : h->dip_m[j];
+          double *out = which ? a.dip_off[j] : a.dip_m[j];
+          for (int c = 0; c < 3; c++) out[c] = v[c];
+          if (om2 > 0.0) {
+            const double omn = sqrt(om2), th = omn * dt, cth = cos(th), sth = sin(th);
+            const double e[3] = {h->sph_om[0] / omn, h->sph_om[1] / omn, h->sph_om[2] / omn};
+            const double ev = e[0] * v[0] + e[1] * v[1] + e[2] * v[2];
+            const double ex[3] = {e[1] * v[2] - e[2] * v[1], e[2] * v[0] - e[0] * v[2], e[0] * v[1] - e[1] * v[0]};
+            for (int c = 0; c < 3; c++) out[c] = v[c] * cth + ex[c] * sth + e[c] * ev * (1.0 - cth);
+          }
+        }
+    }
+  }
+
+  // one launch of the step kernel chosen for this lattice, scheme, precision and grid over the planes
+  // [lo, hi) of the slowest lattice axis
+  static int launch(lbmhd_t *h, StepArgs<real> &a, int lo, int hi) {
+    a.row0 = lo;
+    a.row1 = hi;
+    cudaError_t e;
+    bool launched = false;
+    if constexpr (SCHEME == kResist && Q > 9 && sizeof(real) == 8) {
+      if (h->cluster) { e = launch_step_cluster(h, a, lo, hi); launched = true; h->last_path = LBMHD_PATH_CLUSTER; }
+    }
+    if (launched) {}
+    else if (h->use_tma) { e = launch_step_tma(h, a); h->last_path = LBMHD_PATH_TMA; }
+    else if (CELL_OK && h->cell && h->pair && cell_pays(h)) { e = launch_step_cell(h, a, lo, hi); h->last_path = LBMHD_PATH_CELL; }
+    else if (NC > 1 && h->pair && h->p.nx % VW == 0 && multi_pays(h)) { e = launch_step_multi(h, a, lo, hi); h->last_path = LBMHD_PATH_MULTI; }
+    else { e = launch_step_one(h, a, lo, hi); h->last_path = LBMHD_PATH_ONE; }
+    if (e != cudaSuccess) return fail(LBMHD_ECUDA, "step kernel launch: %s", cudaGetErrorString(e));
+    return LBMHD_OK;
+  }
+
+  static void advance(lbmhd_t *h) {
+    if (h->p.streaming == LBMHD_STREAM_INPLACE) { h->parity ^= 1; h->mcur ^= 1; }
+    else h->cur = 1 - h->cur;
+    h->t += 1;
+  }
+
+  static int n_planes(const lbmhd_t *h) { return L::D == 3 ? h->p.nz : (L::D == 2 ? h->p.ny : 1); }
+
+  // ---- many steps in one cooperative launch (lbmhd_kernels.cuh, step_kernel_persist) --------------
+  static constexpr int MINB_P = minb_for(32 * K, REGS_NEED + 8);
+  static constexpr bool CLP_OK = 64 * K <= 1024;            // the one-cluster variant runs 64-cell tiles: 64 K threads per CTA
+  template <bool INPLACE> static int persist_capacity(const lbmhd_t *h) {
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, step_kernel_persist<LAT, SCHEME, real, 32, MINB_P, INPLACE, false>, 32 * K, 0) != cudaSuccess)
+      return 0;
+    return per_sm * h->num_sms;
+  }
+  // Taken when the caller asks for several steps at once on a lattice small enough that launch latency and the fill and drain
+  // of every launch show (measured: DESIGN.md §5.7), never for slabs (their ghost planes change between steps) or a body
+  // whose dipoles rotate (the host turns them every step).
+  static bool persist_allowed(const lbmhd_t *h, int n_steps) {
+    if (!h->persist || n_steps < 2 || h->use_tma) return false;
+    const int D1 = L::D - 1;
+    if (L::D >= 2 && (h->p.bc[2 * D1] == LBMHD_BC_HALO || h->p.bc[2 * D1 + 1] == LBMHD_BC_HALO)) return false;
+    if (h->has_sphere && (h->sph_om[0] != 0.0 || h->sph_om[1] != 0.0 || h->sph_om[2] != 0.0)) return false;
+    return true;
+  }
+  template <bool INPLACE> static void persist_args(lbmhd_t *h, PersistArgs<real> &p, int n_steps, int tx) {
+    memset(&p, 0, sizeof p);
+    p.n_steps = n_steps;
+    p.inplace = INPLACE ? 1 : 0;
+    p.parity0 = h->parity;
+    p.pop[0] = pops(h, h->cur);
+    p.pop[1] = pops(h, INPLACE ? h->cur : 1 - h->cur);
+    if (INPLACE) {
+      p.M[0] = (double *)(h->ws + h->L.off_M[h->mcur]);
+      p.M[1] = (double *)(h->ws + h->L.off_M[1 - h->mcur]);
+    }
+    p.t_rel0 = h->t - h->sph_t0;
+    for (int c = 0; c < 3; c++) p.sph_c0[c] = h->sph_c0[c];
+    p.tiles_x = (h->p.nx + tx - 1) / tx;
+    p.n_tiles = (long long)p.tiles_x * h->p.ny * h->p.nz;
+  }
+  template <bool INPLACE> static int launch_persist(lbmhd_t *h, StepArgs<real> &a, int n_steps, int capacity) {
+    PersistArgs<real> p;
+    persist_args<INPLACE>(h, p, n_steps, 32);
+    a.row0 = 0;
+    a.row1 = n_planes(h);
+    const long long want = p.n_tiles < (long long)capacity ? p.n_tiles : (long long)capacity;
+    void *params[2] = {(void *)&a, (void *)&p};
+    cudaError_t e = cudaLaunchCooperativeKernel((const void *)step_kernel_persist<LAT, SCHEME, real, 32, MINB_P, INPLACE, false>,
+                                                dim3((unsigned)want), dim3(32, K), params, 0, h->stream);
+    if (e != cudaSuccess) return fail(LBMHD_ECUDA, "cooperative step kernel launch: %s", cudaGetErrorString(e));
+    h->launches += 1;
+    h->last_path = LBMHD_PATH_PERSIST;
+    for (int s = 0; s < n_steps; s++) advance(h);
+    return LBMHD_OK;
+  }
+  // the whole lattice in one cluster of <= 16 CTAs (64-cell tiles, one per CTA): hardware barrier between the steps
+  template <bool INPLACE> static int launch_persist_cluster(lbmhd_t *h, StepArgs<real> &a, int n_steps) {
+    if constexpr (CLP_OK) {
+      PersistArgs<real> p;
+      persist_args<INPLACE>(h, p, n_steps, 64);
+      a.row0 = 0;
+      a.row1 = n_planes(h);
+      auto kern = step_kernel_persist<LAT, SCHEME, real, 64, 1, INPLACE, true>;
+      if (p.n_tiles > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) {
+        cudaGetLastError();
+        h->persist_cluster = false;
+        return 1;
+      }
+      cudaLaunchConfig_t cfg;
+      memset(&cfg, 0, sizeof cfg);
+      cfg.gridDim = dim3((unsigned)p.n_tiles);
+      cfg.blockDim = dim3(64, K);
+      cfg.stream = h->stream;
+      cudaLaunchAttribute attr[1];
+      attr[0].id = cudaLaunchAttributeClusterDimension;
+      attr[0].val.clusterDim.x = (unsigned)p.n_tiles;
+      attr[0].val.clusterDim.y = 1;
+      attr[0].val.clusterDim.z = 1;
+      cfg.attrs = attr;
+      cfg.numAttrs = 1;
+      cudaError_t e = cudaLaunchKernelEx(&cfg, kern, a, p);
+      if (e != cudaSuccess) {      // e.g. a cluster of this size cannot be co-scheduled here: not sticky, the caller takes another path
+        cudaGetLastError();
+        h->persist_cluster = false;
+        return 1;
+      }
+      h->launches += 1;
+      h->last_path = LBMHD_PATH_PERSIST;
+      for (int s = 0; s < n_steps; s++) advance(h);
+      return LBMHD_OK;
+    } else {
+      return 1;
+    }
+  }
+
+  static int step(lbmhd_t *h, int n_steps) {
+    StepArgs<real> a;
+    make_args(h, a);
+    const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
+    if (persist_allowed(h, n_steps)) {
+      const long long tiles64 = (long long)((h->p.nx + 63) / 64) * h->p.ny * h->p.nz;
+      if (CLP_OK && h->persist_cluster && tiles64 <= 16) {
+        step_args(h, a);
+        const int rc = inplace ? launch_persist_cluster<true>(h, a, n_steps) : launch_persist_cluster<false>(h, a, n_steps);
+        if (rc <= 0) return rc;      // > 0: the cluster could not be launched here; go on with the cooperative kernel
+      }
+      const long long n_tiles = (long long)((h->p.nx + 31) / 32) * h->p.ny * h->p.nz;
+      const int cap = inplace ? persist_capacity<true>(h) : persist_capacity<false>(h);
+      if (cap > 0 && (h->persist_force || n_tiles <= (long long)h->persist_waves * cap)) {
+        step_args(h, a);
+        return inplace ? launch_persist<true>(h, a, n_steps, cap) : launch_persist<false>(h, a, n_steps, cap);
+      }
     }
     for (int s = 0; s < n_steps; s++) {
-      const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
-      a.src = pops(h, h->cur);
-      a.dst = pops(h, inplace ? h->cur : 1 - h->cur);
-      if (inplace) {
-        a.M_cur = (const double *)(h->ws + h->L.off_M[h->mcur]);
-        a.M_next = (double *)(h->ws + h->L.off_M[1 - h->mcur]);
-      }
-      if (h->has_sphere) {
-        // A12: centre before step t is c0 + (t - t0) u^B; product and sum rounded separately, like the oracle
-        const volatile double dt = (double)(h->t - h->sph_t0);
-        for (int c = 0; c < 3; c++) {
-          const volatile double prod = dt * h->sph_u[c];
-          a.sph_c[c] = h->sph_c0[c] + prod;
-          a.sph_om[c] = h->sph_om[c];
-        }
-        // body-frame offsets and axes of the dipoles at this step: Rodrigues rotation about Omega by |Omega| (t - t0)
-        const double om2 = h->sph_om[0] * h->sph_om[0] + h->sph_om[1] * h->sph_om[1] + h->sph_om[2] * h->sph_om[2];
-        for (int j = 0; j < h->n_dip; j++)
-          for (int which = 0; which < 2; which++) {
-            const double *v = which ? h->dip_off[j] : h->dip_m[j];
-            double *out = which ? a.dip_off[j] : a.dip_m[j];
-            for (int c = 0; c < 3; c++) out[c] = v[c];
-            if (om2 > 0.0) {
-              const double omn = sqrt(om2), th = omn * dt, cth = cos(th), sth = sin(th);
-              const double e[3] = {h->sph_om[0] / omn, h->sph_om[1] / omn, h->sph_om[2] / omn};
-              const double ev = e[0] * v[0] + e[1] * v[1] + e[2] * v[2];
-              const double ex[3] = {e[1] * v[2] - e[2] * v[1], e[2] * v[0] - e[0] * v[2], e[0] * v[1] - e[1] * v[0]};
-              for (int c = 0; c < 3; c++) out[c] = v[c] * cth + ex[c] * sth + e[c] * ev * (1.0 - cth);
-            }
-          }
-      }
-      cudaError_t e;
-      bool launched = false;
-      if constexpr (SCHEME == kResist && Q > 9 && sizeof(real) == 8) {
-        if (h->cluster) { e = launch_step_cluster(h, a); launched = true; h->last_path = LBMHD_PATH_CLUSTER; }
-      }
-      if (launched) {}
-      else if (h->use_tma) { e = launch_step_tma(h, a); h->last_path = LBMHD_PATH_TMA; }
-      else if (NC > 1 && h->pair && h->p.nx % VW == 0 && multi_pays(h)) { e = launch_step_multi(h, a); h->last_path = LBMHD_PATH_MULTI; }
-      else { e = launch_step_one(h, a); h->last_path = LBMHD_PATH_ONE; }
-      if (e != cudaSuccess) return fail(LBMHD_ECUDA, "step kernel launch: %s", cudaGetErrorString(e));
-      if (inplace) { h->parity ^= 1; h->mcur ^= 1; }
-      else h->cur = 1 - h->cur;
-      h->t += 1;
+      step_args(h, a);
+      if (int rc = launch(h, a, 0, n_planes(h))) return rc;
+      advance(h);
     }
+    return LBMHD_OK;
+  }
+
+  // one step in pieces (slab overlap): the planes [lo, hi) of the slowest lattice axis; `last` completes the step
+  static int step_part(lbmhd_t *h, int lo, int hi, int last) {
+    StepArgs<real> a;
+    make_args(h, a);
+    step_args(h, a);
+    if (hi > lo)
+      if (int rc = launch(h, a, lo, hi)) return rc;
+    if (last) advance(h);
     return LBMHD_OK;
   }
 
@@ -252,7 +432,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
   static int halo_dirs(int sign, int *dirs) {
     int n = 0;
     for (int i = 0; i < Q; i++)
-      if (sign == 0 || lat_c<L>(i, L::D - 1) == sign) dirs[n++] = i;
+      if (sign == 0 || lat_c<L>(i, L::D - 1) == sign)      // entry: dir | (c_x + 1) << 8 | (c_y + 1) << 10 (in-plane components)
+        dirs[n++] = i | ((lat_c<L>(i, 0) + 1) << 8) | (((L::D == 3 ? lat_c<L>(i, 1) : 0) + 1) << 10);
     return n;
   }
 
@@ -277,7 +458,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
 
 template <int LAT, int SCHEME, typename real> OpTable make_table() {
   using O = Ops<LAT, SCHEME, real>;
-  return OpTable{O::step, O::init, O::moments, O::diag, O::pops_export, O::pops_import, O::refresh_published, O::halo_dirs};
+  return OpTable{O::step, O::step_part, O::init, O::moments, O::diag, O::pops_export, O::pops_import, O::refresh_published, O::halo_dirs};
 }
 
 template <int LAT, typename real> OpTable table_for(int scheme) {

@@ -18,6 +18,7 @@ BC_PERIODIC, BC_ZEROGRAD, BC_INFLOW, BC_HALO = 0, 1, 2, 3
 CELL_FLUID, CELL_FROZEN, CELL_SOLID = 0, 1, 2
 STREAM_AB, STREAM_INPLACE = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC = 0, -1, -2, -3, -4
+HALO_CROSSING, HALO_FULL, HALO_RETURN = 0, 1, 2
 LATTICES = {"D1Q3": D1Q3, "D2Q9": D2Q9, "D3Q19": D3Q19, "D2Q5": D2Q5, "D3Q7": D3Q7}
 SCHEMES = {"IDEAL": IDEAL, "INCRES": INCRES, "IDEAL_DIVB": IDEAL_DIVB, "RESIST": RESIST, "FULL": FULL}
 
@@ -68,6 +69,12 @@ def load_library():
     lib.lbmhd_halo_bytes.restype = C.c_size_t
     lib.lbmhd_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
     lib.lbmhd_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
+    lib.lbmhd_halo_pack_on.argtypes = [C.c_void_p, C.c_int, C.c_int, dp, C.c_int, C.c_void_p]
+    lib.lbmhd_halo_unpack_on.argtypes = [C.c_void_p, C.c_int, C.c_int, dp, C.c_int, C.c_void_p]
+    lib.lbmhd_step_part.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
+    lib.lbmhd_diagnostics.argtypes = [C.c_void_p, dp, dp, C.c_int]
+    lib.lbmhd_workspace_bytes_min.argtypes = [pp]
+    lib.lbmhd_workspace_bytes_min.restype = C.c_size_t
     lib.lbmhd_get_populations.argtypes = [C.c_void_p, dp, C.c_int]
     lib.lbmhd_set_populations.argtypes = [C.c_void_p, dp, C.c_int]
     lib.lbmhd_steps_done.argtypes = [C.c_void_p]
@@ -80,6 +87,7 @@ def load_library():
     lib.lbmhd_body_enable.argtypes = [C.c_void_p, C.c_int, dp]
     lib.lbmhd_body_read.argtypes = [C.c_void_p, dp, C.c_int, C.c_int]
     lib.lbmhd_copy_probe.argtypes = [dp, dp, C.c_size_t, C.c_int, C.c_void_p]
+    lib.lbmhd_triad_probe.argtypes = [dp, dp, dp, C.c_double, C.c_size_t, C.c_int, C.c_void_p]
     lib.lbmhd_last_error.restype = C.c_char_p
     _lib = lib
     return lib
@@ -90,7 +98,8 @@ EXPORTS = ["lbmhd_num_vars", "lbmhd_num_dirs", "lbmhd_workspace_bytes", "lbmhd_c
            "lbmhd_set_porosity", "lbmhd_set_sphere_width", "lbmhd_set_sphere_rotation", "lbmhd_halo_bytes", "lbmhd_halo_pack",
            "lbmhd_halo_unpack", "lbmhd_get_populations", "lbmhd_set_populations", "lbmhd_steps_done", "lbmhd_launch_count",
            "lbmhd_copy_probe", "lbmhd_last_error", "lbmhd_body_enable", "lbmhd_body_read",
-           "lbmhd_set_sphere_dipoles", "lbmhd_set_obstacle_rotation", "lbmhd_step_path"]
+           "lbmhd_set_sphere_dipoles", "lbmhd_set_obstacle_rotation", "lbmhd_step_path", "lbmhd_triad_probe",
+           "lbmhd_halo_pack_on", "lbmhd_halo_unpack_on", "lbmhd_step_part", "lbmhd_diagnostics", "lbmhd_workspace_bytes_min"]
 
 
 def _check(rc, allow=()):
@@ -119,8 +128,10 @@ def make_params(scheme, lattice, shape, precision=64, gamma=5.0 / 3.0, c0sq=1.0 
     return p
 
 
-def workspace_bytes(params):
-    return int(load_library().lbmhd_workspace_bytes(C.byref(params)))
+def workspace_bytes(params, solid_fields=True):
+    """device bytes a handle needs; solid_fields=False leaves out the per-cell B_solid / porosity storage"""
+    lib = load_library()
+    return int(lib.lbmhd_workspace_bytes(C.byref(params)) if solid_fields else lib.lbmhd_workspace_bytes_min(C.byref(params)))
 
 
 def _host_ptr(a):
@@ -130,7 +141,7 @@ def _host_ptr(a):
 class Lbmhd:
     """Handle wrapper: lbmhd_create / init / step / moments / set_obstacle / set_sphere / destroy."""
 
-    def __init__(self, params, mask=None, stream=None):
+    def __init__(self, params, mask=None, stream=None, solid_fields=True):
         import torch
         self.lib = load_library()
         if not torch.cuda.is_available():
@@ -143,7 +154,7 @@ class Lbmhd:
             raise LbmhdError(EINVAL, "unknown scheme or lattice")
         self.shape = (params.nz, params.ny, params.nx)
         self.N = params.nx * params.ny * params.nz
-        nbytes = workspace_bytes(params)
+        nbytes = workspace_bytes(params, solid_fields)
         if nbytes == 0:
             raise LbmhdError(EINVAL, "bad dims or precision")
         dev = torch.device("cuda", params.device)
@@ -191,6 +202,20 @@ class Lbmhd:
 
     def step(self, n=1):
         _check(self.lib.lbmhd_step(self.h, int(n)))
+
+    def step_part(self, plane_lo, plane_hi, last):
+        """one step in pieces: planes [plane_lo, plane_hi) of the slowest lattice axis; last=True completes the step"""
+        _check(self.lib.lbmhd_step_part(self.h, int(plane_lo), int(plane_hi), int(bool(last))))
+
+    def diagnostics(self, fields_dev, diag_out=None):
+        """the 3K+4 diagnostics of a device fields tensor [K*N]; -> numpy array (host, synchronises) or the given device tensor"""
+        assert fields_dev.is_cuda and fields_dev.dtype == self.torch.float64 and fields_dev.numel() == self.K * self.N
+        if diag_out is not None:
+            _check(self.lib.lbmhd_diagnostics(self.h, C.c_void_p(fields_dev.data_ptr()), C.c_void_p(diag_out.data_ptr()), 1))
+            return diag_out
+        dg = np.empty(3 * self.K + 4, dtype=np.float64)
+        _check(self.lib.lbmhd_diagnostics(self.h, C.c_void_p(fields_dev.data_ptr()), _host_ptr(dg), 0), allow=(ENUMERIC,))
+        return dg
 
     def moments(self, fields_out=None, diag_out=None, want_fields=True, want_diag=True, check=False):
         """-> (fields [K, nz, ny, nx], diag [3K+4]).  Host numpy by default; pass CUDA tensors to stay on device."""
@@ -287,17 +312,25 @@ class Lbmhd:
         _check(self.lib.lbmhd_set_populations(self.h, C.c_void_p(t.data_ptr()), 1))
         self.stream.synchronize()
 
-    def halo_buffer(self, full=False):
+    def halo_buffer(self, what=HALO_CROSSING):
         """device tensor sized for one packed face (element type = precision)"""
         torch = self.torch
-        nbytes = int(self.lib.lbmhd_halo_bytes(self.h, int(full)))
+        nbytes = int(self.lib.lbmhd_halo_bytes(self.h, int(what)))
         return torch.empty(nbytes, dtype=torch.uint8, device=self.workspace.device)
 
-    def halo_pack(self, side, buf, full=False):
-        _check(self.lib.lbmhd_halo_pack(self.h, int(side), int(full), C.c_void_p(buf.data_ptr())))
+    def halo_pack(self, side, buf, what=HALO_CROSSING, next_copy=False, stream=None):
+        if stream is None and not next_copy:
+            _check(self.lib.lbmhd_halo_pack(self.h, int(side), int(what), C.c_void_p(buf.data_ptr())))
+        else:
+            st = (stream if stream is not None else self.stream).cuda_stream
+            _check(self.lib.lbmhd_halo_pack_on(self.h, int(side), int(what), C.c_void_p(buf.data_ptr()), int(bool(next_copy)), st))
 
-    def halo_unpack(self, side, buf, full=False):
-        _check(self.lib.lbmhd_halo_unpack(self.h, int(side), int(full), C.c_void_p(buf.data_ptr())))
+    def halo_unpack(self, side, buf, what=HALO_CROSSING, next_copy=False, stream=None):
+        if stream is None and not next_copy:
+            _check(self.lib.lbmhd_halo_unpack(self.h, int(side), int(what), C.c_void_p(buf.data_ptr())))
+        else:
+            st = (stream if stream is not None else self.stream).cuda_stream
+            _check(self.lib.lbmhd_halo_unpack_on(self.h, int(side), int(what), C.c_void_p(buf.data_ptr()), int(bool(next_copy)), st))
 
     @property
     def steps_done(self):
@@ -309,19 +342,19 @@ class Lbmhd:
 
     @property
     def step_path(self):
-        """PATH_ONE / PATH_MULTI / PATH_CLUSTER / PATH_TMA of the last step launch (-1 before the first)"""
+        """PATH_ONE / PATH_MULTI / PATH_CLUSTER / PATH_TMA / PATH_PERSIST of the last step launch (-1 before the first)"""
         return int(self.lib.lbmhd_step_path(self.h))
 
 
-PATH_ONE, PATH_MULTI, PATH_CLUSTER, PATH_TMA = 0, 1, 2, 3
+PATH_ONE, PATH_MULTI, PATH_CLUSTER, PATH_TMA, PATH_PERSIST, PATH_CELL = 0, 1, 2, 3, 4, 5
 
 
-def from_workload(w, precision=64, device=0, streaming=STREAM_AB):
+def from_workload(w, precision=64, device=0, streaming=STREAM_AB, solid_fields=True):
     """Lbmhd handle configured (boundaries, tau, sphere) for a workloads.py dict; fields not yet initialised."""
     p = make_params(w["scheme"], w["lattice"], w["shape"], precision=precision, gamma=w["gamma"] or 1.4, c0sq=w["c0sq"],
                     nu=w["nu"], eta=w["eta"], tau=w["tau"], powell=w["powell"], bc=w["bc"], streaming=streaming,
                     device=device, tau_relax=w.get("tau_relax", 0.0), eta_jc=w.get("eta_jc", 0.0))
-    sim = Lbmhd(p)
+    sim = Lbmhd(p, solid_fields=solid_fields)
     if w.get("sphere"):
         s = w["sphere"]
         sim.set_sphere(s["centre"], s["radius"], s["u_solid"], s["dipole_dir"], s["B_surface"])
@@ -352,4 +385,26 @@ def copy_probe(n_elems=1 << 28, reps=10, device=0):
         e1.record(st)
         e1.synchronize()
         best = max(best, 2 * 8 * n_elems / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+    return best
+
+
+def triad_probe(n_elems=1 << 27, reps=10, device=0):
+    """measured fp64 triad bandwidth in GB/s (a = b + s c: 24 bytes per element), BabelStream-style"""
+    import torch
+    lib = load_library()
+    dev = torch.device("cuda", device)
+    b = torch.ones(n_elems, dtype=torch.float64, device=dev)
+    c = torch.ones_like(b)
+    a = torch.empty_like(b)
+    st = torch.cuda.current_stream(dev)
+    args = (C.c_void_p(a.data_ptr()), C.c_void_p(b.data_ptr()), C.c_void_p(c.data_ptr()), 0.5, n_elems)
+    _check(lib.lbmhd_triad_probe(*args, 3, st.cuda_stream))
+    best = 0.0
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        _check(lib.lbmhd_triad_probe(*args, 1, st.cuda_stream))
+        e1.record(st)
+        e1.synchronize()
+        best = max(best, 3 * 8 * n_elems / (e0.elapsed_time(e1) * 1e-3) / 1e9)
     return best

@@ -7,7 +7,7 @@ resistive Orszag-Tang :215, compressible Orszag-Tang :231-233, MHD rotor :193, 1
 :281-302) and stand in for them.  All randomness: numpy Generator(PCG64(20260641 + c)).
 
 A workload is a dict:
-  scheme 'IDEAL'|'INCRES', lattice 'D1Q3'|'D2Q9'|'D3Q19', shape (nx[,ny[,nz]]), gamma, c0sq, nu, eta,
+  scheme 'IDEAL'|'INCRES'|'IDEAL_DIVB'|'RESIST'|'FULL', lattice 'D1Q3'|'D2Q9'|'D3Q19', shape (nx[,ny[,nz]]), gamma, c0sq, nu, eta,
   tau (scalar), powell, bc (6 ints: 0 periodic, 1 zero-gradient, 2 inflow), steps,
   fields  float64 [K, nz, ny, nx] in LATTICE units (reading A1),
   sphere  None or dict(centre, radius, u_solid, dipole_dir, B_surface).
@@ -82,15 +82,41 @@ def _fourier_potential(rng, n, nmodes=8, kmax=4):
     return psi
 
 
-def config2(n=512, steps=1000, rms=0.02, nu=1e-3, eta=1e-3, c0sq=1.0 / 36.0, eta_jc=0.0):
-    """C2: 2D incompressible resistive MHD, D2Q9, periodic, 8 random Fourier modes |k| <= 4, lattice units."""
+def _config2_uB(n, rms):
+    """divergence-free (in the lattice sense) u and B from 8 random Fourier modes each, |k| <= 4, rms amplitude `rms`"""
     rng = _rng(2)
     ux, uy = _curl_h(_fourier_potential(rng, n))
     Bx, By = _curl_h(_fourier_potential(rng, n))
     su = rms / np.sqrt((ux * ux + uy * uy).mean())
     sb = rms / np.sqrt((Bx * Bx + By * By).mean())
-    F = np.stack([np.zeros_like(ux), su * ux, su * uy, sb * Bx, sb * By])[:, None]
-    return dict(name="C2", scheme="INCRES", lattice="D2Q9", shape=(n, n), gamma=0.0, c0sq=c0sq, nu=nu, eta=eta,
+    return su * ux, su * uy, sb * Bx, sb * By
+
+
+def config2(n=512, steps=1000, rms=0.05, nu=1e-3, eta=1e-3, sound=0.13, tau=0.5015, tau_relax=4.0):
+    """C2 as BASELINE states it: 2D resistive MHD, D2Q9, periodic, 8 random Fourier modes |k| <= 4 with rms amplitude 0.05 in
+    lattice units, nu = eta = 1e-3, 1000 steps — on the system the paper itself runs this case with: the
+    full dissipative equations (scheme FULL: viscous stress and resistive terms in the FLUX, from the transported gradients)
+    at low Mach number.  rho = 1, p = sound^2 rho / gamma (rms Mach 0.38), gamma = 5/3; tau = 0.5015 is the stabilisation
+    (0.5e-3, half the physical diffusivity; A17 records the stability boundary found in the oracle)."""
+    gamma = 5.0 / 3.0
+    ux, uy, Bx, By = _config2_uB(n, rms)
+    z = np.zeros((n, n))
+    rho = np.ones((1, n, n))
+    u = np.stack([ux, uy, z])[:, None]
+    B = np.stack([Bx, By, z])[:, None]
+    p = (sound * sound / gamma) * np.ones((1, n, n))
+    F8 = _ideal_Q(rho, u, B, p, gamma)
+    F = np.concatenate([F8, np.zeros((12,) + F8.shape[1:])])        # G and H start at 0 and relax to tau_M grad B, tau_M grad u
+    return dict(name="C2", scheme="FULL", lattice="D2Q9", shape=(n, n), gamma=gamma, c0sq=0.0, nu=nu, eta=eta, tau=tau,
+                powell=1.0, bc=(0,) * 6, steps=steps, fields=np.ascontiguousarray(F), sphere=None, scale=1.0, tau_relax=tau_relax)
+
+
+def config2_incres(n=512, steps=1000, rms=0.02, nu=1e-3, eta=1e-3, c0sq=1.0 / 36.0, eta_jc=0.0):
+    """C2 on the artificial-compressibility reading A3 (scheme INCRES: P, u, B sets; nu and eta through tau): the same recipe at
+    rms 0.02 — at BASELINE's 0.05 this closure is unstable at tau = 0.503 whatever c0^2 (A17)."""
+    ux, uy, Bx, By = _config2_uB(n, rms)
+    F = np.stack([np.zeros_like(ux), ux, uy, Bx, By])[:, None]
+    return dict(name="C2i", scheme="INCRES", lattice="D2Q9", shape=(n, n), gamma=0.0, c0sq=c0sq, nu=nu, eta=eta,
                 tau=0.5 + 3.0 * nu, powell=1.0, bc=(0,) * 6, steps=steps, fields=np.ascontiguousarray(F), sphere=None,
                 scale=1.0, eta_jc=eta_jc)      # eta_jc > 0: the paper's eta(j) = eta0 (1 + (j/j_c)^2) (PAPER.md:215), lattice units
 
@@ -217,11 +243,13 @@ def variant(w, scheme=None, lattice=None, tau_relax=8.0, eta=1e-3, mu=1e-3):
 
 
 def get(name, small=False):
-    """the five configs; small=True gives the reduced sizes the oracle finishes in seconds."""
+    """the five configs (and C2i, config 2 on the INCRES reading); small=True gives the reduced sizes the oracle finishes in seconds."""
     if name == "C1":
         return config1()
     if name == "C2":
         return config2(n=128 if small else 512)
+    if name == "C2i":
+        return config2_incres(n=128 if small else 512)
     if name == "C3":
         return config3(n=160 if small else 1024)
     if name == "C4":

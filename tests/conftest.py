@@ -8,6 +8,11 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
 
+# The parity tests step small lattices many times per call; left to itself lbmhd_step would run those calls as ONE cooperative
+# launch (step_kernel_persist) and the one-launch-per-step kernels would go untested.  Default for the test
+# session: per-step launches; tests/test_persist_gpu.py and the graded / full-size tests set LBMHD_PERSIST themselves.
+os.environ.setdefault("LBMHD_PERSIST", "0")
+
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")

@@ -19,7 +19,7 @@ def test_inplace_random_state_parity(scheme, lattice, shape, bc):
     compare(w, 7, streaming=INPLACE)          # odd count: the state is left in layout P1
 
 
-@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
+@pytest.mark.parametrize("name", ["C1", "C2", "C2i", "C3", "C4", "C5"])
 def test_inplace_config_parity_100_steps(name):
     errs = compare(W.get(name, small=True), 100, streaming=INPLACE)
     print(name, "in place, max field error", errs.max())

@@ -96,11 +96,10 @@ def test_config4_fullsize_sampled():
 
 def test_config3_and_2_fullsize_sampled():
     rng = np.random.default_rng(33)
-    for name, n in (("C3", 1024), ("C2", 512)):
+    for name, n in (("C3", 1024), ("C2", 512), ("C2i", 512)):
         S = [(0, 0, 0), (n - 1, n - 1, 0), (0, n // 2, 0), (n // 2, n - 1, 0), (31, 31, 0), (32, 32, 0)]
         S += [(int(rng.integers(0, n)), int(rng.integers(0, n)), 0) for _ in range(8)]
-        # config 2 is small (8192 tiles): it stays on the one-cell kernel
-        print(name, "full size, worst sampled error", run_fullsize(name, S, path="PATH_MULTI" if name == "C3" else "PATH_ONE"))
+        print(name, "full size, worst sampled error", run_fullsize(name, S, path="PATH_MULTI" if name == "C3" else None))
 
 
 def test_config1_full_size_all_cells_500_steps():

@@ -129,7 +129,7 @@ def test_moving_sphere_parity(lattice, shape):
     compare(w, 12)
 
 
-@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
+@pytest.mark.parametrize("name", ["C1", "C2", "C2i", "C3", "C4", "C5"])
 def test_config_parity_100_steps_reduced_size(name):
     """the five BASELINE configs at the reduced sizes the oracle finishes in seconds, 100 steps"""
     w = W.get(name, small=True)

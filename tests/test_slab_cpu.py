@@ -45,6 +45,23 @@ def test_local_geometry():
     assert owned == list(range(30))
 
 
+def test_step_pieces_and_exchange_kinds():
+    # boundary planes first (those next to a ghost), the rest completes the step; every owned plane exactly once
+    assert slab.step_pieces((1, 65), True, True) == ([(1, 2), (64, 65)], (2, 64))
+    assert slab.step_pieces((0, 10), False, True) == ([(9, 10)], (0, 9))
+    assert slab.step_pieces((1, 11), True, False) == ([(1, 2)], (2, 11))
+    assert slab.step_pieces((1, 2), True, True) == ([(1, 2)], (2, 2))          # one owned plane: no interior
+    assert slab.step_pieces((1, 3), True, True) == ([(1, 2), (2, 3)], (2, 2))
+    assert slab.step_pieces((0, 8), False, False) == ([], (0, 8))
+    for owned, lo, hi in (((1, 65), True, True), ((0, 10), False, True), ((1, 2), True, True), ((1, 3), True, True)):
+        b, (i0, i1) = slab.step_pieces(owned, lo, hi)
+        planes = [p for r in b for p in range(*r)] + list(range(i0, i1))
+        assert sorted(planes) == list(range(*owned))
+    # A/B: always the crossing populations; in place: what a pull-push step pushed goes back, a local step is followed by a refresh
+    assert slab.exchange_kind(0, 0) == slab.CROSSING and slab.exchange_kind(0, 1) == slab.CROSSING
+    assert slab.exchange_kind(1, 0) == slab.RETURN and slab.exchange_kind(1, 1) == slab.CROSSING
+
+
 def test_combine_diag():
     K = 2
     a = np.array([1, 2, 3, 4, 5, 6, 0.1, 1.0, 0.5, 1], dtype=float)
@@ -58,15 +75,20 @@ class FakeSlab:
 
     def __init__(self, rank, lo, hi):
         self.rank, self.lo, self.hi, self.got = rank, lo, hi, {}
+        sides = [side for side, nb in ((0, lo), (1, hi)) if nb is not None]
+        self.send = {s: torch.zeros(4, dtype=torch.float64) for s in sides}
+        self.recv = {s: torch.zeros(4, dtype=torch.float64) for s in sides}
+        self.allocations = 2 * len(sides)
 
-    def halo_buffer(self, full=False):
-        return torch.zeros(4 + 4 * int(full), dtype=torch.float64)
+    def full_buffers(self):
+        self.allocations += 2 * len(self.send)
+        return ({s: torch.zeros(8, dtype=torch.float64) for s in self.send}, {s: torch.zeros(8, dtype=torch.float64) for s in self.recv})
 
-    def halo_pack(self, side, buf, full=False):
-        buf.fill_(100.0 * self.rank + 10.0 * side + int(full))
+    def halo_pack(self, side, buf, what=0, next_copy=False, stream=None):
+        buf.fill_(100.0 * self.rank + 10.0 * side + int(what))
 
-    def halo_unpack(self, side, buf, full=False):
-        self.got[(side, full)] = float(buf[0])
+    def halo_unpack(self, side, buf, what=0, next_copy=False, stream=None):
+        self.got[(side, what)] = float(buf[0])
 
 
 def _worker(rank, world, port, periodic, q):
@@ -74,8 +96,12 @@ def _worker(rank, world, port, periodic, q):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     lo, hi = slab.neighbours(rank, world, periodic)
     s = FakeSlab(rank, lo, hi)
-    slab.exchange_distributed(s, dist, full=False)
-    slab.exchange_distributed(s, dist, full=True)
+    n0 = s.allocations
+    for _ in range(3):                               # crossing / return exchanges reuse the slab's buffers: nothing is allocated per step
+        slab.exchange_distributed(s, dist, slab.CROSSING)
+        slab.exchange_distributed(s, dist, slab.RETURN)
+    assert s.allocations == n0
+    slab.exchange_distributed(s, dist, slab.FULL)
     dist.barrier()
     q.put((rank, s.got))
     dist.destroy_process_group()
@@ -95,7 +121,7 @@ def test_exchange_schedule_over_gloo(world, periodic):
         assert p.exitcode == 0
     for r in range(world):
         lo, hi = slab.neighbours(r, world, periodic)
-        for full in (False, True):
+        for full in (slab.CROSSING, slab.FULL, slab.RETURN):
             # our low ghost holds what the low neighbour packed on ITS high side, and vice versa
             if lo is not None:
                 assert res[r][(0, full)] == 100.0 * lo + 10.0 * 1 + int(full)

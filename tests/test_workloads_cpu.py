@@ -26,6 +26,24 @@ def test_variant_extends_fields_and_parameters():
         W.variant(W.get("C2", small=True), scheme="RESIST")
 
 
+def test_config2_as_stated_and_its_incres_variant_run_in_the_oracle():
+    """C2 = BASELINE's numbers (rms 0.05, nu = eta = 1e-3) on scheme FULL; C2i = the INCRES reading at rms 0.02"""
+    from parity_util import oracle_from_workload
+    w = W.get("C2", small=True)
+    assert w["scheme"] == "FULL" and w["fields"].shape == (20, 1, 128, 128) and w["nu"] == 1e-3 and w["eta"] == 1e-3
+    u = w["fields"][1:3] / w["fields"][0]
+    assert abs(np.sqrt((u * u).sum(0).mean()) - 0.05) < 1e-12 and abs(np.sqrt((w["fields"][5:7] ** 2).sum(0).mean()) - 0.05) < 1e-12
+    wi = W.get("C2i", small=True)
+    assert wi["scheme"] == "INCRES" and wi["fields"].shape == (5, 1, 128, 128)
+    assert abs(np.sqrt((wi["fields"][1:3] ** 2).sum(0).mean()) - 0.02) < 1e-12
+    for ww in (w, wi):
+        o = oracle_from_workload(ww)
+        o.init(ww["fields"])
+        o.step(40)
+        Q, dg = o.moments()
+        assert dg[-1] == 0 and np.isfinite(Q).all()
+
+
 def test_variant_runs_in_the_oracle():
     from parity_util import oracle_from_workload
     w = W.variant(W.config5(shape=(24, 16, 16)), scheme="FULL", lattice="D3Q7")
