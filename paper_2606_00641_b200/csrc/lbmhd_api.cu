@@ -218,8 +218,6 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     h->persist_waves = 2;
     if (const char *e6 = getenv("LBMHD_PERSIST")) { h->persist = atoi(e6) != 0; h->persist_force = atoi(e6) == 2; }
     if (const char *e7 = getenv("LBMHD_PERSIST_WAVES")) h->persist_waves = atoi(e7);
-    h->persist_cluster = true;
-    if (const char *e9 = getenv("LBMHD_PERSIST_CLUSTER")) h->persist_cluster = atoi(e9) != 0;
     h->multi_force = false;
     if (const char *e5 = getenv("LBMHD_MULTI")) h->multi_force = atoi(e5) != 0;
     const char *path = getenv("LBMHD_PATH");      // tuning knob: "plain" forces the register-pull kernel

@@ -68,7 +68,6 @@ struct lbmhd {
   bool cell_force;       // LBMHD_CELL=2: on small grids too (tests)
   bool persist;          // many steps of a small lattice in one cooperative launch (LBMHD_PERSIST=0 turns it off)
   bool persist_force;    // LBMHD_PERSIST=2: take it whatever the lattice size (tests, measurements)
-  bool persist_cluster;  // lattices of <= 16 64-cell tiles: the one-cluster variant with the hardware barrier (LBMHD_PERSIST_CLUSTER=0 turns it off)
   int persist_waves;     // taken when tiles <= persist_waves x co-resident blocks (LBMHD_PERSIST_WAVES)
   bool use_tma;          // TMA-staged persistent step kernel (needs nx * sizeof(real) % 16 == 0)
   bool tma_attr_set;     // its dynamic shared memory attribute has been set on this handle's device

@@ -1051,13 +1051,47 @@ template <typename real, int NC> struct StoreMultiOwn {
 template <class L, typename real, int NC> struct StoreMultiPP {
   char *base;
   const long long *ld_off;
+  int tx;
+  // fp32: a direction with an x-shift lands one cell beside the thread's aligned NC-vector.  Scalar stores there half-fill
+  // 32-byte sectors (ncu: +14 % DRAM write bytes for fp32 in place).  Instead the value that crosses into the
+  // neighbouring lane's vector travels by shuffle and every lane writes its own aligned vector; only the two ends of the
+  // tile (lane 0 / lane 31) still store scalars.  All 32 lanes of the warp call put() together (interior tile).
+  static constexpr bool SHUFFLE = sizeof(real) == 4;
   __device__ __forceinline__ void put(int j, const real (&v)[NC]) const {
     const int i = opp(j);
     if (L::cx(i) == 0) {
       stv<real, NC>(base + ld_off[i], v);
-    } else {
+    } else if (!SHUFFLE) {
 #pragma unroll
       for (int c = 0; c < NC; c++) *reinterpret_cast<real *>(base + ld_off[i] + (long long)(c * sizeof(real))) = v[c];
+    } else if (L::cx(i) < 0) {      // c_jx = +1: cell c goes to x + 1; the own vector is [left lane's last, v[0..NC-2]]
+      char *a0 = base + ld_off[i];                       // where v[0] goes: one element right of the vector start
+      const real left = __shfl_up_sync(0xffffffffu, v[NC - 1], 1);
+      real w[NC];
+      w[0] = left;
+#pragma unroll
+      for (int c = 1; c < NC; c++) w[c] = v[c - 1];
+      if (tx > 0) {
+        stv<real, NC>(a0 - (long long)sizeof(real), w);
+      } else {
+#pragma unroll
+        for (int c = 0; c < NC - 1; c++) *reinterpret_cast<real *>(a0 + (long long)(c * sizeof(real))) = v[c];
+      }
+      if (tx == 31) *reinterpret_cast<real *>(a0 + (long long)((NC - 1) * sizeof(real))) = v[NC - 1];
+    } else {                        // c_jx = -1: cell c goes to x - 1; the own vector is [v[1..NC-1], right lane's first]
+      char *a0 = base + ld_off[i];                       // where v[0] goes: one element left of the vector start
+      const real right = __shfl_down_sync(0xffffffffu, v[0], 1);
+      real w[NC];
+#pragma unroll
+      for (int c = 0; c < NC - 1; c++) w[c] = v[c + 1];
+      w[NC - 1] = right;
+      if (tx < 31) {
+        stv<real, NC>(a0 + (long long)sizeof(real), w);
+      } else {
+#pragma unroll
+        for (int c = 1; c < NC; c++) *reinterpret_cast<real *>(a0 + (long long)(c * sizeof(real))) = v[c];
+      }
+      if (tx == 0) *reinterpret_cast<real *>(a0) = v[0];
     }
   }
 };
@@ -1215,7 +1249,7 @@ step_kernel_multi(const __grid_constant__ StepArgs<real> a, const int nmulti) {
       const StoreMultiOwn<real, NC> st{reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + n)), a.st_off};
       finish_multi<LAT, SCHEME, real, NC, STREAM>(a, tx, k, n, wM, f, st, sQ, sTr);
     } else if (STREAM == ST_PP) {
-      const StoreMultiPP<L, real, NC> st{pb, a.ld_off};
+      const StoreMultiPP<L, real, NC> st{pb, a.ld_off, tx};
       finish_multi<LAT, SCHEME, real, NC, STREAM>(a, tx, k, n, wM, f, st, sQ, sTr);
     } else {
       const StoreMultiOwn<real, NC> st{pb, a.st_off};
@@ -1364,28 +1398,24 @@ template <typename real> struct PersistArgs {
   long long n_tiles;            // tiles_x * ny * nz
 };
 
-// CLBAR = false: a cooperative launch of any size, grid barrier between the steps.
-// CLBAR = true:  the whole lattice fits ONE thread-block cluster (at most 16 CTAs of TX = 64 cells: config 1's 800 cells):
-//                the barrier between the steps is the cluster's hardware barrier (release / acquire: the stores of a step
-//                are visible to the pulls of the next), several times faster than a grid barrier through global memory.
-template <int LAT, int SCHEME, typename real, int TX, int MINB, bool INPLACE, bool CLBAR>
-__global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
+template <int LAT, int SCHEME, typename real, int MINB, bool INPLACE>
+__global__ void __launch_bounds__(32 * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
 step_kernel_persist(const __grid_constant__ StepArgs<real> a0, const __grid_constant__ PersistArgs<real> p) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, K = Vars<SCHEME, D>::K;
-  __shared__ real sQ[K][TX];
-  __shared__ real sTr[D * D][TX];
+  __shared__ real sQ[K][32];
+  __shared__ real sTr[D * D][32];
   __shared__ real sNb[K];
   __shared__ StepArgs<real> sa;
   static_assert(sizeof(StepArgs<real>) % 4 == 0, "word copy");
   namespace cg = cooperative_groups;
-  const int tid = threadIdx.y * TX + threadIdx.x, nthr = TX * K;
+  const int tid = threadIdx.y * 32 + threadIdx.x, nthr = 32 * K;
   {
     const uint32_t *src = reinterpret_cast<const uint32_t *>(&a0);
     uint32_t *dst = reinterpret_cast<uint32_t *>(&sa);
     for (int j = tid; j < (int)(sizeof(StepArgs<real>) / 4); j += nthr) dst[j] = src[j];
   }
-  const Share<real, TX, false> sh{sQ, sTr, sNb, nullptr, nullptr, nullptr, SyncBlock{}};
+  const Share<real, 32, false> sh{sQ, sTr, sNb, nullptr, nullptr, nullptr, SyncBlock{}};
   for (int s = 0; s < p.n_steps; s++) {
     __syncthreads();
     if (tid == 0) {
@@ -1405,19 +1435,12 @@ step_kernel_persist(const __grid_constant__ StepArgs<real> a0, const __grid_cons
       const int bx = (int)(tile % p.tiles_x);
       const long long row = tile / p.tiles_x;
       const int y = (int)(row % a0.ny), z = (int)(row / a0.ny);
-      if constexpr (!INPLACE) run_tile<LAT, SCHEME, real, TX, 0, ST_AB>(sa, threadIdx.x, threadIdx.y, bx * TX, y, z, 0, sh);
-      else if (pullpush) run_tile<LAT, SCHEME, real, TX, 0, ST_PP>(sa, threadIdx.x, threadIdx.y, bx * TX, y, z, 0, sh);
-      else run_tile<LAT, SCHEME, real, TX, 0, ST_LOC>(sa, threadIdx.x, threadIdx.y, bx * TX, y, z, 0, sh);
+      if constexpr (!INPLACE) run_tile<LAT, SCHEME, real, 32, 0, ST_AB>(sa, threadIdx.x, threadIdx.y, bx * 32, y, z, 0, sh);
+      else if (pullpush) run_tile<LAT, SCHEME, real, 32, 0, ST_PP>(sa, threadIdx.x, threadIdx.y, bx * 32, y, z, 0, sh);
+      else run_tile<LAT, SCHEME, real, 32, 0, ST_LOC>(sa, threadIdx.x, threadIdx.y, bx * 32, y, z, 0, sh);
       __syncthreads();      // the exchange arrays are reused by the next tile
     }
-    if (s + 1 < p.n_steps) {      // every store of this step is visible before any pull of the next
-      if constexpr (CLBAR) {
-        cluster_arrive_release();
-        cluster_wait_acquire();
-      } else {
-        cg::this_grid().sync();
-      }
-    }
+    if (s + 1 < p.n_steps) cg::this_grid().sync();      // every store of this step is visible before any pull of the next
   }
 }
 

@@ -256,10 +256,9 @@ template <int LAT, int SCHEME, typename real> struct Ops {
 
   // ---- many steps in one cooperative launch (lbmhd_kernels.cuh, step_kernel_persist) --------------
   static constexpr int MINB_P = minb_for(32 * K, REGS_NEED + 8);
-  static constexpr bool CLP_OK = 64 * K <= 1024;            // the one-cluster variant runs 64-cell tiles: 64 K threads per CTA
   template <bool INPLACE> static int persist_capacity(const lbmhd_t *h) {
     int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, step_kernel_persist<LAT, SCHEME, real, 32, MINB_P, INPLACE, false>, 32 * K, 0) != cudaSuccess)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, step_kernel_persist<LAT, SCHEME, real, MINB_P, INPLACE>, 32 * K, 0) != cudaSuccess)
       return 0;
     return per_sm * h->num_sms;
   }
@@ -273,7 +272,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     if (h->has_sphere && (h->sph_om[0] != 0.0 || h->sph_om[1] != 0.0 || h->sph_om[2] != 0.0)) return false;
     return true;
   }
-  template <bool INPLACE> static void persist_args(lbmhd_t *h, PersistArgs<real> &p, int n_steps, int tx) {
+  template <bool INPLACE> static void persist_args(lbmhd_t *h, PersistArgs<real> &p, int n_steps) {
     memset(&p, 0, sizeof p);
     p.n_steps = n_steps;
     p.inplace = INPLACE ? 1 : 0;
@@ -286,17 +285,17 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     }
     p.t_rel0 = h->t - h->sph_t0;
     for (int c = 0; c < 3; c++) p.sph_c0[c] = h->sph_c0[c];
-    p.tiles_x = (h->p.nx + tx - 1) / tx;
+    p.tiles_x = (h->p.nx + 31) / 32;
     p.n_tiles = (long long)p.tiles_x * h->p.ny * h->p.nz;
   }
   template <bool INPLACE> static int launch_persist(lbmhd_t *h, StepArgs<real> &a, int n_steps, int capacity) {
     PersistArgs<real> p;
-    persist_args<INPLACE>(h, p, n_steps, 32);
+    persist_args<INPLACE>(h, p, n_steps);
     a.row0 = 0;
     a.row1 = n_planes(h);
     const long long want = p.n_tiles < (long long)capacity ? p.n_tiles : (long long)capacity;
     void *params[2] = {(void *)&a, (void *)&p};
-    cudaError_t e = cudaLaunchCooperativeKernel((const void *)step_kernel_persist<LAT, SCHEME, real, 32, MINB_P, INPLACE, false>,
+    cudaError_t e = cudaLaunchCooperativeKernel((const void *)step_kernel_persist<LAT, SCHEME, real, MINB_P, INPLACE>,
                                                 dim3((unsigned)want), dim3(32, K), params, 0, h->stream);
     if (e != cudaSuccess) return fail(LBMHD_ECUDA, "cooperative step kernel launch: %s", cudaGetErrorString(e));
     h->launches += 1;
@@ -304,57 +303,11 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     for (int s = 0; s < n_steps; s++) advance(h);
     return LBMHD_OK;
   }
-  // the whole lattice in one cluster of <= 16 CTAs (64-cell tiles, one per CTA): hardware barrier between the steps
-  template <bool INPLACE> static int launch_persist_cluster(lbmhd_t *h, StepArgs<real> &a, int n_steps) {
-    if constexpr (CLP_OK) {
-      PersistArgs<real> p;
-      persist_args<INPLACE>(h, p, n_steps, 64);
-      a.row0 = 0;
-      a.row1 = n_planes(h);
-      auto kern = step_kernel_persist<LAT, SCHEME, real, 64, 1, INPLACE, true>;
-      if (p.n_tiles > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) {
-        cudaGetLastError();
-        h->persist_cluster = false;
-        return 1;
-      }
-      cudaLaunchConfig_t cfg;
-      memset(&cfg, 0, sizeof cfg);
-      cfg.gridDim = dim3((unsigned)p.n_tiles);
-      cfg.blockDim = dim3(64, K);
-      cfg.stream = h->stream;
-      cudaLaunchAttribute attr[1];
-      attr[0].id = cudaLaunchAttributeClusterDimension;
-      attr[0].val.clusterDim.x = (unsigned)p.n_tiles;
-      attr[0].val.clusterDim.y = 1;
-      attr[0].val.clusterDim.z = 1;
-      cfg.attrs = attr;
-      cfg.numAttrs = 1;
-      cudaError_t e = cudaLaunchKernelEx(&cfg, kern, a, p);
-      if (e != cudaSuccess) {      // e.g. a cluster of this size cannot be co-scheduled here: not sticky, the caller takes another path
-        cudaGetLastError();
-        h->persist_cluster = false;
-        return 1;
-      }
-      h->launches += 1;
-      h->last_path = LBMHD_PATH_PERSIST;
-      for (int s = 0; s < n_steps; s++) advance(h);
-      return LBMHD_OK;
-    } else {
-      return 1;
-    }
-  }
-
   static int step(lbmhd_t *h, int n_steps) {
     StepArgs<real> a;
     make_args(h, a);
     const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
     if (persist_allowed(h, n_steps)) {
-      const long long tiles64 = (long long)((h->p.nx + 63) / 64) * h->p.ny * h->p.nz;
-      if (CLP_OK && h->persist_cluster && tiles64 <= 16) {
-        step_args(h, a);
-        const int rc = inplace ? launch_persist_cluster<true>(h, a, n_steps) : launch_persist_cluster<false>(h, a, n_steps);
-        if (rc <= 0) return rc;      // > 0: the cluster could not be launched here; go on with the cooperative kernel
-      }
       const long long n_tiles = (long long)((h->p.nx + 31) / 32) * h->p.ny * h->p.nz;
       const int cap = inplace ? persist_capacity<true>(h) : persist_capacity<false>(h);
       if (cap > 0 && (h->persist_force || n_tiles <= (long long)h->persist_waves * cap)) {
