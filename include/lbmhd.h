@@ -248,6 +248,25 @@ int lbmhd_copy_probe(const double *a, double *b, size_t n, int reps, void *strea
  * element: 24 n bytes per launch), the second probe SURVEY.md:546-549 asks for beside the copy.  DEVICE pointers. */
 int lbmhd_triad_probe(double *a, const double *b, const double *c, double s, size_t n, int reps, void *stream);
 
+/* The same diagnostics with NO device allocation, NO handle and NO workspace, for callers that cannot allocate: code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc (csrc/lbmhd_noalloc.cu).  The per-block partials
+ * of the two-stage reduction live in one file-scope device array of 1184 x 82 doubles = 776 704 bytes that every GPU which
+ * loads the library holds until the process exits; the call itself allocates nothing.
+ *   scheme, lattice, nx, ny, nz, bc[6] (HOST), gamma   as in lbmhd_params (bc: periodic faces wrap div_h B, the others clamp;
+ *                                                       LBMHD_BC_HALO faces are ghost planes and are not counted)
+ *   fields    DEVICE fp64 [K][N]  (input, e.g. written by lbmhd_moments(on_device))
+ *   diag_out  DEVICE fp64 [3K+4]  (output, the slots of lbmhd_moments)
+ *   device, stream   CUDA device ordinal and cudaStream_t; the two kernels are enqueued on `stream`, nothing synchronises.
+ * Limit: nx * ny * nz <= LBMHD_STATIC_DIAG_MAX_CELLS, else LBMHD_ENOMEM with a message (use lbmhd_diagnostics).
+ * Set-up: the first call on a device looks the array's device address up (cudaGetSymbolAddress); calling with fields == NULL
+ * and diag_out == NULL does only that — do it once per device before capturing a graph.
+ * Sharing: all calls on a device use the one array.  A call writes every slot it reads, so nothing carries over from the
+ * previous call; calls that OVERLAP on the GPU (two streams, two unordered host threads) race on it — serialise them.
+ * The result is bit-identical to lbmhd_diagnostics / lbmhd_moments on the same fields (same kernels, same block count). */
+#define LBMHD_STATIC_DIAG_MAX_CELLS (1ull << 30)
+int lbmhd_diagnostics_static(int scheme, int lattice, int nx, int ny, int nz, const int bc[6], double gamma,
+                             const double *fields, double *diag_out, int device, void *stream);
+
 /* Text of the last error on this thread ("" if none). */
 const char *lbmhd_last_error(void);
 

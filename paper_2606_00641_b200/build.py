@@ -1,7 +1,7 @@
 """Builds the C-ABI CUDA library in-tree for sm_100a with nvcc (no torch in the build).
 
 The kernel templates are instantiated once per (lattice, precision) in csrc/lbmhd_inst.cu; those ten translation units and
-csrc/lbmhd_api.cu compile in parallel into build/*.o and link into liblbmhd.so."""
+csrc/lbmhd_api.cu and csrc/lbmhd_noalloc.cu compile in parallel into build/*.o and link into liblbmhd.so."""
 import os
 import shutil
 import subprocess
@@ -11,7 +11,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "liblbmhd.so")
 OBJ_DIR = os.path.join(_HERE, "build")
-DEPS = [os.path.join(_CSRC, f) for f in ("lbmhd_api.cu", "lbmhd_inst.cu", "lbmhd_host.h", "lbmhd_ops.cuh", "lbmhd_kernels.cuh",
+DEPS = [os.path.join(_CSRC, f) for f in ("lbmhd_api.cu", "lbmhd_inst.cu", "lbmhd_noalloc.cu", "lbmhd_host.h", "lbmhd_ops.cuh", "lbmhd_kernels.cuh",
                                          "lbmhd_lattice.cuh", "lbmhd_tma.cuh")] + \
        [os.path.join(os.path.dirname(_HERE), "include", "lbmhd.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
@@ -24,7 +24,7 @@ def needs_build():
 
 
 def _units():
-    units = [("api", os.path.join(_CSRC, "lbmhd_api.cu"), [])]
+    units = [("api", os.path.join(_CSRC, "lbmhd_api.cu"), []), ("noalloc", os.path.join(_CSRC, "lbmhd_noalloc.cu"), [])]
     for lat in LATTICES:
         for bits in PRECISIONS:
             units.append(("inst_%d_%d" % (lat, bits), os.path.join(_CSRC, "lbmhd_inst.cu"),

@@ -88,6 +88,8 @@ def load_library():
     lib.lbmhd_body_read.argtypes = [C.c_void_p, dp, C.c_int, C.c_int]
     lib.lbmhd_copy_probe.argtypes = [dp, dp, C.c_size_t, C.c_int, C.c_void_p]
     lib.lbmhd_triad_probe.argtypes = [dp, dp, dp, C.c_double, C.c_size_t, C.c_int, C.c_void_p]
+    lib.lbmhd_diagnostics_static.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.c_double, dp, dp, C.c_int,
+                                             C.c_void_p]
     lib.lbmhd_last_error.restype = C.c_char_p
     _lib = lib
     return lib
@@ -99,7 +101,8 @@ EXPORTS = ["lbmhd_num_vars", "lbmhd_num_dirs", "lbmhd_workspace_bytes", "lbmhd_c
            "lbmhd_halo_unpack", "lbmhd_get_populations", "lbmhd_set_populations", "lbmhd_steps_done", "lbmhd_launch_count",
            "lbmhd_copy_probe", "lbmhd_last_error", "lbmhd_body_enable", "lbmhd_body_read",
            "lbmhd_set_sphere_dipoles", "lbmhd_set_obstacle_rotation", "lbmhd_step_path", "lbmhd_triad_probe",
-           "lbmhd_halo_pack_on", "lbmhd_halo_unpack_on", "lbmhd_step_part", "lbmhd_diagnostics", "lbmhd_workspace_bytes_min"]
+           "lbmhd_halo_pack_on", "lbmhd_halo_unpack_on", "lbmhd_step_part", "lbmhd_diagnostics", "lbmhd_workspace_bytes_min",
+           "lbmhd_diagnostics_static"]
 
 
 def _check(rc, allow=()):
@@ -408,3 +411,25 @@ def triad_probe(n_elems=1 << 27, reps=10, device=0):
         e1.synchronize()
         best = max(best, 3 * 8 * n_elems / (e0.elapsed_time(e1) * 1e-3) / 1e9)
     return best
+
+
+STATIC_DIAG_MAX_CELLS = 1 << 30
+
+
+def diagnostics_static(scheme, lattice, shape, bc, gamma, fields_dev, diag_dev, device=0, stream=None):
+    """lbmhd_diagnostics_static: the 3K+4 diagnostics of a device fields tensor with no allocation, no handle, no workspace
+    (scratch in a static device array of the library).  fields_dev [K*N] and diag_dev [3K+4] are CUDA fp64 tensors (both None:
+    set-up only); enqueued on `stream` (default: torch's current stream), nothing synchronises."""
+    import torch
+    lib = load_library()
+    dims = list(shape) + [1] * (3 - len(shape))
+    bcv = (C.c_int * 6)(*[int(b) for b in bc])
+    st = stream if stream is not None else torch.cuda.current_stream(torch.device("cuda", device))
+    fp = None if fields_dev is None else C.c_void_p(fields_dev.data_ptr())
+    dg = None if diag_dev is None else C.c_void_p(diag_dev.data_ptr())
+    if fields_dev is not None:
+        assert fields_dev.is_cuda and fields_dev.dtype == torch.float64 and fields_dev.is_contiguous()
+        assert diag_dev is not None and diag_dev.is_cuda and diag_dev.dtype == torch.float64 and diag_dev.is_contiguous()
+    _check(lib.lbmhd_diagnostics_static(SCHEMES.get(scheme, scheme), LATTICES.get(lattice, lattice), dims[0], dims[1], dims[2], bcv,
+                                        float(gamma), fp, dg, int(device), st.cuda_stream))
+    return diag_dev
