@@ -261,7 +261,8 @@ def run_native(args, rank, world, local_rank):
 
     def leg(streaming):
         """device-resident timing of one streaming layout: inputs already in HBM"""
-        sim = lbmhd.from_workload(w, precision=prec, device=local_rank, streaming=1 if streaming == "inplace" else 0)
+        # no per-cell solid field or porosity in these workloads: the workspace leaves that optional storage out
+        sim = lbmhd.from_workload(w, precision=prec, device=local_rank, streaming=1 if streaming == "inplace" else 0, solid_fields=False)
         sim.init(F_dev)
         sim.step(args.warmup)
         sampler = ClockSampler(local_rank)

@@ -32,25 +32,28 @@ def _units():
     return units
 
 
-def build(force=False, verbose=False, jobs=None):
-    if not force and not needs_build():
+def build(force=False, verbose=False, jobs=None, extra_flags=(), out=None):
+    """extra_flags: more nvcc flags for every unit; out: path of the library to write (default: the in-tree liblbmhd.so)"""
+    out = out or SO
+    if out == SO and not force and not needs_build():
         return SO
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    os.makedirs(OBJ_DIR, exist_ok=True)
+    obj_dir = OBJ_DIR if out == SO else out + ".build"
+    os.makedirs(obj_dir, exist_ok=True)
     jobs = jobs or int(os.environ.get("LBMHD_BUILD_JOBS", "0")) or min(os.cpu_count() or 1, 11)
     extra = ["-Xptxas", "-v"] if verbose else []
 
     def compile_one(unit):
         name, src, defs = unit
-        obj = os.path.join(OBJ_DIR, name + ".o")
-        subprocess.run([nvcc] + NVCC_FLAGS + extra + defs + ["-c", src, "-o", obj], check=True, cwd=_CSRC)
+        obj = os.path.join(obj_dir, name + ".o")
+        subprocess.run([nvcc] + NVCC_FLAGS + extra + list(extra_flags) + defs + ["-c", src, "-o", obj], check=True, cwd=_CSRC)
         return obj
 
     with ThreadPoolExecutor(max_workers=jobs) as pool:
         objs = list(pool.map(compile_one, _units()))
-    subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a"] + objs + ["-o", SO], check=True, cwd=_CSRC)
-    shutil.rmtree(OBJ_DIR, ignore_errors=True)      # intermediates only: every unit depends on the same headers
-    return SO
+    subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a"] + objs + ["-o", out], check=True, cwd=_CSRC)
+    shutil.rmtree(obj_dir, ignore_errors=True)      # intermediates only: every unit depends on the same headers
+    return out
 
 
 if __name__ == "__main__":

@@ -210,7 +210,9 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     h->cluster = p->scheme == LBMHD_RESIST && g.Q > 9 && p->precision == 64;      // measured: pays there only
     if (const char *e4 = getenv("LBMHD_CLUSTER")) h->cluster = h->cluster && atoi(e4) != 0;
     h->last_path = -1;
-    h->cell = true;
+    h->edge_multi = -1;
+    if (const char *e10 = getenv("LBMHD_EDGE_MULTI")) h->edge_multi = atoi(e10) != 0 ? 1 : 0;
+    h->cell = false;      // measured slower than the multi-cell kernel on B200 in all but one case: opt-in
     h->cell_force = false;
     if (const char *e8 = getenv("LBMHD_CELL")) { h->cell = atoi(e8) != 0; h->cell_force = atoi(e8) == 2; }
     h->persist = true;

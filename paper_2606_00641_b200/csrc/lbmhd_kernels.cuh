@@ -33,6 +33,7 @@ template <typename real> struct StepArgs {
   int nx, ny, nz;
   int bc[6];
   real omega[26];               // 1 / tau_k (K <= 26)
+  real tau[26];                 // tau_k (fp32 collide: inj / omega without a division)
   real inv_tauB_cs2;            // 1 / (tau_B c_s^2)
   real kappa, gamma, c0sq;
   real inv_tau_relax;           // kIdealD, kResist: 1 / tau_M of the relaxation variables (Eq.6)
@@ -137,6 +138,102 @@ template <int K, typename real> __device__ __forceinline__ real pick(const real 
     if (k == l) r = v[l];
   return r;
 }
+
+// ---- S2: zeroth moment Q_k = sum_i f_i (Eq.4) ---------------------------------------------------------------
+// fp64: index order, the order of the oracle.  fp32: the rounding error d of this sum re-enters the populations as w_i omega d
+// (Eq.2-3) and so lands, amplified by omega ~ 2, in the conserved sum itself every step: it is the largest single source of
+// fp32 drift (config 4, 100 steps: 1.2e-5 on rho with the index-order sum).  So fp32 adds the small populations first —
+// diagonal directions (w = 1/36), then axis directions, the rest population (the largest) last — with two accumulators per
+// weight class: the same Q - 1 additions, shorter dependency chains, partial sums that stay small until the last two adds.
+// two_sum: s = fl(a + b) and e with a + b = s + e exactly (Knuth); no multiplication, so nothing here can be contracted.
+template <typename real> __device__ __forceinline__ void two_sum(real a, real b, real &s, real &e) {
+  s = a + b;
+  const real bb = s - a;
+  e = (a - (s - bb)) + (b - bb);
+}
+
+// lo (fp32 only; 0 in fp64): what the last two additions of the sum rounded away, Q_k = result + lo to second order.
+template <class L, typename real, class FA> __device__ __forceinline__ real moment_sum(const FA &f, real &lo) {
+  constexpr int Q = L::Q;
+  if constexpr (sizeof(real) == 8) {
+    real s = real(0);
+#pragma unroll
+    for (int i = 0; i < Q; i++) s += f[i];
+    lo = real(0);
+    return s;
+  } else {
+    real d0 = real(0), d1 = real(0), a0 = real(0), a1 = real(0);
+    int nd = 0, na = 0;
+#pragma unroll
+    for (int i = 1; i < Q; i++) {
+      const int c2 = L::cx(i) * L::cx(i) + L::cy(i) * L::cy(i) + L::cz(i) * L::cz(i);
+      if (c2 > 1) {
+        if (nd++ & 1) d1 += f[i];
+        else d0 += f[i];
+      } else {
+        if (na++ & 1) a1 += f[i];
+        else a0 += f[i];
+      }
+    }
+    real s1, e1, hi, e2;
+    two_sum<real>(d0 + d1, a0 + a1, s1, e1);
+    two_sum<real>(s1, f[0], hi, e2);
+    lo = e1 + e2;
+    return hi;
+  }
+}
+template <class L, typename real, class FA> __device__ __forceinline__ real moment_sum(const FA &f) {
+  real lo;
+  return moment_sum<L, real>(f, lo);
+}
+
+// ---- S7 BGK + direct injection (Eq.2-3, A5), the populations of one (cell, variable) ------------------------
+//   g'_i = f_i + w [ w_i (Q_k + c_i.Phi/c_s^2) - f_i ] + w_i inj          (w = omega_k)
+// fp64: evaluated as (1 - w) f_i + w_i [w Q_k + inj] + w_i c_i.(3 w Phi): 52 instructions per thread on D3Q19.
+// fp32: that form rounds w Q_k + inj and w_i [..] to 6e-8 of Q_k, and those roundings — like the one of the moment sum — land
+// in sum_i g'_i, i.e. in the conserved quantity, every step (config 4, 100 steps: 1.2e-5 .. 2.4e-5 on rho and B_y).  Here the
+// relaxation acts on the DEVIATION e_i = w_i Qe - f_i + w_i c_i.Phi/c_s^2, a small number whose rounding is small in absolute
+// terms, with Qe = fl(Q_k + inj / w); what the additions that formed Q_k and Qe rounded away (lo, err: error-free
+// transformations) is handed to the rest population, so that sum_i g'_i = Q_k + inj up to the rounding of the Q stores
+// themselves.  Same instruction count per population (one FFMA instead of the FMUL).
+template <class L, typename real> struct Collide {
+  Collide() = default;
+  real om, a0, a1, P0, P1, P2;      // fp64: a0 = 1 - w, a1 = w Q_k + inj, P = 3 w Phi | fp32: a0 = Qe, a1 = lo + err, P = 3 Phi
+  __device__ __forceinline__ Collide(real om_, real tau, real Qk, real lo, real inj, const real (&Phi)[3]) : om(om_) {
+    if constexpr (sizeof(real) == 8) {
+      a0 = real(1) - om;
+      a1 = om * Qk + inj;
+      P0 = real(L::inv_cs2) * om * Phi[0]; P1 = real(L::inv_cs2) * om * Phi[1]; P2 = real(L::inv_cs2) * om * Phi[2];
+    } else {
+      real err;
+      two_sum<real>(Qk, inj * tau, a0, err);
+      a1 = lo + err;
+      P0 = real(L::inv_cs2) * Phi[0]; P1 = real(L::inv_cs2) * Phi[1]; P2 = real(L::inv_cs2) * Phi[2];
+    }
+  }
+  // out(i, f) == f: a frozen cell that goes through the tile's update unchanged
+  __device__ __forceinline__ void identity() {
+    if constexpr (sizeof(real) == 8) { a0 = real(1); a1 = real(0); }
+    else { om = real(0); a0 = real(0); a1 = real(0); }
+    P0 = P1 = P2 = real(0);
+  }
+  __device__ __forceinline__ real out(int i, real fi) const {
+    if constexpr (sizeof(real) == 8) {
+      real t = real(L::w(i)) * a1;
+      if (L::cx(i) != 0) t = fma(real(L::cx(i) * L::w(i)), P0, t);
+      if (L::cy(i) != 0) t = fma(real(L::cy(i) * L::w(i)), P1, t);
+      if (L::cz(i) != 0) t = fma(real(L::cz(i) * L::w(i)), P2, t);
+      return fma(fi, a0, t);
+    } else {
+      real e = fma(real(L::w(i)), a0, -fi);
+      if (L::cx(i) != 0) e = fma(real(L::cx(i) * L::w(i)), P0, e);
+      if (L::cy(i) != 0) e = fma(real(L::cy(i) * L::w(i)), P1, e);
+      if (L::cz(i) != 0) e = fma(real(L::cz(i) * L::w(i)), P2, e);
+      if (i == 0) e += a1;
+      return fma(om, e, fi);
+    }
+  }
+};
 
 // ---- flux row of variable k: Phi_k,alpha(Qh), alpha < D (Eq.11, Eq.8; A3) -------
 // Qh is the (possibly solid-blended) state: an array in registers or a column of the shared exchange array (QCol) — the
@@ -622,9 +719,8 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   }
 
   // S2 zeroth moment of this set (index order) and S3 this set's share of tr Pi_B
-  real Qk = real(0);
-#pragma unroll
-  for (int i = 0; i < Q; i++) Qk += f[i];
+  real Qlo;
+  const real Qk = moment_sum<L, real>(f, Qlo);
   sh.putQ(k, tx, Qk);
   if (k >= iB && k < iB + D) {
     const int b = k - iB;   // warp-uniform
@@ -736,20 +832,12 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   // in place: cells next to a non-periodic face publish their post-collision moment (sum_i g'_i = Q_k + inj)
   if (STREAM != ST_AB && c.writeM) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + c.n] = (double)(Qk + inj);
 
-  // S7 BGK + direct injection, S8 store:
-  //   g'_i = (1 - w) f_i + w_i [ w Q_k + inj ] + w_i (c_i . 3 w Phi)       (w = omega_k; Eq.2-3, 3 = 1/c_s^2)
+  // S7 BGK + direct injection (Collide), S8 store
   const real om = (SCHEME == kIncres && omB > real(0) && k >= iB) ? omB : a.omega[k];
-  const real omc = real(1) - om;
-  const real b0 = om * Qk + inj;
-  const real P0 = real(L::inv_cs2) * om * Phi[0], P1 = real(L::inv_cs2) * om * Phi[1], P2 = real(L::inv_cs2) * om * Phi[2];
+  const real tauk = (SCHEME == kIncres && omB > real(0) && k >= iB) ? real(1) / omB : a.tau[k];
+  const Collide<L, real> col(om, tauk, Qk, Qlo, inj, Phi);
 #pragma unroll
-  for (int i = 0; i < Q; i++) {
-    real t = real(L::w(i)) * b0;
-    if (L::cx(i) != 0) t = fma(real(L::cx(i) * L::w(i)), P0, t);
-    if (L::cy(i) != 0) t = fma(real(L::cy(i) * L::w(i)), P1, t);
-    if (L::cz(i) != 0) t = fma(real(L::cz(i) * L::w(i)), P2, t);
-    store.put(i, fma(f[i], omc, t));
-  }
+  for (int i = 0; i < Q; i++) store.put(i, col.out(i, f[i]));
 }
 
 // =====================================================================================================
@@ -1048,22 +1136,41 @@ template <typename real, int NC> struct StoreMultiOwn {
   const long long *st_off;
   __device__ __forceinline__ void put(int j, const real (&v)[NC]) const { stv<real, NC>(base + st_off[j], v); }
 };
-template <class L, typename real, int NC> struct StoreMultiPP {
+// EDGE (step_kernel_multi<.., EDGE = true> only): `edge` = 1 / 2 when the tile holds the cell ON the x = 0 / x = nx - 1 face
+// (lane 0's first cell / lane 31's last cell): its pushes across the face go to the other end of the row (periodic) or stay in
+// the cell's own slot j; 0 for a tile that is interior in x.
+template <class L, typename real, int NC, bool EDGE = false> struct StoreMultiPP {
   char *base;
   const long long *ld_off;
   int tx;
+  const long long *st_off;      // EDGE only
+  int edge;                     // EDGE only
+  bool wrap;                    // EDGE only: periodic x
+  long long wrap_adj;           // EDGE only: +- nx * sizeof(real)
   // fp32: a direction with an x-shift lands one cell beside the thread's aligned NC-vector.  Scalar stores there half-fill
   // 32-byte sectors (ncu: +14 % DRAM write bytes for fp32 in place).  Instead the value that crosses into the
   // neighbouring lane's vector travels by shuffle and every lane writes its own aligned vector; only the two ends of the
-  // tile (lane 0 / lane 31) still store scalars.  All 32 lanes of the warp call put() together (interior tile).
+  // tile (lane 0 / lane 31) still store scalars.  All 32 lanes of the warp call put() together.
   static constexpr bool SHUFFLE = sizeof(real) == 4;
+  // where the value of the cell at the low (c = 0 of lane 0) / high (c = NC - 1 of lane 31) end of the tile goes
+  __device__ __forceinline__ char *end_target(int j, char *plain, int c, bool low_end) const {
+    if constexpr (EDGE) {
+      if (edge == (low_end ? 1 : 2)) return wrap ? plain + wrap_adj : base + st_off[j] + (long long)(c * sizeof(real));
+    }
+    return plain;
+  }
   __device__ __forceinline__ void put(int j, const real (&v)[NC]) const {
     const int i = opp(j);
     if (L::cx(i) == 0) {
       stv<real, NC>(base + ld_off[i], v);
     } else if (!SHUFFLE) {
 #pragma unroll
-      for (int c = 0; c < NC; c++) *reinterpret_cast<real *>(base + ld_off[i] + (long long)(c * sizeof(real))) = v[c];
+      for (int c = 0; c < NC; c++) {
+        char *t = base + ld_off[i] + (long long)(c * sizeof(real));
+        if (EDGE && c == 0 && L::cx(i) > 0 && tx == 0) t = end_target(j, t, 0, true);
+        if (EDGE && c == NC - 1 && L::cx(i) < 0 && tx == 31) t = end_target(j, t, NC - 1, false);
+        *reinterpret_cast<real *>(t) = v[c];
+      }
     } else if (L::cx(i) < 0) {      // c_jx = +1: cell c goes to x + 1; the own vector is [left lane's last, v[0..NC-2]]
       char *a0 = base + ld_off[i];                       // where v[0] goes: one element right of the vector start
       const real left = __shfl_up_sync(0xffffffffu, v[NC - 1], 1);
@@ -1077,7 +1184,7 @@ template <class L, typename real, int NC> struct StoreMultiPP {
 #pragma unroll
         for (int c = 0; c < NC - 1; c++) *reinterpret_cast<real *>(a0 + (long long)(c * sizeof(real))) = v[c];
       }
-      if (tx == 31) *reinterpret_cast<real *>(a0 + (long long)((NC - 1) * sizeof(real))) = v[NC - 1];
+      if (tx == 31) *reinterpret_cast<real *>(end_target(j, a0 + (long long)((NC - 1) * sizeof(real)), NC - 1, false)) = v[NC - 1];
     } else {                        // c_jx = -1: cell c goes to x - 1; the own vector is [v[1..NC-1], right lane's first]
       char *a0 = base + ld_off[i];                       // where v[0] goes: one element left of the vector start
       const real right = __shfl_down_sync(0xffffffffu, v[0], 1);
@@ -1091,28 +1198,27 @@ template <class L, typename real, int NC> struct StoreMultiPP {
 #pragma unroll
         for (int c = 1; c < NC; c++) *reinterpret_cast<real *>(a0 + (long long)(c * sizeof(real))) = v[c];
       }
-      if (tx == 0) *reinterpret_cast<real *>(a0) = v[0];
+      if (tx == 0) *reinterpret_cast<real *>(end_target(j, a0, 0, true)) = v[0];
     }
   }
 };
 
 // S2-S8 of NC fluid cells of an interior tile (no boundary, no solid, constant eta).  sQ / sTr rows are laid out
 // [c][32] (cell c of lane tx at c*32 + tx): conflict-free scalar accesses.
-template <int LAT, int SCHEME, typename real, int NC, int STREAM, class Store>
+// pass[c] (EDGE tiles only): cell c is a frozen face cell whose f already holds what it keeps / emits (A10): unchanged.
+template <int LAT, int SCHEME, typename real, int NC, int STREAM, bool EDGE = false, class Store>
 __device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, int k, uint32_t n, const bool (&writeM)[NC],
-                                             real (&f)[NC][Lattice<LAT>::Q], const Store &store, real (*sQ)[32 * NC],
-                                             real (*sTr)[32 * NC]) {
+                                             const bool (&pass)[NC], real (&f)[NC][Lattice<LAT>::Q], const Store &store,
+                                             real (*sQ)[32 * NC], real (*sTr)[32 * NC]) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
   using V = Vars<SCHEME, D>;
   constexpr int K = V::K, iB = V::iB;
   constexpr bool use_tr = !has_relax(SCHEME);       // A6; the schemes with gradient sets take div B from them
-  real Qk[NC];
+  real Qk[NC], Qlo[NC];
 #pragma unroll
   for (int c = 0; c < NC; c++) {
-    real s = real(0);
-#pragma unroll
-    for (int i = 0; i < Q; i++) s += f[c][i];
+    const real s = moment_sum<L, real>(f[c], Qlo[c]);
     Qk[c] = s;
     sQ[k][c * 32 + tx] = s;
   }
@@ -1130,9 +1236,8 @@ __device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, in
     }
   }
   __syncthreads();
-  const real om = a.omega[k], omc = real(1) - om;
-  const real ic = real(L::inv_cs2) * om;
-  real b0[NC], P[NC][3];
+  const real om = a.omega[k];
+  real injv[NC], P[NC][3];
   // The flux / source code of the NC cells, with the row either a compile-time constant (one copy of the code per row, chosen
   // by dispatch_row: no selects, no unused terms, but K times the code) or the run-time k.  Measured on B200:
   // the constant-row form pays where the kernel is bound by instruction issue (fp32; fp64 on the short lattices; the 20 / 26
@@ -1176,32 +1281,130 @@ __device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, in
         if (has_relax(SCHEME) && KC >= 8) inj = -Qk[c] * a.inv_tau_relax;      // relaxation source of Eq.6
       }
       if (STREAM != ST_AB && writeM[c]) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + n + c] = (double)(Qk[c] + inj);
-      b0[c] = om * Qk[c] + inj;
-      P[c][0] = ic * Phi[0]; P[c][1] = ic * Phi[1]; P[c][2] = ic * Phi[2];
+      injv[c] = inj;
+      P[c][0] = Phi[0]; P[c][1] = Phi[1]; P[c][2] = Phi[2];
     }
   };
   if constexpr (ROWCONST) dispatch_row<0, K>(k, cells);
   else cells(k);
+  Collide<L, real> col[NC];
+#pragma unroll
+  for (int c = 0; c < NC; c++) {
+    col[c] = Collide<L, real>(om, a.tau[k], Qk[c], Qlo[c], injv[c], P[c]);
+    if (EDGE && pass[c]) col[c].identity();
+  }
 #pragma unroll
   for (int i = 0; i < Q; i++) {
     real out[NC];
 #pragma unroll
-    for (int c = 0; c < NC; c++) {
-      real t = real(L::w(i)) * b0[c];
-      if (L::cx(i) != 0) t = fma(real(L::cx(i) * L::w(i)), P[c][0], t);
-      if (L::cy(i) != 0) t = fma(real(L::cy(i) * L::w(i)), P[c][1], t);
-      if (L::cz(i) != 0) t = fma(real(L::cz(i) * L::w(i)), P[c][2], t);
-      out[c] = fma(f[c][i], omc, t);
-    }
+    for (int c = 0; c < NC; c++) out[c] = col[c].out(i, f[c][i]);
     store.put(i, out);
   }
 }
 
-// Row layout: [32-cell edge tile][nmulti tiles of 32*NC cells][rest in 32-cell tiles], one block each, so that the
-// multi-cell tiles are all interior in x; blocks 0..nmulti-1 are those tiles, block nmulti the first edge tile.
-template <int LAT, int SCHEME, typename real, int NC, int MINB, int STREAM>
+// Pulls of a multi-cell tile that holds the cell ON an x face of an otherwise interior row (no mask, sphere out of reach).
+// Only the face cell (first cell of lane 0 in the tile at x = 0, last cell of lane 31 in the tile that ends at nx) differs
+// from the interior tile (A9-A11), as in the 32-cell x-edge path of run_tile():
+//   periodic x   its pulls across the face come from the other end of the row (its in-place pushes go there: StoreMultiPP);
+//   ZEROGRAD     those pulls are replaced by f^eq of the inward neighbour's state Q^nb (A/B: its Q stored populations fetched
+//                one per lane and summed by shuffles; in place: published in M_cur), exchanged through sNb: one more barrier;
+//   INFLOW       the cell is frozen: f takes what it holds (A/B: its own stored populations; in place: f^eq of its constant
+//                state in M_cur) and finish_multi passes it through unchanged.
+template <int LAT, int SCHEME, typename real, int NC, int STREAM>
+__device__ __forceinline__ void edge_multi_pull(const StepArgs<real> &a, const int tx, const int k, char *__restrict__ pb, const int y, const int z,
+                                                const bool edge_lo, real (&f)[NC][Lattice<LAT>::Q], real *sNb) {
+  using L = Lattice<LAT>;
+  constexpr int D = L::D, Q = L::Q;
+  constexpr int K = Vars<SCHEME, D>::K;
+  const int nx = a.nx, ny = a.ny, nz = a.nz;
+  const int bcf = edge_lo ? a.bc[0] : a.bc[1];
+  const bool frozen = bcf == BC_INFLOW, zg = bcf == BC_ZEROGRAD, wrap = bcf == BC_PERIODIC;      // tile-uniform
+  const bool face_thread = edge_lo ? tx == 0 : tx == 31;
+  const long long wrap_adj = (long long)nx * (long long)sizeof(real) * (edge_lo ? 1 : -1);
+#pragma unroll
+  for (int i = 0; i < Q; i++) {
+    if (STREAM == ST_LOC || L::cx(i) == 0) {
+      real v[NC];
+      ldv<real, NC>(pb + (STREAM == ST_LOC ? a.st_off[opp(i)] : a.ld_off[i]), v);
+#pragma unroll
+      for (int c = 0; c < NC; c++) f[c][i] = v[c];
+    } else {
+#pragma unroll
+      for (int c = 0; c < NC; c++) {
+        long long off = a.ld_off[i] + (long long)(c * sizeof(real));
+        // the pull of the face cell that crosses the face: c_ix = +1 at x = 0 (first cell), c_ix = -1 at x = nx - 1 (last cell)
+        const bool cross = face_thread && ((c == 0 && L::cx(i) > 0 && edge_lo) || (c == NC - 1 && L::cx(i) < 0 && !edge_lo));
+        if (cross && wrap) off += wrap_adj;
+        f[c][i] = (cross && !wrap) ? real(0) : *reinterpret_cast<const real *>(pb + off);
+      }
+    }
+  }
+  const uint32_t nrow = ((uint32_t)z * ny + y) * nx;
+  if (frozen && face_thread) {
+    const int cf = edge_lo ? 0 : NC - 1;
+    if (STREAM == ST_AB) {      // the face cell's own stored populations
+#pragma unroll
+      for (int i = 0; i < Q; i++) {
+        const real own = *reinterpret_cast<const real *>(pb + a.st_off[i] + (long long)(cf * sizeof(real)));
+        if (edge_lo) f[0][i] = own;
+        else f[NC - 1][i] = own;
+      }
+    } else {                    // in place its slots are in flux: f^eq of its constant state
+      const size_t N = (size_t)nx * ny * nz;
+      const uint32_t nface = nrow + (edge_lo ? 0 : nx - 1);
+      real Qf[K], Phi[3];
+#pragma unroll
+      for (int l = 0; l < K; l++) Qf[l] = (real)a.M_cur[(size_t)l * N + nface];
+      const real Qfk = pick<K, real>(Qf, k);
+      flux_row<SCHEME, D, real>(k, Qf, Qfk, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
+#pragma unroll
+      for (int i = 0; i < Q; i++) {
+        const real cPhi = real(L::cx(i)) * Phi[0] + real(L::cy(i)) * Phi[1] + real(L::cz(i)) * Phi[2];
+        const real fe = real(L::w(i)) * (Qfk + real(L::inv_cs2) * cPhi);
+        if (edge_lo) f[0][i] = fe;
+        else f[NC - 1][i] = fe;
+      }
+    }
+  }
+  if (zg) {
+    const uint32_t nb = nrow + (edge_lo ? 1 : nx - 2);
+    if (STREAM == ST_AB) {      // lane j < Q fetches g_{k,j}(nb); butterfly sum -> Q^nb_k in every lane
+      real v = tx < Q ? a.src[(size_t)k * Q * a.pstride + (size_t)tx * a.pstride + nb] : real(0);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+      if (tx == 0) sNb[k] = v;
+    } else {
+      if (tx == 0) sNb[k] = (real)a.M_cur[(size_t)k * ((size_t)nx * ny * nz) + nb];
+    }
+    __syncthreads();
+    if (face_thread) {
+      real Qnb[K], Phi[3];
+#pragma unroll
+      for (int l = 0; l < K; l++) Qnb[l] = sNb[l];
+      const real Qnbk = pick<K, real>(Qnb, k);
+      flux_row<SCHEME, D, real>(k, Qnb, Qnbk, a.gamma, a.c0sq, a.eta, a.mu, a.inv_tau_relax, Phi);
+#pragma unroll
+      for (int i = 0; i < Q; i++) {
+        if (L::cx(i) != 0) {
+          const real cPhi = real(L::cx(i)) * Phi[0] + real(L::cy(i)) * Phi[1] + real(L::cz(i)) * Phi[2];
+          const real fe = real(L::w(i)) * (Qnbk + real(L::inv_cs2) * cPhi);
+          if (L::cx(i) > 0 && edge_lo) f[0][i] = fe;
+          if (L::cx(i) < 0 && !edge_lo) f[NC - 1][i] = fe;
+        }
+      }
+    }
+  }
+}
+
+// Row layout.  EDGE = false (any nx that is a multiple of the vector width): [32-cell edge tile][nmulti tiles of 32*NC cells]
+// [rest in 32-cell tiles], one block each, so that the multi-cell tiles are all interior in x; blocks 0..nmulti-1 are those
+// tiles, block nmulti the first edge tile; xbase = 32.  EDGE = true (nx a multiple of the tile width W = 32 NC, at least two
+// tiles; xbase = 0): nmulti = nx / W multi-cell tiles cover the whole row, the first and the last hold the face cells
+// (edge_multi_pull).  EDGE is a template parameter so that the kernels of the lattices / precisions where it does not pay
+// are compiled exactly as without it.
+template <int LAT, int SCHEME, typename real, int NC, int MINB, int STREAM, bool EDGE>
 __global__ void __launch_bounds__(32 * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
-step_kernel_multi(const __grid_constant__ StepArgs<real> a, const int nmulti) {
+step_kernel_multi(const __grid_constant__ StepArgs<real> a, const int nmulti, const int xbase) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, Q = L::Q;
   using V = Vars<SCHEME, D>;
@@ -1220,40 +1423,52 @@ step_kernel_multi(const __grid_constant__ StepArgs<real> a, const int nmulti) {
     run_tile<LAT, SCHEME, real, 32, 0, STREAM>(a, tx, k, t == 0 ? 0 : 32 + W * nmulti + 32 * (t - 1), y, z, 0, sh32);
     return;
   }
-  const int x0 = 32 + (int)blockIdx.x * W;
+  const int x0 = xbase + (int)blockIdx.x * W;
   const bool npx = a.bc[0] != BC_PERIODIC, npy = D > 1 && a.bc[2] != BC_PERIODIC, npz = D > 2 && a.bc[4] != BC_PERIODIC;
   const bool row_inner = (D < 2 || (y >= 1 && y <= ny - 2)) && (D < 3 || (z >= 1 && z <= nz - 2));
-  const bool interior = x0 >= 1 && x0 + W <= nx - 1 && row_inner && a.mask == nullptr && !sphere_may_touch<real, D>(a, x0, W, y, z);
-  if (interior) {
+  const int edge = !EDGE ? 0 : (x0 == 0 ? 1 : (x0 + W >= nx ? 2 : 0));
+  const bool lean = (EDGE || (x0 >= 1 && x0 + W <= nx - 1)) && row_inner && a.mask == nullptr && !sphere_may_touch<real, D>(a, x0, W, y, z);
+  if (lean) {
     const int x = x0 + NC * tx;
     const uint32_t n = ((uint32_t)z * ny + y) * nx + x;
     char *__restrict__ pb = reinterpret_cast<char *>(const_cast<real *>(a.src) + ((size_t)k * Q * a.pstride + n));
     real f[NC][Q];
+    if (!EDGE || edge == 0) {
 #pragma unroll
-    for (int i = 0; i < Q; i++) {
-      if (STREAM == ST_LOC || L::cx(i) == 0) {
-        real v[NC];
-        ldv<real, NC>(pb + (STREAM == ST_LOC ? a.st_off[opp(i)] : a.ld_off[i]), v);
+      for (int i = 0; i < Q; i++) {
+        if (STREAM == ST_LOC || L::cx(i) == 0) {
+          real v[NC];
+          ldv<real, NC>(pb + (STREAM == ST_LOC ? a.st_off[opp(i)] : a.ld_off[i]), v);
 #pragma unroll
-        for (int c = 0; c < NC; c++) f[c][i] = v[c];
-      } else {
+          for (int c = 0; c < NC; c++) f[c][i] = v[c];
+        } else {
 #pragma unroll
-        for (int c = 0; c < NC; c++) f[c][i] = *reinterpret_cast<const real *>(pb + a.ld_off[i] + (long long)(c * sizeof(real)));
+          for (int c = 0; c < NC; c++) f[c][i] = *reinterpret_cast<const real *>(pb + a.ld_off[i] + (long long)(c * sizeof(real)));
+        }
       }
+    } else {
+      if constexpr (EDGE) edge_multi_pull<LAT, SCHEME, real, NC, STREAM>(a, tx, k, pb, y, z, edge == 1, f, sNb);
     }
     const bool rowM = STREAM != ST_AB && ((npy && (y == 1 || y == ny - 2)) || (npz && (z == 1 || z == nz - 2)));
-    bool wM[NC];
+    const bool frozen_face = EDGE && edge != 0 && (edge == 1 ? a.bc[0] : a.bc[1]) == BC_INFLOW;
+    bool wM[NC], pass[NC];
 #pragma unroll
-    for (int c = 0; c < NC; c++) wM[c] = rowM || (npx && (x + c == 1 || x + c == nx - 2));
+    for (int c = 0; c < NC; c++) {
+      // EDGE: the frozen face cell goes through unchanged and publishes nothing (its state is constant); the face cell of a
+      // zero-gradient face publishes its moment like its neighbour does (every cell of an x-edge tile does in run_tile)
+      pass[c] = frozen_face && ((edge == 1 && tx == 0 && c == 0) || (edge == 2 && tx == 31 && c == NC - 1));
+      wM[c] = (rowM || (npx && (EDGE ? (x + c <= 1 || x + c >= nx - 2) : (x + c == 1 || x + c == nx - 2)))) && !pass[c];
+    }
     if (STREAM == ST_AB) {
       const StoreMultiOwn<real, NC> st{reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + n)), a.st_off};
-      finish_multi<LAT, SCHEME, real, NC, STREAM>(a, tx, k, n, wM, f, st, sQ, sTr);
+      finish_multi<LAT, SCHEME, real, NC, STREAM, EDGE>(a, tx, k, n, wM, pass, f, st, sQ, sTr);
     } else if (STREAM == ST_PP) {
-      const StoreMultiPP<L, real, NC> st{pb, a.ld_off, tx};
-      finish_multi<LAT, SCHEME, real, NC, STREAM>(a, tx, k, n, wM, f, st, sQ, sTr);
+      const StoreMultiPP<L, real, NC, EDGE> st{pb, a.ld_off, tx, a.st_off, edge, !npx,
+                                               (long long)nx * (long long)sizeof(real) * (edge == 1 ? 1 : -1)};
+      finish_multi<LAT, SCHEME, real, NC, STREAM, EDGE>(a, tx, k, n, wM, pass, f, st, sQ, sTr);
     } else {
       const StoreMultiOwn<real, NC> st{pb, a.st_off};
-      finish_multi<LAT, SCHEME, real, NC, STREAM>(a, tx, k, n, wM, f, st, sQ, sTr);
+      finish_multi<LAT, SCHEME, real, NC, STREAM, EDGE>(a, tx, k, n, wM, pass, f, st, sQ, sTr);
     }
     return;
   }
@@ -1334,13 +1549,10 @@ step_kernel_cell(const __grid_constant__ StepArgs<real> a, const int ncell) {
 #pragma unroll
     for (int i = 0; i < Q; i++)
       f[l][i] = *reinterpret_cast<const real *>(pb + (long long)l * a.kplane + (STREAM == ST_LOC ? a.st_off[opp(i)] : a.ld_off[i]));
-  real Qv[K];
+  real Qv[K], Qlo[K];
 #pragma unroll
-  for (int l = 0; l < K; l++) {      // S2 zeroth moments, index order
-    real s = real(0);
-#pragma unroll
-    for (int i = 0; i < Q; i++) s += f[l][i];
-    Qv[l] = s;
+  for (int l = 0; l < K; l++) {      // S2 zeroth moments
+    Qv[l] = moment_sum<L, real>(f[l], Qlo[l]);
   }
   real delta;                        // S3 (A6) or the relaxation variable (A19)
   if constexpr (SCHEME == kIdealD) {
@@ -1366,17 +1578,10 @@ step_kernel_cell(const __grid_constant__ StepArgs<real> a, const int ncell) {
     real inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(l, Qv);
     if (has_relax(SCHEME) && l >= 8) inj = -Qv[l] * a.inv_tau_relax;
     if (STREAM != ST_AB && wM) a.M_next[(size_t)l * ((size_t)nx * ny * nz) + n] = (double)(Qv[l] + inj);
-    const real om = a.omega[l], omc = real(1) - om;
-    const real b0 = om * Qv[l] + inj;
-    const real P0 = real(L::inv_cs2) * om * Phi[0], P1 = real(L::inv_cs2) * om * Phi[1], P2 = real(L::inv_cs2) * om * Phi[2];
+    const Collide<L, real> col(a.omega[l], a.tau[l], Qv[l], Qlo[l], inj, Phi);
 #pragma unroll
-    for (int i = 0; i < Q; i++) {
-      real t = real(L::w(i)) * b0;
-      if (L::cx(i) != 0) t = fma(real(L::cx(i) * L::w(i)), P0, t);
-      if (L::cy(i) != 0) t = fma(real(L::cy(i) * L::w(i)), P1, t);
-      if (L::cz(i) != 0) t = fma(real(L::cz(i) * L::w(i)), P2, t);
-      *reinterpret_cast<real *>(ob + (long long)l * a.kplane + (STREAM == ST_PP ? a.ld_off[opp(i)] : a.st_off[i])) = fma(f[l][i], omc, t);
-    }
+    for (int i = 0; i < Q; i++)
+      *reinterpret_cast<real *>(ob + (long long)l * a.kplane + (STREAM == ST_PP ? a.ld_off[opp(i)] : a.st_off[i])) = col.out(i, f[l][i]);
   }
 }
 
@@ -1481,10 +1686,10 @@ moments_kernel(const real *__restrict__ g, size_t pstride, double *__restrict__ 
   const size_t N = (size_t)nx * ny * nz;
   const size_t n = ((size_t)blockIdx.z * ny + blockIdx.y) * nx + x;
   const real *gk = g + (size_t)k * Q * pstride;
-  real s = real(0);
+  double s = 0.0;      // fp64 accumulation in both precisions: the output is fp64 and an fp32 sum would only add its own rounding
 #pragma unroll
-  for (int i = 0; i < Q; i++) s += gk[(size_t)i * pstride + n];
-  out[(size_t)k * N + n] = (double)s;
+  for (int i = 0; i < Q; i++) s += (double)gk[(size_t)i * pstride + n];
+  out[(size_t)k * N + n] = s;
 }
 
 // ---- in-place layout P1 (after a pull-push step): g_{k,j}(x) lives at (x + c_j, slot opp(j)), or at (x, slot j) when
@@ -1513,10 +1718,10 @@ moments_p1_kernel(const real *__restrict__ g, size_t pstride, double *__restrict
   const size_t n = ((size_t)z * ny + y) * nx + x;
   const real *gk = g + (size_t)k * Q * pstride;
   const bool npx = bc0 != BC_PERIODIC, npy = D > 1 && bc2 != BC_PERIODIC, npz = D > 2 && bc4 != BC_PERIODIC;
-  real s = real(0);
+  double s = 0.0;
 #pragma unroll
-  for (int j = 0; j < Q; j++) s += p1_fetch<L, real>(gk, pstride, j, x, y, z, nx, ny, nz, npx, npy, npz);
-  out[(size_t)k * N + n] = (double)s;
+  for (int j = 0; j < Q; j++) s += (double)p1_fetch<L, real>(gk, pstride, j, x, y, z, nx, ny, nz, npx, npy, npz);
+  out[(size_t)k * N + n] = s;
 }
 
 template <int LAT, typename real>

@@ -55,8 +55,11 @@ template <int LAT, int SCHEME, typename real> struct Ops {
   // its SM anyway (K = 17 rows) loses nothing.  Measured on B200: fp64 NC = 2 lifts config 5 from 0.955
   // to 0.975 of the copy bandwidth, D2Q5 0.76 -> 0.98; fp32 NC = 4 on D3Q19 / D2Q9 does not pay (scalar x-shifted loads).
   static constexpr int NCMAX = sizeof(real) == 8 ? 2 : (Q <= 7 ? 4 : 2);
+#ifndef LBMHD_MULTI_REGS_EXTRA32
+#define LBMHD_MULTI_REGS_EXTRA32 0      // measurement knob: more registers for the fp32 multi-cell kernels (fewer blocks per SM)
+#endif
   static constexpr int regs_need_multi(int nc) {
-    const int pops = nc * Q * (int)sizeof(real) / 4;
+    const int pops = nc * Q * (int)sizeof(real) / 4 + (sizeof(real) == 4 ? LBMHD_MULTI_REGS_EXTRA32 : 0);
     return (pops + (pops > 64 ? 52 : 36) + 7) / 8 * 8;        // D3Q19 fp64 x 2 cells: 76 + 52 = 128 (measured: no spills at 128, slower at 96)
   }
   static constexpr int pick_nc() {
@@ -72,18 +75,31 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     const long long blocks = (long long)((h->p.nx + 32 * NC - 1) / (32 * NC) + 1) * h->p.ny * h->p.nz;
     return h->multi_force || blocks >= 16LL * h->num_sms * MINB_M;
   }
+  // Rows made of whole multi-cell tiles, the end tiles holding the face cells (step_kernel_multi<.., EDGE = true>), whenever nx is
+  // a multiple of the tile width: measured faster in 20 of 22 cases (fp32 on config 5 in place 0.785 -> 0.877,
+  // D3Q7 fp32 0.63 -> 0.75; the one loss: RESIST on config 4 in place 0.944 -> 0.920).  LBMHD_EDGE_MULTI=0 turns it off.
+  static constexpr bool EDGE_COMPILED = NC > 1;
+  static constexpr bool EDGE_DEFAULT = true;
+  template <bool EDGE> static cudaError_t launch_multi_t(lbmhd_t *h, const StepArgs<real> &a, int lo, int hi) {
+    constexpr int W = 32 * NC;
+    const int xbase = EDGE ? 0 : 32;
+    const int nm = EDGE ? h->p.nx / W : (h->p.nx >= 64 + W ? (h->p.nx - 64) / W : 0);      // multi-cell tiles at x0 = xbase + W j
+    const int ntail = EDGE ? 0 : (h->p.nx - (32 + W * nm) + 31) / 32;                       // 32-cell tiles after them (>= 0)
+    const dim3 g = grid_planes(h, EDGE ? nm : nm + 1 + (ntail > 0 ? ntail : 0), lo, hi), b(32, K);
+    const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
+    if (!inplace) step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_AB, EDGE><<<g, b, 0, h->stream>>>(a, nm, xbase);
+    else if (h->parity == 0) step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_PP, EDGE><<<g, b, 0, h->stream>>>(a, nm, xbase);
+    else step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_LOC, EDGE><<<g, b, 0, h->stream>>>(a, nm, xbase);
+    h->launches += 1;
+    return cudaGetLastError();
+  }
   static cudaError_t launch_step_multi(lbmhd_t *h, const StepArgs<real> &a, int lo, int hi) {
     if constexpr (NC > 1) {
-      constexpr int W = 32 * NC;
-      const int nm = h->p.nx >= 64 + W ? (h->p.nx - 64) / W : 0;      // multi-cell tiles at x0 = 32 + W j, all interior in x
-      const int ntail = (h->p.nx - (32 + W * nm) + 31) / 32;           // 32-cell tiles after them (>= 0)
-      const dim3 g = grid_planes(h, nm + 1 + (ntail > 0 ? ntail : 0), lo, hi), b(32, K);
-      const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
-      if (!inplace) step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_AB><<<g, b, 0, h->stream>>>(a, nm);
-      else if (h->parity == 0) step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_PP><<<g, b, 0, h->stream>>>(a, nm);
-      else step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_LOC><<<g, b, 0, h->stream>>>(a, nm);
-      h->launches += 1;
-      return cudaGetLastError();
+      if constexpr (EDGE_COMPILED) {
+        const bool want = h->edge_multi < 0 ? EDGE_DEFAULT : h->edge_multi != 0;
+        if (want && h->p.nx % (32 * NC) == 0 && h->p.nx >= 2 * 32 * NC) return launch_multi_t<true>(h, a, lo, hi);
+      }
+      return launch_multi_t<false>(h, a, lo, hi);
     } else {
       return cudaErrorInvalidValue;
     }
@@ -157,7 +173,7 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     a.pstride = h->L.pstride;
     a.nx = h->p.nx; a.ny = h->p.ny; a.nz = h->p.nz;
     for (int j = 0; j < 6; j++) a.bc[j] = h->p.bc[j];
-    for (int k = 0; k < K; k++) a.omega[k] = (real)(1.0 / h->tau[k]);
+    for (int k = 0; k < K; k++) { a.omega[k] = (real)(1.0 / h->tau[k]); a.tau[k] = (real)h->tau[k]; }
     a.inv_tauB_cs2 = (real)(1.0 / (h->tau[h->g.iB] * h->g.cs2));
     a.kappa = (real)h->p.powell; a.gamma = (real)h->p.gamma; a.c0sq = (real)h->p.c0sq;
     a.inv_tau_relax = h->p.tau_relax > 0.0 ? (real)(1.0 / h->p.tau_relax) : real(0);

@@ -46,9 +46,10 @@ def load_library():
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(_build.SO):
-        raise ImportError("CUDA extension %s is missing; run __graft_entry__.build() (nvcc, sm_100a)" % _build.SO)
-    lib = C.CDLL(_build.SO)
+    so = os.environ.get("LBMHD_LIBRARY", _build.SO)      # another build of this library (same ABI), e.g. with other compile flags
+    if not os.path.exists(so):
+        raise ImportError("CUDA extension %s is missing; run __graft_entry__.build() (nvcc, sm_100a)" % so)
+    lib = C.CDLL(so)
     dp, up, pp = C.c_void_p, C.c_void_p, C.POINTER(LbmhdParams)
     lib.lbmhd_num_vars.argtypes = [pp]
     lib.lbmhd_num_dirs.argtypes = [pp]
@@ -161,9 +162,16 @@ class Lbmhd:
         if nbytes == 0:
             raise LbmhdError(EINVAL, "bad dims or precision")
         dev = torch.device("cuda", params.device)
-        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev)
+        # LBMHD_GUARD_BYTES=n (debugging aid, tests/test_guard_gpu.py): n bytes of 0xA5 before and after the workspace, checked by
+        # close(): a kernel that writes outside the memory it was given trips it (compute-sanitizer is not available everywhere)
+        guard = int(os.environ.get("LBMHD_GUARD_BYTES", "0"))
+        if guard:
+            self.workspace = torch.full((nbytes + 256 + 2 * guard,), 0xA5, dtype=torch.uint8, device=dev)
+        else:
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev)
         base = self.workspace.data_ptr()
-        aligned = (base + 255) // 256 * 256
+        aligned = (base + guard + 255) // 256 * 256
+        self._guard = (aligned - base, nbytes) if guard else None
         params.workspace = aligned
         params.workspace_bytes = nbytes
         self.stream = stream if stream is not None else torch.cuda.current_stream(dev)
@@ -177,11 +185,22 @@ class Lbmhd:
         _check(self.lib.lbmhd_create(C.byref(params), m, C.byref(h)))
         self.h = h
 
+    def guards_intact(self):
+        """True if the guard bands around the workspace (LBMHD_GUARD_BYTES) still hold their pattern"""
+        if self._guard is None or self.workspace is None:
+            return True
+        lo, n = self._guard
+        self.torch.cuda.synchronize(self.workspace.device)
+        return bool((self.workspace[:lo] == 0xA5).all().item()) and bool((self.workspace[lo + n:] == 0xA5).all().item())
+
     def close(self):
         if getattr(self, "h", None):
+            ok = self.guards_intact() if getattr(self, "_guard", None) else True
             self.lib.lbmhd_destroy(self.h)
             self.h = None
             self.workspace = None
+            if not ok:
+                raise LbmhdError(ECUDA, "a kernel wrote outside the workspace (guard band damaged)")
 
     def __del__(self):
         try:

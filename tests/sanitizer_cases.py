@@ -7,8 +7,9 @@ The places where a mis-indexed slot would be a silent race or an out-of-bounds a
 step types with x-edge, general and sphere tiles; the 2-CTA cluster exchange through distributed shared memory
 (step_kernel_cl); the multi-cell and cell-per-thread kernels with their vector accesses and shuffled stores; the cooperative
 many-step launch; the slab halo pack / unpack with the in-place return exchange.  Each case is also compared with the
-oracle, so a run that passes the tool but computes garbage still fails.  Summaries of the two runs are kept under
-profiles/ (r2_sanitizer.md).  Not collected by pytest (no test_ prefix)."""
+oracle, so a run that passes the tool but computes garbage still fails.  On this project's GPU pool compute-sanitizer is
+closed (profiles/r2_sanitizer.md records the refusal); there tests/test_guard_gpu.py runs these same cases with guard bands
+around every workspace instead.  Not collected by pytest (no test_ prefix)."""
 import os
 import sys
 
