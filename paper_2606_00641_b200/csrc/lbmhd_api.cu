@@ -207,8 +207,8 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     h->num_sms = sms;
     h->pair = p->eta_jc == 0.0;      // several cells per thread where the lattice has a multi-cell kernel; eta(j): one-cell kernels
     if (const char *e3 = getenv("LBMHD_PAIR")) h->pair = h->pair && atoi(e3) != 0;
-    h->cluster = p->scheme == LBMHD_RESIST && g.Q > 9 && p->precision == 64;      // measured: pays there only
-    if (const char *e4 = getenv("LBMHD_CLUSTER")) h->cluster = h->cluster && atoi(e4) != 0;
+    h->cluster = -1;
+    if (const char *e4 = getenv("LBMHD_CLUSTER")) h->cluster = atoi(e4) != 0 ? 1 : 0;
     h->last_path = -1;
     h->edge_multi = -1;
     if (const char *e10 = getenv("LBMHD_EDGE_MULTI")) h->edge_multi = atoi(e10) != 0 ? 1 : 0;

@@ -62,7 +62,7 @@ struct lbmhd {
   double obs_om[3], obs_c[3];   // rigid rotation of masked bodies
   long long sph_t0;
   bool multi_force;      // LBMHD_MULTI=1: take the multi-cell kernel on small grids too (tests)
-  bool cluster;          // RESIST on D3Q19, fp64: variable rows of a tile split over a 2-CTA cluster; LBMHD_CLUSTER=0 turns it off
+  int cluster;           // variable rows of a tile split over a 2-CTA cluster: -1 = where measured to pay, 0 / 1 = LBMHD_CLUSTER
   bool pair;             // several cells per thread on interior tiles (fp32; fp64 on the short lattices); LBMHD_PAIR=0 turns it off
   int edge_multi;        // rows of whole multi-cell tiles with the face cells inside the end tiles: -1 = where measured to pay, 0 / 1 = LBMHD_EDGE_MULTI
   bool cell;             // one thread per cell on the short lattices (off by default; LBMHD_CELL=1 turns it on)

@@ -624,6 +624,52 @@ __device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier
 __device__ __forceinline__ void cluster_arrive_release() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait_acquire() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
+// The exchange of the lean tiles of the 2-CTA cluster kernel WITHOUT a fence: on sm_100a the release half of a
+// cluster barrier is a GPU-scope MEMBAR (ncu: 5.0 of 24 stall cycles per issued instruction in step_kernel_cl).  Here every
+// row-thread delivers its moment into the partner CTA's copy with st.async, which signals the partner's mbarrier by byte
+// count (complete_tx): the partner waits for exactly the bytes its partner's rows deliver, and the data is visible to it when
+// the wait returns.  One phase per kernel (a cluster owns one tile), so the parity is always 0.
+__device__ __forceinline__ uint32_t cl_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t cl_mapa(uint32_t local_addr, uint32_t peer) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(peer));
+  return r;
+}
+__device__ __forceinline__ void cl_st_async(uint32_t remote_addr, double v, uint32_t remote_bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];" ::"r"(remote_addr),
+               "l"(__double_as_longlong(v)), "r"(remote_bar)
+               : "memory");
+}
+__device__ __forceinline__ void cl_st_async(uint32_t remote_addr, float v, uint32_t remote_bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(remote_addr),
+               "r"(__float_as_uint(v)), "r"(remote_bar)
+               : "memory");
+}
+template <typename real, int W> struct ShareAsync {
+  real (*sQ)[W];
+  real (*sTr)[W];
+  real *sNb;
+  uint32_t rQ, rbar;       // shared::cluster addresses of the partner's sQ[0][0] and of its mbarrier
+  unsigned long long *bar; // this CTA's mbarrier
+  uint32_t expect;         // bytes the partner's rows deliver
+  __device__ __forceinline__ void begin() const { cluster_wait_acquire(); }      // start barrier: the partner is resident, its mbarrier initialised
+  __device__ __forceinline__ void putQ(int l, int tx, real v) const {
+    sQ[l][tx] = v;
+    cl_st_async(rQ + (uint32_t)((l * W + tx) * (int)sizeof(real)), v, rbar);
+  }
+  __device__ __forceinline__ void putTr(int, int, real) const {}      // the schemes this kernel serves take div B from G
+  __device__ __forceinline__ void putNb(int, real) const {}
+  __device__ __forceinline__ void sync() const {
+    const uint32_t b = cl_smem_u32(bar);
+    if (threadIdx.x == 0 && threadIdx.y == 0) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(b), "r"(expect) : "memory");
+    __syncthreads();      // this CTA's own rows
+    uint32_t ok;
+    do {
+      asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }" : "=r"(ok) : "r"(b) : "memory");
+    } while (!ok);
+  }
+};
+
 template <typename real, int W, bool CL, class Sync = SyncBlock> struct Share {
   real (*sQ)[W];
   real (*sTr)[W];
@@ -632,6 +678,13 @@ template <typename real, int W, bool CL, class Sync = SyncBlock> struct Share {
   real (*rTr)[W];
   real *rNb;
   Sync sync_;
+  uint32_t rQa = 0, rbar = 0, expect = 0;      // CL with the fence-free exchange (ShareAsync): see lean()
+  unsigned long long *bar = nullptr;
+  // the policy of the lean tiles (interior, fluid): the fence-free exchange where the kernel set it up, else this one
+  __device__ __forceinline__ auto lean() const {
+    if constexpr (CL) return ShareAsync<real, W>{sQ, sTr, sNb, rQa, rbar, bar, expect};
+    else return *this;
+  }
   __device__ __forceinline__ void begin() const {
     if (CL) cluster_wait_acquire();
   }
@@ -722,7 +775,7 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
   real Qlo;
   const real Qk = moment_sum<L, real>(f, Qlo);
   sh.putQ(k, tx, Qk);
-  if (k >= iB && k < iB + D) {
+  if (!has_relax(SCHEME) && k >= iB && k < iB + D) {      // A6 (the schemes with gradient sets take div B from them)
     const int b = k - iB;   // warp-uniform
     // first moment of this B set, Pi_{a,b} = sum_i c_ia f_i: the diagonal entry is its share of tr Pi_B (A6); the
     // resistive scheme keeps all D entries, their antisymmetric part gives the current (A20)
@@ -759,8 +812,10 @@ __device__ __forceinline__ void finish_cell(const StepArgs<real> &a, const CellC
     for (int l = 0; l < K; l++) Qv[l] = sh.sQ[l][tx];
   }
   real tr = real(0);
+  if constexpr (!has_relax(SCHEME)) {
 #pragma unroll
-  for (int b = 0; b < D; b++) tr += sh.sTr[b * D + b][tx];
+    for (int b = 0; b < D; b++) tr += sh.sTr[b * D + b][tx];
+  }
   // A20: current-dependent resistivity -> cell-local tau_B (6 Newton steps on tau^3 - tau0 tau^2 - c = 0 from tau0 + cbrt(c))
   real inv_tauB_cs2 = a.inv_tauB_cs2;
   real omB = real(0);
@@ -956,16 +1011,17 @@ __device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, 
     for (int i = 0; i < Q; i++) f[i] = *reinterpret_cast<const real *>(pb + (STREAM == ST_LOC ? a.st_off[opp(i)] : a.ld_off[i]));
     const bool writeM = STREAM != ST_AB && (rowM || (npx && (x == 1 || x == nx - 2)));
     CellCtx c{tx, k, x, y, z, n, true, false, false, false, false, false, false, writeM};
-    sh.begin();
+    const auto shl = sh.lean();      // cluster kernel: the fence-free exchange (ShareAsync); every other kernel: sh itself
+    shl.begin();
     if (STREAM == ST_AB) {
       const StoreOwn<real> st{reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + n)), a.st_off};
-      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sh);
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, shl);
     } else if (STREAM == ST_PP) {
       const StorePPInterior<real> st{pb, a.ld_off};
-      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sh);
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, shl);
     } else {
       const StoreOwn<real> st{pb, a.st_off};
-      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, sh);
+      finish_cell<LAT, SCHEME, real, TX, false, false, STREAM>(a, c, f, st, shl);
     }
     return;
   }
@@ -1078,14 +1134,24 @@ step_kernel_cl(const __grid_constant__ StepArgs<real> a) {
   __shared__ real sQ[K][32];
   __shared__ real sTr[D * D][32];
   __shared__ real sNb[K];
+  __shared__ __align__(8) unsigned long long mbar;      // arrival of the partner's moments on the lean tiles (ShareAsync)
+  static_assert(has_relax(SCHEME), "the fence-free exchange carries the zeroth moments only");
   const unsigned rank = blockIdx.x & 1u;
   const int k = (int)rank * KH + (int)threadIdx.y;
   if (k >= K) return;
-  cluster_arrive_relaxed();      // start barrier; Share::begin() waits for it
+  if (threadIdx.x == 0 && threadIdx.y == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(cl_smem_u32(&mbar)) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  cluster_arrive_relaxed();      // start barrier; begin() waits for it: the partner is resident and its mbarrier initialised
   namespace cg = cooperative_groups;
   cg::cluster_group cl = cg::this_cluster();
-  const Share<real, 32, true> sh{sQ, sTr, sNb, cl.map_shared_rank(sQ, rank ^ 1u), cl.map_shared_rank(sTr, rank ^ 1u),
-                                 cl.map_shared_rank(sNb, rank ^ 1u), SyncBlock{}};
+  Share<real, 32, true> sh{sQ, sTr, sNb, cl.map_shared_rank(sQ, rank ^ 1u), cl.map_shared_rank(sTr, rank ^ 1u),
+                           cl.map_shared_rank(sNb, rank ^ 1u), SyncBlock{}};
+  sh.rQa = cl_mapa(cl_smem_u32(&sQ[0][0]), rank ^ 1u);
+  sh.rbar = cl_mapa(cl_smem_u32(&mbar), rank ^ 1u);
+  sh.bar = &mbar;
+  sh.expect = (uint32_t)((rank == 0 ? K - KH : KH) * 32 * (int)sizeof(real));      // the partner's rows, 32 cells each
   run_tile<LAT, SCHEME, real, 32, 0, STREAM>(a, threadIdx.x, k, (int)(blockIdx.x >> 1) * 32, (int)blockIdx.y + (D == 2 ? a.row0 : 0),
                                              (int)blockIdx.z + (D == 3 ? a.row0 : 0), 0, sh);
 }

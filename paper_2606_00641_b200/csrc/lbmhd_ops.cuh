@@ -139,7 +139,10 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     }
   }
 
-  // RESIST: the K = 11 / 14 / 17 rows of a tile split over a 2-CTA cluster (lbmhd_kernels.cuh, Share)
+  // The rows of a tile split over a 2-CTA cluster (lbmhd_kernels.cuh, Share / ShareAsync): compiled for the schemes with gradient
+  // sets on D3Q19 in fp64 (measured slower on D3Q7 and in fp32); the default is where it was measured to pay, LBMHD_CLUSTER=0 / 1 overrides.
+  static constexpr bool CLUSTER_COMPILED = has_G(SCHEME) && Q > 9 && sizeof(real) == 8;
+  static constexpr bool CLUSTER_DEFAULT = SCHEME == kResist && Q > 9 && sizeof(real) == 8;
   static constexpr int KH = (K + 1) / 2;
   static constexpr int MINB_CL = minb_for(32 * KH, REGS_NEED);
   static cudaError_t launch_step_cluster(lbmhd_t *h, const StepArgs<real> &a, int lo, int hi) {
@@ -250,8 +253,9 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     a.row1 = hi;
     cudaError_t e;
     bool launched = false;
-    if constexpr (SCHEME == kResist && Q > 9 && sizeof(real) == 8) {
-      if (h->cluster) { e = launch_step_cluster(h, a, lo, hi); launched = true; h->last_path = LBMHD_PATH_CLUSTER; }
+    if constexpr (CLUSTER_COMPILED) {
+      const bool want = h->cluster < 0 ? CLUSTER_DEFAULT : h->cluster != 0;
+      if (want && h->p.eta_jc == 0.0) { e = launch_step_cluster(h, a, lo, hi); launched = true; h->last_path = LBMHD_PATH_CLUSTER; }
     }
     if (launched) {}
     else if (h->use_tma) { e = launch_step_tma(h, a); h->last_path = LBMHD_PATH_TMA; }
