@@ -6,12 +6,15 @@ the kernel bench.py times for that config (`step_path` asserted), A/B and in pla
   C2  512 x 512      100 steps        scheme FULL (20 sets) as BASELINE states the case; C2i: the INCRES reading at rms 0.02
   C3  1024 x 1024    100 steps        step_kernel_multi
   C4  2048 x 2048    100 steps        step_kernel_multi
-  C5  192 x 128 x 128, R = 12, 100 steps: HALF SCALE (SURVEY.md:516-518 names this fallback: the oracle needs ~60 GB
+  C5  192 x 128 x 128, R = 12, 100 steps: HALF SCALE by default; the FULL 384 x 256 x 256 with LBMHD_GRADED_FULL_C5=1
+      (last run: fp64 7.0e-15, fp32 2.9e-6, profiles/r2_graded_c5_full.md) (SURVEY.md:516-518 names this fallback: the oracle needs ~60 GB
       and ~40 min for the full 384 x 256 x 256); step_kernel_multi with nm = 2 multi-cell tiles per row.  The full-size
       C5 is covered by sampled cells in tests/test_parity_fullsize_gpu.py.
 
 The oracle (plain per-cell C, ~10 MLUPS on the box) runs each config once; the result is shared by the A/B, in-place and
 fp32 comparisons.  Eq.2 PAPER.md:78 iterated; reading A15 for the norm."""
+import os
+
 import numpy as np
 import pytest
 
@@ -26,6 +29,8 @@ _CACHE = {}
 def graded_workload(name):
     if name == "C5":
         return W.config5(shape=(192, 128, 128))
+    if name == "C5full":
+        return W.get("C5")
     return W.get(name)
 
 
@@ -118,3 +123,11 @@ def test_graded_c5_multi_tiles_exist():
     w = graded_workload("C5")
     nx = w["shape"][0]
     assert (nx - 64) // 64 >= 2
+
+
+@pytest.mark.skipif(os.environ.get("LBMHD_GRADED_FULL_C5") != "1",
+                    reason="config 5 at its FULL size (384x256x256), all cells, 100 steps: the oracle needs ~100 GB of host memory and "
+                           "~6 min on 16 cores; opt in with LBMHD_GRADED_FULL_C5=1 (last run recorded in DESIGN.md §4)")
+def test_graded_c5_full_size_all_cells():
+    """the same protocol on the full config 5, through the kernel and launch configuration bench.py times"""
+    test_graded_100_steps_all_cells("C5full", "PATH_MULTI")
