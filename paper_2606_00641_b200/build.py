@@ -1,6 +1,6 @@
 """Builds the C-ABI CUDA library in-tree for sm_100a with nvcc (no torch in the build).
 
-The kernel templates are instantiated once per (lattice, precision) in csrc/lbmhd_inst.cu; those ten translation units and
+The kernel templates are instantiated once per (lattice, precision, scheme group) in csrc/lbmhd_inst.cu; those twenty translation units and
 csrc/lbmhd_api.cu and csrc/lbmhd_noalloc.cu compile in parallel into build/*.o and link into liblbmhd.so."""
 import os
 import shutil
@@ -27,8 +27,9 @@ def _units():
     units = [("api", os.path.join(_CSRC, "lbmhd_api.cu"), []), ("noalloc", os.path.join(_CSRC, "lbmhd_noalloc.cu"), [])]
     for lat in LATTICES:
         for bits in PRECISIONS:
-            units.append(("inst_%d_%d" % (lat, bits), os.path.join(_CSRC, "lbmhd_inst.cu"),
-                          ["-DLBMHD_INST_LAT=%d" % lat, "-DLBMHD_INST_BITS=%d" % bits]))
+            for grp in (1, 0):      # RESIST / FULL first: the heavier half
+                units.append(("inst_%d_%d_g%d" % (lat, bits, grp), os.path.join(_CSRC, "lbmhd_inst.cu"),
+                              ["-DLBMHD_INST_LAT=%d" % lat, "-DLBMHD_INST_BITS=%d" % bits, "-DLBMHD_INST_GROUP=%d" % grp]))
     return units
 
 
@@ -40,7 +41,7 @@ def build(force=False, verbose=False, jobs=None, extra_flags=(), out=None):
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     obj_dir = OBJ_DIR if out == SO else out + ".build"
     os.makedirs(obj_dir, exist_ok=True)
-    jobs = jobs or int(os.environ.get("LBMHD_BUILD_JOBS", "0")) or min(os.cpu_count() or 1, 11)
+    jobs = jobs or int(os.environ.get("LBMHD_BUILD_JOBS", "0")) or min(os.cpu_count() or 1, 22)
     extra = ["-Xptxas", "-v"] if verbose else []
 
     def compile_one(unit):

@@ -248,12 +248,16 @@ namespace {
 
 OpTable pick(const lbmhd_t *h) {
   const bool f64 = h->p.precision == 64;
+  const int sc = h->p.scheme;
+  const bool grp = sc == LBMHD_RESIST || sc == LBMHD_FULL;      // scheme group of the translation units (lbmhd_inst.cu)
   switch (h->p.lattice) {
-    case LBMHD_D1Q3: return f64 ? ops_table_1_64(h->p.scheme) : ops_table_1_32(h->p.scheme);
-    case LBMHD_D2Q9: return f64 ? ops_table_2_64(h->p.scheme) : ops_table_2_32(h->p.scheme);
-    case LBMHD_D2Q5: return f64 ? ops_table_4_64(h->p.scheme) : ops_table_4_32(h->p.scheme);
-    case LBMHD_D3Q7: return f64 ? ops_table_5_64(h->p.scheme) : ops_table_5_32(h->p.scheme);
-    default: return f64 ? ops_table_3_64(h->p.scheme) : ops_table_3_32(h->p.scheme);
+#define LBH_PICK(LATID) (grp ? (f64 ? ops_table_##LATID##_64_g1(sc) : ops_table_##LATID##_32_g1(sc)) : (f64 ? ops_table_##LATID##_64_g0(sc) : ops_table_##LATID##_32_g0(sc)))
+    case LBMHD_D1Q3: return LBH_PICK(1);
+    case LBMHD_D2Q9: return LBH_PICK(2);
+    case LBMHD_D2Q5: return LBH_PICK(4);
+    case LBMHD_D3Q7: return LBH_PICK(5);
+    default: return LBH_PICK(3);
+#undef LBH_PICK
   }
 }
 

@@ -90,12 +90,14 @@ struct OpTable {
   int (*halo_dirs)(int, int *);
 };
 
-// defined by lbmhd_inst.cu, one translation unit per (lattice, precision)
-#define LBH_DECLARE_TABLES(P) \
-  OpTable ops_table_1_##P(int scheme); OpTable ops_table_2_##P(int scheme); OpTable ops_table_3_##P(int scheme); \
-  OpTable ops_table_4_##P(int scheme); OpTable ops_table_5_##P(int scheme);
-LBH_DECLARE_TABLES(64)
-LBH_DECLARE_TABLES(32)
+// defined by lbmhd_inst.cu, one translation unit per (lattice, precision, scheme group: 0 = IDEAL / INCRES / IDEAL_DIVB, 1 = RESIST / FULL)
+#define LBH_DECLARE_TABLES(P, G) \
+  OpTable ops_table_1_##P##_g##G(int scheme); OpTable ops_table_2_##P##_g##G(int scheme); OpTable ops_table_3_##P##_g##G(int scheme); \
+  OpTable ops_table_4_##P##_g##G(int scheme); OpTable ops_table_5_##P##_g##G(int scheme);
+LBH_DECLARE_TABLES(64, 0)
+LBH_DECLARE_TABLES(64, 1)
+LBH_DECLARE_TABLES(32, 0)
+LBH_DECLARE_TABLES(32, 1)
 #undef LBH_DECLARE_TABLES
 
 inline int use_device(const lbmhd_t *h) {

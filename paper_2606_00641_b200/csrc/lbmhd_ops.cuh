@@ -1,5 +1,5 @@
 // lbmhd_ops.cuh — kernel dispatch: Ops<LAT, SCHEME, real> launches the kernels of lbmhd_kernels.cuh / lbmhd_tma.cuh for one
-// (lattice, scheme, precision); table_for collects its entry points.  Included by lbmhd_inst.cu only.
+// (lattice, scheme, precision); table_for collects the entry points of a scheme group.  Included by lbmhd_inst.cu only.
 #pragma once
 #include <math.h>
 #include <string.h>
@@ -434,12 +434,17 @@ template <int LAT, int SCHEME, typename real> OpTable make_table() {
   return OpTable{O::step, O::step_part, O::init, O::moments, O::diag, O::pops_export, O::pops_import, O::refresh_published, O::halo_dirs};
 }
 
-template <int LAT, typename real> OpTable table_for(int scheme) {
-  if (scheme == LBMHD_IDEAL) return make_table<LAT, kIdeal, real>();
-  if (scheme == LBMHD_IDEAL_DIVB) return make_table<LAT, kIdealD, real>();
-  if (scheme == LBMHD_RESIST) return make_table<LAT, kResist, real>();
-  if (scheme == LBMHD_FULL) return make_table<LAT, kFull, real>();
-  return make_table<LAT, kIncres, real>();
+// GROUP 0: the schemes without gradient tensors (IDEAL, INCRES, IDEAL_DIVB); GROUP 1: RESIST, FULL.  One translation unit per
+// (lattice, precision, group): 20 units of similar weight compile in parallel (build.py).
+template <int LAT, typename real, int GROUP> OpTable table_for(int scheme) {
+  if constexpr (GROUP == 0) {
+    if (scheme == LBMHD_IDEAL) return make_table<LAT, kIdeal, real>();
+    if (scheme == LBMHD_IDEAL_DIVB) return make_table<LAT, kIdealD, real>();
+    return make_table<LAT, kIncres, real>();
+  } else {
+    if (scheme == LBMHD_RESIST) return make_table<LAT, kResist, real>();
+    return make_table<LAT, kFull, real>();
+  }
 }
 
 }  // namespace lbh
