@@ -1109,11 +1109,22 @@ __device__ __forceinline__ void run_tile(const StepArgs<real> &a, const int tx, 
   general_tile<LAT, SCHEME, real, TX, STREAM>(a, tx, k, x, y, z, sh);
 }
 
+// Programmatic dependent launch (lbmhd_ops.cuh, launch_pdl): a step kernel launched with the stream-serialisation attribute may
+// be scheduled while the previous step's last blocks are still running.  Every block first lets ITS dependent grid go
+// (`launch_dependents`: the next step is released once all blocks of this one have started, so its blocks take the slots
+// this step's blocks free), then waits until the grid it depends on has completed and its stores are visible (`wait`), before
+// its first global access.  Launched without the attribute both instructions do nothing.
+__device__ __forceinline__ void pdl_enter() {
+  asm volatile("griddepcontrol.launch_dependents;");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 template <int LAT, int SCHEME, typename real, int TX, int MINB, int MODE, int STREAM>
 __global__ void __launch_bounds__(TX * Vars<SCHEME, Lattice<LAT>::D>::K, MINB)
 step_kernel(const __grid_constant__ StepArgs<real> a, const Region r, const int sphere_only) {
   using L = Lattice<LAT>;
   constexpr int D = L::D, K = Vars<SCHEME, D>::K;
+  pdl_enter();
   __shared__ real sQ[K][TX];
   __shared__ real sTr[D * D][TX];
   __shared__ real sNb[K];
@@ -1481,6 +1492,7 @@ step_kernel_multi(const __grid_constant__ StepArgs<real> a, const int nmulti, co
   const int tx = threadIdx.x, k = threadIdx.y;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
   const int y = (int)blockIdx.y + (D == 2 ? a.row0 : 0), z = (int)blockIdx.z + (D == 3 ? a.row0 : 0);
+  pdl_enter();
   if (ghost_row<real, D>(a, y, z)) return;
   const Share<real, 32, false> sh32{reinterpret_cast<real(*)[32]>(&sQ[0][0]), reinterpret_cast<real(*)[32]>(&sTr[0][0]), sNb,
                                     nullptr, nullptr, nullptr, SyncBlock{}};

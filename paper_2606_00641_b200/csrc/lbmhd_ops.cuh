@@ -38,15 +38,36 @@ template <int LAT, int SCHEME, typename real> struct Ops {
   static dim3 grid_planes(const lbmhd_t *h, int gx, int lo, int hi) {
     return L::D == 3 ? dim3(gx, h->p.ny, hi - lo) : (L::D == 2 ? dim3(gx, hi - lo, 1) : dim3(gx, 1, 1));
   }
+  // A step kernel launched so that it may be scheduled while the previous kernel of the stream drains (programmatic dependent
+  // launch; the kernel's pdl_enter() is the matching wait).  What precedes it in the stream need not be a step kernel: a
+  // predecessor that never releases its dependents does so when it ends, which is the plain stream order.
+  template <typename... P, typename... A> static cudaError_t launch_pdl(lbmhd_t *h, void (*kern)(P...), dim3 g, dim3 b, A... args) {
+    if (!h->pdl) {
+      kern<<<g, b, 0, h->stream>>>(args...);
+      return cudaGetLastError();
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = g;
+    cfg.blockDim = b;
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = h->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, args...);
+  }
   static cudaError_t launch_step_one(lbmhd_t *h, const StepArgs<real> &a, int lo, int hi) {
     constexpr int TX = 32;
     const dim3 g = grid_planes(h, (h->p.nx + TX - 1) / TX, lo, hi), b(TX, K);
     const Region all{0, 1, 0, 1, 0, 1};
-    if (h->p.streaming != LBMHD_STREAM_INPLACE) step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_AB><<<g, b, 0, h->stream>>>(a, all, 0);
-    else if (h->parity == 0) step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_PP><<<g, b, 0, h->stream>>>(a, all, 0);
-    else step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_LOC><<<g, b, 0, h->stream>>>(a, all, 0);
+    cudaError_t e;
+    if (h->p.streaming != LBMHD_STREAM_INPLACE) e = launch_pdl(h, step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_AB>, g, b, a, all, 0);
+    else if (h->parity == 0) e = launch_pdl(h, step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_PP>, g, b, a, all, 0);
+    else e = launch_pdl(h, step_kernel<LAT, SCHEME, real, TX, MINB, 0, ST_LOC>, g, b, a, all, 0);
     h->launches += 1;
-    return cudaGetLastError();
+    return e;
   }
 
   // several cells per thread on interior tiles (lbmhd_kernels.cuh, step_kernel_multi): NC-wide vector accesses need nx % NC == 0
@@ -87,11 +108,12 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     const int ntail = EDGE ? 0 : (h->p.nx - (32 + W * nm) + 31) / 32;                       // 32-cell tiles after them (>= 0)
     const dim3 g = grid_planes(h, EDGE ? nm : nm + 1 + (ntail > 0 ? ntail : 0), lo, hi), b(32, K);
     const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
-    if (!inplace) step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_AB, EDGE><<<g, b, 0, h->stream>>>(a, nm, xbase);
-    else if (h->parity == 0) step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_PP, EDGE><<<g, b, 0, h->stream>>>(a, nm, xbase);
-    else step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_LOC, EDGE><<<g, b, 0, h->stream>>>(a, nm, xbase);
+    cudaError_t e;
+    if (!inplace) e = launch_pdl(h, step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_AB, EDGE>, g, b, a, nm, xbase);
+    else if (h->parity == 0) e = launch_pdl(h, step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_PP, EDGE>, g, b, a, nm, xbase);
+    else e = launch_pdl(h, step_kernel_multi<LAT, SCHEME, real, NC, MINB_M, ST_LOC, EDGE>, g, b, a, nm, xbase);
     h->launches += 1;
-    return cudaGetLastError();
+    return e;
   }
   static cudaError_t launch_step_multi(lbmhd_t *h, const StepArgs<real> &a, int lo, int hi) {
     if constexpr (NC > 1) {
