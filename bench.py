@@ -31,7 +31,8 @@ sys.path.insert(0, ROOT)
 METRIC = "MLUPS (fused VLBM MHD stream-collide step)"
 HALF_C5 = (192, 128, 128)      # the oracle's sample of config 5 (half-scale domain when the full one is too slow)
 REPEATS = 3
-KERNEL_NAMES = {0: "step_kernel", 1: "step_kernel_multi", 2: "step_kernel_cl", 3: "step_kernel_tma", 4: "step_kernel_persist", 5: "step_kernel_cell"}
+KERNEL_NAMES = {0: "step_kernel", 1: "step_kernel_multi", 2: "step_kernel_cl", 3: "step_kernel_tma", 4: "step_kernel_persist", 5: "step_kernel_cell",
+                6: "step_kernel_resident"}
 
 
 def load_peaks():

@@ -238,9 +238,11 @@ long long lbmhd_launch_count(const lbmhd_t *h);
  * n x co-resident blocks); LBMHD_EDGE_MULTI=0 / 1 the x-face cells outside / inside the multi-cell tiles
  * (where that kernel variant is compiled); LBMHD_CELL=1 the cell-per-thread kernel on the short lattices
  * (off by default: measured slower), =2 that kernel on small grids too; LBMHD_PDL=0 plain launches instead of
- * programmatic dependent launches of the one-cell and multi-cell step kernels. */
+ * programmatic dependent launches of the one-cell and multi-cell step kernels; LBMHD_RESIDENT=0 no
+ * register-resident many-step kernel on 1D lattices. */
 enum { LBMHD_PATH_ONE = 0, LBMHD_PATH_MULTI = 1, LBMHD_PATH_CLUSTER = 2, LBMHD_PATH_TMA = 3, LBMHD_PATH_PERSIST = 4,
-       LBMHD_PATH_CELL = 5 /* one thread per cell, all K sets in its registers: the short lattices D1Q3 / D2Q5 / D3Q7 */ };
+       LBMHD_PATH_CELL = 5 /* one thread per cell, all K sets in its registers: the short lattices D1Q3 / D2Q5 / D3Q7 */,
+       LBMHD_PATH_RESIDENT = 6 /* 1D lattices of <= 1024 cells, n >= 2 steps in one launch: populations resident in registers, one cluster */ };
 int lbmhd_step_path(const lbmhd_t *h);
 
 /* Measured-bandwidth probe (BabelStream-style copy b[i] = a[i] over n fp64 elements, the paper's roofline

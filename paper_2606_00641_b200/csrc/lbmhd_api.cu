@@ -212,6 +212,8 @@ int lbmhd_create(const lbmhd_params *p, const unsigned char *cell_mask, lbmhd_t 
     h->last_path = -1;
     h->edge_multi = -1;
     if (const char *e10 = getenv("LBMHD_EDGE_MULTI")) h->edge_multi = atoi(e10) != 0 ? 1 : 0;
+    h->resident = true;
+    if (const char *e12 = getenv("LBMHD_RESIDENT")) h->resident = atoi(e12) != 0;
     h->pdl = true;
     if (const char *e11 = getenv("LBMHD_PDL")) h->pdl = atoi(e11) != 0;
     h->cell = false;      // measured slower than the multi-cell kernel on B200 in all but one case: opt-in

@@ -65,6 +65,7 @@ struct lbmhd {
   int cluster;           // variable rows of a tile split over a 2-CTA cluster: -1 = where measured to pay, 0 / 1 = LBMHD_CLUSTER
   bool pair;             // several cells per thread on interior tiles (fp32; fp64 on the short lattices); LBMHD_PAIR=0 turns it off
   int edge_multi;        // rows of whole multi-cell tiles with the face cells inside the end tiles: -1 = where measured to pay, 0 / 1 = LBMHD_EDGE_MULTI
+  bool resident;         // 1D lattices: many steps with the populations resident in registers, one cluster (LBMHD_RESIDENT=0 turns it off)
   bool pdl;              // step kernels launched as programmatic dependents of the previous kernel in the stream (LBMHD_PDL=0 turns it off)
   bool cell;             // one thread per cell on the short lattices (off by default; LBMHD_CELL=1 turns it on)
   bool cell_force;       // LBMHD_CELL=2: on small grids too (tests)

@@ -7,6 +7,7 @@
 #include "lbmhd_host.h"
 #include "lbmhd_kernels.cuh"
 #include "lbmhd_tma.cuh"
+#include "lbmhd_resident.cuh"
 
 namespace lbh {
 
@@ -345,10 +346,98 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     for (int s = 0; s < n_steps; s++) advance(h);
     return LBMHD_OK;
   }
+  // ---- many steps of a 1D lattice with the populations resident in registers (lbmhd_resident.cuh) --------------
+  // One cluster of <= 16 CTAs of TXR cells (TXR = 32 or 64: nx <= 1024), fluid cells only, no body; in place from parity 0 for an
+  // even number of steps (the kernel reads and leaves layout P0).  A zero-gradient face and its inward neighbour share a CTA.
+  template <int TXR> static bool resident_fits(const lbmhd_t *h) {
+    const int nx = h->p.nx, ncta = (nx + TXR - 1) / TXR;
+    if (TXR * K > 1024 || ncta > 16) return false;
+    const bool periodic = h->p.bc[0] == LBMHD_BC_PERIODIC;
+    return periodic || (nx - 1) % TXR != 0;
+  }
+  static bool resident_allowed(const lbmhd_t *h) {
+    if constexpr (L::D != 1) return false;
+    if (!h->resident || h->use_tma) return false;
+    if (h->have_mask || h->have_dfield || h->body_on || h->has_sphere || h->p.nx < 3) return false;
+    if ((h->p.bc[0] == LBMHD_BC_PERIODIC) != (h->p.bc[1] == LBMHD_BC_PERIODIC)) return false;
+    if (h->p.bc[0] == LBMHD_BC_HALO || h->p.bc[1] == LBMHD_BC_HALO) return false;
+    return resident_fits<32>(h) || resident_fits<64>(h);
+  }
+  // returns LBMHD_OK and *done = true if the steps were run; *done = false (nothing launched) when no cluster of that size can be
+  // co-scheduled on this device
+  template <int TXR, bool INPLACE> static int launch_resident_t(lbmhd_t *h, StepArgs<real> &a, int n_steps, bool *done) {
+    *done = false;
+    if constexpr (L::D == 1) {
+      auto kern = step_kernel_resident<LAT, SCHEME, real, TXR, INPLACE>;
+      ResidentArgs<real> p;
+      memset(&p, 0, sizeof p);
+      p.n_steps = n_steps;
+      p.ncta = (h->p.nx + TXR - 1) / TXR;
+      p.pop_in = pops(h, h->cur);
+      p.pop_out = pops(h, INPLACE ? h->cur : (h->cur + n_steps) & 1);
+      if (INPLACE) {
+        p.M_in = (const double *)(h->ws + h->L.off_M[h->mcur]);
+        p.M_out[0] = (double *)(h->ws + h->L.off_M[0]);
+        p.M_out[1] = (double *)(h->ws + h->L.off_M[1]);
+      }
+      if (p.ncta > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) {
+        cudaGetLastError();
+        return LBMHD_OK;
+      }
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)p.ncta);
+      cfg.blockDim = dim3(TXR, K);
+      cfg.stream = h->stream;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = (unsigned)p.ncta;
+      at[0].val.clusterDim.y = 1;
+      at[0].val.clusterDim.z = 1;
+      cfg.attrs = at;
+      cfg.numAttrs = 1;
+      int nclusters = 0;
+      if (cudaOccupancyMaxActiveClusters(&nclusters, kern, &cfg) != cudaSuccess || nclusters < 1) {
+        cudaGetLastError();
+        return LBMHD_OK;
+      }
+      a.row0 = 0;
+      a.row1 = 1;
+      cudaError_t e = cudaLaunchKernelEx(&cfg, kern, a, p);
+      if (e != cudaSuccess) return fail(LBMHD_ECUDA, "resident step kernel launch: %s", cudaGetErrorString(e));
+      h->launches += 1;
+      h->last_path = LBMHD_PATH_RESIDENT;
+      for (int s = 0; s < n_steps; s++) advance(h);
+      *done = true;
+    }
+    return LBMHD_OK;
+  }
+  static int launch_resident(lbmhd_t *h, StepArgs<real> &a, int n_steps, bool *done) {
+    const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
+    if (resident_fits<32>(h)) return inplace ? launch_resident_t<32, true>(h, a, n_steps, done) : launch_resident_t<32, false>(h, a, n_steps, done);
+    return inplace ? launch_resident_t<64, true>(h, a, n_steps, done) : launch_resident_t<64, false>(h, a, n_steps, done);
+  }
   static int step(lbmhd_t *h, int n_steps) {
     StepArgs<real> a;
     make_args(h, a);
     const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
+    if (resident_allowed(h)) {
+      // in place the resident kernel runs an even number of steps from layout P0: a plain step before it if the lattice is in
+      // layout P1, the odd step left over by the launches below
+      const int pre = inplace && h->parity != 0 ? 1 : 0;
+      const int mid = inplace ? ((n_steps - pre) & ~1) : n_steps;
+      if (mid >= 2) {
+        if (pre) {
+          step_args(h, a);
+          if (int rc = launch(h, a, 0, n_planes(h))) return rc;
+          advance(h);
+        }
+        step_args(h, a);
+        bool done = false;
+        if (int rc = launch_resident(h, a, mid, &done)) return rc;
+        n_steps -= pre + (done ? mid : 0);
+        if (n_steps == 0) return LBMHD_OK;
+      }
+    }
     if (persist_allowed(h, n_steps)) {
       const long long n_tiles = (long long)((h->p.nx + 31) / 32) * h->p.ny * h->p.nz;
       const int cap = inplace ? persist_capacity<true>(h) : persist_capacity<false>(h);

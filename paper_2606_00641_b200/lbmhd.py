@@ -368,7 +368,7 @@ class Lbmhd:
         return int(self.lib.lbmhd_step_path(self.h))
 
 
-PATH_ONE, PATH_MULTI, PATH_CLUSTER, PATH_TMA, PATH_PERSIST, PATH_CELL = 0, 1, 2, 3, 4, 5
+PATH_ONE, PATH_MULTI, PATH_CLUSTER, PATH_TMA, PATH_PERSIST, PATH_CELL, PATH_RESIDENT = 0, 1, 2, 3, 4, 5, 6
 
 
 def from_workload(w, precision=64, device=0, streaming=STREAM_AB, solid_fields=True):

@@ -12,6 +12,8 @@ sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
 # launch (step_kernel_persist) and the one-launch-per-step kernels would go untested.  Default for the test
 # session: per-step launches; tests/test_persist_gpu.py and the graded / full-size tests set LBMHD_PERSIST themselves.
 os.environ.setdefault("LBMHD_PERSIST", "0")
+# likewise the register-resident many-step kernel of the 1D lattices: tests/test_resident_gpu.py turns it on
+os.environ.setdefault("LBMHD_RESIDENT", "0")
 
 
 def pytest_configure(config):

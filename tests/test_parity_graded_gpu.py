@@ -70,12 +70,14 @@ def fp32_tolerance(ratio):
 def gpu_result(w, precision, streaming):
     import os
     from paper_2606_00641_b200 import lbmhd
-    saved = os.environ.get("LBMHD_PERSIST")
-    os.environ["LBMHD_PERSIST"] = "1"           # the library's own choice of kernel (tests/conftest.py turns the persistent path off)
+    saved = {v: os.environ.get(v) for v in ("LBMHD_PERSIST", "LBMHD_RESIDENT")}
+    for v in saved:
+        os.environ[v] = "1"                     # the library's own choice of kernel (tests/conftest.py turns the many-step paths off)
     try:
         g = lbmhd.from_workload(w, precision=precision, streaming=streaming)
     finally:
-        os.environ["LBMHD_PERSIST"] = saved if saved is not None else "0"
+        for v, old in saved.items():
+            os.environ[v] = old if old is not None else "0"
     g.init(w["fields"])
     g.step(NSTEPS)
     path = g.step_path

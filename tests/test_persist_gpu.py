@@ -26,6 +26,7 @@ def env():
 def run(w, steps, persist, streaming=0, precision=64, chunks=None, mask=None, obstacle=None):
     from paper_2606_00641_b200 import lbmhd
     os.environ["LBMHD_PERSIST"] = persist
+    os.environ["LBMHD_RESIDENT"] = "0"          # (the 1D lattices would otherwise take the register-resident kernel)
     g = gpu_from_workload(w, precision=precision, streaming=streaming)
     if obstacle is not None:
         g.set_obstacle(*obstacle)

@@ -1,0 +1,135 @@
+"""Many steps of a 1D lattice with the populations resident in registers (step_kernel_resident): the path
+lbmhd_step(n >= 2) takes on 1D lattices of up to 1024 cells (BASELINE config 1), checked
+  * against the oracle over config 1's whole run (the graded bar of north_star), both streaming modes and precisions,
+  * against the one-launch-per-step kernels over every boundary kind, scheme, ragged and whole last tiles, one- and many-CTA
+    clusters, odd and even step counts and several calls in a row (the same per-cell code runs in both: bit for bit),
+  * followed by plain steps (in place: the published moments it leaves behind are the ones the next step reads)."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2606_00641_b200 import workloads as W
+from parity_util import oracle_from_workload, field_errors, TOL64, TOL32
+from test_parity_gpu import random_workload, gpu_from_workload, resist_workload, full_workload, divb_workload
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture
+def env():
+    saved = dict(os.environ)
+    yield os.environ
+    os.environ.clear()
+    os.environ.update(saved)
+
+
+def run(w, chunks, resident, streaming=0, precision=64):
+    os.environ["LBMHD_RESIDENT"] = resident
+    os.environ["LBMHD_PERSIST"] = "0"
+    g = gpu_from_workload(w, precision=precision, streaming=streaming)
+    g.init(w["fields"])
+    l0 = g.launch_count
+    paths = []
+    for n in chunks:
+        g.step(n)
+        paths.append(g.step_path)
+    launches = g.launch_count - l0
+    Q, dg = g.moments()
+    pops = g.populations()
+    g.close()
+    return Q, dg, pops, paths, launches
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+@pytest.mark.parametrize("precision", [64, 32])
+def test_config1_whole_run_resident(env, streaming, precision):
+    """C1: 800 cells = 13 CTAs of 64 cells in one cluster, all 500 steps in ONE launch, all cells against the oracle"""
+    from paper_2606_00641_b200 import lbmhd
+    w = W.get("C1")
+    Q, dg, _, paths, launches = run(w, [500], "1", streaming=streaming, precision=precision)
+    assert paths == [lbmhd.PATH_RESIDENT] and launches == 1
+    o = oracle_from_workload(w)
+    o.init(w["fields"])
+    o.step(500)
+    errs = field_errors(Q, o.moments(diag=False))
+    print("C1 500 steps resident, fp%d streaming %d: %.2e" % (precision, streaming, errs.max()))
+    if precision == 64:
+        assert (errs <= TOL64).all(), errs
+    else:       # fp32: north_star's bar is stated for 100 steps (tests/test_parity_graded_gpu.py); here the per-step kernels are the reference
+        Qp, _, _, _, _ = run(w, [500], "0", streaming=streaming, precision=32)
+        assert (field_errors(Q, Qp) <= TOL32).all(), field_errors(Q, Qp)
+
+
+# (scheme, nx, bc): 32-cell CTAs (nx <= 512) and 64-cell CTAs, ragged and whole last CTA, one CTA, nx - 1 a multiple of 32
+CASES = [
+    ("IDEAL", 800, (1, 1)), ("IDEAL", 131, (1, 1)), ("IDEAL", 70, (2, 1)), ("IDEAL", 96, (0, 0)), ("IDEAL", 100, (0, 0)),
+    ("IDEAL", 20, (0, 0)), ("IDEAL", 20, (1, 2)), ("IDEAL", 33, (1, 1)), ("IDEAL", 1024, (0, 0)), ("IDEAL", 1000, (1, 2)),
+    ("IDEAL", 481, (1, 1)), ("INCRES", 200, (1, 1)), ("INCRES", 75, (0, 0)), ("IDEAL_DIVB", 300, (1, 1)), ("IDEAL_DIVB", 64, (0, 0)),
+]
+
+
+def make(scheme, nx, bc2, seed=81):
+    bc = tuple(bc2) + (0, 0, 0, 0)
+    if scheme == "RESIST":
+        return resist_workload("D1Q3", (nx,), bc, seed=seed)
+    if scheme == "FULL":
+        return full_workload("D1Q3", (nx,), bc, seed=seed)
+    if scheme == "IDEAL_DIVB":
+        return divb_workload("D1Q3", (nx,), bc, seed=seed)
+    return random_workload(scheme, "D1Q3", (nx,), bc, seed=seed)
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+@pytest.mark.parametrize("scheme,nx,bc", CASES)
+def test_resident_equals_per_step_launches(env, scheme, nx, bc, streaming):
+    from paper_2606_00641_b200 import lbmhd
+    w = make(scheme, nx, bc)
+    Qa, da, pa, paths_a, la = run(w, [30], "0", streaming=streaming)
+    # A/B: 12 | 1 (a single step is a plain launch) | 2 | 15.  In place the resident kernel runs an even count from layout P0:
+    # 12 | 1 plain | 5 = 1 plain (P1 -> P0) + 4 resident | 12 resident, i.e. 5 launches, the last one resident
+    Qb, db, pb, paths_b, lb = run(w, [12, 1, 2, 15] if streaming == 0 else [12, 1, 5, 12], "1", streaming=streaming)
+    assert lbmhd.PATH_RESIDENT not in paths_a and la == 30
+    assert paths_b == [lbmhd.PATH_RESIDENT, paths_a[0], lbmhd.PATH_RESIDENT, lbmhd.PATH_RESIDENT]
+    assert lb == (4 if streaming == 0 else 5)
+    scale = np.abs(pa).max()
+    assert np.abs(pa - pb).max() <= 1e-13 * scale, np.abs(pa - pb).max() / scale
+    print("resident vs per-step launches %s nx %d bc %s streaming %d: max population difference %.1e (bit-equal: %s)" % (
+        scheme, nx, bc, streaming, np.abs(pa - pb).max() / scale, np.array_equal(pa, pb)))
+    assert (field_errors(Qb, Qa) <= 1e-13).all()
+
+
+@pytest.mark.parametrize("scheme,nx,bc", [("RESIST", 150, (1, 1)), ("RESIST", 90, (0, 0)), ("FULL", 800, (1, 1)), ("FULL", 64, (0, 0))])
+@pytest.mark.parametrize("streaming", [0, 1])
+def test_resident_gradient_schemes(env, scheme, nx, bc, streaming):
+    """RESIST / FULL on D1Q3 (11 / 14 sets): 64 x 14 = 896 threads per CTA"""
+    from paper_2606_00641_b200 import lbmhd
+    w = make(scheme, nx, bc, seed=83)
+    Qa, da, pa, paths_a, _ = run(w, [20], "0", streaming=streaming)
+    Qb, db, pb, paths_b, lb = run(w, [20], "1", streaming=streaming)
+    assert paths_b == [lbmhd.PATH_RESIDENT] and lb == 1
+    scale = np.abs(pa).max()
+    assert np.abs(pa - pb).max() <= 1e-13 * scale
+
+
+@pytest.mark.parametrize("streaming", [0, 1])
+def test_plain_steps_after_resident_steps(env, streaming):
+    """in place the resident kernel leaves the published moments of its last step in both M arrays: the plain step that follows reads them"""
+    from paper_2606_00641_b200 import lbmhd
+    w = make("IDEAL", 300, (1, 1), seed=84)
+    Qa, da, pa, _, _ = run(w, [26], "0", streaming=streaming)
+    Qb, db, pb, paths_b, _ = run(w, [10, 1, 1, 12, 1, 1], "1", streaming=streaming)
+    assert paths_b[0] == lbmhd.PATH_RESIDENT and paths_b[3] == lbmhd.PATH_RESIDENT and paths_b[1] != lbmhd.PATH_RESIDENT
+    scale = np.abs(pa).max()
+    assert np.abs(pa - pb).max() <= 1e-13 * scale
+
+
+def test_fallbacks(env):
+    """what the resident kernel does not take goes to the other kernels: longer lattices, odd step counts in place, 2D"""
+    from paper_2606_00641_b200 import lbmhd
+    _, _, _, paths, _ = run(make("IDEAL", 1025, (0, 0)), [4], "1")
+    assert paths[0] != lbmhd.PATH_RESIDENT
+    _, _, _, paths, _ = run(make("IDEAL", 513, (1, 1)), [4], "1")
+    assert paths[0] != lbmhd.PATH_RESIDENT          # a zero-gradient face cell alone in the last CTA, for 32- and 64-cell CTAs
+    _, _, _, paths, _ = run(random_workload("IDEAL", "D2Q9", (64, 8), (0,) * 6, seed=85), [4], "1")
+    assert paths[0] != lbmhd.PATH_RESIDENT
