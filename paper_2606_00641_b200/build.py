@@ -12,7 +12,7 @@ _CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "liblbmhd.so")
 OBJ_DIR = os.path.join(_HERE, "build")
 DEPS = [os.path.join(_CSRC, f) for f in ("lbmhd_api.cu", "lbmhd_inst.cu", "lbmhd_noalloc.cu", "lbmhd_host.h", "lbmhd_ops.cuh", "lbmhd_kernels.cuh",
-                                         "lbmhd_lattice.cuh", "lbmhd_tma.cuh")] + \
+                                         "lbmhd_lattice.cuh", "lbmhd_tma.cuh", "lbmhd_resident.cuh")] + \
        [os.path.join(os.path.dirname(_HERE), "include", "lbmhd.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 LATTICES = (3, 2, 5, 4, 1)          # heaviest first: D3Q19, D2Q9, D3Q7, D2Q5, D1Q3
