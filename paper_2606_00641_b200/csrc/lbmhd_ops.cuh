@@ -347,8 +347,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     return LBMHD_OK;
   }
   // ---- many steps of a 1D lattice with the populations resident in registers (lbmhd_resident.cuh) --------------
-  // One cluster of <= 16 CTAs of TXR cells (TXR = 32 or 64: nx <= 1024), fluid cells only, no body; in place from parity 0 for an
-  // even number of steps (the kernel reads and leaves layout P0).  A zero-gradient face and its inward neighbour share a CTA.
+  // One cluster of <= 16 CTAs of TXR cells (TXR = 32 or 64: nx <= 1024), fluid cells only, no body; in place from either layout
+  // for any number of steps.  A zero-gradient face and its inward neighbour share a CTA.
   template <int TXR> static bool resident_fits(const lbmhd_t *h) {
     const int nx = h->p.nx, ncta = (nx + TXR - 1) / TXR;
     if (TXR * K > 1024 || ncta > 16) return false;
@@ -376,6 +376,8 @@ template <int LAT, int SCHEME, typename real> struct Ops {
       p.pop_in = pops(h, h->cur);
       p.pop_out = pops(h, INPLACE ? h->cur : (h->cur + n_steps) & 1);
       if (INPLACE) {
+        p.layout_in = h->parity;
+        p.layout_out = (h->parity + n_steps) & 1;
         p.M_in = (const double *)(h->ws + h->L.off_M[h->mcur]);
         p.M_out[0] = (double *)(h->ws + h->L.off_M[0]);
         p.M_out[1] = (double *)(h->ws + h->L.off_M[1]);
@@ -420,23 +422,11 @@ template <int LAT, int SCHEME, typename real> struct Ops {
     StepArgs<real> a;
     make_args(h, a);
     const bool inplace = h->p.streaming == LBMHD_STREAM_INPLACE;
-    if (resident_allowed(h)) {
-      // in place the resident kernel runs an even number of steps from layout P0: a plain step before it if the lattice is in
-      // layout P1, the odd step left over by the launches below
-      const int pre = inplace && h->parity != 0 ? 1 : 0;
-      const int mid = inplace ? ((n_steps - pre) & ~1) : n_steps;
-      if (mid >= 2) {
-        if (pre) {
-          step_args(h, a);
-          if (int rc = launch(h, a, 0, n_planes(h))) return rc;
-          advance(h);
-        }
-        step_args(h, a);
-        bool done = false;
-        if (int rc = launch_resident(h, a, mid, &done)) return rc;
-        n_steps -= pre + (done ? mid : 0);
-        if (n_steps == 0) return LBMHD_OK;
-      }
+    if (n_steps >= 2 && resident_allowed(h)) {
+      step_args(h, a);
+      bool done = false;
+      if (int rc = launch_resident(h, a, n_steps, &done)) return rc;
+      if (done) return LBMHD_OK;
     }
     if (persist_allowed(h, n_steps)) {
       const long long n_tiles = (long long)((h->p.nx + 31) / 32) * h->p.ny * h->p.nz;

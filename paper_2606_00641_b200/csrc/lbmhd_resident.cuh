@@ -20,8 +20,11 @@
 // phase parity j & 1).  A cluster barrier after the mbarrier initialisation makes every CTA resident before anything is sent;
 // one before the exit keeps every CTA alive until nothing more can arrive.
 //
-// Layouts: the kernel reads and writes the A/B layout (g_i of a cell stored at the cell, = layout P0 of the in-place scheme), so
-// in place it is taken from parity 0 for an even number of steps only; it then also leaves the published moments M behind.
+// Layouts: the resident state is g_i(x), the post-collision population of direction i at cell x.  A/B and layout P0 of the in-place
+// scheme store it at (slot i, cell x); layout P1 (after a pull-push step) at (slot opp(i), cell x + c_i), wrapped on a periodic
+// axis, and parked at (slot i, cell x) when x + c_i is outside a non-periodic face (StorePPEdge).  The kernel reads either layout
+// and writes the one the step count leads to, so any n from any parity is one launch; in place it also leaves the published
+// moments M of its last step behind.
 #pragma once
 #include "lbmhd_kernels.cuh"
 
@@ -32,6 +35,7 @@ template <typename real> struct ResidentArgs {
   int ncta;              // CTAs of the one cluster = ceil(nx / TXR)
   const real *pop_in;    // the copy the first step reads
   real *pop_out;         // the copy the last step's result belongs in (A/B: copy (cur + n) & 1; in place: the single copy)
+  int layout_in, layout_out;   // in place: 0 = P0, 1 = P1 (A/B: 0)
   const double *M_in;    // in place: the published moments the first step reads (M_cur)
   double *M_out[2];      // in place: both published-moment arrays take the last step's moments
 };
@@ -129,9 +133,23 @@ step_kernel_resident(const __grid_constant__ StepArgs<real> a0, const __grid_con
   if (send_l) { lG = cl_mapa(sG0, (uint32_t)left); lbar = cl_mapa(bar0, (uint32_t)left); lslot = (uint32_t)((1 * K + k) * (TXR + 2) + na_left + 1); }
   constexpr uint32_t BUF = (uint32_t)(2 * K * (TXR + 2));      // elements per buffer
 
+  // (slot, cell) of g_i(x) in layout P0 / P1
+  auto where = [&](int i, int layout, int &slot_i, int &cell) {
+    slot_i = i;
+    cell = x;
+    if (layout != 0 && L::cx(i) != 0) {
+      int xs = x + L::cx(i);
+      if (periodic) xs = xs < 0 ? xs + nx : (xs >= nx ? xs - nx : xs);
+      if (xs >= 0 && xs < nx) { slot_i = opp(i); cell = xs; }
+    }
+  };
   real g[Q], f[Q];
 #pragma unroll
-  for (int i = 0; i < Q; i++) g[i] = active ? p.pop_in[((size_t)k * Q + i) * a0.pstride + x] : real(0);
+  for (int i = 0; i < Q; i++) {
+    int si, xc;
+    where(i, INPLACE ? p.layout_in : 0, si, xc);
+    g[i] = active ? p.pop_in[((size_t)k * Q + si) * a0.pstride + xc] : real(0);
+  }
   real pub = real(0);      // in place: this cell's published moment Q_k + inj of the previous step
   if (INPLACE && (nb_lo || nb_hi)) pub = (real)p.M_in[(size_t)k * nx + x];
   const Share<real, TXR, false> sh{sQ, sTr, sNb, nullptr, nullptr, nullptr, SyncBlock{}};
@@ -183,7 +201,11 @@ step_kernel_resident(const __grid_constant__ StepArgs<real> a0, const __grid_con
 
   if (active) {
 #pragma unroll
-    for (int i = 0; i < Q; i++) p.pop_out[((size_t)k * Q + i) * a0.pstride + x] = g[i];
+    for (int i = 0; i < Q; i++) {
+      int si, xc;
+      where(i, INPLACE ? p.layout_out : 0, si, xc);
+      p.pop_out[((size_t)k * Q + si) * a0.pstride + xc] = g[i];
+    }
     if (INPLACE && !frozen && p.n_steps > 0) {
       p.M_out[0][(size_t)k * nx + x] = (double)pub;
       p.M_out[1][(size_t)k * nx + x] = (double)pub;

@@ -86,12 +86,11 @@ def test_resident_equals_per_step_launches(env, scheme, nx, bc, streaming):
     from paper_2606_00641_b200 import lbmhd
     w = make(scheme, nx, bc)
     Qa, da, pa, paths_a, la = run(w, [30], "0", streaming=streaming)
-    # A/B: 12 | 1 (a single step is a plain launch) | 2 | 15.  In place the resident kernel runs an even count from layout P0:
-    # 12 | 1 plain | 5 = 1 plain (P1 -> P0) + 4 resident | 12 resident, i.e. 5 launches, the last one resident
-    Qb, db, pb, paths_b, lb = run(w, [12, 1, 2, 15] if streaming == 0 else [12, 1, 5, 12], "1", streaming=streaming)
+    # 12 | 1 (a single step is a plain launch) | 2 | 15: in place the resident launches start from layouts P0, P1, P1 and end in
+    # P0, P1, P0 (odd and even counts from either layout)
+    Qb, db, pb, paths_b, lb = run(w, [12, 1, 2, 15], "1", streaming=streaming)
     assert lbmhd.PATH_RESIDENT not in paths_a and la == 30
-    assert paths_b == [lbmhd.PATH_RESIDENT, paths_a[0], lbmhd.PATH_RESIDENT, lbmhd.PATH_RESIDENT]
-    assert lb == (4 if streaming == 0 else 5)
+    assert paths_b == [lbmhd.PATH_RESIDENT, paths_a[0], lbmhd.PATH_RESIDENT, lbmhd.PATH_RESIDENT] and lb == 4
     scale = np.abs(pa).max()
     assert np.abs(pa - pb).max() <= 1e-13 * scale, np.abs(pa - pb).max() / scale
     print("resident vs per-step launches %s nx %d bc %s streaming %d: max population difference %.1e (bit-equal: %s)" % (
@@ -114,12 +113,14 @@ def test_resident_gradient_schemes(env, scheme, nx, bc, streaming):
 
 @pytest.mark.parametrize("streaming", [0, 1])
 def test_plain_steps_after_resident_steps(env, streaming):
-    """in place the resident kernel leaves the published moments of its last step in both M arrays: the plain step that follows reads them"""
+    """in place the resident kernel leaves the published moments of its last step in both M arrays and the layout its step count
+    leads to (P0 after 10 from P0, P0 after 3 from P1, P1 after 10 from P1): the plain steps that follow read them"""
     from paper_2606_00641_b200 import lbmhd
     w = make("IDEAL", 300, (1, 1), seed=84)
     Qa, da, pa, _, _ = run(w, [26], "0", streaming=streaming)
-    Qb, db, pb, paths_b, _ = run(w, [10, 1, 1, 12, 1, 1], "1", streaming=streaming)
-    assert paths_b[0] == lbmhd.PATH_RESIDENT and paths_b[3] == lbmhd.PATH_RESIDENT and paths_b[1] != lbmhd.PATH_RESIDENT
+    Qb, db, pb, paths_b, _ = run(w, [10, 1, 3, 1, 10, 1], "1", streaming=streaming)
+    assert paths_b[0] == lbmhd.PATH_RESIDENT and paths_b[2] == lbmhd.PATH_RESIDENT and paths_b[4] == lbmhd.PATH_RESIDENT
+    assert paths_b[1] != lbmhd.PATH_RESIDENT
     scale = np.abs(pa).max()
     assert np.abs(pa - pb).max() <= 1e-13 * scale
 
