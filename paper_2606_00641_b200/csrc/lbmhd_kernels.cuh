@@ -1280,11 +1280,20 @@ template <class L, typename real, int NC, bool EDGE = false> struct StoreMultiPP
   }
 };
 
+// Which cells of a multi-cell tile publish their post-collision moment (in-place modes, A9): every cell of a row next to a
+// non-periodic y / z face (`row`), and the two cells at each end of a row whose x faces are not periodic.  `any`, `row`, `edge`
+// and `npx` are block-uniform; `any` is false on the interior tiles of interior rows.
+struct PubM {
+  bool any, row, npx;
+  int edge;      // EDGE tiles: 1 = the tile starts at x = 0, 2 = it ends at nx, 0 = neither
+  int x, nx;     // first cell of this thread
+};
+
 // S2-S8 of NC fluid cells of an interior tile (no boundary, no solid, constant eta).  sQ / sTr rows are laid out
 // [c][32] (cell c of lane tx at c*32 + tx): conflict-free scalar accesses.
 // pass[c] (EDGE tiles only): cell c is a frozen face cell whose f already holds what it keeps / emits (A10): unchanged.
 template <int LAT, int SCHEME, typename real, int NC, int STREAM, bool EDGE = false, class Store>
-__device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, int k, uint32_t n, const bool (&writeM)[NC],
+__device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, int k, uint32_t n, const PubM pm,
                                              const bool (&pass)[NC], real (&f)[NC][Lattice<LAT>::Q], const Store &store,
                                              real (*sQ)[32 * NC], real (*sTr)[32 * NC]) {
   using L = Lattice<LAT>;
@@ -1357,13 +1366,34 @@ __device__ __forceinline__ void finish_multi(const StepArgs<real> &a, int tx, in
         inj = -(a.kappa * delta) * powell_row<SCHEME, D, real>(KC, Qv);
         if (has_relax(SCHEME) && KC >= 8) inj = -Qk[c] * a.inv_tau_relax;      // relaxation source of Eq.6
       }
-      if (STREAM != ST_AB && writeM[c]) a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + n + c] = (double)(Qk[c] + inj);
       injv[c] = inj;
       P[c][0] = Phi[0]; P[c][1] = Phi[1]; P[c][2] = Phi[2];
     }
   };
   if constexpr (ROWCONST) dispatch_row<0, K>(k, cells);
   else cells(k);
+  // in place: the cells next to a non-periodic face publish their post-collision moment (A9).  `anyM` is block-uniform and false
+  // on the interior tiles of interior rows, which then pay one uniform branch for all of this.
+  if (STREAM != ST_AB && pm.any) {
+    auto put = [&](int c) { a.M_next[(size_t)k * ((size_t)a.nx * a.ny * a.nz) + n + c] = (double)(Qk[c] + injv[c]); };
+    if (pm.row) {
+#pragma unroll
+      for (int c = 0; c < NC; c++)
+        if (!(EDGE && pass[c])) put(c);
+    } else if (EDGE) {      // cells x = 0, 1 are the first two of lane 0 in the tile at x = 0; x = nx - 2, nx - 1 the last two of lane 31
+      if (pm.npx && pm.edge == 1 && tx == 0) {
+        if (!pass[0]) put(0);
+        put(1);
+      } else if (pm.npx && pm.edge == 2 && tx == 31) {
+        put(NC - 2);
+        if (!pass[NC - 1]) put(NC - 1);
+      }
+    } else {
+#pragma unroll
+      for (int c = 0; c < NC; c++)
+        if (pm.x + c == 1 || pm.x + c == pm.nx - 2) put(c);
+    }
+  }
   Collide<L, real> col[NC];
 #pragma unroll
   for (int c = 0; c < NC; c++) {
@@ -1529,24 +1559,26 @@ step_kernel_multi(const __grid_constant__ StepArgs<real> a, const int nmulti, co
     }
     const bool rowM = STREAM != ST_AB && ((npy && (y == 1 || y == ny - 2)) || (npz && (z == 1 || z == nz - 2)));
     const bool frozen_face = EDGE && edge != 0 && (edge == 1 ? a.bc[0] : a.bc[1]) == BC_INFLOW;
-    bool wM[NC], pass[NC];
+    // block-uniform: does the tile hold a cell that publishes (x <= 1 or x >= nx - 2 on a non-periodic axis, or a row next to a face)
+    const bool anyM = STREAM != ST_AB && (rowM || (npx && (x0 <= 1 || x0 + W >= nx - 1)));
+    const PubM pm{anyM, rowM, npx, edge, x, nx};
+    bool pass[NC];
 #pragma unroll
     for (int c = 0; c < NC; c++) {
       // EDGE: the frozen face cell goes through unchanged and publishes nothing (its state is constant); the face cell of a
       // zero-gradient face publishes its moment like its neighbour does (every cell of an x-edge tile does in run_tile)
       pass[c] = frozen_face && ((edge == 1 && tx == 0 && c == 0) || (edge == 2 && tx == 31 && c == NC - 1));
-      wM[c] = (rowM || (npx && (EDGE ? (x + c <= 1 || x + c >= nx - 2) : (x + c == 1 || x + c == nx - 2)))) && !pass[c];
     }
     if (STREAM == ST_AB) {
       const StoreMultiOwn<real, NC> st{reinterpret_cast<char *>(a.dst + ((size_t)k * Q * a.pstride + n)), a.st_off};
-      finish_multi<LAT, SCHEME, real, NC, STREAM, EDGE>(a, tx, k, n, wM, pass, f, st, sQ, sTr);
+      finish_multi<LAT, SCHEME, real, NC, STREAM, EDGE>(a, tx, k, n, pm, pass, f, st, sQ, sTr);
     } else if (STREAM == ST_PP) {
       const StoreMultiPP<L, real, NC, EDGE> st{pb, a.ld_off, tx, a.st_off, edge, !npx,
                                                (long long)nx * (long long)sizeof(real) * (edge == 1 ? 1 : -1)};
-      finish_multi<LAT, SCHEME, real, NC, STREAM, EDGE>(a, tx, k, n, wM, pass, f, st, sQ, sTr);
+      finish_multi<LAT, SCHEME, real, NC, STREAM, EDGE>(a, tx, k, n, pm, pass, f, st, sQ, sTr);
     } else {
       const StoreMultiOwn<real, NC> st{pb, a.st_off};
-      finish_multi<LAT, SCHEME, real, NC, STREAM, EDGE>(a, tx, k, n, wM, pass, f, st, sQ, sTr);
+      finish_multi<LAT, SCHEME, real, NC, STREAM, EDGE>(a, tx, k, n, pm, pass, f, st, sQ, sTr);
     }
     return;
   }
