@@ -6,7 +6,7 @@
 The places where a mis-indexed slot would be a silent race or an out-of-bounds access: the in-place (AA) kernels in both
 step types with x-edge, general and sphere tiles; the 2-CTA cluster exchange through distributed shared memory
 (step_kernel_cl); the multi-cell and cell-per-thread kernels with their vector accesses and shuffled stores; the cooperative
-many-step launch; the slab halo pack / unpack with the in-place return exchange.  Each case is also compared with the
+many-step launch; the register-resident cluster kernel of the 1D lattices; the slab halo pack / unpack with the in-place return exchange.  Each case is also compared with the
 oracle, so a run that passes the tool but computes garbage still fails.  On this project's GPU pool compute-sanitizer is
 closed (profiles/r2_sanitizer.md records the refusal); there tests/test_guard_gpu.py runs these same cases with guard bands
 around every workspace instead.  Not collected by pytest (no test_ prefix)."""
@@ -63,6 +63,30 @@ def main():
     wp = random_workload("IDEAL", "D2Q9", (90, 21), (1, 1, 2, 1, 0, 0), seed=307)
     for streaming in (0, 1):
         case("step_kernel_persist streaming %d" % streaming, {"LBMHD_PERSIST": "2"}, lambda: compare(wp, 7, streaming=streaming))
+
+    # 1D lattices, populations resident in registers: one cluster, halo cells through distributed shared memory; both in-place
+    # layouts read and written (7 steps from P0 end in P1, 6 more from P1 end in P1 ... ), ragged last CTA, every face kind
+    def resident(w, streaming):
+        from paper_2606_00641_b200 import lbmhd
+        from parity_util import oracle_from_workload
+        o = oracle_from_workload(w)
+        o.init(w["fields"])
+        o.step(18)
+        g = gpu_from_workload(w, streaming=streaming)
+        g.init(w["fields"])
+        for n in (7, 6, 5):
+            g.step(n)
+            assert g.step_path == lbmhd.PATH_RESIDENT
+        Q = g.moments()[0]
+        g.close()
+        assert (field_errors(Q, o.moments(diag=False)) <= TOL64).all()
+        o.close()
+    for nx, bc in ((800, (1, 1)), (131, (2, 1)), (100, (0, 0)), (20, (1, 2))):
+        w1 = random_workload("IDEAL", "D1Q3", (nx,), bc + (0, 0, 0, 0), seed=308)
+        for streaming in (0, 1):
+            case("step_kernel_resident nx %d bc %s streaming %d" % (nx, bc, streaming), {"LBMHD_RESIDENT": "1", "LBMHD_PERSIST": "0"},
+                 lambda: resident(w1, streaming))
+    # dependent launches (griddepcontrol) are on in every case above (LBMHD_PDL default)
 
     # slabs: halo pack / unpack, in-place return exchange, overlapped schedule
     def slabs(streaming):

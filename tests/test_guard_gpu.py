@@ -2,7 +2,8 @@
 
 * Guard bands: every handle the cases of tests/sanitizer_cases.py create gets 1 MiB of 0xA5 before and after its workspace
   (LBMHD_GUARD_BYTES); closing the handle checks them.  The cases cover every step-kernel family (one cell per thread, several
-  cells per thread with vector accesses and shuffled stores, cell per thread, 2-CTA cluster, cooperative many-step launch), both
+  cells per thread with vector accesses and shuffled stores, cell per thread, 2-CTA cluster, cooperative many-step launch, the
+  register-resident cluster kernel of the 1D lattices), both
   in-place step types, x-edge / general / sphere tiles and the slab halo kernels, each also compared with the oracle: an
   out-of-bounds WRITE trips a guard, an out-of-bounds or misplaced READ changes a result.
 * Races: the in-place (AA) kernels and the cluster exchange are the places where a mis-indexed slot would be a silent race.
@@ -46,11 +47,14 @@ def test_guard_band_check_is_live(env):
         g.close()
 
 
-@pytest.mark.parametrize("case", ["multi64", "multi32", "cluster", "cell", "edge"])
+@pytest.mark.parametrize("case", ["multi64", "multi32", "cluster", "cell", "edge", "resident"])
 def test_in_place_runs_are_bit_reproducible(env, case):
     env["LBMHD_PERSIST"] = "0"
     prec = 64
-    if case == "multi64":
+    if case == "resident":       # halo cells through st.async + mbarrier between the CTAs of one cluster
+        env["LBMHD_RESIDENT"] = "1"
+        w = random_workload("IDEAL", "D1Q3", (800,), (1, 1, 0, 0, 0, 0), seed=507)
+    elif case == "multi64":
         env["LBMHD_MULTI"] = "1"
         w = random_workload("IDEAL", "D3Q19", (292, 6, 5), (2, 1, 0, 0, 0, 0), seed=502)
     elif case == "multi32":
